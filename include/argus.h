@@ -1,0 +1,178 @@
+/*
+ * argus.h -- C ABI of the B200-native calibrate + HEALPix-resample hot path of Argus-HDPS
+ * (arXiv 2207.14304).  Plain C99, no torch types: device/host pointers, sizes, a cudaStream_t
+ * passed as void*.
+ *
+ * What the path computes (citations are PAPER.md line + section; the paper states the steps in
+ * words only, DESIGN.md lists the readings taken where it is silent):
+ *   - "standard image calibrations (dark subtraction, flat fielding, masking of bad pixels)"
+ *     PAPER.md:141 (sec. 5.1), on the GPU PAPER.md:135 (sec. 5), Table 2 PAPER.md:192;
+ *   - "Each full-frame image is reprojected into equal-sky-area tiles (based on the HEALPix
+ *     pixelization scheme with NSIDE=256)" PAPER.md:145 (sec. 5.1.1), Table 2, using the
+ *     "one-directional mapping from celestial to pixel-plane coordinates" of PAPER.md:141;
+ *   - coaddition on the pre-aligned HEALPix grid PAPER.md:153 (sec. 5.1.3): plain sum / weight-sum.
+ *   Calibration masters are caller-owned device buffers that stay resident across frames
+ *   (uploaded "at the start of each pointing").
+ *
+ * Conventions
+ *   - Every function returns ARGUS_OK (0) or a negative argus_status; nothing throws.
+ *   - Unless stated otherwise every array pointer is a DEVICE pointer owned by the caller; the library
+ *     never frees it and never keeps it after the call returns.  argus_wcs / argus_frame / argus_coadd
+ *     structs are HOST structs read during the call.
+ *   - All work is enqueued on the caller's stream (cudaStream_t passed as void*; NULL = legacy default
+ *     stream) and is asynchronous, except where a function documents a synchronisation.
+ *   - Pixel convention: 0-based, pixel centres at integers, frame[y*W + x], x <-> FITS axis 1,
+ *     crpix 0-based.  HEALPix: NESTED scheme, nside a power of two, 32 <= nside <= 2^29; sky
+ *     convention alpha = phi, delta = pi/2 - theta (ICRS).
+ *   - Footprint domain: a HEALPix pixel belongs to the frame footprint iff its centre maps to
+ *     -0.5 <= x < W-0.5, -0.5 <= y < H-0.5 and lies within rho_max of CRVAL,
+ *     rho_max = atan(1.25 * scale * hypot(W,H)/2), scale = sqrt|det CD|.
+ */
+#ifndef ARGUS_H_
+#define ARGUS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum argus_status {
+    ARGUS_OK = 0,
+    ARGUS_ERR_NULL = -1,     /* a required pointer is NULL */
+    ARGUS_ERR_SHAPE = -2,    /* W, H, n or a size argument is out of range */
+    ARGUS_ERR_NSIDE = -3,    /* nside is not a power of two in [32, 2^29] */
+    ARGUS_ERR_KERNEL = -4,   /* unknown interpolation kernel */
+    ARGUS_ERR_WCS = -5,      /* singular CD matrix, non-finite entries, sip_order outside [0,5] */
+    ARGUS_ERR_CAPACITY = -6, /* an output or scratch capacity is too small (required size is reported) */
+    ARGUS_ERR_ALIGN = -7,    /* a pointer is not aligned to its element type */
+    ARGUS_ERR_CUDA = -8,     /* a CUDA runtime call failed: see argus_last_cuda_error() */
+    ARGUS_ERR_STATE = -9     /* call sequence error (e.g. no plan for this WCS and n does not match) */
+} argus_status;
+
+enum { ARGUS_BILINEAR = 0, ARGUS_LANCZOS3 = 1 };
+
+/* Options for argus_ctx_set_option. */
+enum {
+    ARGUS_OPT_PLAN_CACHE = 1 /* 1 (default): a plan built for (wcs, W, H, nside) is reused by the next
+                                call with identical arguments; 0: every call re-plans on the device */
+};
+
+typedef struct argus_ctx argus_ctx;
+
+/* Sky -> pixel WCS.  TAN (gnomonic) about crval, pixel = CD^-1 (xi, eta) [+ SIP] + crpix.
+ * SIP uses the sky->pixel ("inverse", AP/BP) polynomials applied directly:
+ *   u = U + sum_{p+q<=sip_order} ap[p*6+q] U^p V^q,   v = V + sum bp[p*6+q] U^p V^q. */
+typedef struct argus_wcs {
+    double crval[2];   /* deg: alpha0, delta0 */
+    double crpix[2];   /* px, 0-based */
+    double cd[2][2];   /* deg/px: (xi, eta)^T = cd (U, V)^T */
+    int32_t sip_order; /* 0 = no SIP, else 2..5 */
+    int32_t reserved;
+    double ap[36];
+    double bp[36];
+} argus_wcs;
+
+/* One frame.  Either the raw frame + masters (raw != NULL: calibration is fused into the resampling,
+ * the calibrated frame never exists in HBM) or an already calibrated frame (raw == NULL: cal + mask,
+ * e.g. argus_calibrate's outputs).  All pointers are device pointers, row-major [H][W]. */
+typedef struct argus_frame {
+    const uint16_t* raw;  /* ADU */
+    const float* bias;    /* ADU */
+    const float* dark;    /* ADU / s */
+    const float* flat;    /* dimensionless */
+    const uint8_t* bpm;   /* optional (may be NULL); non-zero = bad pixel */
+    float t_exp;          /* s: dark is scaled by t_exp */
+    int32_t sat_adu;      /* raw >= sat_adu is masked (65535 = clipped pixels only) */
+    float flat_min;       /* !(flat >= flat_min) is masked */
+    const float* cal;     /* used when raw == NULL: calibrated ADU */
+    const uint8_t* mask;  /* used when raw == NULL: 1 = good, 0 = masked */
+} argus_frame;
+
+/* Coadd buffer layout: sorted tile ids at resolution nside_tile (NSIDE = 256 in the
+ * paper); each tile owns ppt = (nside/nside_tile)^2 consecutive nested pixels:
+ *   slot(p) = rank(p / ppt) * ppt + (p mod ppt);  sum and wsum hold n_tiles * ppt floats. */
+typedef struct argus_coadd {
+    const int64_t* tiles; /* device, ascending, unique */
+    int64_t n_tiles;
+    int64_t nside_tile;   /* power of two, 1 <= nside_tile <= nside/32 */
+} argus_coadd;
+
+/* Plan statistics of the most recent plan (diagnostics; filled by argus_plan_info). */
+typedef struct argus_plan_stats {
+    int64_t n_footprint;  /* footprint size */
+    int64_t n_tiles;      /* 32x32-pixel output tiles visited */
+    int64_t n_inside;     /* tiles entirely inside the footprint, polynomial coordinates */
+    int64_t n_border;     /* tiles cut by the frame border */
+    int64_t n_exact;      /* tiles evaluated per pixel in FP64 (belt/cap ring, poles, failed fits) */
+    int64_t n_empty;      /* candidate tiles that turned out empty */
+} argus_plan_stats;
+
+const char* argus_strerror(int status);
+int argus_version(void);
+
+/* Context: owns scratch only (tile records, prefix sums, counters), sized for frames of up to
+ * max_tiles output tiles (0 = default 1<<20, enough for a 61-MPix frame at nside 2^18).
+ * device = CUDA ordinal.  Synchronous. */
+int argus_ctx_create(argus_ctx** ctx, int device, int64_t max_tiles);
+int argus_ctx_destroy(argus_ctx* ctx);
+int argus_ctx_set_option(argus_ctx* ctx, int option, int64_t value);
+/* cudaError_t of the last failed CUDA call made through this context (0 if none). */
+int argus_last_cuda_error(const argus_ctx* ctx);
+
+/* A2 (standalone; the paper's unfused order).  Per pixel:
+ *   good = raw < sat_adu && (bpm == NULL || bpm == 0) && flat >= flat_min && all masters finite
+ *   cal_out  = good ? (raw - bias - dark * t_exp) / flat : 0      (float32)
+ *   mask_out = good ? 1 : 0
+ * Asynchronous on stream. */
+int argus_calibrate(argus_ctx* ctx, const uint16_t* raw, const float* bias, const float* dark,
+                    const float* flat, const uint8_t* bpm, int64_t W, int64_t H, float t_exp,
+                    int32_t sat_adu, float flat_min, float* cal_out, uint8_t* mask_out, void* stream);
+
+/* A0 + A1: builds the resampling plan for (wcs, W, H, nside) on the device and reports the footprint.
+ *   idx_out  : device int64[capacity] or NULL.  When non-NULL receives the footprint: all nested pixel
+ *              indices whose centre falls on the frame, ascending, unique.
+ *   n_out    : HOST pointer, receives the footprint size (always, also on ARGUS_ERR_CAPACITY).
+ * Synchronises the stream (the count travels to the host).  The plan stays cached in ctx for the
+ * following argus_resample / argus_resample_coadd calls with the same (wcs, W, H, nside). */
+int argus_healpix_footprint(argus_ctx* ctx, const argus_wcs* wcs, int64_t W, int64_t H, int64_t nside,
+                            int64_t* idx_out, size_t capacity, size_t* n_out, void* stream);
+
+/* A3-A5 (+ fused A2 when frame->raw != NULL): per footprint pixel pix2ang -> inverse TAN (+SIP) ->
+ * masked, normalised bilinear / Lanczos-3 interpolation (BASELINE.json north_star):
+ *   S0 = sum k, B = sum k (1 - m), V1 = sum k m cal over the 2x2 / 6x6 taps (off-frame taps have m = 0)
+ *   w = 1 - B/S0;  w < w_min ? (value, weight) = (0, 0) : (V1 / (S0 - B), min(w, 1)).
+ *   idx == NULL : the library uses its own plan for (wcs, W, H, nside) (built here, on the device, if not
+ *                 cached); output element i belongs to the i-th footprint pixel in ascending order; n is
+ *                 the capacity of value_out / weight_out; fully asynchronous.  If the footprint is
+ *                 larger than n nothing beyond n is written and the next synchronising call
+ *                 (argus_healpix_footprint / argus_plan_info) reports ARGUS_ERR_CAPACITY.
+ *   idx != NULL : device int64[n], arbitrary nested pixels (any order); output element i belongs to
+ *                 idx[i]; coordinates are evaluated per pixel in FP64 (general, slower path).
+ * Outputs are never NaN/Inf. */
+int argus_resample(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                   int64_t nside, int kernel, float w_min, const int64_t* idx, size_t n, float* value_out,
+                   float* weight_out, void* stream);
+
+/* A6: sum[slot(idx[i])] += weight[i] * value[i]; wsum[slot] += weight[i] for i < n.  idx must hold
+ * unique pixels (a footprint); pixels whose tile is absent from the layout are skipped and counted in
+ * *n_skipped_dev (device int64, may be NULL, accumulated with atomics).  Asynchronous. */
+int argus_coadd_accumulate(argus_ctx* ctx, const argus_coadd* layout, int64_t nside, float* sum, float* wsum,
+                           const int64_t* idx, const float* value, const float* weight, size_t n,
+                           int64_t* n_skipped_dev, void* stream);
+
+/* A2-A6 fused: resample with the library's plan and accumulate straight into the coadd buffer
+ * (value / weight are never written to HBM).  Asynchronous. */
+int argus_resample_coadd(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                         int64_t nside, int kernel, float w_min, const argus_coadd* layout, float* sum,
+                         float* wsum, int64_t* n_skipped_dev, void* stream);
+
+/* Synchronises the stream and reports the statistics of the cached plan.  Returns ARGUS_ERR_CAPACITY if
+ * an asynchronous call since the last check overflowed its output capacity or the context's max_tiles. */
+int argus_plan_info(argus_ctx* ctx, argus_plan_stats* out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARGUS_H_ */

@@ -1,0 +1,20 @@
+"""B200-native calibrate + HEALPix-resample hot path of Argus-HDPS (arXiv 2207.14304).
+
+The product is the C-ABI library ``libargus.so`` (include/argus.h, csrc/); this package is a thin ctypes
+binding with the same entry-point names.  There is no CPU fallback: importing :mod:`binding` without the
+compiled library raises.
+"""
+from .binding import (  # noqa: F401
+    ARGUS_BILINEAR,
+    ARGUS_LANCZOS3,
+    ArgusError,
+    Context,
+    argus_calibrate,
+    argus_coadd_accumulate,
+    argus_healpix_footprint,
+    argus_plan_info,
+    argus_resample,
+    argus_resample_coadd,
+    library_path,
+    load_library,
+)

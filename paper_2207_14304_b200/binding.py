@@ -1,0 +1,279 @@
+"""ctypes binding over libargus.so: argument marshalling only (every step of the path runs in the
+CUDA kernels behind the C ABI of include/argus.h).  PyTorch supplies device memory and streams.
+
+No CPU fallback exists: if the library cannot be loaded, every entry point raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+ARGUS_BILINEAR, ARGUS_LANCZOS3 = 0, 1
+ARGUS_OPT_PLAN_CACHE = 1
+_KERNELS = {"bilinear": ARGUS_BILINEAR, "lanczos3": ARGUS_LANCZOS3, 0: 0, 1: 1}
+
+EXPORTS = [
+    "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
+    "argus_last_cuda_error", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
+    "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info",
+]
+
+
+class ArgusError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        msg = "%s failed: %s (%d)" % (where, _strerror(status), status)
+        super().__init__(msg + (" " + detail if detail else ""))
+
+
+class _Wcs(C.Structure):
+    _fields_ = [("crval", C.c_double * 2), ("crpix", C.c_double * 2), ("cd", (C.c_double * 2) * 2),
+                ("sip_order", C.c_int32), ("reserved", C.c_int32), ("ap", C.c_double * 36), ("bp", C.c_double * 36)]
+
+
+class _Frame(C.Structure):
+    _fields_ = [("raw", C.c_void_p), ("bias", C.c_void_p), ("dark", C.c_void_p), ("flat", C.c_void_p),
+                ("bpm", C.c_void_p), ("t_exp", C.c_float), ("sat_adu", C.c_int32), ("flat_min", C.c_float),
+                ("cal", C.c_void_p), ("mask", C.c_void_p)]
+
+
+class _Coadd(C.Structure):
+    _fields_ = [("tiles", C.c_void_p), ("n_tiles", C.c_int64), ("nside_tile", C.c_int64)]
+
+
+class _PlanStats(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in ("n_footprint", "n_tiles", "n_inside", "n_border", "n_exact", "n_empty")]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libargus.so")
+
+
+def load_library():
+    """Load libargus.so (built in-tree by ``_build.build()``).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path):
+        raise ImportError("libargus.so not built: run `python -m paper_2207_14304_b200._build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    L = C.CDLL(path)
+    vp, i64, i32, f32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_size_t
+    L.argus_strerror.restype = C.c_char_p
+    L.argus_strerror.argtypes = [C.c_int]
+    L.argus_version.restype = C.c_int
+    L.argus_ctx_create.argtypes = [C.POINTER(vp), C.c_int, i64]
+    L.argus_ctx_destroy.argtypes = [vp]
+    L.argus_ctx_set_option.argtypes = [vp, C.c_int, i64]
+    L.argus_last_cuda_error.argtypes = [vp]
+    L.argus_calibrate.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, f32, i32, f32, vp, vp, vp]
+    L.argus_healpix_footprint.argtypes = [vp, C.POINTER(_Wcs), i64, i64, i64, vp, sz, C.POINTER(sz), vp]
+    L.argus_resample.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, vp, sz, vp, vp, vp]
+    L.argus_coadd_accumulate.argtypes = [vp, C.POINTER(_Coadd), i64, vp, vp, vp, vp, vp, sz, vp, vp]
+    L.argus_resample_coadd.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32,
+                                       C.POINTER(_Coadd), vp, vp, vp, vp]
+    L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
+    _lib = L
+    return L
+
+
+def _strerror(status: int) -> str:
+    try:
+        return load_library().argus_strerror(int(status)).decode()
+    except Exception:  # pragma: no cover
+        return "status %d" % status
+
+
+def _wcs_struct(w) -> _Wcs:
+    """Accepts synth.Wcs-like objects (crval, crpix, cd, sip_order, ap, bp) or a flat float64[81] array."""
+    s = _Wcs()
+    if hasattr(w, "crval"):
+        crval, crpix, cd, order, ap, bp = w.crval, w.crpix, w.cd, w.sip_order, w.ap, w.bp
+    else:
+        a = [float(v) for v in w]
+        crval, crpix, cd = a[0:2], a[2:4], ((a[4], a[5]), (a[6], a[7]))
+        order, ap, bp = int(a[8]), a[9:45], a[45:81]
+    s.crval[0], s.crval[1] = float(crval[0]), float(crval[1])
+    s.crpix[0], s.crpix[1] = float(crpix[0]), float(crpix[1])
+    for i in range(2):
+        for j in range(2):
+            s.cd[i][j] = float(cd[i][j])
+    s.sip_order = int(order)
+    for i in range(36):
+        s.ap[i] = float(ap[i])
+        s.bp[i] = float(bp[i])
+    return s
+
+
+def _dev(t, dtype, name, allow_none=False):
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError("%s is required" % name)
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA tensor" % name)
+    if t.dtype != dtype:
+        raise TypeError("%s must have dtype %s, got %s" % (name, dtype, t.dtype))
+    if not t.is_contiguous():
+        raise ValueError("%s must be contiguous" % name)
+    return t.data_ptr()
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _frame_struct(raw=None, bias=None, dark=None, flat=None, bpm=None, t_exp=0.0, sat_adu=65535, flat_min=0.1,
+                  cal=None, mask=None) -> _Frame:
+    f = _Frame()
+    if raw is not None:
+        f.raw = _dev(raw, torch.uint16, "raw")
+        f.bias = _dev(bias, torch.float32, "bias")
+        f.dark = _dev(dark, torch.float32, "dark")
+        f.flat = _dev(flat, torch.float32, "flat")
+        f.bpm = _dev(bpm, torch.uint8, "bpm", allow_none=True)
+        for t in (bias, dark, flat) + ((bpm,) if bpm is not None else ()):
+            if t.shape != raw.shape:
+                raise ValueError("masters must have the frame's shape")
+    else:
+        f.cal = _dev(cal, torch.float32, "cal")
+        f.mask = _dev(mask, torch.uint8, "mask")
+        if cal.shape != mask.shape:
+            raise ValueError("cal and mask must have the same shape")
+    f.t_exp, f.sat_adu, f.flat_min = float(t_exp), int(sat_adu), float(flat_min)
+    return f
+
+
+class Context:
+    """argus_ctx handle: owns the plan scratch on one device."""
+
+    def __init__(self, device: int | None = None, max_tiles: int = 0):
+        L = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("CUDA device required: the argus hot path has no CPU fallback")
+        self.device = torch.cuda.current_device() if device is None else int(device)
+        h = C.c_void_p()
+        rc = L.argus_ctx_create(C.byref(h), self.device, int(max_tiles))
+        if rc:
+            raise ArgusError(rc, "argus_ctx_create")
+        self._h = h
+
+    def set_plan_cache(self, on: bool):
+        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_PLAN_CACHE, 1 if on else 0)
+        if rc:
+            raise ArgusError(rc, "argus_ctx_set_option")
+
+    def last_cuda_error(self) -> int:
+        return int(load_library().argus_last_cuda_error(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load_library().argus_ctx_destroy(self._h)
+            self._h = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _check(ctx, rc, where):
+    if rc:
+        detail = ""
+        if rc == -8:
+            detail = "cudaError=%d" % ctx.last_cuda_error()
+        raise ArgusError(rc, where, detail)
+
+
+def argus_calibrate(ctx, raw, bias, dark, flat, bpm, t_exp, sat_adu=65535, flat_min=0.1, cal_out=None, mask_out=None,
+                    stream=None):
+    """A2 standalone.  Returns (cal float32 [H][W], mask uint8 [H][W])."""
+    H, W = raw.shape
+    if cal_out is None:
+        cal_out = torch.empty((H, W), dtype=torch.float32, device=raw.device)
+    if mask_out is None:
+        mask_out = torch.empty((H, W), dtype=torch.uint8, device=raw.device)
+    f = _frame_struct(raw, bias, dark, flat, bpm, t_exp, sat_adu, flat_min)
+    rc = load_library().argus_calibrate(ctx._h, f.raw, f.bias, f.dark, f.flat, f.bpm, W, H, float(t_exp), int(sat_adu),
+                                        float(flat_min), _dev(cal_out, torch.float32, "cal_out"),
+                                        _dev(mask_out, torch.uint8, "mask_out"), _stream(stream))
+    _check(ctx, rc, "argus_calibrate")
+    return cal_out, mask_out
+
+
+def argus_healpix_footprint(ctx, wcs, W, H, nside, idx_out=None, want_indices=True, stream=None):
+    """A0 + A1.  Returns (n, idx) with idx an ascending int64 CUDA tensor (None if want_indices is False)."""
+    L = load_library()
+    w = _wcs_struct(wcs)
+    n = C.c_size_t(0)
+    if idx_out is None:
+        rc = L.argus_healpix_footprint(ctx._h, C.byref(w), W, H, nside, None, 0, C.byref(n), _stream(stream))
+        _check(ctx, rc, "argus_healpix_footprint")
+        if not want_indices:
+            return int(n.value), None
+        idx_out = torch.empty(int(n.value), dtype=torch.int64, device="cuda:%d" % ctx.device)
+    rc = L.argus_healpix_footprint(ctx._h, C.byref(w), W, H, nside, _dev(idx_out, torch.int64, "idx_out"),
+                                   idx_out.numel(), C.byref(n), _stream(stream))
+    _check(ctx, rc, "argus_healpix_footprint")
+    return int(n.value), idx_out[: int(n.value)]
+
+
+def argus_resample(ctx, wcs, W, H, nside, kernel, value_out, weight_out, idx=None, w_min=0.5, stream=None, **frame):
+    """A3-A5 (+A2 fused when raw/bias/dark/flat are given, else cal/mask).  Asynchronous."""
+    f = _frame_struct(**frame)
+    w = _wcs_struct(wcs)
+    n = idx.numel() if idx is not None else min(value_out.numel(), weight_out.numel())
+    if idx is not None and (value_out.numel() < n or weight_out.numel() < n):
+        raise ValueError("outputs smaller than idx")
+    rc = load_library().argus_resample(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min),
+                                       _dev(idx, torch.int64, "idx", allow_none=True), n,
+                                       _dev(value_out, torch.float32, "value_out"),
+                                       _dev(weight_out, torch.float32, "weight_out"), _stream(stream))
+    _check(ctx, rc, "argus_resample")
+
+
+def _coadd_struct(tiles, nside_tile) -> _Coadd:
+    c = _Coadd()
+    c.tiles = _dev(tiles, torch.int64, "tiles")
+    c.n_tiles = tiles.numel()
+    c.nside_tile = int(nside_tile)
+    return c
+
+
+def argus_coadd_accumulate(ctx, tiles, nside_tile, nside, sum_, wsum, idx, value, weight, n_skipped=None, stream=None):
+    """A6 on an explicit (idx, value, weight) list.  Asynchronous."""
+    lay = _coadd_struct(tiles, nside_tile)
+    rc = load_library().argus_coadd_accumulate(ctx._h, C.byref(lay), nside, _dev(sum_, torch.float32, "sum"),
+                                               _dev(wsum, torch.float32, "wsum"), _dev(idx, torch.int64, "idx"),
+                                               _dev(value, torch.float32, "value"), _dev(weight, torch.float32, "weight"),
+                                               idx.numel(), _dev(n_skipped, torch.int64, "n_skipped", allow_none=True),
+                                               _stream(stream))
+    _check(ctx, rc, "argus_coadd_accumulate")
+
+
+def argus_resample_coadd(ctx, wcs, W, H, nside, kernel, tiles, nside_tile, sum_, wsum, n_skipped=None, w_min=0.5,
+                         stream=None, **frame):
+    """A2-A6 fused.  Asynchronous."""
+    f = _frame_struct(**frame)
+    w = _wcs_struct(wcs)
+    lay = _coadd_struct(tiles, nside_tile)
+    rc = load_library().argus_resample_coadd(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min),
+                                             C.byref(lay), _dev(sum_, torch.float32, "sum"),
+                                             _dev(wsum, torch.float32, "wsum"),
+                                             _dev(n_skipped, torch.int64, "n_skipped", allow_none=True), _stream(stream))
+    _check(ctx, rc, "argus_resample_coadd")
+
+
+def argus_plan_info(ctx, stream=None) -> dict:
+    s = _PlanStats()
+    rc = load_library().argus_plan_info(ctx._h, C.byref(s), _stream(stream))
+    _check(ctx, rc, "argus_plan_info")
+    return {n: int(getattr(s, n)) for n, _ in _PlanStats._fields_}

@@ -1,0 +1,487 @@
+// argus_api.cu -- the C ABI declared in include/argus.h: validation, host-side frame constants (FP64),
+// coarse cell selection, kernel launches.  Every step of the hot path runs in the kernels of
+// plan.cuh / resample.cuh; nothing here touches pixel data.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/argus.h"
+#include "resample.cuh"
+
+#define ARGUS_VERSION_NUM 100
+
+struct argus_ctx {
+    int device;
+    int last_cuda;
+    int sm_count;
+    bool plan_cache;
+    bool plan_valid;
+    argus_wcs key_wcs;
+    int64_t key_W, key_H, key_nside;
+    DevWcs dw;
+    PlanBuffers pb;
+    PlanStats* h_stats;   // pinned
+    void* d_block;        // the single device allocation behind pb
+};
+
+static const double kPi = 3.14159265358979323846264338327950288;
+
+#define CUDA_TRY(ctx, expr)                          \
+    do {                                             \
+        cudaError_t e_ = (expr);                     \
+        if (e_ != cudaSuccess) {                     \
+            if (ctx) (ctx)->last_cuda = (int)e_;     \
+            return ARGUS_ERR_CUDA;                   \
+        }                                            \
+    } while (0)
+
+extern "C" const char* argus_strerror(int s) {
+    switch (s) {
+        case ARGUS_OK: return "ok";
+        case ARGUS_ERR_NULL: return "required pointer is NULL";
+        case ARGUS_ERR_SHAPE: return "size argument out of range";
+        case ARGUS_ERR_NSIDE: return "nside must be a power of two in [32, 2^29]";
+        case ARGUS_ERR_KERNEL: return "unknown interpolation kernel";
+        case ARGUS_ERR_WCS: return "invalid WCS (singular CD, non-finite value or bad sip_order)";
+        case ARGUS_ERR_CAPACITY: return "capacity too small";
+        case ARGUS_ERR_ALIGN: return "pointer not aligned to its element type";
+        case ARGUS_ERR_CUDA: return "CUDA runtime error (see argus_last_cuda_error)";
+        case ARGUS_ERR_STATE: return "call sequence error";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int argus_version(void) { return ARGUS_VERSION_NUM; }
+
+// ---------------------------------------------------------------------------------------- context
+static void lsq_pinv(double* pinv /*[10][25]*/) {
+    // design matrix of the 5x5 node grid S,T in {-1,-.5,0,.5,1}; pinv = (A^T A)^-1 A^T
+    double A[25][10];
+    for (int n = 0; n < 25; ++n) {
+        double S = -1.0 + 0.5 * (n % 5), T = -1.0 + 0.5 * (n / 5);
+        double m[10] = {1.0, S, T, S * S, S * T, T * T, S * S * S, S * S * T, S * T * T, T * T * T};
+        for (int i = 0; i < 10; ++i) A[n][i] = m[i];
+    }
+    double G[10][20];
+    for (int i = 0; i < 10; ++i)
+        for (int j = 0; j < 10; ++j) {
+            double s = 0;
+            for (int n = 0; n < 25; ++n) s += A[n][i] * A[n][j];
+            G[i][j] = s;
+            G[i][10 + j] = (i == j) ? 1.0 : 0.0;
+        }
+    for (int c = 0; c < 10; ++c) {   // Gauss-Jordan with partial pivoting
+        int piv = c;
+        for (int r = c + 1; r < 10; ++r)
+            if (fabs(G[r][c]) > fabs(G[piv][c])) piv = r;
+        if (piv != c)
+            for (int j = 0; j < 20; ++j) { double t = G[c][j]; G[c][j] = G[piv][j]; G[piv][j] = t; }
+        double d = 1.0 / G[c][c];
+        for (int j = 0; j < 20; ++j) G[c][j] *= d;
+        for (int r = 0; r < 10; ++r)
+            if (r != c) {
+                double fct = G[r][c];
+                for (int j = 0; j < 20; ++j) G[r][j] -= fct * G[c][j];
+            }
+    }
+    for (int i = 0; i < 10; ++i)
+        for (int n = 0; n < 25; ++n) {
+            double s = 0;
+            for (int j = 0; j < 10; ++j) s += G[i][10 + j] * A[n][j];
+            pinv[i * 25 + n] = s;
+        }
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) {
+    if (!out) return ARGUS_ERR_NULL;
+    *out = nullptr;
+    if (max_tiles == 0) max_tiles = 1 << 19;
+    if (max_tiles < 64 || max_tiles > (1 << 24)) return ARGUS_ERR_SHAPE;
+    argus_ctx* c = new (std::nothrow) argus_ctx();
+    if (!c) return ARGUS_ERR_CAPACITY;
+    memset(c, 0, sizeof(*c));
+    c->device = device;
+    c->plan_cache = true;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
+    PlanBuffers& pb = c->pb;
+    pb.max_tiles = (int)max_tiles;
+    pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
+    pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv;
+    o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
+    o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
+    o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
+    o_rec = o;   o = align_up(o + sizeof(TileRec) * pb.max_tiles, 256);
+    o_cnt = o;   o = align_up(o + sizeof(int) * pb.max_tiles, 256);
+    o_off = o;   o = align_up(o + sizeof(long long) * (pb.max_tiles + 1), 256);
+    o_nt = o;    o = align_up(o + sizeof(int), 256);
+    o_hc = o;    o = align_up(o + sizeof(int), 256);
+    o_hl = o;    o = align_up(o + sizeof(int) * pb.max_hard, 256);
+    o_mask = o;  o = align_up(o + sizeof(unsigned) * 32 * (size_t)pb.max_hard, 256);
+    o_stats = o; o = align_up(o + sizeof(PlanStats), 256);
+    o_pinv = o;  o = align_up(o + sizeof(double) * 250, 256);
+    e = cudaMalloc(&c->d_block, o);
+    if (e == cudaSuccess) e = cudaMemset(c->d_block, 0, o);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
+    if (e != cudaSuccess) {
+        if (c->d_block) cudaFree(c->d_block);
+        delete c;
+        return ARGUS_ERR_CUDA;
+    }
+    char* b = (char*)c->d_block;
+    pb.slot_flag = (unsigned char*)(b + o_flag);
+    pb.block_count = (int*)(b + o_bc);
+    pb.tile_id = (long long*)(b + o_tid);
+    pb.rec = (TileRec*)(b + o_rec);
+    pb.tile_count = (int*)(b + o_cnt);
+    pb.tile_offset = (long long*)(b + o_off);
+    pb.n_tiles = (int*)(b + o_nt);
+    pb.hard_count = (int*)(b + o_hc);
+    pb.hard_list = (int*)(b + o_hl);
+    pb.masks = (unsigned*)(b + o_mask);
+    pb.stats = (PlanStats*)(b + o_stats);
+    pb.pinv = (double*)(b + o_pinv);
+    double pinv[250];
+    lsq_pinv(pinv);
+    e = cudaMemcpy(pb.pinv, pinv, sizeof(pinv), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(c->d_block);
+        cudaFreeHost(c->h_stats);
+        delete c;
+        return ARGUS_ERR_CUDA;
+    }
+    *out = c;
+    return ARGUS_OK;
+}
+
+extern "C" int argus_ctx_destroy(argus_ctx* c) {
+    if (!c) return ARGUS_ERR_NULL;
+    cudaSetDevice(c->device);
+    cudaFree(c->d_block);
+    cudaFreeHost(c->h_stats);
+    delete c;
+    return ARGUS_OK;
+}
+
+extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
+    if (!c) return ARGUS_ERR_NULL;
+    if (option == ARGUS_OPT_PLAN_CACHE) {
+        c->plan_cache = value != 0;
+        if (!c->plan_cache) c->plan_valid = false;
+        return ARGUS_OK;
+    }
+    return ARGUS_ERR_SHAPE;
+}
+
+extern "C" int argus_last_cuda_error(const argus_ctx* c) { return c ? c->last_cuda : 0; }
+
+// ------------------------------------------------------------------------------- frame constants
+static bool is_pow2(int64_t v) { return v > 0 && (v & (v - 1)) == 0; }
+static int ilog2(int64_t v) { int k = 0; while ((1ll << k) < v) ++k; return k; }
+
+static int make_devwcs(const argus_wcs* w, int64_t W, int64_t H, int64_t nside, DevWcs* d, double* rho_max,
+                       double* scale_rad) {
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20)) return ARGUS_ERR_SHAPE;
+    if (!is_pow2(nside) || nside < 32 || nside > (1ll << 29)) return ARGUS_ERR_NSIDE;
+    if (w->sip_order < 0 || w->sip_order > 5 || w->sip_order == 1) return ARGUS_ERR_WCS;
+    const double* v = &w->crval[0];
+    for (int i = 0; i < 8; ++i)
+        if (!isfinite(v[i])) return ARGUS_ERR_WCS;   // crval, crpix, cd are contiguous doubles
+    for (int i = 0; i < 36; ++i)
+        if (!isfinite(w->ap[i]) || !isfinite(w->bp[i])) return ARGUS_ERR_WCS;
+    double det = w->cd[0][0] * w->cd[1][1] - w->cd[0][1] * w->cd[1][0];
+    if (!(fabs(det) > 1e-300)) return ARGUS_ERR_WCS;
+    double a0 = w->crval[0] * kPi / 180.0, d0 = w->crval[1] * kPi / 180.0;
+    double sa = sin(a0), ca = cos(a0), sd = sin(d0), cd = cos(d0);
+    d->er[0] = cd * ca; d->er[1] = cd * sa; d->er[2] = sd;
+    d->ee[0] = -sa;     d->ee[1] = ca;      d->ee[2] = 0.0;
+    d->en[0] = -sd * ca; d->en[1] = -sd * sa; d->en[2] = cd;
+    double r2d = 180.0 / kPi;
+    d->m[0][0] = w->cd[1][1] / det * r2d;  d->m[0][1] = -w->cd[0][1] / det * r2d;
+    d->m[1][0] = -w->cd[1][0] / det * r2d; d->m[1][1] = w->cd[0][0] / det * r2d;
+    d->crpix[0] = w->crpix[0]; d->crpix[1] = w->crpix[1];
+    double s_rad = sqrt(fabs(det)) * kPi / 180.0;
+    double rho = atan(1.25 * s_rad * hypot((double)W, (double)H) / 2.0);
+    d->cos_rho = cos(rho);
+    for (int i = 0; i < 36; ++i) { d->ap[i] = w->ap[i]; d->bp[i] = w->bp[i]; }
+    d->sip_order = w->sip_order;
+    d->W = (int)W; d->H = (int)H;
+    d->k = ilog2(nside);
+    d->nside = (double)nside;
+    d->tile_ang = 1.3 * 32.0 / (double)nside;
+    *rho_max = rho;
+    *scale_rad = s_rad;
+    return ARGUS_OK;
+}
+
+// host-side centre of a nested cell (only used to pick the coarse candidate cells)
+static void host_cell_centre(int64_t nside, int64_t p, double v[3]) {
+    int k = ilog2(nside), face, ix, iy;
+    nest_to_xyf(p, k, face, ix, iy);
+    double ns = (double)nside;
+    int64_t jr = (int64_t)face_ring_offset(face) * nside - ix - iy - 1;
+    double z, sth, nr;
+    if (jr < nside) { nr = (double)jr; double t = nr * nr / (3 * ns * ns); z = 1 - t; sth = sqrt(t * (2 - t)); }
+    else if (jr > 3 * nside) { nr = (double)(4 * nside - jr); double t = nr * nr / (3 * ns * ns); z = t - 1; sth = sqrt(t * (2 - t)); }
+    else { nr = ns; z = (2.0 / 3.0) * (2.0 - jr / ns); sth = sqrt((1 - z) * (1 + z)); }
+    double phi = (kPi / 4) * (face_phi_offset(face) + (double)(ix - iy) / nr);
+    v[0] = sth * cos(phi); v[1] = sth * sin(phi); v[2] = z;
+}
+
+static void coarse_descend(const double er[3], double rho, int64_t nside_c, int64_t p, int64_t stop,
+                           std::vector<long long>& out) {
+    double v[3];
+    host_cell_centre(nside_c, p, v);
+    double dx = v[0] - er[0], dy = v[1] - er[1], dz = v[2] - er[2];
+    double ang = 2.0 * asin(fmin(1.0, 0.5 * sqrt(dx * dx + dy * dy + dz * dz)));
+    if (ang > rho + 1.3 / (double)nside_c) return;
+    if (nside_c >= stop) { out.push_back(p); return; }
+    for (int c = 0; c < 4; ++c) coarse_descend(er, rho, 2 * nside_c, 4 * p + c, stop, out);
+}
+
+static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside) {
+    return c->plan_cache && c->plan_valid && c->key_W == W && c->key_H == H && c->key_nside == nside &&
+           memcmp(&c->key_wcs, w, sizeof(argus_wcs)) == 0;
+}
+
+// Enqueue the plan kernels (A0 + A1).  No host synchronisation.
+static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
+                      cudaStream_t st) {
+    DevWcs dw;
+    double rho, s_rad;
+    int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
+    if (rc) return rc;
+    if (same_key(c, w, W, H, nside)) return ARGUS_OK;
+    c->plan_valid = false;
+    int64_t nside_t = nside >> ARGUS_TILE_LOG2;
+    // coarse resolution: cells comparable to the search cone, list passed by value
+    int64_t nside_c = 1;
+    while (nside_c < nside_t && (double)nside_c < 2.0 / rho) nside_c <<= 1;
+    std::vector<long long> cells;
+    for (;;) {
+        cells.clear();
+        for (int b = 0; b < 12; ++b) coarse_descend(dw.er, rho, 1, b, nside_c, cells);
+        if ((int)cells.size() <= ARGUS_MAX_COARSE || nside_c == 1) break;
+        nside_c >>= 1;
+    }
+    if ((int)cells.size() > ARGUS_MAX_COARSE) return ARGUS_ERR_CAPACITY;
+    CoarseList cl;
+    memset(&cl, 0, sizeof(cl));
+    cl.n = (int)cells.size();
+    cl.ratio_log2 = ilog2(nside_t / nside_c);
+    for (int i = 0; i < cl.n; ++i) cl.cell[i] = cells[i];
+    long long n_slots = (long long)cl.n << (2 * cl.ratio_log2);
+    if (cl.ratio_log2 > 12 || n_slots > c->pb.max_slots) return ARGUS_ERR_CAPACITY;
+    if (n_slots == 0) n_slots = 1;
+    double rad_px = 1.05 * dw.tile_ang / s_rad + 2.0;
+    int nblk = (int)((n_slots + 255) / 256);
+    plan_scan_kernel<<<nblk, 256, 0, st>>>(dw, cl, c->pb, rad_px);
+    plan_compact_kernel<<<nblk, 256, 0, st>>>(cl, c->pb);
+    plan_fit_kernel<<<c->sm_count * 4, 32 * FIT_WARPS, 0, st>>>(dw, c->pb);
+    plan_members_kernel<<<c->sm_count * 4, 256, 0, st>>>(dw, c->pb);
+    plan_offsets_kernel<<<1, 1024, 0, st>>>(c->pb, out_cap);
+    CUDA_TRY(c, cudaGetLastError());
+    c->dw = dw;
+    c->key_wcs = *w;
+    c->key_W = W; c->key_H = H; c->key_nside = nside;
+    c->plan_valid = true;
+    return ARGUS_OK;
+}
+
+static bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+static int make_frameargs(const argus_frame* fr, int64_t W, FrameArgs* f, bool* fused) {
+    memset(f, 0, sizeof(*f));
+    if (fr->raw) {
+        if (!fr->bias || !fr->dark || !fr->flat) return ARGUS_ERR_NULL;
+        if (!aligned(fr->raw, 2) || !aligned(fr->bias, 4) || !aligned(fr->dark, 4) || !aligned(fr->flat, 4)) return ARGUS_ERR_ALIGN;
+        f->raw = fr->raw; f->bias = fr->bias; f->dark = fr->dark; f->flat = fr->flat; f->bpm = fr->bpm;
+        f->t_exp = fr->t_exp; f->flat_min = fr->flat_min; f->sat_adu = fr->sat_adu;
+        f->vec_ok = (W % 4 == 0) && aligned(fr->raw, 8) && aligned(fr->bias, 16) && aligned(fr->dark, 16) &&
+                    aligned(fr->flat, 16) && (!fr->bpm || aligned(fr->bpm, 4));
+        *fused = true;
+    } else {
+        if (!fr->cal || !fr->mask) return ARGUS_ERR_NULL;
+        if (!aligned(fr->cal, 4)) return ARGUS_ERR_ALIGN;
+        f->cal = fr->cal; f->mask = fr->mask;
+        f->vec_ok = (W % 4 == 0) && aligned(fr->cal, 16) && aligned(fr->mask, 4);
+        *fused = false;
+    }
+    return ARGUS_OK;
+}
+
+// ------------------------------------------------------------------------------------- A2 standalone
+extern "C" int argus_calibrate(argus_ctx* c, const uint16_t* raw, const float* bias, const float* dark,
+                               const float* flat, const uint8_t* bpm, int64_t W, int64_t H, float t_exp,
+                               int32_t sat_adu, float flat_min, float* cal_out, uint8_t* mask_out, void* stream) {
+    if (!c || !raw || !bias || !dark || !flat || !cal_out || !mask_out) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20)) return ARGUS_ERR_SHAPE;
+    argus_frame fr;
+    memset(&fr, 0, sizeof(fr));
+    fr.raw = raw; fr.bias = bias; fr.dark = dark; fr.flat = flat; fr.bpm = bpm;
+    fr.t_exp = t_exp; fr.sat_adu = sat_adu; fr.flat_min = flat_min;
+    FrameArgs f;
+    bool fused;
+    int rc = make_frameargs(&fr, W, &f, &fused);
+    if (rc) return rc;
+    if (!aligned(cal_out, 4)) return ARGUS_ERR_ALIGN;
+    long long n = W * H;
+    // the flat vector path needs n % 4 == 0 and aligned outputs (rows need not be aligned: 1-D sweep)
+    f.vec_ok = (n % 4 == 0) && aligned(raw, 8) && aligned(bias, 16) && aligned(dark, 16) && aligned(flat, 16) &&
+               (!bpm || aligned(bpm, 4)) && aligned(cal_out, 16) && aligned(mask_out, 4);
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    calibrate_kernel<<<c->sm_count * 8, 256, 0, (cudaStream_t)stream>>>(f, n, cal_out, mask_out);
+    CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+// --------------------------------------------------------------------------------------- A0 + A1
+static int fetch_stats(argus_ctx* c, cudaStream_t st) {
+    CUDA_TRY(c, cudaMemcpyAsync(c->h_stats, c->pb.stats, sizeof(PlanStats), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    return ARGUS_OK;
+}
+
+extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64_t W, int64_t H, int64_t nside,
+                                       int64_t* idx_out, size_t capacity, size_t* n_out, void* stream) {
+    if (!c || !wcs || !n_out) return ARGUS_ERR_NULL;
+    if (idx_out && !aligned(idx_out, 8)) return ARGUS_ERR_ALIGN;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    int rc = build_plan(c, wcs, W, H, nside, -1, st);
+    if (rc) return rc;
+    rc = fetch_stats(c, st);
+    if (rc) return rc;
+    *n_out = (size_t)c->h_stats->n_footprint;
+    if (c->h_stats->overflow & 3) { c->plan_valid = false; return ARGUS_ERR_CAPACITY; }
+    if (idx_out) {
+        if ((size_t)c->h_stats->n_footprint > capacity) return ARGUS_ERR_CAPACITY;
+        plan_write_indices_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->pb, (long long*)idx_out, (long long)capacity);
+        CUDA_TRY(c, cudaGetLastError());
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+    }
+    return ARGUS_OK;
+}
+
+extern "C" int argus_plan_info(argus_ctx* c, argus_plan_stats* out, void* stream) {
+    if (!c || !out) return ARGUS_ERR_NULL;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    int rc = fetch_stats(c, (cudaStream_t)stream);
+    if (rc) return rc;
+    const PlanStats* s = c->h_stats;
+    out->n_footprint = s->n_footprint; out->n_tiles = s->n_tiles; out->n_inside = s->n_inside;
+    out->n_border = s->n_border; out->n_exact = s->n_exact; out->n_empty = s->n_empty;
+    if (s->overflow) { c->plan_valid = false; return ARGUS_ERR_CAPACITY; }
+    return ARGUS_OK;
+}
+
+// ------------------------------------------------------------------------------------- A3..A6
+template <bool COADD>
+static void launch_tiles(argus_ctx* c, int kernel, bool fused, const FrameArgs& f, float w_min, float* v, float* wt,
+                         long long cap, const CoaddArgs& ca, cudaStream_t st) {
+    int grid = c->sm_count * 8;
+#define LT(K, F) resample_tiles_kernel<K, F, COADD><<<grid, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca)
+    if (kernel == ARGUS_BILINEAR) { if (fused) LT(0, true); else LT(0, false); }
+    else { if (fused) LT(1, true); else LT(1, false); }
+#undef LT
+}
+
+extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                              int64_t nside, int kernel, float w_min, const int64_t* idx, size_t n, float* value_out,
+                              float* weight_out, void* stream) {
+    if (!c || !frame || !wcs || !value_out || !weight_out) return ARGUS_ERR_NULL;
+    if (kernel != ARGUS_BILINEAR && kernel != ARGUS_LANCZOS3) return ARGUS_ERR_KERNEL;
+    if (!aligned(value_out, 4) || !aligned(weight_out, 4) || (idx && !aligned(idx, 8))) return ARGUS_ERR_ALIGN;
+    if (n > ((size_t)1 << 40)) return ARGUS_ERR_SHAPE;
+    FrameArgs f;
+    bool fused;
+    int rc = make_frameargs(frame, W, &f, &fused);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (idx) {
+        DevWcs dw;
+        double rho, s_rad;
+        rc = make_devwcs(wcs, W, H, nside, &dw, &rho, &s_rad);
+        if (rc) return rc;
+        if (n == 0) return ARGUS_OK;
+        int nblk = (int)((n + 255) / 256);
+        const long long* ip = (const long long*)idx;
+#define LL(K, F) resample_list_kernel<K, F><<<nblk, 256, 0, st>>>(dw, f, w_min, ip, (long long)n, value_out, weight_out)
+        if (kernel == ARGUS_BILINEAR) { if (fused) LL(0, true); else LL(0, false); }
+        else { if (fused) LL(1, true); else LL(1, false); }
+#undef LL
+        CUDA_TRY(c, cudaGetLastError());
+        return ARGUS_OK;
+    }
+    rc = build_plan(c, wcs, W, H, nside, (long long)n, st);
+    if (rc) return rc;
+    CoaddArgs ca;
+    memset(&ca, 0, sizeof(ca));
+    launch_tiles<false>(c, kernel, fused, f, w_min, value_out, weight_out, (long long)n, ca, st);
+    CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+static int make_coaddargs(const argus_coadd* lay, int64_t nside, float* sum, float* wsum, int64_t* skipped,
+                          CoaddArgs* ca, int* ppt_log2) {
+    if (!lay || !lay->tiles || !sum || !wsum) return ARGUS_ERR_NULL;
+    if (!is_pow2(nside) || nside < 32 || nside > (1ll << 29)) return ARGUS_ERR_NSIDE;
+    if (!is_pow2(lay->nside_tile) || lay->nside_tile > (nside >> ARGUS_TILE_LOG2) || lay->n_tiles < 0) return ARGUS_ERR_SHAPE;
+    if (!aligned(lay->tiles, 8) || !aligned(sum, 4) || !aligned(wsum, 4) || (skipped && !aligned(skipped, 8))) return ARGUS_ERR_ALIGN;
+    int kk = ilog2(nside) - ilog2(lay->nside_tile);
+    ca->tiles = (const long long*)lay->tiles;
+    ca->n_tiles = lay->n_tiles;
+    ca->shift = 2 * kk - 10;
+    ca->sum = sum; ca->wsum = wsum;
+    ca->n_skipped = (unsigned long long*)skipped;
+    *ppt_log2 = 2 * kk;
+    return ARGUS_OK;
+}
+
+extern "C" int argus_coadd_accumulate(argus_ctx* c, const argus_coadd* layout, int64_t nside, float* sum, float* wsum,
+                                      const int64_t* idx, const float* value, const float* weight, size_t n,
+                                      int64_t* n_skipped_dev, void* stream) {
+    if (!c || !idx || !value || !weight) return ARGUS_ERR_NULL;
+    CoaddArgs ca;
+    int ppt_log2;
+    int rc = make_coaddargs(layout, nside, sum, wsum, n_skipped_dev, &ca, &ppt_log2);
+    if (rc) return rc;
+    if (!aligned(idx, 8) || !aligned(value, 4) || !aligned(weight, 4)) return ARGUS_ERR_ALIGN;
+    if (n == 0) return ARGUS_OK;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    coadd_list_kernel<<<(int)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(ca, ppt_log2, (const long long*)idx, value,
+                                                                              weight, (long long)n);
+    CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                                    int64_t nside, int kernel, float w_min, const argus_coadd* layout, float* sum,
+                                    float* wsum, int64_t* n_skipped_dev, void* stream) {
+    if (!c || !frame || !wcs) return ARGUS_ERR_NULL;
+    if (kernel != ARGUS_BILINEAR && kernel != ARGUS_LANCZOS3) return ARGUS_ERR_KERNEL;
+    CoaddArgs ca;
+    int ppt_log2;
+    int rc = make_coaddargs(layout, nside, sum, wsum, n_skipped_dev, &ca, &ppt_log2);
+    if (rc) return rc;
+    FrameArgs f;
+    bool fused;
+    rc = make_frameargs(frame, W, &f, &fused);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    rc = build_plan(c, wcs, W, H, nside, -1, st);
+    if (rc) return rc;
+    launch_tiles<true>(c, kernel, fused, f, w_min, nullptr, nullptr, 0, ca, st);
+    CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}

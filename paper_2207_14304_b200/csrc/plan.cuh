@@ -1,0 +1,419 @@
+// plan.cuh -- A0/A1: the per-frame resampling plan, built entirely on the device (no host sync).
+//
+//   scan    : every tile-level child of the host-chosen coarse cells is tested with one exact FP64
+//             evaluation of its centre (conservative radius) -> flag + per-block count
+//   compact : order-preserving compaction -> ascending list of candidate tiles
+//   fit     : one warp per tile: 25 exact nodes -> least-squares cubic in local coordinates, residual
+//             check against 7 extra exact points, classification (inside / border / exact / empty)
+//   members : border / exact tiles: per-pixel membership mask (exact FP64 decision inside a guard band),
+//             count and source bounding box
+//   offsets : exclusive scan of the per-tile counts -> output positions, statistics
+//
+// The footprint (A1) is represented as this range plan; argus_healpix_footprint expands it
+// into the explicit ascending int64 list on request.
+#pragma once
+#include "common.cuh"
+
+#define PLAN_GUARD_PX 2e-5f      // |distance to the domain border| below which membership is decided in FP64
+#define PLAN_FIT_TOL 3e-8        // max residual (px) of the cubic fit at the 32 exact points
+#define PLAN_NODE_MARGIN 0.25    // px margin on node extents for the inside / empty classification
+
+struct PlanBuffers {
+    unsigned char* slot_flag;   // [max_slots]
+    int* block_count;           // [max_slots/256]
+    long long* tile_id;         // [max_tiles]
+    TileRec* rec;               // [max_tiles]
+    int* tile_count;            // [max_tiles]
+    long long* tile_offset;     // [max_tiles + 1]
+    int* n_tiles;               // device scalar
+    int* hard_count;            // device scalar
+    int* hard_list;             // [max_hard] tile positions
+    unsigned* masks;            // [max_hard][32]
+    PlanStats* stats;           // device
+    double* pinv;               // [10][25] least-squares pseudo-inverse of the node design matrix
+    int max_slots, max_tiles, max_hard;
+};
+
+// --------------------------------------------------------------------------------------------- scan
+__global__ void __launch_bounds__(256) plan_scan_kernel(DevWcs w, CoarseList cl, PlanBuffers pb, double rad_px) {
+    long long slot = (long long)blockIdx.x * 256 + threadIdx.x;
+    long long n_slots = (long long)cl.n << (2 * cl.ratio_log2);
+    int keep = 0;
+    if (slot < n_slots) {
+        int c = (int)(slot >> (2 * cl.ratio_log2));
+        long long tile = (cl.cell[c] << (2 * cl.ratio_log2)) | (slot & ((1ll << (2 * cl.ratio_log2)) - 1));
+        int face, tx, ty;
+        nest_to_xyf(tile, w.k - ARGUS_TILE_LOG2, face, tx, ty);
+        double ixc = tx * 32.0 + 15.5, iyc = ty * 32.0 + 15.5;
+        long long ns = 1ll << w.k;
+        long long jr = (long long)face_ring_offset(face) * ns - (long long)(ixc + iyc) - 1;
+        double v[3], x, y;
+        hp_vec(face, ixc, iyc, w.nside, ring_zone(jr, ns), v);
+        double cosc = vec_to_xy(w, v, x, y);
+        if (cosc > 0.05 && cosc >= w.cos_rho - w.tile_ang) {
+            keep = (x >= -0.5 - rad_px) && (x < w.W - 0.5 + rad_px) && (y >= -0.5 - rad_px) && (y < w.H - 0.5 + rad_px);
+        }
+        pb.slot_flag[slot] = (unsigned char)keep;
+    }
+    int cnt = __syncthreads_count(keep);
+    if (threadIdx.x == 0) pb.block_count[blockIdx.x] = cnt;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        *pb.hard_count = 0;
+        pb.stats->overflow = 0;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ compact
+__global__ void __launch_bounds__(256) plan_compact_kernel(CoarseList cl, PlanBuffers pb) {
+    __shared__ int s_part[8];
+    __shared__ int s_base;
+    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    // prefix of the block counts before this block
+    int acc = 0;
+    for (int b = tid; b < (int)blockIdx.x; b += 256) acc += pb.block_count[b];
+    for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) s_part[wid] = acc;
+    __syncthreads();
+    if (tid == 0) {
+        int t = 0;
+        for (int i = 0; i < 8; ++i) t += s_part[i];
+        s_base = t;
+    }
+    __syncthreads();
+    int base = s_base;
+    __syncthreads();
+    long long slot = (long long)blockIdx.x * 256 + tid;
+    long long n_slots = (long long)cl.n << (2 * cl.ratio_log2);
+    int keep = (slot < n_slots) ? pb.slot_flag[slot] : 0;
+    unsigned bal = __ballot_sync(0xffffffffu, keep);
+    if (lane == 0) s_part[wid] = __popc(bal);
+    __syncthreads();
+    int woff = 0;
+    for (int i = 0; i < wid; ++i) woff += s_part[i];
+    int pos = base + woff + __popc(bal & ((1u << lane) - 1u));
+    if (keep) {
+        if (pos < pb.max_tiles) {
+            int c = (int)(slot >> (2 * cl.ratio_log2));
+            pb.tile_id[pos] = (cl.cell[c] << (2 * cl.ratio_log2)) | (slot & ((1ll << (2 * cl.ratio_log2)) - 1));
+        } else {
+            atomicOr(&pb.stats->overflow, 1);
+        }
+    }
+    if (blockIdx.x == gridDim.x - 1 && tid == 0) {
+        int total = base;
+        for (int i = 0; i < 8; ++i) total += s_part[i];
+        *pb.n_tiles = total < pb.max_tiles ? total : pb.max_tiles;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------- fit
+__device__ inline double warp_min(double v) {
+    for (int o = 16; o; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ inline double warp_max(double v) {
+    for (int o = 16; o; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// monomials of the total-degree-3 basis at (S, T)
+__device__ inline void cubic_basis(double S, double T, double m[10]) {
+    m[0] = 1.0; m[1] = S; m[2] = T; m[3] = S * S; m[4] = S * T; m[5] = T * T;
+    m[6] = S * S * S; m[7] = S * S * T; m[8] = S * T * T; m[9] = T * T * T;
+}
+
+#define FIT_WARPS 8
+__global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, PlanBuffers pb) {
+    __shared__ double s_pinv[250];
+    __shared__ double s_coef[FIT_WARPS][20];
+    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int i = tid; i < 250; i += blockDim.x) s_pinv[i] = pb.pinv[i];
+    __syncthreads();
+    int n_tiles = *pb.n_tiles;
+    long long ns = 1ll << w.k;
+    // node coordinates: lanes 0..24 the 5x5 fit grid, lanes 25..31 extra check points
+    double S, T;
+    if (lane < 25) {
+        S = -1.0 + 0.5 * (lane % 5);
+        T = -1.0 + 0.5 * (lane / 5);
+    } else {
+        const double cs[7] = {0.77, -0.77, 0.33, -0.33, 0.9, -0.2, 0.61};
+        const double ct[7] = {0.33, 0.61, -0.77, -0.9, 0.9, 0.15, -0.41};
+        S = cs[lane - 25];
+        T = ct[lane - 25];
+    }
+    for (int t = blockIdx.x * FIT_WARPS + wid; t < n_tiles; t += gridDim.x * FIT_WARPS) {
+        long long tile = pb.tile_id[t];
+        int face, tx, ty;
+        nest_to_xyf(tile, w.k - ARGUS_TILE_LOG2, face, tx, ty);
+        int ix0 = tx * 32, iy0 = ty * 32;
+        long long jr_max = (long long)face_ring_offset(face) * ns - ix0 - iy0 - 1, jr_min = jr_max - 62;
+        int z0 = ring_zone(jr_min, ns), z1 = ring_zone(jr_max, ns);
+        TileRec r;
+        r.tile = tile; r.offset = 0; r.count = 0; r.mask_slot = -1;
+        r.zone = (z0 == z1) ? z0 : -1;
+        r.bx0 = r.bx1 = r.by0 = r.by1 = 0; r.X0 = r.Y0 = 0; r.ax = r.bx = r.ay = r.by = 0;
+        r.pad[0] = r.pad[1] = 0;
+        for (int i = 0; i < 10; ++i) { r.cx[i] = 0.f; r.cy[i] = 0.f; }
+        int cls = TC_EXACT;
+        if (z0 == z1) {
+            double v[3], x, y;
+            hp_vec(face, ix0 + 15.5 + 16.0 * S, iy0 + 15.5 + 16.0 * T, w.nside, z0, v);
+            double cosc = vec_to_xy(w, v, x, y);
+            bool node = lane < 25;
+            double xmin = warp_min(node ? x : 1e300), xmax = warp_max(node ? x : -1e300);
+            double ymin = warp_min(node ? y : 1e300), ymax = warp_max(node ? y : -1e300);
+            double cmin = warp_min(cosc), cmax = warp_max(cosc);
+            double xc = __shfl_sync(0xffffffffu, x, 12), yc = __shfl_sync(0xffffffffu, y, 12);
+            // least squares: lanes 0..9 -> x coefficients, lanes 10..19 -> y coefficients
+            double acc = 0.0;
+            int row = lane < 10 ? lane : lane - 10;
+            for (int n = 0; n < 25; ++n) {
+                double xn = __shfl_sync(0xffffffffu, x, n) - xc, yn = __shfl_sync(0xffffffffu, y, n) - yc;
+                if (lane < 20) acc = fma(s_pinv[row * 25 + n], lane < 10 ? xn : yn, acc);
+            }
+            if (lane == 0) acc += xc;
+            if (lane == 10) acc += yc;
+            if (lane < 20) s_coef[wid][lane] = acc;
+            __syncwarp();
+            double m[10];
+            cubic_basis(S, T, m);
+            double fxv = 0.0, fyv = 0.0;
+            for (int i = 0; i < 10; ++i) {
+                fxv = fma(s_coef[wid][i], m[i], fxv);
+                fyv = fma(s_coef[wid][10 + i], m[i], fyv);
+            }
+            double res = warp_max(fmax(fabs(fxv - x), fabs(fyv - y)));
+            bool finite_ok = (xmin > -1e8) && (xmax < 1e8) && (ymin > -1e8) && (ymax < 1e8) && (cmin > 0.05);
+            bool fit_ok = finite_ok && (res <= PLAN_FIT_TOL);   // NaN compares false
+            double mg = PLAN_NODE_MARGIN;
+            bool cone_in = cmin - w.tile_ang >= w.cos_rho, cone_out = cmax + w.tile_ang < w.cos_rho;
+            if (fit_ok && !cone_out) {
+                bool all_out = (xmax + mg < -0.5) || (xmin - mg >= w.W - 0.5) || (ymax + mg < -0.5) || (ymin - mg >= w.H - 0.5);
+                bool all_in = (xmin - mg >= -0.5) && (xmax + mg < w.W - 0.5) && (ymin - mg >= -0.5) && (ymax + mg < w.H - 0.5);
+                if (all_out) cls = TC_EMPTY;
+                else if (cone_in) cls = all_in ? TC_INSIDE : TC_BORDER;
+                // cone-straddling tiles stay TC_EXACT
+            } else if (finite_ok && cone_out) {
+                cls = TC_EMPTY;
+            }
+            if (cls == TC_INSIDE || cls == TC_BORDER) {
+                // split: x = X0 + (a*s + b*t) 2^-12 + lo(S,T); s = 32 S, so c1 S = (c1/32) s
+                const double* cf = s_coef[wid];
+                for (int axis = 0; axis < 2; ++axis) {
+                    const double* c = cf + 10 * axis;
+                    double base = floor(c[0]);
+                    int a = (int)rint(c[1] * (4096.0 / 32.0)), b = (int)rint(c[2] * (4096.0 / 32.0));
+                    float* out = axis ? r.cy : r.cx;
+                    out[0] = (float)(c[0] - base);
+                    out[1] = (float)(c[1] - a * (32.0 / 4096.0));
+                    out[2] = (float)(c[2] - b * (32.0 / 4096.0));
+                    for (int i = 3; i < 10; ++i) out[i] = (float)c[i];
+                    if (axis) { r.Y0 = (int)base; r.ay = a; r.by = b; } else { r.X0 = (int)base; r.ax = a; r.bx = b; }
+                }
+                r.bx0 = (int)floor(xmin - mg); r.bx1 = (int)floor(xmax + mg);
+                r.by0 = (int)floor(ymin - mg); r.by1 = (int)floor(ymax + mg);
+                if (cls == TC_INSIDE) r.count = ARGUS_TILE_PIX;
+            }
+        }
+        if (lane == 0) {
+            if (cls == TC_BORDER || cls == TC_EXACT) {
+                int slot = atomicAdd(pb.hard_count, 1);
+                if (slot < pb.max_hard) {
+                    pb.hard_list[slot] = t;
+                    r.mask_slot = slot;
+                } else {
+                    atomicOr(&pb.stats->overflow, 2);
+                    cls = TC_EMPTY;
+                }
+            }
+            r.cls = cls;
+            pb.rec[t] = r;
+            pb.tile_count[t] = r.count;
+        }
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------ members
+// Thread -> 2x2 block of pixels = 4 consecutive Morton (nested) indices 4*tid .. 4*tid+3.
+__device__ inline void thread_block_origin(int tid, int& u0, int& v0) {
+    u0 = 2 * (int)compact_even_bits((unsigned)tid);
+    v0 = 2 * (int)compact_even_bits((unsigned)tid >> 1);
+}
+
+// Membership of pixel (u, v) of a TC_BORDER tile from the tile polynomial; the decision is re-taken in
+// FP64 with the exact mapping whenever the FP32 position is within PLAN_GUARD_PX of a border line.
+__device__ inline bool border_member(const DevWcs& w, const PolyAxis& px, const PolyAxis& py, int face, int ix0,
+                                     int iy0, int u, int v, int& ci, int& cj) {
+    float fx, fy;
+    poly_axis_eval(px, 2 * u - 31, 2 * v - 31, ci, fx);
+    poly_axis_eval(py, 2 * u - 31, 2 * v - 31, cj, fy);
+    bool near = ((ci == -1 || ci == w.W - 1) && fabsf(fx - 0.5f) < PLAN_GUARD_PX) ||
+                ((cj == -1 || cj == w.H - 1) && fabsf(fy - 0.5f) < PLAN_GUARD_PX);
+    if (near) {
+        double x, y;
+        double cosc = pixel_to_xy(w, face, ix0 + u, iy0 + v, x, y);
+        return in_domain(w, cosc, x, y);
+    }
+    bool inx = (ci >= 0 || (ci == -1 && fx >= 0.5f)) && (ci < w.W - 1 || (ci == w.W - 1 && fx < 0.5f));
+    bool iny = (cj >= 0 || (cj == -1 && fy >= 0.5f)) && (cj < w.H - 1 || (cj == w.H - 1 && fy < 0.5f));
+    return inx && iny;
+}
+
+__global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers pb) {
+    __shared__ unsigned s_mask[32];
+    __shared__ int s_ext[4];
+    __shared__ int s_cnt;
+    int tid = threadIdx.x;
+    int n_hard = *pb.hard_count;
+    if (n_hard > pb.max_hard) n_hard = pb.max_hard;
+    int u0, v0;
+    thread_block_origin(tid, u0, v0);
+    for (int h = blockIdx.x; h < n_hard; h += gridDim.x) {
+        int t = pb.hard_list[h];
+        if (tid < 32) s_mask[tid] = 0u;
+        if (tid == 0) { s_ext[0] = 0x7fffffff; s_ext[1] = -0x7fffffff; s_ext[2] = 0x7fffffff; s_ext[3] = -0x7fffffff; s_cnt = 0; }
+        __syncthreads();
+        const TileRec& r = pb.rec[t];
+        int face, tx, ty;
+        nest_to_xyf(r.tile, w.k - ARGUS_TILE_LOG2, face, tx, ty);
+        int ix0 = tx * 32, iy0 = ty * 32;
+        int cls = r.cls;
+        PolyAxis px, py;
+        if (cls == TC_BORDER) { poly_axis_load(r, 0, px); poly_axis_load(r, 1, py); }
+        unsigned nib = 0;
+        int xmin = 0x7fffffff, xmax = -0x7fffffff, ymin = 0x7fffffff, ymax = -0x7fffffff;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            int u = u0 + (q & 1), v = v0 + (q >> 1);
+            int ci, cj;
+            bool in;
+            if (cls == TC_BORDER) {
+                in = border_member(w, px, py, face, ix0, iy0, u, v, ci, cj);
+            } else {
+                double x, y;
+                double cosc = pixel_to_xy(w, face, ix0 + u, iy0 + v, x, y);
+                in = in_domain(w, cosc, x, y);
+                ci = in ? (int)floor(x) : 0;
+                cj = in ? (int)floor(y) : 0;
+            }
+            if (in) {
+                nib |= 1u << q;
+                xmin = min(xmin, ci); xmax = max(xmax, ci); ymin = min(ymin, cj); ymax = max(ymax, cj);
+            }
+        }
+        if (nib) {
+            atomicOr(&s_mask[tid >> 3], nib << (4 * (tid & 7)));
+            atomicMin(&s_ext[0], xmin); atomicMax(&s_ext[1], xmax);
+            atomicMin(&s_ext[2], ymin); atomicMax(&s_ext[3], ymax);
+            atomicAdd(&s_cnt, __popc(nib));
+        }
+        __syncthreads();
+        if (tid < 32) pb.masks[(size_t)h * 32 + tid] = s_mask[tid];
+        if (tid == 0) {
+            TileRec* wr = &pb.rec[t];
+            int c = s_cnt;
+            wr->count = c;
+            pb.tile_count[t] = c;
+            if (c == 0) {
+                wr->cls = TC_EMPTY;
+            } else {
+                wr->bx0 = s_ext[0]; wr->bx1 = s_ext[1]; wr->by0 = s_ext[2]; wr->by1 = s_ext[3];
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------ offsets
+// Single block: exclusive scan of the per-tile counts (<= ~1M tiles) + statistics.
+__global__ void __launch_bounds__(1024) plan_offsets_kernel(PlanBuffers pb, long long out_capacity) {
+    __shared__ long long s_warp[32];
+    __shared__ int s_cls[4];
+    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int n = *pb.n_tiles;
+    int per = (n + 1023) / 1024;
+    int b = tid * per, e = min(n, b + per);
+    if (tid < 4) s_cls[tid] = 0;
+    __syncthreads();
+    long long sum = 0;
+    int c_in = 0, c_bo = 0, c_ex = 0, c_em = 0;
+    for (int i = b; i < e; ++i) {
+        sum += pb.tile_count[i];
+        int cls = pb.rec[i].cls;
+        c_in += cls == TC_INSIDE; c_bo += cls == TC_BORDER; c_ex += cls == TC_EXACT; c_em += cls == TC_EMPTY;
+    }
+    long long inc = sum;
+    for (int o = 1; o < 32; o <<= 1) {
+        long long v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    atomicAdd(&s_cls[0], c_in); atomicAdd(&s_cls[1], c_bo); atomicAdd(&s_cls[2], c_ex); atomicAdd(&s_cls[3], c_em);
+    __syncthreads();
+    if (wid == 0) {
+        long long v = s_warp[lane], iv = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            long long u = __shfl_up_sync(0xffffffffu, iv, o);
+            if (lane >= o) iv += u;
+        }
+        s_warp[lane] = iv - v;  // exclusive
+    }
+    __syncthreads();
+    long long run = s_warp[wid] + inc - sum;
+    for (int i = b; i < e; ++i) {
+        pb.tile_offset[i] = run;
+        pb.rec[i].offset = run;
+        run += pb.tile_count[i];
+    }
+    __syncthreads();
+    if (tid == 0) {
+        long long total = (n > 0) ? pb.tile_offset[n - 1] + pb.tile_count[n - 1] : 0;
+        pb.tile_offset[n] = total;
+        PlanStats* st = pb.stats;
+        st->n_footprint = total;
+        st->n_tiles = n;
+        st->n_inside = s_cls[0]; st->n_border = s_cls[1]; st->n_exact = s_cls[2]; st->n_empty = s_cls[3];
+        if (out_capacity >= 0 && total > out_capacity) atomicOr(&st->overflow, 4);
+    }
+}
+
+// ------------------------------------------------------------------------------------ explicit list
+// Expands the range plan into the ascending int64 footprint list (A1's explicit form).
+__global__ void __launch_bounds__(256) plan_write_indices_kernel(PlanBuffers pb, long long* idx_out, long long capacity) {
+    __shared__ unsigned s_mask[32];
+    __shared__ int s_pref[33];
+    int tid = threadIdx.x;
+    int n = *pb.n_tiles;
+    for (int t = blockIdx.x; t < n; t += gridDim.x) {
+        const TileRec& r = pb.rec[t];
+        int cls = r.cls;
+        if (cls == TC_EMPTY) continue;
+        long long base = r.tile << 10, off = r.offset;
+        if (cls == TC_INSIDE) {
+            for (int q = 0; q < 4; ++q) {
+                int m = q * 256 + tid;
+                if (off + m < capacity) idx_out[off + m] = base + m;
+            }
+        } else {
+            __syncthreads();
+            if (tid < 32) s_mask[tid] = pb.masks[(size_t)r.mask_slot * 32 + tid];
+            __syncthreads();
+            if (tid == 0) {
+                int a = 0;
+                for (int i = 0; i < 32; ++i) { s_pref[i] = a; a += __popc(s_mask[i]); }
+                s_pref[32] = a;
+            }
+            __syncthreads();
+            for (int q = 0; q < 4; ++q) {
+                int m = q * 256 + tid;
+                unsigned wd = s_mask[m >> 5];
+                if ((wd >> (m & 31)) & 1u) {
+                    long long pos = off + s_pref[m >> 5] + __popc(wd & ((1u << (m & 31)) - 1u));
+                    if (pos < capacity) idx_out[pos] = base + m;
+                }
+            }
+        }
+    }
+}

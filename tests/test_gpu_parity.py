@@ -1,0 +1,212 @@
+"""GPU parity (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle, element by
+element on the same seeded inputs.  Footprints bit-exact; values within 1e-3 ADU + 1e-5 relative."""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+import synth  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def argus():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2207_14304_b200 as a
+    a.load_library()
+    return a
+
+
+@pytest.fixture(scope="module")
+def ctx(argus):
+    c = argus.Context(0)
+    yield c
+    c.close()
+
+
+def test_calibrate_matches_oracle(argus, ctx):
+    from gpu_util import upload
+    fr = synth.inject_defects(synth.config0())
+    d = upload(fr)
+    cal, mask = argus.argus_calibrate(ctx, d["raw"], d["bias"], d["dark"], d["flat"], d["bpm"], fr.t_exp, fr.sat_adu, fr.flat_min)
+    torch.cuda.synchronize()
+    oc, om = oracle.calibrate_frame(fr)
+    assert np.array_equal(mask.cpu().numpy(), om)
+    dv = np.abs(cal.cpu().numpy().astype(np.float64) - oc)
+    assert np.all(dv <= 1e-3 + 1e-5 * np.abs(oc))
+    assert om.sum() < om.size  # the defects are really there
+    # odd width: scalar path
+    fr2 = synth.make_frame(3, 37, 19, 5, fr.wcs, fr.nside, "bilinear")
+    d2 = upload(fr2)
+    cal2, mask2 = argus.argus_calibrate(ctx, d2["raw"], d2["bias"], d2["dark"], d2["flat"], None, fr2.t_exp)
+    oc2, om2 = oracle.calibrate_frame(fr2)
+    assert np.array_equal(mask2.cpu().numpy(), om2)
+    assert np.all(np.abs(cal2.cpu().numpy() - oc2) <= 1e-3 + 1e-5 * np.abs(oc2))
+
+
+def test_config0_footprint_bit_exact(argus, ctx, cfg0, cfg0_fp):
+    idx_or, dmin = cfg0_fp
+    n, idx = argus.argus_healpix_footprint(ctx, cfg0.wcs, 512, 512, cfg0.nside)
+    assert n == len(idx_or)
+    assert np.array_equal(idx.cpu().numpy(), idx_or)
+    info = argus.argus_plan_info(ctx)
+    assert info["n_footprint"] == n and info["n_inside"] > 0 and info["n_border"] > 0
+
+
+@pytest.mark.parametrize("kernel", ["bilinear", "lanczos3"])
+def test_config0_values(argus, ctx, cfg0, cfg0_fp, kernel):
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    idx_or, _ = cfg0_fp
+    d = upload(cfg0)
+    n, v, w = gpu_resample_planned(ctx, cfg0, d, kernel)
+    assert n == len(idx_or)
+    vo, wo, fl = oracle_reference(cfg0, idx_or, kernel)
+    assert_values_match(v, w, vo, wo, fl, "config0 planned " + kernel)
+    # general list path (explicit idx, FP64 coordinates), shuffled order
+    rng = np.random.default_rng(0)
+    perm = rng.permutation(len(idx_or))[:50000]
+    sub = torch.from_numpy(idx_or[perm]).cuda()
+    v2 = torch.empty(len(perm), dtype=torch.float32, device="cuda")
+    w2 = torch.empty_like(v2)
+    argus.argus_resample(ctx, cfg0.wcs, 512, 512, cfg0.nside, kernel, v2, w2, idx=sub, **d)
+    torch.cuda.synchronize()
+    assert_values_match(v2.cpu().numpy(), w2.cpu().numpy(), vo[perm], wo[perm], fl[perm], "config0 list " + kernel)
+
+
+def test_p10_fused_equals_unfused(argus, ctx, cfg0, cfg0_fp):
+    from gpu_util import gpu_resample_planned, upload
+    d = upload(cfg0)
+    n, v, w = gpu_resample_planned(ctx, cfg0, d, "bilinear")
+    cal, mask = argus.argus_calibrate(ctx, d["raw"], d["bias"], d["dark"], d["flat"], None, cfg0.t_exp)
+    n2, v2, w2 = gpu_resample_planned(ctx, cfg0, dict(cal=cal, mask=mask), "bilinear")
+    assert n == n2
+    assert np.array_equal(w, w2)
+    assert np.all(np.abs(v - v2) <= 1e-6 * np.maximum(1.0, np.abs(v)))
+
+
+def test_mask_logic_frame(argus, ctx):
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    fr = synth.inject_defects(synth.config0())
+    idx_or, _ = oracle.footprint(fr.wcs, 512, 512, fr.nside)
+    d = upload(fr)
+    for kernel, w_min in (("bilinear", 0.5), ("bilinear", 1.0), ("lanczos3", 0.5)):
+        n, v, w = gpu_resample_planned(ctx, fr, d, kernel, w_min)
+        vo, wo, fl = oracle_reference(fr, idx_or, kernel, w_min)
+        assert (wo < 1).sum() > 100 and (wo == 0).sum() > 10
+        assert_values_match(v, w, vo, wo, fl, "defects %s w_min=%g" % (kernel, w_min))
+
+
+@pytest.mark.parametrize("name", sorted(synth.special_pointings()))
+def test_special_pointings(argus, ctx, name):
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    crval, rot, nside = synth.special_pointings()[name]
+    W = H = 512
+    wcs = synth.make_wcs(crval, (255.5, 255.5), rot)
+    fr = synth.make_frame(77, W, H, 200, wcs, nside, "bilinear")
+    idx_or, dmin = oracle.footprint(wcs, W, H, nside)
+    assert dmin > 1e-9, "seeded pointing sits on a decision boundary; re-seed"
+    n, idx = argus.argus_healpix_footprint(ctx, wcs, W, H, nside)
+    assert n == len(idx_or), name
+    assert np.array_equal(idx.cpu().numpy(), idx_or), name
+    d = upload(fr)
+    n, v, w = gpu_resample_planned(ctx, fr, d, "bilinear")
+    vo, wo, fl = oracle_reference(fr, idx_or, "bilinear")
+    assert_values_match(v, w, vo, wo, fl, name)
+
+
+def test_sip_and_rectangular_odd_width(argus, ctx):
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    rng = np.random.default_rng(5)
+    W, H = 601, 333  # W % 4 != 0 -> scalar staging path
+    sip = synth.make_sip(rng, 3, 300.0)
+    sip = (3, sip[1] * 30, sip[2] * 30)
+    wcs = synth.make_wcs((211.0, 47.0), ((W - 1) / 2, (H - 1) / 2), 23.0, sip=sip)
+    fr = synth.make_frame(9, W, H, 150, wcs, 1 << 17, "bilinear")
+    idx_or, dmin = oracle.footprint(wcs, W, H, fr.nside)
+    assert dmin > 1e-9
+    n, idx = argus.argus_healpix_footprint(ctx, wcs, W, H, fr.nside)
+    assert np.array_equal(idx.cpu().numpy(), idx_or)
+    d = upload(fr)
+    for kernel in ("bilinear", "lanczos3"):
+        n, v, w = gpu_resample_planned(ctx, fr, d, kernel)
+        vo, wo, fl = oracle_reference(fr, idx_or, kernel)
+        assert_values_match(v, w, vo, wo, fl, "sip " + kernel)
+
+
+def test_small_nside_coarse_wcs(argus, ctx):
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    nside = 1 << 10
+    hp = math.degrees(math.sqrt(4 * math.pi / (12.0 * nside * nside)))
+    W = H = 256
+    wcs = synth.make_wcs((75.0, -33.0), (127.5, 127.5), 12.0, scale_deg=hp / 1.2)
+    fr = synth.make_frame(4, W, H, 50, wcs, nside, "bilinear")
+    idx_or, dmin = oracle.footprint(wcs, W, H, nside)
+    n, idx = argus.argus_healpix_footprint(ctx, wcs, W, H, nside)
+    assert np.array_equal(idx.cpu().numpy(), idx_or)
+    d = upload(fr)
+    n, v, w = gpu_resample_planned(ctx, fr, d, "bilinear")
+    vo, wo, fl = oracle_reference(fr, idx_or, "bilinear")
+    assert_values_match(v, w, vo, wo, fl, "nside 2^10")
+
+
+def test_coadd_three_frames(argus, ctx):
+    from gpu_util import upload
+    W = H = 512
+    nside = 1 << 17
+    frames = [synth.config3_frame(k, W, H) for k in range(3)]
+    fps = [oracle.footprint(f.wcs, W, H, nside)[0] for f in frames]
+    tiles = np.unique(np.concatenate([fp >> 18 for fp in fps]))[:-1]  # drop one tile: exercises "skipped"
+    ppt = 1 << 18
+    s_or = np.zeros(len(tiles) * ppt)
+    w_or = np.zeros(len(tiles) * ppt)
+    skipped_or = 0
+    for f, fp in zip(frames, fps):
+        cal, mask = oracle.calibrate_frame(f)
+        v, w, fl = oracle.resample(cal, mask, f.wcs, nside, fp, oracle.BILINEAR)
+        skipped_or += oracle.coadd_accumulate(tiles, ppt, s_or, w_or, fp, v, w)
+    dt = torch.from_numpy(tiles).cuda()
+    for fused in (True, False):
+        s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
+        ws = torch.zeros_like(s)
+        sk = torch.zeros(1, dtype=torch.int64, device="cuda")
+        for f, fp in zip(frames, fps):
+            d = upload(f)
+            if fused:
+                argus.argus_resample_coadd(ctx, f.wcs, W, H, nside, "bilinear", dt, 256, s, ws, sk, **d)
+            else:
+                n, idx = argus.argus_healpix_footprint(ctx, f.wcs, W, H, nside)
+                v = torch.empty(n, dtype=torch.float32, device="cuda")
+                w = torch.empty_like(v)
+                argus.argus_resample(ctx, f.wcs, W, H, nside, "bilinear", v, w, **d)
+                argus.argus_coadd_accumulate(ctx, dt, 256, nside, s, ws, idx, v, w, sk)
+        torch.cuda.synchronize()
+        assert int(sk.item()) == skipped_or > 0
+        sg, wg = s.cpu().numpy().astype(np.float64), ws.cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(wg - w_or) <= 1e-5 * 3)
+        assert np.all(np.abs(sg - s_or) <= 3 * 1e-3 + 1e-5 * np.abs(s_or))
+
+
+def test_capacity_and_errors(argus, ctx, cfg0):
+    from gpu_util import upload
+    d = upload(cfg0)
+    v = torch.zeros(1000, dtype=torch.float32, device="cuda")
+    w = torch.zeros_like(v)
+    argus.argus_resample(ctx, cfg0.wcs, 512, 512, cfg0.nside, "bilinear", v, w, **d)  # footprint >> 1000
+    with pytest.raises(argus.ArgusError) as e:
+        argus.argus_plan_info(ctx)
+    assert e.value.status == -6
+    with pytest.raises(argus.ArgusError):
+        argus.argus_healpix_footprint(ctx, cfg0.wcs, 512, 512, 1000)  # nside not a power of two
+    bad = synth.make_wcs((0, 0), (0, 0), 0.0, scale_deg=0.0)
+    with pytest.raises(argus.ArgusError):
+        argus.argus_healpix_footprint(ctx, bad, 512, 512, 1 << 17)
+    # frame that does not see the sky region at all is impossible (every TAN frame has a footprint), but a
+    # 1x1 frame must work: footprint of 0 or 1 pixels
+    n, idx = argus.argus_healpix_footprint(ctx, synth.make_wcs((10, 10), (0, 0), 0.0), 1, 1, 1 << 17)
+    n_or = len(oracle.footprint(synth.make_wcs((10, 10), (0, 0), 0.0), 1, 1, 1 << 17)[0])
+    assert n == n_or
