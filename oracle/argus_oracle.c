@@ -496,7 +496,8 @@ void orc_interp(const double* cal, const uint8_t* mask, int64_t W, int64_t H, do
                     if (orc_any_bad(mask, W, H, i0 + di, j0 + dj, lo, hi)) f = 1;
                 }
         }
-        if (fabs(w - w_min) < eps) f = 1;
+        /* B == 0 gives w == 1 exactly on any implementation: not ambiguous even when w_min == 1 */
+        if (B != 0.0 && fabs(w - w_min) < eps) f = 1;
         *flag = f;
     }
 }

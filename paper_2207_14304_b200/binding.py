@@ -60,6 +60,12 @@ def load_library():
     if _lib is not None:
         return _lib
     path = library_path()
+    try:  # rebuild in-tree when the sources are newer than the library (needs nvcc; never falls back to CPU)
+        from . import _build
+        _build.build()
+    except Exception:
+        if not os.path.exists(path):
+            raise
     if not os.path.exists(path):
         raise ImportError("libargus.so not built: run `python -m paper_2207_14304_b200._build` "
                           "(or __graft_entry__.build()); there is no CPU fallback")

@@ -211,6 +211,7 @@ static int make_devwcs(const argus_wcs* w, int64_t W, int64_t H, int64_t nside, 
     double s_rad = sqrt(fabs(det)) * kPi / 180.0;
     double rho = atan(1.25 * s_rad * hypot((double)W, (double)H) / 2.0);
     d->cos_rho = cos(rho);
+    d->rho = rho;
     for (int i = 0; i < 36; ++i) { d->ap[i] = w->ap[i]; d->bp[i] = w->bp[i]; }
     d->sip_order = w->sip_order;
     d->W = (int)W; d->H = (int)H;

@@ -25,6 +25,7 @@ struct DevWcs {
     double m[2][2];              // (U,V) = m (xi, eta), xi/eta in radians  (= CD^-1 * 180/pi)
     double crpix[2];
     double cos_rho;              // cos(rho_max)
+    double rho;                  // rho_max (rad)
     double ap[36], bp[36];
     int sip_order;
     int W, H;

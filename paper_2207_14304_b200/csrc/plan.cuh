@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(256) plan_scan_kernel(DevWcs w, CoarseList cl,
         double v[3], x, y;
         hp_vec(face, ixc, iyc, w.nside, ring_zone(jr, ns), v);
         double cosc = vec_to_xy(w, v, x, y);
-        if (cosc > 0.05 && cosc >= w.cos_rho - w.tile_ang) {
+        if (cosc > 0.05 && acos(fmin(cosc, 1.0)) <= w.rho + w.tile_ang) {
             keep = (x >= -0.5 - rad_px) && (x < w.W - 0.5 + rad_px) && (y >= -0.5 - rad_px) && (y < w.H - 0.5 + rad_px);
         }
         pb.slot_flag[slot] = (unsigned char)keep;
@@ -187,7 +187,10 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
             bool finite_ok = (xmin > -1e8) && (xmax < 1e8) && (ymin > -1e8) && (ymax < 1e8) && (cmin > 0.05);
             bool fit_ok = finite_ok && (res <= PLAN_FIT_TOL);   // NaN compares false
             double mg = PLAN_NODE_MARGIN;
-            bool cone_in = cmin - w.tile_ang >= w.cos_rho, cone_out = cmax + w.tile_ang < w.cos_rho;
+            // angular distance from CRVAL is convex over the (near-planar) tile: its maximum sits on a corner
+            // node; only the drop decision needs the full conservative tile radius
+            bool cone_in = acos(fmin(cmin, 1.0)) + 0.1 * w.tile_ang <= w.rho;
+            bool cone_out = acos(fmin(cmax, 1.0)) - w.tile_ang > w.rho;
             if (fit_ok && !cone_out) {
                 bool all_out = (xmax + mg < -0.5) || (xmin - mg >= w.W - 0.5) || (ymax + mg < -0.5) || (ymin - mg >= w.H - 0.5);
                 bool all_in = (xmin - mg >= -0.5) && (xmax + mg < w.W - 0.5) && (ymin - mg >= -0.5) && (ymax + mg < w.H - 0.5);
