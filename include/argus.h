@@ -55,8 +55,11 @@ enum { ARGUS_BILINEAR = 0, ARGUS_LANCZOS3 = 1 };
 
 /* Options for argus_ctx_set_option. */
 enum {
-    ARGUS_OPT_PLAN_CACHE = 1 /* 1 (default): a plan built for (wcs, W, H, nside) is reused by the next
-                                call with identical arguments; 0: every call re-plans on the device */
+    ARGUS_OPT_PLAN_CACHE = 1, /* 1 (default): a plan built for (wcs, W, H, nside) is reused by the next
+                                 call with identical arguments; 0: every call re-plans on the device */
+    ARGUS_OPT_PROFILE = 2     /* 1: argus_resample / argus_resample_coadd (idx == NULL) record CUDA events on
+                                 the caller's stream around the plan kernels and around the fused kernel
+                                 (ring of 256 calls); read them back with argus_profile_read.  Default 0. */
 };
 
 typedef struct argus_ctx argus_ctx;
@@ -171,6 +174,11 @@ int argus_resample_coadd(argus_ctx* ctx, const argus_frame* frame, const argus_w
 /* Synchronises the stream and reports the statistics of the cached plan.  Returns ARGUS_ERR_CAPACITY if
  * an asynchronous call since the last check overflowed its output capacity or the context's max_tiles. */
 int argus_plan_info(argus_ctx* ctx, argus_plan_stats* out, void* stream);
+
+/* Synchronises the stream and returns, for the calls recorded since ARGUS_OPT_PROFILE was last set to 1,
+ * the summed device time (ms) of the plan kernels and of the fused resample kernel, and the number of
+ * calls summed (at most the last 256).  HOST pointers.  Resets the ring. */
+int argus_profile_read(argus_ctx* ctx, double* plan_ms, double* kernel_ms, int64_t* n_calls, void* stream);
 
 #ifdef __cplusplus
 }

@@ -12,12 +12,13 @@ import torch
 
 ARGUS_BILINEAR, ARGUS_LANCZOS3 = 0, 1
 ARGUS_OPT_PLAN_CACHE = 1
+ARGUS_OPT_PROFILE = 2
 _KERNELS = {"bilinear": ARGUS_BILINEAR, "lanczos3": ARGUS_LANCZOS3, 0: 0, 1: 1}
 
 EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
-    "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info",
+    "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
 ]
 
 
@@ -85,6 +86,7 @@ def load_library():
     L.argus_resample_coadd.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32,
                                        C.POINTER(_Coadd), vp, vp, vp, vp]
     L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
+    L.argus_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64), vp]
     _lib = L
     return L
 
@@ -175,6 +177,19 @@ class Context:
         rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_PLAN_CACHE, 1 if on else 0)
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")
+
+    def set_profile(self, on: bool):
+        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_PROFILE, 1 if on else 0)
+        if rc:
+            raise ArgusError(rc, "argus_ctx_set_option")
+
+    def profile_read(self, stream=None):
+        """Returns (plan_ms_total, kernel_ms_total, n_calls) of the calls recorded since profiling was enabled."""
+        p, k, n = C.c_double(), C.c_double(), C.c_int64()
+        rc = load_library().argus_profile_read(self._h, C.byref(p), C.byref(k), C.byref(n), _stream(stream))
+        if rc:
+            raise ArgusError(rc, "argus_profile_read")
+        return p.value, k.value, int(n.value)
 
     def last_cuda_error(self) -> int:
         return int(load_library().argus_last_cuda_error(self._h))

@@ -26,6 +26,10 @@ struct argus_ctx {
     PlanBuffers pb;
     PlanStats* h_stats;   // pinned
     void* d_block;        // the single device allocation behind pb
+    bool profile;
+    int prof_n;           // calls recorded since the last read
+    cudaEvent_t ev[256][3];
+    bool ev_plan[256];    // the call re-planned (ev[i][0] -> ev[i][1] is meaningful)
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -158,6 +162,8 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
         delete c;
         return ARGUS_ERR_CUDA;
     }
+    for (int i = 0; i < 256; ++i)
+        for (int j = 0; j < 3; ++j) cudaEventCreate(&c->ev[i][j]);
     *out = c;
     return ARGUS_OK;
 }
@@ -165,6 +171,8 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
 extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (!c) return ARGUS_ERR_NULL;
     cudaSetDevice(c->device);
+    for (int i = 0; i < 256; ++i)
+        for (int j = 0; j < 3; ++j) cudaEventDestroy(c->ev[i][j]);
     cudaFree(c->d_block);
     cudaFreeHost(c->h_stats);
     delete c;
@@ -178,7 +186,29 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
         if (!c->plan_cache) c->plan_valid = false;
         return ARGUS_OK;
     }
+    if (option == ARGUS_OPT_PROFILE) {
+        c->profile = value != 0;
+        c->prof_n = 0;
+        return ARGUS_OK;
+    }
     return ARGUS_ERR_SHAPE;
+}
+
+extern "C" int argus_profile_read(argus_ctx* c, double* plan_ms, double* kernel_ms, int64_t* n_calls, void* stream) {
+    if (!c || !plan_ms || !kernel_ms || !n_calls) return ARGUS_ERR_NULL;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
+    int n = c->prof_n < 256 ? c->prof_n : 256;
+    double p = 0, k = 0;
+    for (int i = 0; i < n; ++i) {
+        float a = 0.f, b = 0.f;
+        if (c->ev_plan[i]) CUDA_TRY(c, cudaEventElapsedTime(&a, c->ev[i][0], c->ev[i][1]));
+        CUDA_TRY(c, cudaEventElapsedTime(&b, c->ev[i][1], c->ev[i][2]));
+        p += a; k += b;
+    }
+    *plan_ms = p; *kernel_ms = k; *n_calls = n;
+    c->prof_n = 0;
+    return ARGUS_OK;
 }
 
 extern "C" int argus_last_cuda_error(const argus_ctx* c) { return c ? c->last_cuda : 0; }
@@ -423,11 +453,16 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
         CUDA_TRY(c, cudaGetLastError());
         return ARGUS_OK;
     }
+    int slot = c->prof_n & 255;
+    bool replanned = !same_key(c, wcs, W, H, nside);
+    if (c->profile) cudaEventRecord(c->ev[slot][0], st);
     rc = build_plan(c, wcs, W, H, nside, (long long)n, st);
     if (rc) return rc;
+    if (c->profile) cudaEventRecord(c->ev[slot][1], st);
     CoaddArgs ca;
     memset(&ca, 0, sizeof(ca));
     launch_tiles<false>(c, kernel, fused, f, w_min, value_out, weight_out, (long long)n, ca, st);
+    if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
 }
@@ -480,9 +515,14 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
+    int slot = c->prof_n & 255;
+    bool replanned = !same_key(c, wcs, W, H, nside);
+    if (c->profile) cudaEventRecord(c->ev[slot][0], st);
     rc = build_plan(c, wcs, W, H, nside, -1, st);
     if (rc) return rc;
+    if (c->profile) cudaEventRecord(c->ev[slot][1], st);
     launch_tiles<true>(c, kernel, fused, f, w_min, nullptr, nullptr, 0, ca, st);
+    if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
 }

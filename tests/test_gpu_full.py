@@ -1,0 +1,106 @@
+"""GPU parity at BASELINE.json's full sizes (-m gpu), in the launch configuration bench.py times:
+configs[1] (all outputs), configs[2] (three frames: lowest dec, belt/cap transition, highest dec; Lanczos-3 +
+SIP), configs[3] (coadd of the first three frames) and configs[4] (one frame, nside 2^18, sampled outputs)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+import synth  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def argus():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2207_14304_b200 as a
+    a.load_library()
+    return a
+
+
+@pytest.fixture(scope="module")
+def ctx(argus):
+    c = argus.Context(0)
+    c.set_plan_cache(False)
+    yield c
+    c.close()
+
+
+def _full_frame_parity(argus, ctx, fr, what, sample=None):
+    from gpu_util import assert_values_match, upload
+    H, W = fr.shape
+    idx_or, dmin = oracle.footprint(fr.wcs, W, H, fr.nside)
+    assert dmin > 1e-9, what + ": seeded frame sits on a decision boundary"
+    n, idx = argus.argus_healpix_footprint(ctx, fr.wcs, W, H, fr.nside)
+    assert n == len(idx_or), what
+    assert torch.equal(idx.cpu(), torch.from_numpy(idx_or)), what + ": footprint list differs"
+    del idx
+    d = upload(fr)
+    v = torch.empty(n, dtype=torch.float32, device="cuda")
+    w = torch.empty_like(v)
+    argus.argus_resample(ctx, fr.wcs, W, H, fr.nside, fr.kernel, v, w, **d)
+    torch.cuda.synchronize()
+    info = argus.argus_plan_info(ctx)
+    vg, wg = v.cpu().numpy(), w.cpu().numpy()
+    cal, mask = oracle.calibrate_frame(fr)
+    if sample is not None and sample < n:
+        rng = np.random.default_rng(0)
+        sel = np.sort(rng.choice(n, sample, replace=False))
+        idx_or, vg, wg = idx_or[sel], vg[sel], wg[sel]
+    vo, wo, fl = oracle.resample(cal, mask, fr.wcs, fr.nside, idx_or, oracle.KERNELS[fr.kernel])
+    worst = assert_values_match(vg, wg, vo, wo, fl, what)
+    print("%s: n_fp=%d worst=%.3f x tol plan=%s" % (what, n, worst, info))
+    return info
+
+
+def test_config1_full_frame(argus, ctx):
+    info = _full_frame_parity(argus, ctx, synth.config1(), "config1")
+    assert info["n_footprint"] == 44887802          # SURVEY.md 8(a), confirmed by the oracle
+    assert info["n_inside"] > 0.9 * info["n_tiles"] * 0.9
+
+
+@pytest.mark.parametrize("k", [0, 25, 37])
+def test_config2_frames(argus, ctx, k):
+    info = _full_frame_parity(argus, ctx, synth.config2_frame(k), "config2[%d]" % k)
+    if k == 25:
+        assert info["n_exact"] > 0  # the belt/cap ring crosses this frame
+
+
+def test_config4_one_frame_nside_2p18(argus, ctx):
+    _full_frame_parity(argus, ctx, synth.config4_frame(4), "config4[4]", sample=20_000_000)
+
+
+def test_config3_coadd_full(argus, ctx):
+    from gpu_util import upload
+    W, H, nside = synth.frames.FULL_W, synth.frames.FULL_H, 1 << 17
+    base = synth.config3_frame(0)
+    masters = (base.bias, base.dark, base.flat)
+    frames = [base] + [synth.config3_frame(k, masters=masters) for k in (1, 2)]
+    fps = [oracle.footprint(f.wcs, W, H, nside)[0] for f in frames]
+    tiles = np.unique(np.concatenate([fp >> 18 for fp in fps]))
+    ppt = 1 << 18
+    s_or = np.zeros(len(tiles) * ppt)
+    w_or = np.zeros(len(tiles) * ppt)
+    for f, fp in zip(frames, fps):
+        cal, mask = oracle.calibrate_frame(f)
+        v, w, fl = oracle.resample(cal, mask, f.wcs, nside, fp, oracle.BILINEAR)
+        assert oracle.coadd_accumulate(tiles, ppt, s_or, w_or, fp, v, w) == 0
+    dt = torch.from_numpy(tiles).cuda()
+    s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
+    ws = torch.zeros_like(s)
+    sk = torch.zeros(1, dtype=torch.int64, device="cuda")
+    dm = [torch.from_numpy(m).cuda() for m in masters]
+    for f in frames:
+        d = dict(raw=torch.from_numpy(f.raw).cuda(), bias=dm[0], dark=dm[1], flat=dm[2], bpm=None, t_exp=f.t_exp,
+                 sat_adu=f.sat_adu, flat_min=f.flat_min)
+        argus.argus_resample_coadd(ctx, f.wcs, W, H, nside, "bilinear", dt, 256, s, ws, sk, **d)
+    torch.cuda.synchronize()
+    assert int(sk.item()) == 0
+    sg, wg = s.cpu().numpy().astype(np.float64), ws.cpu().numpy().astype(np.float64)
+    assert np.abs(wg - w_or).max() <= 3e-5
+    # dithered frames: pixels within 1e-4 px of an integer next to a masked pixel are margin-ambiguous; bound them
+    bad = np.abs(sg - s_or) > 3e-3 + 1e-5 * np.abs(s_or)
+    assert bad.mean() <= 1e-4, bad.mean()
