@@ -119,7 +119,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
@@ -132,6 +132,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     o_mask = o;  o = align_up(o + sizeof(unsigned) * 32 * (size_t)pb.max_hard, 256);
     o_stats = o; o = align_up(o + sizeof(PlanStats), 256);
     o_pinv = o;  o = align_up(o + sizeof(double) * 250, 256);
+    o_dc = o;    o = align_up(o + sizeof(double) * 20 * (size_t)pb.max_tiles, 256);
     e = cudaMalloc(&c->d_block, o);
     if (e == cudaSuccess) e = cudaMemset(c->d_block, 0, o);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
@@ -153,6 +154,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.masks = (unsigned*)(b + o_mask);
     pb.stats = (PlanStats*)(b + o_stats);
     pb.pinv = (double*)(b + o_pinv);
+    pb.dcoef = (double*)(b + o_dc);
     double pinv[250];
     lsq_pinv(pinv);
     e = cudaMemcpy(pb.pinv, pinv, sizeof(pinv), cudaMemcpyHostToDevice);

@@ -189,4 +189,22 @@ __device__ inline void poly_axis_eval(const PolyAxis& p, int s, int t, int& cell
     frac = g - fl;
     cell = p.base + (hi >> 12) + (int)fl;
 }
+
+// Same coordinates with the remainder polynomial evaluated in FP64 from the unsplit double coefficients
+// dc[10] (constant term includes the integer base): used by the Lanczos-3 path (error ~1e-10 px).
+__device__ inline void poly_axis_eval_f64(const double* __restrict__ dc, const PolyAxis& p, int s, int t, int& cell,
+                                          double& frac) {
+    double S = (double)s * 0.03125, T = (double)t * 0.03125;
+    // remove the fixed-point linear part and the integer base exactly, as in the FP32 split
+    double c0 = dc[0] - (double)p.base, c1 = dc[1] - (double)p.a * (32.0 / 4096.0), c2 = dc[2] - (double)p.b * (32.0 / 4096.0);
+    double A = fma(S, fma(S, fma(S, dc[6], dc[3]), c1), c0);
+    double B = fma(S, fma(S, dc[7], dc[4]), c2);
+    double C = fma(S, dc[8], dc[5]);
+    double lo = fma(T, fma(T, fma(T, dc[9], C), B), A);
+    int hi = p.a * s + p.b * t;
+    double g = fma((double)(hi & 4095), 0.000244140625, lo);
+    double fl = floor(g);
+    frac = g - fl;
+    cell = p.base + (hi >> 12) + (int)fl;
+}
 #endif  // __CUDACC__

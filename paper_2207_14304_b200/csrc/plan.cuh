@@ -31,6 +31,7 @@ struct PlanBuffers {
     unsigned* masks;            // [max_hard][32]
     PlanStats* stats;           // device
     double* pinv;               // [10][25] least-squares pseudo-inverse of the node design matrix
+    double* dcoef;              // [max_tiles][20] unsplit FP64 polynomial coefficients (x then y)
     int max_slots, max_tiles, max_hard;
 };
 
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
             }
             if (lane == 0) acc += xc;
             if (lane == 10) acc += yc;
-            if (lane < 20) s_coef[wid][lane] = acc;
+            if (lane < 20) { s_coef[wid][lane] = acc; pb.dcoef[(size_t)t * 20 + lane] = acc; }
             __syncwarp();
             double m[10];
             cubic_basis(S, T, m);

@@ -47,14 +47,26 @@ __device__ __forceinline__ float calib_px(float r, float b, float d, float fl, b
     return good ? __fdividef(t, fl) : nanf_();
 }
 
-template <bool FUSED>
+// Lanczos-3 variant: the negative lobes cancel bright taps against each other, so the calibrated value is
+// formed in FP64 and rounded once to float32 (0.5 ulp) -- DESIGN.md "Lanczos precision".
+__device__ __forceinline__ float calib_px_precise(float r, float b, float d, float fl, bool bad, float t_exp, float flat_min) {
+    double t = (double)r - (double)b - (double)d * (double)t_exp;
+    bool good = !bad && (fl >= flat_min) && (fl < INFINITY) && (fabs(t) < (double)INFINITY);
+    return good ? (float)(t / (double)fl) : nanf_();
+}
+template <bool PRECISE>
+__device__ __forceinline__ float calib_sel(float r, float b, float d, float fl, bool bad, float t_exp, float flat_min) {
+    return PRECISE ? calib_px_precise(r, b, d, fl, bad, t_exp, flat_min) : calib_px(r, b, d, fl, bad, t_exp, flat_min);
+}
+
+template <bool FUSED, bool PRECISE = false>
 __device__ __forceinline__ float load_px(const FrameArgs& f, int W, int H, int gx, int gy) {
     if (gx < 0 || gx >= W || gy < 0 || gy >= H) return nanf_();
     size_t o = (size_t)gy * W + gx;
     if (FUSED) {
         int r = f.raw[o];
         bool bad = (r >= f.sat_adu) || (f.bpm && f.bpm[o] != 0);
-        return calib_px((float)r, f.bias[o], f.dark[o], f.flat[o], bad, f.t_exp, f.flat_min);
+        return calib_sel<PRECISE>((float)r, f.bias[o], f.dark[o], f.flat[o], bad, f.t_exp, f.flat_min);
     } else {
         return f.mask[o] ? f.cal[o] : nanf_();
     }
@@ -62,7 +74,7 @@ __device__ __forceinline__ float load_px(const FrameArgs& f, int W, int H, int g
 
 // Stage the box [gx0, gx0+bw) x [gy0, gy0+bh) (gx0, bw multiples of 4) into s_box (pitch bw).
 // Returns non-zero for threads that stored a masked pixel.
-template <bool FUSED>
+template <bool FUSED, bool PRECISE>
 __device__ __forceinline__ int stage_box(const FrameArgs& f, int W, int H, int gx0, int gy0, int bw, int bh,
                                          float* s_box, int tid) {
     int bad_any = 0;
@@ -83,10 +95,10 @@ __device__ __forceinline__ int stage_box(const FrameArgs& f, int W, int H, int g
                 int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
                 unsigned bp = 0;
                 if (f.bpm) bp = __ldg(reinterpret_cast<const unsigned*>(f.bpm + o));
-                o4.x = calib_px((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
-                o4.y = calib_px((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
-                o4.z = calib_px((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
-                o4.w = calib_px((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+                o4.x = calib_sel<PRECISE>((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
+                o4.y = calib_sel<PRECISE>((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
+                o4.z = calib_sel<PRECISE>((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
+                o4.w = calib_sel<PRECISE>((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
             } else {
                 float4 c = __ldg(reinterpret_cast<const float4*>(f.cal + o));
                 unsigned mk = __ldg(reinterpret_cast<const unsigned*>(f.mask + o));
@@ -96,10 +108,10 @@ __device__ __forceinline__ int stage_box(const FrameArgs& f, int W, int H, int g
                 o4.w = (mk & 0xff000000u) ? c.w : nanf_();
             }
         } else {
-            o4.x = load_px<FUSED>(f, W, H, gx, gy);
-            o4.y = load_px<FUSED>(f, W, H, gx + 1, gy);
-            o4.z = load_px<FUSED>(f, W, H, gx + 2, gy);
-            o4.w = load_px<FUSED>(f, W, H, gx + 3, gy);
+            o4.x = load_px<FUSED, PRECISE>(f, W, H, gx, gy);
+            o4.y = load_px<FUSED, PRECISE>(f, W, H, gx + 1, gy);
+            o4.z = load_px<FUSED, PRECISE>(f, W, H, gx + 2, gy);
+            o4.w = load_px<FUSED, PRECISE>(f, W, H, gx + 3, gy);
         }
         bad_any |= (o4.x != o4.x) | (o4.y != o4.y) | (o4.z != o4.z) | (o4.w != o4.w);
         *reinterpret_cast<float4*>(s_box + row * bw + 4 * c4) = o4;
@@ -113,11 +125,11 @@ struct SmemTaps {
     int gx0, gy0, pitch;
     __device__ __forceinline__ float operator()(int i, int j) const { return s[(j - gy0) * pitch + (i - gx0)]; }
 };
-template <bool FUSED>
+template <bool FUSED, bool PRECISE = false>
 struct GlobalTaps {
     const FrameArgs* f;
     int W, H;
-    __device__ __forceinline__ float operator()(int i, int j) const { return load_px<FUSED>(*f, W, H, i, j); }
+    __device__ __forceinline__ float operator()(int i, int j) const { return load_px<FUSED, PRECISE>(*f, W, H, i, j); }
 };
 
 // A5 masked, normalised bilinear (general path).
@@ -140,8 +152,7 @@ __device__ __forceinline__ void interp_bilinear_masked(const Taps& tp, int i, in
 
 // Lanczos-3 weights of the six taps i0-2 .. i0+3 for fraction f in [0,1): L(t) = sinc(t) sinc(t/3).
 // Evaluated in FP64 (v1: correctness first).
-__device__ __forceinline__ void lanczos3_weights(float f, double k[6]) {
-    double fd = (double)f;
+__device__ __forceinline__ void lanczos3_weights(double fd, double k[6]) {
     double s1 = sinpi(fd);
 #pragma unroll
     for (int q = 0; q < 6; ++q) {
@@ -154,7 +165,7 @@ __device__ __forceinline__ void lanczos3_weights(float f, double k[6]) {
 }
 
 template <class Taps>
-__device__ __forceinline__ void interp_lanczos3_masked(const Taps& tp, int i, int j, float fx, float fy, float w_min,
+__device__ __forceinline__ void interp_lanczos3_masked(const Taps& tp, int i, int j, double fx, double fy, float w_min,
                                                        float& val, float& wgt) {
     double kx[6], ky[6];
     lanczos3_weights(fx, kx);
@@ -208,7 +219,7 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
         const bool fits = (bw > 0 && bh > 0 && bw * bh <= RS_BOX_FLOATS);
         __syncthreads();                            // previous tile's gathers are done with s_box / s_mask
         int bad = 1;
-        if (fits) bad = stage_box<FUSED>(f, w.W, w.H, gx0, gy0, bw, bh, s_box, tid);
+        if (fits) bad = stage_box<FUSED, KERNEL == 1>(f, w.W, w.H, gx0, gy0, bw, bh, s_box, tid);
         if (cls != TC_INSIDE && wid == 0) {
             unsigned mk = pb.masks[(size_t)rp->mask_slot * 32 + lane];
             int c = __popc(mk), inc = c;
@@ -242,7 +253,8 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
             poly_axis_load(*rp, 1, py);
         }
         SmemTaps st{s_box, gx0, gy0, bw};
-        GlobalTaps<FUSED> gt{&f, w.W, w.H};
+        GlobalTaps<FUSED, KERNEL == 1> gt{&f, w.W, w.H};
+        const double* dc = pb.dcoef + (size_t)t * 20;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const int m = tid + 256 * q;
@@ -255,12 +267,18 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
             }
             int ci, cj;
             float fx, fy;
+            double dfx = 0.0, dfy = 0.0;   // Lanczos-3 carries the fractions in FP64
             if (cls == TC_EXACT) {
                 double x, y;
                 pixel_to_xy(w, face, ix0 + u, iy0 + v, x, y);
                 double flx = floor(x), fly = floor(y);
                 ci = (int)flx; cj = (int)fly;
-                fx = (float)(x - flx); fy = (float)(y - fly);
+                dfx = x - flx; dfy = y - fly;
+                fx = (float)dfx; fy = (float)dfy;
+            } else if (KERNEL == 1) {
+                poly_axis_eval_f64(dc, px, 2 * u - 31, 2 * v - 31, ci, dfx);
+                poly_axis_eval_f64(dc + 10, py, 2 * u - 31, 2 * v - 31, cj, dfy);
+                fx = (float)dfx; fy = (float)dfy;
             } else {
                 poly_axis_eval(px, 2 * u - 31, 2 * v - 31, ci, fx);
                 poly_axis_eval(py, 2 * u - 31, 2 * v - 31, cj, fy);
@@ -281,11 +299,11 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
                         interp_bilinear_masked(st, ci, cj, fx, fy, w_min, val, wgt);
                     }
                 } else {
-                    interp_lanczos3_masked(st, ci, cj, fx, fy, w_min, val, wgt);
+                    interp_lanczos3_masked(st, ci, cj, dfx, dfy, w_min, val, wgt);
                 }
             } else {
                 if (KERNEL == 0) interp_bilinear_masked(gt, ci, cj, fx, fy, w_min, val, wgt);
-                else interp_lanczos3_masked(gt, ci, cj, fx, fy, w_min, val, wgt);
+                else interp_lanczos3_masked(gt, ci, cj, dfx, dfy, w_min, val, wgt);
             }
             if (COADD) {
                 long long sb = s_slot;
@@ -328,9 +346,9 @@ __global__ void __launch_bounds__(256) resample_list_kernel(DevWcs w, FrameArgs 
         double cosc = pixel_to_xy(w, face, ix, iy, x, y);
         if (cosc > 0.0 && fabs(x) < 1e9 && fabs(y) < 1e9) {
             double flx = floor(x), fly = floor(y);
-            GlobalTaps<FUSED> gt{&f, w.W, w.H};
+            GlobalTaps<FUSED, KERNEL == 1> gt{&f, w.W, w.H};
             if (KERNEL == 0) interp_bilinear_masked(gt, (int)flx, (int)fly, (float)(x - flx), (float)(y - fly), w_min, val, wgt);
-            else interp_lanczos3_masked(gt, (int)flx, (int)fly, (float)(x - flx), (float)(y - fly), w_min, val, wgt);
+            else interp_lanczos3_masked(gt, (int)flx, (int)fly, x - flx, y - fly, w_min, val, wgt);
         }
     }
     value_out[i] = val;
