@@ -119,13 +119,16 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
     o_rec = o;   o = align_up(o + sizeof(TileRec) * pb.max_tiles, 256);
     o_cnt = o;   o = align_up(o + sizeof(int) * pb.max_tiles, 256);
-    o_off = o;   o = align_up(o + sizeof(long long) * (pb.max_tiles + 1), 256);
+    o_off = o;   o = align_up(o + sizeof(int) * (pb.max_tiles + 1), 256);
+    o_cls = o;   o = align_up(o + (size_t)pb.max_tiles, 256);
+    o_bs = o;    o = align_up(o + sizeof(int) * (pb.max_tiles / 1024 + 2), 256);
+    o_bb = o;    o = align_up(o + sizeof(long long) * (pb.max_tiles / 1024 + 2), 256);
     o_nt = o;    o = align_up(o + sizeof(int), 256);
     o_hc = o;    o = align_up(o + sizeof(int), 256);
     o_hl = o;    o = align_up(o + sizeof(int) * pb.max_hard, 256);
@@ -147,7 +150,10 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.tile_id = (long long*)(b + o_tid);
     pb.rec = (TileRec*)(b + o_rec);
     pb.tile_count = (int*)(b + o_cnt);
-    pb.tile_offset = (long long*)(b + o_off);
+    pb.tile_offset = (int*)(b + o_off);
+    pb.tile_cls = (unsigned char*)(b + o_cls);
+    pb.block_sum = (int*)(b + o_bs);
+    pb.block_base = (long long*)(b + o_bb);
     pb.n_tiles = (int*)(b + o_nt);
     pb.hard_count = (int*)(b + o_hc);
     pb.hard_list = (int*)(b + o_hl);
@@ -320,7 +326,11 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     plan_compact_kernel<<<nblk, 256, 0, st>>>(cl, c->pb);
     plan_fit_kernel<<<c->sm_count * 4, 32 * FIT_WARPS, 0, st>>>(dw, c->pb);
     plan_members_kernel<<<c->sm_count * 4, 256, 0, st>>>(dw, c->pb);
-    plan_offsets_kernel<<<1, 1024, 0, st>>>(c->pb, out_cap);
+    {
+        long long bound = n_slots < c->pb.max_tiles ? n_slots : c->pb.max_tiles;
+        plan_offsets_local_kernel<<<(int)((bound + 1023) / 1024), 1024, 0, st>>>(c->pb);
+        plan_offsets_final_kernel<<<1, 1024, 0, st>>>(c->pb, out_cap);
+    }
     CUDA_TRY(c, cudaGetLastError());
     c->dw = dw;
     c->key_wcs = *w;
@@ -331,21 +341,22 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
 
 static bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 
-static int make_frameargs(const argus_frame* fr, int64_t W, FrameArgs* f, bool* fused) {
+static int make_frameargs(const argus_frame* fr, int64_t W, int64_t H, FrameArgs* f, bool* fused) {
     memset(f, 0, sizeof(*f));
     if (fr->raw) {
         if (!fr->bias || !fr->dark || !fr->flat) return ARGUS_ERR_NULL;
+        if (!(fr->flat_min > 0.0f) || !(fr->flat_min < INFINITY) || fr->sat_adu < 0) return ARGUS_ERR_SHAPE;
         if (!aligned(fr->raw, 2) || !aligned(fr->bias, 4) || !aligned(fr->dark, 4) || !aligned(fr->flat, 4)) return ARGUS_ERR_ALIGN;
         f->raw = fr->raw; f->bias = fr->bias; f->dark = fr->dark; f->flat = fr->flat; f->bpm = fr->bpm;
         f->t_exp = fr->t_exp; f->flat_min = fr->flat_min; f->sat_adu = fr->sat_adu;
-        f->vec_ok = (W % 4 == 0) && aligned(fr->raw, 8) && aligned(fr->bias, 16) && aligned(fr->dark, 16) &&
+        f->vec_ok = (W % 4 == 0) && (W * H < (1ll << 31)) && aligned(fr->raw, 8) && aligned(fr->bias, 16) && aligned(fr->dark, 16) &&
                     aligned(fr->flat, 16) && (!fr->bpm || aligned(fr->bpm, 4));
         *fused = true;
     } else {
         if (!fr->cal || !fr->mask) return ARGUS_ERR_NULL;
         if (!aligned(fr->cal, 4)) return ARGUS_ERR_ALIGN;
         f->cal = fr->cal; f->mask = fr->mask;
-        f->vec_ok = (W % 4 == 0) && aligned(fr->cal, 16) && aligned(fr->mask, 4);
+        f->vec_ok = (W % 4 == 0) && (W * H < (1ll << 31)) && aligned(fr->cal, 16) && aligned(fr->mask, 4);
         *fused = false;
     }
     return ARGUS_OK;
@@ -363,7 +374,7 @@ extern "C" int argus_calibrate(argus_ctx* c, const uint16_t* raw, const float* b
     fr.t_exp = t_exp; fr.sat_adu = sat_adu; fr.flat_min = flat_min;
     FrameArgs f;
     bool fused;
-    int rc = make_frameargs(&fr, W, &f, &fused);
+    int rc = make_frameargs(&fr, W, H, &f, &fused);
     if (rc) return rc;
     if (!aligned(cal_out, 4)) return ARGUS_ERR_ALIGN;
     long long n = W * H;
@@ -436,7 +447,7 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     if (n > ((size_t)1 << 40)) return ARGUS_ERR_SHAPE;
     FrameArgs f;
     bool fused;
-    int rc = make_frameargs(frame, W, &f, &fused);
+    int rc = make_frameargs(frame, W, H, &f, &fused);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
@@ -513,7 +524,7 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     if (rc) return rc;
     FrameArgs f;
     bool fused;
-    rc = make_frameargs(frame, W, &f, &fused);
+    rc = make_frameargs(frame, W, H, &f, &fused);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));

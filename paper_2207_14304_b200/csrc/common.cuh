@@ -39,7 +39,7 @@ struct DevWcs {
 // total-degree-3 polynomial, monomial order 1, S, T, S^2, ST, T^2, S^3, S^2 T, S T^2, T^3.
 struct __align__(16) TileRec {
     long long tile;      // nested tile id = pixel index >> 10
-    long long offset;    // exclusive prefix of count over tiles (output position of the tile's first pixel)
+    long long reserved;
     int cls;
     int count;
     int mask_slot;       // row of the membership-mask array (TC_BORDER / TC_EXACT), else -1

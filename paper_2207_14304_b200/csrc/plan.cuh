@@ -24,7 +24,10 @@ struct PlanBuffers {
     long long* tile_id;         // [max_tiles]
     TileRec* rec;               // [max_tiles]
     int* tile_count;            // [max_tiles]
-    long long* tile_offset;     // [max_tiles + 1]
+    int* tile_offset;           // [max_tiles] exclusive prefix of tile_count inside its block of 1024 tiles
+    unsigned char* tile_cls;    // [max_tiles] compact copy of TileRec.cls
+    int* block_sum;             // [max_tiles/1024 + 1]
+    long long* block_base;      // [max_tiles/1024 + 1] exclusive prefix of block_sum
     int* n_tiles;               // device scalar
     int* hard_count;            // device scalar
     int* hard_list;             // [max_hard] tile positions
@@ -60,7 +63,9 @@ __global__ void __launch_bounds__(256) plan_scan_kernel(DevWcs w, CoarseList cl,
     if (threadIdx.x == 0) pb.block_count[blockIdx.x] = cnt;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         *pb.hard_count = 0;
-        pb.stats->overflow = 0;
+        PlanStats* st = pb.stats;
+        st->overflow = 0;
+        st->n_inside = st->n_border = st->n_exact = st->n_empty = 0;
     }
 }
 
@@ -151,7 +156,7 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
         long long jr_max = (long long)face_ring_offset(face) * ns - ix0 - iy0 - 1, jr_min = jr_max - 62;
         int z0 = ring_zone(jr_min, ns), z1 = ring_zone(jr_max, ns);
         TileRec r;
-        r.tile = tile; r.offset = 0; r.count = 0; r.mask_slot = -1;
+        r.tile = tile; r.reserved = 0; r.count = 0; r.mask_slot = -1;
         r.zone = (z0 == z1) ? z0 : -1;
         r.bx0 = r.bx1 = r.by0 = r.by1 = 0; r.X0 = r.Y0 = 0; r.ax = r.bx = r.ay = r.by = 0;
         r.pad[0] = r.pad[1] = 0;
@@ -234,6 +239,7 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
             r.cls = cls;
             pb.rec[t] = r;
             pb.tile_count[t] = r.count;
+            pb.tile_cls[t] = (unsigned char)cls;
         }
         __syncwarp();
     }
@@ -322,6 +328,7 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
             pb.tile_count[t] = c;
             if (c == 0) {
                 wr->cls = TC_EMPTY;
+                pb.tile_cls[t] = TC_EMPTY;
             } else {
                 wr->bx0 = s_ext[0]; wr->bx1 = s_ext[1]; wr->by0 = s_ext[2]; wr->by1 = s_ext[3];
             }
@@ -331,56 +338,91 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
 }
 
 // ------------------------------------------------------------------------------------------ offsets
-// Single block: exclusive scan of the per-tile counts (<= ~1M tiles) + statistics.
-__global__ void __launch_bounds__(1024) plan_offsets_kernel(PlanBuffers pb, long long out_capacity) {
-    __shared__ long long s_warp[32];
-    __shared__ int s_cls[4];
+// Exclusive scan of the per-tile counts in two small launches: block-local scan (1024 tiles per block,
+// coalesced reads of the compact count / class arrays) + one block that scans the block sums.
+// Output position of tile t = block_base[t >> 10] + tile_offset[t].
+__global__ void __launch_bounds__(1024) plan_offsets_local_kernel(PlanBuffers pb) {
+    __shared__ int s_warp[32];
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int n = *pb.n_tiles;
-    int per = (n + 1023) / 1024;
-    int b = tid * per, e = min(n, b + per);
-    if (tid < 4) s_cls[tid] = 0;
-    __syncthreads();
-    long long sum = 0;
-    int c_in = 0, c_bo = 0, c_ex = 0, c_em = 0;
-    for (int i = b; i < e; ++i) {
-        sum += pb.tile_count[i];
-        int cls = pb.rec[i].cls;
-        c_in += cls == TC_INSIDE; c_bo += cls == TC_BORDER; c_ex += cls == TC_EXACT; c_em += cls == TC_EMPTY;
-    }
-    long long inc = sum;
+    int i = blockIdx.x * 1024 + tid;
+    if (blockIdx.x * 1024 >= n) return;
+    int c = (i < n) ? pb.tile_count[i] : 0;
+    int cls = (i < n) ? pb.tile_cls[i] : -1;
+    int inc = c;
     for (int o = 1; o < 32; o <<= 1) {
-        long long v = __shfl_up_sync(0xffffffffu, inc, o);
+        int v = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += v;
     }
     if (lane == 31) s_warp[wid] = inc;
-    atomicAdd(&s_cls[0], c_in); atomicAdd(&s_cls[1], c_bo); atomicAdd(&s_cls[2], c_ex); atomicAdd(&s_cls[3], c_em);
+    unsigned m_in = __ballot_sync(0xffffffffu, cls == TC_INSIDE), m_bo = __ballot_sync(0xffffffffu, cls == TC_BORDER);
+    unsigned m_ex = __ballot_sync(0xffffffffu, cls == TC_EXACT), m_em = __ballot_sync(0xffffffffu, cls == TC_EMPTY);
+    if (lane == 0) {
+        PlanStats* st = pb.stats;
+        if (m_in) atomicAdd((unsigned long long*)&st->n_inside, (unsigned long long)__popc(m_in));
+        if (m_bo) atomicAdd((unsigned long long*)&st->n_border, (unsigned long long)__popc(m_bo));
+        if (m_ex) atomicAdd((unsigned long long*)&st->n_exact, (unsigned long long)__popc(m_ex));
+        if (m_em) atomicAdd((unsigned long long*)&st->n_empty, (unsigned long long)__popc(m_em));
+    }
     __syncthreads();
     if (wid == 0) {
-        long long v = s_warp[lane], iv = v;
+        int v = s_warp[lane], iv = v;
         for (int o = 1; o < 32; o <<= 1) {
-            long long u = __shfl_up_sync(0xffffffffu, iv, o);
+            int u = __shfl_up_sync(0xffffffffu, iv, o);
             if (lane >= o) iv += u;
         }
-        s_warp[lane] = iv - v;  // exclusive
+        s_warp[lane] = iv - v;
+        if (lane == 31) pb.block_sum[blockIdx.x] = iv;
+    }
+    __syncthreads();
+    if (i < n) pb.tile_offset[i] = s_warp[wid] + inc - c;
+}
+
+__global__ void __launch_bounds__(1024) plan_offsets_final_kernel(PlanBuffers pb, long long out_capacity) {
+    __shared__ long long s_warp[32];
+    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int n = *pb.n_tiles;
+    int nb = (n + 1023) >> 10;   // <= 1024 * 16 blocks (max_tiles <= 2^24): each thread handles up to 16
+    long long v[16], sum = 0;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        int b = tid * 16 + j;
+        v[j] = (b < nb) ? (long long)pb.block_sum[b] : 0;
+        sum += v[j];
+    }
+    long long inc = sum;
+    for (int o = 1; o < 32; o <<= 1) {
+        long long u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        long long w = s_warp[lane], iw = w;
+        for (int o = 1; o < 32; o <<= 1) {
+            long long u = __shfl_up_sync(0xffffffffu, iw, o);
+            if (lane >= o) iw += u;
+        }
+        s_warp[lane] = iw - w;
     }
     __syncthreads();
     long long run = s_warp[wid] + inc - sum;
-    for (int i = b; i < e; ++i) {
-        pb.tile_offset[i] = run;
-        pb.rec[i].offset = run;
-        run += pb.tile_count[i];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        int b = tid * 16 + j;
+        if (b < nb) pb.block_base[b] = run;
+        run += v[j];
     }
-    __syncthreads();
-    if (tid == 0) {
-        long long total = (n > 0) ? pb.tile_offset[n - 1] + pb.tile_count[n - 1] : 0;
-        pb.tile_offset[n] = total;
+    if (tid == 1023) {
         PlanStats* st = pb.stats;
-        st->n_footprint = total;
+        st->n_footprint = run;
         st->n_tiles = n;
-        st->n_inside = s_cls[0]; st->n_border = s_cls[1]; st->n_exact = s_cls[2]; st->n_empty = s_cls[3];
-        if (out_capacity >= 0 && total > out_capacity) atomicOr(&st->overflow, 4);
+        if (out_capacity >= 0 && run > out_capacity) atomicOr(&st->overflow, 4);
     }
+}
+
+__device__ __forceinline__ long long tile_out_offset(const PlanBuffers& pb, int t) {
+    return pb.block_base[t >> 10] + pb.tile_offset[t];
 }
 
 // ------------------------------------------------------------------------------------ explicit list
@@ -394,7 +436,7 @@ __global__ void __launch_bounds__(256) plan_write_indices_kernel(PlanBuffers pb,
         const TileRec& r = pb.rec[t];
         int cls = r.cls;
         if (cls == TC_EMPTY) continue;
-        long long base = r.tile << 10, off = r.offset;
+        long long base = r.tile << 10, off = tile_out_offset(pb, t);
         if (cls == TC_INSIDE) {
             for (int q = 0; q < 4; ++q) {
                 int m = q * 256 + tid;

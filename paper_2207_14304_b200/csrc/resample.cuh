@@ -15,6 +15,7 @@
 
 #define RS_THREADS 256
 #define RS_BOX_FLOATS 6144   // shared-memory capacity of the staged source box (24 KB)
+#define RS_MIN_CTAS 4         // register cap 64/thread -> 4 CTAs (32 warps) per SM
 
 struct FrameArgs {
     const unsigned short* raw;
@@ -72,33 +73,58 @@ __device__ __forceinline__ float load_px(const FrameArgs& f, int W, int H, int g
     }
 }
 
+// A2 for one pixel on the fast (bilinear) path: raw arrives as a 16-bit field, converted with the
+// 2^23 magic-number trick (exact), divided with rcp.approx.ftz (2 ulp: DESIGN.md "calibration precision");
+// flat_min <= flat < +inf is one unsigned range compare on the float bits (flat_min > 0 enforced by the API).
+__device__ __forceinline__ float rcp_ftz(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float calib_fast(unsigned magic_r, float b, float d, float fl, bool bpm_bad, float t_exp,
+                                            float sat_f, unsigned fmin_bits, unsigned frange) {
+    float rf = __uint_as_float(magic_r) - 8388608.0f;
+    float c = fmaf(-d, t_exp, rf - b) * rcp_ftz(fl);
+    bool good = !bpm_bad && (rf < sat_f) && ((__float_as_uint(fl) - fmin_bits) < frange) && (fabsf(c) < INFINITY);
+    return good ? c : nanf_();
+}
+
 // Stage the box [gx0, gx0+bw) x [gy0, gy0+bh) (gx0, bw multiples of 4) into s_box (pitch bw).
 // Returns non-zero for threads that stored a masked pixel.
 template <bool FUSED, bool PRECISE>
 __device__ __forceinline__ int stage_box(const FrameArgs& f, int W, int H, int gx0, int gy0, int bw, int bh,
                                          float* s_box, int tid) {
     int bad_any = 0;
-    int bw4 = bw >> 2, nvec = bw4 * bh;
-    unsigned M = (1048576u + bw4 - 1) / bw4;   // exact division by bw4 for v < 2^14
+    const int bw4 = bw >> 2, nvec = bw4 * bh;
+    const unsigned M = (1048576u + bw4 - 1) / bw4;   // exact division by bw4 for v < 2^14
+    const unsigned fmin_bits = __float_as_uint(f.flat_min), frange = 0x7f800000u - fmin_bits;
+    const float sat_f = (float)f.sat_adu;
     for (int v = tid; v < nvec; v += RS_THREADS) {
         int row = (int)(((unsigned)v * M) >> 20);
         int c4 = v - row * bw4;
         int gy = gy0 + row, gx = gx0 + 4 * c4;
         float4 o4;
-        if (f.vec_ok && gy >= 0 && gy < H && gx >= 0 && gx + 3 < W) {
-            size_t o = (size_t)gy * W + gx;
+        if (f.vec_ok && (unsigned)gy < (unsigned)H && gx >= 0 && gx + 3 < W) {
+            unsigned o = (unsigned)gy * (unsigned)W + (unsigned)gx;   // vec_ok implies W*H < 2^31
             if (FUSED) {
                 uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
                 float4 b = __ldg(reinterpret_cast<const float4*>(f.bias + o));
                 float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));
                 float4 fl = __ldg(reinterpret_cast<const float4*>(f.flat + o));
-                int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
                 unsigned bp = 0;
                 if (f.bpm) bp = __ldg(reinterpret_cast<const unsigned*>(f.bpm + o));
-                o4.x = calib_sel<PRECISE>((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
-                o4.y = calib_sel<PRECISE>((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
-                o4.z = calib_sel<PRECISE>((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
-                o4.w = calib_sel<PRECISE>((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+                if (PRECISE) {
+                    int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
+                    o4.x = calib_px_precise((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
+                    o4.y = calib_px_precise((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
+                    o4.z = calib_px_precise((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
+                    o4.w = calib_px_precise((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+                } else {
+                    o4.x = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, d.x, fl.x, bp & 0xffu, f.t_exp, sat_f, fmin_bits, frange);
+                    o4.y = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, d.y, fl.y, bp & 0xff00u, f.t_exp, sat_f, fmin_bits, frange);
+                    o4.z = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, d.z, fl.z, bp & 0xff0000u, f.t_exp, sat_f, fmin_bits, frange);
+                    o4.w = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, d.w, fl.w, bp & 0xff000000u, f.t_exp, sat_f, fmin_bits, frange);
+                }
             } else {
                 float4 c = __ldg(reinterpret_cast<const float4*>(f.cal + o));
                 unsigned mk = __ldg(reinterpret_cast<const unsigned*>(f.mask + o));
@@ -191,7 +217,7 @@ __device__ __forceinline__ void interp_lanczos3_masked(const Taps& tp, int i, in
 // COADD: accumulate into the coadd buffer instead of writing value / weight.
 // ------------------------------------------------------------------------------------------------
 template <int KERNEL, bool FUSED, bool COADD>
-__global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, PlanBuffers pb, FrameArgs f, float w_min,
+__global__ void __launch_bounds__(RS_THREADS, KERNEL == 0 ? RS_MIN_CTAS : 2) resample_tiles_kernel(DevWcs w, PlanBuffers pb, FrameArgs f, float w_min,
                                                                    float* __restrict__ value_out,
                                                                    float* __restrict__ weight_out, long long out_cap,
                                                                    CoaddArgs ca) {
@@ -204,18 +230,20 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
     const int TL = KERNEL ? 2 : 0, TR = KERNEL ? 3 : 1;
     // this thread's pixels: Morton index m_q = tid + 256 q -> (u, v) = (ul + 16 (q & 1), vl + 16 (q >> 1))
     const int ul = (int)compact_even_bits((unsigned)tid), vl = (int)compact_even_bits((unsigned)tid >> 1);
+    const int s0 = 2 * ul - 31, t0 = 2 * vl - 31;           // doubled centred offsets of pixel q = 0
+    const float S0 = (float)s0 * 0.03125f, S1 = S0 + 1.0f, T0 = (float)t0 * 0.03125f, T1 = T0 + 1.0f;
 
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         const TileRec* __restrict__ rp = pb.rec + t;
         const int cls = rp->cls;
         if (cls == TC_EMPTY) continue;              // uniform over the CTA
-        const long long off = rp->offset;
+        const long long off = tile_out_offset(pb, t);
         // source box (cells of floor(x), floor(y) plus the kernel's tap extent), x aligned to 4
         int gx0 = (rp->bx0 - TL) & ~3, gx1 = rp->bx1 + TR;
         int gy0 = rp->by0 - TL, gy1 = rp->by1 + TR;
-        // clip to the frame plus a one-vector apron (everything beyond is off-frame = masked anyway)
+        // clip to the frame plus the tap apron (everything beyond is off-frame = masked anyway)
         gx0 = max(gx0, -4); gx1 = min(gx1, w.W - 1 + TR); gy0 = max(gy0, -1 - TL); gy1 = min(gy1, w.H - 1 + TR);
-        int bw = ((gx1 - gx0 + 1) + 3) & ~3, bh = gy1 - gy0 + 1;
+        const int bw = ((gx1 - gx0 + 1) + 3) & ~3, bh = gy1 - gy0 + 1;
         const bool fits = (bw > 0 && bh > 0 && bw * bh <= RS_BOX_FLOATS);
         __syncthreads();                            // previous tile's gathers are done with s_box / s_mask
         int bad = 1;
@@ -242,6 +270,43 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
         }
         const int any_bad = __syncthreads_or(bad);
 
+        if (KERNEL == 0 && !COADD && cls == TC_INSIDE && fits && !any_bad && off + ARGUS_TILE_PIX <= out_cap) {
+            // ---- hot path: whole tile inside the frame, no masked source pixel, bilinear ----
+            PolyAxis px, py;
+            poly_axis_load(*rp, 0, px);
+            poly_axis_load(*rp, 1, py);
+            // Horner in T with S-dependent coefficients; pixels q and q^2 share S, q and q^1 share T
+            float Ax0 = fmaf(S0, fmaf(S0, fmaf(S0, px.c6, px.c3), px.c1), px.c0), Ax1 = fmaf(S1, fmaf(S1, fmaf(S1, px.c6, px.c3), px.c1), px.c0);
+            float Bx0 = fmaf(S0, fmaf(S0, px.c7, px.c4), px.c2), Bx1 = fmaf(S1, fmaf(S1, px.c7, px.c4), px.c2);
+            float Cx0 = fmaf(S0, px.c8, px.c5), Cx1 = fmaf(S1, px.c8, px.c5);
+            float Ay0 = fmaf(S0, fmaf(S0, fmaf(S0, py.c6, py.c3), py.c1), py.c0), Ay1 = fmaf(S1, fmaf(S1, fmaf(S1, py.c6, py.c3), py.c1), py.c0);
+            float By0 = fmaf(S0, fmaf(S0, py.c7, py.c4), py.c2), By1 = fmaf(S1, fmaf(S1, py.c7, py.c4), py.c2);
+            float Cy0 = fmaf(S0, py.c8, py.c5), Cy1 = fmaf(S1, py.c8, py.c5);
+            const int hx00 = px.a * s0 + px.b * t0, hy00 = py.a * s0 + py.b * t0;
+            const float* sb = s_box - (gy0 * bw + gx0);
+            float* vp = value_out + off + tid;
+            float* wp = weight_out + off + tid;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float T = (q >> 1) ? T1 : T0;
+                const float lox = fmaf(T, fmaf(T, fmaf(T, px.c9, (q & 1) ? Cx1 : Cx0), (q & 1) ? Bx1 : Bx0), (q & 1) ? Ax1 : Ax0);
+                const float loy = fmaf(T, fmaf(T, fmaf(T, py.c9, (q & 1) ? Cy1 : Cy0), (q & 1) ? By1 : By0), (q & 1) ? Ay1 : Ay0);
+                const int hx = hx00 + ((q & 1) ? 32 * px.a : 0) + ((q >> 1) ? 32 * px.b : 0);
+                const int hy = hy00 + ((q & 1) ? 32 * py.a : 0) + ((q >> 1) ? 32 * py.b : 0);
+                const float gxf = fmaf((float)(hx & 4095), 0.000244140625f, lox), gyf = fmaf((float)(hy & 4095), 0.000244140625f, loy);
+                const float flx = floorf(gxf), fly = floorf(gyf);
+                const float fx = gxf - flx, fy = gyf - fly;
+                const int ci = px.base + (hx >> 12) + (int)flx, cj = py.base + (hy >> 12) + (int)fly;
+                const float* a = sb + (cj * bw + ci);
+                const float c00 = a[0], c01 = a[1], c10 = a[bw], c11 = a[bw + 1];
+                const float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);
+                vp[256 * q] = fmaf(fy, bot - top, top);
+                wp[256 * q] = 1.0f;
+            }
+            continue;
+        }
+
+        // ---- general path: border / exact tiles, masked pixels, Lanczos-3, coadd, oversized boxes ----
         PolyAxis px, py;
         int face = 0, ix0 = 0, iy0 = 0;
         if (cls == TC_EXACT) {
@@ -255,7 +320,7 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
         SmemTaps st{s_box, gx0, gy0, bw};
         GlobalTaps<FUSED, KERNEL == 1> gt{&f, w.W, w.H};
         const double* dc = pb.dcoef + (size_t)t * 20;
-#pragma unroll
+#pragma unroll 1
         for (int q = 0; q < 4; ++q) {
             const int m = tid + 256 * q;
             const int u = ul + 16 * (q & 1), v = vl + 16 * (q >> 1);
@@ -288,19 +353,8 @@ __global__ void __launch_bounds__(RS_THREADS) resample_tiles_kernel(DevWcs w, Pl
                 // defensive clamp: the box covers every member pixel's taps by construction
                 ci = min(max(ci, gx0 + TL), gx0 + bw - 1 - TR);
                 cj = min(max(cj, gy0 + TL), gy0 + bh - 1 - TR);
-                if (KERNEL == 0) {
-                    if (!any_bad) {
-                        const float* a = s_box + (cj - gy0) * bw + (ci - gx0);
-                        float c00 = a[0], c01 = a[1], c10 = a[bw], c11 = a[bw + 1];
-                        float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);
-                        val = fmaf(fy, bot - top, top);
-                        wgt = 1.0f;
-                    } else {
-                        interp_bilinear_masked(st, ci, cj, fx, fy, w_min, val, wgt);
-                    }
-                } else {
-                    interp_lanczos3_masked(st, ci, cj, dfx, dfy, w_min, val, wgt);
-                }
+                if (KERNEL == 0) interp_bilinear_masked(st, ci, cj, fx, fy, w_min, val, wgt);
+                else interp_lanczos3_masked(st, ci, cj, dfx, dfy, w_min, val, wgt);
             } else {
                 if (KERNEL == 0) interp_bilinear_masked(gt, ci, cj, fx, fy, w_min, val, wgt);
                 else interp_lanczos3_masked(gt, ci, cj, dfx, dfy, w_min, val, wgt);
