@@ -28,7 +28,7 @@ if ROOT not in sys.path:
 
 METRIC = "calibrated+HEALPix-resampled Mpix/s per B200; achieved HBM GB/s vs peak"
 UNIT = "Mpix/s"  # input (detector) pixels per second
-SAMPLE_SIDE = 2048  # CPU-oracle sample: SAMPLE_SIDE^2 crop of the workload recipe
+SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload recipe per step
 # dram__bytes_read.sum + dram__bytes_write.sum of resample_tiles_kernel<0,true,false> on config 1, one launch,
 # from profiles/ (ncu --set full); None until captured.
 NCU_TRAFFIC_BYTES = None
@@ -99,39 +99,58 @@ def make_workload(name, rank):
     return synth.config1(seed=1 + rank), "configs[1] 9576x6388 nside 2^17 bilinear"
 
 
-def cpu_oracle_sample(threads=None):
-    """The oracle's whole path (calibrate + footprint + resample) on a SAMPLE_SIDE^2 crop of the config-1
-    recipe.  Returns (Mpix/s input, cores, seconds, description)."""
+def cpu_oracle_run(fr):
+    """The oracle's whole path (calibrate + footprint + resample), as it stands, on frame `fr`.
+    Returns (seconds, n_output_px)."""
     import oracle
-    import synth
-    fr = synth.config1(seed=1, W=SAMPLE_SIDE, H=SAMPLE_SIDE)
-    if threads:
-        oracle.set_threads(threads)
-    cores = oracle.max_threads()
-    oracle.lib()
+    H, W = fr.shape
     t0 = time.perf_counter()
     cal, mask = oracle.calibrate_frame(fr)
-    idx, _ = oracle.footprint(fr.wcs, SAMPLE_SIDE, SAMPLE_SIDE, fr.nside)
-    v, w, _ = oracle.resample(cal, mask, fr.wcs, fr.nside, idx, oracle.KERNELS[fr.kernel])
-    dt = time.perf_counter() - t0
-    desc = ("%dx%d crop of the configs[1] recipe (same noise/star/flat model, WCS, nside 2^17, bilinear), whole oracle "
-            "path calibrate+footprint+resample, %d output px" % (SAMPLE_SIDE, SAMPLE_SIDE, len(idx)))
-    return SAMPLE_SIDE * SAMPLE_SIDE / dt / 1e6, cores, dt, desc
+    idx, _ = oracle.footprint(fr.wcs, W, H, fr.nside)
+    oracle.resample(cal, mask, fr.wcs, fr.nside, idx, oracle.KERNELS[fr.kernel])
+    return time.perf_counter() - t0, len(idx)
+
+
+def cpu_sample_frame(side):
+    import synth
+    return synth.config1(seed=1, W=side, H=side)
+
+
+def cpu_desc(fr, n_out):
+    H, W = fr.shape
+    return ("%dx%d frame of the configs[1] recipe (same noise/star/flat model, WCS, nside 2^17, bilinear), whole oracle "
+            "path calibrate+footprint+resample, %d output px" % (W, H, n_out))
+
+
+def reduce_over_ranks(ms, px_in, px_out, dist=None, device=None):
+    """Whole-job accounting under torchrun: time = MAX over ranks, pixels = SUM over ranks.
+    `dist` is torch.distributed (initialised) or None for a single process."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms), float(px_in), float(px_out)
+    import torch
+    tt = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    cnt = torch.tensor([float(px_in), float(px_out)], dtype=torch.float64, device=device)
+    dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    return float(tt.item()), float(cnt[0].item()), float(cnt[1].item())
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
+    import oracle
+    oracle.lib()
+    cores = oracle.max_threads()
+    fr = cpu_sample_frame(SAMPLE_SIDE)  # generated once, outside the timed region
     for _ in range(max(0, min(args.warmup, 1))):
-        cpu_oracle_sample()
-    vals = []
-    t0 = time.perf_counter()
+        cpu_oracle_run(fr)
+    total, n_out = 0.0, 0
     for _ in range(args.steps):
-        v, cores, dt, desc = cpu_oracle_sample()
-        vals.append(v)
-    total = time.perf_counter() - t0
+        dt, n_out = cpu_oracle_run(fr)
+        total += dt
     value = SAMPLE_SIDE * SAMPLE_SIDE * args.steps / total / 1e6
+    desc = cpu_desc(fr, n_out)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -199,15 +218,7 @@ def run_gpu(args):
     plan_ms, kern_ms, ncalls = ctx.profile_read()
     ctx.set_profile(False)
     clocks = sampler.stop(t0, t1) if sampler else None
-    if world > 1:
-        tt = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-        cnt = torch.tensor([float(W * H), float(n_fp)], dtype=torch.float64, device=dev)
-        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
-        px_in_all, px_out_all = float(cnt[0].item()), float(cnt[1].item())
-    else:
-        px_in_all, px_out_all = float(W * H), float(n_fp)
+    ms, px_in_all, px_out_all = reduce_over_ranks(ms, W * H, n_fp, dist if world > 1 else None, dev)
 
     # end to end through the same API call with HOST buffers: raw frame H2D (masters stay resident per pointing,
     # PAPER.md:109,135), plan + fused kernel, value + weight D2H -- all inside the timed region
@@ -232,10 +243,7 @@ def run_gpu(args):
     e1.record()
     barrier()
     e2e_ms = e0.elapsed_time(e1)
-    if world > 1:
-        tt = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tt.item())
+    e2e_ms, _, _ = reduce_over_ranks(e2e_ms, 0, 0, dist if world > 1 else None, dev)
 
     if rank == 0:
         peak, peak_src = _peaks()
@@ -243,7 +251,13 @@ def run_gpu(args):
         alg_bytes = 14.0 * W * H + 8.0 * n_fp  # 14 B per input px + 8 B per output px
         k_ms = kern_ms / max(ncalls, 1)
         achieved = alg_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
-        cpu_v, cores, cpu_dt, cpu_desc = cpu_oracle_sample() if world == 1 else (None, None, None, "rank 0 at N=1 only")
+        if world == 1:  # the oracle, as it stands, on the same full frame the GPU just processed
+            import oracle
+            cores = oracle.max_threads()
+            cpu_dt, n_out = cpu_oracle_run(fr)
+            cpu_v, cpu_d = W * H / cpu_dt / 1e6, cpu_desc(fr, n_out)
+        else:
+            cpu_v, cores, cpu_dt, cpu_d = None, None, None, "rank 0 at N=1 only"
         line = {
             "metric": METRIC, "value": px_in_all * args.steps / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
@@ -258,7 +272,7 @@ def run_gpu(args):
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES,
                          "peak_source": peak_src, "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes,
                          "step_frac": (alg_bytes / (ms_step * 1e-3) / 1e9) / peak},
-            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc,
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_d,
                              "seconds": cpu_dt},
             "e2e": {"value": px_in_all * e2e_steps / (e2e_ms * 1e-3) / 1e6, "unit": UNIT,
                     "h2d_bytes_per_step": int(h_raw.numel() * 2), "d2h_bytes_per_step": int(n_fp * 8),
