@@ -57,6 +57,8 @@ enum { ARGUS_BILINEAR = 0, ARGUS_LANCZOS3 = 1 };
 enum {
     ARGUS_OPT_PLAN_CACHE = 1, /* 1 (default): a plan built for (wcs, W, H, nside) is reused by the next
                                  call with identical arguments; 0: every call re-plans on the device */
+    ARGUS_OPT_FAST_PATH = 3,  /* 1 (default): bilinear resampling of raw + masters (no bpm, W % 8 == 0, 16-byte aligned
+                                 arrays) stages source tiles with TMA (resample_fast_kernel); 0: always the general kernel */
     ARGUS_OPT_PROFILE = 2     /* 1: argus_resample / argus_resample_coadd (idx == NULL) record CUDA events on
                                  the caller's stream around the plan kernels and around the fused kernel
                                  (ring of 256 calls); read them back with argus_profile_read.  Default 0. */
@@ -123,6 +125,8 @@ int argus_ctx_destroy(argus_ctx* ctx);
 int argus_ctx_set_option(argus_ctx* ctx, int option, int64_t value);
 /* cudaError_t of the last failed CUDA call made through this context (0 if none). */
 int argus_last_cuda_error(const argus_ctx* ctx);
+/* Number of CUDA kernels launched through this context since its creation (diagnostics; bench.py's gpu_launches). */
+int64_t argus_launch_count(const argus_ctx* ctx);
 
 /* A2 (standalone; the paper's unfused order).  Per pixel:
  *   good = raw < sat_adu && (bpm == NULL || bpm == 0) && flat >= flat_min && all masters finite

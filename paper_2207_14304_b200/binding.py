@@ -13,11 +13,12 @@ import torch
 ARGUS_BILINEAR, ARGUS_LANCZOS3 = 0, 1
 ARGUS_OPT_PLAN_CACHE = 1
 ARGUS_OPT_PROFILE = 2
+ARGUS_OPT_FAST_PATH = 3
 _KERNELS = {"bilinear": ARGUS_BILINEAR, "lanczos3": ARGUS_LANCZOS3, 0: 0, 1: 1}
 
 EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
-    "argus_last_cuda_error", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
+    "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
 ]
 
@@ -79,6 +80,8 @@ def load_library():
     L.argus_ctx_destroy.argtypes = [vp]
     L.argus_ctx_set_option.argtypes = [vp, C.c_int, i64]
     L.argus_last_cuda_error.argtypes = [vp]
+    L.argus_launch_count.argtypes = [vp]
+    L.argus_launch_count.restype = i64
     L.argus_calibrate.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, f32, i32, f32, vp, vp, vp]
     L.argus_healpix_footprint.argtypes = [vp, C.POINTER(_Wcs), i64, i64, i64, vp, sz, C.POINTER(sz), vp]
     L.argus_resample.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, vp, sz, vp, vp, vp]
@@ -182,6 +185,14 @@ class Context:
         rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_PROFILE, 1 if on else 0)
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")
+
+    def set_fast_path(self, on: bool):
+        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_FAST_PATH, 1 if on else 0)
+        if rc:
+            raise ArgusError(rc, "argus_ctx_set_option")
+
+    def launch_count(self) -> int:
+        return int(load_library().argus_launch_count(self._h))
 
     def profile_read(self, stream=None):
         """Returns (plan_ms_total, kernel_ms_total, n_calls) of the calls recorded since profiling was enabled."""

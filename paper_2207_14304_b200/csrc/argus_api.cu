@@ -11,6 +11,7 @@
 
 #include "../../include/argus.h"
 #include "resample.cuh"
+#include "resample_fast.cuh"
 
 #define ARGUS_VERSION_NUM 100
 
@@ -30,6 +31,15 @@ struct argus_ctx {
     int prof_n;           // calls recorded since the last read
     cudaEvent_t ev[256][3];
     bool ev_plan[256];    // the call re-planned (ev[i][0] -> ev[i][1] is meaningful)
+    // TMA descriptors of the fast kernel, cached per (pointers, W, H)
+    void* encode_fn;      // cuTensorMapEncodeTiled, resolved at first use (no link-time libcuda dependency)
+    bool encode_tried;
+    bool fast_enabled;    // ARGUS_OPT_FAST_PATH
+    bool fast_attr_set;
+    FastMaps maps;
+    const void* maps_key[4];
+    int64_t maps_W, maps_H;
+    int64_t n_launches;   // kernels launched through this context (diagnostics)
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -112,6 +122,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     memset(c, 0, sizeof(*c));
     c->device = device;
     c->plan_cache = true;
+    c->fast_enabled = true;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
@@ -119,7 +130,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
@@ -136,6 +147,9 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     o_stats = o; o = align_up(o + sizeof(PlanStats), 256);
     o_pinv = o;  o = align_up(o + sizeof(double) * 250, 256);
     o_dc = o;    o = align_up(o + sizeof(double) * 20 * (size_t)pb.max_tiles, 256);
+    o_fr = o;    o = align_up(o + sizeof(FastRec) * (size_t)pb.max_tiles, 256);
+    o_sc = o;    o = align_up(o + sizeof(int), 256);
+    o_sl = o;    o = align_up(o + sizeof(int) * pb.max_hard, 256);
     e = cudaMalloc(&c->d_block, o);
     if (e == cudaSuccess) e = cudaMemset(c->d_block, 0, o);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
@@ -161,6 +175,9 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.stats = (PlanStats*)(b + o_stats);
     pb.pinv = (double*)(b + o_pinv);
     pb.dcoef = (double*)(b + o_dc);
+    pb.frec = (FastRec*)(b + o_fr);
+    pb.slow_count = (int*)(b + o_sc);
+    pb.slow_list = (int*)(b + o_sl);
     double pinv[250];
     lsq_pinv(pinv);
     e = cudaMemcpy(pb.pinv, pinv, sizeof(pinv), cudaMemcpyHostToDevice);
@@ -199,6 +216,10 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
         c->prof_n = 0;
         return ARGUS_OK;
     }
+    if (option == ARGUS_OPT_FAST_PATH) {
+        c->fast_enabled = value != 0;
+        return ARGUS_OK;
+    }
     return ARGUS_ERR_SHAPE;
 }
 
@@ -220,6 +241,7 @@ extern "C" int argus_profile_read(argus_ctx* c, double* plan_ms, double* kernel_
 }
 
 extern "C" int argus_last_cuda_error(const argus_ctx* c) { return c ? c->last_cuda : 0; }
+extern "C" int64_t argus_launch_count(const argus_ctx* c) { return c ? c->n_launches : 0; }
 
 // ------------------------------------------------------------------------------- frame constants
 static bool is_pow2(int64_t v) { return v > 0 && (v & (v - 1)) == 0; }
@@ -331,6 +353,7 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
         plan_offsets_local_kernel<<<(int)((bound + 1023) / 1024), 1024, 0, st>>>(c->pb);
         plan_offsets_final_kernel<<<1, 1024, 0, st>>>(c->pb, out_cap);
     }
+    c->n_launches += 6;
     CUDA_TRY(c, cudaGetLastError());
     c->dw = dw;
     c->key_wcs = *w;
@@ -383,6 +406,7 @@ extern "C" int argus_calibrate(argus_ctx* c, const uint16_t* raw, const float* b
                (!bpm || aligned(bpm, 4)) && aligned(cal_out, 16) && aligned(mask_out, 4);
     CUDA_TRY(c, cudaSetDevice(c->device));
     calibrate_kernel<<<c->sm_count * 8, 256, 0, (cudaStream_t)stream>>>(f, n, cal_out, mask_out);
+    c->n_launches++;
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
 }
@@ -409,6 +433,7 @@ extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64
     if (idx_out) {
         if ((size_t)c->h_stats->n_footprint > capacity) return ARGUS_ERR_CAPACITY;
         plan_write_indices_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->pb, (long long*)idx_out, (long long)capacity);
+        c->n_launches++;
         CUDA_TRY(c, cudaGetLastError());
         CUDA_TRY(c, cudaStreamSynchronize(st));
     }
@@ -428,14 +453,70 @@ extern "C" int argus_plan_info(argus_ctx* c, argus_plan_stats* out, void* stream
 }
 
 // ------------------------------------------------------------------------------------- A3..A6
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libargus.so has no link-time libcuda dependency,
+// so it loads on a machine without a driver).
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// TMA descriptors for (raw, bias, dark, flat): 2-D tensors {W, H}, boxes {40..72 step 8, 8}, zero fill outside.
+static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
+    if (!c->fast_enabled || !f.raw || f.bpm) return false;
+    if (W % 8 != 0 || W < 8 || !aligned(f.raw, 16) || !aligned(f.bias, 16) || !aligned(f.dark, 16) || !aligned(f.flat, 16)) return false;
+    if (!c->encode_tried) {
+        c->encode_tried = true;
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            c->encode_fn = fn;
+        else
+            (void)cudaGetLastError();
+    }
+    if (!c->encode_fn) return false;
+    const void* key[4] = {f.raw, f.bias, f.dark, f.flat};
+    if (memcmp(key, c->maps_key, sizeof(key)) == 0 && c->maps_W == W && c->maps_H == H) return true;
+    encode_tiled_fn enc = (encode_tiled_fn)c->encode_fn;
+    for (int wc = 0; wc < 5; ++wc)
+        for (int a = 0; a < 4; ++a) {
+            cuuint64_t dims[2] = {(cuuint64_t)W, (cuuint64_t)H};
+            cuuint64_t strides[1] = {(cuuint64_t)W * (a == 0 ? 2u : 4u)};
+            cuuint32_t box[2] = {(cuuint32_t)(40 + 8 * wc), RF_SLAB_ROWS};
+            cuuint32_t es[2] = {1, 1};
+            CUresult r = enc(&c->maps.m[wc][a], a == 0 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                             const_cast<void*>(key[a]), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) { c->maps_W = -1; return false; }
+        }
+    memcpy(c->maps_key, key, sizeof(key));
+    c->maps_W = W; c->maps_H = H;
+    return true;
+}
+
 template <bool COADD>
-static void launch_tiles(argus_ctx* c, int kernel, bool fused, const FrameArgs& f, float w_min, float* v, float* wt,
-                         long long cap, const CoaddArgs& ca, cudaStream_t st) {
+static int launch_tiles(argus_ctx* c, int kernel, bool fused, const FrameArgs& f, int64_t W, int64_t H, float w_min, float* v,
+                        float* wt, long long cap, const CoaddArgs& ca, cudaStream_t st) {
     int grid = c->sm_count * 8;
-#define LT(K, F) resample_tiles_kernel<K, F, COADD><<<grid, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca)
+    int slow_only = 0;
+    if (kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H)) {
+        // TMA-staged hot kernel for every tile that fits a stage; the general kernel takes the rest
+        if (!c->fast_attr_set) {
+            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+            c->fast_attr_set = true;
+        }
+        resample_fast_kernel<COADD><<<c->sm_count * RF_CTAS_PER_SM, RF_THREADS, sizeof(FastSmem), st>>>(
+            c->maps, c->pb, f.t_exp, f.flat_min, f.sat_adu, w_min, v, wt, cap, ca);
+        c->n_launches++;
+        slow_only = 1;
+        grid = c->sm_count * 2;
+    }
+#define LT(K, F) resample_tiles_kernel<K, F, COADD><<<grid, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca, slow_only)
     if (kernel == ARGUS_BILINEAR) { if (fused) LT(0, true); else LT(0, false); }
     else { if (fused) LT(1, true); else LT(1, false); }
 #undef LT
+    c->n_launches++;
+    return ARGUS_OK;
 }
 
 extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
@@ -463,6 +544,7 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
         if (kernel == ARGUS_BILINEAR) { if (fused) LL(0, true); else LL(0, false); }
         else { if (fused) LL(1, true); else LL(1, false); }
 #undef LL
+        c->n_launches++;
         CUDA_TRY(c, cudaGetLastError());
         return ARGUS_OK;
     }
@@ -474,7 +556,8 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     if (c->profile) cudaEventRecord(c->ev[slot][1], st);
     CoaddArgs ca;
     memset(&ca, 0, sizeof(ca));
-    launch_tiles<false>(c, kernel, fused, f, w_min, value_out, weight_out, (long long)n, ca, st);
+    rc = launch_tiles<false>(c, kernel, fused, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
+    if (rc) return rc;
     if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
@@ -509,6 +592,7 @@ extern "C" int argus_coadd_accumulate(argus_ctx* c, const argus_coadd* layout, i
     CUDA_TRY(c, cudaSetDevice(c->device));
     coadd_list_kernel<<<(int)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(ca, ppt_log2, (const long long*)idx, value,
                                                                               weight, (long long)n);
+    c->n_launches++;
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
 }
@@ -534,7 +618,8 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     rc = build_plan(c, wcs, W, H, nside, -1, st);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][1], st);
-    launch_tiles<true>(c, kernel, fused, f, w_min, nullptr, nullptr, 0, ca, st);
+    rc = launch_tiles<true>(c, kernel, fused, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
+    if (rc) return rc;
     if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;

@@ -52,6 +52,33 @@ struct __align__(16) TileRec {
     int pad[2];
 };
 
+// Compact per-tile record of the TMA-staged bilinear kernel (resample_fast.cuh): 40 words = 10 x 16 B.
+// Source position of the output pixel with doubled centred offsets (s, t) (odd integers in [-31, 31]),
+// in units of 2^-22 px relative to the integer base (X0, Y0):
+//   xf = c0x + ax*s + bx*t + float_as_int( P_x(s/32, t/32) )      (P_x already scaled by 2^22 and offset by
+//   the 1.5*2^23 rounding constant, which c0x compensates);  cell = X0 + (xf >> 22), frac = (xf & (2^22-1)) 2^-22.
+// The linear part is exact integer arithmetic; only the remainder (|.| < 0.9 px) is FP32.
+#define FAST_FRAC_BITS 22
+#define FAST_MAGIC_F 12582912.0f          // 1.5 * 2^23
+#define FAST_MAGIC_I 0x4B400000
+#define FAST_CAP_PX 3584                  // staged source pixels per tile (box width x rows padded to 8)
+#define FAST_CAL_FLOATS 4096              // calibrated box (rows x bank-conflict-free pitch)
+struct __align__(16) FastRec {
+    int cls;             // TC_INSIDE / TC_BORDER when the tile is handled by the fast kernel, else 0
+    int mask_slot;       // TC_BORDER: row of the membership-mask array
+    int gx0, gy0;        // origin (cell) of the staged source box
+    int wclass;          // staged box width: 40 + 8 * wclass px (0..4)
+    int bh;              // rows of the box holding taps
+    int kofs;            // (Y0 - gy0) * pitch + (X0 - gx0): cell -> calibrated-box index offset
+    int X0;
+    int c0x, ax, bx, c0y, ay, by;
+    int Y0, pad;
+    float px[10];        // [0] = rounding constant, [1..9] monomials S, T, S^2, ST, T^2, S^3, S^2 T, S T^2, T^3
+    float py[10];
+    float pad2[4];
+};
+static_assert(sizeof(FastRec) == 160, "FastRec must be 10 x 16 bytes");
+
 struct PlanStats {
     long long n_footprint, n_tiles, n_inside, n_border, n_exact, n_empty;
     int overflow;        // bit0: tile capacity, bit1: mask capacity, bit2: output capacity

@@ -35,6 +35,9 @@ struct PlanBuffers {
     PlanStats* stats;           // device
     double* pinv;               // [10][25] least-squares pseudo-inverse of the node design matrix
     double* dcoef;              // [max_tiles][20] unsplit FP64 polynomial coefficients (x then y)
+    FastRec* frec;              // [max_tiles] records of the TMA-staged bilinear kernel
+    int* slow_count;            // device scalar
+    int* slow_list;             // [max_hard] tiles the fast kernel leaves to the general kernel
     int max_slots, max_tiles, max_hard;
 };
 
@@ -63,6 +66,7 @@ __global__ void __launch_bounds__(256) plan_scan_kernel(DevWcs w, CoarseList cl,
     if (threadIdx.x == 0) pb.block_count[blockIdx.x] = cnt;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         *pb.hard_count = 0;
+        *pb.slow_count = 0;
         PlanStats* st = pb.stats;
         st->overflow = 0;
         st->n_inside = st->n_border = st->n_exact = st->n_empty = 0;
@@ -126,6 +130,29 @@ __device__ inline double warp_max(double v) {
 __device__ inline void cubic_basis(double S, double T, double m[10]) {
     m[0] = 1.0; m[1] = S; m[2] = T; m[3] = S * S; m[4] = S * T; m[5] = T * T;
     m[6] = S * S * S; m[7] = S * S * T; m[8] = S * T * T; m[9] = T * T * T;
+}
+
+// Staged-box geometry of the fast kernel for cells [bx0, bx1] x [by0, by1] (+1 bilinear tap).  The TMA box must
+// start on a 16-byte boundary of every array (8 pixels of the uint16 frame), so the origin is aligned down to 8;
+// widths come in steps of 8 px (40..72).  Returns false when the box does not fit its shared-memory stage.
+__device__ __host__ inline int fast_cal_pitch(int boxw) { return (boxw & 15) == 8 ? boxw : boxw + 8; }   // = 8 or 24 mod 32
+__device__ inline bool fast_box(int bx0, int bx1, int by0, int by1, int X0, int Y0, FastRec& f) {
+    int gx0 = bx0 & ~7;
+    int bw = bx1 + 2 - gx0, bh = by1 - by0 + 2;
+    if (bw < 1 || bh < 1 || bw > 72 || bh > 64) return false;
+    int wclass = bw <= 40 ? 0 : (bw - 40 + 7) >> 3;
+    int boxw = 40 + 8 * wclass, pitch = fast_cal_pitch(boxw);
+    if (((bh + 7) & ~7) * boxw > FAST_CAP_PX || bh * pitch > FAST_CAL_FLOATS) return false;
+    if (gx0 < X0 || by0 < Y0 || bx1 + 2 - X0 > 500 || by1 + 2 - Y0 > 500) return false;
+    f.gx0 = gx0; f.gy0 = by0; f.wclass = wclass; f.bh = bh;
+    f.kofs = (Y0 - by0) * pitch + (X0 - gx0);
+    return true;
+}
+
+__device__ inline void slow_push(const PlanBuffers& pb, int t) {
+    int s = atomicAdd(pb.slow_count, 1);
+    if (s < pb.max_hard) pb.slow_list[s] = t;
+    else atomicOr(&pb.stats->overflow, 2);
 }
 
 #define FIT_WARPS 8
@@ -240,6 +267,38 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
             pb.rec[t] = r;
             pb.tile_count[t] = r.count;
             pb.tile_cls[t] = (unsigned char)cls;
+            // record of the fast (TMA-staged bilinear) kernel
+            FastRec f;
+            memset(&f, 0, sizeof(f));
+            bool poly_ok = false;
+            if (cls == TC_INSIDE || cls == TC_BORDER) {
+                poly_ok = true;
+                for (int axis = 0; axis < 2; ++axis) {
+                    const double* c = s_coef[wid] + 10 * axis;
+                    int base = (axis ? r.by0 : r.bx0) - 8;
+                    double c0l = c[0] - (double)base;
+                    int c0f = (int)rint(c0l * 4194304.0);
+                    int af = (int)rint(c[1] * 131072.0), bf = (int)rint(c[2] * 131072.0);   // c/32 * 2^22
+                    float* pp = axis ? f.py : f.px;
+                    pp[0] = (float)(12582912.0 + (c0l * 4194304.0 - (double)c0f));
+                    pp[1] = (float)((c[1] * 131072.0 - (double)af) * 32.0);
+                    pp[2] = (float)((c[2] * 131072.0 - (double)bf) * 32.0);
+                    double mag = fabs((double)pp[1]) + fabs((double)pp[2]);
+                    for (int i = 3; i < 10; ++i) { pp[i] = (float)(c[i] * 4194304.0); mag += fabs((double)pp[i]); }
+                    if (!(mag < 0.9 * 4194304.0) || !(fabs(c0l) < 400.0)) poly_ok = false;
+                    if (axis) { f.Y0 = base; f.c0y = c0f - FAST_MAGIC_I; f.ay = af; f.by = bf; }
+                    else { f.X0 = base; f.c0x = c0f - FAST_MAGIC_I; f.ax = af; f.bx = bf; }
+                }
+                f.mask_slot = r.mask_slot;
+                f.pad = poly_ok ? 1 : 0;
+                if (cls == TC_INSIDE) {
+                    if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) f.cls = TC_INSIDE;
+                    else slow_push(pb, t);
+                }   // TC_BORDER: plan_members_kernel finalises the box and decides
+            } else if (cls == TC_EXACT) {
+                slow_push(pb, t);
+            }
+            pb.frec[t] = f;
         }
         __syncwarp();
     }
@@ -331,6 +390,16 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
                 pb.tile_cls[t] = TC_EMPTY;
             } else {
                 wr->bx0 = s_ext[0]; wr->bx1 = s_ext[1]; wr->by0 = s_ext[2]; wr->by1 = s_ext[3];
+                if (cls == TC_BORDER) {
+                    FastRec* fr = &pb.frec[t];
+                    FastRec f = *fr;
+                    if (f.pad && fast_box(s_ext[0], s_ext[1], s_ext[2], s_ext[3], f.X0, f.Y0, f)) {
+                        f.cls = TC_BORDER;
+                        *fr = f;
+                    } else {
+                        slow_push(pb, t);
+                    }
+                }
             }
         }
         __syncthreads();

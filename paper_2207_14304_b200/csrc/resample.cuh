@@ -220,7 +220,7 @@ template <int KERNEL, bool FUSED, bool COADD>
 __global__ void __launch_bounds__(RS_THREADS, KERNEL == 0 ? RS_MIN_CTAS : 2) resample_tiles_kernel(DevWcs w, PlanBuffers pb, FrameArgs f, float w_min,
                                                                    float* __restrict__ value_out,
                                                                    float* __restrict__ weight_out, long long out_cap,
-                                                                   CoaddArgs ca) {
+                                                                   CoaddArgs ca, int slow_only) {
     __shared__ __align__(16) float s_box[RS_BOX_FLOATS];
     __shared__ unsigned s_mask[32];
     __shared__ int s_pref[32];
@@ -233,7 +233,10 @@ __global__ void __launch_bounds__(RS_THREADS, KERNEL == 0 ? RS_MIN_CTAS : 2) res
     const int s0 = 2 * ul - 31, t0 = 2 * vl - 31;           // doubled centred offsets of pixel q = 0
     const float S0 = (float)s0 * 0.03125f, S1 = S0 + 1.0f, T0 = (float)t0 * 0.03125f, T1 = T0 + 1.0f;
 
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+    // slow_only: visit only the tiles the TMA-staged kernel (resample_fast.cuh) left to this one
+    const int n_items = slow_only ? min(*pb.slow_count, pb.max_hard) : n_tiles;
+    for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+        const int t = slow_only ? pb.slow_list[it] : it;
         const TileRec* __restrict__ rp = pb.rec + t;
         const int cls = rp->cls;
         if (cls == TC_EMPTY) continue;              // uniform over the CTA

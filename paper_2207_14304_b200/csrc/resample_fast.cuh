@@ -1,0 +1,321 @@
+// resample_fast.cuh -- A2..A5 (+A6) fused, bilinear, TMA-staged: the hot kernel of the path.
+//
+// Persistent CTAs (3 per SM), 8 consumer warps + 1 producer warp, one 32x32 output tile per iteration:
+//   producer  reads the tile's FastRec, writes a descriptor to shared memory and issues one
+//             cp.async.bulk.tensor (TMA) per 8-row slab and per array (raw u16, bias, dark, flat f32) into
+//             the stage buffer; out-of-frame elements arrive as zeros (flat = 0 < flat_min => masked), so no
+//             bounds logic exists anywhere.  The loads of tile i+1 are in flight while tile i is gathered.
+//   consumers wait on the mbarrier, calibrate the staged box ONCE from shared memory into a
+//             float32 box (masked pixels as NaN; the stage is a dense array, so there is no index arithmetic),
+//             release the stage, then gather: coordinates from the tile polynomial (exact integer linear part
+//             + FP32 remainder, common.cuh), four taps, bilinear, value + weight stores of
+//             32 consecutive floats per warp -- or the coadd read-modify-write.
+// Tiles that do not fit a stage, belt/cap-ring and pole tiles are left to resample_tiles_kernel (slow list).
+#pragma once
+#include <cuda.h>
+
+#include "common.cuh"
+#include "plan.cuh"
+#include "resample.cuh"
+
+#define RF_CONSUMERS 256
+#define RF_THREADS (RF_CONSUMERS + 32)
+#define RF_CTAS_PER_SM 3
+#define RF_SLAB_ROWS 8
+
+struct FastMaps {
+    CUtensorMap m[5][4];   // [width class][raw, bias, dark, flat]; box = (40 + 8 wclass) x 8
+};
+
+struct __align__(16) FastDesc {
+    FastRec r;
+    long long off;       // output position of the tile's first pixel
+    long long cslot;     // coadd slot of the tile's first pixel, -1 = tile absent from the layout
+    unsigned mask[32];   // TC_BORDER: membership bits
+    int pref[32];        //            exclusive prefix of popc(mask)
+};
+
+struct __align__(128) FastSmem {
+    unsigned short raw[FAST_CAP_PX];
+    float bias[FAST_CAP_PX];
+    float dark[FAST_CAP_PX];
+    float flat[FAST_CAP_PX];
+    float cal[FAST_CAL_FLOATS];
+    FastDesc desc[2];
+    unsigned long long full[2];
+    unsigned long long empty;
+};
+
+// ---------------------------------------------------------------------------------- PTX wrappers
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(b)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int x, int y, unsigned long long* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y)
+        : "memory");
+}
+// named barrier 1 over the consumer threads, with an OR reduction of a predicate
+__device__ __forceinline__ int consumers_sync_or(int pred) {
+    int r;
+    asm volatile(
+        "{\n"
+        ".reg .pred p, q;\n"
+        "setp.ne.s32 p, %1, 0;\n"
+        "barrier.cta.red.or.pred q, 1, %2, p;\n"
+        "selp.s32 %0, 1, 0, q;\n"
+        "}\n"
+        : "=r"(r)
+        : "r"(pred), "n"(RF_CONSUMERS)
+        : "memory");
+    return r;
+}
+__device__ __forceinline__ void consumers_sync() { asm volatile("barrier.cta.sync 1, %0;" ::"n"(RF_CONSUMERS) : "memory"); }
+
+// ------------------------------------------------------------------------------------ coordinates
+struct FastAxis {
+    float A0, A1, B0, B1, C0, C1, c9;   // Horner in T; index = S variant (pixel column u or u + 16)
+    int lin;                            // c0 + a*s0 + b*t0
+    int da, db;                         // 32 a, 32 b: steps to u + 16 / v + 16
+};
+__device__ __forceinline__ void fast_axis_setup(const float* __restrict__ p, int c0, int a, int b, int s0, int t0, float S0,
+                                                float S1, FastAxis& ax) {
+    ax.A0 = fmaf(S0, fmaf(S0, fmaf(S0, p[6], p[3]), p[1]), p[0]);
+    ax.A1 = fmaf(S1, fmaf(S1, fmaf(S1, p[6], p[3]), p[1]), p[0]);
+    ax.B0 = fmaf(S0, fmaf(S0, p[7], p[4]), p[2]);
+    ax.B1 = fmaf(S1, fmaf(S1, p[7], p[4]), p[2]);
+    ax.C0 = fmaf(S0, p[8], p[5]);
+    ax.C1 = fmaf(S1, p[8], p[5]);
+    ax.c9 = p[9];
+    ax.lin = c0 + a * s0 + b * t0;
+    ax.da = 32 * a;
+    ax.db = 32 * b;
+}
+// q & 1: column variant, q >> 1: row variant (T = T0 or T0 + 1).  Returns the position in 2^-22 px.
+template <int Q>
+__device__ __forceinline__ int fast_axis_eval(const FastAxis& ax, float T0, float T1) {
+    const float T = (Q >> 1) ? T1 : T0;
+    const float h = fmaf(T, fmaf(T, fmaf(T, ax.c9, (Q & 1) ? ax.C1 : ax.C0), (Q & 1) ? ax.B1 : ax.B0), (Q & 1) ? ax.A1 : ax.A0);
+    return ax.lin + ((Q & 1) ? ax.da : 0) + ((Q >> 1) ? ax.db : 0) + __float_as_int(h);
+}
+__device__ __forceinline__ float fast_frac(int xf) {
+    return fmaf(__uint_as_float(((unsigned)xf & 0x3fffffu) | 0x4B000000u), 2.384185791015625e-07f, -2.0f);
+}
+
+// ------------------------------------------------------------------------------------------ kernel
+template <bool COADD>
+__global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
+    resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, float t_exp, float flat_min, int sat_adu,
+                         float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
+                         CoaddArgs ca) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    FastSmem& sm = *reinterpret_cast<FastSmem*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int n_tiles = *pb.n_tiles;
+
+    if (tid == 0) {
+        mbar_init(&sm.full[0], 1);
+        mbar_init(&sm.full[1], 1);
+        mbar_init(&sm.empty, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (tid >= RF_CONSUMERS) {
+        // ================================================================ producer warp
+        const int lane = tid - RF_CONSUMERS;
+        int issued = 0;
+        for (int t = blockIdx.x;; t += gridDim.x) {
+            const bool last = t >= n_tiles;
+            float4 rv = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (!last && lane < 10) rv = __ldg(reinterpret_cast<const float4*>(pb.frec + t) + lane);
+            // lane 0 holds cls, mask_slot, gx0, gy0; lane 1 holds wclass, bh, kofs, X0
+            const int cls = last ? -1 : __shfl_sync(0xffffffffu, __float_as_int(rv.x), 0);
+            if (cls == 0) continue;                         // empty, or left to the general kernel
+            const int slot = issued & 1;
+            if (issued > 0) mbar_wait(&sm.empty, (unsigned)((issued - 1) & 1));   // stage free: tile issued-1 is calibrated
+            FastDesc& d = sm.desc[slot];
+            if (last) {
+                if (lane == 0) {
+                    d.r.cls = -1;
+                    mbar_arrive(&sm.full[slot]);
+                }
+                break;
+            }
+            const int mask_slot = __shfl_sync(0xffffffffu, __float_as_int(rv.y), 0);
+            const int gx0 = __shfl_sync(0xffffffffu, __float_as_int(rv.z), 0), gy0 = __shfl_sync(0xffffffffu, __float_as_int(rv.w), 0);
+            const int wclass = __shfl_sync(0xffffffffu, __float_as_int(rv.x), 1), bh = __shfl_sync(0xffffffffu, __float_as_int(rv.y), 1);
+            if (lane < 10) reinterpret_cast<float4*>(&d.r)[lane] = rv;
+            if (cls == TC_BORDER) {
+                unsigned mk = pb.masks[(size_t)mask_slot * 32 + lane];
+                int c = __popc(mk), inc = c;
+                for (int o = 1; o < 32; o <<= 1) {
+                    int y = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += y;
+                }
+                d.mask[lane] = mk;
+                d.pref[lane] = inc - c;
+            }
+            if (lane == 0) {
+                d.off = tile_out_offset(pb, t);
+                if (COADD) {
+                    long long tile = pb.tile_id[t];
+                    long long key = tile >> ca.shift, lo = 0, hi = ca.n_tiles - 1, pos = -1;
+                    while (lo <= hi) {
+                        long long mid = (lo + hi) >> 1, tv = ca.tiles[mid];
+                        if (tv == key) { pos = mid; break; }
+                        if (tv < key) lo = mid + 1; else hi = mid - 1;
+                    }
+                    long long ppt = 1ll << (ca.shift + 10);
+                    d.cslot = pos < 0 ? -1 : pos * ppt + ((tile << 10) & (ppt - 1));
+                }
+            }
+            __syncwarp();
+            const int boxw = 40 + 8 * wclass;
+            const int nslab = (bh + RF_SLAB_ROWS - 1) / RF_SLAB_ROWS;
+            if (lane == 0) {
+                // one elected thread issues every bulk-tensor copy (descriptor and addresses must be warp-uniform)
+                mbar_arrive_expect_tx(&sm.full[slot], (unsigned)(nslab * RF_SLAB_ROWS * boxw * 14));
+                const CUtensorMap* mp = &maps.m[wclass][0];
+                for (int slab = 0; slab < nslab; ++slab) {
+                    const int px0 = slab * RF_SLAB_ROWS * boxw, y = gy0 + slab * RF_SLAB_ROWS;
+                    tma_load_2d(sm.raw + px0, mp + 0, gx0, y, &sm.full[slot]);
+                    tma_load_2d(sm.bias + px0, mp + 1, gx0, y, &sm.full[slot]);
+                    tma_load_2d(sm.dark + px0, mp + 2, gx0, y, &sm.full[slot]);
+                    tma_load_2d(sm.flat + px0, mp + 3, gx0, y, &sm.full[slot]);
+                }
+            }
+            ++issued;
+        }
+        return;
+    }
+
+    // ==================================================================== consumer warps
+    const int lane = tid & 31;
+    const int ul = (int)compact_even_bits((unsigned)tid), vl = (int)compact_even_bits((unsigned)tid >> 1);
+    const int s0 = 2 * ul - 31, t0 = 2 * vl - 31;
+    const float S0 = (float)s0 * 0.03125f, S1 = S0 + 1.0f, T0 = (float)t0 * 0.03125f, T1 = T0 + 1.0f;
+    const unsigned fmin_bits = __float_as_uint(flat_min), frange = 0x7f800000u - fmin_bits;
+    const float sat_f = (float)sat_adu;
+
+    for (int it = 0;; ++it) {
+        const int slot = it & 1;
+        mbar_wait(&sm.full[slot], (unsigned)((it >> 1) & 1));
+        const FastDesc& d = sm.desc[slot];
+        const int cls = d.r.cls;
+        if (cls < 0) break;
+        const int boxw = 40 + 8 * d.r.wclass, pitch = fast_cal_pitch(boxw);
+        const int bw4 = boxw >> 2, n4 = d.r.bh * bw4;
+        const unsigned M = (1048576u + bw4 - 1) / bw4;   // exact division by bw4 for v < 2^14
+        // ---- A2: calibrate the staged box once, shared -> shared.  The stage is dense (item v <-> float4 v);
+        //      the calibrated box gets a pitch of 8 or 24 mod 32 floats so that the gather is bank-conflict free
+        int bad = 0;
+        for (int v = tid; v < n4; v += RF_CONSUMERS) {
+            const uint2 rw = reinterpret_cast<const uint2*>(sm.raw)[v];
+            const float4 b = reinterpret_cast<const float4*>(sm.bias)[v];
+            const float4 dk = reinterpret_cast<const float4*>(sm.dark)[v];
+            const float4 fl = reinterpret_cast<const float4*>(sm.flat)[v];
+            float4 o4;
+            o4.x = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
+            o4.y = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
+            o4.z = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
+            o4.w = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
+            bad |= (o4.x != o4.x) | (o4.y != o4.y) | (o4.z != o4.z) | (o4.w != o4.w);
+            const int row = (int)(((unsigned)v * M) >> 20);
+            *reinterpret_cast<float4*>(sm.cal + row * pitch + 4 * (v - row * bw4)) = o4;
+        }
+        const int any_bad = consumers_sync_or(bad);
+        if (tid == 0) mbar_arrive(&sm.empty);        // the producer may refill the stage while we gather
+
+        // ---- A3/A4: tile polynomial -> source position; A5: bilinear
+        FastAxis ax, ay;
+        fast_axis_setup(d.r.px, d.r.c0x, d.r.ax, d.r.bx, s0, t0, S0, S1, ax);
+        fast_axis_setup(d.r.py, d.r.c0y, d.r.ay, d.r.by, s0, t0, S0, S1, ay);
+        const float* cb = sm.cal + d.r.kofs;
+        const long long off = d.off;
+
+        if (!COADD && cls == TC_INSIDE && !any_bad && off + ARGUS_TILE_PIX <= out_cap) {
+            float* vp = value_out + off + tid;
+            float* wp = weight_out + off + tid;
+#define RF_HOT(Q)                                                                            \
+    {                                                                                        \
+        const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);    \
+        const float fx = fast_frac(xf), fy = fast_frac(yf);                                  \
+        const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));      \
+        const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];                \
+        const float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);          \
+        vp[256 * Q] = fmaf(fy, bot - top, top);                                              \
+        wp[256 * Q] = 1.0f;                                                                  \
+    }
+            RF_HOT(0) RF_HOT(1) RF_HOT(2) RF_HOT(3)
+#undef RF_HOT
+        } else {
+            // masked source pixels, tiles cut by the frame border, coadd accumulation
+            const long long cslot = COADD ? d.cslot : 0;
+#define RF_GEN(Q)                                                                                          \
+    {                                                                                                      \
+        const int m = tid + 256 * Q;                                                                       \
+        bool member = true;                                                                                \
+        long long pos = m;                                                                                 \
+        if (cls != TC_INSIDE) {                                                                            \
+            const unsigned mk = d.mask[m >> 5];                                                            \
+            member = (mk >> lane) & 1u;                                                                    \
+            pos = d.pref[m >> 5] + __popc(mk & ((1u << lane) - 1u));                                       \
+        }                                                                                                  \
+        if (member) {                                                                                      \
+            const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);              \
+            const float fx = fast_frac(xf), fy = fast_frac(yf);                                            \
+            const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));                \
+            const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];                          \
+            const float gx = 1.0f - fx, gy = 1.0f - fy;                                                    \
+            const float k00 = gx * gy, k01 = fx * gy, k10 = gx * fy, k11 = fx * fy;                        \
+            const float S = (k00 + k01) + (k10 + k11);                                                     \
+            float B = 0.f, V1 = 0.f;                                                                       \
+            if (c00 == c00) V1 = fmaf(k00, c00, V1); else B += k00;                                        \
+            if (c01 == c01) V1 = fmaf(k01, c01, V1); else B += k01;                                        \
+            if (c10 == c10) V1 = fmaf(k10, c10, V1); else B += k10;                                        \
+            if (c11 == c11) V1 = fmaf(k11, c11, V1); else B += k11;                                        \
+            const float w = 1.0f - B / S;                                                                  \
+            float val = 0.f, wgt = 0.f;                                                                    \
+            if (!(w < w_min) && (S - B > 0.f)) { val = V1 / (S - B); wgt = fminf(w, 1.0f); }               \
+            if (COADD) {                                                                                   \
+                if (cslot >= 0) {                                                                          \
+                    ca.sum[cslot + m] = fmaf(wgt, val, ca.sum[cslot + m]);                                 \
+                    ca.wsum[cslot + m] += wgt;                                                             \
+                } else if (ca.n_skipped) {                                                                 \
+                    atomicAdd(ca.n_skipped, 1ull);                                                         \
+                }                                                                                          \
+            } else if (off + pos < out_cap) {                                                              \
+                value_out[off + pos] = val;                                                                \
+                weight_out[off + pos] = wgt;                                                               \
+            }                                                                                              \
+        }                                                                                                  \
+    }
+            RF_GEN(0) RF_GEN(1) RF_GEN(2) RF_GEN(3)
+#undef RF_GEN
+        }
+        consumers_sync();   // all gathers done before the next tile's calibration overwrites sm.cal / desc
+    }
+}
