@@ -459,7 +459,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// TMA descriptors for (raw, bias, dark, flat): 2-D tensors {W, H}, boxes {40..72 step 8, 8}, zero fill outside.
+// TMA descriptors for (raw, bias, dark, flat): 2-D tensors {W, H}, boxes {40..72 step 8} x {48, 56, 64}, zero fill outside.
 static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
     if (!c->fast_enabled || !f.raw || f.bpm) return false;
     if (W % 8 != 0 || W < 8 || !aligned(f.raw, 16) || !aligned(f.bias, 16) || !aligned(f.dark, 16) || !aligned(f.flat, 16)) return false;
@@ -477,13 +477,14 @@ static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
     const void* key[4] = {f.raw, f.bias, f.dark, f.flat};
     if (memcmp(key, c->maps_key, sizeof(key)) == 0 && c->maps_W == W && c->maps_H == H) return true;
     encode_tiled_fn enc = (encode_tiled_fn)c->encode_fn;
-    for (int wc = 0; wc < 5; ++wc)
+    for (int hc = 0; hc < 3; ++hc)
+      for (int wc = 0; wc < 5; ++wc)
         for (int a = 0; a < 4; ++a) {
             cuuint64_t dims[2] = {(cuuint64_t)W, (cuuint64_t)H};
             cuuint64_t strides[1] = {(cuuint64_t)W * (a == 0 ? 2u : 4u)};
-            cuuint32_t box[2] = {(cuuint32_t)(40 + 8 * wc), RF_SLAB_ROWS};
+            cuuint32_t box[2] = {(cuuint32_t)(40 + 8 * wc), (cuuint32_t)(48 + 8 * hc)};
             cuuint32_t es[2] = {1, 1};
-            CUresult r = enc(&c->maps.m[wc][a], a == 0 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+            CUresult r = enc(&c->maps.m[hc][wc][a], a == 0 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
                              const_cast<void*>(key[a]), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) { c->maps_W = -1; return false; }

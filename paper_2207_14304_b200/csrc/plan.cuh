@@ -134,7 +134,8 @@ __device__ inline void cubic_basis(double S, double T, double m[10]) {
 
 // Staged-box geometry of the fast kernel for cells [bx0, bx1] x [by0, by1] (+1 bilinear tap).  The TMA box must
 // start on a 16-byte boundary of every array (8 pixels of the uint16 frame), so the origin is aligned down to 8;
-// widths come in steps of 8 px (40..72).  Returns false when the box does not fit its shared-memory stage.
+// widths come in steps of 8 px (40..72), heights are 48, 56 or 64 rows (a TMA copy costs ~100 cycles per
+// operation whatever its size, so each array is fetched with ONE box).  Returns false when the box does not fit its shared-memory stage.
 __device__ __host__ inline int fast_cal_pitch(int boxw) { return (boxw & 15) == 8 ? boxw : boxw + 8; }   // = 8 or 24 mod 32
 __device__ inline bool fast_box(int bx0, int bx1, int by0, int by1, int X0, int Y0, FastRec& f) {
     int gx0 = bx0 & ~7;
@@ -142,9 +143,10 @@ __device__ inline bool fast_box(int bx0, int bx1, int by0, int by1, int X0, int 
     if (bw < 1 || bh < 1 || bw > 72 || bh > 64) return false;
     int wclass = bw <= 40 ? 0 : (bw - 40 + 7) >> 3;
     int boxw = 40 + 8 * wclass, pitch = fast_cal_pitch(boxw);
-    if (((bh + 7) & ~7) * boxw > FAST_CAP_PX || bh * pitch > FAST_CAL_FLOATS) return false;
+    int hclass = bh <= 48 ? 0 : (bh <= 56 ? 1 : 2);      // one TMA box per array: 48, 56 or 64 rows
+    if ((48 + 8 * hclass) * boxw > FAST_CAP_PX || bh * pitch > FAST_CAL_FLOATS) return false;
     if (gx0 < X0 || by0 < Y0 || bx1 + 2 - X0 > 500 || by1 + 2 - Y0 > 500) return false;
-    f.gx0 = gx0; f.gy0 = by0; f.wclass = wclass; f.bh = bh;
+    f.gx0 = gx0; f.gy0 = by0; f.wclass = wclass | (hclass << 4); f.bh = bh;
     f.kofs = (Y0 - by0) * pitch + (X0 - gx0);
     return true;
 }

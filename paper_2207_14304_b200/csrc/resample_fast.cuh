@@ -2,7 +2,7 @@
 //
 // Persistent CTAs (3 per SM), 8 consumer warps + 1 producer warp, one 32x32 output tile per iteration:
 //   producer  reads the tile's FastRec, writes a descriptor to shared memory and issues one
-//             cp.async.bulk.tensor (TMA) per 8-row slab and per array (raw u16, bias, dark, flat f32) into
+//             cp.async.bulk.tensor (TMA) per array (raw u16, bias, dark, flat f32) into
 //             the stage buffer; out-of-frame elements arrive as zeros (flat = 0 < flat_min => masked), so no
 //             bounds logic exists anywhere.  The loads of tile i+1 are in flight while tile i is gathered.
 //   consumers wait on the mbarrier, calibrate the staged box ONCE from shared memory into a
@@ -21,10 +21,9 @@
 #define RF_CONSUMERS 256
 #define RF_THREADS (RF_CONSUMERS + 32)
 #define RF_CTAS_PER_SM 3
-#define RF_SLAB_ROWS 8
 
 struct FastMaps {
-    CUtensorMap m[5][4];   // [width class][raw, bias, dark, flat]; box = (40 + 8 wclass) x 8
+    CUtensorMap m[3][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
 };
 
 struct __align__(16) FastDesc {
@@ -193,19 +192,16 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
                 }
             }
             __syncwarp();
-            const int boxw = 40 + 8 * wclass;
-            const int nslab = (bh + RF_SLAB_ROWS - 1) / RF_SLAB_ROWS;
             if (lane == 0) {
-                // one elected thread issues every bulk-tensor copy (descriptor and addresses must be warp-uniform)
-                mbar_arrive_expect_tx(&sm.full[slot], (unsigned)(nslab * RF_SLAB_ROWS * boxw * 14));
-                const CUtensorMap* mp = &maps.m[wclass][0];
-                for (int slab = 0; slab < nslab; ++slab) {
-                    const int px0 = slab * RF_SLAB_ROWS * boxw, y = gy0 + slab * RF_SLAB_ROWS;
-                    tma_load_2d(sm.raw + px0, mp + 0, gx0, y, &sm.full[slot]);
-                    tma_load_2d(sm.bias + px0, mp + 1, gx0, y, &sm.full[slot]);
-                    tma_load_2d(sm.dark + px0, mp + 2, gx0, y, &sm.full[slot]);
-                    tma_load_2d(sm.flat + px0, mp + 3, gx0, y, &sm.full[slot]);
-                }
+                // one elected thread issues the four bulk-tensor copies (one box per array)
+                const int wc = wclass & 15, hc = wclass >> 4;
+                const int boxw = 40 + 8 * wc, boxh = 48 + 8 * hc;
+                mbar_arrive_expect_tx(&sm.full[slot], (unsigned)(boxh * boxw * 14));
+                const CUtensorMap* mp = &maps.m[hc][wc][0];
+                tma_load_2d(sm.raw, mp + 0, gx0, gy0, &sm.full[slot]);
+                tma_load_2d(sm.bias, mp + 1, gx0, gy0, &sm.full[slot]);
+                tma_load_2d(sm.dark, mp + 2, gx0, gy0, &sm.full[slot]);
+                tma_load_2d(sm.flat, mp + 3, gx0, gy0, &sm.full[slot]);
             }
             ++issued;
         }
@@ -226,7 +222,7 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
         const FastDesc& d = sm.desc[slot];
         const int cls = d.r.cls;
         if (cls < 0) break;
-        const int boxw = 40 + 8 * d.r.wclass, pitch = fast_cal_pitch(boxw);
+        const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
         const int bw4 = boxw >> 2, n4 = d.r.bh * bw4;
         const unsigned M = (1048576u + bw4 - 1) / bw4;   // exact division by bw4 for v < 2^14
         // ---- A2: calibrate the staged box once, shared -> shared.  The stage is dense (item v <-> float4 v);
