@@ -20,7 +20,8 @@
 
 #define RF_CONSUMERS 256
 #define RF_THREADS (RF_CONSUMERS + 32)
-#define RF_CTAS_PER_SM 3
+#define RF_CTAS_PER_SM 2
+#define RF_STAGES 2
 
 struct FastMaps {
     CUtensorMap m[3][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
@@ -34,16 +35,22 @@ struct __align__(16) FastDesc {
     int pref[32];        //            exclusive prefix of popc(mask)
 };
 
-struct __align__(128) FastSmem {
+// One stage: the raw + master boxes as the TMA delivers them (dense, pitch = box width).  After the consumers have
+// read them into registers, the calibrated box overwrites the stage from `bias` on (pitch 8 or 24 mod 32 floats,
+// up to FAST_CAL_FLOATS floats = bias + the head of dark).
+struct __align__(128) FastStage {
     unsigned short raw[FAST_CAP_PX];
     float bias[FAST_CAP_PX];
     float dark[FAST_CAP_PX];
     float flat[FAST_CAP_PX];
-    float cal[FAST_CAL_FLOATS];
-    FastDesc desc[2];
-    unsigned long long full[2];
-    unsigned long long empty;
 };
+struct __align__(128) FastSmem {
+    FastStage stage[RF_STAGES];
+    FastDesc desc[RF_STAGES];
+    unsigned long long full[RF_STAGES];    // TMA bytes of the stage have landed (1 arrival + tx)
+    unsigned long long empty[RF_STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
+};
+static_assert(FAST_CAL_FLOATS <= 2 * FAST_CAP_PX, "calibrated box must fit bias + dark");
 
 // ---------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -135,9 +142,10 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
     const int n_tiles = *pb.n_tiles;
 
     if (tid == 0) {
-        mbar_init(&sm.full[0], 1);
-        mbar_init(&sm.full[1], 1);
-        mbar_init(&sm.empty, 1);
+        for (int i = 0; i < RF_STAGES; ++i) {
+            mbar_init(&sm.full[i], 1);
+            mbar_init(&sm.empty[i], RF_CONSUMERS);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -153,8 +161,9 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
             // lane 0 holds cls, mask_slot, gx0, gy0; lane 1 holds wclass, bh, kofs, X0
             const int cls = last ? -1 : __shfl_sync(0xffffffffu, __float_as_int(rv.x), 0);
             if (cls == 0) continue;                         // empty, or left to the general kernel
-            const int slot = issued & 1;
-            if (issued > 0) mbar_wait(&sm.empty, (unsigned)((issued - 1) & 1));   // stage free: tile issued-1 is calibrated
+            const int slot = issued % RF_STAGES;
+            // stage free: every consumer is done with the tile that used it RF_STAGES tiles ago
+            if (issued >= RF_STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / RF_STAGES - 1) & 1));
             FastDesc& d = sm.desc[slot];
             if (last) {
                 if (lane == 0) {
@@ -198,10 +207,11 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
                 const int boxw = 40 + 8 * wc, boxh = 48 + 8 * hc;
                 mbar_arrive_expect_tx(&sm.full[slot], (unsigned)(boxh * boxw * 14));
                 const CUtensorMap* mp = &maps.m[hc][wc][0];
-                tma_load_2d(sm.raw, mp + 0, gx0, gy0, &sm.full[slot]);
-                tma_load_2d(sm.bias, mp + 1, gx0, gy0, &sm.full[slot]);
-                tma_load_2d(sm.dark, mp + 2, gx0, gy0, &sm.full[slot]);
-                tma_load_2d(sm.flat, mp + 3, gx0, gy0, &sm.full[slot]);
+                FastStage& sg = sm.stage[slot];
+                tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[slot]);
+                tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[slot]);
+                tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[slot]);
+                tma_load_2d(sg.flat, mp + 3, gx0, gy0, &sm.full[slot]);
             }
             ++issued;
         }
@@ -217,39 +227,52 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
     const float sat_f = (float)sat_adu;
 
     for (int it = 0;; ++it) {
-        const int slot = it & 1;
-        mbar_wait(&sm.full[slot], (unsigned)((it >> 1) & 1));
+        const int slot = it % RF_STAGES;
+        mbar_wait(&sm.full[slot], (unsigned)((it / RF_STAGES) & 1));
         const FastDesc& d = sm.desc[slot];
         const int cls = d.r.cls;
         if (cls < 0) break;
+        FastStage& sg = sm.stage[slot];
+        float* cal = sg.bias;
         const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
         const int bw4 = boxw >> 2, n4 = d.r.bh * bw4;
         const unsigned M = (1048576u + bw4 - 1) / bw4;   // exact division by bw4 for v < 2^14
-        // ---- A2: calibrate the staged box once, shared -> shared.  The stage is dense (item v <-> float4 v);
-        //      the calibrated box gets a pitch of 8 or 24 mod 32 floats so that the gather is bank-conflict free
+        // ---- A2: calibrate the staged box once.  The stage is dense (item v <-> float4 v): four independent items
+        //      per thread are read and calibrated in registers; after a barrier (all reads done) they overwrite the
+        //      stage with a pitch of 8 or 24 mod 32 floats, which makes the gather free of bank conflicts.
+        float4 o4[4];
         int bad = 0;
-        for (int v = tid; v < n4; v += RF_CONSUMERS) {
-            const uint2 rw = reinterpret_cast<const uint2*>(sm.raw)[v];
-            const float4 b = reinterpret_cast<const float4*>(sm.bias)[v];
-            const float4 dk = reinterpret_cast<const float4*>(sm.dark)[v];
-            const float4 fl = reinterpret_cast<const float4*>(sm.flat)[v];
-            float4 o4;
-            o4.x = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
-            o4.y = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
-            o4.z = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
-            o4.w = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
-            bad |= (o4.x != o4.x) | (o4.y != o4.y) | (o4.z != o4.z) | (o4.w != o4.w);
-            const int row = (int)(((unsigned)v * M) >> 20);
-            *reinterpret_cast<float4*>(sm.cal + row * pitch + 4 * (v - row * bw4)) = o4;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int v = tid + RF_CONSUMERS * j;
+            if (v < n4) {
+                const uint2 rw = reinterpret_cast<const uint2*>(sg.raw)[v];
+                const float4 b = reinterpret_cast<const float4*>(sg.bias)[v];
+                const float4 dk = reinterpret_cast<const float4*>(sg.dark)[v];
+                const float4 fl = reinterpret_cast<const float4*>(sg.flat)[v];
+                o4[j].x = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].y = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].z = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].w = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
+                bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
+            }
         }
         const int any_bad = consumers_sync_or(bad);
-        if (tid == 0) mbar_arrive(&sm.empty);        // the producer may refill the stage while we gather
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int v = tid + RF_CONSUMERS * j;
+            if (v < n4) {
+                const int row = (int)(((unsigned)v * M) >> 20);
+                *reinterpret_cast<float4*>(cal + row * pitch + 4 * (v - row * bw4)) = o4[j];
+            }
+        }
+        consumers_sync();
 
         // ---- A3/A4: tile polynomial -> source position; A5: bilinear
         FastAxis ax, ay;
         fast_axis_setup(d.r.px, d.r.c0x, d.r.ax, d.r.bx, s0, t0, S0, S1, ax);
         fast_axis_setup(d.r.py, d.r.c0y, d.r.ay, d.r.by, s0, t0, S0, S1, ay);
-        const float* cb = sm.cal + d.r.kofs;
+        const float* cb = cal + d.r.kofs;
         const long long off = d.off;
 
         if (!COADD && cls == TC_INSIDE && !any_bad && off + ARGUS_TILE_PIX <= out_cap) {
@@ -312,6 +335,6 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
             RF_GEN(0) RF_GEN(1) RF_GEN(2) RF_GEN(3)
 #undef RF_GEN
         }
-        consumers_sync();   // all gathers done before the next tile's calibration overwrites sm.cal / desc
+        mbar_arrive(&sm.empty[slot]);   // this thread is done with the stage and its descriptor
     }
 }
