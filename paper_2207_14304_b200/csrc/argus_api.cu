@@ -507,7 +507,7 @@ static int launch_tiles(argus_ctx* c, int kernel, bool fused, const FrameArgs& f
             c->fast_attr_set = true;
         }
         resample_fast_kernel<COADD><<<c->sm_count * RF_CTAS_PER_SM, RF_THREADS, sizeof(FastSmem), st>>>(
-            c->maps, c->pb, f.t_exp, f.flat_min, f.sat_adu, w_min, v, wt, cap, ca);
+            c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
         c->n_launches++;
         slow_only = 1;
         grid = c->sm_count * 2;

@@ -72,10 +72,11 @@ struct __align__(16) FastRec {
     int kofs;            // (Y0 - gy0) * pitch + (X0 - gx0): cell -> calibrated-box index offset
     int X0;
     int c0x, ax, bx, c0y, ay, by;
-    int Y0, pad;
+    int Y0, poly_ok;     // poly_ok: the FP32 remainder stays inside the rounding-constant range
     float px[10];        // [0] = rounding constant, [1..9] monomials S, T, S^2, ST, T^2, S^3, S^2 T, S T^2, T^3
     float py[10];
-    float pad2[4];
+    int cols;            // float4 columns of the box that hold taps: first | (count << 8)
+    int pad2[3];
 };
 static_assert(sizeof(FastRec) == 160, "FastRec must be 10 x 16 bytes");
 

@@ -148,6 +148,8 @@ __device__ inline bool fast_box(int bx0, int bx1, int by0, int by1, int X0, int 
     if (gx0 < X0 || by0 < Y0 || bx1 + 2 - X0 > 500 || by1 + 2 - Y0 > 500) return false;
     f.gx0 = gx0; f.gy0 = by0; f.wclass = wclass | (hclass << 4); f.bh = bh;
     f.kofs = (Y0 - by0) * pitch + (X0 - gx0);
+    int c_lo = (bx0 - gx0) >> 2, c_hi = (bx1 + 2 - gx0 + 3) >> 2;
+    f.cols = c_lo | ((c_hi - c_lo) << 8);
     return true;
 }
 
@@ -292,7 +294,7 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
                     else { f.X0 = base; f.c0x = c0f - FAST_MAGIC_I; f.ax = af; f.bx = bf; }
                 }
                 f.mask_slot = r.mask_slot;
-                f.pad = poly_ok ? 1 : 0;
+                f.poly_ok = poly_ok ? 1 : 0;
                 if (cls == TC_INSIDE) {
                     if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) f.cls = TC_INSIDE;
                     else slow_push(pb, t);
@@ -395,7 +397,7 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
                 if (cls == TC_BORDER) {
                     FastRec* fr = &pb.frec[t];
                     FastRec f = *fr;
-                    if (f.pad && fast_box(s_ext[0], s_ext[1], s_ext[2], s_ext[3], f.X0, f.Y0, f)) {
+                    if (f.poly_ok && fast_box(s_ext[0], s_ext[1], s_ext[2], s_ext[3], f.X0, f.Y0, f)) {
                         f.cls = TC_BORDER;
                         *fr = f;
                     } else {

@@ -18,10 +18,13 @@
 #include "plan.cuh"
 #include "resample.cuh"
 
-#define RF_CONSUMERS 256
-#define RF_THREADS (RF_CONSUMERS + 32)
+#define RF_CONSUMERS 256                 // threads of one consumer group (one output tile at a time)
+#ifndef RF_GROUPS
+#define RF_GROUPS 1                      // consumer groups per CTA, tiles dealt round-robin
 #define RF_CTAS_PER_SM 2
-#define RF_STAGES 2
+#define RF_STAGES 2                      // TMA stages shared by the groups: more than groups => loads run ahead
+#endif
+#define RF_THREADS (RF_GROUPS * RF_CONSUMERS + 32)
 
 struct FastMaps {
     CUtensorMap m[3][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
@@ -31,6 +34,7 @@ struct __align__(16) FastDesc {
     FastRec r;
     long long off;       // output position of the tile's first pixel
     long long cslot;     // coadd slot of the tile's first pixel, -1 = tile absent from the layout
+    float4 tab[32][2];   // per pixel column u: {Ax, Bx, Cx, Ay}, {By, Cy, -, -}: S-dependent Horner coefficients
     unsigned mask[32];   // TC_BORDER: membership bits
     int pref[32];        //            exclusive prefix of popc(mask)
 };
@@ -84,21 +88,33 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
         : "memory");
 }
 // named barrier 1 over the consumer threads, with an OR reduction of a predicate
-__device__ __forceinline__ int consumers_sync_or(int pred) {
+template <int ID>
+__device__ __forceinline__ int bar_sync_or(int pred) {
     int r;
     asm volatile(
         "{\n"
         ".reg .pred p, q;\n"
         "setp.ne.s32 p, %1, 0;\n"
-        "barrier.cta.red.or.pred q, 1, %2, p;\n"
+        "barrier.cta.red.or.pred q, %3, %2, p;\n"
         "selp.s32 %0, 1, 0, q;\n"
         "}\n"
         : "=r"(r)
-        : "r"(pred), "n"(RF_CONSUMERS)
+        : "r"(pred), "n"(RF_CONSUMERS), "n"(ID)
         : "memory");
     return r;
 }
-__device__ __forceinline__ void consumers_sync() { asm volatile("barrier.cta.sync 1, %0;" ::"n"(RF_CONSUMERS) : "memory"); }
+template <int ID>
+__device__ __forceinline__ void bar_sync() {
+    asm volatile("barrier.cta.sync %1, %0;" ::"n"(RF_CONSUMERS), "n"(ID) : "memory");
+}
+// named barrier 1 + group over the threads of one consumer group (ids must be immediates: a register id makes
+// ptxas reserve all 16 barriers)
+__device__ __forceinline__ int consumers_sync_or(int group, int pred) {
+    return group == 0 ? bar_sync_or<1>(pred) : (group == 1 ? bar_sync_or<2>(pred) : bar_sync_or<3>(pred));
+}
+__device__ __forceinline__ void consumers_sync(int group) {
+    if (group == 0) bar_sync<1>(); else if (group == 1) bar_sync<2>(); else bar_sync<3>();
+}
 
 // ------------------------------------------------------------------------------------ coordinates
 struct FastAxis {
@@ -106,19 +122,6 @@ struct FastAxis {
     int lin;                            // c0 + a*s0 + b*t0
     int da, db;                         // 32 a, 32 b: steps to u + 16 / v + 16
 };
-__device__ __forceinline__ void fast_axis_setup(const float* __restrict__ p, int c0, int a, int b, int s0, int t0, float S0,
-                                                float S1, FastAxis& ax) {
-    ax.A0 = fmaf(S0, fmaf(S0, fmaf(S0, p[6], p[3]), p[1]), p[0]);
-    ax.A1 = fmaf(S1, fmaf(S1, fmaf(S1, p[6], p[3]), p[1]), p[0]);
-    ax.B0 = fmaf(S0, fmaf(S0, p[7], p[4]), p[2]);
-    ax.B1 = fmaf(S1, fmaf(S1, p[7], p[4]), p[2]);
-    ax.C0 = fmaf(S0, p[8], p[5]);
-    ax.C1 = fmaf(S1, p[8], p[5]);
-    ax.c9 = p[9];
-    ax.lin = c0 + a * s0 + b * t0;
-    ax.da = 32 * a;
-    ax.db = 32 * b;
-}
 // q & 1: column variant, q >> 1: row variant (T = T0 or T0 + 1).  Returns the position in 2^-22 px.
 template <int Q>
 __device__ __forceinline__ int fast_axis_eval(const FastAxis& ax, float T0, float T1) {
@@ -133,13 +136,14 @@ __device__ __forceinline__ float fast_frac(int xf) {
 // ------------------------------------------------------------------------------------------ kernel
 template <bool COADD>
 __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
-    resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, float t_exp, float flat_min, int sat_adu,
-                         float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
+    resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, FrameArgs f, int W, int H, float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
                          CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     FastSmem& sm = *reinterpret_cast<FastSmem*>(smem_raw);
     const int tid = threadIdx.x;
     const int n_tiles = *pb.n_tiles;
+    const float t_exp = f.t_exp, flat_min = f.flat_min;
+    const int sat_adu = f.sat_adu;
 
     if (tid == 0) {
         for (int i = 0; i < RF_STAGES; ++i) {
@@ -150,14 +154,29 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
     }
     __syncthreads();
 
-    if (tid >= RF_CONSUMERS) {
+    if (tid >= RF_GROUPS * RF_CONSUMERS) {
         // ================================================================ producer warp
-        const int lane = tid - RF_CONSUMERS;
-        int issued = 0;
-        for (int t = blockIdx.x;; t += gridDim.x) {
+        const int lane = tid - RF_GROUPS * RF_CONSUMERS;
+        int issued = 0, sentinels = 0;
+        // software pipeline: the record and output offset of the NEXT tile are in flight while the current one is
+        // handled (one producer serves RF_GROUPS groups, so its own load latency must stay off the critical path)
+        float4 rv_n = make_float4(0.f, 0.f, 0.f, 0.f);
+        long long off_n = 0;
+        int t_n = blockIdx.x;
+        if (t_n < n_tiles) {
+            if (lane < 10) rv_n = __ldg(reinterpret_cast<const float4*>(pb.frec + t_n) + lane);
+            if (lane == 0) off_n = tile_out_offset(pb, t_n);
+        }
+        for (;;) {
+            const int t = t_n;
             const bool last = t >= n_tiles;
-            float4 rv = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (!last && lane < 10) rv = __ldg(reinterpret_cast<const float4*>(pb.frec + t) + lane);
+            const float4 rv = rv_n;
+            const long long off_c = off_n;
+            t_n = t + gridDim.x;
+            if (t_n < n_tiles) {
+                if (lane < 10) rv_n = __ldg(reinterpret_cast<const float4*>(pb.frec + t_n) + lane);
+                if (lane == 0) off_n = tile_out_offset(pb, t_n);
+            }
             // lane 0 holds cls, mask_slot, gx0, gy0; lane 1 holds wclass, bh, kofs, X0
             const int cls = last ? -1 : __shfl_sync(0xffffffffu, __float_as_int(rv.x), 0);
             if (cls == 0) continue;                         // empty, or left to the general kernel
@@ -166,16 +185,59 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
             if (issued >= RF_STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / RF_STAGES - 1) & 1));
             FastDesc& d = sm.desc[slot];
             if (last) {
+                // end of work: one sentinel per consumer group (consecutive tiles go to distinct groups)
                 if (lane == 0) {
                     d.r.cls = -1;
                     mbar_arrive(&sm.full[slot]);
                 }
-                break;
+                ++issued;
+                if (++sentinels == RF_GROUPS) break;
+                continue;
             }
             const int mask_slot = __shfl_sync(0xffffffffu, __float_as_int(rv.y), 0);
             const int gx0 = __shfl_sync(0xffffffffu, __float_as_int(rv.z), 0), gy0 = __shfl_sync(0xffffffffu, __float_as_int(rv.w), 0);
             const int wclass = __shfl_sync(0xffffffffu, __float_as_int(rv.x), 1), bh = __shfl_sync(0xffffffffu, __float_as_int(rv.y), 1);
+            unsigned tx_bytes = 0;
+            {
+                // one elected thread issues the four bulk-tensor copies (one box per array) as early as possible; the
+                // arrive.expect_tx that completes the phase follows once the descriptor is written
+                const int wc = wclass & 15, hc = wclass >> 4;
+                const int boxw = 40 + 8 * wc, boxh = 48 + 8 * hc;
+                tx_bytes = (unsigned)(boxh * boxw * 14);
+#ifdef RF_ABL_NOTMA
+                tx_bytes = 0;
+                if (false) {
+#else
+                if (lane == 0) {
+#endif
+                    const CUtensorMap* mp = &maps.m[hc][wc][0];
+                    FastStage& sg = sm.stage[slot];
+                    tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[slot]);
+                    tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[slot]);
+                    tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[slot]);
+                    tma_load_2d(sg.flat, mp + 3, gx0, gy0, &sm.full[slot]);
+                }
+            }
             if (lane < 10) reinterpret_cast<float4*>(&d.r)[lane] = rv;
+            __syncwarp();
+            {
+                // Horner coefficients in T for pixel column u = lane: the S-dependent part of the tile polynomial,
+                // shared by every consumer thread of that column
+                const float S = (float)(2 * lane - 31) * 0.03125f;
+                const float* px = d.r.px;
+                const float* py = d.r.py;
+                float4 t0, t1;
+                t0.x = fmaf(S, fmaf(S, fmaf(S, px[6], px[3]), px[1]), px[0]);
+                t0.y = fmaf(S, fmaf(S, px[7], px[4]), px[2]);
+                t0.z = fmaf(S, px[8], px[5]);
+                t0.w = fmaf(S, fmaf(S, fmaf(S, py[6], py[3]), py[1]), py[0]);
+                t1.x = fmaf(S, fmaf(S, py[7], py[4]), py[2]);
+                t1.y = fmaf(S, py[8], py[5]);
+                t1.z = px[9];
+                t1.w = py[9];
+                d.tab[lane][0] = t0;
+                d.tab[lane][1] = t1;
+            }
             if (cls == TC_BORDER) {
                 unsigned mk = pb.masks[(size_t)mask_slot * 32 + lane];
                 int c = __popc(mk), inc = c;
@@ -187,7 +249,7 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
                 d.pref[lane] = inc - c;
             }
             if (lane == 0) {
-                d.off = tile_out_offset(pb, t);
+                d.off = off_c;
                 if (COADD) {
                     long long tile = pb.tile_id[t];
                     long long key = tile >> ca.shift, lo = 0, hi = ca.n_tiles - 1, pos = -1;
@@ -201,55 +263,52 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
                 }
             }
             __syncwarp();
-            if (lane == 0) {
-                // one elected thread issues the four bulk-tensor copies (one box per array)
-                const int wc = wclass & 15, hc = wclass >> 4;
-                const int boxw = 40 + 8 * wc, boxh = 48 + 8 * hc;
-                mbar_arrive_expect_tx(&sm.full[slot], (unsigned)(boxh * boxw * 14));
-                const CUtensorMap* mp = &maps.m[hc][wc][0];
-                FastStage& sg = sm.stage[slot];
-                tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[slot]);
-                tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[slot]);
-                tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[slot]);
-                tma_load_2d(sg.flat, mp + 3, gx0, gy0, &sm.full[slot]);
-            }
+            if (lane == 0) mbar_arrive_expect_tx(&sm.full[slot], tx_bytes);   // releases the descriptor to the consumers
             ++issued;
         }
         return;
     }
 
     // ==================================================================== consumer warps
+    const int group = tid / RF_CONSUMERS;
+    const int gt = tid - group * RF_CONSUMERS;     // thread index within the group
     const int lane = tid & 31;
-    const int ul = (int)compact_even_bits((unsigned)tid), vl = (int)compact_even_bits((unsigned)tid >> 1);
+    const int ul = (int)compact_even_bits((unsigned)gt), vl = (int)compact_even_bits((unsigned)gt >> 1);
     const int s0 = 2 * ul - 31, t0 = 2 * vl - 31;
-    const float S0 = (float)s0 * 0.03125f, S1 = S0 + 1.0f, T0 = (float)t0 * 0.03125f, T1 = T0 + 1.0f;
+    const float T0 = (float)t0 * 0.03125f, T1 = T0 + 1.0f;
     const unsigned fmin_bits = __float_as_uint(flat_min), frange = 0x7f800000u - fmin_bits;
     const float sat_f = (float)sat_adu;
 
-    for (int it = 0;; ++it) {
+    for (int it = group;; it += RF_GROUPS) {
         const int slot = it % RF_STAGES;
         mbar_wait(&sm.full[slot], (unsigned)((it / RF_STAGES) & 1));
         const FastDesc& d = sm.desc[slot];
         const int cls = d.r.cls;
         if (cls < 0) break;
+#ifdef RF_ABL_NOCOMPUTE
+        mbar_arrive(&sm.empty[slot]);
+        continue;
+#endif
         FastStage& sg = sm.stage[slot];
         float* cal = sg.bias;
         const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
-        const int bw4 = boxw >> 2, n4 = d.r.bh * bw4;
-        const unsigned M = (1048576u + bw4 - 1) / bw4;   // exact division by bw4 for v < 2^14
-        // ---- A2: calibrate the staged box once.  The stage is dense (item v <-> float4 v): four independent items
+        const int bw4 = boxw >> 2, c4_lo = d.r.cols & 255, nb4 = d.r.cols >> 8, n4 = d.r.bh * nb4;
+        const unsigned M = (1048576u + nb4 - 1) / nb4;   // exact division by nb4 for v < 2^14
+        // ---- A2: calibrate the staged box once, only the float4 columns that hold taps.  Four independent items
         //      per thread are read and calibrated in registers; after a barrier (all reads done) they overwrite the
         //      stage with a pitch of 8 or 24 mod 32 floats, which makes the gather free of bank conflicts.
         float4 o4[4];
         int bad = 0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const int v = tid + RF_CONSUMERS * j;
+            const int v = gt + RF_CONSUMERS * j;
             if (v < n4) {
-                const uint2 rw = reinterpret_cast<const uint2*>(sg.raw)[v];
-                const float4 b = reinterpret_cast<const float4*>(sg.bias)[v];
-                const float4 dk = reinterpret_cast<const float4*>(sg.dark)[v];
-                const float4 fl = reinterpret_cast<const float4*>(sg.flat)[v];
+                const int row = (int)(((unsigned)v * M) >> 20);
+                const int i = row * bw4 + c4_lo + (v - row * nb4);
+                const uint2 rw = reinterpret_cast<const uint2*>(sg.raw)[i];
+                const float4 b = reinterpret_cast<const float4*>(sg.bias)[i];
+                const float4 dk = reinterpret_cast<const float4*>(sg.dark)[i];
+                const float4 fl = reinterpret_cast<const float4*>(sg.flat)[i];
                 o4[j].x = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
                 o4[j].y = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
                 o4[j].z = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
@@ -257,27 +316,33 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
                 bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
             }
         }
-        const int any_bad = consumers_sync_or(bad);
+        const int any_bad = consumers_sync_or(group, bad);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const int v = tid + RF_CONSUMERS * j;
+            const int v = gt + RF_CONSUMERS * j;
             if (v < n4) {
                 const int row = (int)(((unsigned)v * M) >> 20);
-                *reinterpret_cast<float4*>(cal + row * pitch + 4 * (v - row * bw4)) = o4[j];
+                *reinterpret_cast<float4*>(cal + row * pitch + 4 * (c4_lo + v - row * nb4)) = o4[j];
             }
         }
-        consumers_sync();
+        consumers_sync(group);
 
         // ---- A3/A4: tile polynomial -> source position; A5: bilinear
         FastAxis ax, ay;
-        fast_axis_setup(d.r.px, d.r.c0x, d.r.ax, d.r.bx, s0, t0, S0, S1, ax);
-        fast_axis_setup(d.r.py, d.r.c0y, d.r.ay, d.r.by, s0, t0, S0, S1, ay);
+        {
+            const float4 p0 = d.tab[ul][0], p1 = d.tab[ul][1], q0 = d.tab[ul + 16][0], q1 = d.tab[ul + 16][1];
+            ax.A0 = p0.x; ax.B0 = p0.y; ax.C0 = p0.z; ax.A1 = q0.x; ax.B1 = q0.y; ax.C1 = q0.z; ax.c9 = p1.z;
+            ay.A0 = p0.w; ay.B0 = p1.x; ay.C0 = p1.y; ay.A1 = q0.w; ay.B1 = q1.x; ay.C1 = q1.y; ay.c9 = p1.w;
+            const int axi = d.r.ax, bxi = d.r.bx, ayi = d.r.ay, byi = d.r.by;
+            ax.lin = d.r.c0x + axi * s0 + bxi * t0; ax.da = 32 * axi; ax.db = 32 * bxi;
+            ay.lin = d.r.c0y + ayi * s0 + byi * t0; ay.da = 32 * ayi; ay.db = 32 * byi;
+        }
         const float* cb = cal + d.r.kofs;
         const long long off = d.off;
 
         if (!COADD && cls == TC_INSIDE && !any_bad && off + ARGUS_TILE_PIX <= out_cap) {
-            float* vp = value_out + off + tid;
-            float* wp = weight_out + off + tid;
+            float* vp = value_out + off + gt;
+            float* wp = weight_out + off + gt;
 #define RF_HOT(Q)                                                                            \
     {                                                                                        \
         const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);    \
@@ -295,7 +360,7 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
             const long long cslot = COADD ? d.cslot : 0;
 #define RF_GEN(Q)                                                                                          \
     {                                                                                                      \
-        const int m = tid + 256 * Q;                                                                       \
+        const int m = gt + 256 * Q;                                                                        \
         bool member = true;                                                                                \
         long long pos = m;                                                                                 \
         if (cls != TC_INSIDE) {                                                                            \
