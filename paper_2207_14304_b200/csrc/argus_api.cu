@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/argus.h"
+#include "plan_block.cuh"
 #include "resample.cuh"
 #include "resample_fast.cuh"
 
@@ -72,40 +73,42 @@ extern "C" const char* argus_strerror(int s) {
 extern "C" int argus_version(void) { return ARGUS_VERSION_NUM; }
 
 // ---------------------------------------------------------------------------------------- context
-static void lsq_pinv(double* pinv /*[10][25]*/) {
-    // design matrix of the 5x5 node grid S,T in {-1,-.5,0,.5,1}; pinv = (A^T A)^-1 A^T
-    double A[25][10];
+// Pseudo-inverse (A^T A)^-1 A^T of the design matrix of the 5x5 node grid S, T in {-1,-.5,0,.5,1} for the
+// total-degree-`deg` basis U^i V^j ordered by degree, then by j: nc = (deg+1)(deg+2)/2 rows of 25.
+static void lsq_pinv(int deg, double* pinv) {
+    const int nc = (deg + 1) * (deg + 2) / 2;
+    double A[25][15];
     for (int n = 0; n < 25; ++n) {
         double S = -1.0 + 0.5 * (n % 5), T = -1.0 + 0.5 * (n / 5);
-        double m[10] = {1.0, S, T, S * S, S * T, T * T, S * S * S, S * S * T, S * T * T, T * T * T};
-        for (int i = 0; i < 10; ++i) A[n][i] = m[i];
+        for (int d = 0; d <= deg; ++d)
+            for (int j = 0; j <= d; ++j) A[n][d * (d + 1) / 2 + j] = pow(S, d - j) * pow(T, j);
     }
-    double G[10][20];
-    for (int i = 0; i < 10; ++i)
-        for (int j = 0; j < 10; ++j) {
+    double G[15][30];
+    for (int i = 0; i < nc; ++i)
+        for (int j = 0; j < nc; ++j) {
             double s = 0;
             for (int n = 0; n < 25; ++n) s += A[n][i] * A[n][j];
             G[i][j] = s;
-            G[i][10 + j] = (i == j) ? 1.0 : 0.0;
+            G[i][nc + j] = (i == j) ? 1.0 : 0.0;
         }
-    for (int c = 0; c < 10; ++c) {   // Gauss-Jordan with partial pivoting
+    for (int c = 0; c < nc; ++c) {   // Gauss-Jordan with partial pivoting
         int piv = c;
-        for (int r = c + 1; r < 10; ++r)
+        for (int r = c + 1; r < nc; ++r)
             if (fabs(G[r][c]) > fabs(G[piv][c])) piv = r;
         if (piv != c)
-            for (int j = 0; j < 20; ++j) { double t = G[c][j]; G[c][j] = G[piv][j]; G[piv][j] = t; }
+            for (int j = 0; j < 2 * nc; ++j) { double t = G[c][j]; G[c][j] = G[piv][j]; G[piv][j] = t; }
         double d = 1.0 / G[c][c];
-        for (int j = 0; j < 20; ++j) G[c][j] *= d;
-        for (int r = 0; r < 10; ++r)
+        for (int j = 0; j < 2 * nc; ++j) G[c][j] *= d;
+        for (int r = 0; r < nc; ++r)
             if (r != c) {
                 double fct = G[r][c];
-                for (int j = 0; j < 20; ++j) G[r][j] -= fct * G[c][j];
+                for (int j = 0; j < 2 * nc; ++j) G[r][j] -= fct * G[c][j];
             }
     }
-    for (int i = 0; i < 10; ++i)
+    for (int i = 0; i < nc; ++i)
         for (int n = 0; n < 25; ++n) {
             double s = 0;
-            for (int j = 0; j < 10; ++j) s += G[i][10 + j] * A[n][j];
+            for (int j = 0; j < nc; ++j) s += G[i][nc + j] * A[n][j];
             pinv[i * 25 + n] = s;
         }
 }
@@ -130,7 +133,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
@@ -150,6 +153,12 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     o_fr = o;    o = align_up(o + sizeof(FastRec) * (size_t)pb.max_tiles, 256);
     o_sc = o;    o = align_up(o + sizeof(int), 256);
     o_sl = o;    o = align_up(o + sizeof(int) * pb.max_hard, 256);
+    o_bid = o;   o = align_up(o + sizeof(long long) * (pb.max_tiles / 64 + 1), 256);
+    o_nb = o;    o = align_up(o + sizeof(int), 256);
+    o_fc = o;    o = align_up(o + sizeof(int), 256);
+    o_fl = o;    o = align_up(o + sizeof(int) * (size_t)pb.max_tiles, 256);
+    o_tk = o;    o = align_up(o + sizeof(unsigned), 256);
+    o_p4 = o;    o = align_up(o + sizeof(double) * 375, 256);
     e = cudaMalloc(&c->d_block, o);
     if (e == cudaSuccess) e = cudaMemset(c->d_block, 0, o);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
@@ -178,9 +187,17 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.frec = (FastRec*)(b + o_fr);
     pb.slow_count = (int*)(b + o_sc);
     pb.slow_list = (int*)(b + o_sl);
-    double pinv[250];
-    lsq_pinv(pinv);
+    pb.block_id = (long long*)(b + o_bid);
+    pb.n_blocks = (int*)(b + o_nb);
+    pb.fb_count = (int*)(b + o_fc);
+    pb.fb_list = (int*)(b + o_fl);
+    pb.ticket = (unsigned*)(b + o_tk);
+    pb.pinv4 = (double*)(b + o_p4);
+    double pinv[250], pinv4[375];
+    lsq_pinv(3, pinv);
+    lsq_pinv(4, pinv4);
     e = cudaMemcpy(pb.pinv, pinv, sizeof(pinv), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(pb.pinv4, pinv4, sizeof(pinv4), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         cudaFree(c->d_block);
         cudaFreeHost(c->h_stats);
@@ -322,10 +339,14 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     if (rc) return rc;
     if (same_key(c, w, W, H, nside)) return ARGUS_OK;
     c->plan_valid = false;
-    int64_t nside_t = nside >> ARGUS_TILE_LOG2;
+    // Hierarchical plan (plan_block.cuh) whenever a block of 8x8 tiles exists at this nside; the flat plan (one
+    // scan slot and one fit per tile) serves nside < 256.
+    const bool blocks = dw.k >= ARGUS_TILE_LOG2 + BLOCK_TILES_LOG2;
+    int64_t nside_t = nside >> ARGUS_TILE_LOG2;                      // tile-level nside
+    int64_t nside_s = blocks ? (nside_t >> BLOCK_TILES_LOG2) : nside_t;   // resolution of the scan slots
     // coarse resolution: cells comparable to the search cone, list passed by value
     int64_t nside_c = 1;
-    while (nside_c < nside_t && (double)nside_c < 2.0 / rho) nside_c <<= 1;
+    while (nside_c < nside_s && (double)nside_c < 2.0 / rho) nside_c <<= 1;
     std::vector<long long> cells;
     for (;;) {
         cells.clear();
@@ -337,23 +358,39 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     CoarseList cl;
     memset(&cl, 0, sizeof(cl));
     cl.n = (int)cells.size();
-    cl.ratio_log2 = ilog2(nside_t / nside_c);
+    cl.ratio_log2 = ilog2(nside_s / nside_c);
     for (int i = 0; i < cl.n; ++i) cl.cell[i] = cells[i];
     long long n_slots = (long long)cl.n << (2 * cl.ratio_log2);
     if (cl.ratio_log2 > 12 || n_slots > c->pb.max_slots) return ARGUS_ERR_CAPACITY;
     if (n_slots == 0) n_slots = 1;
-    double rad_px = 1.05 * dw.tile_ang / s_rad + 2.0;
     int nblk = (int)((n_slots + 255) / 256);
-    plan_scan_kernel<<<nblk, 256, 0, st>>>(dw, cl, c->pb, rad_px);
-    plan_compact_kernel<<<nblk, 256, 0, st>>>(cl, c->pb);
-    plan_fit_kernel<<<c->sm_count * 4, 32 * FIT_WARPS, 0, st>>>(dw, c->pb);
+    long long tile_bound;
+    if (blocks) {
+        double block_ang = 8.0 * dw.tile_ang;
+        double rad_px = 1.05 * block_ang / s_rad + 2.0;
+        plan_bscan_kernel<<<nblk, 256, 0, st>>>(dw, cl, c->pb, rad_px, block_ang);
+        int nb_bound = (int)(n_slots < c->pb.max_tiles / 64 ? n_slots : c->pb.max_tiles / 64);
+        int g = (nb_bound + BFIT_WARPS - 1) / BFIT_WARPS;
+        if (g > c->sm_count * 8) g = c->sm_count * 8;
+        plan_blockfit_kernel<<<g < 1 ? 1 : g, 32 * BFIT_WARPS, 0, st>>>(dw, c->pb);
+        plan_fit_kernel<<<c->sm_count * 2, 32 * FIT_WARPS, 0, st>>>(dw, c->pb, 1);
+        tile_bound = n_slots * 64;
+        c->n_launches += 3;
+    } else {
+        double rad_px = 1.05 * dw.tile_ang / s_rad + 2.0;
+        plan_scan_kernel<<<nblk, 256, 0, st>>>(dw, cl, c->pb, rad_px);
+        plan_compact_kernel<<<nblk, 256, 0, st>>>(cl, c->pb);
+        plan_fit_kernel<<<c->sm_count * 4, 32 * FIT_WARPS, 0, st>>>(dw, c->pb, 0);
+        tile_bound = n_slots;
+        c->n_launches += 3;
+    }
     plan_members_kernel<<<c->sm_count * 4, 256, 0, st>>>(dw, c->pb);
     {
-        long long bound = n_slots < c->pb.max_tiles ? n_slots : c->pb.max_tiles;
+        long long bound = tile_bound < c->pb.max_tiles ? tile_bound : c->pb.max_tiles;
         plan_offsets_local_kernel<<<(int)((bound + 1023) / 1024), 1024, 0, st>>>(c->pb);
         plan_offsets_final_kernel<<<1, 1024, 0, st>>>(c->pb, out_cap);
     }
-    c->n_launches += 6;
+    c->n_launches += 3;
     CUDA_TRY(c, cudaGetLastError());
     c->dw = dw;
     c->key_wcs = *w;

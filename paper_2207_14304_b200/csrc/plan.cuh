@@ -38,6 +38,12 @@ struct PlanBuffers {
     FastRec* frec;              // [max_tiles] records of the TMA-staged bilinear kernel
     int* slow_count;            // device scalar
     int* slow_list;             // [max_hard] tiles the fast kernel leaves to the general kernel
+    long long* block_id;        // [max_tiles/64] candidate blocks (8x8 tiles), ascending nested ids at block level
+    int* n_blocks;              // device scalar
+    int* fb_count;              // device scalar
+    int* fb_list;               // [max_tiles] tiles of blocks that need one fit per tile
+    unsigned* ticket;           // device scalar: CTA arrival counter of plan_bscan_kernel
+    double* pinv4;              // [15][25] pseudo-inverse of the quartic design matrix on the 5x5 node grid
     int max_slots, max_tiles, max_hard;
 };
 
@@ -159,14 +165,98 @@ __device__ inline void slow_push(const PlanBuffers& pb, int t) {
     else atomicOr(&pb.stats->overflow, 2);
 }
 
+// Everything a kernel needs to know about one tile, written by ONE thread from the tile's cubic (c[0..9] x,
+// c[10..19] y, in S, T = local offsets / 16 px) and the extent of its source positions.  cls on entry:
+// TC_INSIDE / TC_BORDER / TC_EXACT / TC_EMPTY.
+__device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, int zone, int cls, const double* c,
+                                 double xmin, double xmax, double ymin, double ymax, double mg) {
+    TileRec r;
+    r.tile = tile; r.reserved = 0; r.count = 0; r.mask_slot = -1;
+    r.zone = zone;
+    r.bx0 = r.bx1 = r.by0 = r.by1 = 0; r.X0 = r.Y0 = 0; r.ax = r.bx = r.ay = r.by = 0;
+    r.pad[0] = r.pad[1] = 0;
+    for (int i = 0; i < 10; ++i) { r.cx[i] = 0.f; r.cy[i] = 0.f; }
+    if (cls == TC_INSIDE || cls == TC_BORDER) {
+        // split: x = X0 + (a*s + b*t) 2^-12 + lo(S,T); s = 32 S, so c1 S = (c1/32) s
+#pragma unroll
+        for (int axis = 0; axis < 2; ++axis) {
+            const double* ca = c + 10 * axis;
+            double base = floor(ca[0]);
+            int a = (int)rint(ca[1] * (4096.0 / 32.0)), b = (int)rint(ca[2] * (4096.0 / 32.0));
+            float* out = axis ? r.cy : r.cx;
+            out[0] = (float)(ca[0] - base);
+            out[1] = (float)(ca[1] - a * (32.0 / 4096.0));
+            out[2] = (float)(ca[2] - b * (32.0 / 4096.0));
+#pragma unroll
+            for (int i = 3; i < 10; ++i) out[i] = (float)ca[i];
+            if (axis) { r.Y0 = (int)base; r.ay = a; r.by = b; } else { r.X0 = (int)base; r.ax = a; r.bx = b; }
+        }
+        r.bx0 = (int)floor(xmin - mg); r.bx1 = (int)floor(xmax + mg);
+        r.by0 = (int)floor(ymin - mg); r.by1 = (int)floor(ymax + mg);
+        if (cls == TC_INSIDE) r.count = ARGUS_TILE_PIX;
+    }
+    if (cls == TC_BORDER || cls == TC_EXACT) {
+        int slot = atomicAdd(pb.hard_count, 1);
+        if (slot < pb.max_hard) {
+            pb.hard_list[slot] = t;
+            r.mask_slot = slot;
+        } else {
+            atomicOr(&pb.stats->overflow, 2);
+            cls = TC_EMPTY;
+        }
+    }
+    r.cls = cls;
+    pb.rec[t] = r;
+    pb.tile_id[t] = tile;
+    pb.tile_count[t] = r.count;
+    pb.tile_cls[t] = (unsigned char)cls;
+    // record of the fast (TMA-staged bilinear) kernel
+    FastRec f;
+    memset(&f, 0, sizeof(f));
+    if (cls == TC_INSIDE || cls == TC_BORDER) {
+        bool poly_ok = true;
+#pragma unroll
+        for (int axis = 0; axis < 2; ++axis) {
+            const double* ca = c + 10 * axis;
+            int base = (axis ? r.by0 : r.bx0) - 8;
+            double c0l = ca[0] - (double)base;
+            int c0f = (int)rint(c0l * 4194304.0);
+            int af = (int)rint(ca[1] * 131072.0), bf = (int)rint(ca[2] * 131072.0);   // c/32 * 2^22
+            float* pp = axis ? f.py : f.px;
+            pp[0] = (float)(12582912.0 + (c0l * 4194304.0 - (double)c0f));
+            pp[1] = (float)((ca[1] * 131072.0 - (double)af) * 32.0);
+            pp[2] = (float)((ca[2] * 131072.0 - (double)bf) * 32.0);
+            double mag = fabs((double)pp[1]) + fabs((double)pp[2]);
+#pragma unroll
+            for (int i = 3; i < 10; ++i) { pp[i] = (float)(ca[i] * 4194304.0); mag += fabs((double)pp[i]); }
+            if (!(mag < 0.9 * 4194304.0) || !(fabs(c0l) < 400.0)) poly_ok = false;
+            if (axis) { f.Y0 = base; f.c0y = c0f - FAST_MAGIC_I; f.ay = af; f.by = bf; }
+            else { f.X0 = base; f.c0x = c0f - FAST_MAGIC_I; f.ax = af; f.bx = bf; }
+        }
+        f.mask_slot = r.mask_slot;
+        f.poly_ok = poly_ok ? 1 : 0;
+        if (cls == TC_INSIDE) {
+            if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) f.cls = TC_INSIDE;
+            else slow_push(pb, t);
+        }   // TC_BORDER: plan_members_kernel finalises the box and decides
+        double* dc = pb.dcoef + (size_t)t * 20;
+#pragma unroll
+        for (int i = 0; i < 20; ++i) dc[i] = c[i];
+    } else if (cls == TC_EXACT) {
+        slow_push(pb, t);
+    }
+    pb.frec[t] = f;
+}
+
 #define FIT_WARPS 8
-__global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, PlanBuffers pb) {
+__global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, PlanBuffers pb, int use_list) {
     __shared__ double s_pinv[250];
     __shared__ double s_coef[FIT_WARPS][20];
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     for (int i = tid; i < 250; i += blockDim.x) s_pinv[i] = pb.pinv[i];
     __syncthreads();
-    int n_tiles = *pb.n_tiles;
+    // use_list: only the tiles plan_blockfit_kernel could not derive from a block fit
+    const int n_items = use_list ? *pb.fb_count : *pb.n_tiles;
     long long ns = 1ll << w.k;
     // node coordinates: lanes 0..24 the 5x5 fit grid, lanes 25..31 extra check points
     double S, T;
@@ -179,27 +269,23 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
         S = cs[lane - 25];
         T = ct[lane - 25];
     }
-    for (int t = blockIdx.x * FIT_WARPS + wid; t < n_tiles; t += gridDim.x * FIT_WARPS) {
+    for (int it = blockIdx.x * FIT_WARPS + wid; it < n_items; it += gridDim.x * FIT_WARPS) {
+        const int t = use_list ? pb.fb_list[it] : it;
         long long tile = pb.tile_id[t];
         int face, tx, ty;
         nest_to_xyf(tile, w.k - ARGUS_TILE_LOG2, face, tx, ty);
         int ix0 = tx * 32, iy0 = ty * 32;
         long long jr_max = (long long)face_ring_offset(face) * ns - ix0 - iy0 - 1, jr_min = jr_max - 62;
         int z0 = ring_zone(jr_min, ns), z1 = ring_zone(jr_max, ns);
-        TileRec r;
-        r.tile = tile; r.reserved = 0; r.count = 0; r.mask_slot = -1;
-        r.zone = (z0 == z1) ? z0 : -1;
-        r.bx0 = r.bx1 = r.by0 = r.by1 = 0; r.X0 = r.Y0 = 0; r.ax = r.bx = r.ay = r.by = 0;
-        r.pad[0] = r.pad[1] = 0;
-        for (int i = 0; i < 10; ++i) { r.cx[i] = 0.f; r.cy[i] = 0.f; }
+        double xmin = 0, xmax = 0, ymin = 0, ymax = 0;
         int cls = TC_EXACT;
         if (z0 == z1) {
             double v[3], x, y;
             hp_vec(face, ix0 + 15.5 + 16.0 * S, iy0 + 15.5 + 16.0 * T, w.nside, z0, v);
             double cosc = vec_to_xy(w, v, x, y);
             bool node = lane < 25;
-            double xmin = warp_min(node ? x : 1e300), xmax = warp_max(node ? x : -1e300);
-            double ymin = warp_min(node ? y : 1e300), ymax = warp_max(node ? y : -1e300);
+            xmin = warp_min(node ? x : 1e300); xmax = warp_max(node ? x : -1e300);
+            ymin = warp_min(node ? y : 1e300); ymax = warp_max(node ? y : -1e300);
             double cmin = warp_min(cosc), cmax = warp_max(cosc);
             double xc = __shfl_sync(0xffffffffu, x, 12), yc = __shfl_sync(0xffffffffu, y, 12);
             // least squares: lanes 0..9 -> x coefficients, lanes 10..19 -> y coefficients
@@ -211,7 +297,7 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
             }
             if (lane == 0) acc += xc;
             if (lane == 10) acc += yc;
-            if (lane < 20) { s_coef[wid][lane] = acc; pb.dcoef[(size_t)t * 20 + lane] = acc; }
+            if (lane < 20) s_coef[wid][lane] = acc;
             __syncwarp();
             double m[10];
             cubic_basis(S, T, m);
@@ -237,73 +323,8 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
             } else if (finite_ok && cone_out) {
                 cls = TC_EMPTY;
             }
-            if (cls == TC_INSIDE || cls == TC_BORDER) {
-                // split: x = X0 + (a*s + b*t) 2^-12 + lo(S,T); s = 32 S, so c1 S = (c1/32) s
-                const double* cf = s_coef[wid];
-                for (int axis = 0; axis < 2; ++axis) {
-                    const double* c = cf + 10 * axis;
-                    double base = floor(c[0]);
-                    int a = (int)rint(c[1] * (4096.0 / 32.0)), b = (int)rint(c[2] * (4096.0 / 32.0));
-                    float* out = axis ? r.cy : r.cx;
-                    out[0] = (float)(c[0] - base);
-                    out[1] = (float)(c[1] - a * (32.0 / 4096.0));
-                    out[2] = (float)(c[2] - b * (32.0 / 4096.0));
-                    for (int i = 3; i < 10; ++i) out[i] = (float)c[i];
-                    if (axis) { r.Y0 = (int)base; r.ay = a; r.by = b; } else { r.X0 = (int)base; r.ax = a; r.bx = b; }
-                }
-                r.bx0 = (int)floor(xmin - mg); r.bx1 = (int)floor(xmax + mg);
-                r.by0 = (int)floor(ymin - mg); r.by1 = (int)floor(ymax + mg);
-                if (cls == TC_INSIDE) r.count = ARGUS_TILE_PIX;
-            }
         }
-        if (lane == 0) {
-            if (cls == TC_BORDER || cls == TC_EXACT) {
-                int slot = atomicAdd(pb.hard_count, 1);
-                if (slot < pb.max_hard) {
-                    pb.hard_list[slot] = t;
-                    r.mask_slot = slot;
-                } else {
-                    atomicOr(&pb.stats->overflow, 2);
-                    cls = TC_EMPTY;
-                }
-            }
-            r.cls = cls;
-            pb.rec[t] = r;
-            pb.tile_count[t] = r.count;
-            pb.tile_cls[t] = (unsigned char)cls;
-            // record of the fast (TMA-staged bilinear) kernel
-            FastRec f;
-            memset(&f, 0, sizeof(f));
-            bool poly_ok = false;
-            if (cls == TC_INSIDE || cls == TC_BORDER) {
-                poly_ok = true;
-                for (int axis = 0; axis < 2; ++axis) {
-                    const double* c = s_coef[wid] + 10 * axis;
-                    int base = (axis ? r.by0 : r.bx0) - 8;
-                    double c0l = c[0] - (double)base;
-                    int c0f = (int)rint(c0l * 4194304.0);
-                    int af = (int)rint(c[1] * 131072.0), bf = (int)rint(c[2] * 131072.0);   // c/32 * 2^22
-                    float* pp = axis ? f.py : f.px;
-                    pp[0] = (float)(12582912.0 + (c0l * 4194304.0 - (double)c0f));
-                    pp[1] = (float)((c[1] * 131072.0 - (double)af) * 32.0);
-                    pp[2] = (float)((c[2] * 131072.0 - (double)bf) * 32.0);
-                    double mag = fabs((double)pp[1]) + fabs((double)pp[2]);
-                    for (int i = 3; i < 10; ++i) { pp[i] = (float)(c[i] * 4194304.0); mag += fabs((double)pp[i]); }
-                    if (!(mag < 0.9 * 4194304.0) || !(fabs(c0l) < 400.0)) poly_ok = false;
-                    if (axis) { f.Y0 = base; f.c0y = c0f - FAST_MAGIC_I; f.ay = af; f.by = bf; }
-                    else { f.X0 = base; f.c0x = c0f - FAST_MAGIC_I; f.ax = af; f.bx = bf; }
-                }
-                f.mask_slot = r.mask_slot;
-                f.poly_ok = poly_ok ? 1 : 0;
-                if (cls == TC_INSIDE) {
-                    if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) f.cls = TC_INSIDE;
-                    else slow_push(pb, t);
-                }   // TC_BORDER: plan_members_kernel finalises the box and decides
-            } else if (cls == TC_EXACT) {
-                slow_push(pb, t);
-            }
-            pb.frec[t] = f;
-        }
+        if (lane == 0) emit_tile(pb, t, tile, (z0 == z1) ? z0 : -1, cls, s_coef[wid], xmin, xmax, ymin, ymax, PLAN_NODE_MARGIN);
         __syncwarp();
     }
 }

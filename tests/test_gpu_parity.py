@@ -165,6 +165,24 @@ def test_small_nside_coarse_wcs(argus, ctx):
     assert_values_match(v, w, vo, wo, fl, "nside 2^10")
 
 
+def test_tiny_nside_flat_plan(argus, ctx):
+    """nside < 256 has no 8x8-tile blocks: the flat plan (one fit per tile) must give the same parity."""
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    nside = 1 << 7
+    hp = math.degrees(math.sqrt(4 * math.pi / (12.0 * nside * nside)))
+    W = H = 128
+    wcs = synth.make_wcs((222.0, 31.0), (63.5, 63.5), -7.0, scale_deg=hp / 1.3)
+    fr = synth.make_frame(6, W, H, 30, wcs, nside, "bilinear")
+    idx_or, dmin = oracle.footprint(wcs, W, H, nside)
+    assert dmin > 1e-9
+    n, idx = argus.argus_healpix_footprint(ctx, wcs, W, H, nside)
+    assert np.array_equal(idx.cpu().numpy(), idx_or)
+    d = upload(fr)
+    n, v, w = gpu_resample_planned(ctx, fr, d, "bilinear")
+    vo, wo, fl = oracle_reference(fr, idx_or, "bilinear")
+    assert_values_match(v, w, vo, wo, fl, "nside 2^7")
+
+
 def test_coadd_three_frames(argus, ctx):
     from gpu_util import upload
     W = H = 512
