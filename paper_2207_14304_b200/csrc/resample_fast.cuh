@@ -18,7 +18,11 @@
 #include "plan.cuh"
 #include "resample.cuh"
 
-#define RF_CONSUMERS 256                 // threads of one consumer group (one output tile at a time)
+#ifndef RF_CONSUMERS
+#define RF_CONSUMERS 256                 // threads of one consumer group (one output tile at a time): 256 or 512
+#endif
+#define RF_NQ (ARGUS_TILE_PIX / RF_CONSUMERS)   // output pixels per thread
+#define RF_NI ((FAST_CAP_PX / 4 + RF_CONSUMERS - 1) / RF_CONSUMERS)   // calibration items (float4) per thread
 #ifndef RF_GROUPS
 #define RF_GROUPS 1                      // consumer groups per CTA, tiles dealt round-robin
 #define RF_CTAS_PER_SM 2
@@ -122,12 +126,15 @@ struct FastAxis {
     int lin;                            // c0 + a*s0 + b*t0
     int da, db;                         // 32 a, 32 b: steps to u + 16 / v + 16
 };
-// q & 1: column variant, q >> 1: row variant (T = T0 or T0 + 1).  Returns the position in 2^-22 px.
+// Pixel Q of a thread is Morton index gt + RF_CONSUMERS * Q.  With 256 threads bit 8 (Q & 1) moves the pixel 16
+// columns (S + 1) and bit 9 (Q >> 1) 16 rows (T + 1); with 512 threads Q only moves rows.  Position in 2^-22 px.
 template <int Q>
 __device__ __forceinline__ int fast_axis_eval(const FastAxis& ax, float T0, float T1) {
-    const float T = (Q >> 1) ? T1 : T0;
-    const float h = fmaf(T, fmaf(T, fmaf(T, ax.c9, (Q & 1) ? ax.C1 : ax.C0), (Q & 1) ? ax.B1 : ax.B0), (Q & 1) ? ax.A1 : ax.A0);
-    return ax.lin + ((Q & 1) ? ax.da : 0) + ((Q >> 1) ? ax.db : 0) + __float_as_int(h);
+    constexpr bool CV = (RF_CONSUMERS == 256) && (Q & 1);                 // column variant
+    constexpr bool RV = (RF_CONSUMERS == 256) ? (Q >> 1) != 0 : Q != 0;   // row variant
+    const float T = RV ? T1 : T0;
+    const float h = fmaf(T, fmaf(T, fmaf(T, ax.c9, CV ? ax.C1 : ax.C0), CV ? ax.B1 : ax.B0), CV ? ax.A1 : ax.A0);
+    return ax.lin + (CV ? ax.da : 0) + (RV ? ax.db : 0) + __float_as_int(h);
 }
 __device__ __forceinline__ float fast_frac(int xf) {
     return fmaf(__uint_as_float(((unsigned)xf & 0x3fffffu) | 0x4B000000u), 2.384185791015625e-07f, -2.0f);
@@ -297,10 +304,10 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
         // ---- A2: calibrate the staged box once, only the float4 columns that hold taps.  Four independent items
         //      per thread are read and calibrated in registers; after a barrier (all reads done) they overwrite the
         //      stage with a pitch of 8 or 24 mod 32 floats, which makes the gather free of bank conflicts.
-        float4 o4[4];
+        float4 o4[RF_NI];
         int bad = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < RF_NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;
             if (v < n4) {
                 const int row = (int)(((unsigned)v * M) >> 20);
@@ -318,7 +325,7 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
         }
         const int any_bad = consumers_sync_or(group, bad);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < RF_NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;
             if (v < n4) {
                 const int row = (int)(((unsigned)v * M) >> 20);
@@ -330,9 +337,16 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
         // ---- A3/A4: tile polynomial -> source position; A5: bilinear
         FastAxis ax, ay;
         {
-            const float4 p0 = d.tab[ul][0], p1 = d.tab[ul][1], q0 = d.tab[ul + 16][0], q1 = d.tab[ul + 16][1];
-            ax.A0 = p0.x; ax.B0 = p0.y; ax.C0 = p0.z; ax.A1 = q0.x; ax.B1 = q0.y; ax.C1 = q0.z; ax.c9 = p1.z;
-            ay.A0 = p0.w; ay.B0 = p1.x; ay.C0 = p1.y; ay.A1 = q0.w; ay.B1 = q1.x; ay.C1 = q1.y; ay.c9 = p1.w;
+            const float4 p0 = d.tab[ul][0], p1 = d.tab[ul][1];
+            ax.A0 = p0.x; ax.B0 = p0.y; ax.C0 = p0.z; ax.c9 = p1.z;
+            ay.A0 = p0.w; ay.B0 = p1.x; ay.C0 = p1.y; ay.c9 = p1.w;
+            if (RF_CONSUMERS == 256) {
+                const float4 q0 = d.tab[ul + 16][0], q1 = d.tab[ul + 16][1];
+                ax.A1 = q0.x; ax.B1 = q0.y; ax.C1 = q0.z;
+                ay.A1 = q0.w; ay.B1 = q1.x; ay.C1 = q1.y;
+            } else {
+                ax.A1 = ax.B1 = ax.C1 = ay.A1 = ay.B1 = ay.C1 = 0.f;
+            }
             const int axi = d.r.ax, bxi = d.r.bx, ayi = d.r.ay, byi = d.r.by;
             ax.lin = d.r.c0x + axi * s0 + bxi * t0; ax.da = 32 * axi; ax.db = 32 * bxi;
             ay.lin = d.r.c0y + ayi * s0 + byi * t0; ay.da = 32 * ayi; ay.db = 32 * byi;
@@ -350,17 +364,20 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
         const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));      \
         const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];                \
         const float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);          \
-        vp[256 * Q] = fmaf(fy, bot - top, top);                                              \
-        wp[256 * Q] = 1.0f;                                                                  \
+        vp[RF_CONSUMERS * Q] = fmaf(fy, bot - top, top);                                              \
+        wp[RF_CONSUMERS * Q] = 1.0f;                                                                  \
     }
-            RF_HOT(0) RF_HOT(1) RF_HOT(2) RF_HOT(3)
+            RF_HOT(0) RF_HOT(1)
+#if RF_NQ == 4
+            RF_HOT(2) RF_HOT(3)
+#endif
 #undef RF_HOT
         } else {
             // masked source pixels, tiles cut by the frame border, coadd accumulation
             const long long cslot = COADD ? d.cslot : 0;
 #define RF_GEN(Q)                                                                                          \
     {                                                                                                      \
-        const int m = gt + 256 * Q;                                                                        \
+        const int m = gt + RF_CONSUMERS * Q;                                                                        \
         bool member = true;                                                                                \
         long long pos = m;                                                                                 \
         if (cls != TC_INSIDE) {                                                                            \
@@ -397,7 +414,10 @@ __global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
             }                                                                                              \
         }                                                                                                  \
     }
-            RF_GEN(0) RF_GEN(1) RF_GEN(2) RF_GEN(3)
+            RF_GEN(0) RF_GEN(1)
+#if RF_NQ == 4
+            RF_GEN(2) RF_GEN(3)
+#endif
 #undef RF_GEN
         }
         mbar_arrive(&sm.empty[slot]);   // this thread is done with the stage and its descriptor
