@@ -22,6 +22,7 @@ struct argus_ctx {
     int sm_count;
     bool plan_cache;
     bool plan_valid;
+    bool plan_full;       // the cached plan holds TileRec / FP64 coefficients for every tile (general kernel)
     argus_wcs key_wcs;
     int64_t key_W, key_H, key_nside;
     DevWcs dw;
@@ -133,7 +134,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4, o_bc2;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
@@ -159,6 +160,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     o_fl = o;    o = align_up(o + sizeof(int) * (size_t)pb.max_tiles, 256);
     o_tk = o;    o = align_up(o + sizeof(unsigned), 256);
     o_p4 = o;    o = align_up(o + sizeof(double) * 375, 256);
+    o_bc2 = o;   o = align_up(o + sizeof(double) * 32 * (size_t)(pb.max_tiles / 64 + 1), 256);
     e = cudaMalloc(&c->d_block, o);
     if (e == cudaSuccess) e = cudaMemset(c->d_block, 0, o);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
@@ -193,6 +195,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     pb.fb_list = (int*)(b + o_fl);
     pb.ticket = (unsigned*)(b + o_tk);
     pb.pinv4 = (double*)(b + o_p4);
+    pb.bcoef = (double*)(b + o_bc2);
     double pinv[250], pinv4[375];
     lsq_pinv(3, pinv);
     lsq_pinv(4, pinv4);
@@ -332,13 +335,14 @@ static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t 
 
 // Enqueue the plan kernels (A0 + A1).  No host synchronisation.
 static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
-                      cudaStream_t st) {
+                      cudaStream_t st, bool need_full) {
     DevWcs dw;
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
     if (rc) return rc;
-    if (same_key(c, w, W, H, nside)) return ARGUS_OK;
+    if (same_key(c, w, W, H, nside) && (c->plan_full || !need_full)) return ARGUS_OK;
     c->plan_valid = false;
+    const int lite = need_full ? 0 : 1;
     // Hierarchical plan (plan_block.cuh) whenever a block of 8x8 tiles exists at this nside; the flat plan (one
     // scan slot and one fit per tile) serves nside < 256.
     const bool blocks = dw.k >= ARGUS_TILE_LOG2 + BLOCK_TILES_LOG2;
@@ -373,18 +377,21 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
         int g = (nb_bound + BFIT_WARPS - 1) / BFIT_WARPS;
         if (g > c->sm_count * 8) g = c->sm_count * 8;
         plan_blockfit_kernel<<<g < 1 ? 1 : g, 32 * BFIT_WARPS, 0, st>>>(dw, c->pb);
-        plan_fit_kernel<<<c->sm_count * 2, 32 * FIT_WARPS, 0, st>>>(dw, c->pb, 1);
+        int g2 = (nb_bound + 1) / 2;
+        if (g2 > c->sm_count * 16) g2 = c->sm_count * 16;
+        plan_tilegen_kernel<<<g2 < 1 ? 1 : g2, 128, 0, st>>>(dw, c->pb, lite);
+        plan_fit_kernel<<<c->sm_count * 2, 32 * FIT_WARPS, 0, st>>>(dw, c->pb, 1, lite);
         tile_bound = n_slots * 64;
-        c->n_launches += 3;
+        c->n_launches += 4;
     } else {
         double rad_px = 1.05 * dw.tile_ang / s_rad + 2.0;
         plan_scan_kernel<<<nblk, 256, 0, st>>>(dw, cl, c->pb, rad_px);
         plan_compact_kernel<<<nblk, 256, 0, st>>>(cl, c->pb);
-        plan_fit_kernel<<<c->sm_count * 4, 32 * FIT_WARPS, 0, st>>>(dw, c->pb, 0);
+        plan_fit_kernel<<<c->sm_count * 4, 32 * FIT_WARPS, 0, st>>>(dw, c->pb, 0, lite);
         tile_bound = n_slots;
         c->n_launches += 3;
     }
-    plan_members_kernel<<<c->sm_count * 4, 256, 0, st>>>(dw, c->pb);
+    plan_members_kernel<<<c->sm_count * 16, 256, 0, st>>>(dw, c->pb);
     {
         long long bound = tile_bound < c->pb.max_tiles ? tile_bound : c->pb.max_tiles;
         plan_offsets_local_kernel<<<(int)((bound + 1023) / 1024), 1024, 0, st>>>(c->pb);
@@ -396,6 +403,7 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     c->key_wcs = *w;
     c->key_W = W; c->key_H = H; c->key_nside = nside;
     c->plan_valid = true;
+    c->plan_full = need_full;
     return ARGUS_OK;
 }
 
@@ -461,7 +469,7 @@ extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64
     if (idx_out && !aligned(idx_out, 8)) return ARGUS_ERR_ALIGN;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
-    int rc = build_plan(c, wcs, W, H, nside, -1, st);
+    int rc = build_plan(c, wcs, W, H, nside, -1, st, true);
     if (rc) return rc;
     rc = fetch_stats(c, st);
     if (rc) return rc;
@@ -532,11 +540,11 @@ static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
 }
 
 template <bool COADD>
-static int launch_tiles(argus_ctx* c, int kernel, bool fused, const FrameArgs& f, int64_t W, int64_t H, float w_min, float* v,
-                        float* wt, long long cap, const CoaddArgs& ca, cudaStream_t st) {
+static int launch_tiles(argus_ctx* c, int kernel, bool fused, bool use_fast, const FrameArgs& f, int64_t W, int64_t H, float w_min,
+                        float* v, float* wt, long long cap, const CoaddArgs& ca, cudaStream_t st) {
     int grid = c->sm_count * 8;
     int slow_only = 0;
-    if (kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H)) {
+    if (use_fast) {
         // TMA-staged hot kernel for every tile that fits a stage; the general kernel takes the rest
         if (!c->fast_attr_set) {
             CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
@@ -587,14 +595,15 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
         return ARGUS_OK;
     }
     int slot = c->prof_n & 255;
-    bool replanned = !same_key(c, wcs, W, H, nside);
+    const bool use_fast = kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H);
+    bool replanned = !(same_key(c, wcs, W, H, nside) && (c->plan_full || use_fast));
     if (c->profile) cudaEventRecord(c->ev[slot][0], st);
-    rc = build_plan(c, wcs, W, H, nside, (long long)n, st);
+    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, !use_fast);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][1], st);
     CoaddArgs ca;
     memset(&ca, 0, sizeof(ca));
-    rc = launch_tiles<false>(c, kernel, fused, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
+    rc = launch_tiles<false>(c, kernel, fused, use_fast, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
     if (rc) return rc;
     if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
@@ -651,12 +660,13 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
     int slot = c->prof_n & 255;
-    bool replanned = !same_key(c, wcs, W, H, nside);
+    const bool use_fast = kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H);
+    bool replanned = !(same_key(c, wcs, W, H, nside) && (c->plan_full || use_fast));
     if (c->profile) cudaEventRecord(c->ev[slot][0], st);
-    rc = build_plan(c, wcs, W, H, nside, -1, st);
+    rc = build_plan(c, wcs, W, H, nside, -1, st, !use_fast);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][1], st);
-    rc = launch_tiles<true>(c, kernel, fused, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
+    rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
     if (rc) return rc;
     if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());

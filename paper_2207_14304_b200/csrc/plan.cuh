@@ -44,6 +44,7 @@ struct PlanBuffers {
     int* fb_list;               // [max_tiles] tiles of blocks that need one fit per tile
     unsigned* ticket;           // device scalar: CTA arrival counter of plan_bscan_kernel
     double* pinv4;              // [15][25] pseudo-inverse of the quartic design matrix on the 5x5 node grid
+    double* bcoef;              // [max_tiles/64][32] block quartics (15 x, 15 y), [30] = zone or -1 (no block fit)
     int max_slots, max_tiles, max_hard;
 };
 
@@ -168,8 +169,10 @@ __device__ inline void slow_push(const PlanBuffers& pb, int t) {
 // Everything a kernel needs to know about one tile, written by ONE thread from the tile's cubic (c[0..9] x,
 // c[10..19] y, in S, T = local offsets / 16 px) and the extent of its source positions.  cls on entry:
 // TC_INSIDE / TC_BORDER / TC_EXACT / TC_EMPTY.
+// lite: TileRec and the FP64 coefficients (used by the general kernel only) are written just for the tiles that
+// kernel will visit when the fast kernel runs the frame (border / exact / oversized tiles).
 __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, int zone, int cls, const double* c,
-                                 double xmin, double xmax, double ymin, double ymax, double mg) {
+                                 double xmin, double xmax, double ymin, double ymax, double mg, bool lite) {
     TileRec r;
     r.tile = tile; r.reserved = 0; r.count = 0; r.mask_slot = -1;
     r.zone = zone;
@@ -206,7 +209,7 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
         }
     }
     r.cls = cls;
-    pb.rec[t] = r;
+    bool fast_inside = false;
     pb.tile_id[t] = tile;
     pb.tile_count[t] = r.count;
     pb.tile_cls[t] = (unsigned char)cls;
@@ -236,20 +239,27 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
         f.mask_slot = r.mask_slot;
         f.poly_ok = poly_ok ? 1 : 0;
         if (cls == TC_INSIDE) {
-            if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) f.cls = TC_INSIDE;
+            if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) { f.cls = TC_INSIDE; fast_inside = true; }
             else slow_push(pb, t);
         }   // TC_BORDER: plan_members_kernel finalises the box and decides
-        double* dc = pb.dcoef + (size_t)t * 20;
+        if (!(lite && fast_inside)) {
+            double* dc = pb.dcoef + (size_t)t * 20;
 #pragma unroll
-        for (int i = 0; i < 20; ++i) dc[i] = c[i];
+            for (int i = 0; i < 20; ++i) dc[i] = c[i];
+        }
     } else if (cls == TC_EXACT) {
         slow_push(pb, t);
     }
-    pb.frec[t] = f;
+    if (lite && cls == TC_EMPTY) {
+        pb.frec[t].cls = 0;                 // the fast kernel's producer only reads the class of an empty tile
+    } else {
+        pb.frec[t] = f;
+        if (!(lite && fast_inside)) pb.rec[t] = r;
+    }
 }
 
 #define FIT_WARPS 8
-__global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, PlanBuffers pb, int use_list) {
+__global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, PlanBuffers pb, int use_list, int lite) {
     __shared__ double s_pinv[250];
     __shared__ double s_coef[FIT_WARPS][20];
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -324,7 +334,7 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
                 cls = TC_EMPTY;
             }
         }
-        if (lane == 0) emit_tile(pb, t, tile, (z0 == z1) ? z0 : -1, cls, s_coef[wid], xmin, xmax, ymin, ymax, PLAN_NODE_MARGIN);
+        if (lane == 0) emit_tile(pb, t, tile, (z0 == z1) ? z0 : -1, cls, s_coef[wid], xmin, xmax, ymin, ymax, PLAN_NODE_MARGIN, lite != 0);
         __syncwarp();
     }
 }
@@ -357,19 +367,19 @@ __device__ inline bool border_member(const DevWcs& w, const PolyAxis& px, const 
 
 __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers pb) {
     __shared__ unsigned s_mask[32];
-    __shared__ int s_ext[4];
-    __shared__ int s_cnt;
-    int tid = threadIdx.x;
+    __shared__ int s_wext[8][5];     // per warp: xmin, xmax, ymin, ymax, count
+    __shared__ TileRec s_rec;
+    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int n_hard = *pb.hard_count;
     if (n_hard > pb.max_hard) n_hard = pb.max_hard;
     int u0, v0;
     thread_block_origin(tid, u0, v0);
     for (int h = blockIdx.x; h < n_hard; h += gridDim.x) {
         int t = pb.hard_list[h];
-        if (tid < 32) s_mask[tid] = 0u;
-        if (tid == 0) { s_ext[0] = 0x7fffffff; s_ext[1] = -0x7fffffff; s_ext[2] = 0x7fffffff; s_ext[3] = -0x7fffffff; s_cnt = 0; }
         __syncthreads();
-        const TileRec& r = pb.rec[t];
+        if (tid < (int)(sizeof(TileRec) / 16)) reinterpret_cast<int4*>(&s_rec)[tid] = __ldg(reinterpret_cast<const int4*>(pb.rec + t) + tid);
+        __syncthreads();
+        const TileRec& r = s_rec;
         int face, tx, ty;
         nest_to_xyf(r.tile, w.k - ARGUS_TILE_LOG2, face, tx, ty);
         int ix0 = tx * 32, iy0 = ty * 32;
@@ -397,28 +407,36 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
                 xmin = min(xmin, ci); xmax = max(xmax, ci); ymin = min(ymin, cj); ymax = max(ymax, cj);
             }
         }
-        if (nib) {
-            atomicOr(&s_mask[tid >> 3], nib << (4 * (tid & 7)));
-            atomicMin(&s_ext[0], xmin); atomicMax(&s_ext[1], xmax);
-            atomicMin(&s_ext[2], ymin); atomicMax(&s_ext[3], ymax);
-            atomicAdd(&s_cnt, __popc(nib));
-        }
+        // warp-level reductions (no shared-memory atomics): 8 threads make one mask word
+        unsigned word = nib << (4 * (tid & 7));
+        word |= __shfl_xor_sync(0xffffffffu, word, 1);
+        word |= __shfl_xor_sync(0xffffffffu, word, 2);
+        word |= __shfl_xor_sync(0xffffffffu, word, 4);
+        if ((tid & 7) == 0) s_mask[tid >> 3] = word;
+        xmin = __reduce_min_sync(0xffffffffu, xmin); xmax = __reduce_max_sync(0xffffffffu, xmax);
+        ymin = __reduce_min_sync(0xffffffffu, ymin); ymax = __reduce_max_sync(0xffffffffu, ymax);
+        int cnt = __reduce_add_sync(0xffffffffu, __popc(nib));
+        if (lane == 0) { s_wext[wid][0] = xmin; s_wext[wid][1] = xmax; s_wext[wid][2] = ymin; s_wext[wid][3] = ymax; s_wext[wid][4] = cnt; }
         __syncthreads();
         if (tid < 32) pb.masks[(size_t)h * 32 + tid] = s_mask[tid];
         if (tid == 0) {
+            int e0 = 0x7fffffff, e1 = -0x7fffffff, e2 = 0x7fffffff, e3 = -0x7fffffff, c = 0;
+            for (int i = 0; i < 8; ++i) {
+                e0 = min(e0, s_wext[i][0]); e1 = max(e1, s_wext[i][1]); e2 = min(e2, s_wext[i][2]); e3 = max(e3, s_wext[i][3]);
+                c += s_wext[i][4];
+            }
             TileRec* wr = &pb.rec[t];
-            int c = s_cnt;
             wr->count = c;
             pb.tile_count[t] = c;
             if (c == 0) {
                 wr->cls = TC_EMPTY;
                 pb.tile_cls[t] = TC_EMPTY;
             } else {
-                wr->bx0 = s_ext[0]; wr->bx1 = s_ext[1]; wr->by0 = s_ext[2]; wr->by1 = s_ext[3];
+                wr->bx0 = e0; wr->bx1 = e1; wr->by0 = e2; wr->by1 = e3;
                 if (cls == TC_BORDER) {
                     FastRec* fr = &pb.frec[t];
                     FastRec f = *fr;
-                    if (f.poly_ok && fast_box(s_ext[0], s_ext[1], s_ext[2], s_ext[3], f.X0, f.Y0, f)) {
+                    if (f.poly_ok && fast_box(e0, e1, e2, e3, f.X0, f.Y0, f)) {
                         f.cls = TC_BORDER;
                         *fr = f;
                     } else {
@@ -427,7 +445,6 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
                 }
             }
         }
-        __syncthreads();
     }
 }
 
@@ -527,10 +544,9 @@ __global__ void __launch_bounds__(256) plan_write_indices_kernel(PlanBuffers pb,
     int tid = threadIdx.x;
     int n = *pb.n_tiles;
     for (int t = blockIdx.x; t < n; t += gridDim.x) {
-        const TileRec& r = pb.rec[t];
-        int cls = r.cls;
+        int cls = pb.tile_cls[t];
         if (cls == TC_EMPTY) continue;
-        long long base = r.tile << 10, off = tile_out_offset(pb, t);
+        long long base = pb.tile_id[t] << 10, off = tile_out_offset(pb, t);
         if (cls == TC_INSIDE) {
             for (int q = 0; q < 4; ++q) {
                 int m = q * 256 + tid;
@@ -538,7 +554,7 @@ __global__ void __launch_bounds__(256) plan_write_indices_kernel(PlanBuffers pb,
             }
         } else {
             __syncthreads();
-            if (tid < 32) s_mask[tid] = pb.masks[(size_t)r.mask_slot * 32 + tid];
+            if (tid < 32) s_mask[tid] = pb.masks[(size_t)pb.rec[t].mask_slot * 32 + tid];
             __syncthreads();
             if (tid == 0) {
                 int a = 0;

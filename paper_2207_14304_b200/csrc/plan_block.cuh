@@ -6,8 +6,8 @@
 //
 //   bscan    : every block-level child of the host-chosen coarse cells is tested with one exact evaluation of its
 //              centre; the last CTA to finish compacts the survivors into the ascending block list
-//   blockfit : one warp per block: 25 nodes + 7 check points -> least-squares quartic, residual check; then two
-//              tiles per lane: re-expansion, extent from the tile corners, classification, tile records.
+//   blockfit : one warp per block: 25 nodes + 7 check points -> least-squares quartic, residual check
+//   tilegen  : one thread per tile: re-expansion, extent from the tile corners, classification, tile records.
 //              Blocks that are not smooth (belt/cap ring, poles), not inside the search cone or badly fitted hand
 //              their 64 tiles to plan_fit_kernel (one fit per tile, list mode).
 // Tile index t = 64 * (position of the block) + (tile's Morton index in the block): ascending nested order.
@@ -51,24 +51,35 @@ __global__ void __launch_bounds__(256) plan_bscan_kernel(DevWcs w, CoarseList cl
     __threadfence();
     if (tid == 0) pb.stats->overflow = 0;
     __syncthreads();
+    // 8 consecutive slots per thread and pass (flags read as one 64-bit word: slot_flag is 256-byte aligned)
     int base = 0;
-    for (long long s0 = 0; s0 < n_slots; s0 += 256) {
-        const long long s = s0 + tid;
-        const int k = (s < n_slots) ? (int)__ldcg(pb.slot_flag + s) : 0;
-        const unsigned bal = __ballot_sync(0xffffffffu, k);
-        if (lane == 0) s_part[wid] = __popc(bal);
+    for (long long s0 = 0; s0 < n_slots; s0 += 2048) {
+        const long long s = s0 + 8ll * tid;
+        unsigned long long fl8 = 0ull;
+        if (s < n_slots) fl8 = __ldcg(reinterpret_cast<const unsigned long long*>(pb.slot_flag + s));
+        if (s + 8 > n_slots && s < n_slots) fl8 &= (1ull << (8 * (int)(n_slots - s))) - 1ull;   // tail: stale bytes beyond n_slots
+        const int cnt = __popcll(fl8 & 0x0101010101010101ull);
+        int inc = cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += y;
+        }
+        if (lane == 31) s_part[wid] = inc;
         __syncthreads();
         int woff = 0, tot = 0;
         for (int i = 0; i < 8; ++i) { if (i < wid) woff += s_part[i]; tot += s_part[i]; }
-        if (k) {
-            const int pos = base + woff + __popc(bal & ((1u << lane) - 1u));
-            if ((long long)(pos + 1) * 64 <= pb.max_tiles) {
-                const int c = (int)(s >> (2 * rl));
-                pb.block_id[pos] = (cl.cell[c] << (2 * rl)) | (s & ((1ll << (2 * rl)) - 1));
-            } else {
-                atomicOr(&pb.stats->overflow, 1);
+        int pos = base + woff + inc - cnt;
+        for (int j = 0; j < 8; ++j)
+            if ((fl8 >> (8 * j)) & 1ull) {
+                if ((long long)(pos + 1) * 64 <= pb.max_tiles) {
+                    const long long sj = s + j;
+                    const int c = (int)(sj >> (2 * rl));
+                    pb.block_id[pos] = (cl.cell[c] << (2 * rl)) | (sj & ((1ll << (2 * rl)) - 1));
+                } else {
+                    atomicOr(&pb.stats->overflow, 1);
+                }
+                ++pos;
             }
-        }
         base += tot;
         __syncthreads();
     }
@@ -181,48 +192,63 @@ __global__ void __launch_bounds__(32 * BFIT_WARPS) plan_blockfit_kernel(DevWcs w
             const bool cone_in = acos(fmin(cmin, 1.0)) + 0.1 * w.tile_ang <= w.rho;   // nodes include the block corners
             ok = (amax < 1e8) && (cmin > 0.05) && (res <= PLAN_FIT_TOL) && cone_in;   // NaN compares false
         }
-        const int t_base = b * 64;
-        if (!ok) {
-            int fb = 0;
-            if (lane == 0) fb = atomicAdd(pb.fb_count, 64);
-            fb = __shfl_sync(0xffffffffu, fb, 0);
-#pragma unroll
-            for (int jj = 0; jj < 2; ++jj) {
-                const int j = lane + 32 * jj;
-                pb.tile_id[t_base + j] = (blk << 6) | j;
-                pb.fb_list[fb + j] = t_base + j;     // fb + 64 <= 64 n_blocks <= max_tiles
-            }
-        } else {
-#pragma unroll 1
-            for (int jj = 0; jj < 2; ++jj) {
-                const int j = lane + 32 * jj;
-                const int ta = (int)compact_even_bits((unsigned)j), tb = (int)compact_even_bits((unsigned)j >> 1);
-                const double Uc = ((double)ta - 3.5) * 0.25, Vc = ((double)tb - 3.5) * 0.25;
-                double c[20];
-                reexpand_cubic(s_bc[wid], Uc, Vc, c);
-                reexpand_cubic(s_bc[wid] + 15, Uc, Vc, c + 10);
-                // extent of the source positions: the four tile corners (S, T = +-1) plus the size of the nonlinear part
-                double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const double s = (q & 1) ? 1.0 : -1.0, tt = (q >> 1) ? 1.0 : -1.0;
-                    double m[10];
-                    cubic_basis(s, tt, m);
-                    double xv = 0.0, yv = 0.0;
-#pragma unroll
-                    for (int i = 0; i < 10; ++i) { xv = fma(c[i], m[i], xv); yv = fma(c[10 + i], m[i], yv); }
-                    xmin = fmin(xmin, xv); xmax = fmax(xmax, xv); ymin = fmin(ymin, yv); ymax = fmax(ymax, yv);
-                }
-                double nl = 0.0;
-#pragma unroll
-                for (int i = 3; i < 10; ++i) nl = fmax(nl, 0.0) + fmax(fabs(c[i]), fabs(c[10 + i]));
-                const double mg = PLAN_NODE_MARGIN + nl;
-                const bool all_out = (xmax + mg < -0.5) || (xmin - mg >= w.W - 0.5) || (ymax + mg < -0.5) || (ymin - mg >= w.H - 0.5);
-                const bool all_in = (xmin - mg >= -0.5) && (xmax + mg < w.W - 0.5) && (ymin - mg >= -0.5) && (ymax + mg < w.H - 0.5);
-                const int cls = all_out ? TC_EMPTY : (all_in ? TC_INSIDE : TC_BORDER);
-                emit_tile(pb, t_base + j, (blk << 6) | j, z0, cls, c, xmin, xmax, ymin, ymax, mg);
-            }
-        }
+        // hand over to plan_tilegen_kernel: 30 coefficients (x then y) + status word (zone, or -1 = no block fit)
+        if (lane < 30) pb.bcoef[(size_t)b * 32 + lane] = ok ? s_bc[wid][lane] : 0.0;
+        if (lane == 30) pb.bcoef[(size_t)b * 32 + 30] = ok ? (double)z0 : -1.0;
         __syncwarp();
+    }
+}
+
+// ----------------------------------------------------------------------------------------- tilegen
+// One thread per tile: re-expansion of the block quartic about the tile centre, extent from the tile corners,
+// classification, tile records.  Tiles of blocks without a fit go to the per-tile fit list.
+__global__ void __launch_bounds__(128) plan_tilegen_kernel(DevWcs w, PlanBuffers pb, int lite) {
+    __shared__ double s_bc[2][32];
+    const int tid = threadIdx.x;
+    const int n_blocks = *pb.n_blocks;
+    for (int b0 = blockIdx.x * 2; b0 < n_blocks; b0 += gridDim.x * 2) {
+        __syncthreads();
+        if (tid < 64) {
+            const int b = b0 + (tid >> 5);
+            s_bc[tid >> 5][tid & 31] = (b < n_blocks) ? pb.bcoef[(size_t)b * 32 + (tid & 31)] : -1.0;
+        }
+        __syncthreads();
+        const int half = tid >> 6, j = tid & 63, b = b0 + half;
+        if (b >= n_blocks) continue;
+        const long long blk = pb.block_id[b];
+        const int t = b * 64 + j;
+        const long long tile = (blk << 6) | j;
+        const double* bc = s_bc[half];
+        if (bc[30] < 0.0) {
+            pb.tile_id[t] = tile;
+            const int fb = atomicAdd(pb.fb_count, 1);      // fb < 64 n_blocks <= max_tiles
+            pb.fb_list[fb] = t;
+            continue;
+        }
+        const int ta = (int)compact_even_bits((unsigned)j), tb = (int)compact_even_bits((unsigned)j >> 1);
+        const double Uc = ((double)ta - 3.5) * 0.25, Vc = ((double)tb - 3.5) * 0.25;
+        double c[20];
+        reexpand_cubic(bc, Uc, Vc, c);
+        reexpand_cubic(bc + 15, Uc, Vc, c + 10);
+        // extent of the source positions: the four tile corners (S, T = +-1) plus the size of the nonlinear part
+        double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const double s = (q & 1) ? 1.0 : -1.0, tt = (q >> 1) ? 1.0 : -1.0;
+            double m[10];
+            cubic_basis(s, tt, m);
+            double xv = 0.0, yv = 0.0;
+#pragma unroll
+            for (int i = 0; i < 10; ++i) { xv = fma(c[i], m[i], xv); yv = fma(c[10 + i], m[i], yv); }
+            xmin = fmin(xmin, xv); xmax = fmax(xmax, xv); ymin = fmin(ymin, yv); ymax = fmax(ymax, yv);
+        }
+        double nl = 0.0;
+#pragma unroll
+        for (int i = 3; i < 10; ++i) nl += fmax(fabs(c[i]), fabs(c[10 + i]));
+        const double mg = PLAN_NODE_MARGIN + nl;
+        const bool all_out = (xmax + mg < -0.5) || (xmin - mg >= w.W - 0.5) || (ymax + mg < -0.5) || (ymin - mg >= w.H - 0.5);
+        const bool all_in = (xmin - mg >= -0.5) && (xmax + mg < w.W - 0.5) && (ymin - mg >= -0.5) && (ymax + mg < w.H - 0.5);
+        const int cls = all_out ? TC_EMPTY : (all_in ? TC_INSIDE : TC_BORDER);
+        emit_tile(pb, t, tile, (int)bc[30], cls, c, xmin, xmax, ymin, ymax, mg, lite != 0);
     }
 }
