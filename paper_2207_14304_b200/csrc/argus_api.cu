@@ -394,10 +394,10 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     plan_members_kernel<<<c->sm_count * 16, 256, 0, st>>>(dw, c->pb);
     {
         long long bound = tile_bound < c->pb.max_tiles ? tile_bound : c->pb.max_tiles;
-        plan_offsets_local_kernel<<<(int)((bound + 1023) / 1024), 1024, 0, st>>>(c->pb);
-        plan_offsets_final_kernel<<<1, 1024, 0, st>>>(c->pb, out_cap);
+        int gb = (int)((bound + 1023) / 1024);
+        plan_offsets_kernel<<<gb < 1 ? 1 : gb, 1024, 0, st>>>(c->pb, out_cap);
     }
-    c->n_launches += 3;
+    c->n_launches += 2;
     CUDA_TRY(c, cudaGetLastError());
     c->dw = dw;
     c->key_wcs = *w;

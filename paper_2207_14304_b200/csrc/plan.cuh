@@ -263,10 +263,11 @@ __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, Plan
     __shared__ double s_pinv[250];
     __shared__ double s_coef[FIT_WARPS][20];
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    // use_list: only the tiles plan_blockfit_kernel could not derive from a block fit (usually none)
+    const int n_items = use_list ? *pb.fb_count : *pb.n_tiles;
+    if ((int)blockIdx.x * FIT_WARPS >= n_items) return;
     for (int i = tid; i < 250; i += blockDim.x) s_pinv[i] = pb.pinv[i];
     __syncthreads();
-    // use_list: only the tiles plan_blockfit_kernel could not derive from a block fit
-    const int n_items = use_list ? *pb.fb_count : *pb.n_tiles;
     long long ns = 1ll << w.k;
     // node coordinates: lanes 0..24 the 5x5 fit grid, lanes 25..31 extra check points
     double S, T;
@@ -365,7 +366,7 @@ __device__ inline bool border_member(const DevWcs& w, const PolyAxis& px, const 
     return inx && iny;
 }
 
-__global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers pb) {
+__global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuffers pb) {
     __shared__ unsigned s_mask[32];
     __shared__ int s_wext[8][5];     // per warp: xmin, xmax, ymin, ymax, count
     __shared__ TileRec s_rec;
@@ -449,48 +450,10 @@ __global__ void __launch_bounds__(256) plan_members_kernel(DevWcs w, PlanBuffers
 }
 
 // ------------------------------------------------------------------------------------------ offsets
-// Exclusive scan of the per-tile counts in two small launches: block-local scan (1024 tiles per block,
-// coalesced reads of the compact count / class arrays) + one block that scans the block sums.
+// Exclusive scan of the per-tile counts in one launch: block-local scan (1024 tiles per CTA, coalesced reads of
+// the compact count / class arrays); the last CTA to finish scans the per-CTA sums.
 // Output position of tile t = block_base[t >> 10] + tile_offset[t].
-__global__ void __launch_bounds__(1024) plan_offsets_local_kernel(PlanBuffers pb) {
-    __shared__ int s_warp[32];
-    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    int n = *pb.n_tiles;
-    int i = blockIdx.x * 1024 + tid;
-    if (blockIdx.x * 1024 >= n) return;
-    int c = (i < n) ? pb.tile_count[i] : 0;
-    int cls = (i < n) ? pb.tile_cls[i] : -1;
-    int inc = c;
-    for (int o = 1; o < 32; o <<= 1) {
-        int v = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += v;
-    }
-    if (lane == 31) s_warp[wid] = inc;
-    unsigned m_in = __ballot_sync(0xffffffffu, cls == TC_INSIDE), m_bo = __ballot_sync(0xffffffffu, cls == TC_BORDER);
-    unsigned m_ex = __ballot_sync(0xffffffffu, cls == TC_EXACT), m_em = __ballot_sync(0xffffffffu, cls == TC_EMPTY);
-    if (lane == 0) {
-        PlanStats* st = pb.stats;
-        if (m_in) atomicAdd((unsigned long long*)&st->n_inside, (unsigned long long)__popc(m_in));
-        if (m_bo) atomicAdd((unsigned long long*)&st->n_border, (unsigned long long)__popc(m_bo));
-        if (m_ex) atomicAdd((unsigned long long*)&st->n_exact, (unsigned long long)__popc(m_ex));
-        if (m_em) atomicAdd((unsigned long long*)&st->n_empty, (unsigned long long)__popc(m_em));
-    }
-    __syncthreads();
-    if (wid == 0) {
-        int v = s_warp[lane], iv = v;
-        for (int o = 1; o < 32; o <<= 1) {
-            int u = __shfl_up_sync(0xffffffffu, iv, o);
-            if (lane >= o) iv += u;
-        }
-        s_warp[lane] = iv - v;
-        if (lane == 31) pb.block_sum[blockIdx.x] = iv;
-    }
-    __syncthreads();
-    if (i < n) pb.tile_offset[i] = s_warp[wid] + inc - c;
-}
-
-__global__ void __launch_bounds__(1024) plan_offsets_final_kernel(PlanBuffers pb, long long out_capacity) {
-    __shared__ long long s_warp[32];
+__device__ inline void offsets_final_body(const PlanBuffers& pb, long long out_capacity, long long* s_warp) {
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int n = *pb.n_tiles;
     int nb = (n + 1023) >> 10;   // <= 1024 * 16 blocks (max_tiles <= 2^24): each thread handles up to 16
@@ -498,7 +461,7 @@ __global__ void __launch_bounds__(1024) plan_offsets_final_kernel(PlanBuffers pb
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
         int b = tid * 16 + j;
-        v[j] = (b < nb) ? (long long)pb.block_sum[b] : 0;
+        v[j] = (b < nb) ? (long long)__ldcg(pb.block_sum + b) : 0;
         sum += v[j];
     }
     long long inc = sum;
@@ -530,6 +493,55 @@ __global__ void __launch_bounds__(1024) plan_offsets_final_kernel(PlanBuffers pb
         st->n_tiles = n;
         if (out_capacity >= 0 && run > out_capacity) atomicOr(&st->overflow, 4);
     }
+}
+
+__global__ void __launch_bounds__(1024) plan_offsets_kernel(PlanBuffers pb, long long out_capacity) {
+    __shared__ int s_warp[32];
+    __shared__ long long s_warp64[32];
+    __shared__ int s_last;
+    int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int n = *pb.n_tiles;
+    int i = blockIdx.x * 1024 + tid;
+    if (blockIdx.x * 1024 < n) {
+        int c = (i < n) ? pb.tile_count[i] : 0;
+        int cls = (i < n) ? pb.tile_cls[i] : -1;
+        int inc = c;
+        for (int o = 1; o < 32; o <<= 1) {
+            int v = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        if (lane == 31) s_warp[wid] = inc;
+        unsigned m_in = __ballot_sync(0xffffffffu, cls == TC_INSIDE), m_bo = __ballot_sync(0xffffffffu, cls == TC_BORDER);
+        unsigned m_ex = __ballot_sync(0xffffffffu, cls == TC_EXACT), m_em = __ballot_sync(0xffffffffu, cls == TC_EMPTY);
+        if (lane == 0) {
+            PlanStats* st = pb.stats;
+            if (m_in) atomicAdd((unsigned long long*)&st->n_inside, (unsigned long long)__popc(m_in));
+            if (m_bo) atomicAdd((unsigned long long*)&st->n_border, (unsigned long long)__popc(m_bo));
+            if (m_ex) atomicAdd((unsigned long long*)&st->n_exact, (unsigned long long)__popc(m_ex));
+            if (m_em) atomicAdd((unsigned long long*)&st->n_empty, (unsigned long long)__popc(m_em));
+        }
+        __syncthreads();
+        if (wid == 0) {
+            int v = s_warp[lane], iv = v;
+            for (int o = 1; o < 32; o <<= 1) {
+                int u = __shfl_up_sync(0xffffffffu, iv, o);
+                if (lane >= o) iv += u;
+            }
+            s_warp[lane] = iv - v;
+            if (lane == 31) pb.block_sum[blockIdx.x] = iv;
+        }
+        __syncthreads();
+        if (i < n) pb.tile_offset[i] = s_warp[wid] + inc - c;
+    }
+    // the last CTA to arrive scans the per-CTA sums (block_base) and closes the statistics
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(pb.ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    offsets_final_body(pb, out_capacity, s_warp64);
+    if (tid == 0) *pb.ticket = 0u;
 }
 
 __device__ __forceinline__ long long tile_out_offset(const PlanBuffers& pb, int t) {
