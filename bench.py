@@ -29,9 +29,9 @@ if ROOT not in sys.path:
 METRIC = "calibrated+HEALPix-resampled Mpix/s per B200; achieved HBM GB/s vs peak"
 UNIT = "Mpix/s"  # input (detector) pixels per second
 SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload recipe per step
-# dram__bytes_read.sum + dram__bytes_write.sum of resample_tiles_kernel<0,true,false> on config 1, one launch,
-# from profiles/ (ncu --set full); None until captured.
-NCU_TRAFFIC_BYTES = None
+# dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
+# profiles/r1_final_ncu_summary.txt (ncu --set full).
+NCU_TRAFFIC_BYTES = 957322496 + 339269376  # profiles/r1_final_ncu_summary.txt
 
 
 def _peaks():
@@ -270,8 +270,8 @@ def run_gpu(args):
                        "parallelism": "1 frame per GPU per step, frames independent (replicas)"},
             "output_mpix_per_s": px_out_all * args.steps / (ms * 1e-3) / 1e6,
             "plan_ms_per_step": plan_ms / max(ncalls, 1),
-            "roofline": {"bound": "hbm", "kernel": "resample_tiles_kernel<bilinear,fused>", "achieved": achieved,
-                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES,
+            "roofline": {"bound": "hbm", "kernel": "resample_fast_kernel<false> (TMA-staged bilinear, fused calibration)", "achieved": achieved,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if args.workload == "config1" else None,
                          "peak_source": peak_src, "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes,
                          "step_frac": (alg_bytes / (ms_step * 1e-3) / 1e9) / peak},
             "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_d,
