@@ -75,8 +75,7 @@ struct __align__(16) FastRec {
     int Y0, poly_ok;     // poly_ok: the FP32 remainder stays inside the rounding-constant range
     float px[10];        // [0] = rounding constant, [1..9] monomials S, T, S^2, ST, T^2, S^3, S^2 T, S T^2, T^3
     float py[10];
-    int cols;            // float4 columns of the box that hold taps: first | (count << 8)
-    int pad2[3];
+    int pad2[4];
 };
 static_assert(sizeof(FastRec) == 160, "FastRec must be 10 x 16 bytes");
 

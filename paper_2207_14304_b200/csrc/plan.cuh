@@ -155,8 +155,6 @@ __device__ inline bool fast_box(int bx0, int bx1, int by0, int by1, int X0, int 
     if (gx0 < X0 || by0 < Y0 || bx1 + 2 - X0 > 500 || by1 + 2 - Y0 > 500) return false;
     f.gx0 = gx0; f.gy0 = by0; f.wclass = wclass | (hclass << 4); f.bh = bh;
     f.kofs = (Y0 - by0) * pitch + (X0 - gx0);
-    int c_lo = (bx0 - gx0) >> 2, c_hi = (bx1 + 2 - gx0 + 3) >> 2;
-    f.cols = c_lo | ((c_hi - c_lo) << 8);
     return true;
 }
 
