@@ -266,6 +266,7 @@ def run_gpu(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl, "frames_per_step_per_gpu": 1, "W": W, "H": H, "nside": fr.nside,
                        "kernel": fr.kernel, "n_footprint": n_fp, "fused": True, "plan_every_step": True,
+                       "plan_overlap": "the plan of step k+1 runs on the library's side streams underneath the kernels of step k",
                        "l2": "inputs (856 MB/frame) larger than L2 (126 MB)", "plan": stats,
                        "parallelism": "1 frame per GPU per step, frames independent (replicas)"},
             "output_mpix_per_s": px_out_all * args.steps / (ms * 1e-3) / 1e6,

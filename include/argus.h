@@ -59,6 +59,9 @@ enum {
                                  call with identical arguments; 0: every call re-plans on the device */
     ARGUS_OPT_FAST_PATH = 3,  /* 1 (default): bilinear resampling of raw + masters (no bpm, W % 8 == 0, 16-byte aligned
                                  arrays) stages source tiles with TMA (resample_fast_kernel); 0: always the general kernel */
+    ARGUS_OPT_PLAN_OVERLAP = 4, /* 1 (default): the plan of a new WCS is built on an internal high-priority stream in a second
+                                 set of scratch buffers, so that it runs underneath the previous frame's kernels; the
+                                 caller's stream waits for it (stream order of results is unchanged); 0: in place */
     ARGUS_OPT_PROFILE = 2     /* 1: argus_resample / argus_resample_coadd (idx == NULL) record CUDA events on
                                  the caller's stream around the plan kernels and around the fused kernel
                                  (ring of 256 calls); read them back with argus_profile_read.  Default 0. */

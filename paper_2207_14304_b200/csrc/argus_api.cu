@@ -15,6 +15,7 @@
 #include "resample_fast.cuh"
 
 #define ARGUS_VERSION_NUM 100
+#define PLAN_SLOTS 3
 
 struct argus_ctx {
     int device;
@@ -28,11 +29,22 @@ struct argus_ctx {
     DevWcs dw;
     PlanBuffers pb;
     PlanStats* h_stats;   // pinned
-    void* d_block;        // the single device allocation behind pb
     bool profile;
     int prof_n;           // calls recorded since the last read
-    cudaEvent_t ev[256][3];
+    cudaEvent_t ev[256][4];   // plan begin / end (on the stream the plan ran on), resample begin / end (caller's stream)
     bool ev_plan[256];    // the call re-planned (ev[i][0] -> ev[i][1] is meaningful)
+    // PLAN_SLOTS sets of plan scratch: with ARGUS_OPT_PLAN_OVERLAP the plan of a new WCS is built on a high-priority
+    // side stream in the set whose last reader is oldest, so it runs underneath the previous frames' kernels (up to
+    // PLAN_SLOTS - 1 frames ahead of them).
+    PlanBuffers slot_pb[PLAN_SLOTS];
+    void* slot_block[PLAN_SLOTS];
+    int cur_slot;
+    bool overlap;
+    bool slot_used[PLAN_SLOTS];   // ev_free[s] has been recorded
+    cudaStream_t side[2];     // plans of consecutive frames alternate between two side streams (two plans in flight)
+    int side_next;
+    cudaEvent_t ev_done[PLAN_SLOTS];   // plan of the slot complete (side stream)
+    cudaEvent_t ev_free[PLAN_SLOTS];   // last kernel reading the slot complete (caller's stream)
     // TMA descriptors of the fast kernel, cached per (pointers, W, H)
     void* encode_fn;      // cuTensorMapEncodeTiled, resolved at first use (no link-time libcuda dependency)
     bool encode_tried;
@@ -116,21 +128,8 @@ static void lsq_pinv(int deg, double* pinv) {
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) {
-    if (!out) return ARGUS_ERR_NULL;
-    *out = nullptr;
-    if (max_tiles == 0) max_tiles = 1 << 19;
-    if (max_tiles < 64 || max_tiles > (1 << 24)) return ARGUS_ERR_SHAPE;
-    argus_ctx* c = new (std::nothrow) argus_ctx();
-    if (!c) return ARGUS_ERR_CAPACITY;
-    memset(c, 0, sizeof(*c));
-    c->device = device;
-    c->plan_cache = true;
-    c->fast_enabled = true;
-    cudaError_t e = cudaSetDevice(device);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
-    if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
-    PlanBuffers& pb = c->pb;
+// One set of plan scratch: a single device allocation carved into the PlanBuffers arrays.
+static cudaError_t alloc_plan_slot(int64_t max_tiles, PlanBuffers& pb, void** block) {
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
@@ -161,15 +160,10 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     o_tk = o;    o = align_up(o + sizeof(unsigned), 256);
     o_p4 = o;    o = align_up(o + sizeof(double) * 375, 256);
     o_bc2 = o;   o = align_up(o + sizeof(double) * 32 * (size_t)(pb.max_tiles / 64 + 1), 256);
-    e = cudaMalloc(&c->d_block, o);
-    if (e == cudaSuccess) e = cudaMemset(c->d_block, 0, o);
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
-    if (e != cudaSuccess) {
-        if (c->d_block) cudaFree(c->d_block);
-        delete c;
-        return ARGUS_ERR_CUDA;
-    }
-    char* b = (char*)c->d_block;
+    cudaError_t e = cudaMalloc(block, o);
+    if (e == cudaSuccess) e = cudaMemset(*block, 0, o);
+    if (e != cudaSuccess) return e;
+    char* b = (char*)*block;
     pb.slot_flag = (unsigned char*)(b + o_flag);
     pb.block_count = (int*)(b + o_bc);
     pb.tile_id = (long long*)(b + o_tid);
@@ -201,14 +195,45 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     lsq_pinv(4, pinv4);
     e = cudaMemcpy(pb.pinv, pinv, sizeof(pinv), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(pb.pinv4, pinv4, sizeof(pinv4), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) {
-        cudaFree(c->d_block);
-        cudaFreeHost(c->h_stats);
+    return e;
+}
+
+extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) {
+    if (!out) return ARGUS_ERR_NULL;
+    *out = nullptr;
+    if (max_tiles == 0) max_tiles = 1 << 19;
+    if (max_tiles < 64 || max_tiles > (1 << 24)) return ARGUS_ERR_SHAPE;
+    argus_ctx* c = new (std::nothrow) argus_ctx();
+    if (!c) return ARGUS_ERR_CAPACITY;
+    memset(c, 0, sizeof(*c));
+    c->device = device;
+    c->plan_cache = true;
+    c->fast_enabled = true;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
+    cudaError_t e2 = cudaSuccess;
+    for (int sidx = 0; sidx < PLAN_SLOTS && e2 == cudaSuccess; ++sidx) e2 = alloc_plan_slot(max_tiles, c->slot_pb[sidx], &c->slot_block[sidx]);
+    if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
+    int prio_lo = 0, prio_hi = 0;
+    if (e2 == cudaSuccess) e2 = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    for (int i = 0; i < 2 && e2 == cudaSuccess; ++i) e2 = cudaStreamCreateWithPriority(&c->side[i], cudaStreamNonBlocking, prio_hi);
+    for (int sidx = 0; sidx < PLAN_SLOTS && e2 == cudaSuccess; ++sidx) {
+        e2 = cudaEventCreateWithFlags(&c->ev_done[sidx], cudaEventDisableTiming);
+        if (e2 == cudaSuccess) e2 = cudaEventCreateWithFlags(&c->ev_free[sidx], cudaEventDisableTiming);
+    }
+    if (e2 != cudaSuccess) {
+        c->last_cuda = (int)e2;
+        for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) if (c->slot_block[sidx]) cudaFree(c->slot_block[sidx]);
+        if (c->h_stats) cudaFreeHost(c->h_stats);
         delete c;
         return ARGUS_ERR_CUDA;
     }
+    c->pb = c->slot_pb[0];
+    c->cur_slot = 0;
+    c->overlap = true;
     for (int i = 0; i < 256; ++i)
-        for (int j = 0; j < 3; ++j) cudaEventCreate(&c->ev[i][j]);
+        for (int j = 0; j < 4; ++j) cudaEventCreate(&c->ev[i][j]);
     *out = c;
     return ARGUS_OK;
 }
@@ -217,8 +242,13 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (!c) return ARGUS_ERR_NULL;
     cudaSetDevice(c->device);
     for (int i = 0; i < 256; ++i)
-        for (int j = 0; j < 3; ++j) cudaEventDestroy(c->ev[i][j]);
-    cudaFree(c->d_block);
+        for (int j = 0; j < 4; ++j) cudaEventDestroy(c->ev[i][j]);
+    for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
+        cudaFree(c->slot_block[sidx]);
+        cudaEventDestroy(c->ev_done[sidx]);
+        cudaEventDestroy(c->ev_free[sidx]);
+    }
+    for (int i = 0; i < 2; ++i) cudaStreamDestroy(c->side[i]);
     cudaFreeHost(c->h_stats);
     delete c;
     return ARGUS_OK;
@@ -234,6 +264,10 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
     if (option == ARGUS_OPT_PROFILE) {
         c->profile = value != 0;
         c->prof_n = 0;
+        return ARGUS_OK;
+    }
+    if (option == ARGUS_OPT_PLAN_OVERLAP) {
+        c->overlap = value != 0;
         return ARGUS_OK;
     }
     if (option == ARGUS_OPT_FAST_PATH) {
@@ -252,7 +286,7 @@ extern "C" int argus_profile_read(argus_ctx* c, double* plan_ms, double* kernel_
     for (int i = 0; i < n; ++i) {
         float a = 0.f, b = 0.f;
         if (c->ev_plan[i]) CUDA_TRY(c, cudaEventElapsedTime(&a, c->ev[i][0], c->ev[i][1]));
-        CUDA_TRY(c, cudaEventElapsedTime(&b, c->ev[i][1], c->ev[i][2]));
+        CUDA_TRY(c, cudaEventElapsedTime(&b, c->ev[i][2], c->ev[i][3]));
         p += a; k += b;
     }
     *plan_ms = p; *kernel_ms = k; *n_calls = n;
@@ -335,7 +369,7 @@ static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t 
 
 // Enqueue the plan kernels (A0 + A1).  No host synchronisation.
 static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
-                      cudaStream_t st, bool need_full) {
+                      cudaStream_t caller, bool need_full, int prof_slot) {
     DevWcs dw;
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
@@ -343,6 +377,19 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     if (same_key(c, w, W, H, nside) && (c->plan_full || !need_full)) return ARGUS_OK;
     c->plan_valid = false;
     const int lite = need_full ? 0 : 1;
+    // where the plan is built: in place on the caller's stream, or (overlap) in the other scratch set on the side
+    // stream, after the last kernel that read that set
+    int ps = c->cur_slot;
+    cudaStream_t st = caller;
+    if (c->overlap) {
+        ps = (c->cur_slot + 1) % PLAN_SLOTS;
+        st = c->side[c->side_next];
+        c->side_next ^= 1;
+        if (c->slot_used[ps]) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_free[ps], 0));
+    }
+    c->pb = c->slot_pb[ps];
+    c->cur_slot = ps;
+    if (prof_slot >= 0) cudaEventRecord(c->ev[prof_slot][0], st);
     // Hierarchical plan (plan_block.cuh) whenever a block of 8x8 tiles exists at this nside; the flat plan (one
     // scan slot and one fit per tile) serves nside < 256.
     const bool blocks = dw.k >= ARGUS_TILE_LOG2 + BLOCK_TILES_LOG2;
@@ -395,10 +442,15 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     {
         long long bound = tile_bound < c->pb.max_tiles ? tile_bound : c->pb.max_tiles;
         int gb = (int)((bound + 1023) / 1024);
-        plan_offsets_kernel<<<gb < 1 ? 1 : gb, 1024, 0, st>>>(c->pb, out_cap);
+        plan_offsets_kernel<<<gb < 1 ? 1 : gb, 256, 0, st>>>(c->pb, out_cap);
     }
     c->n_launches += 2;
     CUDA_TRY(c, cudaGetLastError());
+    if (prof_slot >= 0) cudaEventRecord(c->ev[prof_slot][1], st);
+    if (c->overlap) {
+        CUDA_TRY(c, cudaEventRecord(c->ev_done[ps], st));
+        CUDA_TRY(c, cudaStreamWaitEvent(caller, c->ev_done[ps], 0));
+    }
     c->dw = dw;
     c->key_wcs = *w;
     c->key_W = W; c->key_H = H; c->key_nside = nside;
@@ -408,6 +460,11 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
 }
 
 static bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+// The kernels just enqueued on `caller` read the current scratch set: a later plan into that set waits for them.
+static void mark_slot_read(argus_ctx* c, cudaStream_t caller) {
+    if (cudaEventRecord(c->ev_free[c->cur_slot], caller) == cudaSuccess) c->slot_used[c->cur_slot] = true;
+}
 
 static int make_frameargs(const argus_frame* fr, int64_t W, int64_t H, FrameArgs* f, bool* fused) {
     memset(f, 0, sizeof(*f));
@@ -469,7 +526,7 @@ extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64
     if (idx_out && !aligned(idx_out, 8)) return ARGUS_ERR_ALIGN;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
-    int rc = build_plan(c, wcs, W, H, nside, -1, st, true);
+    int rc = build_plan(c, wcs, W, H, nside, -1, st, true, -1);
     if (rc) return rc;
     rc = fetch_stats(c, st);
     if (rc) return rc;
@@ -597,15 +654,15 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     int slot = c->prof_n & 255;
     const bool use_fast = kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H);
     bool replanned = !(same_key(c, wcs, W, H, nside) && (c->plan_full || use_fast));
-    if (c->profile) cudaEventRecord(c->ev[slot][0], st);
-    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, !use_fast);
+    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, !use_fast, c->profile ? slot : -1);
     if (rc) return rc;
-    if (c->profile) cudaEventRecord(c->ev[slot][1], st);
+    if (c->profile) cudaEventRecord(c->ev[slot][2], st);
     CoaddArgs ca;
     memset(&ca, 0, sizeof(ca));
     rc = launch_tiles<false>(c, kernel, fused, use_fast, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
     if (rc) return rc;
-    if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
+    mark_slot_read(c, st);
+    if (c->profile) { cudaEventRecord(c->ev[slot][3], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
 }
@@ -662,13 +719,13 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     int slot = c->prof_n & 255;
     const bool use_fast = kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H);
     bool replanned = !(same_key(c, wcs, W, H, nside) && (c->plan_full || use_fast));
-    if (c->profile) cudaEventRecord(c->ev[slot][0], st);
-    rc = build_plan(c, wcs, W, H, nside, -1, st, !use_fast);
+    rc = build_plan(c, wcs, W, H, nside, -1, st, !use_fast, c->profile ? slot : -1);
     if (rc) return rc;
-    if (c->profile) cudaEventRecord(c->ev[slot][1], st);
+    if (c->profile) cudaEventRecord(c->ev[slot][2], st);
     rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
     if (rc) return rc;
-    if (c->profile) { cudaEventRecord(c->ev[slot][2], st); c->ev_plan[slot] = replanned; c->prof_n++; }
+    mark_slot_read(c, st);
+    if (c->profile) { cudaEventRecord(c->ev[slot][3], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
 }

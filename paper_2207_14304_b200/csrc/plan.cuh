@@ -256,7 +256,7 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
     }
 }
 
-#define FIT_WARPS 8
+#define FIT_WARPS 4
 __global__ void __launch_bounds__(32 * FIT_WARPS) plan_fit_kernel(DevWcs w, PlanBuffers pb, int use_list, int lite) {
     __shared__ double s_pinv[250];
     __shared__ double s_coef[FIT_WARPS][20];
@@ -451,16 +451,15 @@ __global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuff
 // Exclusive scan of the per-tile counts in one launch: block-local scan (1024 tiles per CTA, coalesced reads of
 // the compact count / class arrays); the last CTA to finish scans the per-CTA sums.
 // Output position of tile t = block_base[t >> 10] + tile_offset[t].
+// 256 threads per CTA (so that a CTA fits beside the resample kernel's CTAs), 4 consecutive tiles per thread.
 __device__ inline void offsets_final_body(const PlanBuffers& pb, long long out_capacity, long long* s_warp) {
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int n = *pb.n_tiles;
-    int nb = (n + 1023) >> 10;   // <= 1024 * 16 blocks (max_tiles <= 2^24): each thread handles up to 16
-    long long v[16], sum = 0;
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        int b = tid * 16 + j;
-        v[j] = (b < nb) ? (long long)__ldcg(pb.block_sum + b) : 0;
-        sum += v[j];
+    int nb = (n + 1023) >> 10;   // <= 16384 CTA sums (max_tiles <= 2^24): each of the 256 threads handles up to 64
+    long long sum = 0;
+    for (int j = 0; j < 64; ++j) {
+        int b = tid * 64 + j;
+        if (b < nb) sum += (long long)__ldcg(pb.block_sum + b);
     }
     long long inc = sum;
     for (int o = 1; o < 32; o <<= 1) {
@@ -469,67 +468,73 @@ __device__ inline void offsets_final_body(const PlanBuffers& pb, long long out_c
     }
     if (lane == 31) s_warp[wid] = inc;
     __syncthreads();
-    if (wid == 0) {
-        long long w = s_warp[lane], iw = w;
-        for (int o = 1; o < 32; o <<= 1) {
-            long long u = __shfl_up_sync(0xffffffffu, iw, o);
-            if (lane >= o) iw += u;
+    long long woff = 0, total = 0;
+    for (int i = 0; i < 8; ++i) { if (i < wid) woff += s_warp[i]; total += s_warp[i]; }
+    long long run = woff + inc - sum;
+    for (int j = 0; j < 64; ++j) {
+        int b = tid * 64 + j;
+        if (b < nb) {
+            pb.block_base[b] = run;
+            run += (long long)__ldcg(pb.block_sum + b);
         }
-        s_warp[lane] = iw - w;
     }
-    __syncthreads();
-    long long run = s_warp[wid] + inc - sum;
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        int b = tid * 16 + j;
-        if (b < nb) pb.block_base[b] = run;
-        run += v[j];
-    }
-    if (tid == 1023) {
+    if (tid == 0) {
         PlanStats* st = pb.stats;
-        st->n_footprint = run;
+        st->n_footprint = total;
         st->n_tiles = n;
-        if (out_capacity >= 0 && run > out_capacity) atomicOr(&st->overflow, 4);
+        if (out_capacity >= 0 && total > out_capacity) atomicOr(&st->overflow, 4);
     }
 }
 
-__global__ void __launch_bounds__(1024) plan_offsets_kernel(PlanBuffers pb, long long out_capacity) {
-    __shared__ int s_warp[32];
-    __shared__ long long s_warp64[32];
+__global__ void __launch_bounds__(256) plan_offsets_kernel(PlanBuffers pb, long long out_capacity) {
+    __shared__ int s_warp[8];
+    __shared__ long long s_warp64[8];
     __shared__ int s_last;
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int n = *pb.n_tiles;
-    int i = blockIdx.x * 1024 + tid;
+    int i0 = blockIdx.x * 1024 + 4 * tid;       // this thread's 4 consecutive tiles (arrays are 256-byte aligned)
     if (blockIdx.x * 1024 < n) {
-        int c = (i < n) ? pb.tile_count[i] : 0;
-        int cls = (i < n) ? pb.tile_cls[i] : -1;
-        int inc = c;
+        int4 c4 = make_int4(0, 0, 0, 0);
+        uchar4 k4 = make_uchar4(255, 255, 255, 255);
+        if (i0 + 3 < n) {
+            c4 = *reinterpret_cast<const int4*>(pb.tile_count + i0);
+            k4 = *reinterpret_cast<const uchar4*>(pb.tile_cls + i0);
+        } else {
+            if (i0 < n) { c4.x = pb.tile_count[i0]; k4.x = pb.tile_cls[i0]; }
+            if (i0 + 1 < n) { c4.y = pb.tile_count[i0 + 1]; k4.y = pb.tile_cls[i0 + 1]; }
+            if (i0 + 2 < n) { c4.z = pb.tile_count[i0 + 2]; k4.z = pb.tile_cls[i0 + 2]; }
+        }
+        int c = c4.x + c4.y + c4.z + c4.w, inc = c;
         for (int o = 1; o < 32; o <<= 1) {
             int v = __shfl_up_sync(0xffffffffu, inc, o);
             if (lane >= o) inc += v;
         }
         if (lane == 31) s_warp[wid] = inc;
-        unsigned m_in = __ballot_sync(0xffffffffu, cls == TC_INSIDE), m_bo = __ballot_sync(0xffffffffu, cls == TC_BORDER);
-        unsigned m_ex = __ballot_sync(0xffffffffu, cls == TC_EXACT), m_em = __ballot_sync(0xffffffffu, cls == TC_EMPTY);
+        int n_in = (k4.x == TC_INSIDE) + (k4.y == TC_INSIDE) + (k4.z == TC_INSIDE) + (k4.w == TC_INSIDE);
+        int n_bo = (k4.x == TC_BORDER) + (k4.y == TC_BORDER) + (k4.z == TC_BORDER) + (k4.w == TC_BORDER);
+        int n_ex = (k4.x == TC_EXACT) + (k4.y == TC_EXACT) + (k4.z == TC_EXACT) + (k4.w == TC_EXACT);
+        int n_em = (k4.x == TC_EMPTY) + (k4.y == TC_EMPTY) + (k4.z == TC_EMPTY) + (k4.w == TC_EMPTY);
+        n_in = __reduce_add_sync(0xffffffffu, n_in); n_bo = __reduce_add_sync(0xffffffffu, n_bo);
+        n_ex = __reduce_add_sync(0xffffffffu, n_ex); n_em = __reduce_add_sync(0xffffffffu, n_em);
         if (lane == 0) {
             PlanStats* st = pb.stats;
-            if (m_in) atomicAdd((unsigned long long*)&st->n_inside, (unsigned long long)__popc(m_in));
-            if (m_bo) atomicAdd((unsigned long long*)&st->n_border, (unsigned long long)__popc(m_bo));
-            if (m_ex) atomicAdd((unsigned long long*)&st->n_exact, (unsigned long long)__popc(m_ex));
-            if (m_em) atomicAdd((unsigned long long*)&st->n_empty, (unsigned long long)__popc(m_em));
+            if (n_in) atomicAdd((unsigned long long*)&st->n_inside, (unsigned long long)n_in);
+            if (n_bo) atomicAdd((unsigned long long*)&st->n_border, (unsigned long long)n_bo);
+            if (n_ex) atomicAdd((unsigned long long*)&st->n_exact, (unsigned long long)n_ex);
+            if (n_em) atomicAdd((unsigned long long*)&st->n_empty, (unsigned long long)n_em);
         }
         __syncthreads();
-        if (wid == 0) {
-            int v = s_warp[lane], iv = v;
-            for (int o = 1; o < 32; o <<= 1) {
-                int u = __shfl_up_sync(0xffffffffu, iv, o);
-                if (lane >= o) iv += u;
-            }
-            s_warp[lane] = iv - v;
-            if (lane == 31) pb.block_sum[blockIdx.x] = iv;
+        int woff = 0, tot = 0;
+        for (int i = 0; i < 8; ++i) { if (i < wid) woff += s_warp[i]; tot += s_warp[i]; }
+        if (tid == 0) pb.block_sum[blockIdx.x] = tot;
+        int ex = woff + inc - c;
+        if (i0 + 3 < n) {
+            *reinterpret_cast<int4*>(pb.tile_offset + i0) = make_int4(ex, ex + c4.x, ex + c4.x + c4.y, ex + c4.x + c4.y + c4.z);
+        } else {
+            if (i0 < n) pb.tile_offset[i0] = ex;
+            if (i0 + 1 < n) pb.tile_offset[i0 + 1] = ex + c4.x;
+            if (i0 + 2 < n) pb.tile_offset[i0 + 2] = ex + c4.x + c4.y;
         }
-        __syncthreads();
-        if (i < n) pb.tile_offset[i] = s_warp[wid] + inc - c;
     }
     // the last CTA to arrive scans the per-CTA sums (block_base) and closes the statistics
     __threadfence();

@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(32 * BFIT_WARPS) plan_blockfit_kernel(DevWcs w
 // ----------------------------------------------------------------------------------------- tilegen
 // One thread per tile: re-expansion of the block quartic about the tile centre, extent from the tile corners,
 // classification, tile records.  Tiles of blocks without a fit go to the per-tile fit list.
-__global__ void __launch_bounds__(128) plan_tilegen_kernel(DevWcs w, PlanBuffers pb, int lite) {
+__global__ void __launch_bounds__(128, 4) plan_tilegen_kernel(DevWcs w, PlanBuffers pb, int lite) {
     __shared__ double s_bc[2][32];
     const int tid = threadIdx.x;
     const int n_blocks = *pb.n_blocks;

@@ -142,7 +142,9 @@ __device__ __forceinline__ float fast_frac(int xf) {
 
 // ------------------------------------------------------------------------------------------ kernel
 template <bool COADD>
-__global__ void __launch_bounds__(RF_THREADS, RF_CTAS_PER_SM)
+// 80 registers: two CTAs leave 19 K registers per SM free, enough for one CTA of any plan kernel -- the plan of the
+// next frame runs on a side stream underneath this kernel (argus_api.cu, ARGUS_OPT_PLAN_OVERLAP)
+__global__ void __maxnreg__(80)
     resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, FrameArgs f, int W, int H, float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
                          CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
