@@ -24,6 +24,7 @@ struct argus_ctx {
     bool plan_cache;
     bool plan_valid;
     bool plan_full;       // the cached plan holds TileRec / FP64 coefficients for every tile (general kernel)
+    int plan_fast_kernel; // interpolation kernel whose tap apron sized the fast kernel's boxes in the cached plan (-1: none)
     argus_wcs key_wcs;
     int64_t key_W, key_H, key_nside;
     DevWcs dw;
@@ -241,6 +242,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
 extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (!c) return ARGUS_ERR_NULL;
     cudaSetDevice(c->device);
+    for (int i = 0; i < 2; ++i) cudaStreamSynchronize(c->side[i]);   // plans still running underneath the caller's kernels
     for (int i = 0; i < 256; ++i)
         for (int j = 0; j < 4; ++j) cudaEventDestroy(c->ev[i][j]);
     for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
@@ -368,13 +370,19 @@ static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t 
 }
 
 // Enqueue the plan kernels (A0 + A1).  No host synchronisation.
+static bool plan_usable(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, bool need_full, int fast_kernel) {
+    return same_key(c, w, W, H, nside) && (need_full ? c->plan_full : c->plan_fast_kernel == fast_kernel);
+}
+
+// fast_kernel: interpolation kernel the fast (TMA-staged) kernel will run with, -1 = general kernel only (full plan).
 static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
-                      cudaStream_t caller, bool need_full, int prof_slot) {
+                      cudaStream_t caller, int fast_kernel, int prof_slot) {
+    const bool need_full = fast_kernel < 0;
     DevWcs dw;
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
     if (rc) return rc;
-    if (same_key(c, w, W, H, nside) && (c->plan_full || !need_full)) return ARGUS_OK;
+    if (plan_usable(c, w, W, H, nside, need_full, fast_kernel)) return ARGUS_OK;
     c->plan_valid = false;
     const int lite = need_full ? 0 : 1;
     // where the plan is built: in place on the caller's stream, or (overlap) in the other scratch set on the side
@@ -389,6 +397,12 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     }
     c->pb = c->slot_pb[ps];
     c->cur_slot = ps;
+    {   // tap apron and stage capacity the fast kernel's boxes are sized for (a full plan keeps bilinear boxes)
+        const int fk = fast_kernel == ARGUS_LANCZOS3 ? 1 : 0;
+        c->pb.fast_tl = fk ? FastCfg<1>::TL : FastCfg<0>::TL;
+        c->pb.fast_tr = fk ? FastCfg<1>::TR : FastCfg<0>::TR;
+        c->pb.fast_cap = fk ? FastCfg<1>::CAP : FastCfg<0>::CAP;
+    }
     if (prof_slot >= 0) cudaEventRecord(c->ev[prof_slot][0], st);
     // Hierarchical plan (plan_block.cuh) whenever a block of 8x8 tiles exists at this nside; the flat plan (one
     // scan slot and one fit per tile) serves nside < 256.
@@ -456,6 +470,7 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     c->key_W = W; c->key_H = H; c->key_nside = nside;
     c->plan_valid = true;
     c->plan_full = need_full;
+    c->plan_fast_kernel = need_full ? ARGUS_BILINEAR : fast_kernel;
     return ARGUS_OK;
 }
 
@@ -526,7 +541,7 @@ extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64
     if (idx_out && !aligned(idx_out, 8)) return ARGUS_ERR_ALIGN;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
-    int rc = build_plan(c, wcs, W, H, nside, -1, st, true, -1);
+    int rc = build_plan(c, wcs, W, H, nside, -1, st, -1, -1);
     if (rc) return rc;
     rc = fetch_stats(c, st);
     if (rc) return rc;
@@ -604,12 +619,18 @@ static int launch_tiles(argus_ctx* c, int kernel, bool fused, bool use_fast, con
     if (use_fast) {
         // TMA-staged hot kernel for every tile that fits a stage; the general kernel takes the rest
         if (!c->fast_attr_set) {
-            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
-            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<0>)));
+            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<0>)));
+            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<1>)));
+            CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<1>)));
             c->fast_attr_set = true;
         }
-        resample_fast_kernel<COADD><<<c->sm_count * RF_CTAS_PER_SM, RF_THREADS, sizeof(FastSmem), st>>>(
-            c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
+        if (kernel == ARGUS_BILINEAR)
+            resample_fast_kernel<COADD, 0><<<c->sm_count * FastCfg<0>::CTAS, RF_THREADS, sizeof(FastSmem<0>), st>>>(
+                c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
+        else
+            resample_fast_kernel<COADD, 1><<<c->sm_count * FastCfg<1>::CTAS, RF_THREADS, sizeof(FastSmem<1>), st>>>(
+                c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
         c->n_launches++;
         slow_only = 1;
         grid = c->sm_count * 2;
@@ -652,9 +673,9 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
         return ARGUS_OK;
     }
     int slot = c->prof_n & 255;
-    const bool use_fast = kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H);
-    bool replanned = !(same_key(c, wcs, W, H, nside) && (c->plan_full || use_fast));
-    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, !use_fast, c->profile ? slot : -1);
+    const bool use_fast = fused && fast_maps(c, f, W, H);
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !use_fast, kernel);
+    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, use_fast ? kernel : -1, c->profile ? slot : -1);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
     CoaddArgs ca;
@@ -717,9 +738,9 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
     int slot = c->prof_n & 255;
-    const bool use_fast = kernel == ARGUS_BILINEAR && fused && fast_maps(c, f, W, H);
-    bool replanned = !(same_key(c, wcs, W, H, nside) && (c->plan_full || use_fast));
-    rc = build_plan(c, wcs, W, H, nside, -1, st, !use_fast, c->profile ? slot : -1);
+    const bool use_fast = fused && fast_maps(c, f, W, H);
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !use_fast, kernel);
+    rc = build_plan(c, wcs, W, H, nside, -1, st, use_fast ? kernel : -1, c->profile ? slot : -1);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
     rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);

@@ -61,8 +61,9 @@ struct __align__(16) TileRec {
 #define FAST_FRAC_BITS 22
 #define FAST_MAGIC_F 12582912.0f          // 1.5 * 2^23
 #define FAST_MAGIC_I 0x4B400000
-#define FAST_CAP_PX 3584                  // staged source pixels per tile (box width x rows padded to 8)
-#define FAST_CAL_FLOATS 4096              // calibrated box (rows x bank-conflict-free pitch)
+#define FAST_CAP_PX 3584                  // bilinear: staged source pixels per tile (box width x box rows), 2 stages
+#define FAST_CAP_PX_LZ 4608               // Lanczos-3 (6x6 taps: 5 more rows and columns), 1 stage
+                                          // the calibrated box (rows x bank-conflict-free pitch) may use cap * 9/8 floats
 struct __align__(16) FastRec {
     int cls;             // TC_INSIDE / TC_BORDER when the tile is handled by the fast kernel, else 0
     int mask_slot;       // TC_BORDER: row of the membership-mask array

@@ -46,6 +46,7 @@ struct PlanBuffers {
     double* pinv4;              // [15][25] pseudo-inverse of the quartic design matrix on the 5x5 node grid
     double* bcoef;              // [max_tiles/64][32] block quartics (15 x, 15 y), [30] = zone or -1 (no block fit)
     int max_slots, max_tiles, max_hard;
+    int fast_tl, fast_tr, fast_cap;   // tap apron and stage capacity (pixels) of the fast kernel this plan is for
 };
 
 // --------------------------------------------------------------------------------------------- scan
@@ -139,22 +140,24 @@ __device__ inline void cubic_basis(double S, double T, double m[10]) {
     m[6] = S * S * S; m[7] = S * S * T; m[8] = S * T * T; m[9] = T * T * T;
 }
 
-// Staged-box geometry of the fast kernel for cells [bx0, bx1] x [by0, by1] (+1 bilinear tap).  The TMA box must
-// start on a 16-byte boundary of every array (8 pixels of the uint16 frame), so the origin is aligned down to 8;
-// widths come in steps of 8 px (40..72), heights are 48, 56 or 64 rows (a TMA copy costs ~100 cycles per
-// operation whatever its size, so each array is fetched with ONE box).  Returns false when the box does not fit its shared-memory stage.
+// Staged-box geometry of the fast kernel for cells [bx0, bx1] x [by0, by1] plus the interpolation kernel's taps
+// (tl to the left / above, tr to the right / below: 0, 1 bilinear; 2, 3 Lanczos-3).  The TMA box must start on a
+// 16-byte boundary of every array (8 pixels of the uint16 frame), so the origin is aligned down to 8; widths come in
+// steps of 8 px (40..72), heights are 48, 56 or 64 rows (a TMA copy costs ~100 cycles per operation whatever its
+// size, so each array is fetched with ONE box).  Returns false when the box does not fit the kernel's stage.
 __device__ __host__ inline int fast_cal_pitch(int boxw) { return (boxw & 15) == 8 ? boxw : boxw + 8; }   // = 8 or 24 mod 32
-__device__ inline bool fast_box(int bx0, int bx1, int by0, int by1, int X0, int Y0, FastRec& f) {
-    int gx0 = bx0 & ~7;
-    int bw = bx1 + 2 - gx0, bh = by1 - by0 + 2;
+__device__ inline bool fast_box(const PlanBuffers& pb, int bx0, int bx1, int by0, int by1, int X0, int Y0, FastRec& f) {
+    const int tl = pb.fast_tl, tr = pb.fast_tr;
+    int gx0 = (bx0 - tl) & ~7, gy0 = by0 - tl;
+    int bw = bx1 + tr + 1 - gx0, bh = by1 + tr + 1 - gy0;
     if (bw < 1 || bh < 1 || bw > 72 || bh > 64) return false;
     int wclass = bw <= 40 ? 0 : (bw - 40 + 7) >> 3;
     int boxw = 40 + 8 * wclass, pitch = fast_cal_pitch(boxw);
-    int hclass = bh <= 48 ? 0 : (bh <= 56 ? 1 : 2);      // one TMA box per array: 48, 56 or 64 rows
-    if ((48 + 8 * hclass) * boxw > FAST_CAP_PX || bh * pitch > FAST_CAL_FLOATS) return false;
-    if (gx0 < X0 || by0 < Y0 || bx1 + 2 - X0 > 500 || by1 + 2 - Y0 > 500) return false;
-    f.gx0 = gx0; f.gy0 = by0; f.wclass = wclass | (hclass << 4); f.bh = bh;
-    f.kofs = (Y0 - by0) * pitch + (X0 - gx0);
+    int hclass = bh <= 48 ? 0 : (bh <= 56 ? 1 : 2);
+    if ((48 + 8 * hclass) * boxw > pb.fast_cap || bh * pitch > pb.fast_cap + pb.fast_cap / 8) return false;
+    if (bx0 < X0 || by0 < Y0 || bx1 + 4 - X0 > 500 || by1 + 4 - Y0 > 500) return false;
+    f.gx0 = gx0; f.gy0 = gy0; f.wclass = wclass | (hclass << 4); f.bh = bh;
+    f.kofs = (Y0 - gy0) * pitch + (X0 - gx0);
     return true;
 }
 
@@ -237,7 +240,7 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
         f.mask_slot = r.mask_slot;
         f.poly_ok = poly_ok ? 1 : 0;
         if (cls == TC_INSIDE) {
-            if (poly_ok && fast_box(r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) { f.cls = TC_INSIDE; fast_inside = true; }
+            if (poly_ok && fast_box(pb, r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) { f.cls = TC_INSIDE; fast_inside = true; }
             else slow_push(pb, t);
         }   // TC_BORDER: plan_members_kernel finalises the box and decides
         if (!(lite && fast_inside)) {
@@ -435,7 +438,7 @@ __global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuff
                 if (cls == TC_BORDER) {
                     FastRec* fr = &pb.frec[t];
                     FastRec f = *fr;
-                    if (f.poly_ok && fast_box(e0, e1, e2, e3, f.X0, f.Y0, f)) {
+                    if (f.poly_ok && fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f)) {
                         f.cls = TC_BORDER;
                         *fr = f;
                     } else {

@@ -22,13 +22,15 @@
 #define RF_CONSUMERS 256                 // threads of one consumer group (one output tile at a time): 256 or 512
 #endif
 #define RF_NQ (ARGUS_TILE_PIX / RF_CONSUMERS)   // output pixels per thread
-#define RF_NI ((FAST_CAP_PX / 4 + RF_CONSUMERS - 1) / RF_CONSUMERS)   // calibration items (float4) per thread
-#ifndef RF_GROUPS
 #define RF_GROUPS 1                      // consumer groups per CTA, tiles dealt round-robin
-#define RF_CTAS_PER_SM 2
-#define RF_STAGES 2                      // TMA stages shared by the groups: more than groups => loads run ahead
-#endif
 #define RF_THREADS (RF_GROUPS * RF_CONSUMERS + 32)
+
+// Per interpolation kernel: stage capacity, stages per CTA, CTAs per SM, register cap.
+//   bilinear : 2 stages x 50 KB, 2 CTAs / SM, 80 registers (leaves room for a plan CTA beside it, argus_api.cu)
+//   Lanczos-3: the gather dominates (36 taps, 12 kernel weights per pixel): 1 stage x 64.5 KB, 3 CTAs / SM
+template <int KERNEL> struct FastCfg;
+template <> struct FastCfg<0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1; };
+template <> struct FastCfg<1> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3; };
 
 struct FastMaps {
     CUtensorMap m[3][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
@@ -45,20 +47,21 @@ struct __align__(16) FastDesc {
 
 // One stage: the raw + master boxes as the TMA delivers them (dense, pitch = box width).  After the consumers have
 // read them into registers, the calibrated box overwrites the stage from `bias` on (pitch 8 or 24 mod 32 floats,
-// up to FAST_CAL_FLOATS floats = bias + the head of dark).
+// up to CAP * 9/8 floats = bias + the head of dark).
+template <int CAP>
 struct __align__(128) FastStage {
-    unsigned short raw[FAST_CAP_PX];
-    float bias[FAST_CAP_PX];
-    float dark[FAST_CAP_PX];
-    float flat[FAST_CAP_PX];
+    unsigned short raw[CAP];
+    float bias[CAP];
+    float dark[CAP];
+    float flat[CAP];
 };
+template <int KERNEL>
 struct __align__(128) FastSmem {
-    FastStage stage[RF_STAGES];
-    FastDesc desc[RF_STAGES];
-    unsigned long long full[RF_STAGES];    // TMA bytes of the stage have landed (1 arrival + tx)
-    unsigned long long empty[RF_STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
+    FastStage<FastCfg<KERNEL>::CAP> stage[FastCfg<KERNEL>::STAGES];
+    FastDesc desc[FastCfg<KERNEL>::STAGES];
+    unsigned long long full[FastCfg<KERNEL>::STAGES];    // TMA bytes of the stage have landed (1 arrival + tx)
+    unsigned long long empty[FastCfg<KERNEL>::STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
 };
-static_assert(FAST_CAL_FLOATS <= 2 * FAST_CAP_PX, "calibrated box must fit bias + dark");
 
 // ---------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -140,15 +143,101 @@ __device__ __forceinline__ float fast_frac(int xf) {
     return fmaf(__uint_as_float(((unsigned)xf & 0x3fffffu) | 0x4B000000u), 2.384185791015625e-07f, -2.0f);
 }
 
+// ------------------------------------------------------------------------------------ interpolation
+// Lanczos-3 weights of the six taps at offsets t_q = f + 2 - q (q = 0..5) for the fraction f in [0, 1):
+// L(t) = sin(pi t) sin(pi t / 3) * 3 / (pi t)^2.  FP32 with bounded RELATIVE error (~3e-7) on every weight, which is
+// what the value tolerance needs next to bright taps: every argument is reduced EXACTLY before any
+// rounding (f is a multiple of 2^-22, so f + n and 1 - f are exact), and the three distinct sines are reused:
+//   sin(pi t/3): q0  sin(pi (1-f)/3),  q1  cos(pi (2f-1)/6),  q2  sin(pi f/3),  q3 = -q0,  q4 = -q1,  q5 = -q2
+//   sin(pi t)  : (-1)^q sin(pi f)
+__device__ __forceinline__ void lanczos3_weights_f32(float f, float k[6]) {
+    if (f == 0.0f) { k[0] = k[1] = k[3] = k[4] = k[5] = 0.0f; k[2] = 1.0f; return; }
+    const float s1 = sinpif(f);
+    const float A = sinpif((1.0f - f) * 0.33333334f), B = cospif((2.0f * f - 1.0f) * 0.16666667f), C = sinpif(f * 0.33333334f);
+    const float c3 = 0.30396355092701331f * s1;                 // 3 / pi^2
+    const float t0 = f + 2.0f, t1 = f + 1.0f, t3 = f - 1.0f, t4 = f - 2.0f, t5 = f - 3.0f;
+    k[0] = c3 * A * __frcp_rn(t0 * t0);
+    k[1] = -c3 * B * __frcp_rn(t1 * t1);
+    k[2] = c3 * C * __frcp_rn(f * f);
+    k[3] = c3 * A * __frcp_rn(t3 * t3);
+    k[4] = -c3 * B * __frcp_rn(t4 * t4);
+    k[5] = c3 * C * __frcp_rn(t5 * t5);
+}
+
+// No masked tap in the tile's box: weight == 1.  a = address of the cell (floor x, floor y) in the calibrated box.
+template <int KERNEL>
+__device__ __forceinline__ float interp_clean(const float* __restrict__ a, int pitch, float fx, float fy) {
+    if (KERNEL == 0) {
+        const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];
+        const float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);
+        return fmaf(fy, bot - top, top);
+    } else {
+        float kx[6], ky[6];
+        lanczos3_weights_f32(fx, kx);
+        lanczos3_weights_f32(fy, ky);
+        const float* r = a - 2 * pitch - 2;
+        float V = 0.0f;
+#pragma unroll
+        for (int b = 0; b < 6; ++b) {
+            float rs = kx[0] * r[0];
+#pragma unroll
+            for (int q = 1; q < 6; ++q) rs = fmaf(kx[q], r[q], rs);
+            V = fmaf(ky[b], rs, V);
+            r += pitch;
+        }
+        const float sx = ((kx[0] + kx[5]) + (kx[1] + kx[4])) + (kx[2] + kx[3]);
+        const float sy = ((ky[0] + ky[5]) + (ky[1] + ky[4])) + (ky[2] + ky[3]);
+        return V / (sx * sy);
+    }
+}
+
+// Masked, normalised form (NaN = masked tap): S0 = sum k, B = sum k over masked taps, V1 = sum k c over good taps.
+template <int KERNEL>
+__device__ __forceinline__ void interp_masked(const float* __restrict__ a, int pitch, float fx, float fy, float w_min,
+                                              float& val, float& wgt) {
+    float S = 0.0f, B = 0.0f, V1 = 0.0f;
+    if (KERNEL == 0) {
+        const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];
+        const float gx = 1.0f - fx, gy = 1.0f - fy;
+        const float k00 = gx * gy, k01 = fx * gy, k10 = gx * fy, k11 = fx * fy;
+        S = (k00 + k01) + (k10 + k11);
+        if (c00 == c00) V1 = fmaf(k00, c00, V1); else B += k00;
+        if (c01 == c01) V1 = fmaf(k01, c01, V1); else B += k01;
+        if (c10 == c10) V1 = fmaf(k10, c10, V1); else B += k10;
+        if (c11 == c11) V1 = fmaf(k11, c11, V1); else B += k11;
+    } else {
+        float kx[6], ky[6];
+        lanczos3_weights_f32(fx, kx);
+        lanczos3_weights_f32(fy, ky);
+        const float* r = a - 2 * pitch - 2;
+#pragma unroll 1
+        for (int b = 0; b < 6; ++b) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                const float k = kx[q] * ky[b], c = r[q];
+                S += k;
+                if (c == c) V1 = fmaf(k, c, V1); else B += k;
+            }
+            r += pitch;
+        }
+    }
+    const float w = 1.0f - B / S;
+    val = 0.f; wgt = 0.f;
+    if (!(w < w_min) && (S - B > 0.f)) { val = V1 / (S - B); wgt = fminf(w, 1.0f); }
+}
+
 // ------------------------------------------------------------------------------------------ kernel
-template <bool COADD>
-// 80 registers: two CTAs leave 19 K registers per SM free, enough for one CTA of any plan kernel -- the plan of the
-// next frame runs on a side stream underneath this kernel (argus_api.cu, ARGUS_OPT_PLAN_OVERLAP)
-__global__ void __maxnreg__(80)
+// Bilinear, 80 registers: two CTAs leave 19 K registers per SM free, enough for one CTA of any plan kernel -- the plan
+// of the next frame runs on a side stream underneath this kernel (argus_api.cu, ARGUS_OPT_PLAN_OVERLAP).
+template <bool COADD, int KERNEL>
+__global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
     resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, FrameArgs f, int W, int H, float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
                          CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    FastSmem& sm = *reinterpret_cast<FastSmem*>(smem_raw);
+    typedef FastCfg<KERNEL> Cfg;
+    constexpr int RF_STAGES = Cfg::STAGES;
+    constexpr int RF_NI = (Cfg::CAP / 4 + RF_CONSUMERS - 1) / RF_CONSUMERS;   // calibration items (float4) per thread
+    FastSmem<KERNEL>& sm = *reinterpret_cast<FastSmem<KERNEL>*>(smem_raw);
     const int tid = threadIdx.x;
     const int n_tiles = *pb.n_tiles;
     const float t_exp = f.t_exp, flat_min = f.flat_min;
@@ -220,7 +309,7 @@ __global__ void __maxnreg__(80)
                 if (lane == 0) {
 #endif
                     const CUtensorMap* mp = &maps.m[hc][wc][0];
-                    FastStage& sg = sm.stage[slot];
+                    FastStage<Cfg::CAP>& sg = sm.stage[slot];
                     tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[slot]);
                     tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[slot]);
                     tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[slot]);
@@ -298,7 +387,7 @@ __global__ void __maxnreg__(80)
         mbar_arrive(&sm.empty[slot]);
         continue;
 #endif
-        FastStage& sg = sm.stage[slot];
+        FastStage<Cfg::CAP>& sg = sm.stage[slot];
         float* cal = sg.bias;
         const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
         // every column of the box is calibrated: restricting the items to the tap columns made the 128-bit shared
@@ -362,12 +451,9 @@ __global__ void __maxnreg__(80)
 #define RF_HOT(Q)                                                                            \
     {                                                                                        \
         const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);    \
-        const float fx = fast_frac(xf), fy = fast_frac(yf);                                  \
-        const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));      \
-        const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];                \
-        const float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);          \
-        vp[RF_CONSUMERS * Q] = fmaf(fy, bot - top, top);                                              \
-        wp[RF_CONSUMERS * Q] = 1.0f;                                                                  \
+        const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));     \
+        vp[RF_CONSUMERS * Q] = interp_clean<KERNEL>(a, pitch, fast_frac(xf), fast_frac(yf)); \
+        wp[RF_CONSUMERS * Q] = 1.0f;                                                         \
     }
             RF_HOT(0) RF_HOT(1)
 #if RF_NQ == 4
@@ -389,20 +475,9 @@ __global__ void __maxnreg__(80)
         }                                                                                                  \
         if (member) {                                                                                      \
             const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);              \
-            const float fx = fast_frac(xf), fy = fast_frac(yf);                                            \
-            const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));                \
-            const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];                          \
-            const float gx = 1.0f - fx, gy = 1.0f - fy;                                                    \
-            const float k00 = gx * gy, k01 = fx * gy, k10 = gx * fy, k11 = fx * fy;                        \
-            const float S = (k00 + k01) + (k10 + k11);                                                     \
-            float B = 0.f, V1 = 0.f;                                                                       \
-            if (c00 == c00) V1 = fmaf(k00, c00, V1); else B += k00;                                        \
-            if (c01 == c01) V1 = fmaf(k01, c01, V1); else B += k01;                                        \
-            if (c10 == c10) V1 = fmaf(k10, c10, V1); else B += k10;                                        \
-            if (c11 == c11) V1 = fmaf(k11, c11, V1); else B += k11;                                        \
-            const float w = 1.0f - B / S;                                                                  \
-            float val = 0.f, wgt = 0.f;                                                                    \
-            if (!(w < w_min) && (S - B > 0.f)) { val = V1 / (S - B); wgt = fminf(w, 1.0f); }               \
+            const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));               \
+            float val, wgt;                                                                                \
+            interp_masked<KERNEL>(a, pitch, fast_frac(xf), fast_frac(yf), w_min, val, wgt);                \
             if (COADD) {                                                                                   \
                 if (cslot >= 0) {                                                                          \
                     ca.sum[cslot + m] = fmaf(wgt, val, ca.sum[cslot + m]);                                 \
