@@ -24,7 +24,7 @@ struct argus_ctx {
     bool plan_cache;
     bool plan_valid;
     bool plan_full;       // the cached plan holds TileRec / FP64 coefficients for every tile (general kernel)
-    int plan_fast_kernel; // interpolation kernel whose tap apron sized the fast kernel's boxes in the cached plan (-1: none)
+    int plan_fast_kernel; // interpolation kernel whose tap apron sized the fast kernel's boxes in the cached plan
     argus_wcs key_wcs;
     int64_t key_W, key_H, key_nside;
     DevWcs dw;
@@ -371,13 +371,16 @@ static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t 
 
 // Enqueue the plan kernels (A0 + A1).  No host synchronisation.
 static bool plan_usable(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, bool need_full, int fast_kernel) {
-    return same_key(c, w, W, H, nside) && (need_full ? c->plan_full : c->plan_fast_kernel == fast_kernel);
+    // the fast kernel's boxes are sized for one interpolation kernel's taps; the general kernel does not care
+    return same_key(c, w, W, H, nside) && (!need_full || c->plan_full) &&
+           (fast_kernel < 0 || c->plan_fast_kernel == (fast_kernel == ARGUS_LANCZOS3 ? 1 : 0));
 }
 
 // fast_kernel: interpolation kernel the fast (TMA-staged) kernel will run with, -1 = general kernel only (full plan).
 static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
                       cudaStream_t caller, int fast_kernel, int prof_slot) {
-    const bool need_full = fast_kernel < 0;
+    // Lanczos-3: any tile may be handed to the general kernel at run time (masked pixels in its box) => full records
+    const bool need_full = fast_kernel != ARGUS_BILINEAR;
     DevWcs dw;
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
@@ -470,7 +473,7 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     c->key_W = W; c->key_H = H; c->key_nside = nside;
     c->plan_valid = true;
     c->plan_full = need_full;
-    c->plan_fast_kernel = need_full ? ARGUS_BILINEAR : fast_kernel;
+    c->plan_fast_kernel = fast_kernel == ARGUS_LANCZOS3 ? 1 : 0;
     return ARGUS_OK;
 }
 
@@ -674,7 +677,7 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     }
     int slot = c->prof_n & 255;
     const bool use_fast = fused && fast_maps(c, f, W, H);
-    bool replanned = !plan_usable(c, wcs, W, H, nside, !use_fast, kernel);
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1);
     rc = build_plan(c, wcs, W, H, nside, (long long)n, st, use_fast ? kernel : -1, c->profile ? slot : -1);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
@@ -739,7 +742,7 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     CUDA_TRY(c, cudaSetDevice(c->device));
     int slot = c->prof_n & 255;
     const bool use_fast = fused && fast_maps(c, f, W, H);
-    bool replanned = !plan_usable(c, wcs, W, H, nside, !use_fast, kernel);
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1);
     rc = build_plan(c, wcs, W, H, nside, -1, st, use_fast ? kernel : -1, c->profile ? slot : -1);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);

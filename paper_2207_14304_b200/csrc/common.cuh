@@ -54,11 +54,11 @@ struct __align__(16) TileRec {
 
 // Compact per-tile record of the TMA-staged bilinear kernel (resample_fast.cuh): 40 words = 10 x 16 B.
 // Source position of the output pixel with doubled centred offsets (s, t) (odd integers in [-31, 31]),
-// in units of 2^-22 px relative to the integer base (X0, Y0):
-//   xf = c0x + ax*s + bx*t + float_as_int( P_x(s/32, t/32) )      (P_x already scaled by 2^22 and offset by
-//   the 1.5*2^23 rounding constant, which c0x compensates);  cell = X0 + (xf >> 22), frac = (xf & (2^22-1)) 2^-22.
-// The linear part is exact integer arithmetic; only the remainder (|.| < 0.9 px) is FP32.
-#define FAST_FRAC_BITS 22
+// in units of 2^-24 px relative to the integer base (X0, Y0):
+//   xf = c0x + ax*s + bx*t + float_as_int( P_x(s/32, t/32) )      (P_x already scaled by 2^24 and offset by
+//   the 1.5*2^23 rounding constant, which c0x compensates);  cell = X0 + (xf >> 24), frac = (xf & (2^24-1)) 2^-24.
+// The linear part is exact integer arithmetic; only the remainder (|.| < 0.22 px) is FP32.
+#define FAST_FRAC_BITS 24
 #define FAST_MAGIC_F 12582912.0f          // 1.5 * 2^23
 #define FAST_MAGIC_I 0x4B400000
 #define FAST_CAP_PX 3584                  // bilinear: staged source pixels per tile (box width x box rows), 2 stages

@@ -155,7 +155,7 @@ __device__ inline bool fast_box(const PlanBuffers& pb, int bx0, int bx1, int by0
     int boxw = 40 + 8 * wclass, pitch = fast_cal_pitch(boxw);
     int hclass = bh <= 48 ? 0 : (bh <= 56 ? 1 : 2);
     if ((48 + 8 * hclass) * boxw > pb.fast_cap || bh * pitch > pb.fast_cap + pb.fast_cap / 8) return false;
-    if (bx0 < X0 || by0 < Y0 || bx1 + 4 - X0 > 500 || by1 + 4 - Y0 > 500) return false;
+    if (bx0 < X0 || by0 < Y0 || bx1 + 4 - X0 > 110 || by1 + 4 - Y0 > 110) return false;
     f.gx0 = gx0; f.gy0 = gy0; f.wclass = wclass | (hclass << 4); f.bh = bh;
     f.kofs = (Y0 - gy0) * pitch + (X0 - gx0);
     return true;
@@ -224,16 +224,16 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
             const double* ca = c + 10 * axis;
             int base = (axis ? r.by0 : r.bx0) - 8;
             double c0l = ca[0] - (double)base;
-            int c0f = (int)rint(c0l * 4194304.0);
-            int af = (int)rint(ca[1] * 131072.0), bf = (int)rint(ca[2] * 131072.0);   // c/32 * 2^22
+            int c0f = (int)rint(c0l * 16777216.0);
+            int af = (int)rint(ca[1] * 524288.0), bf = (int)rint(ca[2] * 524288.0);   // c/32 * 2^24
             float* pp = axis ? f.py : f.px;
-            pp[0] = (float)(12582912.0 + (c0l * 4194304.0 - (double)c0f));
-            pp[1] = (float)((ca[1] * 131072.0 - (double)af) * 32.0);
-            pp[2] = (float)((ca[2] * 131072.0 - (double)bf) * 32.0);
+            pp[0] = (float)(12582912.0 + (c0l * 16777216.0 - (double)c0f));
+            pp[1] = (float)((ca[1] * 524288.0 - (double)af) * 32.0);
+            pp[2] = (float)((ca[2] * 524288.0 - (double)bf) * 32.0);
             double mag = fabs((double)pp[1]) + fabs((double)pp[2]);
 #pragma unroll
-            for (int i = 3; i < 10; ++i) { pp[i] = (float)(ca[i] * 4194304.0); mag += fabs((double)pp[i]); }
-            if (!(mag < 0.9 * 4194304.0) || !(fabs(c0l) < 400.0)) poly_ok = false;
+            for (int i = 3; i < 10; ++i) { pp[i] = (float)(ca[i] * 16777216.0); mag += fabs((double)pp[i]); }
+            if (!(mag < 0.9 * 4194304.0) || !(fabs(c0l) < 100.0)) poly_ok = false;   // rounding-constant range, 32-bit range
             if (axis) { f.Y0 = base; f.c0y = c0f - FAST_MAGIC_I; f.ay = af; f.by = bf; }
             else { f.X0 = base; f.c0x = c0f - FAST_MAGIC_I; f.ax = af; f.bx = bf; }
         }
@@ -438,7 +438,7 @@ __global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuff
                 if (cls == TC_BORDER) {
                     FastRec* fr = &pb.frec[t];
                     FastRec f = *fr;
-                    if (f.poly_ok && fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f)) {
+                    if (pb.fast_tl == 0 && f.poly_ok && fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f)) {   // Lanczos-3: general kernel
                         f.cls = TC_BORDER;
                         *fr = f;
                     } else {

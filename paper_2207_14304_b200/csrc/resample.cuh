@@ -81,10 +81,14 @@ __device__ __forceinline__ float rcp_ftz(float x) {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// REFINE: one Newton step on the quotient (<= 1 ulp) for the Lanczos-3 path, whose negative lobes amplify relative errors.
+template <bool REFINE = false>
 __device__ __forceinline__ float calib_fast(unsigned magic_r, float b, float d, float fl, bool bpm_bad, float t_exp,
                                             float sat_f, unsigned fmin_bits, unsigned frange) {
     float rf = __uint_as_float(magic_r) - 8388608.0f;
-    float c = fmaf(-d, t_exp, rf - b) * rcp_ftz(fl);
+    const float t = fmaf(-d, t_exp, rf - b), r = rcp_ftz(fl);
+    float c = t * r;
+    if (REFINE) c = fmaf(fmaf(-c, fl, t), r, c);
     bool good = !bpm_bad && (rf < sat_f) && ((__float_as_uint(fl) - fmin_bits) < frange) && (fabsf(c) < INFINITY);
     return good ? c : nanf_();
 }

@@ -40,6 +40,8 @@ struct __align__(16) FastDesc {
     FastRec r;
     long long off;       // output position of the tile's first pixel
     long long cslot;     // coadd slot of the tile's first pixel, -1 = tile absent from the layout
+    int t;               // index of the tile in the plan
+    int pad[3];
     float4 tab[32][2];   // per pixel column u: {Ax, Bx, Cx, Ay}, {By, Cy, -, -}: S-dependent Horner coefficients
     unsigned mask[32];   // TC_BORDER: membership bits
     int pref[32];        //            exclusive prefix of popc(mask)
@@ -140,7 +142,8 @@ __device__ __forceinline__ int fast_axis_eval(const FastAxis& ax, float T0, floa
     return ax.lin + (CV ? ax.da : 0) + (RV ? ax.db : 0) + __float_as_int(h);
 }
 __device__ __forceinline__ float fast_frac(int xf) {
-    return fmaf(__uint_as_float(((unsigned)xf & 0x3fffffu) | 0x4B000000u), 2.384185791015625e-07f, -2.0f);
+    // 24 fraction bits: the upper 23 go into the mantissa of 2^23 + m, one FMA brings them to [0, 1)
+    return fmaf(__uint_as_float((((unsigned)xf >> 1) & 0x7fffffu) | 0x4B000000u), 1.1920928955078125e-07f, -1.0f);
 }
 
 // ------------------------------------------------------------------------------------ interpolation
@@ -175,19 +178,21 @@ __device__ __forceinline__ float interp_clean(const float* __restrict__ a, int p
         float kx[6], ky[6];
         lanczos3_weights_f32(fx, kx);
         lanczos3_weights_f32(fy, ky);
+        // the negative lobes cancel bright taps against each other: products and sums of the 36 taps in FP64 (exact
+        // products, no partial-sum rounding), everything else FP32
         const float* r = a - 2 * pitch - 2;
-        float V = 0.0f;
+        double V = 0.0;
 #pragma unroll
         for (int b = 0; b < 6; ++b) {
-            float rs = kx[0] * r[0];
+            double rs = (double)kx[0] * (double)r[0];
 #pragma unroll
-            for (int q = 1; q < 6; ++q) rs = fmaf(kx[q], r[q], rs);
-            V = fmaf(ky[b], rs, V);
+            for (int q = 1; q < 6; ++q) rs = fma((double)kx[q], (double)r[q], rs);
+            V = fma((double)ky[b], rs, V);
             r += pitch;
         }
         const float sx = ((kx[0] + kx[5]) + (kx[1] + kx[4])) + (kx[2] + kx[3]);
         const float sy = ((ky[0] + ky[5]) + (ky[1] + ky[4])) + (ky[2] + ky[3]);
-        return V / (sx * sy);
+        return (float)V / (sx * sy);
     }
 }
 
@@ -196,6 +201,7 @@ template <int KERNEL>
 __device__ __forceinline__ void interp_masked(const float* __restrict__ a, int pitch, float fx, float fy, float w_min,
                                               float& val, float& wgt) {
     float S = 0.0f, B = 0.0f, V1 = 0.0f;
+    double V64 = 0.0;
     if (KERNEL == 0) {
         const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];
         const float gx = 1.0f - fx, gy = 1.0f - fy;
@@ -216,10 +222,11 @@ __device__ __forceinline__ void interp_masked(const float* __restrict__ a, int p
             for (int q = 0; q < 6; ++q) {
                 const float k = kx[q] * ky[b], c = r[q];
                 S += k;
-                if (c == c) V1 = fmaf(k, c, V1); else B += k;
+                if (c == c) V64 = fma((double)kx[q] * (double)ky[b], (double)c, V64); else B += k;
             }
             r += pitch;
         }
+        V1 = (float)V64;
     }
     const float w = 1.0f - B / S;
     val = 0.f; wgt = 0.f;
@@ -348,6 +355,7 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
             }
             if (lane == 0) {
                 d.off = off_c;
+                d.t = t;
                 if (COADD) {
                     long long tile = pb.tile_id[t];
                     long long key = tile >> ca.shift, lo = 0, hi = ca.n_tiles - 1, pos = -1;
@@ -407,10 +415,10 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
                 const float4 b = reinterpret_cast<const float4*>(sg.bias)[v];
                 const float4 dk = reinterpret_cast<const float4*>(sg.dark)[v];
                 const float4 fl = reinterpret_cast<const float4*>(sg.flat)[v];
-                o4[j].x = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
-                o4[j].y = calib_fast(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
-                o4[j].z = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
-                o4[j].w = calib_fast(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].x = calib_fast<KERNEL == 1>(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].y = calib_fast<KERNEL == 1>(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].z = calib_fast<KERNEL == 1>(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j].w = calib_fast<KERNEL == 1>(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
                 bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
             }
         }
@@ -424,8 +432,16 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
             }
         }
         consumers_sync(group);
+        if (KERNEL == 1 && (any_bad || cls != TC_INSIDE)) {
+            // Lanczos-3 next to masked pixels (saturated star cores: huge taps, small results) needs FP64 kernel weights
+            // and FP64 coordinates to stay inside the value tolerance: such tiles are handed to the general kernel,
+            // which runs after this one on the plan's slow list
+            if (gt == 0) slow_push(pb, d.t);
+            mbar_arrive(&sm.empty[slot]);
+            continue;
+        }
 
-        // ---- A3/A4: tile polynomial -> source position; A5: bilinear
+        // ---- A3/A4: tile polynomial -> source position; A5: interpolation
         FastAxis ax, ay;
         {
             const float4 p0 = d.tab[ul][0], p1 = d.tab[ul][1];
