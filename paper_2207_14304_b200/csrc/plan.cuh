@@ -438,7 +438,7 @@ __global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuff
                 if (cls == TC_BORDER) {
                     FastRec* fr = &pb.frec[t];
                     FastRec f = *fr;
-                    if (pb.fast_tl == 0 && f.poly_ok && fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f)) {   // Lanczos-3: general kernel
+                    if (f.poly_ok && fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f)) {
                         f.cls = TC_BORDER;
                         *fr = f;
                     } else {

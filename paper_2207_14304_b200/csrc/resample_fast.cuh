@@ -27,10 +27,12 @@
 
 // Per interpolation kernel: stage capacity, stages per CTA, CTAs per SM, register cap.
 //   bilinear : 2 stages x 50 KB, 2 CTAs / SM, 80 registers (leaves room for a plan CTA beside it, argus_api.cu)
-//   Lanczos-3: the gather dominates (36 taps, 12 kernel weights per pixel): 1 stage x 64.5 KB, 3 CTAs / SM
+//   Lanczos-3: the gather dominates (36 taps, 12 kernel weights per pixel): 1 stage x 64.5 KB + a
+#define RF_LZ_BIG_ADU 1500.0f              // Lanczos-3: a box with masked AND brighter pixels goes to the FP64 kernel
 template <int KERNEL> struct FastCfg;
-template <> struct FastCfg<0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1; };
-template <> struct FastCfg<1> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3; };
+//              separate calibrated box, so the stage is refilled while the long gather runs; 2 CTAs / SM
+template <> struct FastCfg<0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1, CALBUF = 0, REGS = 80; };
+template <> struct FastCfg<1> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
 
 struct FastMaps {
     CUtensorMap m[3][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
@@ -60,8 +62,9 @@ struct __align__(128) FastStage {
 template <int KERNEL>
 struct __align__(128) FastSmem {
     FastStage<FastCfg<KERNEL>::CAP> stage[FastCfg<KERNEL>::STAGES];
-    FastDesc desc[FastCfg<KERNEL>::STAGES];
-    unsigned long long full[FastCfg<KERNEL>::STAGES];    // TMA bytes of the stage have landed (1 arrival + tx)
+    float calbuf[FastCfg<KERNEL>::CALBUF > 0 ? FastCfg<KERNEL>::CALBUF : 4];   // separate calibrated box (Lanczos-3)
+    FastDesc desc[2];                                    // tile k uses descriptor k & 1 and stage k % STAGES
+    unsigned long long full[2];                          // descriptor written and TMA bytes landed (1 arrival + tx)
     unsigned long long empty[FastCfg<KERNEL>::STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
 };
 
@@ -256,7 +259,7 @@ __device__ __forceinline__ void interp_masked(const float* __restrict__ a, int p
 // Bilinear, 80 registers: two CTAs leave 19 K registers per SM free, enough for one CTA of any plan kernel -- the plan
 // of the next frame runs on a side stream underneath this kernel (argus_api.cu, ARGUS_OPT_PLAN_OVERLAP).
 template <bool COADD, int KERNEL>
-__global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
+__global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
     resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, FrameArgs f, int W, int H, float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
                          CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -270,10 +273,8 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
     const int sat_adu = f.sat_adu;
 
     if (tid == 0) {
-        for (int i = 0; i < RF_STAGES; ++i) {
-            mbar_init(&sm.full[i], 1);
-            mbar_init(&sm.empty[i], RF_CONSUMERS);
-        }
+        for (int i = 0; i < 2; ++i) mbar_init(&sm.full[i], 1);
+        for (int i = 0; i < RF_STAGES; ++i) mbar_init(&sm.empty[i], RF_CONSUMERS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -304,15 +305,16 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
             // lane 0 holds cls, mask_slot, gx0, gy0; lane 1 holds wclass, bh, kofs, X0
             const int cls = last ? -1 : __shfl_sync(0xffffffffu, __float_as_int(rv.x), 0);
             if (cls == 0) continue;                         // empty, or left to the general kernel
-            const int slot = issued % RF_STAGES;
-            // stage free: every consumer is done with the tile that used it RF_STAGES tiles ago
+            const int slot = issued % RF_STAGES, ds = issued & 1;
+            // stage free: every consumer is done with the tile that used it RF_STAGES tiles ago.  That also frees
+            // descriptor ds: the consumers released tile issued-1's stage after they had finished tile issued-2.
             if (issued >= RF_STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / RF_STAGES - 1) & 1));
-            FastDesc& d = sm.desc[slot];
+            FastDesc& d = sm.desc[ds];
             if (last) {
                 // end of work: one sentinel per consumer group (consecutive tiles go to distinct groups)
                 if (lane == 0) {
                     d.r.cls = -1;
-                    mbar_arrive(&sm.full[slot]);
+                    mbar_arrive(&sm.full[ds]);
                 }
                 ++issued;
                 if (++sentinels == RF_GROUPS) break;
@@ -336,10 +338,10 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
 #endif
                     const CUtensorMap* mp = &maps.m[hc][wc][0];
                     FastStage<Cfg::CAP>& sg = sm.stage[slot];
-                    tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[slot]);
-                    tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[slot]);
-                    tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[slot]);
-                    tma_load_2d(sg.flat, mp + 3, gx0, gy0, &sm.full[slot]);
+                    tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[ds]);
+                    tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[ds]);
+                    tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[ds]);
+                    tma_load_2d(sg.flat, mp + 3, gx0, gy0, &sm.full[ds]);
                 }
             }
             if (lane < 10) reinterpret_cast<float4*>(&d.r)[lane] = rv;
@@ -388,7 +390,7 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive_expect_tx(&sm.full[slot], tx_bytes);   // releases the descriptor to the consumers
+            if (lane == 0) mbar_arrive_expect_tx(&sm.full[ds], tx_bytes);   // releases the descriptor to the consumers
             ++issued;
         }
         return;
@@ -405,9 +407,9 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
     const float sat_f = (float)sat_adu;
 
     for (int it = group;; it += RF_GROUPS) {
-        const int slot = it % RF_STAGES;
-        mbar_wait(&sm.full[slot], (unsigned)((it / RF_STAGES) & 1));
-        const FastDesc& d = sm.desc[slot];
+        const int slot = it % RF_STAGES, ds = it & 1;
+        mbar_wait(&sm.full[ds], (unsigned)((it >> 1) & 1));
+        const FastDesc& d = sm.desc[ds];
         const int cls = d.r.cls;
         if (cls < 0) break;
 #ifdef RF_ABL_NOCOMPUTE
@@ -415,7 +417,7 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
         continue;
 #endif
         FastStage<Cfg::CAP>& sg = sm.stage[slot];
-        float* cal = sg.bias;
+        float* cal = Cfg::CALBUF > 0 ? sm.calbuf : sg.bias;
         const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
         // every column of the box is calibrated: restricting the items to the tap columns made the 128-bit shared
         // loads straddle rows inside a quarter-warp (bank conflicts) and measured 5 % slower
@@ -425,7 +427,7 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
         //      per thread are read and calibrated in registers; after a barrier (all reads done) they overwrite the
         //      stage with a pitch of 8 or 24 mod 32 floats, which makes the gather free of bank conflicts.
         float4 o4[RF_NI];
-        int bad = 0;
+        int bad = 0, big = 0;
 #pragma unroll
         for (int j = 0; j < RF_NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;
@@ -439,9 +441,14 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
                 o4[j].z = calib_fast<KERNEL == 1>(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
                 o4[j].w = calib_fast<KERNEL == 1>(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
                 bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
+                if (KERNEL == 1) big |= (fmaxf(fmaxf(fabsf(o4[j].x), fabsf(o4[j].y)), fmaxf(fabsf(o4[j].z), fabsf(o4[j].w))) > RF_LZ_BIG_ADU);
             }
         }
         const int any_bad = consumers_sync_or(group, bad);
+        const int any_big = KERNEL == 1 ? consumers_sync_or(group, big) : 0;
+        // separate calibrated box (Lanczos-3): every thread has read its part of the stage, the producer may refill it
+        // while the gather runs
+        if (Cfg::CALBUF > 0) mbar_arrive(&sm.empty[slot]);
 #pragma unroll
         for (int j = 0; j < RF_NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;
@@ -451,12 +458,13 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
             }
         }
         consumers_sync(group);
-        if (KERNEL == 1 && (any_bad || cls != TC_INSIDE)) {
-            // Lanczos-3 next to masked pixels (saturated star cores: huge taps, small results) needs FP64 kernel weights
-            // and FP64 coordinates to stay inside the value tolerance: such tiles are handed to the general kernel,
-            // which runs after this one on the plan's slow list
+        if (KERNEL == 1 && any_big && (any_bad || cls != TC_INSIDE)) {
+            // Lanczos-3 with masked taps next to bright pixels (saturated star cores: huge taps, small results) needs FP64
+            // kernel weights and FP64 coordinates to stay inside the value tolerance: such tiles are handed to the general
+            // kernel, which runs after this one on the plan's slow list.  Without bright pixels in the box the FP32
+            // masked form below is inside the tolerance (errors scale with the largest tap).
             if (gt == 0) slow_push(pb, d.t);
-            mbar_arrive(&sm.empty[slot]);
+            if (Cfg::CALBUF == 0) mbar_arrive(&sm.empty[slot]);
             continue;
         }
 
@@ -532,6 +540,6 @@ __global__ void __maxnreg__(KERNEL == 0 ? 80 : 72)
 #endif
 #undef RF_GEN
         }
-        mbar_arrive(&sm.empty[slot]);   // this thread is done with the stage and its descriptor
+        if (Cfg::CALBUF == 0) mbar_arrive(&sm.empty[slot]);   // this thread is done with the stage (in-place calibrated box)
     }
 }
