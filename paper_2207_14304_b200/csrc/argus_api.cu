@@ -636,7 +636,8 @@ static int launch_tiles(argus_ctx* c, int kernel, bool fused, bool use_fast, con
                 c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
         c->n_launches++;
         slow_only = 1;
-        grid = c->sm_count * 2;
+        // slow list: a handful of tiles for bilinear; for Lanczos-3 every box with masked + bright pixels (saturated stars)
+        grid = kernel == ARGUS_BILINEAR ? c->sm_count * 2 : c->sm_count * 8;
     }
 #define LT(K, F) resample_tiles_kernel<K, F, COADD><<<grid, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca, slow_only)
     if (kernel == ARGUS_BILINEAR) { if (fused) LT(0, true); else LT(0, false); }

@@ -180,18 +180,21 @@ __device__ __forceinline__ void interp_bilinear_masked(const Taps& tp, int i, in
     else { val = V1 / (S0 - B); wgt = fminf(w, 1.0f); }
 }
 
-// Lanczos-3 weights of the six taps i0-2 .. i0+3 for fraction f in [0,1): L(t) = sinc(t) sinc(t/3).
-// Evaluated in FP64 (v1: correctness first).
+// Lanczos-3 weights of the six taps i0-2 .. i0+3 for fraction f in [0,1), up to a common factor: L(t) = sinc(t)
+// sinc(t/3) = sin(pi t) sin(pi t/3) 3 / (pi t)^2 and sin(pi t_q) = (-1)^q sin(pi f) for t_q = f + 2 - q, so the
+// factor 3 sin(pi f) / pi^2 is shared by all six taps and cancels in value = V1 / (S0 - B) and in weight = 1 - B/S0.
+// FP64 (general kernel: DESIGN.md "Lanczos precision"); three trigonometric evaluations serve the six taps:
+//   sin(pi t/3): q0  sin(pi (1-f)/3),  q1  cos(pi (2f-1)/6),  q2  sin(pi f/3),  q3 = -q0,  q4 = -q1,  q5 = -q2
 __device__ __forceinline__ void lanczos3_weights(double fd, double k[6]) {
-    double s1 = sinpi(fd);
-#pragma unroll
-    for (int q = 0; q < 6; ++q) {
-        double t = fd - (double)(q - 2);
-        if (t == 0.0) { k[q] = 1.0; continue; }
-        double sg = (q & 1) ? -1.0 : 1.0;   // sin(pi (f - (q-2))) = (-1)^(q-2) sin(pi f)
-        double pt = 3.141592653589793 * t;
-        k[q] = sg * s1 * sinpi(t * (1.0 / 3.0)) * 3.0 / (pt * pt);
-    }
+    if (fd == 0.0) { k[0] = k[1] = k[3] = k[4] = k[5] = 0.0; k[2] = 1.0; return; }
+    const double A = sinpi((1.0 - fd) * (1.0 / 3.0)), B = -cospi((2.0 * fd - 1.0) * (1.0 / 6.0)), C = sinpi(fd * (1.0 / 3.0));
+    const double t0 = fd + 2.0, t1 = fd + 1.0, t3 = fd - 1.0, t4 = fd - 2.0, t5 = fd - 3.0;
+    k[0] = A / (t0 * t0);
+    k[1] = B / (t1 * t1);
+    k[2] = C / (fd * fd);
+    k[3] = A / (t3 * t3);
+    k[4] = B / (t4 * t4);
+    k[5] = C / (t5 * t5);
 }
 
 template <class Taps>
