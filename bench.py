@@ -31,7 +31,7 @@ UNIT = "Mpix/s"  # input (detector) pixels per second
 SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload recipe per step
 # dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
 # profiles/r1_final_ncu_summary.txt (ncu --set full).
-NCU_TRAFFIC_BYTES = 978128128 + 338976512  # profiles/r1_final_ncu_summary.txt
+NCU_TRAFFIC_BYTES = 988786688 + 339882496  # profiles/r1_final_ncu_summary.txt
 
 
 def _peaks():
@@ -279,7 +279,7 @@ def run_gpu(args):
             "output_mpix_per_s": px_out_all * args.steps / (ms * 1e-3) / 1e6,
             "plan_ms_per_step": plan_ms / max(ncalls, 1),
             "roofline": {"bound": "hbm", "kernel": ("resample_fast_kernel<false> (TMA-staged bilinear, fused calibration)" if fr.kernel == "bilinear"
-                                                   else "resample_tiles_kernel<1,true,false> (general kernel, Lanczos-3)"), "achieved": achieved,
+                                                   else "resample_fast_kernel<false,1> (TMA-staged Lanczos-3) + general kernel on its slow list"), "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if args.workload == "config1" else None,
                          "peak_source": peak_src, "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes,
                          "step_frac": (alg_bytes / (ms_step * 1e-3) / 1e9) / peak},

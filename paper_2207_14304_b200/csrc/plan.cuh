@@ -454,41 +454,35 @@ __global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuff
 // Exclusive scan of the per-tile counts in one launch: block-local scan (1024 tiles per CTA, coalesced reads of
 // the compact count / class arrays); the last CTA to finish scans the per-CTA sums.
 // Output position of tile t = block_base[t >> 10] + tile_offset[t].
-// 256 threads per CTA (so that a CTA fits beside the resample kernel's CTAs), 4 consecutive tiles per thread.
 __device__ inline void offsets_final_body(const PlanBuffers& pb, long long out_capacity, long long* s_warp) {
     int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int n = *pb.n_tiles;
-    int nb = (n + 1023) >> 10;   // <= 16384 CTA sums (max_tiles <= 2^24): each of the 256 threads handles up to 64
-    long long sum = 0;
-    for (int j = 0; j < 64; ++j) {
-        int b = tid * 64 + j;
-        if (b < nb) sum += (long long)__ldcg(pb.block_sum + b);
-    }
-    long long inc = sum;
-    for (int o = 1; o < 32; o <<= 1) {
-        long long u = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += u;
-    }
-    if (lane == 31) s_warp[wid] = inc;
-    __syncthreads();
-    long long woff = 0, total = 0;
-    for (int i = 0; i < 8; ++i) { if (i < wid) woff += s_warp[i]; total += s_warp[i]; }
-    long long run = woff + inc - sum;
-    for (int j = 0; j < 64; ++j) {
-        int b = tid * 64 + j;
-        if (b < nb) {
-            pb.block_base[b] = run;
-            run += (long long)__ldcg(pb.block_sum + b);
+    int nb = (n + 1023) >> 10;   // per-CTA sums (<= 16384 for max_tiles <= 2^24), scanned 256 at a time
+    long long base = 0;
+    for (int b0 = 0; b0 < nb; b0 += 256) {
+        int b = b0 + tid;
+        long long v = (b < nb) ? (long long)__ldcg(pb.block_sum + b) : 0, inc = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            long long u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
         }
+        __syncthreads();
+        if (lane == 31) s_warp[wid] = inc;
+        __syncthreads();
+        long long woff = 0, total = 0;
+        for (int i = 0; i < 8; ++i) { if (i < wid) woff += s_warp[i]; total += s_warp[i]; }
+        if (b < nb) pb.block_base[b] = base + woff + inc - v;
+        base += total;
     }
     if (tid == 0) {
         PlanStats* st = pb.stats;
-        st->n_footprint = total;
+        st->n_footprint = base;
         st->n_tiles = n;
-        if (out_capacity >= 0 && total > out_capacity) atomicOr(&st->overflow, 4);
+        if (out_capacity >= 0 && base > out_capacity) atomicOr(&st->overflow, 4);
     }
 }
 
+// 256 threads per CTA (so that a CTA fits beside the resample kernel's CTAs), 4 consecutive tiles per thread.
 __global__ void __launch_bounds__(256) plan_offsets_kernel(PlanBuffers pb, long long out_capacity) {
     __shared__ int s_warp[8];
     __shared__ long long s_warp64[8];
