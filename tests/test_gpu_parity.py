@@ -165,6 +165,69 @@ def test_small_nside_coarse_wcs(argus, ctx):
     assert_values_match(v, w, vo, wo, fl, "nside 2^10")
 
 
+def test_lanczos_saturated_stars_handover(argus, ctx):
+    """Saturated star cores: masked pixels next to ~6e4-ADU taps.  The Lanczos-3 fast kernel hands such tiles to the
+    FP64 general kernel at run time (and keeps the others); both kernels, planned path, must meet the tolerance,
+    and the fast path must agree with the general kernel alone."""
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    W = H = 512
+    wcs = synth.make_wcs((30.0, 20.0), (255.5, 255.5), 0.3)
+    fr = synth.make_frame(11, W, H, 40, wcs, 1 << 17, "lanczos3")
+    rng = np.random.default_rng(3)
+    raw = fr.raw.astype(np.float64)
+    yy, xx = np.mgrid[0:H, 0:W]
+    for _ in range(6):   # bright stars whose cores clip at 65535 (=> masked), wings up to ~6e4 ADU
+        sx, sy = rng.uniform(20, W - 20, 2)
+        raw += 4e5 * np.exp(-0.5 * ((xx - sx) ** 2 + (yy - sy) ** 2) / 0.85 ** 2)
+    fr.raw = np.clip(np.rint(raw), 0, 65535).astype(np.uint16)
+    assert (fr.raw == 65535).sum() > 10
+    idx_or, dmin = oracle.footprint(wcs, W, H, fr.nside)
+    d = upload(fr)
+    for kernel in ("lanczos3", "bilinear"):
+        n, v, w = gpu_resample_planned(ctx, fr, d, kernel)
+        vo, wo, fl = oracle_reference(fr, idx_or, kernel)
+        assert (wo < 1).sum() > 50
+        assert_values_match(v, w, vo, wo, fl, "saturated stars " + kernel)
+        ctx.set_fast_path(False)
+        try:
+            n2, v2, w2 = gpu_resample_planned(ctx, fr, d, kernel)
+        finally:
+            ctx.set_fast_path(True)
+        assert_values_match(v2, w2, vo, wo, fl, "saturated stars, general kernel " + kernel)
+
+
+def test_plan_overlap_option_and_stream_order(argus, ctx, cfg0, cfg0_fp):
+    """Plans built on the side streams (default) and in place must give identical outputs; results follow the
+    caller's stream order when frames with different WCS are enqueued back to back without synchronisation."""
+    from gpu_util import upload
+    d = upload(cfg0)
+    wcs2 = synth.make_wcs((30.01, 20.02), (255.5, 255.5), 7.0)
+    outs = {}
+    for overlap in (True, False):
+        ctx.set_plan_overlap(overlap)
+        ctx.set_plan_cache(False)
+        try:
+            res = []
+            for k in range(6):   # alternate two pointings, never synchronise in between
+                wcs = cfg0.wcs if k % 2 == 0 else wcs2
+                v = torch.full((200000,), float("nan"), dtype=torch.float32, device="cuda")
+                w = torch.full_like(v, float("nan"))
+                argus.argus_resample(ctx, wcs, 512, 512, cfg0.nside, "bilinear", v, w, **d)
+                res.append((v, w))
+            torch.cuda.synchronize()
+            outs[overlap] = [(v.cpu().numpy(), w.cpu().numpy()) for v, w in res]
+        finally:
+            ctx.set_plan_overlap(True)
+            ctx.set_plan_cache(True)
+    for k in range(6):
+        assert np.array_equal(outs[True][k][0], outs[False][k][0], equal_nan=True)
+        assert np.array_equal(outs[True][k][1], outs[False][k][1], equal_nan=True)
+    n0 = len(cfg0_fp[0])
+    assert np.isfinite(outs[True][0][0][:n0]).all() and np.isnan(outs[True][0][0][n0:]).all()
+    assert np.array_equal(outs[True][0][0], outs[True][2][0], equal_nan=True)   # same pointing, same result
+    assert not np.array_equal(outs[True][0][0], outs[True][1][0], equal_nan=True)
+
+
 def test_tiny_nside_flat_plan(argus, ctx):
     """nside < 256 has no 8x8-tile blocks: the flat plan (one fit per tile) must give the same parity."""
     from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
