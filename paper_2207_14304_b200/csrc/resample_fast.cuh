@@ -498,8 +498,29 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
             RF_HOT(2) RF_HOT(3)
 #endif
 #undef RF_HOT
+        } else if (COADD && cls == TC_INSIDE && !any_bad && d.cslot >= 0) {
+            // A6 on a clean tile: weight == 1, so sum += value, wsum += 1.  The eight accumulator loads are issued
+            // before the gather so that their latency hides under it (footprint pixels are unique within a frame:
+            // plain read-modify-write, deterministic)
+            float* sp = ca.sum + d.cslot + gt;
+            float* wp = ca.wsum + d.cslot + gt;
+            float s_acc[RF_NQ], w_acc[RF_NQ];
+#pragma unroll
+            for (int q = 0; q < RF_NQ; ++q) { s_acc[q] = sp[RF_CONSUMERS * q]; w_acc[q] = wp[RF_CONSUMERS * q]; }
+#define RF_ACC(Q)                                                                            \
+    {                                                                                        \
+        const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);    \
+        const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));     \
+        sp[RF_CONSUMERS * Q] = s_acc[Q] + interp_clean<KERNEL>(a, pitch, fast_frac(xf), fast_frac(yf)); \
+        wp[RF_CONSUMERS * Q] = w_acc[Q] + 1.0f;                                              \
+    }
+            RF_ACC(0) RF_ACC(1)
+#if RF_NQ == 4
+            RF_ACC(2) RF_ACC(3)
+#endif
+#undef RF_ACC
         } else {
-            // masked source pixels, tiles cut by the frame border, coadd accumulation
+            // masked source pixels, tiles cut by the frame border, coadd tiles outside the layout
             const long long cslot = COADD ? d.cslot : 0;
 #define RF_GEN(Q)                                                                                          \
     {                                                                                                      \
