@@ -325,12 +325,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
                 const int wc = wclass & 15, hc = wclass >> 4;
                 const int boxw = 40 + 8 * wc, boxh = 48 + 8 * hc;
                 tx_bytes = (unsigned)(boxh * boxw * 14);
-#ifdef RF_ABL_NOTMA
-                tx_bytes = 0;
-                if (false) {
-#else
                 if (lane == 0) {
-#endif
                     const CUtensorMap* mp = &maps.m[hc][wc][0];
                     FastStage<Cfg::CAP>& sg = sm.stage[slot];
                     tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[ds]);
@@ -407,10 +402,6 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
         const FastDesc& d = sm.desc[ds];
         const int cls = d.r.cls;
         if (cls < 0) break;
-#ifdef RF_ABL_NOCOMPUTE
-        mbar_arrive(&sm.empty[slot]);
-        continue;
-#endif
         FastStage<Cfg::CAP>& sg = sm.stage[slot];
         float* cal = Cfg::CALBUF > 0 ? sm.calbuf : sg.bias;
         const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
