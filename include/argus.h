@@ -20,7 +20,9 @@
  *     never frees it and never keeps it after the call returns.  argus_wcs / argus_frame / argus_coadd
  *     structs are HOST structs read during the call.
  *   - All work is enqueued on the caller's stream (cudaStream_t passed as void*; NULL = legacy default
- *     stream) and is asynchronous, except where a function documents a synchronisation.
+ *     stream) and is asynchronous, except where a function documents a synchronisation.  With
+ *     ARGUS_OPT_PLAN_OVERLAP (default) the per-frame plan runs on the context's own streams and the caller's
+ *     stream waits for it by event: outputs are complete in the caller's stream order exactly as without it.
  *   - Pixel convention: 0-based, pixel centres at integers, frame[y*W + x], x <-> FITS axis 1,
  *     crpix 0-based.  HEALPix: NESTED scheme, nside a power of two, 32 <= nside <= 2^29; sky
  *     convention alpha = phi, delta = pi/2 - theta (ICRS).
@@ -121,9 +123,11 @@ typedef struct argus_plan_stats {
 const char* argus_strerror(int status);
 int argus_version(void);
 
-/* Context: owns scratch only (tile records, prefix sums, counters), sized for frames of up to
- * max_tiles output tiles (0 = default 1<<20, enough for a 61-MPix frame at nside 2^18).
- * device = CUDA ordinal.  Synchronous. */
+/* Context: owns scratch only -- three sets of plan buffers (tile records, masks, prefix sums, counters; about
+ * 560 bytes per tile each, 290 MB per set at the default), two internal high-priority streams and events for
+ * ARGUS_OPT_PLAN_OVERLAP -- sized for frames of up to max_tiles candidate output tiles (0 = default 1<<19: a 61-MPix
+ * frame needs 5.3e4 at nside 2^17 and 1.95e5 at nside 2^18; valid range 64 .. 2^24).  device = CUDA ordinal.
+ * Synchronous.  A context is not thread-safe: use one per host thread (contexts are independent). */
 int argus_ctx_create(argus_ctx** ctx, int device, int64_t max_tiles);
 int argus_ctx_destroy(argus_ctx* ctx);
 int argus_ctx_set_option(argus_ctx* ctx, int option, int64_t value);
