@@ -31,7 +31,7 @@ UNIT = "Mpix/s"  # input (detector) pixels per second
 SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload recipe per step
 # dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
 # profiles/r1_final_ncu_summary.txt (ncu --set full).
-NCU_TRAFFIC_BYTES = 988786688 + 339882496  # profiles/r1_final_ncu_summary.txt
+NCU_TRAFFIC_BYTES = 983571968 + 339383296  # profiles/r1_final_ncu_summary.txt
 
 
 def _peaks():
@@ -199,6 +199,8 @@ def run_gpu(args):
     value = torch.empty(n_fp, dtype=torch.float32, device=dev)
     weight = torch.empty(n_fp, dtype=torch.float32, device=dev)
     ctx.set_plan_cache(False)  # every step plans its frame again, as a new WCS would
+    if args.no_plan_overlap:
+        ctx.set_plan_overlap(False)
 
     def step():
         argus.argus_resample(ctx, fr.wcs, W, H, fr.nside, fr.kernel, value, weight, **d)
@@ -300,7 +302,8 @@ def run_gpu(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl, "frames_per_step_per_gpu": 1, "W": W, "H": H, "nside": fr.nside,
                        "kernel": fr.kernel, "n_footprint": n_fp, "fused": True, "plan_every_step": True,
-                       "plan_overlap": "the plan of step k+1 runs on the library's side streams underneath the kernels of step k",
+                       "plan_overlap": ("off (diagnostic)" if args.no_plan_overlap else
+                                        "the plan of step k+1 runs on the library's side streams underneath the kernels of step k"),
                        "l2": "inputs (856 MB/frame) larger than L2 (126 MB)", "plan": stats,
                        "parallelism": "1 frame per GPU per step, frames independent (replicas)"},
             "output_mpix_per_s": px_out_all * args.steps / (ms * 1e-3) / 1e6,
@@ -332,6 +335,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-plan-overlap", action="store_true", help="diagnostic: build every plan in place on the caller's stream")
     ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config2", "config3", "config4"])
     args = ap.parse_args()
     if args.impl == "reference":
