@@ -283,6 +283,45 @@ def test_coadd_three_frames(argus, ctx):
         assert np.all(np.abs(sg - s_or) <= 3 * 1e-3 + 1e-5 * np.abs(s_or))
 
 
+def test_coadd_lanczos_fused(argus, ctx):
+    """Fused calibrate + Lanczos-3 resample + accumulate (fast kernel, COADD variant) against the oracle."""
+    from gpu_util import upload
+    W = H = 512
+    nside = 1 << 17
+    frames = [synth.config3_frame(k, W, H) for k in range(2)]
+    fps = [oracle.footprint(f.wcs, W, H, nside)[0] for f in frames]
+    tiles = np.unique(np.concatenate([fp >> 18 for fp in fps]))
+    ppt = 1 << 18
+    s_or = np.zeros(len(tiles) * ppt)
+    w_or = np.zeros(len(tiles) * ppt)
+    for f, fp in zip(frames, fps):
+        cal, mask = oracle.calibrate_frame(f)
+        v, w, fl = oracle.resample(cal, mask, f.wcs, nside, fp, oracle.LANCZOS3)
+        assert oracle.coadd_accumulate(tiles, ppt, s_or, w_or, fp, v, w) == 0
+    dt = torch.from_numpy(tiles).cuda()
+    s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
+    ws = torch.zeros_like(s)
+    for f in frames:
+        argus.argus_resample_coadd(ctx, f.wcs, W, H, nside, "lanczos3", dt, 256, s, ws, None, **upload(f))
+    torch.cuda.synchronize()
+    sg, wg = s.cpu().numpy().astype(np.float64), ws.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(wg - w_or) <= 2e-5)
+    bad = np.abs(sg - s_or) > 2e-3 + 1e-5 * np.abs(s_or)
+    assert bad.mean() <= 1e-4, bad.mean()   # dithered frames: margin-ambiguous pixels beside the frame border
+
+
+def test_plan_scratch_overflow_is_reported(argus):
+    """A context too small for the frame's tiles reports ARGUS_ERR_CAPACITY instead of writing out of bounds."""
+    small = argus.Context(0, max_tiles=64)
+    try:
+        fr = synth.config0()
+        with pytest.raises(argus.ArgusError) as e:
+            argus.argus_healpix_footprint(small, fr.wcs, 512, 512, fr.nside)
+        assert e.value.status == -6
+    finally:
+        small.close()
+
+
 def test_capacity_and_errors(argus, ctx, cfg0):
     from gpu_util import upload
     d = upload(cfg0)
