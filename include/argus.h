@@ -170,6 +170,20 @@ int argus_resample(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wc
                    int64_t nside, int kernel, float w_min, const int64_t* idx, size_t n, float* value_out,
                    float* weight_out, void* stream);
 
+/* A2-A5 with HOST buffers for the per-frame data: frame->raw is a HOST pointer to the uint16 frame (pinned memory
+ * for asynchronous copies; pageable memory works but serialises), the masters stay DEVICE pointers (resident per
+ * pointing), value_host / weight_host are HOST arrays of n floats (n = footprint size, e.g. from
+ * argus_healpix_footprint; the first n outputs are copied).  The library uploads the frame, runs argus_resample with its
+ * own plan on `stream` and downloads value + weight, on internal copy streams and two sets of device staging buffers,
+ * so that the upload of frame k+1 and the download of frame k-1 overlap the kernels of frame k.  Asynchronous: the
+ * host arrays are complete after argus_host_wait(ctx).  The first call (and a call with a larger frame) allocates the
+ * staging buffers and synchronises the device. */
+int argus_resample_host(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                        int64_t nside, int kernel, float w_min, size_t n, float* value_host, float* weight_host,
+                        void* stream);
+/* Blocks until every upload and download enqueued by argus_resample_host has completed. */
+int argus_host_wait(argus_ctx* ctx);
+
 /* A6: sum[slot(idx[i])] += weight[i] * value[i]; wsum[slot] += weight[i] for i < n.  idx must hold
  * unique pixels (a footprint); pixels whose tile is absent from the layout are skipped and counted in
  * *n_skipped_dev (device int64, may be NULL, accumulated with atomics).  Asynchronous. */

@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     argus_plan_info,
     argus_resample,
     argus_resample_coadd,
+    argus_resample_host,
+    argus_host_wait,
     library_path,
     load_library,
 )

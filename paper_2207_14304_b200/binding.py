@@ -21,6 +21,7 @@ EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
+    "argus_resample_host", "argus_host_wait",
 ]
 
 
@@ -89,6 +90,8 @@ def load_library():
     L.argus_coadd_accumulate.argtypes = [vp, C.POINTER(_Coadd), i64, vp, vp, vp, vp, vp, sz, vp, vp]
     L.argus_resample_coadd.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32,
                                        C.POINTER(_Coadd), vp, vp, vp, vp]
+    L.argus_resample_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, sz, vp, vp, vp]
+    L.argus_host_wait.argtypes = [vp]
     L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
     L.argus_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64), vp]
     _lib = L
@@ -276,6 +279,32 @@ def argus_resample(ctx, wcs, W, H, nside, kernel, value_out, weight_out, idx=Non
                                        _dev(value_out, torch.float32, "value_out"),
                                        _dev(weight_out, torch.float32, "weight_out"), _stream(stream))
     _check(ctx, rc, "argus_resample")
+
+
+def argus_resample_host(ctx, wcs, W, H, nside, kernel, n, raw_host, value_host, weight_host, w_min=0.5, stream=None,
+                        bias=None, dark=None, flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1):
+    """A2-A5 with HOST frame / outputs (CPU tensors, pinned for asynchronous copies); masters are CUDA tensors.
+    Asynchronous: call argus_host_wait(ctx) before reading value_host / weight_host."""
+    for t, dt, name in ((raw_host, torch.uint16, "raw_host"), (value_host, torch.float32, "value_host"),
+                        (weight_host, torch.float32, "weight_host")):
+        if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != dt or not t.is_contiguous():
+            raise TypeError("%s must be a contiguous CPU tensor of dtype %s" % (name, dt))
+    if raw_host.numel() != W * H or value_host.numel() < n or weight_host.numel() < n:
+        raise ValueError("host buffers too small")
+    f = _Frame()
+    f.raw = raw_host.data_ptr()
+    f.bias = _dev(bias, torch.float32, "bias")
+    f.dark = _dev(dark, torch.float32, "dark")
+    f.flat = _dev(flat, torch.float32, "flat")
+    f.t_exp, f.sat_adu, f.flat_min = float(t_exp), int(sat_adu), float(flat_min)
+    w = _wcs_struct(wcs)
+    rc = load_library().argus_resample_host(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min), int(n),
+                                            value_host.data_ptr(), weight_host.data_ptr(), _stream(stream))
+    _check(ctx, rc, "argus_resample_host")
+
+
+def argus_host_wait(ctx):
+    _check(ctx, load_library().argus_host_wait(ctx._h), "argus_host_wait")
 
 
 def _coadd_struct(tiles, nside_tile) -> _Coadd:

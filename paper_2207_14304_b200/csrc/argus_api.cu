@@ -55,6 +55,15 @@ struct argus_ctx {
     const void* maps_key[4];
     int64_t maps_W, maps_H;
     int64_t n_launches;   // kernels launched through this context (diagnostics)
+    // argus_resample_host: two sets of device staging buffers, upload / download streams
+    struct HostBuf {
+        uint16_t* raw; float* val; float* wgt;
+        size_t cap_px, cap_n;
+        cudaEvent_t up, run, down;
+        bool used, ev_ok;
+    } hb[2];
+    int hb_next;
+    cudaStream_t s_up, s_down;
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -251,6 +260,14 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
         cudaEventDestroy(c->ev_free[sidx]);
     }
     for (int i = 0; i < 2; ++i) cudaStreamDestroy(c->side[i]);
+    if (c->s_up) { cudaStreamSynchronize(c->s_up); cudaStreamDestroy(c->s_up); }
+    if (c->s_down) { cudaStreamSynchronize(c->s_down); cudaStreamDestroy(c->s_down); }
+    for (int i = 0; i < 2; ++i) {
+        if (c->hb[i].raw) cudaFree(c->hb[i].raw);
+        if (c->hb[i].val) cudaFree(c->hb[i].val);
+        if (c->hb[i].wgt) cudaFree(c->hb[i].wgt);
+        if (c->hb[i].ev_ok) { cudaEventDestroy(c->hb[i].up); cudaEventDestroy(c->hb[i].run); cudaEventDestroy(c->hb[i].down); }
+    }
     cudaFreeHost(c->h_stats);
     delete c;
     return ARGUS_OK;
@@ -385,7 +402,13 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
     if (rc) return rc;
-    if (plan_usable(c, w, W, H, nside, need_full, fast_kernel)) return ARGUS_OK;
+    if (plan_usable(c, w, W, H, nside, need_full, fast_kernel)) {
+        if (out_cap >= 0) {   // cached plan: the capacity of THIS call's outputs still has to be checked
+            plan_check_capacity_kernel<<<1, 32, 0, caller>>>(c->pb, out_cap);
+            c->n_launches++;
+        }
+        return ARGUS_OK;
+    }
     c->plan_valid = false;
     const int lite = need_full ? 0 : 1;
     // where the plan is built: in place on the caller's stream, or (overlap) in the other scratch set on the side
@@ -689,6 +712,67 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     mark_slot_read(c, st);
     if (c->profile) { cudaEventRecord(c->ev[slot][3], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+// ------------------------------------------------------------------------------- host-buffer variant
+extern "C" int argus_resample_host(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                                   int64_t nside, int kernel, float w_min, size_t n, float* value_host, float* weight_host,
+                                   void* stream) {
+    if (!c || !frame || !wcs || !value_host || !weight_host || !frame->raw) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n == 0 || n > ((size_t)1 << 34)) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (!c->s_up) {
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking));
+        CUDA_TRY(c, cudaStreamCreateWithFlags(&c->s_down, cudaStreamNonBlocking));
+    }
+    argus_ctx::HostBuf& b = c->hb[c->hb_next];
+    c->hb_next ^= 1;
+    const size_t px = (size_t)W * (size_t)H;
+    if (!b.ev_ok) {
+        CUDA_TRY(c, cudaEventCreateWithFlags(&b.up, cudaEventDisableTiming));
+        CUDA_TRY(c, cudaEventCreateWithFlags(&b.run, cudaEventDisableTiming));
+        CUDA_TRY(c, cudaEventCreateWithFlags(&b.down, cudaEventDisableTiming));
+        b.ev_ok = true;
+    }
+    if (b.cap_px < px || b.cap_n < n) {      // (re)allocation synchronises: first call per buffer set, or a larger frame
+        CUDA_TRY(c, cudaDeviceSynchronize());
+        if (b.raw) cudaFree(b.raw);
+        if (b.val) cudaFree(b.val);
+        if (b.wgt) cudaFree(b.wgt);
+        b.raw = nullptr; b.val = b.wgt = nullptr; b.cap_px = b.cap_n = 0; b.used = false;
+        CUDA_TRY(c, cudaMalloc((void**)&b.raw, px * sizeof(uint16_t)));
+        CUDA_TRY(c, cudaMalloc((void**)&b.val, n * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc((void**)&b.wgt, n * sizeof(float)));
+        b.cap_px = px; b.cap_n = n;
+    }
+    // upload on its own stream (after the kernels that last read this raw buffer) ...
+    if (b.used) CUDA_TRY(c, cudaStreamWaitEvent(c->s_up, b.run, 0));
+    CUDA_TRY(c, cudaMemcpyAsync(b.raw, frame->raw, px * sizeof(uint16_t), cudaMemcpyHostToDevice, c->s_up));
+    CUDA_TRY(c, cudaEventRecord(b.up, c->s_up));
+    // ... kernels on the caller's stream (after the upload, and after the previous download of this buffer set) ...
+    CUDA_TRY(c, cudaStreamWaitEvent(st, b.up, 0));
+    if (b.used) CUDA_TRY(c, cudaStreamWaitEvent(st, b.down, 0));
+    argus_frame fr = *frame;
+    fr.raw = b.raw;
+    int rc = argus_resample(c, &fr, wcs, W, H, nside, kernel, w_min, nullptr, n, b.val, b.wgt, stream);
+    if (rc) return rc;
+    CUDA_TRY(c, cudaEventRecord(b.run, st));
+    // ... download on its own stream
+    CUDA_TRY(c, cudaStreamWaitEvent(c->s_down, b.run, 0));
+    CUDA_TRY(c, cudaMemcpyAsync(value_host, b.val, n * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaMemcpyAsync(weight_host, b.wgt, n * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaEventRecord(b.down, c->s_down));
+    b.used = true;
+    return ARGUS_OK;
+}
+
+extern "C" int argus_host_wait(argus_ctx* c) {
+    if (!c) return ARGUS_ERR_NULL;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (c->s_up) CUDA_TRY(c, cudaStreamSynchronize(c->s_up));
+    if (c->s_down) CUDA_TRY(c, cudaStreamSynchronize(c->s_down));
     return ARGUS_OK;
 }
 

@@ -544,6 +544,11 @@ __global__ void __launch_bounds__(256) plan_offsets_kernel(PlanBuffers pb, long 
     if (tid == 0) *pb.ticket = 0u;
 }
 
+// Re-check of the caller's output capacity when a cached plan is reused (the scan did it when the plan was built).
+__global__ void plan_check_capacity_kernel(PlanBuffers pb, long long out_capacity) {
+    if (threadIdx.x == 0 && blockIdx.x == 0 && pb.stats->n_footprint > out_capacity) atomicOr(&pb.stats->overflow, 4);
+}
+
 __device__ __forceinline__ long long tile_out_offset(const PlanBuffers& pb, int t) {
     return pb.block_base[t >> 10] + pb.tile_offset[t];
 }

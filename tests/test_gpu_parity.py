@@ -310,6 +310,25 @@ def test_coadd_lanczos_fused(argus, ctx):
     assert bad.mean() <= 1e-4, bad.mean()   # dithered frames: margin-ambiguous pixels beside the frame border
 
 
+def test_resample_host_matches_device_path(argus, ctx, cfg0, cfg0_fp):
+    """C-ABI entry with HOST buffers: same outputs as the device-buffer call, over several pipelined frames."""
+    from gpu_util import upload
+    d = upload(cfg0)
+    n = len(cfg0_fp[0])
+    v = torch.empty(n, dtype=torch.float32, device="cuda")
+    w = torch.empty_like(v)
+    argus.argus_resample(ctx, cfg0.wcs, 512, 512, cfg0.nside, "bilinear", v, w, **d)
+    torch.cuda.synchronize()
+    h_raw = torch.from_numpy(cfg0.raw).pin_memory()
+    outs = [(torch.full((n,), float("nan")).pin_memory(), torch.full((n,), float("nan")).pin_memory()) for _ in range(5)]
+    for hv, hw in outs:
+        argus.argus_resample_host(ctx, cfg0.wcs, 512, 512, cfg0.nside, "bilinear", n, h_raw, hv, hw, bias=d["bias"],
+                                  dark=d["dark"], flat=d["flat"], t_exp=cfg0.t_exp, sat_adu=cfg0.sat_adu, flat_min=cfg0.flat_min)
+    argus.argus_host_wait(ctx)
+    for hv, hw in outs:
+        assert torch.equal(hv, v.cpu()) and torch.equal(hw, w.cpu())
+
+
 def test_plan_scratch_overflow_is_reported(argus):
     """A context too small for the frame's tiles reports ARGUS_ERR_CAPACITY instead of writing out of bounds."""
     small = argus.Context(0, max_tiles=64)
