@@ -1,16 +1,19 @@
-// resample_fast.cuh -- A2..A5 (+A6) fused, bilinear, TMA-staged: the hot kernel of the path.
+// resample_fast.cuh -- A2..A5 (+A6) fused, bilinear or Lanczos-3, TMA-staged: the hot kernel of the path.
 //
-// Persistent CTAs (3 per SM), 8 consumer warps + 1 producer warp, one 32x32 output tile per iteration:
-//   producer  reads the tile's FastRec, writes a descriptor to shared memory and issues one
-//             cp.async.bulk.tensor (TMA) per array (raw u16, bias, dark, flat f32) into
-//             the stage buffer; out-of-frame elements arrive as zeros (flat = 0 < flat_min => masked), so no
-//             bounds logic exists anywhere.  The loads of tile i+1 are in flight while tile i is gathered.
-//   consumers wait on the mbarrier, calibrate the staged box ONCE from shared memory into a
-//             float32 box (masked pixels as NaN; the stage is a dense array, so there is no index arithmetic),
-//             release the stage, then gather: coordinates from the tile polynomial (exact integer linear part
-//             + FP32 remainder, common.cuh), four taps, bilinear, value + weight stores of
-//             32 consecutive floats per warp -- or the coadd read-modify-write.
-// Tiles that do not fit a stage, belt/cap-ring and pole tiles are left to resample_tiles_kernel (slow list).
+// Persistent CTAs (bilinear: 2 per SM, 2 stages; Lanczos-3: 3 per SM, 1 stage), 8 consumer warps + 1 producer warp, one
+// 32x32 output tile (1024 consecutive nested indices) per iteration, tiles dealt round-robin in ascending order:
+//   producer  (software-pipelined) reads the tile's FastRec, issues one cp.async.bulk.tensor (TMA) per array (raw u16,
+//             bias, dark, flat f32) for the tile's source bounding box into a free stage -- out-of-frame elements
+//             arrive as zeros (flat = 0 < flat_min => masked), so no bounds logic exists anywhere -- writes the tile
+//             descriptor (record, output offset, per-column Horner coefficients, membership mask of border tiles) and
+//             completes the stage's mbarrier with arrive.expect_tx.  Loads run one to two tiles ahead of the consumers.
+//   consumers wait on the mbarrier, calibrate the staged box ONCE: shared -> registers, a barrier, then
+//             the float32 box overwrites the stage in place with a bank-conflict-free pitch (masked pixels as NaN);
+//             gather: coordinates from the tile polynomial (exact integer linear part + FP32 remainder, common.cuh),
+//             2x2 or 6x6 taps, value + weight stores of 32 consecutive floats per warp -- or the coadd
+//             read-modify-write; every thread then releases the stage (mbarrier arrive).
+// Tiles that do not fit a stage, belt/cap-ring and pole tiles are left to resample_tiles_kernel (the plan's slow list);
+// the Lanczos-3 variant appends tiles with masked + bright pixels to that list at run time (FP64 path).
 #pragma once
 #include <cuda.h>
 
