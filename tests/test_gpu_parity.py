@@ -228,6 +228,44 @@ def test_plan_overlap_option_and_stream_order(argus, ctx, cfg0, cfg0_fp):
     assert not np.array_equal(outs[True][0][0], outs[True][1][0], equal_nan=True)
 
 
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("ARGUS_FUZZ_SEEDS", "48"))))
+def test_random_geometry_fuzz(argus, ctx, seed):
+    """Seeded random pointings, rotations, pixel scales, nside, frame shapes, SIP and kernels: footprint bit-exact,
+    values within tolerance.  Exercises sheared / oversized tiles (slow list), both fast kernels and the flat plan."""
+    from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
+    rng = np.random.default_rng(1000 + seed)
+    nside = 1 << int(rng.integers(14, 19))
+    hp = math.degrees(math.sqrt(4 * math.pi / (12.0 * nside * nside)))
+    scale = hp / rng.uniform(0.6, 2.5)            # HEALPix pixel = 0.6 .. 2.5 detector pixels
+    W = int(rng.integers(12, 48)) * 8 if rng.random() < 0.7 else int(rng.integers(100, 380))
+    H = int(rng.integers(90, 380))
+    dec = math.degrees(math.asin(rng.uniform(-1, 1)))
+    if seed % 6 == 0:
+        dec = math.copysign(89.0 + rng.uniform(0, 0.99), dec)        # polar caps, near the poles
+    crval = (rng.uniform(0, 360), dec)
+    sip = None
+    if rng.random() < 0.5:
+        o, ap, bp = synth.make_sip(rng, 3, W / 2.0)
+        sip = (o, ap * 20, bp * 20)
+    wcs = synth.make_wcs(crval, ((W - 1) / 2.0 + rng.uniform(-0.5, 0.5), (H - 1) / 2.0 + rng.uniform(-0.5, 0.5)),
+                         rng.uniform(-180, 180), scale_deg=scale, sip=sip)
+    kernel = "lanczos3" if rng.random() < 0.4 else "bilinear"
+    fr = synth.make_frame(2000 + seed, W, H, 60, wcs, nside, kernel)
+    if seed % 3 == 0:
+        fr = synth.inject_defects(fr)
+    idx_or, dmin = oracle.footprint(wcs, W, H, nside)
+    if dmin <= 1e-9:
+        pytest.skip("seeded pointing sits on a decision boundary")
+    n, idx = argus.argus_healpix_footprint(ctx, wcs, W, H, nside)
+    assert n == len(idx_or)
+    assert np.array_equal(idx.cpu().numpy(), idx_or)
+    d = upload(fr)
+    n, v, w = gpu_resample_planned(ctx, fr, d, kernel)
+    vo, wo, fl = oracle_reference(fr, idx_or, kernel)
+    assert_values_match(v, w, vo, wo, fl, "fuzz %d %s nside 2^%d %dx%d dec %.2f" % (seed, kernel, int(math.log2(nside)), W, H, dec),
+                        min_amb_count=4)
+
+
 def test_tiny_nside_flat_plan(argus, ctx):
     """nside < 256 has no 8x8-tile blocks: the flat plan (one fit per tile) must give the same parity."""
     from gpu_util import assert_values_match, gpu_resample_planned, oracle_reference, upload
