@@ -197,6 +197,37 @@ int argus_resample_coadd(argus_ctx* ctx, const argus_frame* frame, const argus_w
                          int64_t nside, int kernel, float w_min, const argus_coadd* layout, float* sum,
                          float* wsum, int64_t* n_skipped_dev, void* stream);
 
+/* Segment products of a resampled frame: 16-bit float segment data, minipix
+ * stamping against a target list and the low-resolution map (readings in DESIGN.md section 10).
+ *   inputs   idx[n]: DEVICE, ascending unique nested pixels at nside (a footprint); value[n], weight[n]: DEVICE,
+ *            the resampled frame on them; nside, nside_mini: powers of two, nside_mini <= nside <= 2^29 (the paper:
+ *            nside_mini = 16384); a minipix is the 4^j consecutive nested pixels idx >> 2j, 2^j = nside / nside_mini;
+ *            targets[n_targets]: DEVICE, minipix ids at nside_mini that hold a science target (any order,
+ *            duplicates and ids outside the footprint allowed).
+ *   outputs  (all DEVICE, caller-owned, any may be NULL except as noted; "n_mini" = number of distinct minipix
+ *            that own at least one pixel of idx)
+ *            mini_id[k]      ascending minipix ids, k < n_mini (required when mini_capacity > 0)
+ *            mini_weight[k]  sum of weight over the minipix' pixels (FP32, fixed summation order)
+ *            mini_value[k]   sum(weight * value) / sum(weight), 0 where the sum of weights is 0
+ *            mini_keep[k]    1 if mini_id[k] is in targets, else 0 (all mini_capacity bytes are written)
+ *            seg16           IEEE binary16 bits (round to nearest even, finite values clamped to +-65504, NaN ->
+ *                            0x7e00) of value where the pixel's minipix is kept, of 0 elsewhere; with
+ *                            mini_keep == NULL nothing is stamped (plain packing).  layout == NULL: element i <->
+ *                            idx[i] (n elements).  layout != NULL (nside_tile <= nside_mini): scattered to the
+ *                            tile-dense layout slot(p) of argus_coadd, n_tiles * ppt elements; slots outside the
+ *                            footprint are not written (zero the buffer once), pixels of absent tiles are dropped.
+ *            n_mini_dev      DEVICE int64, receives n_mini (asynchronous)
+ *            n_mini_out      HOST; when not NULL the call synchronises the stream and stores n_mini here.
+ * mini_capacity = 0 with every per-minipix output and seg16 NULL only counts.  Minipix beyond mini_capacity are
+ * not written (nor are their seg16 pixels): with n_mini_out the call then returns ARGUS_ERR_CAPACITY and
+ * *n_mini_out holds the required capacity.  The context keeps 8 (mini_capacity + 1) + n / 512 bytes of scratch,
+ * grown on demand (which synchronises the device).  Otherwise asynchronous on `stream`. */
+int argus_segment_products(argus_ctx* ctx, int64_t nside, int64_t nside_mini, const int64_t* idx, const float* value,
+                           const float* weight, size_t n, const int64_t* targets, size_t n_targets,
+                           const argus_coadd* layout, uint16_t* seg16, int64_t* mini_id, float* mini_value,
+                           float* mini_weight, uint8_t* mini_keep, size_t mini_capacity, int64_t* n_mini_dev,
+                           size_t* n_mini_out, void* stream);
+
 /* Synchronises the stream and reports the statistics of the cached plan.  Returns ARGUS_ERR_CAPACITY if
  * an asynchronous call since the last check overflowed its output capacity or the context's max_tiles. */
 int argus_plan_info(argus_ctx* ctx, argus_plan_stats* out, void* stream);

@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     argus_resample_coadd,
     argus_resample_host,
     argus_host_wait,
+    argus_segment_products,
     library_path,
     load_library,
 )

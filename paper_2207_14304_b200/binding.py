@@ -21,7 +21,7 @@ EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
-    "argus_resample_host", "argus_host_wait",
+    "argus_resample_host", "argus_host_wait", "argus_segment_products",
 ]
 
 
@@ -92,6 +92,8 @@ def load_library():
                                        C.POINTER(_Coadd), vp, vp, vp, vp]
     L.argus_resample_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, sz, vp, vp, vp]
     L.argus_host_wait.argtypes = [vp]
+    L.argus_segment_products.argtypes = [vp, i64, i64, vp, vp, vp, sz, vp, sz, C.POINTER(_Coadd), vp, vp, vp, vp, vp, sz,
+                                         vp, C.POINTER(sz), vp]
     L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
     L.argus_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64), vp]
     _lib = L
@@ -337,6 +339,43 @@ def argus_resample_coadd(ctx, wcs, W, H, nside, kernel, tiles, nside_tile, sum_,
                                              _dev(wsum, torch.float32, "wsum"),
                                              _dev(n_skipped, torch.int64, "n_skipped", allow_none=True), _stream(stream))
     _check(ctx, rc, "argus_resample_coadd")
+
+
+def argus_segment_products(ctx, nside, nside_mini, idx, value, weight, targets, seg16=None, mini_id=None, mini_value=None,
+                           mini_weight=None, mini_keep=None, tiles=None, nside_tile=None, n_mini_dev=None, sync=True,
+                           stream=None):
+    """Segment products on caller-allocated CUDA tensors; seg16 is an int16/uint16 tensor that
+    receives binary16 bit patterns.  Returns n_mini when sync, else None.  Capacity = mini_id.numel()."""
+    cap = 0 if mini_id is None else mini_id.numel()
+    for name, t, dt in (("mini_value", mini_value, torch.float32), ("mini_weight", mini_weight, torch.float32),
+                        ("mini_keep", mini_keep, torch.uint8)):
+        if t is not None and t.numel() < cap:
+            raise ValueError("%s is shorter than mini_id" % name)
+    lay = _coadd_struct(tiles, nside_tile) if tiles is not None else None
+    n = idx.numel()
+    if value.numel() != n or weight.numel() != n:
+        raise ValueError("idx, value and weight differ in length")
+    if seg16 is not None:
+        if seg16.dtype not in (torch.int16, torch.uint16, torch.float16):
+            raise TypeError("seg16 must be a 16-bit tensor")
+        need = n if tiles is None else tiles.numel() * (nside // int(nside_tile)) ** 2
+        if seg16.numel() < need:
+            raise ValueError("seg16 holds %d elements, %d needed" % (seg16.numel(), need))
+    nm = C.c_size_t(0)
+    rc = load_library().argus_segment_products(
+        ctx._h, int(nside), int(nside_mini), _dev(idx, torch.int64, "idx") if n else None,
+        _dev(value, torch.float32, "value") if n else None, _dev(weight, torch.float32, "weight") if n else None, n,
+        _dev(targets, torch.int64, "targets") if targets is not None and targets.numel() else None,
+        0 if targets is None else targets.numel(), C.byref(lay) if lay is not None else None,
+        _dev(seg16, seg16.dtype, "seg16") if seg16 is not None else None,
+        _dev(mini_id, torch.int64, "mini_id", allow_none=True), _dev(mini_value, torch.float32, "mini_value", allow_none=True),
+        _dev(mini_weight, torch.float32, "mini_weight", allow_none=True),
+        _dev(mini_keep, torch.uint8, "mini_keep", allow_none=True), cap,
+        _dev(n_mini_dev, torch.int64, "n_mini_dev", allow_none=True), C.byref(nm) if sync else None, _stream(stream))
+    if rc == -6 and sync:
+        raise ArgusError(rc, "argus_segment_products", "n_mini=%d" % nm.value)
+    _check(ctx, rc, "argus_segment_products")
+    return int(nm.value) if sync else None
 
 
 def argus_plan_info(ctx, stream=None) -> dict:

@@ -13,6 +13,7 @@
 #include "plan_block.cuh"
 #include "resample.cuh"
 #include "resample_fast.cuh"
+#include "segments.cuh"
 
 #define ARGUS_VERSION_NUM 100
 #define PLAN_SLOTS 3
@@ -64,6 +65,12 @@ struct argus_ctx {
     } hb[2];
     int hb_next;
     cudaStream_t s_up, s_down;
+    // argus_segment_products: head positions, look-back words ([0] ticket, [1] n_mini, [2..] one per head-scan CTA)
+    struct SegScratch {
+        long long* mini_start; size_t cap_mini;
+        unsigned long long* ctl; size_t cap_ctas;
+        long long* h_n;   // pinned
+    } seg;
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -268,6 +275,9 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
         if (c->hb[i].wgt) cudaFree(c->hb[i].wgt);
         if (c->hb[i].ev_ok) { cudaEventDestroy(c->hb[i].up); cudaEventDestroy(c->hb[i].run); cudaEventDestroy(c->hb[i].down); }
     }
+    if (c->seg.mini_start) cudaFree(c->seg.mini_start);
+    if (c->seg.ctl) cudaFree(c->seg.ctl);
+    if (c->seg.h_n) cudaFreeHost(c->seg.h_n);
     cudaFreeHost(c->h_stats);
     delete c;
     return ARGUS_OK;
@@ -836,5 +846,94 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     mark_slot_read(c, st);
     if (c->profile) { cudaEventRecord(c->ev[slot][3], st); c->ev_plan[slot] = replanned; c->prof_n++; }
     CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+// ---------------------------------------------------------------------------------------- segment products
+extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside_mini, const int64_t* idx,
+                                      const float* value, const float* weight, size_t n, const int64_t* targets,
+                                      size_t n_targets, const argus_coadd* layout, uint16_t* seg16, int64_t* mini_id,
+                                      float* mini_value, float* mini_weight, uint8_t* mini_keep, size_t mini_capacity,
+                                      int64_t* n_mini_dev, size_t* n_mini_out, void* stream) {
+    if (!c) return ARGUS_ERR_NULL;
+    if (n_mini_out) *n_mini_out = 0;
+    if (n > 0 && (!idx || !value || !weight)) return ARGUS_ERR_NULL;
+    if (n_targets > 0 && !targets) return ARGUS_ERR_NULL;
+    if (mini_capacity > 0 && !mini_id) return ARGUS_ERR_NULL;   // the other per-minipix outputs hang off mini_id
+    if (mini_capacity == 0 && (seg16 || mini_value || mini_weight || mini_keep)) return ARGUS_ERR_CAPACITY;
+    if (!is_pow2(nside) || nside > (1ll << 29)) return ARGUS_ERR_NSIDE;
+    if (!is_pow2(nside_mini) || nside_mini > nside) return ARGUS_ERR_NSIDE;
+    if (n > (size_t)12 * (size_t)nside * (size_t)nside || mini_capacity > ((size_t)1 << 40)) return ARGUS_ERR_SHAPE;
+    if (!aligned(idx, 8) || !aligned(value, 4) || !aligned(weight, 4) || !aligned(targets, 8) || !aligned(seg16, 2) ||
+        !aligned(mini_id, 8) || !aligned(mini_value, 4) || !aligned(mini_weight, 4) || !aligned(n_mini_dev, 8))
+        return ARGUS_ERR_ALIGN;
+    const int shift = 2 * (ilog2(nside) - ilog2(nside_mini));
+    SegLayout lay;
+    memset(&lay, 0, sizeof(lay));
+    if (layout) {
+        if (!layout->tiles && layout->n_tiles > 0) return ARGUS_ERR_NULL;
+        if (!is_pow2(layout->nside_tile) || layout->nside_tile > nside_mini || layout->n_tiles < 0) return ARGUS_ERR_SHAPE;
+        if (!aligned(layout->tiles, 8)) return ARGUS_ERR_ALIGN;
+        lay.tiles = (const long long*)layout->tiles;
+        lay.n_tiles = layout->n_tiles;
+        lay.mini_per_tile_log2 = 2 * (ilog2(nside_mini) - ilog2(layout->nside_tile));
+        lay.ppt_log2 = 2 * (ilog2(nside) - ilog2(layout->nside_tile));
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    const size_t n_ctas = (n + SEG_CHUNK - 1) / SEG_CHUNK;
+    if (n_ctas > 0x7fffffffull) return ARGUS_ERR_SHAPE;
+    // scratch (grown on demand: synchronises the device the first time and when a larger call arrives)
+    if (!c->seg.h_n) CUDA_TRY(c, cudaMallocHost((void**)&c->seg.h_n, sizeof(long long)));
+    if (c->seg.cap_ctas < n_ctas || !c->seg.ctl) {
+        if (c->seg.ctl) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->seg.ctl); c->seg.ctl = nullptr; }
+        size_t want = align_up(n_ctas + 1, 4096);
+        CUDA_TRY(c, cudaMalloc((void**)&c->seg.ctl, (want + 2) * sizeof(unsigned long long)));
+        c->seg.cap_ctas = want;
+    }
+    if (c->seg.cap_mini < mini_capacity || !c->seg.mini_start) {
+        if (c->seg.mini_start) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->seg.mini_start); c->seg.mini_start = nullptr; }
+        size_t want = align_up(mini_capacity + 1, 65536);
+        CUDA_TRY(c, cudaMalloc((void**)&c->seg.mini_start, (want + 1) * sizeof(long long)));
+        c->seg.cap_mini = want;
+    }
+    CUDA_TRY(c, cudaMemsetAsync(c->seg.ctl, 0, (n_ctas + 2) * sizeof(unsigned long long), st));
+    if (n_mini_dev && n_ctas == 0) CUDA_TRY(c, cudaMemsetAsync(n_mini_dev, 0, sizeof(int64_t), st));
+    if (n_ctas > 0) {
+        seg_heads_kernel<<<(unsigned)n_ctas, 256, 0, st>>>((const long long*)idx, (long long)n, shift, c->seg.ctl,
+                                                          c->seg.ctl + 2, c->seg.mini_start, (long long*)mini_id,
+                                                          (long long)mini_capacity, (long long*)n_mini_dev);
+        c->n_launches++;
+        if (mini_capacity > 0) {
+            if (mini_keep) {
+                CUDA_TRY(c, cudaMemsetAsync(mini_keep, 0, mini_capacity, st));
+                if (n_targets > 0) {
+                    seg_targets_kernel<<<(unsigned)((n_targets + 255) / 256), 256, 0, st>>>(
+                        (const long long*)targets, (long long)n_targets, (const long long*)mini_id, c->seg.ctl,
+                        (long long)mini_capacity, mini_keep);
+                    c->n_launches++;
+                }
+            }
+            if (seg16 || mini_value || mini_weight) {
+                const int grid = c->sm_count * 6;
+                if (layout)
+                    seg_products_kernel<true><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
+                                                                   c->seg.ctl, (long long)mini_capacity, (const long long*)idx,
+                                                                   value, weight, shift, lay, seg16, mini_value, mini_weight);
+                else
+                    seg_products_kernel<false><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
+                                                                    c->seg.ctl, (long long)mini_capacity, (const long long*)idx,
+                                                                    value, weight, shift, lay, seg16, mini_value, mini_weight);
+                c->n_launches++;
+            }
+        }
+        CUDA_TRY(c, cudaGetLastError());
+    }
+    if (n_mini_out) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->seg.h_n, c->seg.ctl + 1, sizeof(long long), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        *n_mini_out = (size_t)*c->seg.h_n;
+        if (mini_capacity > 0 && *n_mini_out > mini_capacity) return ARGUS_ERR_CAPACITY;
+    }
     return ARGUS_OK;
 }

@@ -26,3 +26,4 @@ from .frames import (  # noqa: F401
     config4_frame,
     special_pointings,
 )
+from .segments import footprint_like, target_list  # noqa: F401,E402
