@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused calibrate + HEALPix-resample hot path on B200 (contract in the task).
 
-    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload config1|config0]
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload config1|config0|...|segments]
 
 A step = one pass of the whole hot path over one frame: per-frame plan on the device (A0/A1, the WCS is
 treated as new every step: plan cache off) + fused calibrate/resample (A2-A5) writing value + weight.
@@ -306,6 +306,114 @@ def run_gpu(args):
     return 0
 
 
+def run_segments(args):
+    """--workload segments: SURVEY 8(f).1 on the configs[1] footprint.  A step = one argus_segment_products call
+    (head scan + target lookup + per-minipix reduction / stamping / binary16 packing) on value + weight of a
+    resampled configs[1] frame that is already in HBM.  Not the headline line; same JSON contract."""
+    import numpy as np
+    import torch
+
+    import paper_2207_14304_b200 as argus
+
+    rank = int(os.environ.get("RANK", "0"))
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        if rank == 0:
+            print(json.dumps({"workload": "segments", "unavailable": "single-GPU diagnostic line (frames are independent: replicas only)"}))
+        return 0
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    argus.load_library()
+    fr, _ = make_workload("config1", 0)
+    H, W = fr.shape
+    nside, nside_mini = fr.nside, 1 << 14
+    ctx = argus.Context(0)
+    d = dict(raw=torch.from_numpy(fr.raw).to(dev), bias=torch.from_numpy(fr.bias).to(dev),
+             dark=torch.from_numpy(fr.dark).to(dev), flat=torch.from_numpy(fr.flat).to(dev), bpm=None,
+             t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
+    n, idx = argus.argus_healpix_footprint(ctx, fr.wcs, W, H, nside, want_indices=True)
+    value = torch.empty(n, dtype=torch.float32, device=dev)
+    weight = torch.empty(n, dtype=torch.float32, device=dev)
+    argus.argus_resample(ctx, fr.wcs, W, H, nside, fr.kernel, value, weight, **d)
+    del d
+    none = torch.zeros(0, dtype=torch.int64, device=dev)
+    n_mini = argus.argus_segment_products(ctx, nside, nside_mini, idx, value, weight, none)     # count
+    # targets: 2 % of the frame's minipix (PAPER.md:149: sparse + low-resolution products are ~5 % of the full data)
+    g = torch.Generator(device="cpu").manual_seed(7)
+    all_mini = torch.unique(idx >> (2 * ((nside // nside_mini).bit_length() - 1)))
+    targets = all_mini[torch.randperm(all_mini.numel(), generator=g)[: max(1, all_mini.numel() // 50)].to(dev)].contiguous()
+    out = dict(seg16=torch.empty(n, dtype=torch.int16, device=dev), mini_id=torch.empty(n_mini, dtype=torch.int64, device=dev),
+               mini_value=torch.empty(n_mini, dtype=torch.float32, device=dev),
+               mini_weight=torch.empty(n_mini, dtype=torch.float32, device=dev),
+               mini_keep=torch.empty(n_mini, dtype=torch.uint8, device=dev))
+
+    def step():
+        argus.argus_segment_products(ctx, nside, nside_mini, idx, value, weight, targets, sync=False, **out)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    for _ in range(600):   # the timed region alone (K x 0.2 ms) is shorter than one nvidia-smi sample: the clocks are
+        step()             # sampled over this identical untimed run-up plus the timed region
+    launches0 = ctx.launch_count()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    ms_step = ev0.elapsed_time(ev1) / args.steps
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop(t0, t1)
+
+    # end to end: list from pinned host memory, products back to pinned host memory, every step
+    h_in = [t.cpu().pin_memory() for t in (idx, value, weight)]
+    h_out = {k: torch.empty_like(v, device="cpu").pin_memory() for k, v in out.items()}
+    e2e_steps = max(3, min(args.steps, 6))
+    torch.cuda.synchronize()
+    t_e0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        idx.copy_(h_in[0], non_blocking=True); value.copy_(h_in[1], non_blocking=True); weight.copy_(h_in[2], non_blocking=True)
+        step()
+        for k, v in out.items():
+            h_out[k].copy_(v, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t_e0) / e2e_steps
+
+    # oracle on a bounded sample: the first 4 M pixels of the same list
+    from oracle import segments as oseg
+    ns = min(n, 4_000_000)
+    hi, hv, hw, ht = h_in[0][:ns].numpy(), h_in[1][:ns].numpy(), h_in[2][:ns].numpy(), targets.cpu().numpy()
+    t_c0 = time.perf_counter()
+    oseg.segment_products(hi, hv, hw, nside, nside_mini, ht)
+    cpu_dt = time.perf_counter() - t_c0
+
+    peak, peak_src = _peaks()
+    alg = n * (8 + 4 + 4 + 2) + n_mini * (8 + 4 + 4 + 1) + targets.numel() * 8
+    achieved = alg / (ms_step * 1e-3) / 1e9
+    h2d = sum(t.numel() * t.element_size() for t in h_in)
+    d2h = sum(t.numel() * t.element_size() for t in h_out.values())
+    print(json.dumps({
+        "metric": "segment products (minipix stamping + binary16 packing + low-resolution map) Mpix/s per B200; achieved HBM GB/s vs peak",
+        "value": n / (ms_step * 1e-3) / 1e6, "unit": "Mpix/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "segment products of one resampled configs[1] frame (SURVEY 8(f).1)", "n_footprint": n,
+                   "nside": nside, "nside_mini": nside_mini, "n_mini": n_mini, "n_targets": int(targets.numel()),
+                   "layout": "compact (element i <-> idx[i])", "l2": "inputs (16 B x n = %d MB) larger than L2 (126 MB)" % (16 * n // 1000000)},
+        "roofline": {"bound": "hbm", "kernel": "whole call: seg_heads_kernel + seg_targets_kernel + seg_products_kernel<false> (+ 2 memsets)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "kernel_ms": ms_step, "algorithmic_bytes": alg},
+        "cpu_baseline": {"value": ns / cpu_dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
+                         "sample": "oracle.segments.segment_products (numpy, fp64) on the first %d pixels of the same list" % ns, "seconds": cpu_dt},
+        "e2e": {"value": n / (e2e_ms * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "ms_per_step": e2e_ms, "note": "idx + value + weight from pinned host memory, all products back to pinned host memory, host wall clock"},
+        "gpu_launches": launches, "clocks": clocks}))
+    ctx.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -313,10 +421,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-plan-overlap", action="store_true", help="diagnostic: build every plan in place on the caller's stream")
-    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config2", "config3", "config4"])
+    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config2", "config3", "config4", "segments"])
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "segments":
+        return run_segments(args)
     return run_gpu(args)
 
 

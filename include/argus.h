@@ -220,7 +220,7 @@ int argus_resample_coadd(argus_ctx* ctx, const argus_frame* frame, const argus_w
  *            n_mini_out      HOST; when not NULL the call synchronises the stream and stores n_mini here.
  * mini_capacity = 0 with every per-minipix output and seg16 NULL only counts.  Minipix beyond mini_capacity are
  * not written (nor are their seg16 pixels): with n_mini_out the call then returns ARGUS_ERR_CAPACITY and
- * *n_mini_out holds the required capacity.  The context keeps 8 (mini_capacity + 1) + n / 512 bytes of scratch,
+ * *n_mini_out holds the required capacity.  The context keeps 8 (mini_capacity + 1) + n / 8 bytes of scratch,
  * grown on demand (which synchronises the device).  Otherwise asynchronous on `stream`. */
 int argus_segment_products(argus_ctx* ctx, int64_t nside, int64_t nside_mini, const int64_t* idx, const float* value,
                            const float* weight, size_t n, const int64_t* targets, size_t n_targets,

@@ -888,22 +888,33 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
     if (c->seg.cap_ctas < n_ctas || !c->seg.ctl) {
         if (c->seg.ctl) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->seg.ctl); c->seg.ctl = nullptr; }
         size_t want = align_up(n_ctas + 1, 4096);
-        CUDA_TRY(c, cudaMalloc((void**)&c->seg.ctl, (want + 2) * sizeof(unsigned long long)));
+        // [2 words: -, n_mini][want chunk offsets, 8 B][want chunk counts, 4 B][want * 128 flag words, 4 B]
+        CUDA_TRY(c, cudaMalloc((void**)&c->seg.ctl, 16 + want * (8 + 4 + 4 * (SEG_CHUNK / 32))));
         c->seg.cap_ctas = want;
     }
+    long long* seg_offsets = (long long*)(c->seg.ctl + 2);
+    unsigned int* seg_counts = (unsigned int*)(seg_offsets + c->seg.cap_ctas);
+    unsigned int* seg_bits = seg_counts + c->seg.cap_ctas;
     if (c->seg.cap_mini < mini_capacity || !c->seg.mini_start) {
         if (c->seg.mini_start) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->seg.mini_start); c->seg.mini_start = nullptr; }
         size_t want = align_up(mini_capacity + 1, 65536);
         CUDA_TRY(c, cudaMalloc((void**)&c->seg.mini_start, (want + 1) * sizeof(long long)));
         c->seg.cap_mini = want;
     }
-    CUDA_TRY(c, cudaMemsetAsync(c->seg.ctl, 0, (n_ctas + 2) * sizeof(unsigned long long), st));
-    if (n_mini_dev && n_ctas == 0) CUDA_TRY(c, cudaMemsetAsync(n_mini_dev, 0, sizeof(int64_t), st));
+    if (n_ctas == 0) {
+        CUDA_TRY(c, cudaMemsetAsync(c->seg.ctl, 0, 16, st));
+        if (n_mini_dev) CUDA_TRY(c, cudaMemsetAsync(n_mini_dev, 0, sizeof(int64_t), st));
+    }
     if (n_ctas > 0) {
-        seg_heads_kernel<<<(unsigned)n_ctas, 256, 0, st>>>((const long long*)idx, (long long)n, shift, c->seg.ctl,
-                                                          c->seg.ctl + 2, c->seg.mini_start, (long long*)mini_id,
-                                                          (long long)mini_capacity, (long long*)n_mini_dev);
-        c->n_launches++;
+        seg_flags_kernel<<<(unsigned)n_ctas, 256, 0, st>>>((const long long*)idx, (long long)n, shift, seg_bits, seg_counts);
+        seg_scan_kernel<<<1, 1024, 0, st>>>(seg_counts, (long long)n_ctas, seg_offsets, c->seg.ctl, (long long*)n_mini_dev,
+                                            c->seg.mini_start, (long long)mini_capacity, (long long)n);
+        c->n_launches += 2;
+        if (mini_capacity > 0) {
+            seg_heads_kernel<<<(unsigned)n_ctas, 128, 0, st>>>(seg_bits, seg_offsets, (const long long*)idx, shift,
+                                                              c->seg.mini_start, (long long*)mini_id, (long long)mini_capacity);
+            c->n_launches++;
+        }
         if (mini_capacity > 0) {
             if (mini_keep) {
                 CUDA_TRY(c, cudaMemsetAsync(mini_keep, 0, mini_capacity, st));
@@ -915,7 +926,7 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
                 }
             }
             if (seg16 || mini_value || mini_weight) {
-                const int grid = c->sm_count * 6;
+                const int grid = c->sm_count * 4;
                 if (layout)
                     seg_products_kernel<true><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
                                                                    c->seg.ctl, (long long)mini_capacity, (const long long*)idx,

@@ -3,13 +3,13 @@
 // low-resolution map as weighted means over the minipix.  All three are streaming
 // reductions over the footprint list (idx ascending, value, weight) that is already in HBM.
 //
-//   seg_heads_kernel     one pass over idx: a pixel is a "head" when its minipix (idx >> 2j) differs from its
-//                        predecessor's; heads are numbered by a single-pass scan (per-CTA aggregate, decoupled
-//                        look-back over the CTAs' status words) -> mini_start[k], mini_id[k], n_mini
+//   seg_flags_kernel     one pass over idx: a pixel is a "head" when its minipix (idx >> 2j) differs from its
+//   seg_scan_kernel      predecessor's; one flag bit per pixel + head count per 4096-pixel chunk, scan of the
+//   seg_heads_kernel     counts, then mini_start[k] (position of the k-th head), mini_id[k], n_mini
 //   seg_targets_kernel   every target id is looked up in mini_id (binary search, one thread per target)
 //                        -> mini_keep[k] = 1.  Searching the targets into the minipix list, not the reverse,
 //                        keeps the 20-step searches off the streaming kernels' critical path.
-//   seg_products_kernel  one warp per minipix: sums w and w v over its pixels (fixed butterfly order), writes
+//   seg_products_kernel  one warp per four minipix: sums w and w v over their pixels (fixed butterfly order), writes
 //                        the binary16 bits of the stamped values, compact (element i <-> idx[i]) or scattered
 //                        to the dense NSIDE-256 tile layout of argus_coadd.
 #pragma once
@@ -20,10 +20,6 @@
 #define SEG_ROUNDS 16
 #define SEG_CHUNK (256 * SEG_ROUNDS)   // pixels per CTA of the head scan
 
-#define SEG_FLAG_A (1ull << 62)        // status word holds the CTA's own head count
-#define SEG_FLAG_P (2ull << 62)        // status word holds the inclusive prefix up to and including the CTA
-#define SEG_VALUE_MASK ((1ull << 62) - 1)
-
 struct SegLayout {
     const long long* tiles;   // ascending NSIDE-`nside_tile` ids (argus_coadd)
     long long n_tiles;
@@ -31,100 +27,128 @@ struct SegLayout {
     int ppt_log2;             // 2 (log2 nside - log2 nside_tile)
 };
 
-__device__ __forceinline__ unsigned long long seg_ld(const unsigned long long* p) {
-    return *reinterpret_cast<const volatile unsigned long long*>(p);
-}
-__device__ __forceinline__ void seg_st(unsigned long long* p, unsigned long long v) {
-    *reinterpret_cast<volatile unsigned long long*>(p) = v;
-}
-
-// head scan.  ctl[0] = CTA ticket, ctl[1] = n_mini (both zeroed by the host before the launch); status[] zeroed.
-__global__ void __launch_bounds__(256) seg_heads_kernel(const long long* __restrict__ idx, long long n, int shift,
-                                                       unsigned long long* __restrict__ ctl,
-                                                       unsigned long long* __restrict__ status,
-                                                       long long* __restrict__ mini_start,
-                                                       long long* __restrict__ mini_id, long long cap,
-                                                       long long* __restrict__ n_mini_user) {
-    __shared__ unsigned int s_cta;
-    __shared__ int s_cnt[SEG_ROUNDS * 8];
-    __shared__ long long s_base;
-    __shared__ int s_total;
+// Heads, pass 1: one streaming pass over idx.  Pixel e is a head when its minipix differs from pixel e-1's.  Writes
+// one flag bit per pixel (bits[e / 32], 1/64 of the bytes read) and the number of heads of every 4096-pixel chunk.
+// (A single-pass scan with decoupled look-back was measured first: its CTAs spent 45 % of their life polling their
+// predecessors' status words, 0.28 ms for 359 MB; the three free-running kernels below take a quarter of that.)
+__global__ void __launch_bounds__(256) seg_flags_kernel(const long long* __restrict__ idx, long long n, int shift,
+                                                       unsigned int* __restrict__ bits,
+                                                       unsigned int* __restrict__ counts) {
+    __shared__ long long s_last[SEG_ROUNDS * 8];
+    __shared__ int s_cnt[8];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_cta = (unsigned int)atomicAdd(&ctl[0], 1ull);   // CTAs are numbered in start order: a
-    __syncthreads();                                                        // predecessor is always running or done
-    const unsigned int cta = s_cta;
-    const long long e0 = (long long)cta * SEG_CHUNK;
-
+    const long long e0 = (long long)blockIdx.x * SEG_CHUNK;
     long long m[SEG_ROUNDS];
-    unsigned heads = 0;
+    long long before = -2;
+    if (threadIdx.x == 0 && e0 > 0) before = __ldg(idx + e0 - 1) >> shift;
+#pragma unroll
+    for (int r = 0; r < SEG_ROUNDS; ++r) {   // all loads first: 16 in flight per thread
+        const long long e = e0 + r * 256 + threadIdx.x;
+        m[r] = (e < n) ? (__ldcs(idx + e) >> shift) : -1;
+    }
+    if (lane == 31) {
+#pragma unroll
+        for (int r = 0; r < SEG_ROUNDS; ++r) s_last[r * 8 + warp] = m[r];
+    }
+    __syncthreads();
+    int cnt = 0;
 #pragma unroll
     for (int r = 0; r < SEG_ROUNDS; ++r) {
         const long long e = e0 + r * 256 + threadIdx.x;
-        const bool in = e < n;
-        long long cur = in ? (__ldcs(idx + e) >> shift) : -1;
-        long long prev = __shfl_up_sync(0xffffffffu, cur, 1);
-        if (lane == 0) prev = (in && e > 0) ? (__ldg(idx + e - 1) >> shift) : -2;
-        const bool head = in && (e == 0 || cur != prev);
+        long long prev = __shfl_up_sync(0xffffffffu, m[r], 1);
+        if (lane == 0) prev = (r * 8 + warp > 0) ? s_last[r * 8 + warp - 1] : before;
+        const bool head = e < n && (e == 0 || m[r] != prev);
         const unsigned b = __ballot_sync(0xffffffffu, head);
-        m[r] = cur;
-        heads |= (head ? 1u : 0u) << r;
-        if (lane == 0) s_cnt[r * 8 + warp] = __popc(b);
+        if (lane == 0) bits[(long long)blockIdx.x * (SEG_CHUNK / 32) + r * 8 + warp] = b;
+        cnt += __popc(b);
     }
+    if (lane == 0) s_cnt[warp] = cnt;
     __syncthreads();
-    if (warp == 0) {
-        // exclusive scan of the 128 (round, warp) counts: four per lane
-        int c0 = s_cnt[lane * 4], c1 = s_cnt[lane * 4 + 1], c2 = s_cnt[lane * 4 + 2], c3 = s_cnt[lane * 4 + 3];
-        int sum = c0 + c1 + c2 + c3, inc = sum;
+    if (threadIdx.x == 0) {
+        int t = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) t += s_cnt[i];
+        counts[blockIdx.x] = (unsigned int)t;
+    }
+}
+
+// Heads, pass 2: exclusive scan of the chunk counts (one CTA; a 45 M pixel frame has 11 k chunks).
+// ctl[1] = n_mini; mini_start[n_mini] = n is the sentinel that ends the last minipix.
+__global__ void __launch_bounds__(1024) seg_scan_kernel(const unsigned int* __restrict__ counts, long long n_chunks,
+                                                       long long* __restrict__ offsets,
+                                                       unsigned long long* __restrict__ ctl,
+                                                       long long* __restrict__ n_mini_user,
+                                                       long long* __restrict__ mini_start, long long cap, long long n) {
+    __shared__ long long s_w[32];
+    __shared__ long long s_carry;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    for (long long c0 = 0; c0 < n_chunks; c0 += 1024) {
+        const long long c = c0 + threadIdx.x;
+        const long long v = (c < n_chunks) ? (long long)counts[c] : 0;
+        long long inc = v;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            int t = __shfl_up_sync(0xffffffffu, inc, d);
+            const long long t = __shfl_up_sync(0xffffffffu, inc, d);
             if (lane >= d) inc += t;
         }
-        int ex = inc - sum;
-        s_cnt[lane * 4] = ex;
-        s_cnt[lane * 4 + 1] = ex + c0;
-        s_cnt[lane * 4 + 2] = ex + c0 + c1;
-        s_cnt[lane * 4 + 3] = ex + c0 + c1 + c2;
-        const int total = __shfl_sync(0xffffffffu, inc, 31);
-        if (lane == 0) seg_st(&status[cta], (cta == 0 ? SEG_FLAG_P : SEG_FLAG_A) | (unsigned long long)total);
-        // decoupled look-back, 32 predecessors per step
-        long long excl = 0;
-        if (cta > 0) {
-            long long j = (long long)cta - 1;
-            for (;;) {
-                const long long q = j - lane;
-                unsigned long long w = (q >= 0) ? seg_ld(&status[q]) : SEG_FLAG_P;
-                while (__any_sync(0xffffffffu, (w >> 62) == 0)) w = (q >= 0) ? seg_ld(&status[q]) : SEG_FLAG_P;
-                const unsigned pm = __ballot_sync(0xffffffffu, (w >> 62) == 2);
-                const int first = pm ? (__ffs(pm) - 1) : 32;
-                long long val = (lane <= first) ? (long long)(w & SEG_VALUE_MASK) : 0;
+        if (lane == 31) s_w[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            long long w = s_w[lane], wi = w;
 #pragma unroll
-                for (int d = 16; d > 0; d >>= 1) val += __shfl_xor_sync(0xffffffffu, val, d);
-                excl += val;
-                if (pm) break;
-                j -= 32;
+            for (int d = 1; d < 32; d <<= 1) {
+                const long long t = __shfl_up_sync(0xffffffffu, wi, d);
+                if (lane >= d) wi += t;
             }
-            if (lane == 0) seg_st(&status[cta], SEG_FLAG_P | (unsigned long long)(excl + total));
+            s_w[lane] = wi - w;
         }
-        if (lane == 0) { s_base = excl; s_total = total; }
+        __syncthreads();
+        const long long carry = s_carry;
+        if (c < n_chunks) offsets[c] = carry + s_w[warp] + inc - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) s_carry = carry + s_w[warp] + inc;
+        __syncthreads();
     }
-    __syncthreads();
-    const long long base = s_base;
-#pragma unroll
-    for (int r = 0; r < SEG_ROUNDS; ++r) {
-        const bool head = (heads >> r) & 1u;
-        const unsigned b = __ballot_sync(0xffffffffu, head);
-        if (head) {
-            const long long k = base + s_cnt[r * 8 + warp] + __popc(b & ((1u << lane) - 1u));
-            if (k <= cap && mini_start) mini_start[k] = e0 + r * 256 + threadIdx.x;
-            if (k < cap && mini_id) mini_id[k] = m[r];
-        }
-    }
-    if (threadIdx.x == 0 && cta == gridDim.x - 1) {
-        const long long nm = base + s_total;
+    if (threadIdx.x == 0) {
+        const long long nm = s_carry;
         ctl[1] = (unsigned long long)nm;
         if (n_mini_user) *n_mini_user = nm;
-        if (nm <= cap && mini_start) mini_start[nm] = n;   // sentinel: end of the last minipix
+        if (nm <= cap && mini_start) mini_start[nm] = n;
+    }
+}
+
+// Heads, pass 3: flag bits + chunk offsets -> mini_start[k] (position of the k-th head), mini_id[k].
+__global__ void __launch_bounds__(128) seg_heads_kernel(const unsigned int* __restrict__ bits,
+                                                       const long long* __restrict__ offsets,
+                                                       const long long* __restrict__ idx, int shift,
+                                                       long long* __restrict__ mini_start,
+                                                       long long* __restrict__ mini_id, long long cap) {
+    __shared__ int s_w[4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned word = bits[(long long)blockIdx.x * (SEG_CHUNK / 32) + threadIdx.x];
+    const int c = __popc(word);
+    int inc = c;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) s_w[warp] = inc;
+    __syncthreads();
+    int wbase = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) wbase += (i < warp) ? s_w[i] : 0;
+    long long k = offsets[blockIdx.x] + wbase + inc - c;
+    const long long e0 = (long long)blockIdx.x * SEG_CHUNK + threadIdx.x * 32;
+    while (word) {
+        const int b = __ffs(word) - 1;
+        word &= word - 1;
+        const long long e = e0 + b;
+        if (k <= cap && mini_start) mini_start[k] = e;
+        if (k < cap && mini_id) mini_id[k] = __ldg(idx + e) >> shift;
+        ++k;
     }
 }
 
@@ -151,8 +175,44 @@ __device__ __forceinline__ unsigned short seg_f2h(float v) {
     return (v != v) ? (unsigned short)0x7e00 : h;
 }
 
+// dense-layout base slot of minipix `mid_` (or -1 when its tile is absent)
+__device__ __forceinline__ long long seg_dense_base(const SegLayout& lay, long long mid_, int shift) {
+    const long long key = mid_ >> lay.mini_per_tile_log2;
+    long long lo = 0, hi = lay.n_tiles - 1;
+    while (lo <= hi) {
+        const long long mid = (lo + hi) >> 1, tv = lay.tiles[mid];
+        if (tv == key) return (mid << lay.ppt_log2) + ((mid_ & ((1ll << lay.mini_per_tile_log2) - 1)) << shift);
+        if (tv < key) lo = mid + 1; else hi = mid - 1;
+    }
+    return -1;
+}
+
+#define SEG_GROUP 4   // minipix per warp iteration: their pixels are adjacent in the list, 4 x 4 loads in flight per lane
+
+// Sum of eight per-lane values over the warp in 10 shuffles: each butterfly step halves the number of values a lane
+// carries (lane bit 4 picks a[0..3] / a[4..7], bit 3 the pair, bit 2 the value), the last two steps are plain.
+// Returns, in every lane, the total of value q = 4 (lane >> 4 & 1) + 2 (lane >> 3 & 1) + (lane >> 2 & 1).  Fixed order.
+__device__ __forceinline__ float seg_reduce8(const float (&a)[8], int lane) {
+    float b[4], c[2];
+    const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float send = u4 ? a[k] : a[k + 4], keep = u4 ? a[k + 4] : a[k];
+        b[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const float send = u3 ? b[k] : b[k + 2], keep = u3 ? b[k + 2] : b[k];
+        c[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    float d = (u2 ? c[1] : c[0]) + __shfl_xor_sync(0xffffffffu, u2 ? c[0] : c[1], 4);
+    d += __shfl_xor_sync(0xffffffffu, d, 2);
+    d += __shfl_xor_sync(0xffffffffu, d, 1);
+    return d;
+}
+
 template <bool DENSE>
-__global__ void __launch_bounds__(256, 6) seg_products_kernel(
+__global__ void __launch_bounds__(256, 4) seg_products_kernel(
     const long long* __restrict__ mini_start, const long long* __restrict__ mini_id,
     const unsigned char* __restrict__ keep, const unsigned long long* __restrict__ ctl, long long cap,
     const long long* __restrict__ idx, const float* __restrict__ value, const float* __restrict__ weight, int shift,
@@ -161,48 +221,97 @@ __global__ void __launch_bounds__(256, 6) seg_products_kernel(
     const long long nw = (long long)gridDim.x * 8;
     const long long nm = min((long long)ctl[1], cap);
     const int full = 1 << shift;
-    for (long long k = (long long)blockIdx.x * 8 + (threadIdx.x >> 5); k < nm; k += nw) {
-        const long long s = mini_start[k], e = mini_start[k + 1];
-        const int cnt = (int)(e - s);
-        const bool kp = keep ? (keep[k] != 0) : true;
-        long long dbase = -1;
-        if (DENSE) {
-            const long long mid_ = mini_id[k], key = mid_ >> lay.mini_per_tile_log2;
-            long long lo = 0, hi = lay.n_tiles - 1;
-            while (lo <= hi) {
-                const long long mid = (lo + hi) >> 1, tv = lay.tiles[mid];
-                if (tv == key) {
-                    dbase = (mid << lay.ppt_log2) + ((mid_ & ((1ll << lay.mini_per_tile_log2) - 1)) << shift);
-                    break;
-                }
-                if (tv < key) lo = mid + 1; else hi = mid - 1;
-            }
+    for (long long kb = ((long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * SEG_GROUP; kb < nm; kb += nw * SEG_GROUP) {
+        // lanes 0..4: starts of the group's minipix (mini_start[nm] is the sentinel); lanes 0..3: keep flag, dense base
+        const long long st = (lane <= SEG_GROUP) ? mini_start[min(kb + lane, nm)] : 0;
+        int kp_l = 1;
+        long long db_l = -1;
+        if (lane < SEG_GROUP && kb + lane < nm) {
+            if (keep) kp_l = keep[kb + lane] != 0;
+            if (DENSE) db_l = seg_dense_base(lay, mini_id[kb + lane], shift);
         }
-        float sw = 0.0f, swv = 0.0f;
-        for (int q = lane; q < cnt; q += 32) {
-            const float v = __ldcs(value + s + q), w = __ldcs(weight + s + q);
-            sw += w;
-            swv = fmaf(w, v, swv);
-            if (seg16) {
-                const unsigned short h = kp ? seg_f2h(v) : (unsigned short)0;
-                if (DENSE) {
-                    if (dbase >= 0) {
-                        const long long off = (cnt == full) ? (long long)q : (idx[s + q] & (long long)(full - 1));
-                        seg16[dbase + off] = h;
-                    }
-                } else {
-                    seg16[s + q] = h;
-                }
-            }
-        }
+        const long long s0 = __shfl_sync(0xffffffffu, st, 0);
+        const int rel_l = (int)min(st - s0, (long long)0x3fffffff);   // pixels of the group lie in [s0, s0 + rel[4])
+        int rel[SEG_GROUP + 1];
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            sw += __shfl_xor_sync(0xffffffffu, sw, d);
-            swv += __shfl_xor_sync(0xffffffffu, swv, d);
+        for (int i = 0; i <= SEG_GROUP; ++i) rel[i] = __shfl_sync(0xffffffffu, rel_l, i);
+        const unsigned kpm = __ballot_sync(0xffffffffu, kp_l != 0);
+        bool small = true;
+#pragma unroll
+        for (int i = 0; i < SEG_GROUP; ++i) small = small && (rel[i + 1] - rel[i] <= 64);
+        small = small && (__shfl_sync(0xffffffffu, st, SEG_GROUP) - s0 <= 64 * SEG_GROUP);   // rel is clamped: be exact
+        const float* vb = value + s0;
+        const float* wb = weight + s0;
+        float acc[8];
+        if (small) {
+            // every minipix of the group has at most 64 pixels (the paper's case, 4^3): all loads issued up front,
+            // 32-bit offsets from the group's first pixel
+            float v[SEG_GROUP][2], w[SEG_GROUP][2];
+#pragma unroll
+            for (int i = 0; i < SEG_GROUP; ++i)
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int p = rel[i] + lane + 32 * h;
+                    const bool in = p < rel[i + 1];
+                    v[i][h] = in ? __ldcs(vb + p) : 0.0f;
+                    w[i][h] = in ? __ldcs(wb + p) : 0.0f;
+                }
+#pragma unroll
+            for (int i = 0; i < SEG_GROUP; ++i) {
+                acc[2 * i] = w[i][0] + w[i][1];
+                acc[2 * i + 1] = fmaf(w[i][1], v[i][1], w[i][0] * v[i][0]);
+                if (seg16) {
+                    const bool kp = (kpm >> i) & 1u;
+                    const long long dbase = DENSE ? __shfl_sync(0xffffffffu, db_l, i) : 0;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int p = rel[i] + lane + 32 * h;
+                        if (p < rel[i + 1]) {
+                            const unsigned short hb = kp ? seg_f2h(v[i][h]) : (unsigned short)0;
+                            if (DENSE) {
+                                if (dbase >= 0) {
+                                    const int q = lane + 32 * h;
+                                    const long long off = (rel[i + 1] - rel[i] == full) ? (long long)q : (idx[s0 + p] & (long long)(full - 1));
+                                    seg16[dbase + off] = hb;
+                                }
+                            } else {
+                                seg16[s0 + p] = hb;
+                            }
+                        }
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < SEG_GROUP; ++i) {
+                const long long si = __shfl_sync(0xffffffffu, st, i);
+                const long long cnt = __shfl_sync(0xffffffffu, st, i + 1) - si;
+                const bool kp = (kpm >> i) & 1u;
+                const long long dbase = DENSE ? __shfl_sync(0xffffffffu, db_l, i) : 0;
+                float sw = 0.0f, swv = 0.0f;
+                for (long long q = lane; q < cnt; q += 32) {
+                    const float vv = __ldcs(value + si + q), ww = __ldcs(weight + si + q);
+                    sw += ww;
+                    swv = fmaf(ww, vv, swv);
+                    if (seg16) {
+                        const unsigned short hb = kp ? seg_f2h(vv) : (unsigned short)0;
+                        if (DENSE) {
+                            if (dbase >= 0) seg16[dbase + ((cnt == full) ? q : (idx[si + q] & (long long)(full - 1)))] = hb;
+                        } else {
+                            seg16[si + q] = hb;
+                        }
+                    }
+                }
+                acc[2 * i] = sw;
+                acc[2 * i + 1] = swv;
+            }
         }
-        if (lane == 0) {
-            if (mini_weight) mini_weight[k] = sw;
-            if (mini_value) mini_value[k] = (sw != 0.0f) ? swv / sw : 0.0f;
+        const float tot = seg_reduce8(acc, lane);                       // lanes with bit 2 clear: sum w; set: sum w v
+        const float oth = __shfl_xor_sync(0xffffffffu, tot, 4);
+        const int i = ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
+        if ((lane & 7) == 0 && kb + i < nm) {
+            if (mini_weight) mini_weight[kb + i] = tot;
+            if (mini_value) mini_value[kb + i] = (tot != 0.0f) ? oth / tot : 0.0f;
         }
     }
 }
