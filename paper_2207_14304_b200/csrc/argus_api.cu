@@ -906,12 +906,13 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
         if (n_mini_dev) CUDA_TRY(c, cudaMemsetAsync(n_mini_dev, 0, sizeof(int64_t), st));
     }
     if (n_ctas > 0) {
+        if (n_ctas % 32) CUDA_TRY(c, cudaMemsetAsync(seg_counts + n_ctas, 0, (32 - n_ctas % 32) * sizeof(unsigned int), st));
         seg_flags_kernel<<<(unsigned)n_ctas, 256, 0, st>>>((const long long*)idx, (long long)n, shift, seg_bits, seg_counts);
         seg_scan_kernel<<<1, 1024, 0, st>>>(seg_counts, (long long)n_ctas, seg_offsets, c->seg.ctl, (long long*)n_mini_dev,
                                             c->seg.mini_start, (long long)mini_capacity, (long long)n);
         c->n_launches += 2;
         if (mini_capacity > 0) {
-            seg_heads_kernel<<<(unsigned)n_ctas, 128, 0, st>>>(seg_bits, seg_offsets, (const long long*)idx, shift,
+            seg_heads_kernel<<<(unsigned)n_ctas, SEG_CHUNK / 32, 0, st>>>(seg_bits, seg_counts, seg_offsets, (const long long*)idx, shift,
                                                               c->seg.mini_start, (long long*)mini_id, (long long)mini_capacity);
             c->n_launches++;
         }

@@ -17,7 +17,7 @@
 
 #include "common.cuh"
 
-#define SEG_ROUNDS 16
+#define SEG_ROUNDS 8
 #define SEG_CHUNK (256 * SEG_ROUNDS)   // pixels per CTA of the head scan
 
 struct SegLayout {
@@ -72,21 +72,31 @@ __global__ void __launch_bounds__(256) seg_flags_kernel(const long long* __restr
     }
 }
 
-// Heads, pass 2: exclusive scan of the chunk counts (one CTA; a 45 M pixel frame has 11 k chunks).
-// ctl[1] = n_mini; mini_start[n_mini] = n is the sentinel that ends the last minipix.
+// Heads, pass 2: exclusive scan of the chunk counts at the granularity of 32 chunks (one CTA: thread t sums chunks
+// 32 t .. 32 t + 31 with eight independent 16-byte loads, so a 45 M pixel frame is one round of one load latency);
+// pass 3 adds the up to 31 counts in front of its own chunk.  ctl[1] = n_mini; mini_start[n_mini] = n is the
+// sentinel that ends the last minipix.  `counts` is padded to a multiple of 32 chunks (zeros past n_chunks).
 __global__ void __launch_bounds__(1024) seg_scan_kernel(const unsigned int* __restrict__ counts, long long n_chunks,
-                                                       long long* __restrict__ offsets,
+                                                       long long* __restrict__ offsets32,
                                                        unsigned long long* __restrict__ ctl,
                                                        long long* __restrict__ n_mini_user,
                                                        long long* __restrict__ mini_start, long long cap, long long n) {
     __shared__ long long s_w[32];
     __shared__ long long s_carry;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_carry = 0;
-    __syncthreads();
-    for (long long c0 = 0; c0 < n_chunks; c0 += 1024) {
-        const long long c = c0 + threadIdx.x;
-        const long long v = (c < n_chunks) ? (long long)counts[c] : 0;
+    const long long n32 = (n_chunks + 31) / 32;
+    long long carry = 0;
+    for (long long base = 0; base < n32; base += 1024) {
+        const long long g = base + threadIdx.x;
+        long long v = 0;
+        if (g < n32) {
+            const uint4* q = reinterpret_cast<const uint4*>(counts + g * 32);
+            uint4 r[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) r[i] = q[i];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v += (long long)r[i].x + r[i].y + r[i].z + r[i].w;
+        }
         long long inc = v;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -103,16 +113,15 @@ __global__ void __launch_bounds__(1024) seg_scan_kernel(const unsigned int* __re
                 if (lane >= d) wi += t;
             }
             s_w[lane] = wi - w;
+            if (lane == 31) s_carry = wi;
         }
         __syncthreads();
-        const long long carry = s_carry;
-        if (c < n_chunks) offsets[c] = carry + s_w[warp] + inc - v;
-        __syncthreads();
-        if (threadIdx.x == 1023) s_carry = carry + s_w[warp] + inc;
+        if (g < n32) offsets32[g] = carry + s_w[warp] + inc - v;
+        carry += s_carry;
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        const long long nm = s_carry;
+        const long long nm = carry;
         ctl[1] = (unsigned long long)nm;
         if (n_mini_user) *n_mini_user = nm;
         if (nm <= cap && mini_start) mini_start[nm] = n;
@@ -120,13 +129,21 @@ __global__ void __launch_bounds__(1024) seg_scan_kernel(const unsigned int* __re
 }
 
 // Heads, pass 3: flag bits + chunk offsets -> mini_start[k] (position of the k-th head), mini_id[k].
-__global__ void __launch_bounds__(128) seg_heads_kernel(const unsigned int* __restrict__ bits,
-                                                       const long long* __restrict__ offsets,
+__global__ void __launch_bounds__(SEG_CHUNK / 32) seg_heads_kernel(const unsigned int* __restrict__ bits,
+                                                       const unsigned int* __restrict__ counts,
+                                                       const long long* __restrict__ offsets32,
                                                        const long long* __restrict__ idx, int shift,
                                                        long long* __restrict__ mini_start,
                                                        long long* __restrict__ mini_id, long long cap) {
-    __shared__ int s_w[4];
+    __shared__ int s_w[SEG_CHUNK / 1024];
+    __shared__ int s_front;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (warp == 0) {   // heads of the chunks in front of this one inside its group of 32
+        int f = (lane < (int)(blockIdx.x & 31u)) ? (int)counts[(blockIdx.x & ~31u) + lane] : 0;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) f += __shfl_xor_sync(0xffffffffu, f, d);
+        if (lane == 0) s_front = f;
+    }
     unsigned word = bits[(long long)blockIdx.x * (SEG_CHUNK / 32) + threadIdx.x];
     const int c = __popc(word);
     int inc = c;
@@ -139,8 +156,8 @@ __global__ void __launch_bounds__(128) seg_heads_kernel(const unsigned int* __re
     __syncthreads();
     int wbase = 0;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) wbase += (i < warp) ? s_w[i] : 0;
-    long long k = offsets[blockIdx.x] + wbase + inc - c;
+    for (int i = 0; i < SEG_CHUNK / 1024; ++i) wbase += (i < warp) ? s_w[i] : 0;
+    long long k = offsets32[blockIdx.x >> 5] + s_front + wbase + inc - c;
     const long long e0 = (long long)blockIdx.x * SEG_CHUNK + threadIdx.x * 32;
     while (word) {
         const int b = __ffs(word) - 1;
@@ -247,37 +264,37 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
             // every minipix of the group has at most 64 pixels (the paper's case, 4^3): all loads issued up front,
             // 32-bit offsets from the group's first pixel
             float v[SEG_GROUP][2], w[SEG_GROUP][2];
+            int left[SEG_GROUP];                           // pixels of minipix i from this lane's first one on
 #pragma unroll
-            for (int i = 0; i < SEG_GROUP; ++i)
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int p = rel[i] + lane + 32 * h;
-                    const bool in = p < rel[i + 1];
-                    v[i][h] = in ? __ldcs(vb + p) : 0.0f;
-                    w[i][h] = in ? __ldcs(wb + p) : 0.0f;
-                }
+            for (int i = 0; i < SEG_GROUP; ++i) {
+                const float* vi = vb + (rel[i] + lane);    // one 64-bit address per minipix and array; the second
+                const float* wi = wb + (rel[i] + lane);    // pixel of the lane is 128 B further
+                left[i] = rel[i + 1] - rel[i] - lane;
+                v[i][0] = (left[i] > 0) ? __ldcs(vi) : 0.0f;
+                w[i][0] = (left[i] > 0) ? __ldcs(wi) : 0.0f;
+                v[i][1] = (left[i] > 32) ? __ldcs(vi + 32) : 0.0f;
+                w[i][1] = (left[i] > 32) ? __ldcs(wi + 32) : 0.0f;
+            }
 #pragma unroll
             for (int i = 0; i < SEG_GROUP; ++i) {
                 acc[2 * i] = w[i][0] + w[i][1];
                 acc[2 * i + 1] = fmaf(w[i][1], v[i][1], w[i][0] * v[i][0]);
                 if (seg16) {
                     const bool kp = (kpm >> i) & 1u;
-                    const long long dbase = DENSE ? __shfl_sync(0xffffffffu, db_l, i) : 0;
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int p = rel[i] + lane + 32 * h;
-                        if (p < rel[i + 1]) {
-                            const unsigned short hb = kp ? seg_f2h(v[i][h]) : (unsigned short)0;
-                            if (DENSE) {
-                                if (dbase >= 0) {
-                                    const int q = lane + 32 * h;
-                                    const long long off = (rel[i + 1] - rel[i] == full) ? (long long)q : (idx[s0 + p] & (long long)(full - 1));
-                                    seg16[dbase + off] = hb;
-                                }
-                            } else {
-                                seg16[s0 + p] = hb;
-                            }
+                    const unsigned short h0 = kp ? seg_f2h(v[i][0]) : (unsigned short)0;
+                    const unsigned short h1 = kp ? seg_f2h(v[i][1]) : (unsigned short)0;
+                    if (DENSE) {
+                        const long long dbase = __shfl_sync(0xffffffffu, db_l, i);
+                        if (dbase >= 0) {
+                            const bool complete = rel[i + 1] - rel[i] == full;
+                            const long long* ii = idx + s0 + (rel[i] + lane);
+                            if (left[i] > 0) seg16[dbase + (complete ? (long long)lane : (ii[0] & (long long)(full - 1)))] = h0;
+                            if (left[i] > 32) seg16[dbase + (complete ? (long long)(lane + 32) : (ii[32] & (long long)(full - 1)))] = h1;
                         }
+                    } else {
+                        unsigned short* oi = seg16 + s0 + (rel[i] + lane);
+                        if (left[i] > 0) oi[0] = h0;
+                        if (left[i] > 32) oi[32] = h1;
                     }
                 }
             }
