@@ -32,6 +32,7 @@ SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload reci
 # dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
 # profiles/r1_final_ncu_summary.txt (ncu --set full).
 NCU_TRAFFIC_BYTES = 983571968 + 339383296  # profiles/r1_final_ncu_summary.txt
+NCU_SEG_TRAFFIC_BYTES = 359159552 + 7175936 + 365523712 + 41991424  # profiles/r1_segments_ncu_summary.txt
 
 
 def _peaks():
@@ -382,9 +383,9 @@ def run_segments(args):
         torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t_e0) / e2e_steps
 
-    # oracle on a bounded sample: the first 4 M pixels of the same list
+    # the oracle, as it stands, on the same list
     from oracle import segments as oseg
-    ns = min(n, 4_000_000)
+    ns = n   # the numpy oracle does the whole list in a few seconds
     hi, hv, hw, ht = h_in[0][:ns].numpy(), h_in[1][:ns].numpy(), h_in[2][:ns].numpy(), targets.cpu().numpy()
     t_c0 = time.perf_counter()
     oseg.segment_products(hi, hv, hw, nside, nside_mini, ht)
@@ -402,11 +403,12 @@ def run_segments(args):
         "config": {"workload": "segment products of one resampled configs[1] frame (SURVEY 8(f).1)", "n_footprint": n,
                    "nside": nside, "nside_mini": nside_mini, "n_mini": n_mini, "n_targets": int(targets.numel()),
                    "layout": "compact (element i <-> idx[i])", "l2": "inputs (16 B x n = %d MB) larger than L2 (126 MB)" % (16 * n // 1000000)},
-        "roofline": {"bound": "hbm", "kernel": "whole call: seg_heads_kernel + seg_targets_kernel + seg_products_kernel<false> (+ 2 memsets)",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+        "roofline": {"bound": "hbm", "kernel": "whole call: seg_flags_kernel + seg_scan_kernel + seg_heads_kernel + seg_targets_kernel + seg_products_kernel<false> (+ memsets); the two streaming kernels (flags, products) are 75 % of it",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_SEG_TRAFFIC_BYTES,
+                     "traffic_note": "dram read + write of seg_flags_kernel and seg_products_kernel, one launch each (profiles/r1_segments_ncu_summary.txt)",
                      "peak_source": peak_src, "kernel_ms": ms_step, "algorithmic_bytes": alg},
         "cpu_baseline": {"value": ns / cpu_dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
-                         "sample": "oracle.segments.segment_products (numpy, fp64) on the first %d pixels of the same list" % ns, "seconds": cpu_dt},
+                         "sample": "oracle.segments.segment_products (numpy, fp64) on the same list, all %d pixels" % ns, "seconds": cpu_dt},
         "e2e": {"value": n / (e2e_ms * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "ms_per_step": e2e_ms, "note": "idx + value + weight from pinned host memory, all products back to pinned host memory, host wall clock"},
         "gpu_launches": launches, "clocks": clocks}))

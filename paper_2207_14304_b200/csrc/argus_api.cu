@@ -912,7 +912,8 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
                                             c->seg.mini_start, (long long)mini_capacity, (long long)n);
         c->n_launches += 2;
         if (mini_capacity > 0) {
-            seg_heads_kernel<<<(unsigned)n_ctas, SEG_CHUNK / 32, 0, st>>>(seg_bits, seg_counts, seg_offsets, (const long long*)idx, shift,
+            seg_heads_kernel<<<(unsigned)((n_ctas + SEG_HEADS_CPB - 1) / SEG_HEADS_CPB), SEG_HEADS_CPB * SEG_CHUNK / 32, 0, st>>>(
+                seg_bits, seg_counts, (long long)n_ctas, seg_offsets, (const long long*)idx, shift,
                                                               c->seg.mini_start, (long long*)mini_id, (long long)mini_capacity);
             c->n_launches++;
         }

@@ -129,22 +129,24 @@ __global__ void __launch_bounds__(1024) seg_scan_kernel(const unsigned int* __re
 }
 
 // Heads, pass 3: flag bits + chunk offsets -> mini_start[k] (position of the k-th head), mini_id[k].
-__global__ void __launch_bounds__(SEG_CHUNK / 32) seg_heads_kernel(const unsigned int* __restrict__ bits,
-                                                       const unsigned int* __restrict__ counts,
-                                                       const long long* __restrict__ offsets32,
-                                                       const long long* __restrict__ idx, int shift,
-                                                       long long* __restrict__ mini_start,
-                                                       long long* __restrict__ mini_id, long long cap) {
-    __shared__ int s_w[SEG_CHUNK / 1024];
-    __shared__ int s_front;
+#define SEG_HEADS_CPB 4   // chunks per CTA of pass 3 (64 flag words each: two warps per chunk)
+__global__ void __launch_bounds__(SEG_HEADS_CPB * SEG_CHUNK / 32) seg_heads_kernel(
+    const unsigned int* __restrict__ bits, const unsigned int* __restrict__ counts, long long n_chunks,
+    const long long* __restrict__ offsets32, const long long* __restrict__ idx, int shift,
+    long long* __restrict__ mini_start, long long* __restrict__ mini_id, long long cap) {
+    constexpr int WPC = SEG_CHUNK / 1024;   // warps per chunk
+    __shared__ int s_w[SEG_HEADS_CPB * WPC];
+    __shared__ int s_front[SEG_HEADS_CPB];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (warp == 0) {   // heads of the chunks in front of this one inside its group of 32
-        int f = (lane < (int)(blockIdx.x & 31u)) ? (int)counts[(blockIdx.x & ~31u) + lane] : 0;
+    const long long chunk = (long long)blockIdx.x * SEG_HEADS_CPB + warp / WPC;
+    if (chunk >= n_chunks) { __syncthreads(); return; }   // whole warps leave together; the barrier count stays right
+    if (warp % WPC == 0) {   // heads of the chunks in front of this one inside its group of 32
+        int f = (lane < (int)(chunk & 31)) ? (int)counts[(chunk & ~31ll) + lane] : 0;
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) f += __shfl_xor_sync(0xffffffffu, f, d);
-        if (lane == 0) s_front = f;
+        if (lane == 0) s_front[warp / WPC] = f;
     }
-    unsigned word = bits[(long long)blockIdx.x * (SEG_CHUNK / 32) + threadIdx.x];
+    unsigned word = bits[chunk * (SEG_CHUNK / 32) + (threadIdx.x & (SEG_CHUNK / 32 - 1))];
     const int c = __popc(word);
     int inc = c;
 #pragma unroll
@@ -156,9 +158,9 @@ __global__ void __launch_bounds__(SEG_CHUNK / 32) seg_heads_kernel(const unsigne
     __syncthreads();
     int wbase = 0;
 #pragma unroll
-    for (int i = 0; i < SEG_CHUNK / 1024; ++i) wbase += (i < warp) ? s_w[i] : 0;
-    long long k = offsets32[blockIdx.x >> 5] + s_front + wbase + inc - c;
-    const long long e0 = (long long)blockIdx.x * SEG_CHUNK + threadIdx.x * 32;
+    for (int i = 0; i < WPC; ++i) wbase += (i < warp % WPC) ? s_w[warp / WPC * WPC + i] : 0;
+    long long k = offsets32[chunk >> 5] + s_front[warp / WPC] + wbase + inc - c;
+    const long long e0 = chunk * SEG_CHUNK + (threadIdx.x & (SEG_CHUNK / 32 - 1)) * 32;
     while (word) {
         const int b = __ffs(word) - 1;
         word &= word - 1;
