@@ -209,7 +209,7 @@ int argus_resample_coadd(argus_ctx* ctx, const argus_frame* frame, const argus_w
  *            mini_id[k]      ascending minipix ids, k < n_mini (required when mini_capacity > 0)
  *            mini_weight[k]  sum of weight over the minipix' pixels (FP32, fixed summation order)
  *            mini_value[k]   sum(weight * value) / sum(weight), 0 where the sum of weights is 0
- *            mini_keep[k]    1 if mini_id[k] is in targets, else 0 (all mini_capacity bytes are written)
+ *            mini_keep[k]    1 if mini_id[k] is in targets, else 0 (k < n_mini; the rest is left untouched)
  *            seg16           IEEE binary16 bits (round to nearest even, finite values clamped to +-65504, NaN ->
  *                            0x7e00) of value where the pixel's minipix is kept, of 0 elsewhere; with
  *                            mini_keep == NULL nothing is stamped (plain packing).  layout == NULL: element i <->

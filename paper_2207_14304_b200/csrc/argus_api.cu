@@ -906,7 +906,6 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
         if (n_mini_dev) CUDA_TRY(c, cudaMemsetAsync(n_mini_dev, 0, sizeof(int64_t), st));
     }
     if (n_ctas > 0) {
-        if (n_ctas % 32) CUDA_TRY(c, cudaMemsetAsync(seg_counts + n_ctas, 0, (32 - n_ctas % 32) * sizeof(unsigned int), st));
         seg_flags_kernel<<<(unsigned)n_ctas, 256, 0, st>>>((const long long*)idx, (long long)n, shift, seg_bits, seg_counts);
         seg_scan_kernel<<<1, 1024, 0, st>>>(seg_counts, (long long)n_ctas, seg_offsets, c->seg.ctl, (long long*)n_mini_dev,
                                             c->seg.mini_start, (long long)mini_capacity, (long long)n);
@@ -914,12 +913,11 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
         if (mini_capacity > 0) {
             seg_heads_kernel<<<(unsigned)((n_ctas + SEG_HEADS_CPB - 1) / SEG_HEADS_CPB), SEG_HEADS_CPB * SEG_CHUNK / 32, 0, st>>>(
                 seg_bits, seg_counts, (long long)n_ctas, seg_offsets, (const long long*)idx, shift,
-                                                              c->seg.mini_start, (long long*)mini_id, (long long)mini_capacity);
+                c->seg.mini_start, (long long*)mini_id, mini_keep, (long long)mini_capacity);
             c->n_launches++;
         }
         if (mini_capacity > 0) {
             if (mini_keep) {
-                CUDA_TRY(c, cudaMemsetAsync(mini_keep, 0, mini_capacity, st));
                 if (n_targets > 0) {
                     seg_targets_kernel<<<(unsigned)((n_targets + 255) / 256), 256, 0, st>>>(
                         (const long long*)targets, (long long)n_targets, (const long long*)mini_id, c->seg.ctl,

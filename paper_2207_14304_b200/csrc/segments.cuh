@@ -70,6 +70,8 @@ __global__ void __launch_bounds__(256) seg_flags_kernel(const long long* __restr
         for (int i = 0; i < 8; ++i) t += s_cnt[i];
         counts[blockIdx.x] = (unsigned int)t;
     }
+    // the scan reads counts in groups of 32 chunks: the last CTA zeroes the rest of the last group
+    if (blockIdx.x == gridDim.x - 1 && warp == 1 && gridDim.x + lane < ((gridDim.x + 31u) & ~31u)) counts[gridDim.x + lane] = 0;
 }
 
 // Heads, pass 2: exclusive scan of the chunk counts at the granularity of 32 chunks (one CTA: thread t sums chunks
@@ -133,7 +135,7 @@ __global__ void __launch_bounds__(1024) seg_scan_kernel(const unsigned int* __re
 __global__ void __launch_bounds__(SEG_HEADS_CPB * SEG_CHUNK / 32) seg_heads_kernel(
     const unsigned int* __restrict__ bits, const unsigned int* __restrict__ counts, long long n_chunks,
     const long long* __restrict__ offsets32, const long long* __restrict__ idx, int shift,
-    long long* __restrict__ mini_start, long long* __restrict__ mini_id, long long cap) {
+    long long* __restrict__ mini_start, long long* __restrict__ mini_id, unsigned char* __restrict__ keep, long long cap) {
     constexpr int WPC = SEG_CHUNK / 1024;   // warps per chunk
     __shared__ int s_w[SEG_HEADS_CPB * WPC];
     __shared__ int s_front[SEG_HEADS_CPB];
@@ -167,6 +169,7 @@ __global__ void __launch_bounds__(SEG_HEADS_CPB * SEG_CHUNK / 32) seg_heads_kern
         const long long e = e0 + b;
         if (k <= cap && mini_start) mini_start[k] = e;
         if (k < cap && mini_id) mini_id[k] = __ldg(idx + e) >> shift;
+        if (k < cap && keep) keep[k] = 0;   // seg_targets_kernel sets the kept ones afterwards
         ++k;
     }
 }
@@ -175,11 +178,23 @@ __global__ void __launch_bounds__(256) seg_targets_kernel(const long long* __res
                                                          const long long* __restrict__ mini_id,
                                                          const unsigned long long* __restrict__ ctl, long long cap,
                                                          unsigned char* __restrict__ keep) {
+    // 256 evenly spaced entries of mini_id in shared memory take the first 8 of the ~20 search steps off the
+    // dependent chain of L2 reads (the kernel is that chain: 13 us -> 9 us for 14 k targets in 703 k minipix)
+    __shared__ long long s_tab[256];
+    const long long nm = min((long long)ctl[1], cap);
+    if (nm <= 0) return;
+    s_tab[threadIdx.x] = mini_id[(long long)(threadIdx.x + 1) * nm / 257];
+    __syncthreads();
     const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
     if (i >= n_targets) return;
-    const long long nm = min((long long)ctl[1], cap);
     const long long t = targets[i];
-    long long lo = 0, hi = nm - 1;
+    int a = 0, b = 256;                    // first table entry >= t
+    while (a < b) {
+        const int mid = (a + b) >> 1;
+        if (s_tab[mid] < t) a = mid + 1; else b = mid;
+    }
+    long long lo = (a == 0) ? 0 : (long long)a * nm / 257;            // position of table entry a - 1
+    long long hi = (a == 256) ? nm - 1 : (long long)(a + 1) * nm / 257;   // position of table entry a
     while (lo <= hi) {
         const long long mid = (lo + hi) >> 1, v = mini_id[mid];
         if (v == t) { keep[mid] = 1; return; }

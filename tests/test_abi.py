@@ -54,6 +54,9 @@ def test_host_side_validation_without_device(lib):
     assert lib.argus_calibrate(None, None, None, None, None, None, 4, 4, 1.0, 65535, 0.1, None, None, None) == -1
     n = C.c_size_t()
     assert lib.argus_healpix_footprint(None, None, 4, 4, 1 << 17, None, 0, C.byref(n), None) == -1
+    n.value = 77
+    assert lib.argus_segment_products(None, 1 << 17, 1 << 14, None, None, None, 0, None, 0, None, None, None, None, None,
+                                      None, 0, None, C.byref(n), None) == -1
 
 
 def test_no_cpu_fallback():
