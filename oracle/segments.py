@@ -17,6 +17,7 @@ Functions
   minipix_of(idx, nside, nside_mini)        parent pixel at nside_mini (pinned against ang2pix(pix2ang))
   pack_f16(v)                               IEEE binary16 bits, round-to-nearest-even, finite values clamped to
                                             +-65504, NaN -> 0x7e00 (pinned against struct 'e' and hand values)
+  raster_offset(local, side)                row-major position of an in-tile nested index (pinned against nest2xyf)
   segment_products(...)                     stamping + packing + low-resolution weighted means
 """
 from __future__ import annotations
@@ -52,7 +53,21 @@ def pack_f16(v):
     return bits
 
 
-def segment_products(idx, value, weight, nside, nside_mini, targets, layout_tiles=None, nside_tile=None):
+def raster_offset(local, side):
+    """Row-major position iy * side + ix inside a tile of side x side pixels of the pixel whose in-tile nested
+    index is `local` (ref [10]: ix = the even bits of the nested index, iy = the odd bits; reading R-S5: x runs
+    fastest).  Written out bit by bit."""
+    local = np.asarray(local, dtype=np.int64)
+    nb = _log2_exact(side)
+    ix = np.zeros_like(local)
+    iy = np.zeros_like(local)
+    for b in range(nb):
+        ix |= ((local >> (2 * b)) & 1) << b
+        iy |= ((local >> (2 * b + 1)) & 1) << b
+    return iy * side + ix
+
+
+def segment_products(idx, value, weight, nside, nside_mini, targets, layout_tiles=None, nside_tile=None, raster=False):
     """idx: ascending unique nested pixels at nside (a footprint); value, weight: the resampled frame on them.
     targets: minipix ids (at nside_mini) that hold a science target (any order, duplicates allowed).
 
@@ -63,7 +78,8 @@ def segment_products(idx, value, weight, nside, nside_mini, targets, layout_tile
       mini_value   sum(weight * value) / sum(weight), 0 where the sum of weights is 0     (fp64)
       seg16        binary16 bits of value where the pixel's minipix is kept, of 0 elsewhere; element i <-> idx[i]
       dense16      (when layout_tiles is given) seg16 scattered to slot(p) = rank(p / ppt) * ppt + p % ppt with
-                   ppt = (nside / nside_tile)^2, zeros elsewhere; pixels whose tile is absent are dropped
+                   ppt = (nside / nside_tile)^2, zeros elsewhere; pixels whose tile is absent are dropped;
+                   raster=True: each tile is a row-major image, p % ppt replaced by raster_offset(p % ppt)
     """
     idx = np.asarray(idx, dtype=np.int64)
     value = np.asarray(value, dtype=np.float64)
@@ -89,6 +105,7 @@ def segment_products(idx, value, weight, nside, nside_mini, targets, layout_tile
         pos = np.searchsorted(tiles, key)
         ok = (pos < tiles.size)
         ok[ok] &= tiles[pos[ok]] == key[ok]
-        dense[pos[ok] * ppt + (idx[ok] & (ppt - 1))] = seg16[ok]
+        local = idx[ok] & (ppt - 1)
+        dense[pos[ok] * ppt + (raster_offset(local, 1 << kk) if raster else local)] = seg16[ok]
         out["dense16"] = dense
     return out

@@ -185,6 +185,32 @@ def test_s5_dense_tile_layout_brute_force():
     assert r["dense16"].size == tiles.size * 1024
 
 
+def test_s5_raster_layout_against_pixel_coordinates():
+    # the C oracle's nest2xyf gives (ix, iy) in the face; inside an NSIDE-256 tile the image position is (ix mod side,
+    # iy mod side), x fastest -- independent of raster_offset's bit loop
+    rng = np.random.default_rng(12)
+    nside, nside_tile = 1 << 17, 1 << 8
+    side = nside // nside_tile
+    p = rng.integers(0, 12 * nside * nside, 4000)
+    off = seg.raster_offset(p & (side * side - 1), side)
+    for pi, oi in zip(p.tolist(), off.tolist()):
+        _face, ix, iy = oracle.nest2xyf(nside, pi)
+        assert oi == (iy % side) * side + (ix % side)
+    assert sorted(seg.raster_offset(np.arange(64 * 64), 64).tolist()) == list(range(64 * 64))   # a permutation
+    assert seg.raster_offset(np.array([0, 1, 2, 3, 4]), 512).tolist() == [0, 1, 512, 513, 2]
+    # through segment_products: same multiset per tile, placed by brute force
+    nside, nside_mini, nside_tile = 1 << 10, 1 << 7, 1 << 5
+    idx, value, weight = _random_footprint(rng, nside, 5000)
+    tiles = np.unique(idx // 1024)
+    r = seg.segment_products(idx, value, weight, nside, nside_mini, np.unique(idx // 64), layout_tiles=tiles, nside_tile=nside_tile, raster=True)
+    dense = np.zeros(tiles.size * 1024, np.uint16)
+    tl = tiles.tolist()
+    for pi, b in zip(idx.tolist(), r["seg16"].tolist()):
+        _face, ix, iy = oracle.nest2xyf(nside, pi)
+        dense[tl.index(pi // 1024) * 1024 + (iy % 32) * 32 + (ix % 32)] = b
+    assert np.array_equal(r["dense16"], dense)
+
+
 def test_empty_and_errors():
     e = np.zeros(0, np.int64)
     r = seg.segment_products(e, np.zeros(0, np.float32), np.zeros(0, np.float32), 1 << 17, 1 << 14, e)
