@@ -65,6 +65,10 @@ enum {
     ARGUS_OPT_PLAN_OVERLAP = 4, /* 1 (default): the plan of a new WCS is built on an internal high-priority stream in a second
                                  set of scratch buffers, so that it runs underneath the previous frame's kernels; the
                                  caller's stream waits for it (stream order of results is unchanged); 0: in place */
+    ARGUS_OPT_SEGMENT_RASTER = 5, /* 0 (default): argus_segment_products with a layout writes every tile in nested pixel
+                               * order (slot(p) of argus_coadd).  1: every tile is a row-major image of side
+                               * nside / nside_tile: pixel (ix, iy) of the tile (ix = even bits, iy = odd bits of the
+                               * in-tile nested index, the HEALPix face coordinates) goes to iy * side + ix. */
     ARGUS_OPT_PROFILE = 2     /* 1: argus_resample / argus_resample_coadd (idx == NULL) record CUDA events on
                                  the caller's stream around the plan kernels and around the fused kernel
                                  (ring of 256 calls); read them back with argus_profile_read.  Default 0. */
@@ -216,6 +220,7 @@ int argus_resample_coadd(argus_ctx* ctx, const argus_frame* frame, const argus_w
  *                            idx[i] (n elements).  layout != NULL (nside_tile <= nside_mini): scattered to the
  *                            tile-dense layout slot(p) of argus_coadd, n_tiles * ppt elements; slots outside the
  *                            footprint are not written (zero the buffer once), pixels of absent tiles are dropped.
+ *                            ARGUS_OPT_SEGMENT_RASTER selects row-major tiles instead of nested order.
  *            n_mini_dev      DEVICE int64, receives n_mini (asynchronous)
  *            n_mini_out      HOST; when not NULL the call synchronises the stream and stores n_mini here.
  * mini_capacity = 0 with every per-minipix output and seg16 NULL only counts.  Minipix beyond mini_capacity are

@@ -15,6 +15,7 @@ ARGUS_OPT_PLAN_CACHE = 1
 ARGUS_OPT_PROFILE = 2
 ARGUS_OPT_FAST_PATH = 3
 ARGUS_OPT_PLAN_OVERLAP = 4
+ARGUS_OPT_SEGMENT_RASTER = 5
 _KERNELS = {"bilinear": ARGUS_BILINEAR, "lanczos3": ARGUS_LANCZOS3, 0: 0, 1: 1}
 
 EXPORTS = [
@@ -199,6 +200,11 @@ class Context:
 
     def set_plan_overlap(self, on: bool):
         rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_PLAN_OVERLAP, 1 if on else 0)
+        if rc:
+            raise ArgusError(rc, "argus_ctx_set_option")
+
+    def set_segment_raster(self, on: bool):
+        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_SEGMENT_RASTER, 1 if on else 0)
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")
 

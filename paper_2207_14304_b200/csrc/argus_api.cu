@@ -71,6 +71,7 @@ struct argus_ctx {
         unsigned long long* ctl; size_t cap_ctas;
         long long* h_n;   // pinned
     } seg;
+    bool seg_raster;      // ARGUS_OPT_SEGMENT_RASTER
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -297,6 +298,10 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
     }
     if (option == ARGUS_OPT_PLAN_OVERLAP) {
         c->overlap = value != 0;
+        return ARGUS_OK;
+    }
+    if (option == ARGUS_OPT_SEGMENT_RASTER) {
+        c->seg_raster = value != 0;
         return ARGUS_OK;
     }
     if (option == ARGUS_OPT_FAST_PATH) {
@@ -927,12 +932,16 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
             }
             if (seg16 || mini_value || mini_weight) {
                 const int grid = c->sm_count * 4;
-                if (layout)
-                    seg_products_kernel<true><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
-                                                                   c->seg.ctl, (long long)mini_capacity, (const long long*)idx,
-                                                                   value, weight, shift, lay, seg16, mini_value, mini_weight);
+                if (layout && c->seg_raster)
+                    seg_products_kernel<2><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
+                                                                c->seg.ctl, (long long)mini_capacity, (const long long*)idx,
+                                                                value, weight, shift, lay, seg16, mini_value, mini_weight);
+                else if (layout)
+                    seg_products_kernel<1><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
+                                                                c->seg.ctl, (long long)mini_capacity, (const long long*)idx,
+                                                                value, weight, shift, lay, seg16, mini_value, mini_weight);
                 else
-                    seg_products_kernel<false><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
+                    seg_products_kernel<0><<<grid, 256, 0, st>>>(c->seg.mini_start, (const long long*)mini_id, mini_keep,
                                                                     c->seg.ctl, (long long)mini_capacity, (const long long*)idx,
                                                                     value, weight, shift, lay, seg16, mini_value, mini_weight);
                 c->n_launches++;

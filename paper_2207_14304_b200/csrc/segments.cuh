@@ -209,13 +209,22 @@ __device__ __forceinline__ unsigned short seg_f2h(float v) {
     return (v != v) ? (unsigned short)0x7e00 : h;
 }
 
+// row-major position iy * side + ix of an in-tile nested index (ix = even bits, iy = odd bits)
+__device__ __forceinline__ long long seg_raster(long long local, int side_log2) {
+    return (long long)compact_even_bits((unsigned long long)local) +
+           ((long long)compact_even_bits((unsigned long long)local >> 1) << side_log2);
+}
+
 // dense-layout base slot of minipix `mid_` (or -1 when its tile is absent)
-__device__ __forceinline__ long long seg_dense_base(const SegLayout& lay, long long mid_, int shift) {
+__device__ __forceinline__ long long seg_dense_base(const SegLayout& lay, long long mid_, int shift, bool raster) {
     const long long key = mid_ >> lay.mini_per_tile_log2;
     long long lo = 0, hi = lay.n_tiles - 1;
     while (lo <= hi) {
         const long long mid = (lo + hi) >> 1, tv = lay.tiles[mid];
-        if (tv == key) return (mid << lay.ppt_log2) + ((mid_ & ((1ll << lay.mini_per_tile_log2) - 1)) << shift);
+        if (tv == key) {
+            const long long local = (mid_ & ((1ll << lay.mini_per_tile_log2) - 1)) << shift;   // minipix' first pixel
+            return (mid << lay.ppt_log2) + (raster ? seg_raster(local, lay.ppt_log2 >> 1) : local);
+        }
         if (tv < key) lo = mid + 1; else hi = mid - 1;
     }
     return -1;
@@ -245,7 +254,8 @@ __device__ __forceinline__ float seg_reduce8(const float (&a)[8], int lane) {
     return d;
 }
 
-template <bool DENSE>
+// DENSE: 0 = seg16 element i <-> idx[i]; 1 = tile-dense layout, nested order inside a tile; 2 = tile-dense, row-major
+template <int DENSE>
 __global__ void __launch_bounds__(256, 4) seg_products_kernel(
     const long long* __restrict__ mini_start, const long long* __restrict__ mini_id,
     const unsigned char* __restrict__ keep, const unsigned long long* __restrict__ ctl, long long cap,
@@ -262,7 +272,7 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
         long long db_l = -1;
         if (lane < SEG_GROUP && kb + lane < nm) {
             if (keep) kp_l = keep[kb + lane] != 0;
-            if (DENSE) db_l = seg_dense_base(lay, mini_id[kb + lane], shift);
+            if (DENSE) db_l = seg_dense_base(lay, mini_id[kb + lane], shift, DENSE == 2);
         }
         const long long s0 = __shfl_sync(0xffffffffu, st, 0);
         const int rel_l = (int)min(st - s0, (long long)0x3fffffff);   // pixels of the group lie in [s0, s0 + rel[4])
@@ -305,8 +315,11 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
                         if (dbase >= 0) {
                             const bool complete = rel[i + 1] - rel[i] == full;
                             const long long* ii = idx + s0 + (rel[i] + lane);
-                            if (left[i] > 0) seg16[dbase + (complete ? (long long)lane : (ii[0] & (long long)(full - 1)))] = h0;
-                            if (left[i] > 32) seg16[dbase + (complete ? (long long)(lane + 32) : (ii[32] & (long long)(full - 1)))] = h1;
+                            long long o0 = complete ? (long long)lane : (left[i] > 0 ? (ii[0] & (long long)(full - 1)) : 0);
+                            long long o1 = complete ? (long long)(lane + 32) : (left[i] > 32 ? (ii[32] & (long long)(full - 1)) : 0);
+                            if (DENSE == 2) { o0 = seg_raster(o0, lay.ppt_log2 >> 1); o1 = seg_raster(o1, lay.ppt_log2 >> 1); }
+                            if (left[i] > 0) seg16[dbase + o0] = h0;
+                            if (left[i] > 32) seg16[dbase + o1] = h1;
                         }
                     } else {
                         unsigned short* oi = seg16 + s0 + (rel[i] + lane);
@@ -330,7 +343,11 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
                     if (seg16) {
                         const unsigned short hb = kp ? seg_f2h(vv) : (unsigned short)0;
                         if (DENSE) {
-                            if (dbase >= 0) seg16[dbase + ((cnt == full) ? q : (idx[si + q] & (long long)(full - 1)))] = hb;
+                            if (dbase >= 0) {
+                                long long o = (cnt == full) ? q : (idx[si + q] & (long long)(full - 1));
+                                if (DENSE == 2) o = seg_raster(o, lay.ppt_log2 >> 1);
+                                seg16[dbase + o] = hb;
+                            }
                         } else {
                             seg16[si + q] = hb;
                         }

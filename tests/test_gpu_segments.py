@@ -108,6 +108,32 @@ def test_dense_tile_layout(argus, ctx):
     g = _run(argus, ctx, nside, nside_mini, idx, value, weight, targets, tiles=tiles, nside_tile=nside_tile)
     _compare(g, o, dense=True)
     assert o["dense16"].any()
+    # the same tiles as row-major 512 x 512 images (ARGUS_OPT_SEGMENT_RASTER)
+    o_r = oseg.segment_products(idx, value, weight, nside, nside_mini, targets, layout_tiles=tiles, nside_tile=nside_tile, raster=True)
+    assert not np.array_equal(o_r["dense16"], o["dense16"])
+    ctx.set_segment_raster(True)
+    try:
+        g_r = _run(argus, ctx, nside, nside_mini, idx, value, weight, targets, tiles=tiles, nside_tile=nside_tile)
+    finally:
+        ctx.set_segment_raster(False)
+    _compare(g_r, o_r, dense=True)
+
+
+@pytest.mark.parametrize("raster", [False, True])
+def test_dense_layout_with_large_and_small_minipix(argus, ctx, raster):
+    # 1024-pixel minipix (generic path of the products kernel) and 4-pixel minipix, tiles of 64 x 64 pixels
+    for nside, nside_mini, nside_tile in (((1 << 12), 1 << 7, 1 << 6), ((1 << 12), 1 << 11, 1 << 6)):
+        idx, value, weight = synth.footprint_like(41 + nside_mini, 12 * nside * nside, 60_001, run=5000)
+        m = oseg.minipix_of(idx, nside, nside_mini)
+        targets = synth.target_list(42, int(m[0]), int(m[-1]) + 1, 0.5)
+        tiles = np.unique(idx >> 12)[1:]
+        o = oseg.segment_products(idx, value, weight, nside, nside_mini, targets, layout_tiles=tiles, nside_tile=nside_tile, raster=raster)
+        ctx.set_segment_raster(raster)
+        try:
+            g = _run(argus, ctx, nside, nside_mini, idx, value, weight, targets, tiles=tiles, nside_tile=nside_tile)
+        finally:
+            ctx.set_segment_raster(False)
+        _compare(g, o, dense=True)
 
 
 def test_special_values_pack_bit_exactly(argus, ctx):
