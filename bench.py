@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused calibrate + HEALPix-resample hot path on B200 (contract in the task).
 
-    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload config1|config0|...|segments]
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload config1|config0|...|segments|detect]
 
 A step = one pass of the whole hot path over one frame: per-frame plan on the device (A0/A1, the WCS is
 treated as new every step: plan cache off) + fused calibrate/resample (A2-A5) writing value + weight.
@@ -32,6 +32,7 @@ SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload reci
 # dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
 # profiles/r1_final_ncu_summary.txt (ncu --set full).
 NCU_TRAFFIC_BYTES = 983571968 + 339383296  # profiles/r1_final_ncu_summary.txt
+NCU_DET_TRAFFIC_BYTES = None   # profiles/r1_detect_ncu_summary.txt
 NCU_SEG_TRAFFIC_BYTES = 359159552 + 7175936 + 365523712 + 41991424  # profiles/r1_segments_ncu_summary.txt
 
 
@@ -416,6 +417,131 @@ def run_segments(args):
     return 0
 
 
+def run_detect(args):
+    """--workload detect: SURVEY 8(f).2 on the configs[1] frame.  A step = argus_background_map + argus_detect_sources
+    with fused calibration (raw + masters resident in HBM) -> background / noise grids and the source catalogue.
+    Not the headline line; same JSON contract."""
+    import numpy as np
+    import torch
+
+    import paper_2207_14304_b200 as argus
+
+    rank = int(os.environ.get("RANK", "0"))
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        if rank == 0:
+            print(json.dumps({"workload": "detect", "unavailable": "single-GPU diagnostic line (frames are independent: replicas only)"}))
+        return 0
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    argus.load_library()
+    fr, _ = make_workload("config1", 0)
+    H, W = fr.shape
+    B, n_min, k_sigma, cap = 64, 16, 5.0, 1 << 18
+    ctx = argus.Context(0)
+    d = dict(raw=torch.from_numpy(fr.raw).to(dev), bias=torch.from_numpy(fr.bias).to(dev),
+             dark=torch.from_numpy(fr.dark).to(dev), flat=torch.from_numpy(fr.flat).to(dev), bpm=None,
+             t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
+    G = -(-H // B) * -(-W // B)
+    bkg = torch.empty(G, dtype=torch.float32, device=dev)
+    nse = torch.empty(G, dtype=torch.float32, device=dev)
+    cat = torch.empty(cap * 32, dtype=torch.uint8, device=dev)
+    n_dev = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    def step_map():
+        argus.argus_background_map(ctx, W, H, bkg, nse, cell=B, n_min=n_min, **d)
+
+    def step_det():
+        argus.argus_detect_sources(ctx, W, H, bkg, nse, cat, cell=B, k_sigma=k_sigma, n_dev=n_dev, sync=False, **d)
+
+    def step():
+        step_map()
+        step_det()
+
+    n_src = None
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    n_src = int(n_dev.item())
+    sampler = ClockSampler(0)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+    t0 = time.time()
+    for _ in range(300):   # run-up for the clock sampler (the timed region is shorter than one nvidia-smi sample)
+        step()
+    launches0 = ctx.launch_count()
+    ev[0].record()
+    for _ in range(args.steps):
+        step()
+    ev[1].record()
+    launches = ctx.launch_count() - launches0
+    ev[2].record()
+    for _ in range(args.steps):
+        step_map()
+    ev[3].record()
+    ev[4].record()
+    for _ in range(args.steps):
+        step_det()
+    ev[5].record()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    ms_step = ev[0].elapsed_time(ev[1]) / args.steps
+    ms_map = ev[2].elapsed_time(ev[3]) / args.steps
+    ms_det = ev[4].elapsed_time(ev[5]) / args.steps
+    clocks = sampler.stop(t0, t1)
+
+    # end to end: raw frame from pinned host memory, grids + catalogue back to pinned host memory, every step
+    h_raw = torch.from_numpy(fr.raw).pin_memory()
+    h_out = [torch.empty_like(t, device="cpu").pin_memory() for t in (bkg, nse, cat, n_dev)]
+    e2e_steps = max(3, min(args.steps, 6))
+    torch.cuda.synchronize()
+    t_e0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        d["raw"].copy_(h_raw, non_blocking=True)
+        step()
+        h_out[3].copy_(n_dev, non_blocking=True)
+        h_out[0].copy_(bkg, non_blocking=True); h_out[1].copy_(nse, non_blocking=True)
+        torch.cuda.synchronize()
+        k = int(h_out[3].item())
+        h_out[2][:k * 32].copy_(cat[:k * 32])
+    e2e_ms = 1e3 * (time.perf_counter() - t_e0) / e2e_steps
+    d2h = 2 * G * 4 + 8 + n_src * 32
+
+    # the oracle, as it stands, on a bounded crop of the same frame (cell-aligned 6144 x 6144 corner, 62 % of the frame)
+    import oracle
+    from oracle import background as ob
+    side = 6144
+    cal, mask = oracle.calibrate_frame(fr)
+    cal, mask = np.ascontiguousarray(cal[:side, :side]), np.ascontiguousarray(mask[:side, :side])
+    t_c0 = time.perf_counter()
+    ob_b, ob_n = ob.background(cal, mask, B, n_min)
+    o_src = ob.detect(cal, mask, ob_b, ob_n, B=B, k_sigma=k_sigma)
+    cpu_dt = time.perf_counter() - t_c0
+
+    peak, peak_src = _peaks()
+    px = W * H
+    alg = px * 14 + 2 * G * 4 + n_src * 32
+    achieved = alg / (ms_step * 1e-3) / 1e9
+    print(json.dumps({
+        "metric": "background map + source detection (fused calibration) Mpix/s per B200; achieved HBM GB/s vs peak",
+        "value": px / (ms_step * 1e-3) / 1e6, "unit": "Mpix/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "background map + source detection on one configs[1] frame (SURVEY 8(f).2)", "W": W, "H": H,
+                   "cell": B, "n_min": n_min, "k_sigma": k_sigma, "n_sources": n_src, "fused": True,
+                   "l2": "inputs (856 MB/frame) larger than L2 (126 MB)"},
+        "roofline": {"bound": "hbm", "kernel": "whole step: bg_cells_kernel<true> + bg_filter_kernel + det_tiles_kernel<true> + det_scan_kernel + det_gather_kernel",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_DET_TRAFFIC_BYTES,
+                     "traffic_note": "dram read + write of bg_cells_kernel and det_tiles_kernel, one launch each (profiles/r1_detect_ncu_summary.txt); the step reads raw + masters twice (once per pass), the algorithmic bytes count them once",
+                     "peak_source": peak_src, "kernel_ms": ms_step, "algorithmic_bytes": alg,
+                     "background_map_ms": ms_map, "detect_sources_ms": ms_det},
+        "cpu_baseline": {"value": side * side / cpu_dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
+                         "sample": "oracle.background.background + detect (numpy, fp64) on the %d x %d corner of the same frame, %d sources" % (side, side, o_src["x"].size),
+                         "seconds": cpu_dt},
+        "e2e": {"value": px / (e2e_ms * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": int(h_raw.numel() * 2), "d2h_bytes_per_step": int(d2h),
+                "ms_per_step": e2e_ms, "note": "raw frame from pinned host memory, grids + catalogue back to pinned host memory, masters resident, host wall clock"},
+        "gpu_launches": launches, "clocks": clocks}))
+    ctx.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -423,12 +549,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-plan-overlap", action="store_true", help="diagnostic: build every plan in place on the caller's stream")
-    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config2", "config3", "config4", "segments"])
+    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config2", "config3", "config4", "segments", "detect"])
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.workload == "segments":
         return run_segments(args)
+    if args.workload == "detect":
+        return run_detect(args)
     return run_gpu(args)
 
 

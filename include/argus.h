@@ -233,6 +233,50 @@ int argus_segment_products(argus_ctx* ctx, int64_t nside, int64_t nside_mini, co
                            float* mini_weight, uint8_t* mini_keep, size_t mini_capacity, int64_t* n_mini_dev,
                            size_t* n_mini_out, void* stream);
 
+/* ---- Background map and source detection: the paper's two GPU stages between calibration and
+ * resampling, "Median-filtered background map" and "Source detection" (PAPER.md:193-194 Table 2; :135; the
+ * per-camera "intermediate background and noise maps" of :109).  The paper gives no formula; DESIGN.md section 11
+ * lists the readings R-D1 .. R-D6 restated here.  "median" of n values = mean of the order statistics (n-1)/2 and n/2.
+ *
+ * argus_background_map: frame as for argus_resample (raw + masters: calibration fused; or cal + mask).  The frame is
+ * cut into cell x cell pixel cells (cell in {8, 16, 32, 64}; ragged at the right / bottom edge), GX = ceil(W / cell),
+ * GY = ceil(H / cell), row-major [GY][GX] grids:
+ *   med   = median of the cell's good pixels; sig = 1.4826 * median |v - med|; ngood = number of good pixels;
+ *           a cell with ngood < max(n_min, 1) is invalid (med = sig = 0)                      (optional outputs)
+ *   bkg   = median of med over the valid cells of the 3 x 3 cell neighbourhood (clipped to the grid); nse likewise
+ *           from sig; no valid cell: bkg = 0, nse = +inf                                      (required outputs)
+ * All DEVICE pointers, GX * GY elements.  Medians are exact selections (bit-exact for a given float32 frame).
+ * Asynchronous on stream; the context keeps 12 bytes of scratch per cell. */
+int argus_background_map(argus_ctx* ctx, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
+                         float* bkg_out, float* nse_out, float* med_out, float* sig_out, int32_t* ngood_out,
+                         void* stream);
+
+/* One detected source (32 bytes). */
+typedef struct argus_source {
+    int32_t x, y;      /* peak pixel */
+    float peak;        /* s = cal - bkg(x, y) at the peak, ADU */
+    float flux;        /* sum of s over the good in-frame pixels of the 3 x 3 window */
+    float cx, cy;      /* centroid offsets sum(s dx) / flux, sum(s dy) / flux (0 when flux <= 0): centroid = (x + cx, y + cy) */
+    float bkg, nse;    /* interpolated background and noise at the peak */
+} argus_source;
+
+/* argus_detect_sources: bkg / nse are the DEVICE grids of argus_background_map for the same (W, H, cell), evaluated
+ * per pixel by bilinear interpolation between the cell centres gx * cell + (cell - 1) / 2 (clamped outside the
+ * outermost centres).  Pixel p is a source iff it is good, s_p > k_sigma * nse(p), s_p > 0, and s_p is the maximum of
+ * its good in-frame 8-neighbours (s_p > s_q for q before p in raster order, s_p >= s_q for q after p).  Pixels whose
+ * interpolation touches a cell with nse = +inf are never sources.
+ *   out       DEVICE argus_source[capacity], 16-byte aligned.  Catalogue order (deterministic): by 64 x 32-pixel tile
+ *             ((y / 32) * ceil(W / 64) + x / 64 ascending), raster order inside a tile.
+ *   n_dev     DEVICE int64 (may be NULL): number of sources found (asynchronous)
+ *   n_out     HOST (may be NULL): when given the call synchronises the stream and stores the number found; if that
+ *             exceeds a non-zero capacity the call returns ARGUS_ERR_CAPACITY, the contents of out are unspecified
+ *             (nothing is written beyond capacity) and *n_out is the capacity to call again with.
+ * capacity = 0 only counts.  Scratch: 12 bytes per tile + 32 bytes per record of capacity, grown on demand (which
+ * synchronises the device).  Otherwise asynchronous on stream. */
+int argus_detect_sources(argus_ctx* ctx, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, const float* bkg,
+                         const float* nse, float k_sigma, argus_source* out, size_t capacity, int64_t* n_dev,
+                         size_t* n_out, void* stream);
+
 /* Synchronises the stream and reports the statistics of the cached plan.  Returns ARGUS_ERR_CAPACITY if
  * an asynchronous call since the last check overflowed its output capacity or the context's max_tiles. */
 int argus_plan_info(argus_ctx* ctx, argus_plan_stats* out, void* stream);

@@ -9,8 +9,11 @@ from .binding import (  # noqa: F401
     ARGUS_LANCZOS3,
     ArgusError,
     Context,
+    SOURCE_DTYPE,
+    argus_background_map,
     argus_calibrate,
     argus_coadd_accumulate,
+    argus_detect_sources,
     argus_healpix_footprint,
     argus_plan_info,
     argus_resample,

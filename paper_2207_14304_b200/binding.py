@@ -22,7 +22,7 @@ EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
-    "argus_resample_host", "argus_host_wait", "argus_segment_products",
+    "argus_resample_host", "argus_host_wait", "argus_segment_products", "argus_background_map", "argus_detect_sources",
 ]
 
 
@@ -95,6 +95,8 @@ def load_library():
     L.argus_host_wait.argtypes = [vp]
     L.argus_segment_products.argtypes = [vp, i64, i64, vp, vp, vp, sz, vp, sz, C.POINTER(_Coadd), vp, vp, vp, vp, vp, sz,
                                          vp, C.POINTER(sz), vp]
+    L.argus_background_map.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.argus_detect_sources.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, vp, vp, f32, vp, sz, vp, C.POINTER(sz), vp]
     L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
     L.argus_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64), vp]
     _lib = L
@@ -382,6 +384,50 @@ def argus_segment_products(ctx, nside, nside_mini, idx, value, weight, targets, 
         raise ArgusError(rc, "argus_segment_products", "n_mini=%d" % nm.value)
     _check(ctx, rc, "argus_segment_products")
     return int(nm.value) if sync else None
+
+
+# numpy view of argus_source records (argus.h)
+SOURCE_DTYPE = [("x", "<i4"), ("y", "<i4"), ("peak", "<f4"), ("flux", "<f4"), ("cx", "<f4"), ("cy", "<f4"), ("bkg", "<f4"),
+                ("nse", "<f4")]
+
+
+def argus_background_map(ctx, W, H, bkg_out, nse_out, cell=64, n_min=16, med_out=None, sig_out=None, ngood_out=None,
+                         stream=None, **frame):
+    """Median-filtered background and noise grids into caller-allocated float32 CUDA tensors of
+    ceil(H / cell) * ceil(W / cell) elements.  frame: raw= bias= dark= flat= [bpm=] t_exp= ... or cal= mask=."""
+    g = -(-int(H) // int(cell)) * -(-int(W) // int(cell))
+    for name, t in (("bkg_out", bkg_out), ("nse_out", nse_out), ("med_out", med_out), ("sig_out", sig_out),
+                    ("ngood_out", ngood_out)):
+        if t is not None and t.numel() < g:
+            raise ValueError("%s holds %d elements, %d needed" % (name, t.numel(), g))
+    f = _frame_struct(**frame)
+    rc = load_library().argus_background_map(
+        ctx._h, C.byref(f), int(W), int(H), int(cell), int(n_min), _dev(bkg_out, torch.float32, "bkg_out"),
+        _dev(nse_out, torch.float32, "nse_out"), _dev(med_out, torch.float32, "med_out", allow_none=True),
+        _dev(sig_out, torch.float32, "sig_out", allow_none=True), _dev(ngood_out, torch.int32, "ngood_out", allow_none=True),
+        _stream(stream))
+    _check(ctx, rc, "argus_background_map")
+
+
+def argus_detect_sources(ctx, W, H, bkg, nse, out, cell=64, k_sigma=5.0, n_dev=None, sync=True, stream=None, **frame):
+    """Source detection.  out: uint8 CUDA tensor of 32 * capacity bytes (argus_source records, view the
+    host copy with SOURCE_DTYPE) or None to count.  Returns the number of sources found when sync, else None."""
+    cap = 0 if out is None else out.numel() // 32
+    if out is not None and out.dtype != torch.uint8:
+        raise TypeError("out must be a uint8 tensor (32 bytes per record)")
+    g = -(-int(H) // int(cell)) * -(-int(W) // int(cell))
+    if bkg.numel() < g or nse.numel() < g:
+        raise ValueError("bkg / nse hold fewer than %d cells" % g)
+    f = _frame_struct(**frame)
+    n = C.c_size_t(0)
+    rc = load_library().argus_detect_sources(
+        ctx._h, C.byref(f), int(W), int(H), int(cell), _dev(bkg, torch.float32, "bkg"), _dev(nse, torch.float32, "nse"),
+        float(k_sigma), _dev(out, torch.uint8, "out", allow_none=True), cap, _dev(n_dev, torch.int64, "n_dev", allow_none=True),
+        C.byref(n) if sync else None, _stream(stream))
+    if rc == -6 and sync:
+        raise ArgusError(rc, "argus_detect_sources", "n_sources=%d" % n.value)
+    _check(ctx, rc, "argus_detect_sources")
+    return int(n.value) if sync else None
 
 
 def argus_plan_info(ctx, stream=None) -> dict:

@@ -14,6 +14,7 @@
 #include "resample.cuh"
 #include "resample_fast.cuh"
 #include "segments.cuh"
+#include "background.cuh"
 
 #define ARGUS_VERSION_NUM 100
 #define PLAN_SLOTS 3
@@ -72,6 +73,14 @@ struct argus_ctx {
         long long* h_n;   // pinned
     } seg;
     bool seg_raster;      // ARGUS_OPT_SEGMENT_RASTER
+    // argus_background_map / argus_detect_sources: cell grid, per-tile (base, count) + offsets, record staging
+    struct BgScratch {
+        float* cells; size_t cap_cells;          // med | sig | ngood, cap_cells each
+        uint2* tiles; size_t cap_tiles;          // tile_info | offsets (4 B) behind it
+        ArgusSourceRec* tmp; size_t cap_tmp;
+        unsigned* ctl;                           // [0] running total (atomics), [1] final count
+        long long* h_n;                          // pinned
+    } bg;
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -279,6 +288,11 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (c->seg.mini_start) cudaFree(c->seg.mini_start);
     if (c->seg.ctl) cudaFree(c->seg.ctl);
     if (c->seg.h_n) cudaFreeHost(c->seg.h_n);
+    if (c->bg.cells) cudaFree(c->bg.cells);
+    if (c->bg.tiles) cudaFree(c->bg.tiles);
+    if (c->bg.tmp) cudaFree(c->bg.tmp);
+    if (c->bg.ctl) cudaFree(c->bg.ctl);
+    if (c->bg.h_n) cudaFreeHost(c->bg.h_n);
     cudaFreeHost(c->h_stats);
     delete c;
     return ARGUS_OK;
@@ -954,6 +968,104 @@ extern "C" int argus_segment_products(argus_ctx* c, int64_t nside, int64_t nside
         CUDA_TRY(c, cudaStreamSynchronize(st));
         *n_mini_out = (size_t)*c->seg.h_n;
         if (mini_capacity > 0 && *n_mini_out > mini_capacity) return ARGUS_ERR_CAPACITY;
+    }
+    return ARGUS_OK;
+}
+
+// ------------------------------------------------------------------------- background map + source detection
+static int bg_check_cell(int32_t cell) { return (cell == 8 || cell == 16 || cell == 32 || cell == 64) ? ARGUS_OK : ARGUS_ERR_SHAPE; }
+
+extern "C" int argus_background_map(argus_ctx* c, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
+                                    float* bkg_out, float* nse_out, float* med_out, float* sig_out, int32_t* ngood_out,
+                                    void* stream) {
+    if (!c || !frame || !bkg_out || !nse_out) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n_min < 0) return ARGUS_ERR_SHAPE;
+    if (bg_check_cell(cell)) return ARGUS_ERR_SHAPE;
+    if (!aligned(bkg_out, 4) || !aligned(nse_out, 4) || !aligned(med_out, 4) || !aligned(sig_out, 4) || !aligned(ngood_out, 4))
+        return ARGUS_ERR_ALIGN;
+    FrameArgs f;
+    bool fused;
+    int rc = make_frameargs(frame, W, H, &f, &fused);
+    if (rc) return rc;
+    const int64_t GX = (W + cell - 1) / cell, GY = (H + cell - 1) / cell, G = GX * GY;
+    if (G > 0x7fffffffll) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (c->bg.cap_cells < (size_t)G || !c->bg.cells) {
+        if (c->bg.cells) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.cells); c->bg.cells = nullptr; }
+        size_t want = align_up((size_t)G, 4096);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.cells, want * 12));
+        c->bg.cap_cells = want;
+    }
+    float* med = med_out ? med_out : c->bg.cells;
+    float* sig = sig_out ? sig_out : c->bg.cells + c->bg.cap_cells;
+    int* ngood = ngood_out ? (int*)ngood_out : (int*)(c->bg.cells + 2 * c->bg.cap_cells);
+    if (fused)
+        bg_cells_kernel<true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+    else
+        bg_cells_kernel<false><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+    bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
+    c->n_launches += 2;
+    CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int64_t W, int64_t H, int32_t cell,
+                                    const float* bkg, const float* nse, float k_sigma, argus_source* out, size_t capacity,
+                                    int64_t* n_dev, size_t* n_out, void* stream) {
+    if (!c) return ARGUS_ERR_NULL;
+    if (n_out) *n_out = 0;
+    if (!frame || !bkg || !nse || (capacity > 0 && !out)) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || capacity > 0x7fffffffull) return ARGUS_ERR_SHAPE;
+    if (bg_check_cell(cell) || !(k_sigma >= 0.0f) || !(k_sigma < INFINITY)) return ARGUS_ERR_SHAPE;
+    if (!aligned(bkg, 4) || !aligned(nse, 4) || !aligned(out, 16) || !aligned(n_dev, 8)) return ARGUS_ERR_ALIGN;
+    FrameArgs f;
+    bool fused;
+    int rc = make_frameargs(frame, W, H, &f, &fused);
+    if (rc) return rc;
+    const int64_t tiles_x = (W + DET_TW - 1) / DET_TW, tiles_y = (H + DET_TH - 1) / DET_TH, n_tiles = tiles_x * tiles_y;
+    if (n_tiles > 0x7fffffffll) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (!c->bg.h_n) CUDA_TRY(c, cudaMallocHost((void**)&c->bg.h_n, sizeof(long long)));
+    if (!c->bg.ctl) CUDA_TRY(c, cudaMalloc((void**)&c->bg.ctl, 16));
+    if (c->bg.cap_tiles < (size_t)n_tiles || !c->bg.tiles) {
+        if (c->bg.tiles) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tiles); c->bg.tiles = nullptr; }
+        size_t want = align_up((size_t)n_tiles, 4096);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tiles, want * 12));
+        c->bg.cap_tiles = want;
+    }
+    if (c->bg.cap_tmp < capacity || !c->bg.tmp) {
+        if (c->bg.tmp) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tmp); c->bg.tmp = nullptr; }
+        size_t want = align_up(capacity + 1, 65536);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tmp, want * sizeof(ArgusSourceRec)));
+        c->bg.cap_tmp = want;
+    }
+    unsigned* offsets = (unsigned*)(c->bg.tiles + c->bg.cap_tiles);
+    DetGrid g;
+    g.bkg = bkg; g.nse = nse; g.B = cell;
+    g.GX = (int)((W + cell - 1) / cell); g.GY = (int)((H + cell - 1) / cell);
+    g.inv_B = 1.0f / (float)cell; g.half = 0.5f * (float)(cell - 1); g.k_sigma = k_sigma;
+    CUDA_TRY(c, cudaMemsetAsync(c->bg.ctl, 0, 16, st));
+    if (fused)
+        det_tiles_kernel<true><<<(unsigned)n_tiles, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity,
+                                                               c->bg.tiles, c->bg.ctl);
+    else
+        det_tiles_kernel<false><<<(unsigned)n_tiles, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity,
+                                                                c->bg.tiles, c->bg.ctl);
+    det_scan_kernel<<<1, 1024, 0, st>>>(c->bg.tiles, (int)n_tiles, offsets, c->bg.ctl, (long long*)n_dev);
+    c->n_launches += 2;
+    if (capacity > 0) {
+        det_gather_kernel<<<(unsigned)((n_tiles + 7) / 8), 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, c->bg.tmp,
+                                                                        (ArgusSourceRec*)out, (unsigned)capacity);
+        c->n_launches++;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    if (n_out) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->bg.h_n, c->bg.ctl, 8, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        *n_out = (size_t)(((unsigned long long)*c->bg.h_n) >> 32);     // ctl[1]
+        if (capacity > 0 && *n_out > capacity) return ARGUS_ERR_CAPACITY;
     }
     return ARGUS_OK;
 }

@@ -1,0 +1,475 @@
+// background.cuh -- median-filtered background / noise map and source detection on the calibrated frame
+// (DESIGN.md section 11): the two GPU stages the paper runs between calibration and
+// resampling (PAPER.md:193-194 Table 2, :135; "intermediate background and noise maps" :109).  Calibration is
+// fused into both passes when the frame arrives as raw + masters (the calibrated frame never exists in HBM).
+//
+//   bg_cells_kernel    one CTA per B x B cell (B <= 64): the cell's pixels live in registers (16 per thread) as
+//                      order-preserving 32-bit keys; the two central order statistics are found EXACTLY by a
+//                      bitwise bisection on the key (count of keys below a candidate, one CTA-wide sum per bit),
+//                      started below the common prefix of the cell's min and max and finished by ranking the
+//                      survivors once 32 or fewer remain.  Same again on |v - med| for the MAD noise estimate.
+//   bg_filter_kernel   3x3 median over the valid cells of the grid (one thread per cell).
+//   det_tiles_kernel   one CTA per 64 x 32-pixel tile: s = cal - bkg(x, y) for the tile + 1-pixel apron in shared
+//                      memory, thresholded raster-first local maxima, 3x3 flux and centroid; records go to a
+//                      scratch list at an atomically reserved base, (base, count) per tile.
+//   det_scan_kernel    exclusive scan of the per-tile counts (tile order = catalogue order).
+//   det_gather_kernel  one warp per tile copies its records to their final, deterministic position.
+#pragma once
+#include "resample.cuh"
+
+#define BG_THREADS 256
+#define BG_KPT 16                    // keys per thread: 256 x 16 = 4096 = 64 x 64
+#define BG_SENTINEL 0xffffffffu      // masked / outside the cell: sorts after every value
+#define BG_FINISH 32                 // rank the survivors directly once this few remain
+#define BG_MAD_TO_SIGMA 1.4826f
+
+struct ArgusSourceRec {              // == argus_source (argus.h)
+    int x, y;
+    float peak, flux, cx, cy, bkg, nse;
+};
+
+__device__ __forceinline__ unsigned bg_key(float v) {
+    unsigned u = __float_as_uint(v);
+    return (v != v) ? BG_SENTINEL : ((u & 0x80000000u) ? ~u : (u | 0x80000000u));
+}
+__device__ __forceinline__ float bg_unkey(unsigned k) {
+    return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k);
+}
+
+// Four consecutive pixels starting at (x, y), x % 4 == 0: calibrated value, NaN where masked / outside [0, x_end).
+template <bool FUSED>
+__device__ __forceinline__ void bg_load4(const FrameArgs& f, int W, int H, int x, int y, int x_end, float v[4]) {
+    if (y >= H || x >= x_end) { v[0] = v[1] = v[2] = v[3] = nanf_(); return; }
+    if (f.vec_ok && x + 3 < x_end) {
+        size_t o = (size_t)y * W + x;
+        if (FUSED) {
+            uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
+            float4 b = __ldg(reinterpret_cast<const float4*>(f.bias + o));
+            float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));
+            float4 fl = __ldg(reinterpret_cast<const float4*>(f.flat + o));
+            unsigned bp = f.bpm ? __ldg(reinterpret_cast<const unsigned*>(f.bpm + o)) : 0u;
+            int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
+            v[0] = calib_px((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
+            v[1] = calib_px((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
+            v[2] = calib_px((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
+            v[3] = calib_px((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+        } else {
+            float4 c = __ldg(reinterpret_cast<const float4*>(f.cal + o));
+            unsigned m = __ldg(reinterpret_cast<const unsigned*>(f.mask + o));
+            v[0] = (m & 0xffu) ? c.x : nanf_();
+            v[1] = (m & 0xff00u) ? c.y : nanf_();
+            v[2] = (m & 0xff0000u) ? c.z : nanf_();
+            v[3] = (m & 0xff000000u) ? c.w : nanf_();
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] = (x + i < x_end) ? load_px<FUSED>(f, W, H, x + i, y) : nanf_();
+    }
+}
+
+// CTA-wide sum of one int per thread; s_red is [2][8] ints, `par` alternates between calls (one barrier per call).
+__device__ __forceinline__ int bg_block_sum(int v, int* s_red, int& par) {
+    v = __reduce_add_sync(0xffffffffu, v);
+    int* r = s_red + par * 8;
+    if ((threadIdx.x & 31) == 0) r[threadIdx.x >> 5] = v;
+    __syncthreads();
+    int4 a = *reinterpret_cast<const int4*>(r), b = *reinterpret_cast<const int4*>(r + 4);
+    par ^= 1;
+    return a.x + a.y + a.z + a.w + b.x + b.y + b.z + b.w;
+}
+__device__ __forceinline__ unsigned bg_block_min(unsigned v, int* s_red, int& par) {
+    v = __reduce_min_sync(0xffffffffu, v);
+    unsigned* r = reinterpret_cast<unsigned*>(s_red + par * 8);
+    if ((threadIdx.x & 31) == 0) r[threadIdx.x >> 5] = v;
+    __syncthreads();
+    uint4 a = *reinterpret_cast<const uint4*>(r), b = *reinterpret_cast<const uint4*>(r + 4);
+    par ^= 1;
+    return min(min(min(a.x, a.y), min(a.z, a.w)), min(min(b.x, b.y), min(b.z, b.w)));
+}
+__device__ __forceinline__ unsigned bg_block_max_valid(unsigned v, int* s_red, int& par) {   // v = 0 for "none"
+    v = __reduce_max_sync(0xffffffffu, v);
+    unsigned* r = reinterpret_cast<unsigned*>(s_red + par * 8);
+    if ((threadIdx.x & 31) == 0) r[threadIdx.x >> 5] = v;
+    __syncthreads();
+    uint4 a = *reinterpret_cast<const uint4*>(r), b = *reinterpret_cast<const uint4*>(r + 4);
+    par ^= 1;
+    return max(max(max(a.x, a.y), max(a.z, a.w)), max(max(b.x, b.y), max(b.z, b.w)));
+}
+
+// k-th smallest (0-based, k < n) of the n non-sentinel keys held by the CTA (BG_KPT per thread); kmin / kmax are
+// their extremes.  Bitwise bisection: the answer is the largest v with #{key < v} <= k; bits above the highest
+// bit in which kmin and kmax differ are common to every key.  s_list: 33 words, s_cnt: 1 word of shared memory.
+__device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned kmin, unsigned kmax,
+                                              int* s_red, int& par, unsigned* s_list, int* s_cnt) {
+    if (kmin == kmax) return kmin;
+    int bit = 31 - __clz(kmin ^ kmax);
+    unsigned prefix = (bit == 31) ? 0u : ((kmax >> (bit + 1)) << (bit + 1));
+    int c_lo = 0, c_hi = n;                        // #{key < prefix}, #{key <= prefix | low bits}
+    while (bit >= 0 && c_hi - c_lo > BG_FINISH) {
+        const unsigned cand = prefix | (1u << bit);
+        int c = 0;
+#pragma unroll
+        for (int i = 0; i < BG_KPT; ++i) c += (key[i] < cand) ? 1 : 0;
+        c = bg_block_sum(c, s_red, par);
+        if (c <= k) { prefix = cand; c_lo = c; } else c_hi = c;
+        --bit;
+    }
+    if (bit < 0) return prefix;
+    // at most BG_FINISH keys remain in [prefix, prefix | mask]: rank them directly (ties by list position)
+    const unsigned upper = prefix | ((2u << bit) - 1u);
+    if (threadIdx.x == 0) *s_cnt = 0;
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < BG_KPT; ++i)
+        if (key[i] >= prefix && key[i] <= upper && key[i] != BG_SENTINEL) {
+            int p = atomicAdd(s_cnt, 1);
+            if (p < BG_FINISH) s_list[p] = key[i];
+        }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int m = min(*s_cnt, BG_FINISH), lane = threadIdx.x;
+        const unsigned mine = (lane < m) ? s_list[lane] : BG_SENTINEL;
+        int rank = 0;
+        for (int j = 0; j < m; ++j) {
+            unsigned kj = __shfl_sync(0xffffffffu, mine, j);
+            rank += (kj < mine || (kj == mine && j < lane)) ? 1 : 0;
+        }
+        if (lane < m && rank == k - c_lo) s_list[BG_FINISH] = mine;
+    }
+    __syncthreads();
+    return s_list[BG_FINISH];
+}
+
+// median rule of R-D1: (v_((n-1)/2) + v_(n/2)) / 2 as keys -> the two central keys.
+__device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], int n, unsigned kmin, unsigned kmax, int* s_red,
+                                                int& par, unsigned* s_list, int* s_cnt, unsigned& k1, unsigned& k2) {
+    const int r = (n - 1) >> 1;
+    k1 = bg_select(key, r, n, kmin, kmax, s_red, par, s_list, s_cnt);
+    k2 = k1;
+    if ((n & 1) == 0) {                             // rank r + 1: k1 again if it repeats, else the next larger key
+        int c = 0;
+        unsigned nxt = BG_SENTINEL;
+#pragma unroll
+        for (int i = 0; i < BG_KPT; ++i) {
+            c += (key[i] <= k1) ? 1 : 0;
+            if (key[i] > k1) nxt = min(nxt, key[i]);
+        }
+        c = bg_block_sum(c, s_red, par);
+        nxt = bg_block_min(nxt, s_red, par);
+        if (r + 1 >= c) k2 = nxt;
+    }
+}
+
+// R-D1: per-cell median, 1.4826 MAD and good-pixel count.  grid = GX * GY CTAs of 256 threads; B in {8,16,32,64}.
+template <bool FUSED>
+__global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W, int H, int B, int GX, int n_min,
+                                                              float* __restrict__ med_out, float* __restrict__ sig_out,
+                                                              int* __restrict__ ngood_out) {
+    __shared__ __align__(16) int s_red[16];
+    __shared__ unsigned s_list[BG_FINISH + 1];
+    __shared__ int s_cnt;
+    const int cell = blockIdx.x, gx = cell % GX, gy = cell / GX;
+    const int x0 = gx * B, y0 = gy * B, x_end = min(x0 + B, W), y_end = min(y0 + B, H);
+    const int col = (threadIdx.x & 15) * 4, row = threadIdx.x >> 4;
+    unsigned key[BG_KPT];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        float v[4];
+        bg_load4<FUSED>(f, W, y_end, x0 + col, y0 + row + 16 * j, x_end, v);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) key[4 * j + i] = bg_key(v[i]);
+    }
+    int par = 0;
+    int n = 0;
+    unsigned lo = BG_SENTINEL, hi = 0u;
+#pragma unroll
+    for (int i = 0; i < BG_KPT; ++i) {
+        const bool ok = key[i] != BG_SENTINEL;
+        n += ok ? 1 : 0;
+        lo = min(lo, key[i]);
+        hi = max(hi, ok ? key[i] : 0u);
+    }
+    n = bg_block_sum(n, s_red, par);
+    if (n < max(n_min, 1)) {
+        if (threadIdx.x == 0) { med_out[cell] = 0.f; sig_out[cell] = 0.f; ngood_out[cell] = n; }
+        return;
+    }
+    lo = bg_block_min(lo, s_red, par);
+    hi = bg_block_max_valid(hi, s_red, par);
+    unsigned k1, k2;
+    bg_central_pair(key, n, lo, hi, s_red, par, s_list, &s_cnt, k1, k2);
+    const float med = 0.5f * (bg_unkey(k1) + bg_unkey(k2));
+    // MAD: |v - med| >= 0, whose bit patterns are already ordered
+    lo = BG_SENTINEL; hi = 0u;
+#pragma unroll
+    for (int i = 0; i < BG_KPT; ++i) {
+        const bool ok = key[i] != BG_SENTINEL;
+        const unsigned d = ok ? __float_as_uint(fabsf(bg_unkey(key[i]) - med)) : BG_SENTINEL;
+        key[i] = d;
+        lo = min(lo, d);
+        hi = max(hi, ok ? d : 0u);
+    }
+    lo = bg_block_min(lo, s_red, par);
+    hi = bg_block_max_valid(hi, s_red, par);
+    bg_central_pair(key, n, lo, hi, s_red, par, s_list, &s_cnt, k1, k2);
+    const float mad = 0.5f * (__uint_as_float(k1) + __uint_as_float(k2));
+    if (threadIdx.x == 0) { med_out[cell] = med; sig_out[cell] = BG_MAD_TO_SIGMA * mad; ngood_out[cell] = n; }
+}
+
+// R-D2: 3x3 median over the valid cells (clipped to the grid); no valid cell: bkg = 0, nse = +inf.
+__device__ __forceinline__ float bg_median_small(float* v, int m) {
+    for (int i = 1; i < m; ++i) {
+        float x = v[i];
+        int j = i - 1;
+        while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; --j; }
+        v[j + 1] = x;
+    }
+    return 0.5f * (v[(m - 1) >> 1] + v[m >> 1]);
+}
+__global__ void __launch_bounds__(128) bg_filter_kernel(const float* __restrict__ med, const float* __restrict__ sig,
+                                                        const int* __restrict__ ngood, int GX, int GY, int n_min,
+                                                        float* __restrict__ bkg, float* __restrict__ nse) {
+    const int c = blockIdx.x * 128 + threadIdx.x;
+    if (c >= GX * GY) return;
+    const int gx = c % GX, gy = c / GX;
+    float a[9], b[9];
+    int m = 0;
+    for (int y = max(gy - 1, 0); y <= min(gy + 1, GY - 1); ++y)
+        for (int x = max(gx - 1, 0); x <= min(gx + 1, GX - 1); ++x) {
+            const int q = y * GX + x;
+            if (ngood[q] >= max(n_min, 1)) { a[m] = med[q]; b[m] = sig[q]; ++m; }
+        }
+    bkg[c] = m ? bg_median_small(a, m) : 0.f;
+    nse[c] = m ? bg_median_small(b, m) : __int_as_float(0x7f800000);
+}
+
+// ------------------------------------------------------------------------------------------------ detection
+#define DET_TW 64
+#define DET_TH 32
+#define DET_PITCH 66                 // 64 + 2 apron columns; 66 mod 32 = 2 spreads a warp's four rows over the banks
+#define DET_PROWS 8                  // node patch: (DET_TH + 2) / 8 + 2 rows, (DET_TW + 2) / 8 + 2 columns at B = 8
+#define DET_PCOLS 12
+
+struct DetGrid {
+    const float* bkg;
+    const float* nse;
+    int B, GX, GY;
+    float inv_B, half;               // 1 / B, (B - 1) / 2
+    float k_sigma;
+};
+
+// R-D3 along one axis: lower node and fraction of pixel coordinate p (clamped outside the outermost centres).
+__device__ __forceinline__ void det_node(int p, const DetGrid& g, int G, int& g0, float& t) {
+    const float u = fminf(fmaxf(((float)p - g.half) * g.inv_B, 0.f), (float)(G - 1));
+    g0 = min((int)u, max(G - 2, 0));
+    t = u - (float)g0;
+}
+__device__ __forceinline__ float det_interp(const float (*patch)[DET_PCOLS], int lx, int ly, int lx1, int ly1, float tx, float ty) {
+    const float top = fmaf(tx, patch[ly][lx1] - patch[ly][lx], patch[ly][lx]);
+    const float bot = fmaf(tx, patch[ly1][lx1] - patch[ly1][lx], patch[ly1][lx]);
+    return fmaf(ty, bot - top, top);
+}
+
+// R-D4 / R-D5 on one 64 x 32 tile.  tile_info[tile] = (base of the tile's records in tmp, count); *total counts all.
+// Staging: the node patch is interpolated along y once per tile row (s_rb / s_rn), the x node and fraction of every
+// tile column are tabulated (s_col), so a pixel's background costs two shared loads and one FMA.
+template <bool FUSED>
+__global__ void __launch_bounds__(256, 3) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
+                                                           ArgusSourceRec* __restrict__ tmp, unsigned capacity,
+                                                           uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
+    __shared__ float s_s[(DET_TH + 2) * DET_PITCH];
+    __shared__ float s_b[DET_PROWS][DET_PCOLS], s_n[DET_PROWS][DET_PCOLS];
+    __shared__ float s_rb[DET_TH + 2][DET_PCOLS], s_rn[DET_TH + 2][DET_PCOLS];
+    __shared__ float2 s_col[DET_PITCH];              // (.x: node offsets lx | lx1 << 8 as int bits, .y: tx)
+    __shared__ int s_warp[8];
+    __shared__ unsigned s_base;
+    const int tile = blockIdx.x, x0 = (tile % tiles_x) * DET_TW, y0 = (tile / tiles_x) * DET_TH, tid = threadIdx.x;
+    int pgx, pgy;
+    float tdummy;
+    det_node(x0 - 1, g, g.GX, pgx, tdummy);
+    det_node(y0 - 1, g, g.GY, pgy, tdummy);
+    if (tid < DET_PROWS * DET_PCOLS) {
+        const int r = tid / DET_PCOLS, c = tid % DET_PCOLS;
+        const int q = min(pgy + r, g.GY - 1) * g.GX + min(pgx + c, g.GX - 1);
+        s_b[r][c] = __ldg(g.bkg + q);
+        s_n[r][c] = __ldg(g.nse + q);
+    } else if (tid >= 128 && tid < 128 + DET_PITCH) {
+        int gx0;
+        float tx;
+        det_node(x0 - 1 + (tid - 128), g, g.GX, gx0, tx);
+        s_col[tid - 128] = make_float2(__int_as_float((gx0 - pgx) | ((min(gx0 + 1, g.GX - 1) - pgx) << 8)), tx);
+    }
+    __syncthreads();
+    for (int e = tid; e < (DET_TH + 2) * DET_PCOLS; e += 256) {
+        const int r = e / DET_PCOLS, c = e - r * DET_PCOLS;
+        int gy0;
+        float ty;
+        det_node(y0 - 1 + r, g, g.GY, gy0, ty);
+        const int ly = gy0 - pgy, ly1 = min(gy0 + 1, g.GY - 1) - pgy;
+        s_rb[r][c] = fmaf(ty, s_b[ly1][c] - s_b[ly][c], s_b[ly][c]);
+        s_rn[r][c] = fmaf(ty, s_n[ly1][c] - s_n[ly][c], s_n[ly][c]);
+    }
+    __syncthreads();
+    const float ninf = __int_as_float(0xff800000);   // -inf: masked and off-frame pixels never win, never count
+    // interior: (DET_TH + 2) rows x 16 groups of four pixels (vector loads); apron columns: one pixel each side
+    for (int e = tid; e < (DET_TH + 2) * 16; e += 256) {
+        const int r = e >> 4, q = e & 15, py = y0 - 1 + r;
+        float v[4];
+        if (py >= 0) bg_load4<FUSED>(f, W, H, x0 + 4 * q, py, W, v);
+        else v[0] = v[1] = v[2] = v[3] = nanf_();
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int c = 1 + 4 * q + i;
+            const float2 ci = s_col[c];
+            const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
+            const float b0 = s_rb[r][lx];
+            const float s = v[i] - fmaf(ci.y, s_rb[r][lx1] - b0, b0);
+            s_s[r * DET_PITCH + c] = (v[i] == v[i]) ? s : ninf;
+        }
+    }
+    if (tid < 2 * (DET_TH + 2)) {
+        const int r = tid >> 1, c = (tid & 1) ? DET_PITCH - 1 : 0;
+        const float v = load_px<FUSED>(f, W, H, x0 - 1 + c, y0 - 1 + r);
+        const float2 ci = s_col[c];
+        const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
+        const float b0 = s_rb[r][lx];
+        s_s[r * DET_PITCH + c] = (v == v) ? v - fmaf(ci.y, s_rb[r][lx1] - b0, b0) : ninf;
+    }
+    __syncthreads();
+    // each thread: 8 consecutive pixels of one row; 3 x 10 window in registers
+    const int ry = tid >> 3, cx0 = (tid & 7) * 8;
+    float w[3][10];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 10; ++c) w[r][c] = s_s[(ry + r) * DET_PITCH + cx0 + c];
+    unsigned bits = 0;
+    const int py = y0 + ry;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const float c = w[1][j + 1];
+        bool ok = c > 0.f;                               // also false for -inf
+        ok = ok && c > w[0][j] && c > w[0][j + 1] && c > w[0][j + 2] && c > w[1][j];
+        ok = ok && c >= w[1][j + 2] && c >= w[2][j] && c >= w[2][j + 1] && c >= w[2][j + 2];
+        if (ok) {
+            const float2 ci = s_col[cx0 + j + 1];
+            const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
+            const float n0 = s_rn[ry + 1][lx];
+            const float nse = fmaf(ci.y, s_rn[ry + 1][lx1] - n0, n0);
+            ok = c > g.k_sigma * nse;                    // false for nse = +inf or NaN (undefined background)
+        }
+        bits |= ok ? (1u << j) : 0u;
+    }
+    // CTA-wide exclusive scan of the per-thread counts (thread order = raster order inside the tile)
+    const int cnt = __popc(bits), lane = tid & 31, wid = tid >> 5;
+    int inc = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += o;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    int before = inc - cnt, tile_cnt = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int c = s_warp[k];
+        before += (k < wid) ? c : 0;
+        tile_cnt += c;
+    }
+    if (tid == 0) {
+        const unsigned base = tile_cnt ? atomicAdd(total, (unsigned)tile_cnt) : 0u;
+        tile_info[tile] = make_uint2(base, (unsigned)tile_cnt);
+        s_base = base;
+    }
+    if (tile_cnt == 0) return;
+    __syncthreads();
+    unsigned pos = s_base + (unsigned)before;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        if (!((bits >> j) & 1u)) continue;
+        float flux = 0.f, mx = 0.f, my = 0.f;
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float q = w[r][j + c];
+                if (q != ninf) { flux += q; mx += q * (float)(c - 1); my += q * (float)(r - 1); }
+            }
+        const float2 ci = s_col[cx0 + j + 1];
+        const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
+        const float b0 = s_rb[ry + 1][lx], n0 = s_rn[ry + 1][lx];
+        ArgusSourceRec rec;
+        rec.x = x0 + cx0 + j; rec.y = py;
+        rec.peak = w[1][j + 1]; rec.flux = flux;
+        rec.cx = flux > 0.f ? mx / flux : 0.f;
+        rec.cy = flux > 0.f ? my / flux : 0.f;
+        rec.bkg = fmaf(ci.y, s_rb[ry + 1][lx1] - b0, b0);
+        rec.nse = fmaf(ci.y, s_rn[ry + 1][lx1] - n0, n0);
+        if (pos < capacity) {
+            uint4* dst = reinterpret_cast<uint4*>(tmp + pos);
+            dst[0] = make_uint4((unsigned)rec.x, (unsigned)rec.y, __float_as_uint(rec.peak), __float_as_uint(rec.flux));
+            dst[1] = make_uint4(__float_as_uint(rec.cx), __float_as_uint(rec.cy), __float_as_uint(rec.bkg), __float_as_uint(rec.nse));
+        }
+        ++pos;
+    }
+}
+
+// Exclusive scan of the tile counts in tile order; *n_dev (may be NULL) and ctl[1] receive the total.
+__global__ void __launch_bounds__(1024) det_scan_kernel(const uint2* __restrict__ tile_info, int n_tiles,
+                                                        unsigned* __restrict__ offsets, unsigned* __restrict__ ctl,
+                                                        long long* __restrict__ n_dev) {
+    __shared__ unsigned s_w[32];
+    __shared__ unsigned s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (int b = 0; b < n_tiles; b += 1024) {
+        const int i = b + tid;
+        const unsigned c = i < n_tiles ? tile_info[i].y : 0u;
+        unsigned inc = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += o;
+        }
+        if (lane == 31) s_w[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            unsigned v = s_w[lane], x = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                unsigned o = __shfl_up_sync(0xffffffffu, x, d);
+                if (lane >= d) x += o;
+            }
+            s_w[lane] = x - v;
+        }
+        __syncthreads();
+        const unsigned carry = s_carry;
+        if (i < n_tiles) offsets[i] = carry + s_w[wid] + inc - c;
+        __syncthreads();
+        if (tid == 1023) s_carry = carry + s_w[31] + inc;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        ctl[1] = s_carry;
+        if (n_dev) *n_dev = (long long)s_carry;
+    }
+}
+
+// One warp per tile: tmp[base .. base + cnt) -> out[offset .. offset + cnt).
+__global__ void __launch_bounds__(256) det_gather_kernel(const uint2* __restrict__ tile_info, const unsigned* __restrict__ offsets,
+                                                         int n_tiles, const ArgusSourceRec* __restrict__ tmp,
+                                                         ArgusSourceRec* __restrict__ out, unsigned capacity) {
+    const int tile = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (tile >= n_tiles) return;
+    const uint2 info = tile_info[tile];
+    const unsigned off = offsets[tile];
+    for (unsigned j = lane; j < info.y; j += 32) {
+        if (info.x + j >= capacity || off + j >= capacity) break;
+        const uint4* src = reinterpret_cast<const uint4*>(tmp + info.x + j);
+        uint4* dst = reinterpret_cast<uint4*>(out + off + j);
+        dst[0] = src[0];
+        dst[1] = src[1];
+    }
+}

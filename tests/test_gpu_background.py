@@ -1,0 +1,214 @@
+"""GPU parity (-m gpu) of argus_background_map / argus_detect_sources against oracle/background.py,
+through the C ABI.
+
+Tolerances: the medians are exact selections, so on an identical float32 calibrated frame the
+cell medians are compared BIT-EXACTLY and the good-pixel counts exactly; the filtered background (a mean of two
+float32 medians where the oracle has fp64 ones) to one float32 ulp; the MAD noise is formed from float32 differences.  With fused calibration the float32 calibrated value
+differs from the oracle's fp64 one, and everything is held to the north_star tolerance 1e-3 ADU + 1e-5 relative.
+Detection is a floating-point decision: the oracle reports the decision margins, sources whose margins exceed the value
+tolerance must be found, sources found must have margins above minus the tolerance, the rest is counted as ambiguous.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+import synth  # noqa: E402
+from oracle import background as ob  # noqa: E402
+from synth import frames as sf  # noqa: E402
+from gpu_util import VALUE_ATOL, VALUE_RTOL, upload  # noqa: E402
+
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def argus():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2207_14304_b200 as a
+    a.load_library()
+    return a
+
+
+@pytest.fixture(scope="module")
+def ctx(argus):
+    c = argus.Context(0)
+    yield c
+    c.close()
+
+
+def _grid(W, H, B):
+    return -(-H // B), -(-W // B)
+
+
+def gpu_background(argus, ctx, W, H, B, n_min, frame):
+    GY, GX = _grid(W, H, B)
+    o = {k: torch.full((GY * GX,), float("nan"), dtype=torch.float32, device=DEV) for k in ("bkg", "nse", "med", "sig")}
+    ng = torch.full((GY * GX,), -1, dtype=torch.int32, device=DEV)
+    argus.argus_background_map(ctx, W, H, o["bkg"], o["nse"], cell=B, n_min=n_min, med_out=o["med"], sig_out=o["sig"],
+                               ngood_out=ng, **frame)
+    torch.cuda.synchronize()
+    out = {k: v.cpu().numpy().reshape(GY, GX) for k, v in o.items()}
+    out["ngood"] = ng.cpu().numpy().reshape(GY, GX)
+    out["dev"] = o
+    return out
+
+
+def gpu_detect(argus, ctx, W, H, B, k, bkg_dev, nse_dev, frame, cap=200000):
+    out = torch.zeros((cap * 32,), dtype=torch.uint8, device=DEV)
+    n_dev = torch.full((1,), -1, dtype=torch.int64, device=DEV)
+    n = argus.argus_detect_sources(ctx, W, H, bkg_dev, nse_dev, out, cell=B, k_sigma=k, n_dev=n_dev, **frame)
+    assert int(n_dev.item()) == n
+    return out.cpu().numpy()[:n * 32].view(argus.SOURCE_DTYPE)
+
+
+def tol(v):
+    return VALUE_ATOL + VALUE_RTOL * np.abs(v)
+
+
+def compare_grids(g, cal64, mask, B, n_min, exact):
+    med, sig, valid, ngood = ob.cell_stats(cal64, mask, B, n_min)
+    bkg, nse = ob.filter_grid(med, sig, valid)
+    assert np.array_equal(g["ngood"], ngood)
+    if exact:
+        assert np.array_equal(g["med"], med.astype(np.float32)), "cell medians not bit-exact"
+        # the 3x3 filter averages two float32 medians where the oracle averages two fp64 ones: one float32 ulp
+        assert np.all(np.abs(g["bkg"] - bkg) <= np.spacing(np.abs(bkg).astype(np.float32))), "filtered background off by > 1 ulp"
+    else:
+        assert np.all(np.abs(g["med"] - med) <= tol(med)) and np.all(np.abs(g["bkg"] - bkg) <= tol(bkg))
+    fin = np.isfinite(nse)
+    assert np.array_equal(np.isinf(g["nse"]), ~fin)
+    # sig = 1.4826 * median |v - med|: float32 differences about a float32 median
+    assert np.all(np.abs(g["sig"] - sig) <= tol(sig) + 2e-6 * np.abs(med))
+    assert np.all(np.abs(g["nse"][fin] - nse[fin]) <= tol(nse[fin]) + 2e-6 * np.abs(bkg[fin]))
+    return bkg, nse
+
+
+def compare_catalogue(rec, cal64, mask, bkg_or, nse_or, W, B, k, max_ambiguous=3):
+    """rec: GPU records (GPU map -> GPU detection); bkg_or / nse_or: the ORACLE's grids.  The decision margin allowance
+    covers the value tolerance on the calibrated pixel, on the interpolated background and on k * noise."""
+    d = ob.detect(cal64, mask, bkg_or, nse_or, B=B, k_sigma=k, slack=1.0)
+    eps = 2 * tol(d["peak"] + d["bkg"]) + k * tol(np.where(np.isfinite(d["nse"]), d["nse"], 0.0))
+    must = d["strict"] & (d["m_thr"] > eps) & (d["m_max"] > eps)
+    may = (d["m_thr"] > -eps) & (d["m_max"] > -eps)
+    key_o = d["y"].astype(np.int64) * W + d["x"]
+    key_g = rec["y"].astype(np.int64) * W + rec["x"]
+    assert np.unique(key_g).size == key_g.size
+    tile_key = (rec["y"] // 32).astype(np.int64) * (-(-W // 64)) + rec["x"] // 64
+    order = np.lexsort((rec["x"], rec["y"], tile_key))
+    assert np.array_equal(order, np.arange(rec.size)), "catalogue not in tile-major order"
+    assert np.isin(key_o[must], key_g).all(), "a clear source is missing"
+    assert np.isin(key_g, key_o[may]).all(), "a record is not a source"
+    n_amb = int((may & ~must).sum())
+    assert n_amb <= max(max_ambiguous, 1e-3 * max(int(must.sum()), 1)), "%d ambiguous decisions" % n_amb
+    # matched records: fields
+    pos = {kk: i for i, kk in enumerate(key_o.tolist())}
+    j = np.array([pos[kk] for kk in key_g.tolist()], dtype=np.int64)
+    t9 = 9 * tol(d["peak"][j] + d["bkg"][j])
+    assert np.all(np.abs(rec["peak"] - d["peak"][j]) <= t9 / 9 * 2)
+    assert np.all(np.abs(rec["bkg"] - d["bkg"][j]) <= tol(d["bkg"][j]))
+    assert np.all(np.abs(rec["nse"] - d["nse"][j]) <= tol(d["nse"][j]) + 2e-6 * np.abs(d["bkg"][j]))
+    assert np.all(np.abs(rec["flux"] - d["flux"][j]) <= t9 + tol(d["flux"][j]))
+    well = d["flux"][j] > 100 * t9
+    for c in ("cx", "cy"):
+        assert np.all(np.abs(rec[c][well] - d[c][j][well]) <= 4 * t9[well] / d["flux"][j][well] + 1e-5)
+        assert np.all(np.isfinite(rec[c]))
+    return int(must.sum()), n_amb
+
+
+def _cal32(fr):
+    """The oracle's calibrated frame rounded to float32 (an identical input for both sides) and its mask."""
+    cal, mask = oracle.calibrate_frame(fr)
+    cal32 = cal.astype(np.float32)
+    return cal32, mask.astype(np.uint8)
+
+
+def _dev_cal(cal32, mask):
+    return dict(cal=torch.from_numpy(cal32).to(DEV), mask=torch.from_numpy(mask).to(DEV))
+
+
+@pytest.mark.parametrize("B,n_min", [(64, 16), (32, 16), (16, 4), (8, 1)])
+def test_config0_calibrated_frame_is_bit_exact(argus, ctx, B, n_min):
+    fr = sf.config0()
+    H, W = fr.shape
+    cal32, mask = _cal32(fr)
+    g = gpu_background(argus, ctx, W, H, B, n_min, _dev_cal(cal32, mask))
+    bkg, nse = compare_grids(g, cal32.astype(np.float64), mask, B, n_min, exact=True)
+    rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
+    n_must, _ = compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0)
+    assert n_must > 50          # config 0 plants 300 stars
+
+
+@pytest.mark.parametrize("B", [64, 16])
+def test_config0_fused_calibration(argus, ctx, B):
+    fr = sf.config0()
+    H, W = fr.shape
+    cal, mask = oracle.calibrate_frame(fr)
+    d = upload(fr)
+    g = gpu_background(argus, ctx, W, H, B, 16, d)
+    bkg, nse = compare_grids(g, cal, mask, B, 16, exact=False)
+    rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], d)
+    compare_catalogue(rec, cal, mask, bkg, nse, W, B, 5.0)
+    # fused == calibrate -> map / detect on the GPU (same float32 arithmetic): identical bits
+    calg = torch.empty((H, W), dtype=torch.float32, device=DEV)
+    maskg = torch.empty((H, W), dtype=torch.uint8, device=DEV)
+    argus.argus_calibrate(ctx, d["raw"], d["bias"], d["dark"], d["flat"], d["bpm"], d["t_exp"], d["sat_adu"], d["flat_min"],
+                          cal_out=calg, mask_out=maskg)
+    g2 = gpu_background(argus, ctx, W, H, B, 16, dict(cal=calg, mask=maskg))
+    for k in ("med", "sig", "bkg", "nse", "ngood"):
+        assert np.array_equal(g[k], g2[k]), k
+    rec2 = gpu_detect(argus, ctx, W, H, B, 5.0, g2["dev"]["bkg"], g2["dev"]["nse"], dict(cal=calg, mask=maskg))
+    assert rec.tobytes() == rec2.tobytes()
+
+
+@pytest.mark.parametrize("W,H,B", [(500, 391, 64), (333, 130, 32), (70, 45, 16), (64, 32, 64), (5, 3, 8)])
+def test_ragged_shapes_defects_and_unaligned_rows(argus, ctx, W, H, B):
+    rng = np.random.default_rng(W * 1000 + H)
+    cal32 = rng.normal(150.0, 9.0, (H, W)).astype(np.float32)
+    mask = (rng.random((H, W)) > 0.03).astype(np.uint8)
+    if W > 100:
+        mask[10:90, 20:120] = 0                      # invalid cells: a hole larger than a cell
+        cal32[5:8, 60:63] += 4000.0                  # a bright blob with equal neighbours (ties)
+        cal32[200 % H, :] += 300.0                   # a bright row: ties along x
+    cal32[mask == 0] = 0.0
+    n_min = 8 if W > 100 else 1
+    g = gpu_background(argus, ctx, W, H, B, n_min, _dev_cal(cal32, mask))
+    bkg, nse = compare_grids(g, cal32.astype(np.float64), mask, B, n_min, exact=True)
+    rec = gpu_detect(argus, ctx, W, H, B, 4.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
+    compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 4.0, max_ambiguous=6)
+
+
+def test_hand_built_sources_and_capacity(argus, ctx):
+    H, W, B = 48, 64, 16
+    cal = np.zeros((H, W), np.float32)
+    cal[10, 20] = 100.0; cal[30, 40] = cal[30, 41] = 50.0; cal[20, 8] = cal[21, 8] = 30.0; cal[40, 50] = 80.0; cal[40, 51] = 20.0
+    mask = np.ones((H, W), np.uint8)
+    fr = _dev_cal(cal, mask)
+    g = gpu_background(argus, ctx, W, H, B, 16, fr)
+    assert np.all(g["bkg"] == 0) and np.all(g["nse"] == 0)
+    rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], fr, cap=16)
+    assert list(zip(rec["y"].tolist(), rec["x"].tolist())) == [(10, 20), (20, 8), (30, 40), (40, 50)]
+    assert rec["peak"].tolist() == [100, 30, 50, 80] and rec["flux"].tolist() == [100, 60, 100, 100]
+    assert rec["cx"].tolist() == [0, 0, 0.5, pytest.approx(0.2)] and rec["cy"].tolist() == [0, 0.5, 0, 0]
+    # count only, then too small a capacity: the count is reported with ARGUS_ERR_CAPACITY
+    assert argus.argus_detect_sources(ctx, W, H, g["dev"]["bkg"], g["dev"]["nse"], None, cell=B, **fr) == 4
+    small = torch.zeros((2 * 32,), dtype=torch.uint8, device=DEV)
+    with pytest.raises(argus.ArgusError) as e:
+        argus.argus_detect_sources(ctx, W, H, g["dev"]["bkg"], g["dev"]["nse"], small, cell=B, **fr)
+    assert e.value.status == -6 and "n_sources=4" in str(e.value)
+    # bad arguments
+    with pytest.raises(argus.ArgusError):
+        argus.argus_background_map(ctx, W, H, g["dev"]["bkg"], g["dev"]["nse"], cell=48, **fr)
+
+
+def test_undefined_background_suppresses_detection(argus, ctx):
+    cal = np.zeros((32, 64), np.float32); mask = np.ones((32, 64), np.uint8)
+    mask[:, 32:] = 0; mask[4, 40] = 1; cal[4, 40] = 500.0; cal[8, 8] = 9.0
+    fr = _dev_cal(cal, mask)
+    g = gpu_background(argus, ctx, 64, 32, 16, 16, fr)
+    assert np.isinf(g["nse"][:, 3]).all() and np.isfinite(g["nse"][:, :3]).all() and np.all(g["bkg"][:, 3] == 0)
+    rec = gpu_detect(argus, ctx, 64, 32, 16, 5.0, g["dev"]["bkg"], g["dev"]["nse"], fr)
+    assert list(zip(rec["y"].tolist(), rec["x"].tolist())) == [(8, 8)]

@@ -134,7 +134,7 @@ def test_hand_built_sources_position_flux_centroid_and_ties():
     cal[40, 50] = 80.0; cal[40, 51] = 20.0      # asymmetric pair: cx = 20 / 100
     d, bkg, nse = _detect_on_zero_background(cal)
     assert np.all(bkg == 0) and np.all(nse == 0)
-    assert list(zip(d["y"], d["x"])) == [(10, 20), (20, 8), (30, 40), (40, 50)]      # ascending raster order
+    assert list(zip(d["y"], d["x"])) == [(10, 20), (20, 8), (30, 40), (40, 50)]      # catalogue order
     assert np.allclose(d["peak"], [100, 30, 50, 80]) and np.allclose(d["flux"], [100, 60, 100, 100])
     assert np.allclose(d["cx"], [0, 0, 0.5, 0.2]) and np.allclose(d["cy"], [0, 0.5, 0, 0])
     assert d["strict"].all()
@@ -191,3 +191,16 @@ def test_gaussian_star_found_at_its_peak_pixel_with_signed_centroid():
     d, _, _ = _detect_on_zero_background(cal, k=5.0)
     assert list(zip(d["y"], d["x"])) == [(13, 45), (30, 20)]
     assert d["cx"][1] > 0.05 and abs(d["cy"][1]) < 1e-12 and d["cy"][0] < -0.05 and abs(d["cx"][0]) < 1e-12
+
+
+def test_catalogue_order_is_tile_major():
+    cal = np.zeros((70, 200))
+    for (y, x) in [(2, 150), (3, 10), (31, 70), (33, 5), (40, 199), (69, 64)]:
+        cal[y, x] = 10.0 + x
+    mask = np.ones(cal.shape, np.uint8)
+    bkg, nse = ob.background(cal, mask, B=16)
+    d = ob.detect(cal, mask, bkg, nse, B=16)
+    # tiles are 64 wide, 32 tall: row of tiles 0 holds y < 32 (x-tiles 0, 1, 2), then y in 32..63, then y >= 64
+    assert list(zip(d["y"], d["x"])) == [(3, 10), (31, 70), (2, 150), (33, 5), (40, 199), (69, 64)]
+    r = ob.detect(cal, mask, bkg, nse, B=16, tile=None)
+    assert list(zip(r["y"], r["x"])) == [(2, 150), (3, 10), (31, 70), (33, 5), (40, 199), (69, 64)]
