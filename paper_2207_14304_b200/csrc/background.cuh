@@ -67,15 +67,26 @@ __device__ __forceinline__ void bg_load4(const FrameArgs& f, int W, int H, int x
     }
 }
 
-// CTA-wide sum of one int per thread; s_red is [2][8] ints, `par` alternates between calls (one barrier per call).
-__device__ __forceinline__ int bg_block_sum(int v, int* s_red, int& par) {
+// CTA-wide sum of one int per thread.  s_red[16..18] are three rotating counters (zero at kernel start): call n adds
+// into counter n mod 3 and clears counter (n + 1) mod 3, whose last readers passed the previous barrier; `it` is the
+// caller's rotating index.  One warp reduction, one shared atomic per warp, one barrier, one load.
+__device__ __forceinline__ int bg_block_sum(int v, int* s_red, int& par, int& it) {
+    (void)par;
     v = __reduce_add_sync(0xffffffffu, v);
-    int* r = s_red + par * 8;
-    if ((threadIdx.x & 31) == 0) r[threadIdx.x >> 5] = v;
+    int* ctr = s_red + 16;
+    const int nxt = it == 2 ? 0 : it + 1;
+    if ((threadIdx.x & 31) == 0) atomicAdd(ctr + it, v);
+    if (threadIdx.x == 32) ctr[nxt] = 0;
     __syncthreads();
-    int4 a = *reinterpret_cast<const int4*>(r), b = *reinterpret_cast<const int4*>(r + 4);
-    par ^= 1;
-    return a.x + a.y + a.z + a.w + b.x + b.y + b.z + b.w;
+    const int r = ctr[it];
+    it = nxt;
+    return r;
+}
+// #{key < cand} added to c.  The compare runs on the ALU pipe; the increment is written as c = one * one + c with a
+// run-time `one` (blockDim.x / 256) so that it is an IMAD on the FMA pipe: both pipes issue one warp instruction
+// per two cycles per SM sub-partition, and a compare + integer add pair would queue both on the ALU pipe.
+__device__ __forceinline__ void bg_count_lt(int& c, unsigned key, unsigned cand, int one) {
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p mad.lo.s32 %0, %3, %3, %0;\n\t}" : "+r"(c) : "r"(key), "r"(cand), "r"(one));
 }
 __device__ __forceinline__ unsigned bg_block_min(unsigned v, int* s_red, int& par) {
     v = __reduce_min_sync(0xffffffffu, v);
@@ -100,17 +111,19 @@ __device__ __forceinline__ unsigned bg_block_max_valid(unsigned v, int* s_red, i
 // their extremes.  Bitwise bisection: the answer is the largest v with #{key < v} <= k; bits above the highest
 // bit in which kmin and kmax differ are common to every key.  s_list: 33 words, s_cnt: 1 word of shared memory.
 __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned kmin, unsigned kmax,
-                                              int* s_red, int& par, unsigned* s_list, int* s_cnt) {
+                                              int* s_red, int& par, int& it, unsigned* s_list, int* s_cnt) {
     if (kmin == kmax) return kmin;
     int bit = 31 - __clz(kmin ^ kmax);
     unsigned prefix = (bit == 31) ? 0u : ((kmax >> (bit + 1)) << (bit + 1));
     int c_lo = 0, c_hi = n;                        // #{key < prefix}, #{key <= prefix | low bits}
     while (bit >= 0 && c_hi - c_lo > BG_FINISH) {
         const unsigned cand = prefix | (1u << bit);
-        int c = 0;
+        int c = 0, c2 = 0;
+        const int one = (int)(blockDim.x >> 8);
 #pragma unroll
-        for (int i = 0; i < BG_KPT; ++i) c += (key[i] < cand) ? 1 : 0;
-        c = bg_block_sum(c, s_red, par);
+        for (int i = 0; i < BG_KPT; i += 2) { bg_count_lt(c, key[i], cand, one); bg_count_lt(c2, key[i + 1], cand, one); }
+        c += c2;
+        c = bg_block_sum(c, s_red, par, it);
         if (c <= k) { prefix = cand; c_lo = c; } else c_hi = c;
         --bit;
     }
@@ -142,9 +155,9 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
 
 // median rule of R-D1: (v_((n-1)/2) + v_(n/2)) / 2 as keys -> the two central keys.
 __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], int n, unsigned kmin, unsigned kmax, int* s_red,
-                                                int& par, unsigned* s_list, int* s_cnt, unsigned& k1, unsigned& k2) {
+                                                int& par, int& it, unsigned* s_list, int* s_cnt, unsigned& k1, unsigned& k2) {
     const int r = (n - 1) >> 1;
-    k1 = bg_select(key, r, n, kmin, kmax, s_red, par, s_list, s_cnt);
+    k1 = bg_select(key, r, n, kmin, kmax, s_red, par, it, s_list, s_cnt);
     k2 = k1;
     if ((n & 1) == 0) {                             // rank r + 1: k1 again if it repeats, else the next larger key
         int c = 0;
@@ -154,7 +167,7 @@ __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], i
             c += (key[i] <= k1) ? 1 : 0;
             if (key[i] > k1) nxt = min(nxt, key[i]);
         }
-        c = bg_block_sum(c, s_red, par);
+        c = bg_block_sum(c, s_red, par, it);
         nxt = bg_block_min(nxt, s_red, par);
         if (r + 1 >= c) k2 = nxt;
     }
@@ -165,9 +178,11 @@ template <bool FUSED>
 __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W, int H, int B, int GX, int n_min,
                                                               float* __restrict__ med_out, float* __restrict__ sig_out,
                                                               int* __restrict__ ngood_out) {
-    __shared__ __align__(16) int s_red[16];
+    __shared__ __align__(16) int s_red[20];
     __shared__ unsigned s_list[BG_FINISH + 1];
     __shared__ int s_cnt;
+    if (threadIdx.x < 3) s_red[16 + threadIdx.x] = 0;
+    __syncthreads();
     const int cell = blockIdx.x, gx = cell % GX, gy = cell / GX;
     const int x0 = gx * B, y0 = gy * B, x_end = min(x0 + B, W), y_end = min(y0 + B, H);
     const int col = (threadIdx.x & 15) * 4, row = threadIdx.x >> 4;
@@ -179,7 +194,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
 #pragma unroll
         for (int i = 0; i < 4; ++i) key[4 * j + i] = bg_key(v[i]);
     }
-    int par = 0;
+    int par = 0, it = 0;
     int n = 0;
     unsigned lo = BG_SENTINEL, hi = 0u;
 #pragma unroll
@@ -189,7 +204,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
         lo = min(lo, key[i]);
         hi = max(hi, ok ? key[i] : 0u);
     }
-    n = bg_block_sum(n, s_red, par);
+    n = bg_block_sum(n, s_red, par, it);
     if (n < max(n_min, 1)) {
         if (threadIdx.x == 0) { med_out[cell] = 0.f; sig_out[cell] = 0.f; ngood_out[cell] = n; }
         return;
@@ -197,7 +212,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
     lo = bg_block_min(lo, s_red, par);
     hi = bg_block_max_valid(hi, s_red, par);
     unsigned k1, k2;
-    bg_central_pair(key, n, lo, hi, s_red, par, s_list, &s_cnt, k1, k2);
+    bg_central_pair(key, n, lo, hi, s_red, par, it, s_list, &s_cnt, k1, k2);
     const float med = 0.5f * (bg_unkey(k1) + bg_unkey(k2));
     // MAD: |v - med| >= 0, whose bit patterns are already ordered
     lo = BG_SENTINEL; hi = 0u;
@@ -211,7 +226,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
     }
     lo = bg_block_min(lo, s_red, par);
     hi = bg_block_max_valid(hi, s_red, par);
-    bg_central_pair(key, n, lo, hi, s_red, par, s_list, &s_cnt, k1, k2);
+    bg_central_pair(key, n, lo, hi, s_red, par, it, s_list, &s_cnt, k1, k2);
     const float mad = 0.5f * (__uint_as_float(k1) + __uint_as_float(k2));
     if (threadIdx.x == 0) { med_out[cell] = med; sig_out[cell] = BG_MAD_TO_SIGMA * mad; ngood_out[cell] = n; }
 }
@@ -247,8 +262,7 @@ __global__ void __launch_bounds__(128) bg_filter_kernel(const float* __restrict_
 #define DET_TW 64
 #define DET_TH 32
 #define DET_PITCH 66                 // 64 + 2 apron columns; 66 mod 32 = 2 spreads a warp's four rows over the banks
-#define DET_PROWS 8                  // node patch: (DET_TH + 2) / 8 + 2 rows, (DET_TW + 2) / 8 + 2 columns at B = 8
-#define DET_PCOLS 12
+#define DET_PCOLS 12                 // node columns a tile can touch: (DET_TW + 2) / 8 + 2 at B = 8
 
 struct DetGrid {
     const float* bkg;
@@ -264,50 +278,38 @@ __device__ __forceinline__ void det_node(int p, const DetGrid& g, int G, int& g0
     g0 = min((int)u, max(G - 2, 0));
     t = u - (float)g0;
 }
-__device__ __forceinline__ float det_interp(const float (*patch)[DET_PCOLS], int lx, int ly, int lx1, int ly1, float tx, float ty) {
-    const float top = fmaf(tx, patch[ly][lx1] - patch[ly][lx], patch[ly][lx]);
-    const float bot = fmaf(tx, patch[ly1][lx1] - patch[ly1][lx], patch[ly1][lx]);
-    return fmaf(ty, bot - top, top);
-}
-
 // R-D4 / R-D5 on one 64 x 32 tile.  tile_info[tile] = (base of the tile's records in tmp, count); *total counts all.
-// Staging: the node patch is interpolated along y once per tile row (s_rb / s_rn), the x node and fraction of every
-// tile column are tabulated (s_col), so a pixel's background costs two shared loads and one FMA.
+// Staging: the grids are interpolated along y once per tile row (s_rb / s_rn, straight from the L2-resident grids), the
+// x node and fraction of every tile column are tabulated (s_col): a pixel's background costs two shared loads + one FMA.
 template <bool FUSED>
-__global__ void __launch_bounds__(256, 3) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
+__global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
                                                            ArgusSourceRec* __restrict__ tmp, unsigned capacity,
                                                            uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
     __shared__ float s_s[(DET_TH + 2) * DET_PITCH];
-    __shared__ float s_b[DET_PROWS][DET_PCOLS], s_n[DET_PROWS][DET_PCOLS];
     __shared__ float s_rb[DET_TH + 2][DET_PCOLS], s_rn[DET_TH + 2][DET_PCOLS];
     __shared__ float2 s_col[DET_PITCH];              // (.x: node offsets lx | lx1 << 8 as int bits, .y: tx)
     __shared__ int s_warp[8];
     __shared__ unsigned s_base;
     const int tile = blockIdx.x, x0 = (tile % tiles_x) * DET_TW, y0 = (tile / tiles_x) * DET_TH, tid = threadIdx.x;
-    int pgx, pgy;
+    int pgx;
     float tdummy;
     det_node(x0 - 1, g, g.GX, pgx, tdummy);
-    det_node(y0 - 1, g, g.GY, pgy, tdummy);
-    if (tid < DET_PROWS * DET_PCOLS) {
-        const int r = tid / DET_PCOLS, c = tid % DET_PCOLS;
-        const int q = min(pgy + r, g.GY - 1) * g.GX + min(pgx + c, g.GX - 1);
-        s_b[r][c] = __ldg(g.bkg + q);
-        s_n[r][c] = __ldg(g.nse + q);
-    } else if (tid >= 128 && tid < 128 + DET_PITCH) {
-        int gx0;
-        float tx;
-        det_node(x0 - 1 + (tid - 128), g, g.GX, gx0, tx);
-        s_col[tid - 128] = make_float2(__int_as_float((gx0 - pgx) | ((min(gx0 + 1, g.GX - 1) - pgx) << 8)), tx);
-    }
-    __syncthreads();
+    // tables straight from the (L2-resident) grids: y-interpolated node rows and the per-column (node, fraction)
     for (int e = tid; e < (DET_TH + 2) * DET_PCOLS; e += 256) {
         const int r = e / DET_PCOLS, c = e - r * DET_PCOLS;
         int gy0;
         float ty;
         det_node(y0 - 1 + r, g, g.GY, gy0, ty);
-        const int ly = gy0 - pgy, ly1 = min(gy0 + 1, g.GY - 1) - pgy;
-        s_rb[r][c] = fmaf(ty, s_b[ly1][c] - s_b[ly][c], s_b[ly][c]);
-        s_rn[r][c] = fmaf(ty, s_n[ly1][c] - s_n[ly][c], s_n[ly][c]);
+        const int col = min(pgx + c, g.GX - 1), q0 = gy0 * g.GX + col, q1 = min(gy0 + 1, g.GY - 1) * g.GX + col;
+        const float b0 = __ldg(g.bkg + q0), b1 = __ldg(g.bkg + q1), n0 = __ldg(g.nse + q0), n1 = __ldg(g.nse + q1);
+        s_rb[r][c] = fmaf(ty, b1 - b0, b0);
+        s_rn[r][c] = fmaf(ty, n1 - n0, n0);
+    }
+    if (tid >= 128 && tid < 128 + DET_PITCH) {
+        int gx0;
+        float tx;
+        det_node(x0 - 1 + (tid - 128), g, g.GX, gx0, tx);
+        s_col[tid - 128] = make_float2(__int_as_float((gx0 - pgx) | ((min(gx0 + 1, g.GX - 1) - pgx) << 8)), tx);
     }
     __syncthreads();
     const float ninf = __int_as_float(0xff800000);   // -inf: masked and off-frame pixels never win, never count
@@ -348,9 +350,14 @@ __global__ void __launch_bounds__(256, 3) det_tiles_kernel(FrameArgs f, int W, i
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
         const float c = w[1][j + 1];
-        bool ok = c > 0.f;                               // also false for -inf
-        ok = ok && c > w[0][j] && c > w[0][j + 1] && c > w[0][j + 2] && c > w[1][j];
-        ok = ok && c >= w[1][j + 2] && c >= w[2][j] && c >= w[2][j + 1] && c >= w[2][j + 2];
+        // cheap necessary condition first (c >= all eight neighbours), the raster-first tie rule only for survivors
+        const float m8 = fmaxf(fmaxf(fmaxf(w[0][j], w[0][j + 1]), fmaxf(w[0][j + 2], w[1][j])),
+                               fmaxf(fmaxf(w[1][j + 2], w[2][j]), fmaxf(w[2][j + 1], w[2][j + 2])));
+        bool ok = c > 0.f && c >= m8;                    // false for -inf
+        if (ok) {
+            const float e4 = fmaxf(fmaxf(w[0][j], w[0][j + 1]), fmaxf(w[0][j + 2], w[1][j]));
+            ok = c > e4;
+        }
         if (ok) {
             const float2 ci = s_col[cx0 + j + 1];
             const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;

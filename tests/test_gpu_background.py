@@ -212,3 +212,18 @@ def test_undefined_background_suppresses_detection(argus, ctx):
     assert np.isinf(g["nse"][:, 3]).all() and np.isfinite(g["nse"][:, :3]).all() and np.all(g["bkg"][:, 3] == 0)
     rec = gpu_detect(argus, ctx, 64, 32, 16, 5.0, g["dev"]["bkg"], g["dev"]["nse"], fr)
     assert list(zip(rec["y"].tolist(), rec["x"].tolist())) == [(8, 8)]
+
+
+def test_config1_full_frame_fused(argus, ctx):
+    """BASELINE configs[1] at full size, in the configuration bench.py --workload detect times (cell 64, n_min 16,
+    5 sigma, fused calibration): every cell of the grids and the whole catalogue against the oracle."""
+    fr = synth.config1()
+    H, W = fr.shape
+    cal, mask = oracle.calibrate_frame(fr)
+    d = upload(fr)
+    g = gpu_background(argus, ctx, W, H, 64, 16, d)
+    bkg, nse = compare_grids(g, cal, mask, 64, 16, exact=False)
+    rec = gpu_detect(argus, ctx, W, H, 64, 5.0, g["dev"]["bkg"], g["dev"]["nse"], d, cap=1 << 18)
+    n_must, n_amb = compare_catalogue(rec, cal, mask, bkg, nse, W, 64, 5.0, max_ambiguous=40)
+    print("config1 detect: %d records, %d clear sources, %d ambiguous decisions" % (rec.size, n_must, n_amb))
+    assert n_must > 20000
