@@ -5,9 +5,10 @@
 //
 //   bg_cells_kernel    one CTA per B x B cell (B <= 64): the cell's pixels live in registers (16 per thread) as
 //                      order-preserving 32-bit keys; the two central order statistics are found EXACTLY by a
-//                      bitwise bisection on the key (count of keys below a candidate, one CTA-wide sum per bit),
-//                      started below the common prefix of the cell's min and max and finished by ranking the
-//                      survivors once 32 or fewer remain.  Same again on |v - med| for the MAD noise estimate.
+//                      multi-level counting select (256-bin shared histogram over the live key range, CTA-wide
+//                      scan, descend into the bin that holds the rank: 8 bits per level), started at the common
+//                      prefix of the cell's min and max and finished by ranking the survivors once 32 or fewer
+//                      remain.  Same again on |v - med| for the MAD noise estimate.
 //   bg_filter_kernel   3x3 median over the valid cells of the grid (one thread per cell).
 //   det_tiles_kernel   one CTA per 64 x 32-pixel tile: s = cal - bkg(x, y) for the tile + 1-pixel apron in shared
 //                      memory, thresholded raster-first local maxima, 3x3 flux and centroid; records go to a
@@ -82,12 +83,6 @@ __device__ __forceinline__ int bg_block_sum(int v, int* s_red, int& par, int& it
     it = nxt;
     return r;
 }
-// #{key < cand} added to c.  The compare runs on the ALU pipe; the increment is written as c = one * one + c with a
-// run-time `one` (blockDim.x / 256) so that it is an IMAD on the FMA pipe: both pipes issue one warp instruction
-// per two cycles per SM sub-partition, and a compare + integer add pair would queue both on the ALU pipe.
-__device__ __forceinline__ void bg_count_lt(int& c, unsigned key, unsigned cand, int one) {
-    asm("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %1, %2;\n\t@p mad.lo.s32 %0, %3, %3, %0;\n\t}" : "+r"(c) : "r"(key), "r"(cand), "r"(one));
-}
 __device__ __forceinline__ unsigned bg_block_min(unsigned v, int* s_red, int& par) {
     v = __reduce_min_sync(0xffffffffu, v);
     unsigned* r = reinterpret_cast<unsigned*>(s_red + par * 8);
@@ -108,39 +103,62 @@ __device__ __forceinline__ unsigned bg_block_max_valid(unsigned v, int* s_red, i
 }
 
 // k-th smallest (0-based, k < n) of the n non-sentinel keys held by the CTA (BG_KPT per thread); kmin / kmax are
-// their extremes.  Bitwise bisection: the answer is the largest v with #{key < v} <= k; bits above the highest
-// bit in which kmin and kmax differ are common to every key.  s_list: 33 words, s_cnt: 1 word of shared memory.
+// their extremes.  Multi-level counting select: the live key range [lo, hi] is cut into <= 256 equal bins (width a
+// power of two), the keys inside it are counted into a shared histogram, a CTA-wide scan finds the bin that holds
+// rank k, and that bin becomes the new range -- 8 bits per level, the first level starting at the common prefix
+// of kmin and kmax.  Once <= BG_FINISH keys remain they are ranked directly in one warp.  Exact.
+// s_hist: 256 + 12 words, s_list: BG_FINISH + 1 words, s_cnt: 1 word of shared memory.
 __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned kmin, unsigned kmax,
-                                              int* s_red, int& par, int& it, unsigned* s_list, int* s_cnt) {
-    if (kmin == kmax) return kmin;
-    int bit = 31 - __clz(kmin ^ kmax);
-    unsigned prefix = (bit == 31) ? 0u : ((kmax >> (bit + 1)) << (bit + 1));
-    int c_lo = 0, c_hi = n;                        // #{key < prefix}, #{key <= prefix | low bits}
-    while (bit >= 0 && c_hi - c_lo > BG_FINISH) {
-        const unsigned cand = prefix | (1u << bit);
-        int c = 0, c2 = 0;
-        const int one = (int)(blockDim.x >> 8);
+                                              int* s_hist, unsigned* s_list, int* s_cnt) {
+    unsigned lo = kmin, hi = kmax;
+    int c_lo = 0, cnt = n;                          // #{key < lo}, #{lo <= key <= hi}
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int* s_w = s_hist + 256;                        // [0..7] warp totals, [8..10] picked bin, its prefix, its count
+    while (cnt > BG_FINISH && hi > lo) {
+        const int sh = max(0, 24 - __clz(hi - lo)); // (hi - lo) >> sh <= 255
+        s_hist[tid] = 0;
+        __syncthreads();
+        const unsigned span = hi - lo;
 #pragma unroll
-        for (int i = 0; i < BG_KPT; i += 2) { bg_count_lt(c, key[i], cand, one); bg_count_lt(c2, key[i + 1], cand, one); }
-        c += c2;
-        c = bg_block_sum(c, s_red, par, it);
-        if (c <= k) { prefix = cand; c_lo = c; } else c_hi = c;
-        --bit;
+        for (int i = 0; i < BG_KPT; ++i) {
+            const unsigned d = key[i] - lo;             // wraps to a huge value below lo: one compare covers both ends
+            if (d <= span) atomicAdd(s_hist + (d >> sh), 1);
+        }
+        __syncthreads();
+        const int h = s_hist[tid];
+        int inc = h;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += o;
+        }
+        if (lane == 31) s_w[wid] = inc;
+        __syncthreads();
+#pragma unroll
+        for (int w = 0; w < 7; ++w) inc += (w < wid) ? s_w[w] : 0;
+        const int krel = k - c_lo;
+        if (inc - h <= krel && krel < inc) { s_w[8] = tid; s_w[9] = inc - h; s_w[10] = h; }
+        __syncthreads();
+        const unsigned bin = (unsigned)s_w[8];
+        c_lo += s_w[9];
+        cnt = s_w[10];
+        lo += bin << sh;
+        const unsigned top = lo + ((1u << sh) - 1u);
+        hi = (top < lo) ? hi : min(hi, top);          // top < lo: wrapped past 2^32
     }
-    if (bit < 0) return prefix;
-    // at most BG_FINISH keys remain in [prefix, prefix | mask]: rank them directly (ties by list position)
-    const unsigned upper = prefix | ((2u << bit) - 1u);
-    if (threadIdx.x == 0) *s_cnt = 0;
+    if (hi == lo) return lo;
+    // at most BG_FINISH keys remain in [lo, hi]: rank them directly (ties by list position)
+    if (tid == 0) *s_cnt = 0;
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < BG_KPT; ++i)
-        if (key[i] >= prefix && key[i] <= upper && key[i] != BG_SENTINEL) {
+        if (key[i] >= lo && key[i] <= hi) {
             int p = atomicAdd(s_cnt, 1);
             if (p < BG_FINISH) s_list[p] = key[i];
         }
     __syncthreads();
-    if (threadIdx.x < 32) {
-        const int m = min(*s_cnt, BG_FINISH), lane = threadIdx.x;
+    if (tid < 32) {
+        const int m = min(*s_cnt, BG_FINISH);
         const unsigned mine = (lane < m) ? s_list[lane] : BG_SENTINEL;
         int rank = 0;
         for (int j = 0; j < m; ++j) {
@@ -155,9 +173,10 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
 
 // median rule of R-D1: (v_((n-1)/2) + v_(n/2)) / 2 as keys -> the two central keys.
 __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], int n, unsigned kmin, unsigned kmax, int* s_red,
-                                                int& par, int& it, unsigned* s_list, int* s_cnt, unsigned& k1, unsigned& k2) {
+                                                int& par, int& it, int* s_hist, unsigned* s_list, int* s_cnt, unsigned& k1,
+                                                unsigned& k2) {
     const int r = (n - 1) >> 1;
-    k1 = bg_select(key, r, n, kmin, kmax, s_red, par, it, s_list, s_cnt);
+    k1 = bg_select(key, r, n, kmin, kmax, s_hist, s_list, s_cnt);
     k2 = k1;
     if ((n & 1) == 0) {                             // rank r + 1: k1 again if it repeats, else the next larger key
         int c = 0;
@@ -180,6 +199,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
                                                               int* __restrict__ ngood_out) {
     __shared__ __align__(16) int s_red[20];
     __shared__ unsigned s_list[BG_FINISH + 1];
+    __shared__ int s_hist[256 + 12];
     __shared__ int s_cnt;
     if (threadIdx.x < 3) s_red[16 + threadIdx.x] = 0;
     __syncthreads();
@@ -212,7 +232,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
     lo = bg_block_min(lo, s_red, par);
     hi = bg_block_max_valid(hi, s_red, par);
     unsigned k1, k2;
-    bg_central_pair(key, n, lo, hi, s_red, par, it, s_list, &s_cnt, k1, k2);
+    bg_central_pair(key, n, lo, hi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
     const float med = 0.5f * (bg_unkey(k1) + bg_unkey(k2));
     // MAD: |v - med| >= 0, whose bit patterns are already ordered
     lo = BG_SENTINEL; hi = 0u;
@@ -226,7 +246,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
     }
     lo = bg_block_min(lo, s_red, par);
     hi = bg_block_max_valid(hi, s_red, par);
-    bg_central_pair(key, n, lo, hi, s_red, par, it, s_list, &s_cnt, k1, k2);
+    bg_central_pair(key, n, lo, hi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
     const float mad = 0.5f * (__uint_as_float(k1) + __uint_as_float(k2));
     if (threadIdx.x == 0) { med_out[cell] = med; sig_out[cell] = BG_MAD_TO_SIGMA * mad; ngood_out[cell] = n; }
 }
