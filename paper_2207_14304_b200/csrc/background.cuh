@@ -314,9 +314,14 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
     int pgx;
     float tdummy;
     det_node(x0 - 1, g, g.GX, pgx, tdummy);
-    // tables straight from the (L2-resident) grids: y-interpolated node rows and the per-column (node, fraction)
-    for (int e = tid; e < (DET_TH + 2) * DET_PCOLS; e += 256) {
-        const int r = e / DET_PCOLS, c = e - r * DET_PCOLS;
+    // tables straight from the (L2-resident) grids: y-interpolated node rows and the per-column (node, fraction).
+    // Only the node columns the tile touches are built (3 at cell 64, 11 at cell 8).
+    int pgx1;
+    det_node(x0 + DET_TW, g, g.GX, pgx1, tdummy);
+    const int ncols = min(pgx1 + 1, g.GX - 1) - pgx + 1;
+    const float inv_ncols = 1.0f / (float)ncols;
+    for (int e = tid; e < (DET_TH + 2) * ncols; e += 256) {
+        const int r = (int)(((float)e + 0.5f) * inv_ncols), c = e - r * ncols;   // exact: e < 2^10, ncols <= 12
         int gy0;
         float ty;
         det_node(y0 - 1 + r, g, g.GY, gy0, ty);
@@ -442,40 +447,69 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
     }
 }
 
-// Exclusive scan of the tile counts in tile order; *n_dev (may be NULL) and ctl[1] receive the total.
+// Exclusive scan of the tile counts in tile order; *n_dev (may be NULL) and ctl[1] receive the total.  One CTA of
+// 1024 threads; 16 x 1024 tiles per round: every thread loads its (coalesced) element of all 16 chunks at once, scans
+// each within its warp, the 16 x 32 warp totals are scanned once by the whole CTA -- five barriers per round instead
+// of four per chunk (a 61-MPix frame has 30 000 tiles: two rounds).
 __global__ void __launch_bounds__(1024) det_scan_kernel(const uint2* __restrict__ tile_info, int n_tiles,
                                                         unsigned* __restrict__ offsets, unsigned* __restrict__ ctl,
                                                         long long* __restrict__ n_dev) {
+    constexpr int NB = 16;                            // chunks of 1024 tiles per round
+    __shared__ unsigned s_tot[1024];                  // [chunk][warp] inclusive warp totals -> exclusive prefixes (NB * 32 used)
     __shared__ unsigned s_w[32];
     __shared__ unsigned s_carry;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     if (tid == 0) s_carry = 0;
     __syncthreads();
-    for (int b = 0; b < n_tiles; b += 1024) {
-        const int i = b + tid;
-        const unsigned c = i < n_tiles ? tile_info[i].y : 0u;
-        unsigned inc = c;
+    for (int base = 0; base < n_tiles; base += NB * 1024) {
+        unsigned exc[NB];                              // exclusive prefix inside the warp
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
-            if (lane >= d) inc += o;
+        for (int b = 0; b < NB; ++b) {
+            const int i = base + b * 1024 + tid;
+            exc[b] = i < n_tiles ? tile_info[i].y : 0u;
         }
-        if (lane == 31) s_w[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            unsigned v = s_w[lane], x = v;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            unsigned x = exc[b];
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
-                unsigned o = __shfl_up_sync(0xffffffffu, x, d);
+                const unsigned o = __shfl_up_sync(0xffffffffu, x, d);
                 if (lane >= d) x += o;
             }
-            s_w[lane] = x - v;
+            if (lane == 31) s_tot[b * 32 + wid] = x;
+            exc[b] = x - exc[b];
+        }
+        __syncthreads();
+        // scan the 1024 warp totals in (chunk, warp) order: thread t owns total t
+        const unsigned t = tid < NB * 32 ? s_tot[tid] : 0u;
+        unsigned x = t;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, x, d);
+            if (lane >= d) x += o;
+        }
+        if (lane == 31) s_w[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            const unsigned v = s_w[lane];
+            unsigned y = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned o = __shfl_up_sync(0xffffffffu, y, d);
+                if (lane >= d) y += o;
+            }
+            s_w[lane] = y - v;
         }
         __syncthreads();
         const unsigned carry = s_carry;
-        if (i < n_tiles) offsets[i] = carry + s_w[wid] + inc - c;
+        s_tot[tid] = carry + s_w[wid] + x - t;        // exclusive prefix of (chunk, warp) total `tid`
         __syncthreads();
-        if (tid == 1023) s_carry = carry + s_w[31] + inc;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int i = base + b * 1024 + tid;
+            if (i < n_tiles) offsets[i] = s_tot[b * 32 + wid] + exc[b];
+        }
+        if (tid == 1023) s_carry = carry + s_w[31] + x;
         __syncthreads();
     }
     if (tid == 0) {
