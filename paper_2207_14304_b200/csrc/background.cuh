@@ -309,7 +309,9 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
     __shared__ float s_rb[DET_TH + 2][DET_PCOLS], s_rn[DET_TH + 2][DET_PCOLS];
     __shared__ float2 s_col[DET_PITCH];              // (.x: node offsets lx | lx1 << 8 as int bits, .y: tx)
     __shared__ int s_warp[8];
-    __shared__ unsigned s_base;
+    __shared__ unsigned s_base, s_nmin;              // s_nmin: bits of the smallest noise node the tile touches
+    if (threadIdx.x == 0) s_nmin = 0x7f800000u;
+    __syncthreads();
     const int tile = blockIdx.x, x0 = (tile % tiles_x) * DET_TW, y0 = (tile / tiles_x) * DET_TH, tid = threadIdx.x;
     int pgx;
     float tdummy;
@@ -320,6 +322,7 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
     det_node(x0 + DET_TW, g, g.GX, pgx1, tdummy);
     const int ncols = min(pgx1 + 1, g.GX - 1) - pgx + 1;
     const float inv_ncols = 1.0f / (float)ncols;
+    float nmin = __int_as_float(0x7f800000);
     for (int e = tid; e < (DET_TH + 2) * ncols; e += 256) {
         const int r = (int)(((float)e + 0.5f) * inv_ncols), c = e - r * ncols;   // exact: e < 2^10, ncols <= 12
         int gy0;
@@ -329,6 +332,11 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
         const float b0 = __ldg(g.bkg + q0), b1 = __ldg(g.bkg + q1), n0 = __ldg(g.nse + q0), n1 = __ldg(g.nse + q1);
         s_rb[r][c] = fmaf(ty, b1 - b0, b0);
         s_rn[r][c] = fmaf(ty, n1 - n0, n0);
+        nmin = fminf(nmin, fminf(n0, n1));
+    }
+    {   // noise nodes are >= 0 or +inf: their bit patterns order like the values
+        const unsigned m = __reduce_min_sync(0xffffffffu, __float_as_uint(nmin));
+        if ((tid & 31) == 0 && m != 0x7f800000u) atomicMin(&s_nmin, m);
     }
     if (tid >= 128 && tid < 128 + DET_PITCH) {
         int gx0;
@@ -363,34 +371,29 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
         s_s[r * DET_PITCH + c] = (v == v) ? v - fmaf(ci.y, s_rb[r][lx1] - b0, b0) : ninf;
     }
     __syncthreads();
-    // each thread: 8 consecutive pixels of one row; 3 x 10 window in registers
+    // each thread: 8 consecutive pixels of one row.  Threshold first: every interpolated noise value of the tile is a
+    // convex combination of the nodes it touches, so s > k * (smallest node) is necessary -- one compare per pixel
+    // rejects all but ~1e-3 of them; only the survivors look at their neighbours and at the exact threshold.
     const int ry = tid >> 3, cx0 = (tid & 7) * 8;
-    float w[3][10];
-#pragma unroll
-    for (int r = 0; r < 3; ++r)
-#pragma unroll
-        for (int c = 0; c < 10; ++c) w[r][c] = s_s[(ry + r) * DET_PITCH + cx0 + c];
+    const float thr_min = 0.999999f * (g.k_sigma * __uint_as_float(s_nmin));   // slack for the rounding of the lerp
+    const float* row = s_s + (ry + 1) * DET_PITCH + cx0 + 1;
     unsigned bits = 0;
     const int py = y0 + ry;
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-        const float c = w[1][j + 1];
-        // cheap necessary condition first (c >= all eight neighbours), the raster-first tie rule only for survivors
-        const float m8 = fmaxf(fmaxf(fmaxf(w[0][j], w[0][j + 1]), fmaxf(w[0][j + 2], w[1][j])),
-                               fmaxf(fmaxf(w[1][j + 2], w[2][j]), fmaxf(w[2][j + 1], w[2][j + 2])));
-        bool ok = c > 0.f && c >= m8;                    // false for -inf
-        if (ok) {
-            const float e4 = fmaxf(fmaxf(w[0][j], w[0][j + 1]), fmaxf(w[0][j + 2], w[1][j]));
-            ok = c > e4;
+        const float c = row[j];
+        if (c > thr_min && c > 0.f) {                    // false for -inf (masked, off-frame) and for thr_min NaN
+            const float* q = row + j;
+            const float e4 = fmaxf(fmaxf(q[-DET_PITCH - 1], q[-DET_PITCH]), fmaxf(q[-DET_PITCH + 1], q[-1]));
+            const float l4 = fmaxf(fmaxf(q[1], q[DET_PITCH - 1]), fmaxf(q[DET_PITCH], q[DET_PITCH + 1]));
+            if (c > e4 && c >= l4) {                     // raster-first pixel wins ties
+                const float2 ci = s_col[cx0 + j + 1];
+                const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
+                const float n0 = s_rn[ry + 1][lx];
+                const float nse = fmaf(ci.y, s_rn[ry + 1][lx1] - n0, n0);
+                if (c > g.k_sigma * nse) bits |= 1u << j;   // false for nse = +inf or NaN (undefined background)
+            }
         }
-        if (ok) {
-            const float2 ci = s_col[cx0 + j + 1];
-            const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
-            const float n0 = s_rn[ry + 1][lx];
-            const float nse = fmaf(ci.y, s_rn[ry + 1][lx1] - n0, n0);
-            ok = c > g.k_sigma * nse;                    // false for nse = +inf or NaN (undefined background)
-        }
-        bits |= ok ? (1u << j) : 0u;
     }
     // CTA-wide exclusive scan of the per-thread counts (thread order = raster order inside the tile)
     const int cnt = __popc(bits), lane = tid & 31, wid = tid >> 5;
@@ -425,7 +428,7 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
         for (int r = 0; r < 3; ++r)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float q = w[r][j + c];
+                const float q = row[j + (r - 1) * DET_PITCH + (c - 1)];
                 if (q != ninf) { flux += q; mx += q * (float)(c - 1); my += q * (float)(r - 1); }
             }
         const float2 ci = s_col[cx0 + j + 1];
@@ -433,7 +436,7 @@ __global__ void __launch_bounds__(256, 5) det_tiles_kernel(FrameArgs f, int W, i
         const float b0 = s_rb[ry + 1][lx], n0 = s_rn[ry + 1][lx];
         ArgusSourceRec rec;
         rec.x = x0 + cx0 + j; rec.y = py;
-        rec.peak = w[1][j + 1]; rec.flux = flux;
+        rec.peak = row[j]; rec.flux = flux;
         rec.cx = flux > 0.f ? mx / flux : 0.f;
         rec.cy = flux > 0.f ? my / flux : 0.f;
         rec.bkg = fmaf(ci.y, s_rb[ry + 1][lx1] - b0, b0);
