@@ -302,7 +302,7 @@ __device__ __forceinline__ void det_node(int p, const DetGrid& g, int G, int& g0
 // Staging: the grids are interpolated along y once per tile row (s_rb / s_rn, straight from the L2-resident grids), the
 // x node and fraction of every tile column are tabulated (s_col): a pixel's background costs two shared loads + one FMA.
 template <bool FUSED>
-__global__ void __launch_bounds__(256, 6) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
+__global__ void __launch_bounds__(256, 8) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
                                                            ArgusSourceRec* __restrict__ tmp, unsigned capacity,
                                                            uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
     __shared__ float s_s[(DET_TH + 2) * DET_PITCH];
