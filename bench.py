@@ -32,7 +32,7 @@ SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload reci
 # dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
 # profiles/r1_final_ncu_summary.txt (ncu --set full).
 NCU_TRAFFIC_BYTES = 983571968 + 339383296  # profiles/r1_final_ncu_summary.txt
-NCU_DET_TRAFFIC_BYTES = 856469504 + 4033792 + 856804096 + 4923392  # profiles/r1_detect_ncu_summary.txt
+NCU_DET_TRAFFIC_BYTES = 856468736 + 4660224 + 856615936 + 6127360  # profiles/r1_detect_ncu_summary.txt
 NCU_SEG_TRAFFIC_BYTES = 359159552 + 7175936 + 365523712 + 41991424  # profiles/r1_segments_ncu_summary.txt
 
 

@@ -57,6 +57,24 @@ def test_host_side_validation_without_device(lib):
     n.value = 77
     assert lib.argus_segment_products(None, 1 << 17, 1 << 14, None, None, None, 0, None, 0, None, None, None, None, None,
                                       None, 0, None, C.byref(n), None) == -1
+    # background map / source detection: NULL context before any CUDA call, count reset
+    assert lib.argus_background_map(None, None, 64, 64, 64, 16, None, None, None, None, None, None) == -1
+    n.value = 77
+    assert lib.argus_detect_sources(None, None, 64, 64, 64, None, None, C.c_float(5.0), None, 0, None, C.byref(n), None) == -1
+    assert n.value == 77                                      # a NULL context touches nothing
+
+
+def test_argus_source_record_layout_matches_binding():
+    """argus_source (argus.h) is 32 bytes: int32 x, y; float peak, flux, cx, cy, bkg, nse -- the binding's SOURCE_DTYPE."""
+    import numpy as np
+
+    from paper_2207_14304_b200.binding import SOURCE_DTYPE
+    dt = np.dtype(SOURCE_DTYPE)
+    assert dt.itemsize == 32 and dt.names == ("x", "y", "peak", "flux", "cx", "cy", "bkg", "nse")
+    text = open(os.path.join(ROOT, "include", "argus.h")).read()
+    body = text[text.index("typedef struct argus_source {"):text.index("} argus_source;")]
+    fields = [w.strip(" ,;") for line in body.splitlines()[1:] for w in line.split("/*")[0].replace("int32_t", "").replace("float", "").split(",")]
+    assert [f for f in fields if f] == list(dt.names)
 
 
 def test_no_cpu_fallback():
