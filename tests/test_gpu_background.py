@@ -227,3 +227,21 @@ def test_config1_full_frame_fused(argus, ctx):
     n_must, n_amb = compare_catalogue(rec, cal, mask, bkg, nse, W, 64, 5.0, max_ambiguous=40)
     print("config1 detect: %d records, %d clear sources, %d ambiguous decisions" % (rec.size, n_must, n_amb))
     assert n_must > 20000
+
+
+@pytest.mark.parametrize("B", [64, 8])
+def test_mixed_sign_values_zeros_and_duplicates(argus, ctx, B):
+    """Sky-subtracted frames straddle zero: the order-preserving keys must order negatives, -0.0, +0.0 and positives,
+    and heavy duplication (quantised values) must not break the counting select."""
+    rng = np.random.default_rng(77)
+    H, W = 192, 256
+    cal32 = np.round(rng.normal(0.0, 3.0, (H, W)) * 4.0).astype(np.float32) / 4.0      # quarter-ADU steps: many ties
+    cal32[::7, ::5] = -0.0
+    cal32[3::11, 2::9] = 0.0
+    cal32[100:103, 50:53] += 400.0
+    cal32[20, 200] = -5000.0                                                             # a negative outlier
+    mask = (rng.random((H, W)) > 0.01).astype(np.uint8)
+    g = gpu_background(argus, ctx, W, H, B, 4, _dev_cal(cal32, mask))
+    bkg, nse = compare_grids(g, cal32.astype(np.float64), mask, B, 4, exact=True)
+    rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
+    compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0, max_ambiguous=400)
