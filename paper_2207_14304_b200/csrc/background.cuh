@@ -107,9 +107,9 @@ __device__ __forceinline__ unsigned bg_block_max_valid(unsigned v, int* s_red, i
 // power of two), the keys inside it are counted into a shared histogram, a CTA-wide scan finds the bin that holds
 // rank k, and that bin becomes the new range -- 8 bits per level, the first level starting at the common prefix
 // of kmin and kmax.  Once <= BG_FINISH keys remain they are ranked directly in one warp.  Exact.
-// s_hist: 256 + 12 words, s_list: BG_FINISH + 1 words, s_cnt: 1 word of shared memory.
+// s_hist: 256 + 12 words, s_list: BG_FINISH + 2 words, s_cnt: 1 word of shared memory.
 __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned kmin, unsigned kmax,
-                                              int* s_hist, unsigned* s_list, int* s_cnt) {
+                                              int* s_hist, unsigned* s_list, int* s_cnt, unsigned& next, bool& have_next) {
     unsigned lo = kmin, hi = kmax;
     int c_lo = 0, cnt = n;                          // #{key < lo}, #{lo <= key <= hi}
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -146,7 +146,8 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
         const unsigned top = lo + ((1u << sh) - 1u);
         hi = (top < lo) ? hi : min(hi, top);          // top < lo: wrapped past 2^32
     }
-    if (hi == lo) return lo;
+    // `next` = the key of rank k + 1 when it lies in the same final range (have_next), for the even-n median
+    if (hi == lo) { have_next = (k - c_lo + 1 < cnt); next = lo; return lo; }
     // at most BG_FINISH keys remain in [lo, hi]: rank them directly (ties by list position)
     if (tid == 0) *s_cnt = 0;
     __syncthreads();
@@ -157,8 +158,8 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
             if (p < BG_FINISH) s_list[p] = key[i];
         }
     __syncthreads();
+    const int m = min(*s_cnt, BG_FINISH);           // read by every thread before the last barrier of this call
     if (tid < 32) {
-        const int m = min(*s_cnt, BG_FINISH);
         const unsigned mine = (lane < m) ? s_list[lane] : BG_SENTINEL;
         int rank = 0;
         for (int j = 0; j < m; ++j) {
@@ -166,8 +167,11 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
             rank += (kj < mine || (kj == mine && j < lane)) ? 1 : 0;
         }
         if (lane < m && rank == k - c_lo) s_list[BG_FINISH] = mine;
+        if (lane < m && rank == k - c_lo + 1) s_list[BG_FINISH + 1] = mine;
     }
     __syncthreads();
+    have_next = (k - c_lo + 1 < m);
+    next = s_list[BG_FINISH + 1];
     return s_list[BG_FINISH];
 }
 
@@ -176,19 +180,25 @@ __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], i
                                                 int& par, int& it, int* s_hist, unsigned* s_list, int* s_cnt, unsigned& k1,
                                                 unsigned& k2) {
     const int r = (n - 1) >> 1;
-    k1 = bg_select(key, r, n, kmin, kmax, s_hist, s_list, s_cnt);
+    unsigned nxt_sel;
+    bool have_next;
+    k1 = bg_select(key, r, n, kmin, kmax, s_hist, s_list, s_cnt, nxt_sel, have_next);
     k2 = k1;
-    if ((n & 1) == 0) {                             // rank r + 1: k1 again if it repeats, else the next larger key
-        int c = 0;
-        unsigned nxt = BG_SENTINEL;
+    if ((n & 1) == 0) {
+        if (have_next) {                            // rank r + 1 fell into the same final range (the usual case)
+            k2 = nxt_sel;
+        } else {                                    // k1 again if it repeats, else the next larger key
+            int c = 0;
+            unsigned nxt = BG_SENTINEL;
 #pragma unroll
-        for (int i = 0; i < BG_KPT; ++i) {
-            c += (key[i] <= k1) ? 1 : 0;
-            if (key[i] > k1) nxt = min(nxt, key[i]);
+            for (int i = 0; i < BG_KPT; ++i) {
+                c += (key[i] <= k1) ? 1 : 0;
+                if (key[i] > k1) nxt = min(nxt, key[i]);
+            }
+            c = bg_block_sum(c, s_red, par, it);
+            nxt = bg_block_min(nxt, s_red, par);
+            if (r + 1 >= c) k2 = nxt;
         }
-        c = bg_block_sum(c, s_red, par, it);
-        nxt = bg_block_min(nxt, s_red, par);
-        if (r + 1 >= c) k2 = nxt;
     }
 }
 
@@ -198,7 +208,7 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
                                                               float* __restrict__ med_out, float* __restrict__ sig_out,
                                                               int* __restrict__ ngood_out) {
     __shared__ __align__(16) int s_red[20];
-    __shared__ unsigned s_list[BG_FINISH + 1];
+    __shared__ unsigned s_list[BG_FINISH + 2];
     __shared__ int s_hist[256 + 12];
     __shared__ int s_cnt;
     if (threadIdx.x < 3) s_red[16 + threadIdx.x] = 0;
