@@ -25,7 +25,11 @@
  *     stream waits for it by event: outputs are complete in the caller's stream order exactly as without it.
  *   - Pixel convention: 0-based, pixel centres at integers, frame[y*W + x], x <-> FITS axis 1,
  *     crpix 0-based.  HEALPix: NESTED scheme, nside a power of two, 32 <= nside <= 2^29; sky
- *     convention alpha = phi, delta = pi/2 - theta (ICRS).
+ *     convention alpha = phi, delta = pi/2 - theta (ICRS).  (Lower bound: the unit of work of the plan and of
+ *     every resample kernel is a tile of 32 x 32 pixels of one base face = 1024 consecutive nested indices,
+ *     which does not exist below nside 32 -- a whole sky of at most 3072 pixels, far from the paper's
+ *     NSIDE-256 tiles of 1.38 arcsec pixels.  argus_resample with an explicit idx list has no
+ *     such unit but keeps the same bound for uniformity.)
  *   - Footprint domain: a HEALPix pixel belongs to the frame footprint iff its centre maps to
  *     -0.5 <= x < W-0.5, -0.5 <= y < H-0.5 and lies within rho_max of CRVAL,
  *     rho_max = atan(1.25 * scale * hypot(W,H)/2), scale = sqrt|det CD|.
@@ -128,10 +132,14 @@ const char* argus_strerror(int status);
 int argus_version(void);
 
 /* Context: owns scratch only -- three sets of plan buffers (tile records, masks, prefix sums, counters; about
- * 560 bytes per tile each, 290 MB per set at the default), two internal high-priority streams and events for
- * ARGUS_OPT_PLAN_OVERLAP -- sized for frames of up to max_tiles candidate output tiles (0 = default 1<<19: a 61-MPix
- * frame needs 5.3e4 at nside 2^17 and 1.95e5 at nside 2^18; valid range 64 .. 2^24).  device = CUDA ordinal.
- * Synchronous.  A context is not thread-safe: use one per host thread (contexts are independent). */
+ * 560 bytes per candidate output tile each), two internal high-priority streams and events for ARGUS_OPT_PLAN_OVERLAP.
+ *   max_tiles = 0 (default): the sets are sized from (W, H, nside, pixel scale) by the first call that plans a frame
+ *               (1.5 x the frame's area in 32 x 32-pixel tiles + margin: 3 x 48 MB for a 61-MPix frame at nside 2^17,
+ *               which has 5.3e4 candidate tiles; 1.95e5 at nside 2^18) and grown -- which synchronises the device --
+ *               when a later frame needs more; never shrunk.
+ *   max_tiles in 64 .. 2^24: allocated now, fixed; a frame with more candidate tiles reports ARGUS_ERR_CAPACITY.
+ * device = CUDA ordinal.  Synchronous.  A context is not thread-safe: use one per host thread (contexts are
+ * independent). */
 int argus_ctx_create(argus_ctx** ctx, int device, int64_t max_tiles);
 int argus_ctx_destroy(argus_ctx* ctx);
 int argus_ctx_set_option(argus_ctx* ctx, int option, int64_t value);
@@ -185,7 +193,13 @@ int argus_resample(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wc
 int argus_resample_host(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
                         int64_t nside, int kernel, float w_min, size_t n, float* value_host, float* weight_host,
                         void* stream);
-/* Blocks until every upload and download enqueued by argus_resample_host has completed. */
+/* A2-A6 fused with the raw frame in HOST memory (frame->raw as for argus_resample_host; masters, layout, sum and wsum
+ * are DEVICE pointers as for argus_resample_coadd): the upload of frame k+1 overlaps the kernels of frame k (two device
+ * staging buffers, the library's upload stream).  The accumulation is ordered on `stream`. */
+int argus_resample_coadd_host(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                              int64_t nside, int kernel, float w_min, const argus_coadd* layout, float* sum, float* wsum,
+                              int64_t* n_skipped_dev, void* stream);
+/* Blocks until every upload and download enqueued by argus_resample_host / argus_resample_coadd_host has completed. */
 int argus_host_wait(argus_ctx* ctx);
 
 /* A6: sum[slot(idx[i])] += weight[i] * value[i]; wsum[slot] += weight[i] for i < n.  idx must hold
@@ -265,20 +279,22 @@ typedef struct argus_source {
  * outermost centres).  Pixel p is a source iff it is good, s_p > k_sigma * nse(p), s_p > 0, and s_p is the maximum of
  * its good in-frame 8-neighbours (s_p > s_q for q before p in raster order, s_p >= s_q for q after p).  Pixels whose
  * interpolation touches a cell with nse = +inf are never sources.
- *   out       DEVICE argus_source[capacity], 16-byte aligned.  Catalogue order (deterministic): by 64 x 32-pixel tile
- *             ((y / 32) * ceil(W / 64) + x / 64 ascending), raster order inside a tile.
+ *   out       DEVICE argus_source[capacity], 16-byte aligned.  Catalogue order: ascending raster index y * W + x
+ *             (the paper states none; DESIGN.md R-D6).
  *   n_dev     DEVICE int64 (may be NULL): number of sources found (asynchronous)
  *   n_out     HOST (may be NULL): when given the call synchronises the stream and stores the number found; if that
  *             exceeds a non-zero capacity the call returns ARGUS_ERR_CAPACITY, the contents of out are unspecified
  *             (nothing is written beyond capacity) and *n_out is the capacity to call again with.
- * capacity = 0 only counts.  Scratch: 12 bytes per tile + 32 bytes per record of capacity, grown on demand (which
+ * capacity = 0 only counts.  Scratch: 12 bytes per 64 x 32-pixel work tile + 40 bytes per record of capacity, grown on demand (which
  * synchronises the device).  Otherwise asynchronous on stream. */
 int argus_detect_sources(argus_ctx* ctx, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, const float* bkg,
                          const float* nse, float k_sigma, argus_source* out, size_t capacity, int64_t* n_dev,
                          size_t* n_out, void* stream);
 
-/* Synchronises the stream and reports the statistics of the cached plan.  Returns ARGUS_ERR_CAPACITY if
- * an asynchronous call since the last check overflowed its output capacity or the context's max_tiles. */
+/* Synchronises the stream and reports the statistics of the most recent plan.  Returns ARGUS_ERR_CAPACITY if ANY
+ * asynchronous call since the last check (argus_plan_info or argus_healpix_footprint) overflowed its output capacity
+ * or the context's max_tiles -- the condition is latched in the context, not in the per-frame plan, so a check after
+ * a batch of frames sees the overflow of any of them; reading clears it. */
 int argus_plan_info(argus_ctx* ctx, argus_plan_stats* out, void* stream);
 
 /* Synchronises the stream and returns, for the calls recorded since ARGUS_OPT_PROFILE was last set to 1,

@@ -23,8 +23,8 @@ v_(n-1) is (v_((n-1)//2) + v_(n//2)) / 2):
                   s_p >= s_q for q after p (of equal neighbours the raster-first one is the source).  A pixel touching an interpolation node with nse = +inf is never a source.
   R-D5 record     x, y, peak = s_p, flux = sum of s over the good in-frame pixels of the 3x3 window, centroid offsets
                   cx = sum(s * dx) / flux, cy = sum(s * dy) / flux (0 when flux <= 0), bkg and nse at p.
-  R-D6 order      catalogue order = by 64 x 32-pixel tile ((y // 32) * ceil(W / 64) + x // 64 ascending), raster order
-                  inside a tile (the paper hands the catalogue to CPU cross-matching: any fixed order serves).
+  R-D6 order      ascending raster index y * W + x (the paper hands the catalogue to CPU cross-matching, PAPER.md:135,
+                  and states no order; raster order is the one that depends on nothing but the frame).
 """
 from __future__ import annotations
 
@@ -111,8 +111,8 @@ def background(cal, mask, B=64, n_min=16):
 _NEIGH = [(-1, -1), (-1, 0), (-1, 1), (0, -1), (0, 1), (1, -1), (1, 0), (1, 1)]   # (dy, dx), raster order
 
 
-def detect(cal, mask, bkg, nse, B=64, k_sigma=5.0, slack=0.0, tile=(64, 32)):
-    """R-D4 .. R-D6.  Returns a dict of arrays over the sources in catalogue order (tile=None: raster order): x, y, peak, flux, cx, cy,
+def detect(cal, mask, bkg, nse, B=64, k_sigma=5.0, slack=0.0):
+    """R-D4 .. R-D6.  Returns a dict of arrays over the sources in ascending raster order: x, y, peak, flux, cx, cy,
     bkg, nse, plus the decision margins m_thr = s - max(k * nse, 0) and m_max = min over neighbours of (s_p - s_q)
     (+inf without neighbours).  slack > 0 also returns the near misses (m_thr > -slack and m_max > -slack, ties
     included); the strict set is m_thr > 0 and `strict`."""
@@ -135,10 +135,7 @@ def detect(cal, mask, bkg, nse, B=64, k_sigma=5.0, slack=0.0, tile=(64, 32)):
         m_max = np.minimum(m_max, d)
         strict &= (d > 0) if i < 4 else (d >= 0)
     cand = (m_thr > -slack) & (m_max > -slack) if slack > 0 else (m_thr > 0) & strict
-    ys, xs = np.nonzero(cand)
-    if tile is not None:
-        order = np.lexsort((xs, ys, (ys // tile[1]) * (-(-W // tile[0])) + xs // tile[0]))
-        ys, xs = ys[order], xs[order]
+    ys, xs = np.nonzero(cand)                          # row-major scan: ascending y * W + x
     flux = np.zeros(xs.size); mx = np.zeros(xs.size); my = np.zeros(xs.size)
     for dy in (-1, 0, 1):
         for dx in (-1, 0, 1):

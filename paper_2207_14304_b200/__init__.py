@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     argus_resample,
     argus_resample_coadd,
     argus_resample_host,
+    argus_resample_coadd_host,
     argus_host_wait,
     argus_segment_products,
     library_path,

@@ -22,7 +22,7 @@ EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
-    "argus_resample_host", "argus_host_wait", "argus_segment_products", "argus_background_map", "argus_detect_sources",
+    "argus_resample_host", "argus_resample_coadd_host", "argus_host_wait", "argus_segment_products", "argus_background_map", "argus_detect_sources",
 ]
 
 
@@ -65,10 +65,13 @@ def load_library():
     if _lib is not None:
         return _lib
     path = library_path()
-    try:  # rebuild in-tree when the sources are newer than the library (needs nvcc; never falls back to CPU)
-        from . import _build
+    # rebuild in-tree when the sources are newer than the library (needs nvcc; never falls back to CPU).  A failed rebuild
+    # of stale sources is an error: running an old library against new sources would hide it.  Without nvcc (a box that
+    # only received the built .so) the existing library is used as it is.
+    from . import _build
+    try:
         _build.build()
-    except Exception:
+    except FileNotFoundError:
         if not os.path.exists(path):
             raise
     if not os.path.exists(path):
@@ -92,6 +95,8 @@ def load_library():
     L.argus_resample_coadd.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32,
                                        C.POINTER(_Coadd), vp, vp, vp, vp]
     L.argus_resample_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, sz, vp, vp, vp]
+    L.argus_resample_coadd_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32,
+                                            C.POINTER(_Coadd), vp, vp, vp, vp]
     L.argus_host_wait.argtypes = [vp]
     L.argus_segment_products.argtypes = [vp, i64, i64, vp, vp, vp, sz, vp, sz, C.POINTER(_Coadd), vp, vp, vp, vp, vp, sz,
                                          vp, C.POINTER(sz), vp]
@@ -347,6 +352,28 @@ def argus_resample_coadd(ctx, wcs, W, H, nside, kernel, tiles, nside_tile, sum_,
                                              _dev(wsum, torch.float32, "wsum"),
                                              _dev(n_skipped, torch.int64, "n_skipped", allow_none=True), _stream(stream))
     _check(ctx, rc, "argus_resample_coadd")
+
+
+def argus_resample_coadd_host(ctx, wcs, W, H, nside, kernel, raw_host, tiles, nside_tile, sum_, wsum, n_skipped=None,
+                              w_min=0.5, stream=None, bias=None, dark=None, flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1):
+    """A2-A6 fused with the raw frame in HOST memory (pinned CPU tensor); masters and the coadd are CUDA tensors."""
+    if not isinstance(raw_host, torch.Tensor) or raw_host.is_cuda or raw_host.dtype != torch.uint16 or not raw_host.is_contiguous():
+        raise TypeError("raw_host must be a contiguous CPU uint16 tensor")
+    if raw_host.numel() != W * H:
+        raise ValueError("raw_host does not hold W * H pixels")
+    f = _Frame()
+    f.raw = raw_host.data_ptr()
+    f.bias = _dev(bias, torch.float32, "bias")
+    f.dark = _dev(dark, torch.float32, "dark")
+    f.flat = _dev(flat, torch.float32, "flat")
+    f.t_exp, f.sat_adu, f.flat_min = float(t_exp), int(sat_adu), float(flat_min)
+    w = _wcs_struct(wcs)
+    lay = _coadd_struct(tiles, nside_tile)
+    rc = load_library().argus_resample_coadd_host(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min),
+                                                  C.byref(lay), _dev(sum_, torch.float32, "sum"),
+                                                  _dev(wsum, torch.float32, "wsum"),
+                                                  _dev(n_skipped, torch.int64, "n_skipped", allow_none=True), _stream(stream))
+    _check(ctx, rc, "argus_resample_coadd_host")
 
 
 def argus_segment_products(ctx, nside, nside_mini, idx, value, weight, targets, seg16=None, mini_id=None, mini_value=None,

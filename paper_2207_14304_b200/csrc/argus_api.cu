@@ -57,12 +57,16 @@ struct argus_ctx {
     const void* maps_key[4];
     int64_t maps_W, maps_H;
     int64_t n_launches;   // kernels launched through this context (diagnostics)
+    bool auto_tiles;      // max_tiles = 0 at creation: the plan scratch is sized from (W, H, nside, pixel scale) at first use
+    int64_t cap_tiles, cap_slots;   // capacity of the allocated scratch sets (0 = none yet)
+    int* d_latch;         // [0] overflow bits of every asynchronous call since the last read, [1] the value last fetched
+    int* h_latch;         // pinned copy of d_latch[1]
     // argus_resample_host: two sets of device staging buffers, upload / download streams
     struct HostBuf {
         uint16_t* raw; float* val; float* wgt;
         size_t cap_px, cap_n;
         cudaEvent_t up, run, down;
-        bool used, ev_ok;
+        bool used, down_used, ev_ok;
     } hb[2];
     int hb_next;
     cudaStream_t s_up, s_down;
@@ -78,6 +82,7 @@ struct argus_ctx {
         float* cells; size_t cap_cells;          // med | sig | ngood, cap_cells each
         uint2* tiles; size_t cap_tiles;          // tile_info | offsets (4 B) behind it
         ArgusSourceRec* tmp; size_t cap_tmp;
+        uint2* ord;                              // (band-local raster key, position in tmp) per record, cap_tmp entries
         unsigned* ctl;                           // [0] running total (atomics), [1] final count
         long long* h_n;                          // pinned
     } bg;
@@ -156,11 +161,11 @@ static void lsq_pinv(int deg, double* pinv) {
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // One set of plan scratch: a single device allocation carved into the PlanBuffers arrays.
-static cudaError_t alloc_plan_slot(int64_t max_tiles, PlanBuffers& pb, void** block) {
+static cudaError_t alloc_plan_slot(int64_t max_tiles, int64_t max_slots, PlanBuffers& pb, void** block) {
     pb.max_tiles = (int)max_tiles;
-    pb.max_slots = (int)(max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26));
+    pb.max_slots = (int)max_slots;
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4, o_bc2;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4, o_bc2, o_sp;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
@@ -179,7 +184,8 @@ static cudaError_t alloc_plan_slot(int64_t max_tiles, PlanBuffers& pb, void** bl
     o_dc = o;    o = align_up(o + sizeof(double) * 20 * (size_t)pb.max_tiles, 256);
     o_fr = o;    o = align_up(o + sizeof(FastRec) * (size_t)pb.max_tiles, 256);
     o_sc = o;    o = align_up(o + sizeof(int), 256);
-    o_sl = o;    o = align_up(o + sizeof(int) * pb.max_hard, 256);
+    o_sl = o;    o = align_up(o + sizeof(int) * (size_t)pb.max_tiles, 256);   // any tile may end up on the slow list
+    o_sp = o;    o = align_up(o + sizeof(int), 256);
     o_bid = o;   o = align_up(o + sizeof(long long) * (pb.max_tiles / 64 + 1), 256);
     o_nb = o;    o = align_up(o + sizeof(int), 256);
     o_fc = o;    o = align_up(o + sizeof(int), 256);
@@ -210,6 +216,7 @@ static cudaError_t alloc_plan_slot(int64_t max_tiles, PlanBuffers& pb, void** bl
     pb.frec = (FastRec*)(b + o_fr);
     pb.slow_count = (int*)(b + o_sc);
     pb.slow_list = (int*)(b + o_sl);
+    pb.slow_plan = (int*)(b + o_sp);
     pb.block_id = (long long*)(b + o_bid);
     pb.n_blocks = (int*)(b + o_nb);
     pb.fb_count = (int*)(b + o_fc);
@@ -225,23 +232,47 @@ static cudaError_t alloc_plan_slot(int64_t max_tiles, PlanBuffers& pb, void** bl
     return e;
 }
 
+// (Re)allocates the PLAN_SLOTS sets of plan scratch for max_tiles candidate tiles and max_slots scan slots.
+static int alloc_plan_slots(argus_ctx* c, int64_t max_tiles, int64_t max_slots) {
+    if (c->slot_block[0]) {
+        CUDA_TRY(c, cudaDeviceSynchronize());        // plans and kernels still reading the old sets
+        for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) { cudaFree(c->slot_block[sidx]); c->slot_block[sidx] = nullptr; c->slot_used[sidx] = false; }
+    }
+    c->plan_valid = false;
+    c->cap_tiles = 0;
+    for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
+        CUDA_TRY(c, alloc_plan_slot(max_tiles, max_slots, c->slot_pb[sidx], &c->slot_block[sidx]));
+        c->slot_pb[sidx].latch = c->d_latch;
+    }
+    c->pb = c->slot_pb[0];
+    c->cur_slot = 0;
+    c->cap_tiles = max_tiles;
+    c->cap_slots = max_slots;
+    return ARGUS_OK;
+}
+
+static int64_t default_max_slots(int64_t max_tiles) { return max_tiles * 8 < (1 << 26) ? max_tiles * 8 : (1 << 26); }
+
 extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) {
     if (!out) return ARGUS_ERR_NULL;
     *out = nullptr;
-    if (max_tiles == 0) max_tiles = 1 << 19;
-    if (max_tiles < 64 || max_tiles > (1 << 24)) return ARGUS_ERR_SHAPE;
+    if (max_tiles != 0 && (max_tiles < 64 || max_tiles > (1 << 24))) return ARGUS_ERR_SHAPE;
     argus_ctx* c = new (std::nothrow) argus_ctx();
     if (!c) return ARGUS_ERR_CAPACITY;
     memset(c, 0, sizeof(*c));
     c->device = device;
     c->plan_cache = true;
     c->fast_enabled = true;
+    c->auto_tiles = max_tiles == 0;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
-    cudaError_t e2 = cudaSuccess;
-    for (int sidx = 0; sidx < PLAN_SLOTS && e2 == cudaSuccess; ++sidx) e2 = alloc_plan_slot(max_tiles, c->slot_pb[sidx], &c->slot_block[sidx]);
+    cudaError_t e2 = cudaMalloc((void**)&c->d_latch, 2 * sizeof(int));
+    if (e2 == cudaSuccess) e2 = cudaMemset(c->d_latch, 0, 2 * sizeof(int));
+    if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_latch, sizeof(int));
     if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
+    int rc_slots = ARGUS_OK;
+    if (e2 == cudaSuccess && !c->auto_tiles) rc_slots = alloc_plan_slots(c, max_tiles, default_max_slots(max_tiles));
     int prio_lo = 0, prio_hi = 0;
     if (e2 == cudaSuccess) e2 = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
     for (int i = 0; i < 2 && e2 == cudaSuccess; ++i) e2 = cudaStreamCreateWithPriority(&c->side[i], cudaStreamNonBlocking, prio_hi);
@@ -249,15 +280,14 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
         e2 = cudaEventCreateWithFlags(&c->ev_done[sidx], cudaEventDisableTiming);
         if (e2 == cudaSuccess) e2 = cudaEventCreateWithFlags(&c->ev_free[sidx], cudaEventDisableTiming);
     }
-    if (e2 != cudaSuccess) {
-        c->last_cuda = (int)e2;
+    if (e2 != cudaSuccess || rc_slots != ARGUS_OK) {
         for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) if (c->slot_block[sidx]) cudaFree(c->slot_block[sidx]);
         if (c->h_stats) cudaFreeHost(c->h_stats);
+        if (c->h_latch) cudaFreeHost(c->h_latch);
+        if (c->d_latch) cudaFree(c->d_latch);
         delete c;
         return ARGUS_ERR_CUDA;
     }
-    c->pb = c->slot_pb[0];
-    c->cur_slot = 0;
     c->overlap = true;
     for (int i = 0; i < 256; ++i)
         for (int j = 0; j < 4; ++j) cudaEventCreate(&c->ev[i][j]);
@@ -272,7 +302,7 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
     for (int i = 0; i < 256; ++i)
         for (int j = 0; j < 4; ++j) cudaEventDestroy(c->ev[i][j]);
     for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
-        cudaFree(c->slot_block[sidx]);
+        if (c->slot_block[sidx]) cudaFree(c->slot_block[sidx]);
         cudaEventDestroy(c->ev_done[sidx]);
         cudaEventDestroy(c->ev_free[sidx]);
     }
@@ -291,9 +321,12 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (c->bg.cells) cudaFree(c->bg.cells);
     if (c->bg.tiles) cudaFree(c->bg.tiles);
     if (c->bg.tmp) cudaFree(c->bg.tmp);
+    if (c->bg.ord) cudaFree(c->bg.ord);
     if (c->bg.ctl) cudaFree(c->bg.ctl);
     if (c->bg.h_n) cudaFreeHost(c->bg.h_n);
     cudaFreeHost(c->h_stats);
+    cudaFreeHost(c->h_latch);
+    cudaFree(c->d_latch);
     delete c;
     return ARGUS_OK;
 }
@@ -440,6 +473,53 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     }
     c->plan_valid = false;
     const int lite = need_full ? 0 : 1;
+    // Hierarchical plan (plan_block.cuh) whenever a block of 8x8 tiles exists at this nside; the flat plan (one
+    // scan slot and one fit per tile) serves nside < 256.
+    const bool blocks = dw.k >= ARGUS_TILE_LOG2 + BLOCK_TILES_LOG2;
+    int64_t nside_t = nside >> ARGUS_TILE_LOG2;                      // tile-level nside
+    if (nside_t < 1) nside_t = 1;
+    int64_t nside_s = blocks ? (nside_t >> BLOCK_TILES_LOG2) : nside_t;   // resolution of the scan slots
+    // coarse resolution: cells comparable to the search cone, list passed by value
+    int64_t nside_c = 1;
+    while (nside_c < nside_s && (double)nside_c < 2.0 / rho) nside_c <<= 1;
+    std::vector<long long> cells;
+    for (;;) {
+        cells.clear();
+        for (int b = 0; b < 12; ++b) coarse_descend(dw.er, rho, 1, b, nside_c, cells);
+        if ((int)cells.size() <= ARGUS_MAX_COARSE || nside_c == 1) break;
+        nside_c >>= 1;
+    }
+    if ((int)cells.size() > ARGUS_MAX_COARSE) return ARGUS_ERR_CAPACITY;
+    CoarseList cl;
+    memset(&cl, 0, sizeof(cl));
+    cl.n = (int)cells.size();
+    cl.ratio_log2 = ilog2(nside_s / nside_c);
+    for (int i = 0; i < cl.n; ++i) cl.cell[i] = cells[i];
+    long long n_slots = (long long)cl.n << (2 * cl.ratio_log2);
+    if (cl.ratio_log2 > 12) return ARGUS_ERR_CAPACITY;
+    if (c->auto_tiles) {
+        // Scratch sized for this frame: candidate tiles = tiles whose block centre lies within one block radius of the
+        // frame, i.e. (W + 2 r)(H + 2 r) detector pixels' worth of HEALPix pixels (equal area), + 50 % and a margin for
+        // the ragged block boundary; never more than the scan's own bound.  Grown (device synchronised) when a larger
+        // frame arrives, never shrunk.
+        const double omega = 4.0 * kPi / (12.0 * (double)nside * (double)nside);
+        const double unit_ang = (blocks ? 8.0 : 1.0) * dw.tile_ang;
+        const double r_px = 1.05 * unit_ang / s_rad + 2.0;
+        const double hp_px = ((double)W + 2.0 * r_px) * ((double)H + 2.0 * r_px) * s_rad * s_rad / omega;
+        long long est = (long long)(1.5 * hp_px / 1024.0) + 4096;
+        const long long bound = blocks ? n_slots * 64 : n_slots;
+        if (est > bound) est = bound;
+        if (est < 1024) est = 1024;
+        est = (est + 1023) / 1024 * 1024;
+        if (est > (1 << 24)) return ARGUS_ERR_CAPACITY;
+        long long want_slots = n_slots > default_max_slots(est) ? n_slots : default_max_slots(est);
+        if (want_slots > (1 << 26)) return ARGUS_ERR_CAPACITY;
+        if (est > c->cap_tiles || want_slots > c->cap_slots) {
+            int rc2 = alloc_plan_slots(c, est > c->cap_tiles ? est : c->cap_tiles, want_slots > c->cap_slots ? want_slots : c->cap_slots);
+            if (rc2) return rc2;
+        }
+    }
+    if (n_slots > c->slot_pb[0].max_slots) return ARGUS_ERR_CAPACITY;
     // where the plan is built: in place on the caller's stream, or (overlap) in the other scratch set on the side
     // stream, after the last kernel that read that set
     int ps = c->cur_slot;
@@ -459,29 +539,6 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
         c->pb.fast_cap = fk ? FastCfg<1>::CAP : FastCfg<0>::CAP;
     }
     if (prof_slot >= 0) cudaEventRecord(c->ev[prof_slot][0], st);
-    // Hierarchical plan (plan_block.cuh) whenever a block of 8x8 tiles exists at this nside; the flat plan (one
-    // scan slot and one fit per tile) serves nside < 256.
-    const bool blocks = dw.k >= ARGUS_TILE_LOG2 + BLOCK_TILES_LOG2;
-    int64_t nside_t = nside >> ARGUS_TILE_LOG2;                      // tile-level nside
-    int64_t nside_s = blocks ? (nside_t >> BLOCK_TILES_LOG2) : nside_t;   // resolution of the scan slots
-    // coarse resolution: cells comparable to the search cone, list passed by value
-    int64_t nside_c = 1;
-    while (nside_c < nside_s && (double)nside_c < 2.0 / rho) nside_c <<= 1;
-    std::vector<long long> cells;
-    for (;;) {
-        cells.clear();
-        for (int b = 0; b < 12; ++b) coarse_descend(dw.er, rho, 1, b, nside_c, cells);
-        if ((int)cells.size() <= ARGUS_MAX_COARSE || nside_c == 1) break;
-        nside_c >>= 1;
-    }
-    if ((int)cells.size() > ARGUS_MAX_COARSE) return ARGUS_ERR_CAPACITY;
-    CoarseList cl;
-    memset(&cl, 0, sizeof(cl));
-    cl.n = (int)cells.size();
-    cl.ratio_log2 = ilog2(nside_s / nside_c);
-    for (int i = 0; i < cl.n; ++i) cl.cell[i] = cells[i];
-    long long n_slots = (long long)cl.n << (2 * cl.ratio_log2);
-    if (cl.ratio_log2 > 12 || n_slots > c->pb.max_slots) return ARGUS_ERR_CAPACITY;
     if (n_slots == 0) n_slots = 1;
     int nblk = (int)((n_slots + 255) / 256);
     long long tile_bound;
@@ -584,9 +641,16 @@ extern "C" int argus_calibrate(argus_ctx* c, const uint16_t* raw, const float* b
 }
 
 // --------------------------------------------------------------------------------------- A0 + A1
-static int fetch_stats(argus_ctx* c, cudaStream_t st) {
+// Plan statistics of the current scratch set + the context-wide overflow latch (read and cleared).
+static int fetch_stats(argus_ctx* c, cudaStream_t st, int* latched) {
+    *latched = 0;
+    if (!c->slot_block[0]) { memset(c->h_stats, 0, sizeof(PlanStats)); return ARGUS_OK; }   // no plan built yet
     CUDA_TRY(c, cudaMemcpyAsync(c->h_stats, c->pb.stats, sizeof(PlanStats), cudaMemcpyDeviceToHost, st));
+    plan_latch_fetch_kernel<<<1, 32, 0, st>>>(c->d_latch, c->d_latch + 1);
+    c->n_launches++;
+    CUDA_TRY(c, cudaMemcpyAsync(c->h_latch, c->d_latch + 1, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaStreamSynchronize(st));
+    *latched = *c->h_latch;
     return ARGUS_OK;
 }
 
@@ -598,10 +662,12 @@ extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64
     CUDA_TRY(c, cudaSetDevice(c->device));
     int rc = build_plan(c, wcs, W, H, nside, -1, st, -1, -1);
     if (rc) return rc;
-    rc = fetch_stats(c, st);
+    int latched;
+    rc = fetch_stats(c, st, &latched);
     if (rc) return rc;
     *n_out = (size_t)c->h_stats->n_footprint;
     if (c->h_stats->overflow & 3) { c->plan_valid = false; return ARGUS_ERR_CAPACITY; }
+    if (latched) return ARGUS_ERR_CAPACITY;      // an earlier asynchronous call overflowed (this plan itself is intact)
     if (idx_out) {
         if ((size_t)c->h_stats->n_footprint > capacity) return ARGUS_ERR_CAPACITY;
         plan_write_indices_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->pb, (long long*)idx_out, (long long)capacity);
@@ -615,12 +681,14 @@ extern "C" int argus_healpix_footprint(argus_ctx* c, const argus_wcs* wcs, int64
 extern "C" int argus_plan_info(argus_ctx* c, argus_plan_stats* out, void* stream) {
     if (!c || !out) return ARGUS_ERR_NULL;
     CUDA_TRY(c, cudaSetDevice(c->device));
-    int rc = fetch_stats(c, (cudaStream_t)stream);
+    int latched;
+    int rc = fetch_stats(c, (cudaStream_t)stream, &latched);
     if (rc) return rc;
     const PlanStats* s = c->h_stats;
     out->n_footprint = s->n_footprint; out->n_tiles = s->n_tiles; out->n_inside = s->n_inside;
     out->n_border = s->n_border; out->n_exact = s->n_exact; out->n_empty = s->n_empty;
-    if (s->overflow) { c->plan_valid = false; return ARGUS_ERR_CAPACITY; }
+    if (s->overflow) c->plan_valid = false;
+    if (s->overflow || latched) return ARGUS_ERR_CAPACITY;
     return ARGUS_OK;
 }
 
@@ -744,14 +812,12 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     return ARGUS_OK;
 }
 
-// ------------------------------------------------------------------------------- host-buffer variant
-extern "C" int argus_resample_host(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
-                                   int64_t nside, int kernel, float w_min, size_t n, float* value_host, float* weight_host,
-                                   void* stream) {
-    if (!c || !frame || !wcs || !value_host || !weight_host || !frame->raw) return ARGUS_ERR_NULL;
-    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n == 0 || n > ((size_t)1 << 34)) return ARGUS_ERR_SHAPE;
-    cudaStream_t st = (cudaStream_t)stream;
-    CUDA_TRY(c, cudaSetDevice(c->device));
+// ------------------------------------------------------------------------------- host-buffer variants
+// Upload of the HOST raw frame into the next of two device staging sets on the upload stream, ordered after the kernels
+// that last read that set; the caller's stream then waits for the upload (and, with outputs, for the previous download
+// of the set).  n_out = 0: no output staging (coadd form).
+static int host_stage_upload(argus_ctx* c, const argus_frame* frame, int64_t W, int64_t H, size_t n_out, cudaStream_t st,
+                             argus_ctx::HostBuf** out_b) {
     if (!c->s_up) {
         CUDA_TRY(c, cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking));
         CUDA_TRY(c, cudaStreamCreateWithFlags(&c->s_down, cudaStreamNonBlocking));
@@ -765,35 +831,70 @@ extern "C" int argus_resample_host(argus_ctx* c, const argus_frame* frame, const
         CUDA_TRY(c, cudaEventCreateWithFlags(&b.down, cudaEventDisableTiming));
         b.ev_ok = true;
     }
-    if (b.cap_px < px || b.cap_n < n) {      // (re)allocation synchronises: first call per buffer set, or a larger frame
+    if (b.cap_px < px || b.cap_n < n_out) {      // (re)allocation synchronises: first call per buffer set, or a larger frame
         CUDA_TRY(c, cudaDeviceSynchronize());
+        const size_t want_px = b.cap_px > px ? b.cap_px : px, want_n = b.cap_n > n_out ? b.cap_n : n_out;
         if (b.raw) cudaFree(b.raw);
         if (b.val) cudaFree(b.val);
         if (b.wgt) cudaFree(b.wgt);
-        b.raw = nullptr; b.val = b.wgt = nullptr; b.cap_px = b.cap_n = 0; b.used = false;
-        CUDA_TRY(c, cudaMalloc((void**)&b.raw, px * sizeof(uint16_t)));
-        CUDA_TRY(c, cudaMalloc((void**)&b.val, n * sizeof(float)));
-        CUDA_TRY(c, cudaMalloc((void**)&b.wgt, n * sizeof(float)));
-        b.cap_px = px; b.cap_n = n;
+        b.raw = nullptr; b.val = b.wgt = nullptr; b.cap_px = b.cap_n = 0; b.used = false; b.down_used = false;
+        CUDA_TRY(c, cudaMalloc((void**)&b.raw, want_px * sizeof(uint16_t)));
+        if (want_n) {
+            CUDA_TRY(c, cudaMalloc((void**)&b.val, want_n * sizeof(float)));
+            CUDA_TRY(c, cudaMalloc((void**)&b.wgt, want_n * sizeof(float)));
+        }
+        b.cap_px = want_px; b.cap_n = want_n;
     }
-    // upload on its own stream (after the kernels that last read this raw buffer) ...
     if (b.used) CUDA_TRY(c, cudaStreamWaitEvent(c->s_up, b.run, 0));
     CUDA_TRY(c, cudaMemcpyAsync(b.raw, frame->raw, px * sizeof(uint16_t), cudaMemcpyHostToDevice, c->s_up));
     CUDA_TRY(c, cudaEventRecord(b.up, c->s_up));
-    // ... kernels on the caller's stream (after the upload, and after the previous download of this buffer set) ...
     CUDA_TRY(c, cudaStreamWaitEvent(st, b.up, 0));
-    if (b.used) CUDA_TRY(c, cudaStreamWaitEvent(st, b.down, 0));
-    argus_frame fr = *frame;
-    fr.raw = b.raw;
-    int rc = argus_resample(c, &fr, wcs, W, H, nside, kernel, w_min, nullptr, n, b.val, b.wgt, stream);
+    if (n_out && b.down_used) CUDA_TRY(c, cudaStreamWaitEvent(st, b.down, 0));
+    *out_b = &b;
+    return ARGUS_OK;
+}
+
+extern "C" int argus_resample_host(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                                   int64_t nside, int kernel, float w_min, size_t n, float* value_host, float* weight_host,
+                                   void* stream) {
+    if (!c || !frame || !wcs || !value_host || !weight_host || !frame->raw) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n == 0 || n > ((size_t)1 << 34)) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    argus_ctx::HostBuf* b;
+    int rc = host_stage_upload(c, frame, W, H, n, st, &b);
     if (rc) return rc;
-    CUDA_TRY(c, cudaEventRecord(b.run, st));
-    // ... download on its own stream
-    CUDA_TRY(c, cudaStreamWaitEvent(c->s_down, b.run, 0));
-    CUDA_TRY(c, cudaMemcpyAsync(value_host, b.val, n * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
-    CUDA_TRY(c, cudaMemcpyAsync(weight_host, b.wgt, n * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
-    CUDA_TRY(c, cudaEventRecord(b.down, c->s_down));
-    b.used = true;
+    argus_frame fr = *frame;
+    fr.raw = b->raw;
+    rc = argus_resample(c, &fr, wcs, W, H, nside, kernel, w_min, nullptr, n, b->val, b->wgt, stream);
+    if (rc) return rc;
+    CUDA_TRY(c, cudaEventRecord(b->run, st));
+    b->used = true;
+    // download on its own stream
+    CUDA_TRY(c, cudaStreamWaitEvent(c->s_down, b->run, 0));
+    CUDA_TRY(c, cudaMemcpyAsync(value_host, b->val, n * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaMemcpyAsync(weight_host, b->wgt, n * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaEventRecord(b->down, c->s_down));
+    b->down_used = true;
+    return ARGUS_OK;
+}
+
+extern "C" int argus_resample_coadd_host(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                                         int64_t nside, int kernel, float w_min, const argus_coadd* layout, float* sum,
+                                         float* wsum, int64_t* n_skipped_dev, void* stream) {
+    if (!c || !frame || !wcs || !frame->raw) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20)) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    argus_ctx::HostBuf* b;
+    int rc = host_stage_upload(c, frame, W, H, 0, st, &b);
+    if (rc) return rc;
+    argus_frame fr = *frame;
+    fr.raw = b->raw;
+    rc = argus_resample_coadd(c, &fr, wcs, W, H, nside, kernel, w_min, layout, sum, wsum, n_skipped_dev, stream);
+    if (rc) return rc;
+    CUDA_TRY(c, cudaEventRecord(b->run, st));
+    b->used = true;
     return ARGUS_OK;
 }
 
@@ -1036,9 +1137,10 @@ extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int6
         c->bg.cap_tiles = want;
     }
     if (c->bg.cap_tmp < capacity || !c->bg.tmp) {
-        if (c->bg.tmp) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tmp); c->bg.tmp = nullptr; }
+        if (c->bg.tmp) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tmp); cudaFree(c->bg.ord); c->bg.tmp = nullptr; c->bg.ord = nullptr; }
         size_t want = align_up(capacity + 1, 65536);
         CUDA_TRY(c, cudaMalloc((void**)&c->bg.tmp, want * sizeof(ArgusSourceRec)));
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.ord, want * sizeof(uint2)));
         c->bg.cap_tmp = want;
     }
     unsigned* offsets = (unsigned*)(c->bg.tiles + c->bg.cap_tiles);
@@ -1056,8 +1158,8 @@ extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int6
     det_scan_kernel<<<1, 1024, 0, st>>>(c->bg.tiles, (int)n_tiles, offsets, c->bg.ctl, (long long*)n_dev);
     c->n_launches += 2;
     if (capacity > 0) {
-        det_gather_kernel<<<(unsigned)((n_tiles + 7) / 8), 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, c->bg.tmp,
-                                                                        (ArgusSourceRec*)out, (unsigned)capacity);
+        det_order_kernel<<<(unsigned)tiles_y, 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, (int)tiles_x, (int)W, c->bg.ctl,
+                                                           c->bg.tmp, c->bg.ord, (ArgusSourceRec*)out, (unsigned)capacity);
         c->n_launches++;
     }
     CUDA_TRY(c, cudaGetLastError());

@@ -13,8 +13,9 @@
 //   det_tiles_kernel   one CTA per 64 x 32-pixel tile: s = cal - bkg(x, y) for the tile + 1-pixel apron in shared
 //                      memory, thresholded raster-first local maxima, 3x3 flux and centroid; records go to a
 //                      scratch list at an atomically reserved base, (base, count) per tile.
-//   det_scan_kernel    exclusive scan of the per-tile counts (tile order = catalogue order).
-//   det_gather_kernel  one warp per tile copies its records to their final, deterministic position.
+//   det_scan_kernel    exclusive scan of the per-tile counts.
+//   det_order_kernel   one CTA per tile row: ranks the row's records by raster index and writes them to their final
+//                      position (catalogue order = ascending y * W + x, R-D6).
 #pragma once
 #include "resample.cuh"
 
@@ -531,19 +532,53 @@ __global__ void __launch_bounds__(1024) det_scan_kernel(const uint2* __restrict_
     }
 }
 
-// One warp per tile: tmp[base .. base + cnt) -> out[offset .. offset + cnt).
-__global__ void __launch_bounds__(256) det_gather_kernel(const uint2* __restrict__ tile_info, const unsigned* __restrict__ offsets,
-                                                         int n_tiles, const ArgusSourceRec* __restrict__ tmp,
-                                                         ArgusSourceRec* __restrict__ out, unsigned capacity) {
-    const int tile = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (tile >= n_tiles) return;
-    const uint2 info = tile_info[tile];
-    const unsigned off = offsets[tile];
-    for (unsigned j = lane; j < info.y; j += 32) {
-        if (info.x + j >= capacity || off + j >= capacity) break;
-        const uint4* src = reinterpret_cast<const uint4*>(tmp + info.x + j);
-        uint4* dst = reinterpret_cast<uint4*>(out + off + j);
-        dst[0] = src[0];
-        dst[1] = src[1];
+// Catalogue order (R-D6: ascending raster index y * W + x).  det_tiles_kernel leaves every tile's records in raster
+// order at an arbitrary base of tmp; tiles of one tile row ("band", DET_TH image rows) interleave in raster order.  One
+// CTA per band: (1) band-local keys (y - y0) * W + x (< 2^25) and source positions of the band's records, in tile order,
+// to scratch; (2) rank of every record = number of smaller keys in the band (keys are unique), counted against chunks of
+// 1024 keys staged in shared memory (a 61-MPix frame has ~160 records per band); (3) record -> out[band start + rank].
+// Bands are consecutive in tile order, so band start = offsets[first tile of the band].
+#define DET_ORD_CHUNK 1024
+__global__ void __launch_bounds__(256) det_order_kernel(const uint2* __restrict__ tile_info, const unsigned* __restrict__ offsets,
+                                                        int n_tiles, int tiles_x, int W, const unsigned* __restrict__ ctl,
+                                                        const ArgusSourceRec* __restrict__ tmp, uint2* __restrict__ ord,
+                                                        ArgusSourceRec* __restrict__ out, unsigned capacity) {
+    __shared__ unsigned s_key[DET_ORD_CHUNK];
+    const int band = blockIdx.x, t0 = band * tiles_x, t1 = min(t0 + tiles_x, n_tiles);
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const unsigned band_off = offsets[t0], band_end = (t1 < n_tiles) ? offsets[t1] : ctl[1];
+    if (band_end > capacity) {
+        if (band_off >= capacity) return;       // overflow: the contents of out are unspecified, nothing beyond capacity
+    }
+    const unsigned n_b = min(band_end, capacity) - band_off;
+    if (n_b == 0) return;
+    const int y0 = band * DET_TH;
+    for (int tile = t0 + wid; tile < t1; tile += 8) {
+        const uint2 info = tile_info[tile];
+        const unsigned off = offsets[tile];
+        for (unsigned j = lane; j < info.y; j += 32) {
+            if (info.x + j >= capacity || off + j >= capacity) break;
+            const int2 xy = *reinterpret_cast<const int2*>(tmp + info.x + j);
+            ord[off + j] = make_uint2((unsigned)((xy.y - y0) * W + xy.x), info.x + j);
+        }
+    }
+    __syncthreads();
+    for (unsigned i0 = 0; i0 < n_b; i0 += 256) {
+        const unsigned i = i0 + tid;
+        const uint2 mine = i < n_b ? ord[band_off + i] : make_uint2(0u, 0u);
+        unsigned rank = 0;
+        for (unsigned c0 = 0; c0 < n_b; c0 += DET_ORD_CHUNK) {
+            const unsigned m = min((unsigned)DET_ORD_CHUNK, n_b - c0);
+            __syncthreads();
+            for (unsigned e = tid; e < m; e += 256) s_key[e] = ord[band_off + c0 + e].x;
+            __syncthreads();
+            for (unsigned e = 0; e < m; ++e) rank += (s_key[e] < mine.x) ? 1u : 0u;
+        }
+        if (i < n_b && rank < n_b && mine.y < capacity) {   // (garbage entries exist only after a capacity overflow)
+            const uint4* src = reinterpret_cast<const uint4*>(tmp + mine.y);
+            uint4* dst = reinterpret_cast<uint4*>(out + band_off + rank);
+            dst[0] = src[0];
+            dst[1] = src[1];
+        }
     }
 }

@@ -37,7 +37,10 @@ struct PlanBuffers {
     double* dcoef;              // [max_tiles][20] unsplit FP64 polynomial coefficients (x then y)
     FastRec* frec;              // [max_tiles] records of the TMA-staged bilinear kernel
     int* slow_count;            // device scalar
-    int* slow_list;             // [max_hard] tiles the fast kernel leaves to the general kernel
+    int* slow_plan;             // device scalar: slow_count as the plan left it; the Lanczos-3 fast kernel appends behind
+                                // it at run time and the general kernel restores it when it is done (a cached plan is reused)
+    int* slow_list;             // [max_tiles] tiles the fast kernel leaves to the general kernel
+    int* latch;                 // context-wide: every overflow bit is also ORed in here; cleared only when read
     long long* block_id;        // [max_tiles/64] candidate blocks (8x8 tiles), ascending nested ids at block level
     int* n_blocks;              // device scalar
     int* fb_count;              // device scalar
@@ -48,6 +51,13 @@ struct PlanBuffers {
     int max_slots, max_tiles, max_hard;
     int fast_tl, fast_tr, fast_cap;   // tap apron and stage capacity (pixels) of the fast kernel this plan is for
 };
+
+// Overflow bits (PlanStats.overflow) live in the plan slot and are zeroed by the next plan into it; the context-wide
+// latch keeps them until argus_plan_info / argus_healpix_footprint reads them.
+__device__ inline void plan_overflow(const PlanBuffers& pb, int bits) {
+    atomicOr(&pb.stats->overflow, bits);
+    atomicOr(pb.latch, bits);
+}
 
 // --------------------------------------------------------------------------------------------- scan
 __global__ void __launch_bounds__(256) plan_scan_kernel(DevWcs w, CoarseList cl, PlanBuffers pb, double rad_px) {
@@ -114,7 +124,7 @@ __global__ void __launch_bounds__(256) plan_compact_kernel(CoarseList cl, PlanBu
             int c = (int)(slot >> (2 * cl.ratio_log2));
             pb.tile_id[pos] = (cl.cell[c] << (2 * cl.ratio_log2)) | (slot & ((1ll << (2 * cl.ratio_log2)) - 1));
         } else {
-            atomicOr(&pb.stats->overflow, 1);
+            plan_overflow(pb, 1);
         }
     }
     if (blockIdx.x == gridDim.x - 1 && tid == 0) {
@@ -163,8 +173,8 @@ __device__ inline bool fast_box(const PlanBuffers& pb, int bx0, int bx1, int by0
 
 __device__ inline void slow_push(const PlanBuffers& pb, int t) {
     int s = atomicAdd(pb.slow_count, 1);
-    if (s < pb.max_hard) pb.slow_list[s] = t;
-    else atomicOr(&pb.stats->overflow, 2);
+    if (s < pb.max_tiles) pb.slow_list[s] = t;
+    else plan_overflow(pb, 2);
 }
 
 // Everything a kernel needs to know about one tile, written by ONE thread from the tile's cubic (c[0..9] x,
@@ -205,7 +215,7 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
             pb.hard_list[slot] = t;
             r.mask_slot = slot;
         } else {
-            atomicOr(&pb.stats->overflow, 2);
+            plan_overflow(pb, 2);
             cls = TC_EMPTY;
         }
     }
@@ -478,7 +488,9 @@ __device__ inline void offsets_final_body(const PlanBuffers& pb, long long out_c
         PlanStats* st = pb.stats;
         st->n_footprint = base;
         st->n_tiles = n;
-        if (out_capacity >= 0 && base > out_capacity) atomicOr(&st->overflow, 4);
+        if (out_capacity >= 0 && base > out_capacity) plan_overflow(pb, 4);
+        const int sc = *pb.slow_count;              // plan_members_kernel (the last to push) ran before this kernel
+        *pb.slow_plan = sc < pb.max_tiles ? sc : pb.max_tiles;
     }
 }
 
@@ -546,7 +558,13 @@ __global__ void __launch_bounds__(256) plan_offsets_kernel(PlanBuffers pb, long 
 
 // Re-check of the caller's output capacity when a cached plan is reused (the scan did it when the plan was built).
 __global__ void plan_check_capacity_kernel(PlanBuffers pb, long long out_capacity) {
-    if (threadIdx.x == 0 && blockIdx.x == 0 && pb.stats->n_footprint > out_capacity) atomicOr(&pb.stats->overflow, 4);
+    if (threadIdx.x == 0 && blockIdx.x == 0 && pb.stats->n_footprint > out_capacity) plan_overflow(pb, 4);
+}
+
+// *fetched = latch, latch = 0 (one atomic exchange: bits ORed in by kernels still running on other streams are kept
+// for the next read).
+__global__ void plan_latch_fetch_kernel(int* latch, int* fetched) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) *fetched = atomicExch(latch, 0);
 }
 
 __device__ __forceinline__ long long tile_out_offset(const PlanBuffers& pb, int t) {

@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(256) plan_bscan_kernel(DevWcs w, CoarseList cl
                     const int c = (int)(sj >> (2 * rl));
                     pb.block_id[pos] = (cl.cell[c] << (2 * rl)) | (sj & ((1ll << (2 * rl)) - 1));
                 } else {
-                    atomicOr(&pb.stats->overflow, 1);
+                    plan_overflow(pb, 1);
                 }
                 ++pos;
             }

@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(RS_THREADS, KERNEL == 0 ? RS_MIN_CTAS : 2) res
     const float S0 = (float)s0 * 0.03125f, S1 = S0 + 1.0f, T0 = (float)t0 * 0.03125f, T1 = T0 + 1.0f;
 
     // slow_only: visit only the tiles the TMA-staged kernel (resample_fast.cuh) left to this one
-    const int n_items = slow_only ? min(*pb.slow_count, pb.max_hard) : n_tiles;
+    const int n_items = slow_only ? min(*pb.slow_count, pb.max_tiles) : n_tiles;
     for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
         const int t = slow_only ? pb.slow_list[it] : it;
         const TileRec* __restrict__ rp = pb.rec + t;
@@ -384,6 +384,20 @@ __global__ void __launch_bounds__(RS_THREADS, KERNEL == 0 ? RS_MIN_CTAS : 2) res
                     value_out[o] = val;
                     weight_out[o] = wgt;
                 }
+            }
+        }
+    }
+    if (slow_only) {
+        // The Lanczos-3 fast kernel appended run-time entries behind the plan's own (slow_plan).  The last CTA to finish
+        // restores the list to the plan's state, so that a cached plan serves the next frame unchanged (no duplicates:
+        // the coadd accumulation is not idempotent).  Every CTA read slow_count before it takes a ticket.
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            if (atomicAdd(pb.ticket, 1u) == gridDim.x - 1) {
+                *pb.slow_count = *pb.slow_plan;
+                __threadfence();
+                *pb.ticket = 0u;
             }
         }
     }

@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
     const int lane = threadIdx.x & 31;
     const long long nw = (long long)gridDim.x * 8;
     const long long nm = min((long long)ctl[1], cap);
-    const int full = 1 << shift;
+    const long long full = 1ll << shift;   // pixels per minipix: up to 4^29 (nside 2^29, nside_mini 1)
     for (long long kb = ((long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * SEG_GROUP; kb < nm; kb += nw * SEG_GROUP) {
         // lanes 0..4: starts of the group's minipix (mini_start[nm] is the sentinel); lanes 0..3: keep flag, dense base
         const long long st = (lane <= SEG_GROUP) ? mini_start[min(kb + lane, nm)] : 0;
@@ -315,8 +315,8 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
                         if (dbase >= 0) {
                             const bool complete = rel[i + 1] - rel[i] == full;
                             const long long* ii = idx + s0 + (rel[i] + lane);
-                            long long o0 = complete ? (long long)lane : (left[i] > 0 ? (ii[0] & (long long)(full - 1)) : 0);
-                            long long o1 = complete ? (long long)(lane + 32) : (left[i] > 32 ? (ii[32] & (long long)(full - 1)) : 0);
+                            long long o0 = complete ? (long long)lane : (left[i] > 0 ? (ii[0] & (full - 1)) : 0);
+                            long long o1 = complete ? (long long)(lane + 32) : (left[i] > 32 ? (ii[32] & (full - 1)) : 0);
                             if (DENSE == 2) { o0 = seg_raster(o0, lay.ppt_log2 >> 1); o1 = seg_raster(o1, lay.ppt_log2 >> 1); }
                             if (left[i] > 0) seg16[dbase + o0] = h0;
                             if (left[i] > 32) seg16[dbase + o1] = h1;
@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(256, 4) seg_products_kernel(
                         const unsigned short hb = kp ? seg_f2h(vv) : (unsigned short)0;
                         if (DENSE) {
                             if (dbase >= 0) {
-                                long long o = (cnt == full) ? q : (idx[si + q] & (long long)(full - 1));
+                                long long o = (cnt == full) ? q : (idx[si + q] & (full - 1));
                                 if (DENSE == 2) o = seg_raster(o, lay.ppt_log2 >> 1);
                                 seg16[dbase + o] = hb;
                             }

@@ -74,7 +74,7 @@ def test_config4_one_frame_nside_2p18(argus, ctx):
 
 
 def test_config3_coadd_full(argus, ctx):
-    from gpu_util import upload
+    from gpu_util import assert_coadd_matches, coadd_oracle
     W, H, nside = synth.frames.FULL_W, synth.frames.FULL_H, 1 << 17
     base = synth.config3_frame(0)
     masters = (base.bias, base.dark, base.flat)
@@ -82,12 +82,8 @@ def test_config3_coadd_full(argus, ctx):
     fps = [oracle.footprint(f.wcs, W, H, nside)[0] for f in frames]
     tiles = np.unique(np.concatenate([fp >> 18 for fp in fps]))
     ppt = 1 << 18
-    s_or = np.zeros(len(tiles) * ppt)
-    w_or = np.zeros(len(tiles) * ppt)
-    for f, fp in zip(frames, fps):
-        cal, mask = oracle.calibrate_frame(f)
-        v, w, fl = oracle.resample(cal, mask, f.wcs, nside, fp, oracle.BILINEAR)
-        assert oracle.coadd_accumulate(tiles, ppt, s_or, w_or, fp, v, w) == 0
+    ref = coadd_oracle(frames, fps, tiles, ppt, nside, "bilinear")
+    assert ref["skipped"] == 0
     dt = torch.from_numpy(tiles).cuda()
     s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
     ws = torch.zeros_like(s)
@@ -99,8 +95,6 @@ def test_config3_coadd_full(argus, ctx):
         argus.argus_resample_coadd(ctx, f.wcs, W, H, nside, "bilinear", dt, 256, s, ws, sk, **d)
     torch.cuda.synchronize()
     assert int(sk.item()) == 0
-    sg, wg = s.cpu().numpy().astype(np.float64), ws.cpu().numpy().astype(np.float64)
-    assert np.abs(wg - w_or).max() <= 3e-5
-    # dithered frames: pixels within 1e-4 px of an integer next to a masked pixel are margin-ambiguous; bound them
-    bad = np.abs(sg - s_or) > 3e-3 + 1e-5 * np.abs(s_or)
-    assert bad.mean() <= 1e-4, bad.mean()
+    # every slot except those the oracle flags margin-ambiguous in some frame (R18), to the per-slot R20 tolerance
+    worst, n_amb = assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "config3 coadd of 3 frames")
+    print("config3 coadd: worst %.3f x tol, %d ambiguous slots of %d pixels accumulated" % (worst, n_amb, ref["n_px"]))

@@ -193,14 +193,14 @@ def test_gaussian_star_found_at_its_peak_pixel_with_signed_centroid():
     assert d["cx"][1] > 0.05 and abs(d["cy"][1]) < 1e-12 and d["cy"][0] < -0.05 and abs(d["cx"][0]) < 1e-12
 
 
-def test_catalogue_order_is_tile_major():
+def test_catalogue_order_is_raster():
+    """R-D6: ascending y * W + x, whatever tiling an implementation uses (the points straddle 64 x 32 blocks)."""
     cal = np.zeros((70, 200))
     for (y, x) in [(2, 150), (3, 10), (31, 70), (33, 5), (40, 199), (69, 64)]:
         cal[y, x] = 10.0 + x
     mask = np.ones(cal.shape, np.uint8)
     bkg, nse = ob.background(cal, mask, B=16)
     d = ob.detect(cal, mask, bkg, nse, B=16)
-    # tiles are 64 wide, 32 tall: row of tiles 0 holds y < 32 (x-tiles 0, 1, 2), then y in 32..63, then y >= 64
-    assert list(zip(d["y"], d["x"])) == [(3, 10), (31, 70), (2, 150), (33, 5), (40, 199), (69, 64)]
-    r = ob.detect(cal, mask, bkg, nse, B=16, tile=None)
-    assert list(zip(r["y"], r["x"])) == [(2, 150), (3, 10), (31, 70), (33, 5), (40, 199), (69, 64)]
+    assert list(zip(d["y"], d["x"])) == [(2, 150), (3, 10), (31, 70), (33, 5), (40, 199), (69, 64)]
+    key = d["y"].astype(np.int64) * 200 + d["x"]
+    assert np.all(np.diff(key) > 0)
