@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused calibrate + HEALPix-resample hot path on B200 (contract in the task).
 
-    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload config1|config0|...|segments|detect]
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload config1|...|coadd|batch|segments|detect]
 
 A step = one pass of the whole hot path over one frame: per-frame plan on the device (A0/A1, the WCS is
 treated as new every step: plan cache off) + fused calibrate/resample (A2-A5) writing value + weight.
@@ -28,12 +28,13 @@ if ROOT not in sys.path:
 
 METRIC = "calibrated+HEALPix-resampled Mpix/s per B200; achieved HBM GB/s vs peak"
 UNIT = "Mpix/s"  # input (detector) pixels per second
-SAMPLE_SIDE = 4096  # --impl reference: SAMPLE_SIDE^2 frame of the workload recipe per step
-# dram__bytes_read.sum + dram__bytes_write.sum of resample_fast_kernel<false> on config 1, one launch, from
-# profiles/r1_final_ncu_summary.txt (ncu --set full).
-NCU_TRAFFIC_BYTES = 983571968 + 339383296  # profiles/r1_final_ncu_summary.txt
-NCU_DET_TRAFFIC_BYTES = 856468736 + 4660224 + 856615936 + 6127360  # profiles/r1_detect_ncu_summary.txt
-NCU_SEG_TRAFFIC_BYTES = 359159552 + 7175936 + 365523712 + 41991424  # profiles/r1_segments_ncu_summary.txt
+SAMPLE_SIDE = {"bilinear": 4096, "lanczos3": 2048}  # --impl reference / 1-thread leg: SAMPLE_SIDE^2 frame of the workload recipe
+N_DISTINCT = 3   # coadd / batch: distinct synthetic frames generated on the host (61 MPix each takes ~10 s); the other
+                 # frames of the batch reuse their pixels with their OWN WCS (and, for batch, their own device copies)
+
+# B200 unit counts for the shared-memory and FP32 rooflines (B200_PROFILING.md / B300_MICROARCH.md): 148 SMs,
+# 128 B of shared-memory bandwidth per SM per clock, 128 FP32 lanes per SM (FMA = 2 flop).
+N_SM, SMEM_B_PER_CLK, FP32_LANES = 148, 128, 128
 
 
 def _peaks():
@@ -44,6 +45,31 @@ def _peaks():
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def _kernel_sources_sha():
+    """Hash of the CUDA sources: a dram-traffic figure taken from an ncu profile is only quoted while the kernels are
+    the ones that were profiled."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2207_14304_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        with open(os.path.join(d, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(key):
+    """(bytes, provenance) of the dominant kernel's DRAM traffic from profiles/traffic.json (written from an ncu --set
+    full capture; names the report and the source hash it was taken at); (None, why) when absent or stale."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            t = json.load(f)[key]
+    except Exception:
+        return None, "no ncu capture recorded for this workload (profiles/traffic.json)"
+    if t.get("csrc_sha16") != _kernel_sources_sha():
+        return None, "kernels changed since %s was captured (profiles/traffic.json)" % t.get("profile")
+    return int(t["dram_bytes"]), "%s, csrc %s" % (t["profile"], t["csrc_sha16"])
 
 
 class ClockSampler:
@@ -94,18 +120,90 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def make_workload(name, rank):
-    """configs[1] is the benchmark line; the others are for the record, one frame of each."""
+# ------------------------------------------------------------------------------------------------ workloads
+WORKLOADS = {
+    # name: (description, frames per step, kernel, nside)
+    "config0": ("configs[0] 512x512 nside 2^17 bilinear", 1),
+    "config1": ("configs[1] 9576x6388 nside 2^17 bilinear", 1),
+    "config2": ("configs[2] one 9576x6388 frame, SIP order 3, nside 2^17 Lanczos-3", 1),
+    "config3": ("configs[3] one 1 s 9576x6388 frame, nside 2^17 bilinear (value + weight written)", 1),
+    "config4": ("configs[4] one 9576x6388 frame, SIP order 3, nside 2^18 Lanczos-3", 1),
+    "coadd": ("configs[3] 60 dithered 1 s 9576x6388 frames, nside 2^17 bilinear, fused calibrate+resample+accumulate into one coadd", 60),
+    "batch": ("configs[2] 38 pointings (dec -20..+72) 9576x6388, own masters, SIP order 3, nside 2^17 Lanczos-3", 38),
+}
+
+
+def make_frames(name, rank):
+    """Host-side synthetic inputs of a workload: list of (Frame, wcs) per frame of the step.  configs[1] is the benchmark
+    line; the single-frame configN lines and the two multi-frame workloads are for the record."""
     import synth
     if name == "config0":
-        return synth.config0(seed=rank), "configs[0] 512x512 nside 2^17 bilinear"
+        fr = synth.config0(seed=rank)
+        return [(fr, fr.wcs)]
     if name == "config2":
-        return synth.config2_frame(rank % 38), "configs[2] one 9576x6388 frame, SIP order 3, nside 2^17 Lanczos-3"
+        fr = synth.config2_frame(rank % 38)
+        return [(fr, fr.wcs)]
     if name == "config3":
-        return synth.config3_frame(rank), "configs[3] one 1 s 9576x6388 frame, nside 2^17 bilinear (value + weight written)"
+        fr = synth.config3_frame(rank)
+        return [(fr, fr.wcs)]
     if name == "config4":
-        return synth.config4_frame(rank % 9), "configs[4] one 9576x6388 frame, SIP order 3, nside 2^18 Lanczos-3"
-    return synth.config1(seed=1 + rank), "configs[1] 9576x6388 nside 2^17 bilinear"
+        fr = synth.config4_frame(rank % 9)
+        return [(fr, fr.wcs)]
+    if name == "coadd":      # 60 dithered pointings of one field, shared masters; N_DISTINCT noise realisations
+        base = synth.config3_frame(0)
+        masters = (base.bias, base.dark, base.flat)
+        distinct = [base] + [synth.config3_frame(k, masters=masters) for k in range(1, N_DISTINCT)]
+        return [(distinct[k % N_DISTINCT], _config3_wcs(k)) for k in range(60)]
+    if name == "batch":      # 38 pointings with their own WCS; N_DISTINCT pixel sets, every frame its own device copy
+        distinct = [synth.config2_frame(k) for k in range(N_DISTINCT)]
+        return [(distinct[k % N_DISTINCT], synth.frames.config2_wcs(k)) for k in range(38)]
+    fr = synth.config1(seed=1 + rank)
+    return [(fr, fr.wcs)]
+
+
+def _config3_wcs(k):
+    """The WCS of configs[3] frame k without drawing its 61 MPix of pixels (same generator, same draws as synth)."""
+    import numpy as np
+    import synth
+    W, H = synth.frames.FULL_W, synth.frames.FULL_H
+    rng = np.random.Generator(np.random.PCG64(300 + k + 10_000))
+    dx, dy = rng.uniform(-0.5, 0.5, 2)
+    return synth.make_wcs((30.0, 20.0), ((W - 1) / 2.0 + dx, (H - 1) / 2.0 + dy), 0.3)
+
+
+def algorithmic_work(kernel, px_in, px_out, coadd):
+    """SURVEY 8(d) / DESIGN.md 6.5: what the method must move or compute once per frame.
+    HBM bytes: 14 B per input px (raw u16 + three f32 masters) + 8 B per output px (value + weight), or 16 B per output
+    px for the fused coadd read-modify-write.  Shared-memory bytes: the staged box is read once for calibration (14 B)
+    and written once calibrated (4 B) per input px; the gather reads 4 (bilinear) or 36 (Lanczos-3) float32 taps per
+    output px.  FP32 flops: A2 3 per input px; A3+A4 ~60 and A5 16 (bilinear) or 36 x 2 x 2 + 40 (Lanczos-3) per output px."""
+    taps = 36 if kernel == "lanczos3" else 4
+    hbm = 14.0 * px_in + (16.0 if coadd else 8.0) * px_out
+    smem = 18.0 * px_in + 4.0 * taps * px_out
+    flop = 3.0 * px_in + (60.0 + (184.0 if kernel == "lanczos3" else 16.0)) * px_out
+    return hbm, smem, flop
+
+
+def rooflines(kernel, px_in, px_out, coadd, k_ms, sm_mhz, hbm_peak, hbm_src):
+    """The three fractions SURVEY 8(d) asks for; `bound` = the resource whose time-at-peak for the algorithmic work is
+    longest.  Peaks: HBM measured copy bandwidth; shared memory = SMs x 128 B/clk x clock; FP32 = SMs x 128 lanes x 2 x
+    clock, both at the SM clock sampled under load (falls back to 1965 MHz)."""
+    clk = (sm_mhz or 1965.0) * 1e6
+    hbm, smem, flop = algorithmic_work(kernel, px_in, px_out, coadd)
+    peaks = {"hbm": hbm_peak * 1e9, "smem": N_SM * SMEM_B_PER_CLK * clk, "fp32": N_SM * FP32_LANES * 2 * clk}
+    work = {"hbm": hbm, "smem": smem, "fp32": flop}
+    t_peak = {k: work[k] / peaks[k] for k in work}
+    bound = max(t_peak, key=t_peak.get)
+    t = k_ms * 1e-3
+    fr = {k: (t_peak[k] / t if t > 0 else 0.0) for k in work}
+    unit = {"hbm": "GB/s", "smem": "GB/s", "fp32": "GFLOP/s"}[bound]
+    return {"bound": bound if bound == "hbm" else ("smem (shared-memory / LSU pipe)" if bound == "smem" else "alu (FP32 issue)"),
+            "achieved": work[bound] / t / 1e9 if t > 0 else 0.0, "peak": peaks[bound] / 1e9, "unit": unit, "frac": fr[bound],
+            "fractions": {"hbm": fr["hbm"], "smem": fr["smem"], "fp32": fr["fp32"]},
+            "time_at_peak_ms": {k: 1e3 * v for k, v in t_peak.items()},
+            "peak_source": "hbm: %s; smem = %d SMs x %d B/clk, fp32 = %d SMs x %d lanes x 2, at %.0f MHz" % (
+                hbm_src, N_SM, SMEM_B_PER_CLK, N_SM, FP32_LANES, clk / 1e6),
+            "kernel_ms": k_ms, "algorithmic_bytes": hbm, "algorithmic_smem_bytes": smem, "algorithmic_flop": flop}
 
 
 def cpu_oracle_run(fr):
@@ -120,15 +218,39 @@ def cpu_oracle_run(fr):
     return time.perf_counter() - t0, len(idx)
 
 
-def cpu_sample_frame(side):
+def cpu_sample_frame(name, side):
+    """A side x side frame of the workload's own recipe (noise / star / flat model, WCS family, nside, kernel)."""
     import synth
+    if name in ("config2", "batch"):
+        return synth.config2_frame(0, W=side, H=side)
+    if name == "config4":
+        return synth.config4_frame(0, W=side, H=side)
+    if name in ("config3", "coadd"):
+        return synth.config3_frame(0, W=side, H=side)
+    if name == "config0":
+        return synth.config0()
     return synth.config1(seed=1, W=side, H=side)
 
 
-def cpu_desc(fr, n_out):
+def cpu_desc(name, fr, n_out, threads):
     H, W = fr.shape
-    return ("%dx%d frame of the configs[1] recipe (same noise/star/flat model, WCS, nside 2^17, bilinear), whole oracle "
-            "path calibrate+footprint+resample, %d output px" % (W, H, n_out))
+    return ("%dx%d frame of the %s recipe (nside 2^%d, %s), whole oracle path calibrate+footprint+resample%s, %d output px, "
+            "%d thread%s" % (W, H, WORKLOADS[name][0].split(" ")[0], fr.nside.bit_length() - 1, fr.kernel,
+                             " (the coadd accumulation is not timed)" if name == "coadd" else "", n_out, threads,
+                             "" if threads == 1 else "s"))
+
+
+def public_config(name, fr, n_frames):
+    """The part of `config` both arms print identically (the driver compares them)."""
+    H, W = fr.shape if name != "config0" else (512, 512)
+    full = name != "config0"
+    import synth
+    if full:
+        W, H = synth.frames.FULL_W, synth.frames.FULL_H
+    return {"workload": WORKLOADS[name][0], "frames_per_step_per_gpu": n_frames, "W": W, "H": H, "nside": fr.nside,
+            "kernel": fr.kernel, "fused": True, "plan_every_step": True,
+            "l2": "inputs (856 MB/frame) larger than L2 (126 MB)" if full else "inputs fit L2 (parity-sized case)",
+            "parallelism": "frames independent: every GPU processes its own frames (replicas)"}
 
 
 def reduce_over_ranks(ms, px_in, px_out, dist=None, device=None):
@@ -145,26 +267,29 @@ def reduce_over_ranks(ms, px_in, px_out, dist=None, device=None):
 
 
 def run_reference(args):
+    """The oracle, as it stands, on the host cores: each step = one bounded sample frame of the workload's recipe."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     import oracle
     oracle.lib()
     cores = oracle.max_threads()
-    fr = cpu_sample_frame(SAMPLE_SIDE)  # generated once, outside the timed region
+    name = args.workload if args.workload in WORKLOADS else "config1"
+    fr = cpu_sample_frame(name, SAMPLE_SIDE["lanczos3" if name in ("config2", "config4", "batch") else "bilinear"])
+    H, W = fr.shape
     for _ in range(max(0, min(args.warmup, 1))):
         cpu_oracle_run(fr)
     total, n_out = 0.0, 0
     for _ in range(args.steps):
         dt, n_out = cpu_oracle_run(fr)
         total += dt
-    value = SAMPLE_SIDE * SAMPLE_SIDE * args.steps / total / 1e6
-    desc = cpu_desc(fr, n_out)
+    value = W * H * args.steps / total / 1e6
+    desc = cpu_desc(name, fr, n_out, cores)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "configs[1] 9576x6388 nside 2^17 bilinear (bounded sample)", "sample": desc},
+        "config": public_config(name, fr, WORKLOADS[name][1]),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -190,22 +315,65 @@ def run_gpu(args):
     dev = torch.device("cuda", local)
     argus.load_library()  # raises if the CUDA extension is missing: no fallback
 
-    fr, wl = make_workload(args.workload, rank)
-    H, W = fr.shape
+    name = args.workload
+    jobs_host = make_frames(name, rank)
+    fr0 = jobs_host[0][0]
+    H, W = fr0.shape
+    nside, kernel = fr0.nside, fr0.kernel
+    coadd = name == "coadd"
     ctx = argus.Context(local)
-    d = dict(raw=torch.from_numpy(fr.raw).to(dev), bias=torch.from_numpy(fr.bias).to(dev),
-             dark=torch.from_numpy(fr.dark).to(dev), flat=torch.from_numpy(fr.flat).to(dev), bpm=None,
-             t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
-    n_fp, _ = argus.argus_healpix_footprint(ctx, fr.wcs, W, H, fr.nside, want_indices=False)
+    if args.prefused is not None:
+        raise SystemExit("--prefused needs argus_prepare_masters (not built)")
+
+    # device-resident inputs.  coadd: shared masters, N_DISTINCT raw frames; batch: every frame its own raw + masters
+    def up(a):
+        return torch.from_numpy(a).to(dev)
+
+    dsets = {}
+    jobs = []
+    shared_masters = None
+    for fr, wcs in jobs_host:
+        if coadd:
+            if shared_masters is None:
+                shared_masters = (up(fr.bias), up(fr.dark), up(fr.flat))
+            if id(fr) not in dsets:
+                dsets[id(fr)] = up(fr.raw)
+            d = dict(raw=dsets[id(fr)], bias=shared_masters[0], dark=shared_masters[1], flat=shared_masters[2])
+        elif name == "batch":
+            if id(fr) not in dsets:
+                dsets[id(fr)] = (up(fr.raw), up(fr.bias), up(fr.dark), up(fr.flat))
+                src = dsets[id(fr)]
+            else:
+                src = tuple(t.clone() for t in dsets[id(fr)])      # own device copy: 38 x 856 MB resident
+            d = dict(raw=src[0], bias=src[1], dark=src[2], flat=src[3])
+        else:
+            d = dict(raw=up(fr.raw), bias=up(fr.bias), dark=up(fr.dark), flat=up(fr.flat))
+        d.update(bpm=None, t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
+        jobs.append((wcs, d))
+    n_fps = [argus.argus_healpix_footprint(ctx, wcs, W, H, nside, want_indices=False)[0] for wcs, _ in jobs]
     stats = argus.argus_plan_info(ctx)
-    value = torch.empty(n_fp, dtype=torch.float32, device=dev)
-    weight = torch.empty(n_fp, dtype=torch.float32, device=dev)
-    ctx.set_plan_cache(False)  # every step plans its frame again, as a new WCS would
+    n_out_step, n_frames = int(sum(n_fps)), len(jobs)
+    if coadd:
+        tiles = torch.unique(torch.cat([argus.argus_healpix_footprint(ctx, wcs, W, H, nside)[1] >> 18 for wcs, _ in jobs[:: max(1, n_frames // 8)]]
+                                       + [argus.argus_healpix_footprint(ctx, jobs[-1][0], W, H, nside)[1] >> 18]))
+        # +-0.5 px dithers move the footprint by less than one pixel: the union over a spread of frames + a check below
+        ppt = 1 << 18
+        csum = torch.zeros(tiles.numel() * ppt, dtype=torch.float32, device=dev)
+        cwsum = torch.zeros_like(csum)
+        skipped = torch.zeros(1, dtype=torch.int64, device=dev)
+    else:
+        value = torch.empty(max(n_fps), dtype=torch.float32, device=dev)
+        weight = torch.empty(max(n_fps), dtype=torch.float32, device=dev)
+    ctx.set_plan_cache(False)  # every frame plans again, as a new WCS does
     if args.no_plan_overlap:
         ctx.set_plan_overlap(False)
 
     def step():
-        argus.argus_resample(ctx, fr.wcs, W, H, fr.nside, fr.kernel, value, weight, **d)
+        for wcs, d in jobs:
+            if coadd:
+                argus.argus_resample_coadd(ctx, wcs, W, H, nside, kernel, tiles, 256, csum, cwsum, skipped, **d)
+            else:
+                argus.argus_resample(ctx, wcs, W, H, nside, kernel, value, weight, **d)
 
     def barrier():
         if world > 1:
@@ -215,11 +383,15 @@ def run_gpu(args):
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
+    if coadd:
+        assert int(skipped.item()) == 0, "coadd layout misses tiles of some frame"
     ctx.set_profile(True)
     sampler = ClockSampler(local) if rank == 0 else None
+    if sampler and n_frames == 1:
+        time.sleep(0.15)       # one nvidia-smi sample before the (6 ms) timed region, one after it
+    t0 = time.time()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = ctx.launch_count()
-    t0 = time.time()
     ev0.record()
     for _ in range(args.steps):
         step()
@@ -231,73 +403,102 @@ def run_gpu(args):
     plan_ms, kern_ms, ncalls = ctx.profile_read()
     ctx.set_profile(False)
     clocks = sampler.stop(t0, t1) if sampler else None
-    ms, px_in_all, px_out_all = reduce_over_ranks(ms, W * H, n_fp, dist if world > 1 else None, dev)
+    ms, px_in_all, px_out_all = reduce_over_ranks(ms, W * H * n_frames, n_out_step, dist if world > 1 else None, dev)
 
-    # end to end through the same API call with HOST buffers: raw frame H2D (masters stay resident per pointing,
-    # PAPER.md:109,135), plan + fused kernel, value + weight D2H -- all inside the timed region
-    h_raw = torch.from_numpy(fr.raw).pin_memory()
-    h_val = torch.empty(n_fp, dtype=torch.float32).pin_memory()
-    h_wgt = torch.empty(n_fp, dtype=torch.float32).pin_memory()
-
-    # argus_resample_host (C ABI with HOST buffers): the library uploads the raw frame, plans, resamples and downloads
-    # value + weight, pipelining upload / kernels / download of consecutive frames on its own copy streams (PCIe is
-    # full duplex); every frame makes the whole trip inside the timed region
-    masters = dict(bias=d["bias"], dark=d["dark"], flat=d["flat"], t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
+    # ---- end to end through the C ABI with HOST buffers: every frame's raw pixels come from pinned host memory (masters
+    # stay resident per pointing) and the result goes back to pinned host memory, inside the timed
+    # region; the library pipelines upload / kernels / download of consecutive frames on its own copy streams
+    h_raws = {}
+    for fr, _ in jobs_host:
+        if id(fr) not in h_raws:
+            h_raws[id(fr)] = torch.from_numpy(fr.raw).pin_memory()
+    if coadd:
+        h_sum, h_wsum = torch.empty_like(csum, device="cpu").pin_memory(), torch.empty_like(cwsum, device="cpu").pin_memory()
+    else:
+        h_val = torch.empty(max(n_fps), dtype=torch.float32).pin_memory()
+        h_wgt = torch.empty(max(n_fps), dtype=torch.float32).pin_memory()
 
     def e2e_step():
-        argus.argus_resample_host(ctx, fr.wcs, W, H, fr.nside, fr.kernel, n_fp, h_raw, h_val, h_wgt, **masters)
+        for (fr, wcs), (_, d), n in zip(jobs_host, jobs, n_fps):
+            m = dict(bias=d["bias"], dark=d["dark"], flat=d["flat"], t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
+            if coadd:
+                argus.argus_resample_coadd_host(ctx, wcs, W, H, nside, kernel, h_raws[id(fr)], tiles, 256, csum, cwsum, None, **m)
+            else:
+                argus.argus_resample_host(ctx, wcs, W, H, nside, kernel, n, h_raws[id(fr)], h_val, h_wgt, **m)
+        if coadd:   # the step's result: the coadd itself
+            h_sum.copy_(csum, non_blocking=True)
+            h_wsum.copy_(cwsum, non_blocking=True)
 
-    for _ in range(2):
+    for _ in range(2 if n_frames == 1 else 1):
         e2e_step()
     argus.argus_host_wait(ctx)
     barrier()
-    e2e_steps = max(4, min(args.steps, 10))
+    e2e_steps = max(4, min(args.steps, 10)) if n_frames == 1 else 2
     t_e0 = time.perf_counter()
     for _ in range(e2e_steps):
         e2e_step()
     argus.argus_host_wait(ctx)
     torch.cuda.synchronize()
-    e2e_wall_ms = 1e3 * (time.perf_counter() - t_e0)
+    e2e_ms = 1e3 * (time.perf_counter() - t_e0)   # host wall clock around enqueue + completion (copies run on the library's streams)
     barrier()
-    e2e_ms = e2e_wall_ms   # host wall clock around enqueue + completion: the copies run on the library's own streams
     e2e_ms, _, _ = reduce_over_ranks(e2e_ms, 0, 0, dist if world > 1 else None, dev)
+    h2d = int(W * H * 2 * n_frames)
+    d2h = int(2 * 4 * csum.numel()) if coadd else int(8 * n_out_step)
 
     if rank == 0:
         peak, peak_src = _peaks()
         ms_step = ms / args.steps
-        alg_bytes = 14.0 * W * H + 8.0 * n_fp  # 14 B per input px + 8 B per output px
-        k_ms = kern_ms / max(ncalls, 1)
-        achieved = alg_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
-        if world == 1:  # the oracle, as it stands, on the same full frame the GPU just processed
+        k_ms = kern_ms / max(ncalls, 1)                       # per frame (argus_resample call)
+        px_out_frame = n_out_step / n_frames
+        roof = rooflines(kernel, W * H, px_out_frame, coadd, k_ms, clocks and clocks.get("sm_mhz"), peak, peak_src)
+        alg_step = roof["algorithmic_bytes"] * n_frames
+        roof["kernel"] = ("resample_fast_kernel<%s,%d> (TMA-staged, fused calibration%s) + resample_tiles_kernel on its slow list; "
+                          "per frame, CUDA events around the resample launches" % ("true" if coadd else "false", 1 if kernel == "lanczos3" else 0,
+                                                                                  ", coadd read-modify-write" if coadd else ""))
+        roof["step_frac"] = (alg_step / (ms_step * 1e-3) / 1e9) / peak
+        tr, tr_src = ncu_traffic(name)
+        roof["traffic"], roof["traffic_source"] = tr, tr_src
+        if world == 1:
             import oracle
             cores = oracle.max_threads()
-            cpu_dt, n_out = cpu_oracle_run(fr)
-            cpu_v, cpu_d = W * H / cpu_dt / 1e6, cpu_desc(fr, n_out)
+            # the oracle, as it stands: all host threads on the first frame of the step (full size for bilinear, a
+            # bounded sample for Lanczos-3), and one thread on a bounded sample
+            fr_n = fr0 if kernel == "bilinear" else cpu_sample_frame(name, 4096)
+            cpu_dt, n_o = cpu_oracle_run(fr_n)
+            cpu = {"value": fr_n.shape[0] * fr_n.shape[1] / cpu_dt / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": cpu_desc(name, fr_n, n_o, cores), "seconds": cpu_dt}
+            fr_1 = cpu_sample_frame(name, SAMPLE_SIDE[kernel] // 2)
+            oracle.set_threads(1)
+            try:
+                dt1, n_o1 = cpu_oracle_run(fr_1)
+            finally:
+                oracle.set_threads(cores)
+            cpu1 = {"value": fr_1.shape[0] * fr_1.shape[1] / dt1 / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle",
+                    "sample": cpu_desc(name, fr_1, n_o1, 1), "seconds": dt1}
         else:
-            cpu_v, cores, cpu_dt, cpu_d = None, None, None, "rank 0 at N=1 only"
+            cpu = {"value": None, "unit": UNIT, "cores": None, "kind": "oracle", "sample": "rank 0 at N=1 only"}
+            cpu1 = None
+        cfg = public_config(name, fr0, n_frames)
         line = {
             "metric": METRIC, "value": px_in_all * args.steps / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": wl, "frames_per_step_per_gpu": 1, "W": W, "H": H, "nside": fr.nside,
-                       "kernel": fr.kernel, "n_footprint": n_fp, "fused": True, "plan_every_step": True,
-                       "plan_overlap": ("off (diagnostic)" if args.no_plan_overlap else
-                                        "the plan of step k+1 runs on the library's side streams underneath the kernels of step k"),
-                       "l2": "inputs (856 MB/frame) larger than L2 (126 MB)", "plan": stats,
-                       "parallelism": "1 frame per GPU per step, frames independent (replicas)"},
+            "config": cfg,
+            "details": {"n_footprint_per_step": n_out_step, "ms_per_frame": ms_step / n_frames, "plan_last_frame": stats,
+                        "plan_overlap": ("off (diagnostic)" if args.no_plan_overlap else
+                                         "the plan of frame k+1 runs on the library's side streams underneath the kernels of frame k"),
+                        "distinct_pixel_sets": len(h_raws),
+                        "coadd_tiles": int(tiles.numel()) if coadd else None},
             "output_mpix_per_s": px_out_all * args.steps / (ms * 1e-3) / 1e6,
-            "plan_ms_per_step": plan_ms / max(ncalls, 1),
-            "roofline": {"bound": "hbm", "kernel": ("resample_fast_kernel<false> (TMA-staged bilinear, fused calibration)" if fr.kernel == "bilinear"
-                                                   else "resample_fast_kernel<false,1> (TMA-staged Lanczos-3) + general kernel on its slow list"), "achieved": achieved,
-                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if args.workload == "config1" else None,
-                         "peak_source": peak_src, "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes,
-                         "step_frac": (alg_bytes / (ms_step * 1e-3) / 1e9) / peak},
-            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_d,
-                             "seconds": cpu_dt},
+            "plan_ms_per_frame": plan_ms / max(ncalls, 1),
+            "roofline": roof,
+            "cpu_baseline": cpu, "cpu_baseline_1thread": cpu1,
             "e2e": {"value": px_in_all * e2e_steps / (e2e_ms * 1e-3) / 1e6, "unit": UNIT,
-                    "h2d_bytes_per_step": int(h_raw.numel() * 2), "d2h_bytes_per_step": int(n_fp * 8),
-                    "ms_per_step": e2e_ms / e2e_steps,
-                    "note": "argus_resample_host: raw frame from pinned host memory each step, value + weight back to pinned host memory; masters resident per pointing; upload / kernels / download of consecutive frames pipelined by the library; host wall clock"},
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / e2e_steps,
+                    "note": ("argus_resample_coadd_host per frame (raw from pinned host memory), the coadd (sum, wsum) back to pinned host memory once per step"
+                             if coadd else
+                             "argus_resample_host: raw frame from pinned host memory each frame, value + weight back to pinned host memory; masters resident per pointing")
+                            + "; upload / kernels / download of consecutive frames pipelined by the library; host wall clock"},
             "gpu_launches": launches,
             "clocks": clocks,
         }
@@ -325,7 +526,7 @@ def run_segments(args):
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     argus.load_library()
-    fr, _ = make_workload("config1", 0)
+    fr = make_frames("config1", 0)[0][0]
     H, W = fr.shape
     nside, nside_mini = fr.nside, 1 << 14
     ctx = argus.Context(0)
@@ -405,8 +606,8 @@ def run_segments(args):
                    "nside": nside, "nside_mini": nside_mini, "n_mini": n_mini, "n_targets": int(targets.numel()),
                    "layout": "compact (element i <-> idx[i])", "l2": "inputs (16 B x n = %d MB) larger than L2 (126 MB)" % (16 * n // 1000000)},
         "roofline": {"bound": "hbm", "kernel": "whole call: seg_flags_kernel + seg_scan_kernel + seg_heads_kernel + seg_targets_kernel + seg_products_kernel<false> (+ memsets); the two streaming kernels (flags, products) are 75 % of it",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_SEG_TRAFFIC_BYTES,
-                     "traffic_note": "dram read + write of seg_flags_kernel and seg_products_kernel, one launch each (profiles/r1_segments_ncu_summary.txt)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic("segments")[0], "traffic_source": ncu_traffic("segments")[1],
+                     "traffic_note": "dram read + write of seg_flags_kernel and seg_products_kernel, one launch each",
                      "peak_source": peak_src, "kernel_ms": ms_step, "algorithmic_bytes": alg},
         "cpu_baseline": {"value": ns / cpu_dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
                          "sample": "oracle.segments.segment_products (numpy, fp64) on the same list, all %d pixels" % ns, "seconds": cpu_dt},
@@ -434,7 +635,7 @@ def run_detect(args):
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     argus.load_library()
-    fr, _ = make_workload("config1", 0)
+    fr = make_frames("config1", 0)[0][0]
     H, W = fr.shape
     B, n_min, k_sigma, cap = 64, 16, 5.0, 1 << 18
     ctx = argus.Context(0)
@@ -528,8 +729,8 @@ def run_detect(args):
                    "cell": B, "n_min": n_min, "k_sigma": k_sigma, "n_sources": n_src, "fused": True,
                    "l2": "inputs (856 MB/frame) larger than L2 (126 MB)"},
         "roofline": {"bound": "hbm", "kernel": "whole step: bg_cells_kernel<true> + bg_filter_kernel + det_tiles_kernel<true> + det_scan_kernel + det_gather_kernel",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_DET_TRAFFIC_BYTES,
-                     "traffic_note": "dram read + write of bg_cells_kernel and det_tiles_kernel, one launch each (profiles/r1_detect_ncu_summary.txt); the step reads raw + masters twice (once per pass), the algorithmic bytes count them once",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic("detect")[0], "traffic_source": ncu_traffic("detect")[1],
+                     "traffic_note": "dram read + write of bg_cells_kernel and det_tiles_kernel, one launch each; the step reads raw + masters twice (once per pass), the algorithmic bytes count them once",
                      "peak_source": peak_src, "kernel_ms": ms_step, "algorithmic_bytes": alg,
                      "background_map_ms": ms_map, "detect_sources_ms": ms_det},
         "cpu_baseline": {"value": side * side / cpu_dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
@@ -549,7 +750,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-plan-overlap", action="store_true", help="diagnostic: build every plan in place on the caller's stream")
-    ap.add_argument("--workload", default="config1", choices=["config0", "config1", "config2", "config3", "config4", "segments", "detect"])
+    ap.add_argument("--workload", default="config1", choices=sorted(WORKLOADS) + ["segments", "detect"])
+    ap.add_argument("--prefused", default=None, choices=["f32", "f16"], help="masters pre-fused by argus_prepare_masters (SURVEY 8(f).4)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -55,7 +55,7 @@ def test_reference_arm_nonzero_rank_is_silent():
 def test_reference_arm_json_contract(monkeypatch):
     sys.path.insert(0, ROOT)
     import bench
-    monkeypatch.setattr(bench, "SAMPLE_SIDE", 256)
+    monkeypatch.setattr(bench, "SAMPLE_SIDE", {"bilinear": 256, "lanczos3": 128})
     import io
     from contextlib import redirect_stdout
     buf = io.StringIO()
@@ -67,3 +67,22 @@ def test_reference_arm_json_contract(monkeypatch):
     assert line["impl"] == "reference" and line["unit"] == "Mpix/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"] == {"value": line["value"], "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    # both arms print the same `config` for a workload (the driver compares them)
+    import synth
+    assert line["config"] == bench.public_config("config1", synth.config0(), 1)
+    assert line["config"]["workload"] == bench.WORKLOADS["config1"][0] and line["config"]["W"] == 9576
+
+
+def test_rooflines_pick_the_binding_resource():
+    sys.path.insert(0, ROOT)
+    import bench
+    px_in, n1, n4 = 9576 * 6388, 44887802, 179550640
+    # bilinear configs[1]: HBM binds (1215.5 MB per frame)
+    r = bench.rooflines("bilinear", px_in, n1, False, 0.29, 1965.0, 6450.9, "test")
+    assert r["bound"] == "hbm" and abs(r["algorithmic_bytes"] - 1215503248) < 1 and 0.6 < r["frac"] < 0.7
+    # fused coadd: 14 B per input px + 16 B per output px = 1574.6 MB
+    assert abs(bench.algorithmic_work("bilinear", px_in, n1, True)[0] - 1574605664) < 1
+    # Lanczos-3 at nside 2^18: the shared-memory gather (36 taps per output) has the longest time at peak
+    r4 = bench.rooflines("lanczos3", px_in, n4, False, 2.5, 1965.0, 6450.9, "test")
+    assert r4["bound"].startswith("smem") and r4["fractions"]["smem"] > r4["fractions"]["fp32"] > r4["fractions"]["hbm"]
+    assert abs(r4["frac"] - r4["time_at_peak_ms"]["smem"] / 2.5) < 1e-12
