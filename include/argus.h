@@ -107,7 +107,16 @@ typedef struct argus_frame {
     float flat_min;       /* !(flat >= flat_min) is masked */
     const float* cal;     /* used when raw == NULL: calibrated ADU */
     const uint8_t* mask;  /* used when raw == NULL: 1 = good, 0 = masked */
+    /* Pre-fused masters (argus_prepare_masters below).  masters_format != 0 with raw != NULL: the
+     * calibration is (raw - offset) * gain with the two arrays argus_prepare_masters wrote (float32 or binary16 as the
+     * format says); bias, dark, flat, bpm, t_exp and flat_min are then ignored (they are folded into the two arrays). */
+    const void* offset;   /* ADU: bias + dark * t_exp */
+    const void* gain;     /* 1 / flat; NaN = invalid pixel */
+    int32_t masters_format; /* 0 = bias / dark / flat; ARGUS_MASTERS_F32; ARGUS_MASTERS_F16 */
+    int32_t reserved;
 } argus_frame;
+
+enum { ARGUS_MASTERS_F32 = 1, ARGUS_MASTERS_F16 = 2 };
 
 /* Coadd buffer layout: sorted tile ids at resolution nside_tile (NSIDE = 256 in the
  * paper); each tile owns ppt = (nside/nside_tile)^2 consecutive nested pixels:
@@ -156,6 +165,19 @@ int64_t argus_launch_count(const argus_ctx* ctx);
 int argus_calibrate(argus_ctx* ctx, const uint16_t* raw, const float* bias, const float* dark,
                     const float* flat, const uint8_t* bpm, int64_t W, int64_t H, float t_exp,
                     int32_t sat_adu, float flat_min, float* cal_out, uint8_t* mask_out, void* stream);
+
+/* Pre-fused masters (the calibration of PAPER.md:141 with everything that depends only on the masters
+ * formed once per pointing and exposure time).  Per pixel:
+ *   offset = bias + dark * t_exp
+ *   gain   = 1 / flat; NaN where flat < flat_min or not finite, bias or dark not finite, bpm != 0 (bpm may be NULL), or
+ *            where offset or gain cannot be represented in the storage format
+ * format ARGUS_MASTERS_F32: float32 arrays (10 B per input pixel on the hot path instead of 14; results stay within
+ * north_star's tolerance of the definition); ARGUS_MASTERS_F16: IEEE binary16 arrays, round to nearest even (6 B per
+ * pixel; NOT within that tolerance: a 1000-ADU offset is stored to 0.25 ADU -- DESIGN.md section 12 has the numbers).
+ * offset_out / gain_out: DEVICE, W * H elements of the format, 16-byte aligned for the vector paths.  Asynchronous. */
+int argus_prepare_masters(argus_ctx* ctx, const float* bias, const float* dark, const float* flat, const uint8_t* bpm,
+                          int64_t W, int64_t H, float t_exp, float flat_min, int format, void* offset_out, void* gain_out,
+                          void* stream);
 
 /* A0 + A1: builds the resampling plan for (wcs, W, H, nside) on the device and reports the footprint.
  *   idx_out  : device int64[capacity] or NULL.  When non-NULL receives the footprint: all nested pixel

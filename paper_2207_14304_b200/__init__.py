@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     argus_detect_sources,
     argus_healpix_footprint,
     argus_plan_info,
+    argus_prepare_masters,
     argus_resample,
     argus_resample_coadd,
     argus_resample_host,

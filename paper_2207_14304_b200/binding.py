@@ -11,6 +11,7 @@ import os
 import torch
 
 ARGUS_BILINEAR, ARGUS_LANCZOS3 = 0, 1
+ARGUS_MASTERS_F32, ARGUS_MASTERS_F16 = 1, 2
 ARGUS_OPT_PLAN_CACHE = 1
 ARGUS_OPT_PROFILE = 2
 ARGUS_OPT_FAST_PATH = 3
@@ -20,7 +21,7 @@ _KERNELS = {"bilinear": ARGUS_BILINEAR, "lanczos3": ARGUS_LANCZOS3, 0: 0, 1: 1}
 
 EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
-    "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_healpix_footprint", "argus_resample",
+    "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_prepare_masters", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
     "argus_resample_host", "argus_resample_coadd_host", "argus_host_wait", "argus_segment_products", "argus_background_map", "argus_detect_sources",
 ]
@@ -41,7 +42,8 @@ class _Wcs(C.Structure):
 class _Frame(C.Structure):
     _fields_ = [("raw", C.c_void_p), ("bias", C.c_void_p), ("dark", C.c_void_p), ("flat", C.c_void_p),
                 ("bpm", C.c_void_p), ("t_exp", C.c_float), ("sat_adu", C.c_int32), ("flat_min", C.c_float),
-                ("cal", C.c_void_p), ("mask", C.c_void_p)]
+                ("cal", C.c_void_p), ("mask", C.c_void_p), ("offset", C.c_void_p), ("gain", C.c_void_p),
+                ("masters_format", C.c_int32), ("reserved", C.c_int32)]
 
 
 class _Coadd(C.Structure):
@@ -89,6 +91,7 @@ def load_library():
     L.argus_launch_count.argtypes = [vp]
     L.argus_launch_count.restype = i64
     L.argus_calibrate.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, f32, i32, f32, vp, vp, vp]
+    L.argus_prepare_masters.argtypes = [vp, vp, vp, vp, vp, i64, i64, f32, f32, C.c_int, vp, vp, vp]
     L.argus_healpix_footprint.argtypes = [vp, C.POINTER(_Wcs), i64, i64, i64, vp, sz, C.POINTER(sz), vp]
     L.argus_resample.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, vp, sz, vp, vp, vp]
     L.argus_coadd_accumulate.argtypes = [vp, C.POINTER(_Coadd), i64, vp, vp, vp, vp, vp, sz, vp, vp]
@@ -156,9 +159,18 @@ def _stream(stream=None):
 
 
 def _frame_struct(raw=None, bias=None, dark=None, flat=None, bpm=None, t_exp=0.0, sat_adu=65535, flat_min=0.1,
-                  cal=None, mask=None) -> _Frame:
+                  cal=None, mask=None, offset=None, gain=None) -> _Frame:
     f = _Frame()
-    if raw is not None:
+    if raw is not None and offset is not None:      # pre-fused masters (argus_prepare_masters): float32 or float16 tensors
+        if offset.dtype != gain.dtype or offset.dtype not in (torch.float32, torch.float16):
+            raise TypeError("offset and gain must both be float32 or both float16")
+        f.raw = _dev(raw, torch.uint16, "raw")
+        f.offset = _dev(offset, offset.dtype, "offset")
+        f.gain = _dev(gain, gain.dtype, "gain")
+        f.masters_format = ARGUS_MASTERS_F32 if offset.dtype == torch.float32 else ARGUS_MASTERS_F16
+        if offset.shape != raw.shape or gain.shape != raw.shape:
+            raise ValueError("masters must have the frame's shape")
+    elif raw is not None:
         f.raw = _dev(raw, torch.uint16, "raw")
         f.bias = _dev(bias, torch.float32, "bias")
         f.dark = _dev(dark, torch.float32, "dark")
@@ -263,6 +275,26 @@ def argus_calibrate(ctx, raw, bias, dark, flat, bpm, t_exp, sat_adu=65535, flat_
                                         _dev(mask_out, torch.uint8, "mask_out"), _stream(stream))
     _check(ctx, rc, "argus_calibrate")
     return cal_out, mask_out
+
+
+def argus_prepare_masters(ctx, bias, dark, flat, bpm, t_exp, flat_min=0.1, dtype=torch.float32, offset_out=None,
+                          gain_out=None, stream=None):
+    """offset = bias + dark * t_exp and gain = 1 / flat (NaN = invalid) as float32 or float16 CUDA
+    tensors, once per pointing.  Returns (offset, gain): pass them as offset= / gain= instead of bias= / dark= / flat=."""
+    if dtype not in (torch.float32, torch.float16):
+        raise TypeError("dtype must be torch.float32 or torch.float16")
+    H, W = bias.shape
+    if offset_out is None:
+        offset_out = torch.empty((H, W), dtype=dtype, device=bias.device)
+    if gain_out is None:
+        gain_out = torch.empty((H, W), dtype=dtype, device=bias.device)
+    rc = load_library().argus_prepare_masters(
+        ctx._h, _dev(bias, torch.float32, "bias"), _dev(dark, torch.float32, "dark"), _dev(flat, torch.float32, "flat"),
+        _dev(bpm, torch.uint8, "bpm", allow_none=True), W, H, float(t_exp), float(flat_min),
+        ARGUS_MASTERS_F32 if dtype == torch.float32 else ARGUS_MASTERS_F16, _dev(offset_out, dtype, "offset_out"),
+        _dev(gain_out, dtype, "gain_out"), _stream(stream))
+    _check(ctx, rc, "argus_prepare_masters")
+    return offset_out, gain_out
 
 
 def argus_healpix_footprint(ctx, wcs, W, H, nside, idx_out=None, want_indices=True, stream=None):

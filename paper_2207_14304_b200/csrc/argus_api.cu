@@ -595,7 +595,17 @@ static void mark_slot_read(argus_ctx* c, cudaStream_t caller) {
 
 static int make_frameargs(const argus_frame* fr, int64_t W, int64_t H, FrameArgs* f, bool* fused) {
     memset(f, 0, sizeof(*f));
-    if (fr->raw) {
+    if (fr->raw && fr->masters_format != 0) {
+        if (fr->masters_format != ARGUS_MASTERS_F32 && fr->masters_format != ARGUS_MASTERS_F16) return ARGUS_ERR_SHAPE;
+        if (!fr->offset || !fr->gain) return ARGUS_ERR_NULL;
+        if (fr->sat_adu < 0) return ARGUS_ERR_SHAPE;
+        const size_t es = fr->masters_format == ARGUS_MASTERS_F32 ? 4 : 2;
+        if (!aligned(fr->raw, 2) || !aligned(fr->offset, es) || !aligned(fr->gain, es)) return ARGUS_ERR_ALIGN;
+        f->raw = fr->raw; f->offset = fr->offset; f->gain = fr->gain; f->pre = fr->masters_format;
+        f->sat_adu = fr->sat_adu; f->t_exp = 0.f; f->flat_min = 1.f;
+        f->vec_ok = (W % 4 == 0) && (W * H < (1ll << 31)) && aligned(fr->raw, 8) && aligned(fr->offset, 4 * es) && aligned(fr->gain, 4 * es);
+        *fused = true;
+    } else if (fr->raw) {
         if (!fr->bias || !fr->dark || !fr->flat) return ARGUS_ERR_NULL;
         if (!(fr->flat_min > 0.0f) || !(fr->flat_min < INFINITY) || fr->sat_adu < 0) return ARGUS_ERR_SHAPE;
         if (!aligned(fr->raw, 2) || !aligned(fr->bias, 4) || !aligned(fr->dark, 4) || !aligned(fr->flat, 4)) return ARGUS_ERR_ALIGN;
@@ -635,6 +645,27 @@ extern "C" int argus_calibrate(argus_ctx* c, const uint16_t* raw, const float* b
                (!bpm || aligned(bpm, 4)) && aligned(cal_out, 16) && aligned(mask_out, 4);
     CUDA_TRY(c, cudaSetDevice(c->device));
     calibrate_kernel<<<c->sm_count * 8, 256, 0, (cudaStream_t)stream>>>(f, n, cal_out, mask_out);
+    c->n_launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+// ------------------------------------------------------------------------ pre-fused masters (8(f).4)
+extern "C" int argus_prepare_masters(argus_ctx* c, const float* bias, const float* dark, const float* flat, const uint8_t* bpm,
+                                     int64_t W, int64_t H, float t_exp, float flat_min, int format, void* offset_out,
+                                     void* gain_out, void* stream) {
+    if (!c || !bias || !dark || !flat || !offset_out || !gain_out) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20)) return ARGUS_ERR_SHAPE;
+    if (format != ARGUS_MASTERS_F32 && format != ARGUS_MASTERS_F16) return ARGUS_ERR_SHAPE;
+    if (!(flat_min > 0.0f) || !(flat_min < INFINITY) || !(fabsf(t_exp) < INFINITY)) return ARGUS_ERR_SHAPE;
+    const size_t es = format == ARGUS_MASTERS_F32 ? 4 : 2;
+    if (!aligned(bias, 4) || !aligned(dark, 4) || !aligned(flat, 4) || !aligned(offset_out, es) || !aligned(gain_out, es)) return ARGUS_ERR_ALIGN;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    const long long n = W * H;
+    if (format == ARGUS_MASTERS_F32)
+        prepare_masters_kernel<1><<<c->sm_count * 8, 256, 0, (cudaStream_t)stream>>>(bias, dark, flat, bpm, n, t_exp, flat_min, offset_out, gain_out);
+    else
+        prepare_masters_kernel<2><<<c->sm_count * 8, 256, 0, (cudaStream_t)stream>>>(bias, dark, flat, bpm, n, t_exp, flat_min, offset_out, gain_out);
     c->n_launches++;
     CUDA_TRY(c, cudaGetLastError());
     return ARGUS_OK;
@@ -701,7 +732,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 
 // TMA descriptors for (raw, bias, dark, flat): 2-D tensors {W, H}, boxes {40..72 step 8} x {48, 56, 64}, zero fill outside.
 static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
-    if (!c->fast_enabled || !f.raw || f.bpm) return false;
+    if (!c->fast_enabled || !f.raw || f.bpm || f.pre) return false;
     if (W % 8 != 0 || W < 8 || !aligned(f.raw, 16) || !aligned(f.bias, 16) || !aligned(f.dark, 16) || !aligned(f.flat, 16)) return false;
     if (!c->encode_tried) {
         c->encode_tried = true;

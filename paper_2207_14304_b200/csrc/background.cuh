@@ -44,7 +44,10 @@ __device__ __forceinline__ void bg_load4(const FrameArgs& f, int W, int H, int x
     if (y >= H || x >= x_end) { v[0] = v[1] = v[2] = v[3] = nanf_(); return; }
     if (f.vec_ok && x + 3 < x_end) {
         size_t o = (size_t)y * W + x;
-        if (FUSED) {
+        if (FUSED && f.pre) {
+            const float4 c = calib4_pre<false>(f, o);
+            v[0] = c.x; v[1] = c.y; v[2] = c.z; v[3] = c.w;
+        } else if (FUSED) {
             uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
             float4 b = __ldg(reinterpret_cast<const float4*>(f.bias + o));
             float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));

@@ -10,6 +10,8 @@
 //              weight -- or accumulates them into the coadd buffer.
 // Tiles whose box has no masked pixel take a branch-free fast path (weight == 1).
 #pragma once
+#include <cuda_fp16.h>
+
 #include "common.cuh"
 #include "plan.cuh"
 
@@ -28,6 +30,11 @@ struct FrameArgs {
     float t_exp, flat_min;
     int sat_adu;
     int vec_ok;   // W % 4 == 0 and all base pointers 16-byte aligned
+    // pre-fused masters (argus_prepare_masters): offset = bias + dark * t_exp, gain = 1 / flat with NaN
+    // where the pixel is invalid; float32 (pre = 1) or binary16 (pre = 2).  pre = 0: bias / dark / flat above.
+    const void* offset;
+    const void* gain;
+    int pre;
 };
 
 struct CoaddArgs {
@@ -60,10 +67,39 @@ __device__ __forceinline__ float calib_sel(float r, float b, float d, float fl, 
     return PRECISE ? calib_px_precise(r, b, d, fl, bad, t_exp, flat_min) : calib_px(r, b, d, fl, bad, t_exp, flat_min);
 }
 
+// A2 with pre-fused masters (R-M4): cal = (raw - offset) * gain; masked (NaN) where raw is saturated or the gain is NaN.
+template <bool PRECISE>
+__device__ __forceinline__ float calib_pre(float r, float off, float g, bool bad) {
+    const float c = PRECISE ? (float)(((double)r - (double)off) * (double)g) : (r - off) * g;
+    return (!bad && fabsf(c) < INFINITY) ? c : nanf_();
+}
+__device__ __forceinline__ float pre_load(const void* p, size_t o, int pre) {
+    return pre == 1 ? reinterpret_cast<const float*>(p)[o] : __half2float(reinterpret_cast<const __half*>(p)[o]);
+}
+// four consecutive pixels at element offset o (16-byte / 8-byte aligned there)
+__device__ __forceinline__ float4 pre_load4(const void* p, size_t o, int pre) {
+    if (pre == 1) return __ldg(reinterpret_cast<const float4*>(reinterpret_cast<const float*>(p) + o));
+    const uint2 h = __ldg(reinterpret_cast<const uint2*>(reinterpret_cast<const __half*>(p) + o));
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&h.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&h.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+template <bool PRECISE>
+__device__ __forceinline__ float4 calib4_pre(const FrameArgs& f, size_t o) {
+    const uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
+    const float4 off = pre_load4(f.offset, o, f.pre), g = pre_load4(f.gain, o, f.pre);
+    const int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
+    return make_float4(calib_pre<PRECISE>((float)r0, off.x, g.x, r0 >= f.sat_adu), calib_pre<PRECISE>((float)r1, off.y, g.y, r1 >= f.sat_adu),
+                       calib_pre<PRECISE>((float)r2, off.z, g.z, r2 >= f.sat_adu), calib_pre<PRECISE>((float)r3, off.w, g.w, r3 >= f.sat_adu));
+}
+
 template <bool FUSED, bool PRECISE = false>
 __device__ __forceinline__ float load_px(const FrameArgs& f, int W, int H, int gx, int gy) {
     if (gx < 0 || gx >= W || gy < 0 || gy >= H) return nanf_();
     size_t o = (size_t)gy * W + gx;
+    if (FUSED && f.pre) {
+        const int r = f.raw[o];
+        return calib_pre<PRECISE>((float)r, pre_load(f.offset, o, f.pre), pre_load(f.gain, o, f.pre), r >= f.sat_adu);
+    }
     if (FUSED) {
         int r = f.raw[o];
         bool bad = (r >= f.sat_adu) || (f.bpm && f.bpm[o] != 0);
@@ -110,7 +146,9 @@ __device__ __forceinline__ int stage_box(const FrameArgs& f, int W, int H, int g
         float4 o4;
         if (f.vec_ok && (unsigned)gy < (unsigned)H && gx >= 0 && gx + 3 < W) {
             unsigned o = (unsigned)gy * (unsigned)W + (unsigned)gx;   // vec_ok implies W*H < 2^31
-            if (FUSED) {
+            if (FUSED && f.pre) {
+                o4 = calib4_pre<PRECISE>(f, o);
+            } else if (FUSED) {
                 uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
                 float4 b = __ldg(reinterpret_cast<const float4*>(f.bias + o));
                 float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));
@@ -443,16 +481,22 @@ __global__ void __launch_bounds__(256) calibrate_kernel(FrameArgs f, long long n
         long long n4 = n >> 2;
         for (long long v = (long long)blockIdx.x * 256 + threadIdx.x; v < n4; v += stride) {
             size_t o = (size_t)v * 4;
-            uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
-            float4 b = __ldg(reinterpret_cast<const float4*>(f.bias + o));
-            float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));
-            float4 fl = __ldg(reinterpret_cast<const float4*>(f.flat + o));
-            unsigned bp = f.bpm ? __ldg(reinterpret_cast<const unsigned*>(f.bpm + o)) : 0u;
-            int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
-            float c0 = calib_px((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
-            float c1 = calib_px((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
-            float c2 = calib_px((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
-            float c3 = calib_px((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+            float c0, c1, c2, c3;
+            if (f.pre) {
+                const float4 c4 = calib4_pre<false>(f, o);
+                c0 = c4.x; c1 = c4.y; c2 = c4.z; c3 = c4.w;
+            } else {
+                uint2 rw = __ldg(reinterpret_cast<const uint2*>(f.raw + o));
+                float4 b = __ldg(reinterpret_cast<const float4*>(f.bias + o));
+                float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));
+                float4 fl = __ldg(reinterpret_cast<const float4*>(f.flat + o));
+                unsigned bp = f.bpm ? __ldg(reinterpret_cast<const unsigned*>(f.bpm + o)) : 0u;
+                int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
+                c0 = calib_px((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
+                c1 = calib_px((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
+                c2 = calib_px((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
+                c3 = calib_px((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+            }
             unsigned mk = (c0 == c0 ? 1u : 0u) | (c1 == c1 ? 0x100u : 0u) | (c2 == c2 ? 0x10000u : 0u) | (c3 == c3 ? 0x1000000u : 0u);
             float4 o4 = make_float4(c0 == c0 ? c0 : 0.f, c1 == c1 ? c1 : 0.f, c2 == c2 ? c2 : 0.f, c3 == c3 ? c3 : 0.f);
             *reinterpret_cast<float4*>(cal_out + o) = o4;
@@ -461,8 +505,9 @@ __global__ void __launch_bounds__(256) calibrate_kernel(FrameArgs f, long long n
     } else {
         for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += stride) {
             int r = f.raw[i];
-            bool bad = (r >= f.sat_adu) || (f.bpm && f.bpm[i] != 0);
-            float c = calib_px((float)r, f.bias[i], f.dark[i], f.flat[i], bad, f.t_exp, f.flat_min);
+            bool bad = (r >= f.sat_adu) || (!f.pre && f.bpm && f.bpm[i] != 0);
+            float c = f.pre ? calib_pre<false>((float)r, pre_load(f.offset, i, f.pre), pre_load(f.gain, i, f.pre), bad)
+                            : calib_px((float)r, f.bias[i], f.dark[i], f.flat[i], bad, f.t_exp, f.flat_min);
             cal_out[i] = (c == c) ? c : 0.f;
             mask_out[i] = (c == c) ? 1 : 0;
         }
@@ -492,4 +537,37 @@ __global__ void __launch_bounds__(256) coadd_list_kernel(CoaddArgs ca, int ppt_l
     float wv = weight[i];
     ca.sum[s] = fmaf(wv, value[i], ca.sum[s]);
     ca.wsum[s] += wv;
+}
+
+// ------------------------------------------------------------------------------------------------
+// pre-fused masters, once per pointing and exposure time (masters are uploaded at the
+// start of each pointing).  offset = bias + dark * t_exp; gain = 1 / flat, NaN where the pixel is invalid (flat <
+// flat_min or not finite, bias / dark not finite, bpm != 0, or not representable in the storage format).
+// FMT: 1 float32, 2 binary16 (round to nearest even).  28 B in (+1 with a bpm), 8 or 4 B out per pixel.
+// ------------------------------------------------------------------------------------------------
+template <int FMT>
+__global__ void __launch_bounds__(256) prepare_masters_kernel(const float* __restrict__ bias, const float* __restrict__ dark,
+                                                             const float* __restrict__ flat, const unsigned char* __restrict__ bpm,
+                                                             long long n, float t_exp, float flat_min, void* __restrict__ offset_out,
+                                                             void* __restrict__ gain_out) {
+    const long long stride = (long long)gridDim.x * 256;
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += stride) {
+        const float b = bias[i], d = dark[i], fl = flat[i];
+        float off = fmaf(d, t_exp, b);
+        bool ok = (fl >= flat_min) && (fl < INFINITY) && (fabsf(b) < INFINITY) && (fabsf(d) < INFINITY) && !(bpm && bpm[i] != 0);
+        float g = ok ? 1.0f / fl : nanf_();
+        if (FMT == 1) {
+            if (!(fabsf(off) < INFINITY)) { off = 0.f; g = nanf_(); }
+            reinterpret_cast<float*>(offset_out)[i] = off;
+            reinterpret_cast<float*>(gain_out)[i] = g;
+        } else {
+            __half ho = __float2half_rn(off), hg = __float2half_rn(g);
+            if (!(fabsf(__half2float(ho)) < INFINITY) || (ok && !(fabsf(__half2float(hg)) < INFINITY))) {
+                if (!(fabsf(__half2float(ho)) < INFINITY)) ho = __float2half_rn(0.f);
+                hg = __float2half_rn(nanf_());
+            }
+            reinterpret_cast<__half*>(offset_out)[i] = ho;
+            reinterpret_cast<__half*>(gain_out)[i] = hg;
+        }
+    }
 }
