@@ -313,6 +313,59 @@ int argus_detect_sources(argus_ctx* ctx, const argus_frame* frame, int64_t W, in
                          const float* nse, float k_sigma, argus_source* out, size_t capacity, int64_t* n_dev,
                          size_t* n_out, void* stream);
 
+/* ---- Direct image subtraction per tile: "Transient detection is performed using image subtraction in
+ * the reprojected HEALPix image segments, leveraging long-term coadds as reference frames ... the direct image
+ * subtraction method ... for real-time operation in 1-second cadence data" (sec. 5.2), per tile,
+ * on the CPU in the paper (20 ms per tile), "a GPU implementation is in development" (:185).  The method's
+ * formulas are in the paper's ref [17], not in the paper: DESIGN.md section 13 lists the readings R-X1 .. R-X8 restated here.
+ *
+ * Both images live on the tile-dense grid of `layout` (argus_coadd: n_tiles * ppt floats, nested order inside a tile) as
+ * (sum, wsum) pairs, exactly what argus_resample_coadd accumulates: the science image is the pair of ONE frame (or of a
+ * short coadd), the reference the pair of the long-term coadd.  Per pixel and tile:
+ *   s = sci_sum / sci_wsum, r = ref_sum / ref_wsum; VALID iff sci_wsum >= sci_wmin and ref_wsum >= ref_wmin
+ *   match   ARGUS_SUB_MATCH_NONE: alpha = 1, beta = 0.  ARGUS_SUB_MATCH_AFFINE: per tile, least squares of s ~ alpha r + beta
+ *           over the valid pixels (FP64 sums in a fixed order); fewer than n_min valid pixels or a reference without
+ *           structure (variance(r) <= 1e-10 mean(r^2): constant up to rounding): alpha = 1, beta = mean(s - r)
+ *   diff    d = s - (alpha r + beta) at valid pixels, 0 elsewhere
+ *   noise   sigma^2 = (read_noise^2 + max(alpha r + beta, 0) / gain) * (1 / sci_wsum + alpha^2 / ref_wsum)
+ *   sig     S = d / sigma at valid pixels, 0 elsewhere
+ *   candidate iff valid, S > k_sigma, and S is the maximum over the valid 8-neighbours in the tile's (ix, iy) grid (ix =
+ *           even, iy = odd bits of the in-tile nested index; tiles are independent: no neighbours beyond the tile), S_p >
+ *           S_q for neighbours with a smaller nested index, S_p >= S_q for larger ones.
+ * Outputs (DEVICE): diff_out (required) and sig_out (may be NULL): n_tiles * ppt floats; alpha_out, beta_out (float) and
+ * nvalid_out (int32), n_tiles each, may be NULL; cat_out: argus_transient[capacity], 16-byte aligned, ascending nested
+ * pixel index; n_dev / n_out / capacity / ARGUS_ERR_CAPACITY exactly as argus_detect_sources.  Scratch grown on demand.
+ * Asynchronous on stream unless n_out is given. */
+enum { ARGUS_SUB_MATCH_NONE = 0, ARGUS_SUB_MATCH_AFFINE = 1 };
+
+typedef struct argus_subtract_params {
+    int32_t match;      /* ARGUS_SUB_MATCH_* */
+    int32_t n_min;      /* affine match: minimum number of valid pixels of a tile (>= 2; e.g. 16) */
+    float sci_wmin;     /* validity thresholds on the weight sums (> 0; e.g. 0.5) */
+    float ref_wmin;
+    float read_noise;   /* ADU, > 0 */
+    float gain;         /* e- / ADU, > 0 */
+    float k_sigma;      /* detection threshold, >= 0 (the paper's Fig. 3: 5) */
+    float reserved;
+} argus_subtract_params;
+
+/* One transient candidate (32 bytes). */
+typedef struct argus_transient {
+    int64_t pixel;      /* nested pixel index at nside */
+    float sig;          /* S at the peak */
+    float diff;         /* d at the peak, ADU */
+    float flux;         /* sum of d over the valid pixels of the 3 x 3 window in the tile, ADU */
+    float noise;        /* sigma at the peak, ADU */
+    int32_t tile_rank;  /* position of the pixel's tile in layout->tiles */
+    int32_t reserved;
+} argus_transient;
+
+int argus_subtract_tiles(argus_ctx* ctx, const argus_coadd* layout, int64_t nside, const float* sci_sum,
+                         const float* sci_wsum, const float* ref_sum, const float* ref_wsum,
+                         const argus_subtract_params* params, float* diff_out, float* sig_out, float* alpha_out,
+                         float* beta_out, int32_t* nvalid_out, argus_transient* cat_out, size_t capacity, int64_t* n_dev,
+                         size_t* n_out, void* stream);
+
 /* Synchronises the stream and reports the statistics of the most recent plan.  Returns ARGUS_ERR_CAPACITY if ANY
  * asynchronous call since the last check (argus_plan_info or argus_healpix_footprint) overflowed its output capacity
  * or the context's max_tiles -- the condition is latched in the context, not in the per-frame plan, so a check after

@@ -21,7 +21,9 @@ argus_resample_coadd writes them: image = sum / wsum.
   R-X2 match      per tile, over its valid pixels: none: alpha = 1, beta = 0.  affine: least squares of s ~ alpha r +
                   beta (transparency and sky level differ between a 1 s exposure and a long coadd):
                   alpha = (n Srs - Sr Ss) / (n Srr - Sr^2), beta = (Ss - alpha Sr) / n; with fewer than n_min valid
-                  pixels or a non-positive denominator (constant reference): alpha = 1, beta = (Ss - Sr) / n (0 if n = 0).
+                  pixels or a reference without structure -- n Srr - Sr^2 <= 1e-10 n Srr, i.e. variance(r) <= 1e-10
+                  mean(r^2): constant up to rounding, where the slope is undetermined -- alpha = 1, beta = (Ss - Sr) / n
+                  (0 if n = 0).
   R-X3 difference d = s - (alpha r + beta) at valid pixels, 0 elsewhere.
   R-X4 noise      m = alpha r + beta (the reference's prediction of the science pixel);
                   sigma^2 = (read_noise^2 + max(m, 0) / gain) * (1 / sci_wsum + alpha^2 / ref_wsum)
@@ -40,6 +42,7 @@ from __future__ import annotations
 import numpy as np
 
 MATCH_NONE, MATCH_AFFINE = 0, 1
+FLAT_REFERENCE = 1e-10   # R-X2: variance(r) / mean(r^2) below which the reference has no structure to fit a slope to
 
 
 def deinterleave(q, bits):
@@ -78,8 +81,9 @@ def match_tile(s, r, valid, match=MATCH_AFFINE, n_min=16):
     Ss, Sr = sv.sum(), rv.sum()
     if match == MATCH_NONE:
         return 1.0, 0.0, n
-    den = n * (rv * rv).sum() - Sr * Sr
-    if n < n_min or not den > 0.0:
+    Srr = (rv * rv).sum()
+    den = n * Srr - Sr * Sr
+    if n < n_min or not den > FLAT_REFERENCE * n * Srr:
         return 1.0, (Ss - Sr) / n, n
     alpha = (n * (rv * sv).sum() - Sr * Ss) / den
     return alpha, (Ss - alpha * Sr) / n, n

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     ArgusError,
     Context,
     SOURCE_DTYPE,
+    TRANSIENT_DTYPE,
     argus_background_map,
     argus_calibrate,
     argus_coadd_accumulate,
@@ -23,6 +24,7 @@ from .binding import (  # noqa: F401
     argus_resample_coadd_host,
     argus_host_wait,
     argus_segment_products,
+    argus_subtract_tiles,
     library_path,
     load_library,
 )

@@ -23,7 +23,7 @@ EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_prepare_masters", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
-    "argus_resample_host", "argus_resample_coadd_host", "argus_host_wait", "argus_segment_products", "argus_background_map", "argus_detect_sources",
+    "argus_resample_host", "argus_resample_coadd_host", "argus_host_wait", "argus_subtract_tiles", "argus_segment_products", "argus_background_map", "argus_detect_sources",
 ]
 
 
@@ -48,6 +48,11 @@ class _Frame(C.Structure):
 
 class _Coadd(C.Structure):
     _fields_ = [("tiles", C.c_void_p), ("n_tiles", C.c_int64), ("nside_tile", C.c_int64)]
+
+
+class _SubParams(C.Structure):
+    _fields_ = [("match", C.c_int32), ("n_min", C.c_int32), ("sci_wmin", C.c_float), ("ref_wmin", C.c_float),
+                ("read_noise", C.c_float), ("gain", C.c_float), ("k_sigma", C.c_float), ("reserved", C.c_float)]
 
 
 class _PlanStats(C.Structure):
@@ -105,6 +110,8 @@ def load_library():
                                          vp, C.POINTER(sz), vp]
     L.argus_background_map.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, i32, vp, vp, vp, vp, vp, vp]
     L.argus_detect_sources.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, vp, vp, f32, vp, sz, vp, C.POINTER(sz), vp]
+    L.argus_subtract_tiles.argtypes = [vp, C.POINTER(_Coadd), i64, vp, vp, vp, vp, C.POINTER(_SubParams), vp, vp, vp, vp, vp, vp, sz,
+                                       vp, C.POINTER(sz), vp]
     L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
     L.argus_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64), vp]
     _lib = L
@@ -486,6 +493,46 @@ def argus_detect_sources(ctx, W, H, bkg, nse, out, cell=64, k_sigma=5.0, n_dev=N
     if rc == -6 and sync:
         raise ArgusError(rc, "argus_detect_sources", "n_sources=%d" % n.value)
     _check(ctx, rc, "argus_detect_sources")
+    return int(n.value) if sync else None
+
+
+# numpy view of argus_transient records (argus.h)
+TRANSIENT_DTYPE = [("pixel", "<i8"), ("sig", "<f4"), ("diff", "<f4"), ("flux", "<f4"), ("noise", "<f4"), ("tile_rank", "<i4"),
+                   ("reserved", "<i4")]
+_MATCH = {"none": 0, "affine": 1, 0: 0, 1: 1}
+
+
+def argus_subtract_tiles(ctx, tiles, nside_tile, nside, sci_sum, sci_wsum, ref_sum, ref_wsum, diff_out, sig_out=None, out=None,
+                         match="affine", n_min=16, sci_wmin=0.5, ref_wmin=0.5, read_noise=1.7, gain=1.0, k_sigma=5.0,
+                         alpha_out=None, beta_out=None, nvalid_out=None, n_dev=None, sync=True, stream=None):
+    """Direct image subtraction per tile on the tile-dense (sum, wsum) pairs of a science frame and a
+    reference coadd.  out: uint8 CUDA tensor of 32 * capacity bytes (argus_transient records, view the host copy with
+    TRANSIENT_DTYPE) or None to count.  Returns the number of candidates when sync, else None."""
+    lay = _coadd_struct(tiles, nside_tile)
+    n_slots = tiles.numel() * (int(nside) // int(nside_tile)) ** 2
+    for name, t in (("sci_sum", sci_sum), ("sci_wsum", sci_wsum), ("ref_sum", ref_sum), ("ref_wsum", ref_wsum),
+                    ("diff_out", diff_out), ("sig_out", sig_out)):
+        if t is not None and t.numel() < n_slots:
+            raise ValueError("%s holds %d elements, %d needed" % (name, t.numel(), n_slots))
+    for name, t in (("alpha_out", alpha_out), ("beta_out", beta_out), ("nvalid_out", nvalid_out)):
+        if t is not None and t.numel() < tiles.numel():
+            raise ValueError("%s is shorter than the tile list" % name)
+    cap = 0 if out is None else out.numel() // 32
+    if out is not None and out.dtype != torch.uint8:
+        raise TypeError("out must be a uint8 tensor (32 bytes per record)")
+    p = _SubParams(_MATCH[match], int(n_min), float(sci_wmin), float(ref_wmin), float(read_noise), float(gain), float(k_sigma), 0.0)
+    n = C.c_size_t(0)
+    f32 = torch.float32
+    rc = load_library().argus_subtract_tiles(
+        ctx._h, C.byref(lay), int(nside), _dev(sci_sum, f32, "sci_sum"), _dev(sci_wsum, f32, "sci_wsum"),
+        _dev(ref_sum, f32, "ref_sum"), _dev(ref_wsum, f32, "ref_wsum"), C.byref(p), _dev(diff_out, f32, "diff_out"),
+        _dev(sig_out, f32, "sig_out", allow_none=True), _dev(alpha_out, f32, "alpha_out", allow_none=True),
+        _dev(beta_out, f32, "beta_out", allow_none=True), _dev(nvalid_out, torch.int32, "nvalid_out", allow_none=True),
+        _dev(out, torch.uint8, "out", allow_none=True), cap, _dev(n_dev, torch.int64, "n_dev", allow_none=True),
+        C.byref(n) if sync else None, _stream(stream))
+    if rc == -6 and sync:
+        raise ArgusError(rc, "argus_subtract_tiles", "n_candidates=%d" % n.value)
+    _check(ctx, rc, "argus_subtract_tiles")
     return int(n.value) if sync else None
 
 

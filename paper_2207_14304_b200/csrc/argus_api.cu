@@ -15,6 +15,7 @@
 #include "resample_fast.cuh"
 #include "segments.cuh"
 #include "background.cuh"
+#include "subtract.cuh"
 
 #define ARGUS_VERSION_NUM 100
 #define PLAN_SLOTS 3
@@ -86,6 +87,14 @@ struct argus_ctx {
         unsigned* ctl;                           // [0] running total (atomics), [1] final count
         long long* h_n;                          // pinned
     } bg;
+    // argus_subtract_tiles: per-slice partial sums, per-tile fit, per-block (base, count) + offsets, record staging
+    struct SubScratch {
+        double* partial; float2* fit; size_t cap_tiles;
+        uint2* blocks; size_t cap_blocks;           // block_info | offsets (4 B) behind it
+        ArgusTransientRec* tmp; size_t cap_tmp;
+        unsigned* ctl;                              // [0] running total (atomics), [1] final count
+        long long* h_n;                             // pinned
+    } sub;
 };
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -324,6 +333,12 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (c->bg.ord) cudaFree(c->bg.ord);
     if (c->bg.ctl) cudaFree(c->bg.ctl);
     if (c->bg.h_n) cudaFreeHost(c->bg.h_n);
+    if (c->sub.partial) cudaFree(c->sub.partial);
+    if (c->sub.fit) cudaFree(c->sub.fit);
+    if (c->sub.blocks) cudaFree(c->sub.blocks);
+    if (c->sub.tmp) cudaFree(c->sub.tmp);
+    if (c->sub.ctl) cudaFree(c->sub.ctl);
+    if (c->sub.h_n) cudaFreeHost(c->sub.h_n);
     cudaFreeHost(c->h_stats);
     cudaFreeHost(c->h_latch);
     cudaFree(c->d_latch);
@@ -1198,6 +1213,98 @@ extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int6
         CUDA_TRY(c, cudaMemcpyAsync(c->bg.h_n, c->bg.ctl, 8, cudaMemcpyDeviceToHost, st));
         CUDA_TRY(c, cudaStreamSynchronize(st));
         *n_out = (size_t)(((unsigned long long)*c->bg.h_n) >> 32);     // ctl[1]
+        if (capacity > 0 && *n_out > capacity) return ARGUS_ERR_CAPACITY;
+    }
+    return ARGUS_OK;
+}
+
+// ------------------------------------------------------------------------- direct image subtraction per tile (8(f).3)
+extern "C" int argus_subtract_tiles(argus_ctx* c, const argus_coadd* layout, int64_t nside, const float* sci_sum,
+                                    const float* sci_wsum, const float* ref_sum, const float* ref_wsum,
+                                    const argus_subtract_params* prm, float* diff_out, float* sig_out, float* alpha_out,
+                                    float* beta_out, int32_t* nvalid_out, argus_transient* cat_out, size_t capacity,
+                                    int64_t* n_dev, size_t* n_out, void* stream) {
+    if (!c) return ARGUS_ERR_NULL;
+    if (n_out) *n_out = 0;
+    if (!layout || !prm || (capacity > 0 && !cat_out)) return ARGUS_ERR_NULL;
+    if (layout->n_tiles > 0 && (!layout->tiles || !sci_sum || !sci_wsum || !ref_sum || !ref_wsum || !diff_out)) return ARGUS_ERR_NULL;
+    if (!is_pow2(nside) || nside < 32 || nside > (1ll << 29)) return ARGUS_ERR_NSIDE;
+    if (!is_pow2(layout->nside_tile) || layout->nside_tile > (nside >> ARGUS_TILE_LOG2) || layout->n_tiles < 0) return ARGUS_ERR_SHAPE;
+    if (prm->match != ARGUS_SUB_MATCH_NONE && prm->match != ARGUS_SUB_MATCH_AFFINE) return ARGUS_ERR_SHAPE;
+    if (prm->n_min < 2 || !(prm->sci_wmin > 0.f) || !(prm->ref_wmin > 0.f) || !(prm->sci_wmin < INFINITY) || !(prm->ref_wmin < INFINITY) ||
+        !(prm->read_noise > 0.f) || !(prm->read_noise < INFINITY) || !(prm->gain > 0.f) || !(prm->gain < INFINITY) ||
+        !(prm->k_sigma >= 0.f) || !(prm->k_sigma < INFINITY) || capacity > 0x7fffffffull)
+        return ARGUS_ERR_SHAPE;
+    if (!aligned(sci_sum, 16) || !aligned(sci_wsum, 16) || !aligned(ref_sum, 16) || !aligned(ref_wsum, 16) || !aligned(diff_out, 16) ||
+        !aligned(sig_out, 16) || !aligned(alpha_out, 4) || !aligned(beta_out, 4) || !aligned(nvalid_out, 4) || !aligned(cat_out, 16) ||
+        !aligned(n_dev, 8) || !aligned(layout->tiles, 8))
+        return ARGUS_ERR_ALIGN;
+    const int side_log2 = ilog2(nside) - ilog2(layout->nside_tile);     // >= 5
+    if (side_log2 > 15) return ARGUS_ERR_SHAPE;
+    const long long ppt = 1ll << (2 * side_log2);
+    const long long n_tiles = layout->n_tiles, n_blocks = n_tiles * (ppt / SUB_BLOCK);
+    if (n_blocks > 0x7fffffffll) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (!c->sub.h_n) CUDA_TRY(c, cudaMallocHost((void**)&c->sub.h_n, sizeof(long long)));
+    if (!c->sub.ctl) CUDA_TRY(c, cudaMalloc((void**)&c->sub.ctl, 16));
+    if (c->sub.cap_tiles < (size_t)n_tiles || !c->sub.fit) {
+        if (c->sub.fit) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->sub.fit); cudaFree(c->sub.partial); c->sub.fit = nullptr; c->sub.partial = nullptr; }
+        size_t want = align_up((size_t)n_tiles + 1, 256);
+        CUDA_TRY(c, cudaMalloc((void**)&c->sub.fit, want * sizeof(float2)));
+        CUDA_TRY(c, cudaMalloc((void**)&c->sub.partial, want * SUB_SPLIT_MAX * 5 * sizeof(double)));
+        c->sub.cap_tiles = want;
+    }
+    if (c->sub.cap_blocks < (size_t)n_blocks || !c->sub.blocks) {
+        if (c->sub.blocks) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->sub.blocks); c->sub.blocks = nullptr; }
+        size_t want = align_up((size_t)n_blocks + 1, 4096);
+        CUDA_TRY(c, cudaMalloc((void**)&c->sub.blocks, want * 12));
+        c->sub.cap_blocks = want;
+    }
+    if (c->sub.cap_tmp < capacity || !c->sub.tmp) {
+        if (c->sub.tmp) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->sub.tmp); c->sub.tmp = nullptr; }
+        size_t want = align_up(capacity + 1, 65536);
+        CUDA_TRY(c, cudaMalloc((void**)&c->sub.tmp, want * sizeof(ArgusTransientRec)));
+        c->sub.cap_tmp = want;
+    }
+    unsigned* offsets = (unsigned*)(c->sub.blocks + c->sub.cap_blocks);
+    SubParams p;
+    p.match = prm->match; p.n_min = prm->n_min; p.sci_wmin = prm->sci_wmin; p.ref_wmin = prm->ref_wmin;
+    p.rn2 = prm->read_noise * prm->read_noise; p.inv_gain = 1.0f / prm->gain; p.k_sigma = prm->k_sigma;
+    CUDA_TRY(c, cudaMemsetAsync(c->sub.ctl, 0, 16, st));
+    if (n_tiles == 0) {
+        if (n_dev) CUDA_TRY(c, cudaMemsetAsync(n_dev, 0, sizeof(int64_t), st));
+        if (n_out) CUDA_TRY(c, cudaStreamSynchronize(st));
+        return ARGUS_OK;
+    }
+    // statistics pass only when something needs it (the affine fit, or the count of valid pixels)
+    const int have_stats = (prm->match == ARGUS_SUB_MATCH_AFFINE || nvalid_out) ? 1 : 0;
+    int split = (int)(ppt / 8192);
+    if (split < 1) split = 1;
+    if (split > SUB_SPLIT_MAX) split = SUB_SPLIT_MAX;
+    if (have_stats) {
+        if (n_tiles * split > 0x7fffffffll) return ARGUS_ERR_SHAPE;
+        sub_stats_kernel<<<(unsigned)(n_tiles * split), 256, 0, st>>>(sci_sum, sci_wsum, ref_sum, ref_wsum, ppt, split, p, c->sub.partial);
+        c->n_launches++;
+    }
+    sub_fit_kernel<<<(unsigned)((n_tiles + 127) / 128), 128, 0, st>>>(c->sub.partial, n_tiles, split, p, have_stats, c->sub.fit, alpha_out,
+                                                                    beta_out, (int*)nvalid_out);
+    long long grid = n_blocks < (long long)c->sm_count * 32 ? n_blocks : (long long)c->sm_count * 32;
+    sub_tiles_kernel<<<(unsigned)grid, 256, 0, st>>>(sci_sum, sci_wsum, ref_sum, ref_wsum, (const long long*)layout->tiles, ppt, side_log2,
+                                                    n_blocks, p, c->sub.fit, diff_out, sig_out, c->sub.tmp, (unsigned)capacity,
+                                                    c->sub.blocks, c->sub.ctl);
+    det_scan_kernel<<<1, 1024, 0, st>>>(c->sub.blocks, (int)n_blocks, offsets, c->sub.ctl, (long long*)n_dev);
+    c->n_launches += 3;
+    if (capacity > 0) {
+        sub_gather_kernel<<<(unsigned)((n_blocks + 7) / 8), 256, 0, st>>>(c->sub.blocks, offsets, n_blocks, c->sub.tmp,
+                                                                        (ArgusTransientRec*)cat_out, (unsigned)capacity);
+        c->n_launches++;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    if (n_out) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->sub.h_n, c->sub.ctl, 8, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        *n_out = (size_t)(((unsigned long long)*c->sub.h_n) >> 32);     // ctl[1]
         if (capacity > 0 && *n_out > capacity) return ARGUS_ERR_CAPACITY;
     }
     return ARGUS_OK;

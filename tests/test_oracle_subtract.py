@@ -70,6 +70,13 @@ def test_match_fallbacks():
     s = r + 5.0
     out = osub.subtract_tiles([0], PPT, 1 << 10, *_pair(s, r))
     assert out["alpha"][0] == 1.0 and abs(out["beta"][0] - 5.0) < 1e-12 and np.all(np.abs(out["diff"]) < 1e-12)
+    # constant up to float32 rounding (sum / wsum of a float32 coadd): still no slope to fit
+    wr = np.random.default_rng(0).uniform(20, 30, r.shape).astype(np.float32)
+    rs32 = (np.float32(100.0) * wr).astype(np.float32)
+    rq = (rs32 / wr).astype(np.float64)
+    assert rq.std() > 0
+    out = osub.subtract_tiles([0], PPT, 1 << 10, osub.grid_to_tile(s), osub.grid_to_tile(np.ones_like(s)), osub.grid_to_tile(rs32), osub.grid_to_tile(wr))
+    assert out["alpha"][0] == 1.0 and abs(out["beta"][0] - 5.0) < 1e-4
     ws = np.zeros((SIDE, SIDE)); ws[0, :10] = 1.0               # 10 valid pixels < n_min = 16
     r2 = _smooth(4)
     out = osub.subtract_tiles([0], PPT, 1 << 10, *_pair(2 * r2, r2, w_s=ws))
