@@ -98,3 +98,44 @@ def test_config3_coadd_full(argus, ctx):
     # every slot except those the oracle flags margin-ambiguous in some frame (R18), to the per-slot R20 tolerance
     worst, n_amb = assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "config3 coadd of 3 frames")
     print("config3 coadd: worst %.3f x tol, %d ambiguous slots of %d pixels accumulated" % (worst, n_amb, ref["n_px"]))
+
+
+def test_subtract_full_size(argus, ctx):
+    """SURVEY 8(f).3 at the size bench.py --workload subtract times (all NSIDE-256 tiles of a configs[3] field, 2^18 pixels
+    each, affine match, 5 sigma): the GPU runs the whole layout; the oracle checks 5 of the tiles, every pixel and
+    every candidate of them."""
+    from test_gpu_subtract import compare
+    W, H, nside = synth.frames.FULL_W, synth.frames.FULL_H, 1 << 17
+    base = synth.config3_frame(0)
+    masters = (base.bias, base.dark, base.flat)
+    frames = [base] + [synth.config3_frame(k, masters=masters) for k in (1, 2)]
+    wcs = base.wcs
+    dm = [torch.from_numpy(m).cuda() for m in masters]
+    n, idx = argus.argus_healpix_footprint(ctx, wcs, W, H, nside)
+    tiles = torch.unique(idx >> 18)
+    del idx
+    ppt = 1 << 18
+    pairs = [torch.zeros(tiles.numel() * ppt, dtype=torch.float32, device="cuda") for _ in range(4)]
+    for k, f in enumerate(frames):
+        d = dict(raw=torch.from_numpy(f.raw).cuda(), bias=dm[0], dark=dm[1], flat=dm[2], bpm=None, t_exp=f.t_exp, sat_adu=f.sat_adu, flat_min=f.flat_min)
+        reps = 4 if k < 2 else 1                      # reference: frames 0 and 1, four times each; science: frame 2
+        for _ in range(reps):
+            argus.argus_resample_coadd(ctx, wcs, W, H, nside, "bilinear", tiles, 256, pairs[2 if k < 2 else 0], pairs[3 if k < 2 else 1], None, **d)
+    diff = torch.empty_like(pairs[0]); sig = torch.empty_like(pairs[0])
+    nt = tiles.numel()
+    al = torch.empty(nt, dtype=torch.float32, device="cuda"); be = torch.empty_like(al)
+    nv = torch.empty(nt, dtype=torch.int32, device="cuda")
+    cat = torch.zeros((1 << 18) * 32, dtype=torch.uint8, device="cuda")
+    kw = dict(match="affine", k_sigma=5.0, read_noise=1.7, gain=1.0, ref_wmin=2.0)
+    k = argus.argus_subtract_tiles(ctx, tiles, 256, nside, pairs[0], pairs[1], pairs[2], pairs[3], diff, sig, cat, alpha_out=al,
+                                   beta_out=be, nvalid_out=nv, **kw)
+    rec = cat.cpu().numpy()[:k * 32].view(argus.TRANSIENT_DTYPE)
+    assert np.all(np.diff(rec["pixel"]) > 0)
+    th = tiles.cpu().numpy()
+    sel = np.unique(np.linspace(0, nt - 1, 5).astype(np.int64))
+    cut = lambda t: np.concatenate([t[int(i) * ppt:(int(i) + 1) * ppt].cpu().numpy() for i in sel])
+    r = rec[np.isin(rec["tile_rank"], sel)].copy()
+    r["tile_rank"] = np.searchsorted(sel, r["tile_rank"])
+    g = dict(diff=cut(diff), sig=cut(sig), alpha=al.cpu().numpy()[sel], beta=be.cpu().numpy()[sel], n_valid=nv.cpu().numpy()[sel], rec=r)
+    n_must, n_amb = compare(g, th[sel], ppt, nside, [cut(p) for p in pairs], max_ambiguous=10, **kw)
+    print("subtract full size: %d tiles, %d candidates; checked tiles %s: %d clear, %d ambiguous" % (nt, k, sel.tolist(), n_must, n_amb))
