@@ -745,7 +745,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// TMA descriptors for (raw, bias, dark, flat): 2-D tensors {W, H}, boxes {40..72 step 8} x {48, 56, 64}, zero fill outside.
+// TMA descriptors for (raw, bias, dark, flat): 2-D tensors {W, H}, boxes {40..72 step 8} x {48, 56, 64, 72}, zero fill outside.
 static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
     if (!c->fast_enabled || !f.raw || f.bpm || f.pre) return false;
     if (W % 8 != 0 || W < 8 || !aligned(f.raw, 16) || !aligned(f.bias, 16) || !aligned(f.dark, 16) || !aligned(f.flat, 16)) return false;
@@ -763,7 +763,7 @@ static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
     const void* key[4] = {f.raw, f.bias, f.dark, f.flat};
     if (memcmp(key, c->maps_key, sizeof(key)) == 0 && c->maps_W == W && c->maps_H == H) return true;
     encode_tiled_fn enc = (encode_tiled_fn)c->encode_fn;
-    for (int hc = 0; hc < 3; ++hc)
+    for (int hc = 0; hc < 4; ++hc)
       for (int wc = 0; wc < 5; ++wc)
         for (int a = 0; a < 4; ++a) {
             cuuint64_t dims[2] = {(cuuint64_t)W, (cuuint64_t)H};

@@ -68,7 +68,7 @@ struct __align__(16) FastRec {
     int cls;             // TC_INSIDE / TC_BORDER when the tile is handled by the fast kernel, else 0
     int mask_slot;       // TC_BORDER: row of the membership-mask array
     int gx0, gy0;        // origin (cell) of the staged source box
-    int wclass;          // bits 0..3: staged box width 40 + 8 w px (w = 0..4); bits 4..5: box rows 48 + 8 h (h = 0..2)
+    int wclass;          // bits 0..3: staged box width 40 + 8 w px (w = 0..4); bits 4..5: box rows 48 + 8 h (h = 0..3)
     int bh;              // rows of the box holding taps
     int kofs;            // (Y0 - gy0) * pitch + (X0 - gx0): cell -> calibrated-box index offset
     int X0;

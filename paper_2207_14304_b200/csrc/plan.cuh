@@ -153,17 +153,17 @@ __device__ inline void cubic_basis(double S, double T, double m[10]) {
 // Staged-box geometry of the fast kernel for cells [bx0, bx1] x [by0, by1] plus the interpolation kernel's taps
 // (tl to the left / above, tr to the right / below: 0, 1 bilinear; 2, 3 Lanczos-3).  The TMA box must start on a
 // 16-byte boundary of every array (8 pixels of the uint16 frame), so the origin is aligned down to 8; widths come in
-// steps of 8 px (40..72), heights are 48, 56 or 64 rows (a TMA copy costs ~100 cycles per operation whatever its
+// steps of 8 px (40..72), heights are 48, 56, 64 or 72 rows (polar-cap tiles are taller than wide) (a TMA copy costs ~100 cycles per operation whatever its
 // size, so each array is fetched with ONE box).  Returns false when the box does not fit the kernel's stage.
 __device__ __host__ inline int fast_cal_pitch(int boxw) { return (boxw & 15) == 8 ? boxw : boxw + 8; }   // = 8 or 24 mod 32
 __device__ inline bool fast_box(const PlanBuffers& pb, int bx0, int bx1, int by0, int by1, int X0, int Y0, FastRec& f) {
     const int tl = pb.fast_tl, tr = pb.fast_tr;
     int gx0 = (bx0 - tl) & ~7, gy0 = by0 - tl;
     int bw = bx1 + tr + 1 - gx0, bh = by1 + tr + 1 - gy0;
-    if (bw < 1 || bh < 1 || bw > 72 || bh > 64) return false;
+    if (bw < 1 || bh < 1 || bw > 72 || bh > 72) return false;
     int wclass = bw <= 40 ? 0 : (bw - 40 + 7) >> 3;
     int boxw = 40 + 8 * wclass, pitch = fast_cal_pitch(boxw);
-    int hclass = bh <= 48 ? 0 : (bh <= 56 ? 1 : 2);
+    int hclass = bh <= 48 ? 0 : (bh - 48 + 7) >> 3;      // 48, 56, 64 or 72 rows
     if ((48 + 8 * hclass) * boxw > pb.fast_cap || bh * pitch > pb.fast_cap + pb.fast_cap / 8) return false;
     if (bx0 < X0 || by0 < Y0 || bx1 + 4 - X0 > 110 || by1 + 4 - Y0 > 110) return false;
     f.gx0 = gx0; f.gy0 = gy0; f.wclass = wclass | (hclass << 4); f.bh = bh;

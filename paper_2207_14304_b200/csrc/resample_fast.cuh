@@ -38,7 +38,7 @@ template <> struct FastCfg<0> { static constexpr int CAP = FAST_CAP_PX, STAGES =
 template <> struct FastCfg<1> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
 
 struct FastMaps {
-    CUtensorMap m[3][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
+    CUtensorMap m[4][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
 };
 
 struct __align__(16) FastDesc {
