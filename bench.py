@@ -171,25 +171,25 @@ def _config3_wcs(k):
     return synth.make_wcs((30.0, 20.0), ((W - 1) / 2.0 + dx, (H - 1) / 2.0 + dy), 0.3)
 
 
-def algorithmic_work(kernel, px_in, px_out, coadd):
+def algorithmic_work(kernel, px_in, px_out, coadd, in_bytes=14.0):
     """SURVEY 8(d) / DESIGN.md 6.5: what the method must move or compute once per frame.
     HBM bytes: 14 B per input px (raw u16 + three f32 masters) + 8 B per output px (value + weight), or 16 B per output
     px for the fused coadd read-modify-write.  Shared-memory bytes: the staged box is read once for calibration (14 B)
     and written once calibrated (4 B) per input px; the gather reads 4 (bilinear) or 36 (Lanczos-3) float32 taps per
     output px.  FP32 flops: A2 3 per input px; A3+A4 ~60 and A5 16 (bilinear) or 36 x 2 x 2 + 40 (Lanczos-3) per output px."""
     taps = 36 if kernel == "lanczos3" else 4
-    hbm = 14.0 * px_in + (16.0 if coadd else 8.0) * px_out
-    smem = 18.0 * px_in + 4.0 * taps * px_out
+    hbm = in_bytes * px_in + (16.0 if coadd else 8.0) * px_out       # in_bytes: 14, or 10 / 6 with pre-fused masters (8(f).4)
+    smem = (in_bytes + 4.0) * px_in + 4.0 * taps * px_out
     flop = 3.0 * px_in + (60.0 + (184.0 if kernel == "lanczos3" else 16.0)) * px_out
     return hbm, smem, flop
 
 
-def rooflines(kernel, px_in, px_out, coadd, k_ms, sm_mhz, hbm_peak, hbm_src):
+def rooflines(kernel, px_in, px_out, coadd, k_ms, sm_mhz, hbm_peak, hbm_src, in_bytes=14.0):
     """The three fractions SURVEY 8(d) asks for; `bound` = the resource whose time-at-peak for the algorithmic work is
     longest.  Peaks: HBM measured copy bandwidth; shared memory = SMs x 128 B/clk x clock; FP32 = SMs x 128 lanes x 2 x
     clock, both at the SM clock sampled under load (falls back to 1965 MHz)."""
     clk = (sm_mhz or 1965.0) * 1e6
-    hbm, smem, flop = algorithmic_work(kernel, px_in, px_out, coadd)
+    hbm, smem, flop = algorithmic_work(kernel, px_in, px_out, coadd, in_bytes)
     peaks = {"hbm": hbm_peak * 1e9, "smem": N_SM * SMEM_B_PER_CLK * clk, "fp32": N_SM * FP32_LANES * 2 * clk}
     work = {"hbm": hbm, "smem": smem, "fp32": flop}
     t_peak = {k: work[k] / peaks[k] for k in work}
@@ -322,8 +322,10 @@ def run_gpu(args):
     nside, kernel = fr0.nside, fr0.kernel
     coadd = name == "coadd"
     ctx = argus.Context(local)
-    if args.prefused is not None:
-        raise SystemExit("--prefused needs argus_prepare_masters (not built)")
+    if args.unit_kernel:
+        ctx.set_fast_path(3)
+    elif args.tile_kernel:
+        ctx.set_fast_path(2)
 
     # device-resident inputs.  coadd: shared masters, N_DISTINCT raw frames; batch: every frame its own raw + masters
     def up(a):
@@ -350,6 +352,17 @@ def run_gpu(args):
             d = dict(raw=up(fr.raw), bias=up(fr.bias), dark=up(fr.dark), flat=up(fr.flat))
         d.update(bpm=None, t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
         jobs.append((wcs, d))
+    if args.prefused:   # offset / gain formed once per pointing (not timed), 10 or 6 B per input pixel
+        dt = torch.float32 if args.prefused == "f32" else torch.float16
+        done = {}
+        for i, (wcs, d) in enumerate(jobs):
+            k = d["bias"].data_ptr()
+            if k not in done:
+                done[k] = argus.argus_prepare_masters(ctx, d["bias"], d["dark"], d["flat"], None, d["t_exp"], d["flat_min"], dtype=dt)
+            jobs[i] = (wcs, dict(raw=d["raw"], offset=done[k][0], gain=done[k][1], sat_adu=d["sat_adu"]))
+        torch.cuda.synchronize()
+        for wcs, d in jobs:
+            d.pop("bias", None)
     n_fps = [argus.argus_healpix_footprint(ctx, wcs, W, H, nside, want_indices=False)[0] for wcs, _ in jobs]
     stats = argus.argus_plan_info(ctx)
     n_out_step, n_frames = int(sum(n_fps)), len(jobs)
@@ -420,7 +433,8 @@ def run_gpu(args):
 
     def e2e_step():
         for (fr, wcs), (_, d), n in zip(jobs_host, jobs, n_fps):
-            m = dict(bias=d["bias"], dark=d["dark"], flat=d["flat"], t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min)
+            m = (dict(offset=d["offset"], gain=d["gain"], sat_adu=fr.sat_adu) if args.prefused else
+                 dict(bias=d["bias"], dark=d["dark"], flat=d["flat"], t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min))
             if coadd:
                 argus.argus_resample_coadd_host(ctx, wcs, W, H, nside, kernel, h_raws[id(fr)], tiles, 256, csum, cwsum, None, **m)
             else:
@@ -450,13 +464,15 @@ def run_gpu(args):
         ms_step = ms / args.steps
         k_ms = kern_ms / max(ncalls, 1)                       # per frame (argus_resample call)
         px_out_frame = n_out_step / n_frames
-        roof = rooflines(kernel, W * H, px_out_frame, coadd, k_ms, clocks and clocks.get("sm_mhz"), peak, peak_src)
+        in_bytes = {None: 14.0, "f32": 10.0, "f16": 6.0}[args.prefused]
+        roof = rooflines(kernel, W * H, px_out_frame, coadd, k_ms, clocks and clocks.get("sm_mhz"), peak, peak_src, in_bytes)
+        roof["input_bytes_per_px"] = in_bytes
         alg_step = roof["algorithmic_bytes"] * n_frames
         roof["kernel"] = ("resample_fast_kernel<%s,%d> (TMA-staged, fused calibration%s) + resample_tiles_kernel on its slow list; "
                           "per frame, CUDA events around the resample launches" % ("true" if coadd else "false", 1 if kernel == "lanczos3" else 0,
                                                                                   ", coadd read-modify-write" if coadd else ""))
         roof["step_frac"] = (alg_step / (ms_step * 1e-3) / 1e9) / peak
-        tr, tr_src = ncu_traffic(name)
+        tr, tr_src = ncu_traffic(name + ("" if not args.prefused else "_" + args.prefused))
         roof["traffic"], roof["traffic_source"] = tr, tr_src
         if world == 1:
             import oracle
@@ -479,6 +495,8 @@ def run_gpu(args):
             cpu = {"value": None, "unit": UNIT, "cores": None, "kind": "oracle", "sample": "rank 0 at N=1 only"}
             cpu1 = None
         cfg = public_config(name, fr0, n_frames)
+        if args.prefused:
+            cfg["masters"] = "pre-fused offset + gain, %s (SURVEY 8(f).4): %d B per input pixel" % (args.prefused, int(in_bytes))
         line = {
             "metric": METRIC, "value": px_in_all * args.steps / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
@@ -871,6 +889,8 @@ def main():
     ap.add_argument("--no-plan-overlap", action="store_true", help="diagnostic: build every plan in place on the caller's stream")
     ap.add_argument("--workload", default="config1", choices=sorted(WORKLOADS) + ["segments", "detect", "subtract"])
     ap.add_argument("--prefused", default=None, choices=["f32", "f16"], help="masters pre-fused by argus_prepare_masters (SURVEY 8(f).4)")
+    ap.add_argument("--unit-kernel", action="store_true", help="diagnostic: image-aligned unit kernel wherever its geometry allows")
+    ap.add_argument("--tile-kernel", action="store_true", help="diagnostic: tile kernel only")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

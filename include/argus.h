@@ -63,9 +63,11 @@ enum { ARGUS_BILINEAR = 0, ARGUS_LANCZOS3 = 1 };
 enum {
     ARGUS_OPT_PLAN_CACHE = 1, /* 1 (default): a plan built for (wcs, W, H, nside) is reused by the next
                                  call with identical arguments; 0: every call re-plans on the device */
-    ARGUS_OPT_FAST_PATH = 3,  /* 1 (default): resampling of raw + masters (no bpm, W % 8 == 0, 16-byte aligned arrays) stages
-                                 source tiles with TMA (resample_fast_kernel, both interpolation kernels); 0: always the
-                                 general kernel */
+    ARGUS_OPT_FAST_PATH = 3,  /* which kernel runs a planned frame given as raw + masters (no bpm, W % 8 == 0, 16-byte aligned arrays):
+                                 1 (default): the TMA-staged tile kernel (resample_fast_kernel, both interpolation kernels) where
+                                    every 32 x 32-pixel tile's source box fits its stage, else -- and always with pre-fused
+                                    masters -- the image-aligned unit kernel (resample_unit_kernel, bilinear);
+                                 2: tile kernel only; 3: unit kernel wherever its geometry allows; 0: always the general kernel */
     ARGUS_OPT_PLAN_OVERLAP = 4, /* 1 (default): the plan of a new WCS is built on an internal high-priority stream in a second
                                  set of scratch buffers, so that it runs underneath the previous frame's kernels; the
                                  caller's stream waits for it (stream order of results is unchanged); 0: in place */

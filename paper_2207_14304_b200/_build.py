@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libargus.so")
 SOURCES = ["argus_api.cu"]
-HEADERS = ["common.cuh", "plan.cuh", "plan_block.cuh", "resample.cuh", "resample_fast.cuh", "segments.cuh", "background.cuh", "subtract.cuh", os.path.join("..", "..", "include", "argus.h")]
+HEADERS = ["common.cuh", "plan.cuh", "plan_block.cuh", "resample.cuh", "resample_fast.cuh", "resample_unit.cuh", "segments.cuh", "background.cuh", "subtract.cuh", os.path.join("..", "..", "include", "argus.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC"]
 

@@ -219,8 +219,9 @@ class Context:
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")
 
-    def set_fast_path(self, on: bool):
-        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_FAST_PATH, 1 if on else 0)
+    def set_fast_path(self, on):
+        """False / 0: general kernel only; True / 1: default choice; 2: tile kernel only; 3: unit kernel where possible."""
+        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_FAST_PATH, int(on))
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")
 
@@ -335,8 +336,26 @@ def argus_resample(ctx, wcs, W, H, nside, kernel, value_out, weight_out, idx=Non
     _check(ctx, rc, "argus_resample")
 
 
+def _host_frame_struct(raw_host, bias, dark, flat, offset, gain, t_exp, sat_adu, flat_min) -> _Frame:
+    """argus_frame with a HOST raw pointer and DEVICE masters (bias / dark / flat, or the pre-fused offset / gain)."""
+    f = _Frame()
+    f.raw = raw_host.data_ptr()
+    if offset is not None:
+        if offset.dtype != gain.dtype or offset.dtype not in (torch.float32, torch.float16):
+            raise TypeError("offset and gain must both be float32 or both float16")
+        f.offset = _dev(offset, offset.dtype, "offset")
+        f.gain = _dev(gain, gain.dtype, "gain")
+        f.masters_format = ARGUS_MASTERS_F32 if offset.dtype == torch.float32 else ARGUS_MASTERS_F16
+    else:
+        f.bias = _dev(bias, torch.float32, "bias")
+        f.dark = _dev(dark, torch.float32, "dark")
+        f.flat = _dev(flat, torch.float32, "flat")
+    f.t_exp, f.sat_adu, f.flat_min = float(t_exp), int(sat_adu), float(flat_min)
+    return f
+
+
 def argus_resample_host(ctx, wcs, W, H, nside, kernel, n, raw_host, value_host, weight_host, w_min=0.5, stream=None,
-                        bias=None, dark=None, flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1):
+                        bias=None, dark=None, flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1, offset=None, gain=None):
     """A2-A5 with HOST frame / outputs (CPU tensors, pinned for asynchronous copies); masters are CUDA tensors.
     Asynchronous: call argus_host_wait(ctx) before reading value_host / weight_host."""
     for t, dt, name in ((raw_host, torch.uint16, "raw_host"), (value_host, torch.float32, "value_host"),
@@ -345,12 +364,7 @@ def argus_resample_host(ctx, wcs, W, H, nside, kernel, n, raw_host, value_host, 
             raise TypeError("%s must be a contiguous CPU tensor of dtype %s" % (name, dt))
     if raw_host.numel() != W * H or value_host.numel() < n or weight_host.numel() < n:
         raise ValueError("host buffers too small")
-    f = _Frame()
-    f.raw = raw_host.data_ptr()
-    f.bias = _dev(bias, torch.float32, "bias")
-    f.dark = _dev(dark, torch.float32, "dark")
-    f.flat = _dev(flat, torch.float32, "flat")
-    f.t_exp, f.sat_adu, f.flat_min = float(t_exp), int(sat_adu), float(flat_min)
+    f = _host_frame_struct(raw_host, bias, dark, flat, offset, gain, t_exp, sat_adu, flat_min)
     w = _wcs_struct(wcs)
     rc = load_library().argus_resample_host(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min), int(n),
                                             value_host.data_ptr(), weight_host.data_ptr(), _stream(stream))
@@ -394,18 +408,14 @@ def argus_resample_coadd(ctx, wcs, W, H, nside, kernel, tiles, nside_tile, sum_,
 
 
 def argus_resample_coadd_host(ctx, wcs, W, H, nside, kernel, raw_host, tiles, nside_tile, sum_, wsum, n_skipped=None,
-                              w_min=0.5, stream=None, bias=None, dark=None, flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1):
+                              w_min=0.5, stream=None, bias=None, dark=None, flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1,
+                              offset=None, gain=None):
     """A2-A6 fused with the raw frame in HOST memory (pinned CPU tensor); masters and the coadd are CUDA tensors."""
     if not isinstance(raw_host, torch.Tensor) or raw_host.is_cuda or raw_host.dtype != torch.uint16 or not raw_host.is_contiguous():
         raise TypeError("raw_host must be a contiguous CPU uint16 tensor")
     if raw_host.numel() != W * H:
         raise ValueError("raw_host does not hold W * H pixels")
-    f = _Frame()
-    f.raw = raw_host.data_ptr()
-    f.bias = _dev(bias, torch.float32, "bias")
-    f.dark = _dev(dark, torch.float32, "dark")
-    f.flat = _dev(flat, torch.float32, "flat")
-    f.t_exp, f.sat_adu, f.flat_min = float(t_exp), int(sat_adu), float(flat_min)
+    f = _host_frame_struct(raw_host, bias, dark, flat, offset, gain, t_exp, sat_adu, flat_min)
     w = _wcs_struct(wcs)
     lay = _coadd_struct(tiles, nside_tile)
     rc = load_library().argus_resample_coadd_host(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min),

@@ -13,6 +13,7 @@
 #include "plan_block.cuh"
 #include "resample.cuh"
 #include "resample_fast.cuh"
+#include "resample_unit.cuh"
 #include "segments.cuh"
 #include "background.cuh"
 #include "subtract.cuh"
@@ -52,8 +53,20 @@ struct argus_ctx {
     // TMA descriptors of the fast kernel, cached per (pointers, W, H)
     void* encode_fn;      // cuTensorMapEncodeTiled, resolved at first use (no link-time libcuda dependency)
     bool encode_tried;
-    bool fast_enabled;    // ARGUS_OPT_FAST_PATH
+    bool fast_enabled;    // ARGUS_OPT_FAST_PATH != 0
+    bool unit_forced;     // ARGUS_OPT_FAST_PATH == 3: units wherever their geometry allows (diagnostic)
+    bool unit_enabled;    // ARGUS_OPT_FAST_PATH == 1 or 3: image-aligned work units (resample_unit.cuh) where the geometry allows
     bool fast_attr_set;
+    bool unit_attr_set;
+    bool plan_unit;       // the cached plan carries unit segment lists for plan_geom
+    UnitGeom plan_geom;
+    UnitBuffers slot_ub[PLAN_SLOTS];
+    void* unit_block[PLAN_SLOTS];
+    size_t unit_cap;      // units the unit scratch holds
+    UnitMaps umaps;       // TMA descriptors of the unit kernel, cached per (pointers, W, H, box, masters format)
+    const void* umaps_key[4];
+    int64_t umaps_W, umaps_H;
+    int umaps_bw, umaps_bh, umaps_fmt;
     FastMaps maps;
     const void* maps_key[4];
     int64_t maps_W, maps_H;
@@ -272,6 +285,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     c->device = device;
     c->plan_cache = true;
     c->fast_enabled = true;
+    c->unit_enabled = true;
     c->auto_tiles = max_tiles == 0;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -312,6 +326,7 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
         for (int j = 0; j < 4; ++j) cudaEventDestroy(c->ev[i][j]);
     for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
         if (c->slot_block[sidx]) cudaFree(c->slot_block[sidx]);
+        if (c->unit_block[sidx]) cudaFree(c->unit_block[sidx]);
         cudaEventDestroy(c->ev_done[sidx]);
         cudaEventDestroy(c->ev_free[sidx]);
     }
@@ -368,6 +383,8 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
     }
     if (option == ARGUS_OPT_FAST_PATH) {
         c->fast_enabled = value != 0;
+        c->unit_enabled = value == 1 || value == 3;
+        c->unit_forced = value == 3;
         return ARGUS_OK;
     }
     return ARGUS_ERR_SHAPE;
@@ -464,22 +481,49 @@ static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t 
 }
 
 // Enqueue the plan kernels (A0 + A1).  No host synchronisation.
-static bool plan_usable(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, bool need_full, int fast_kernel) {
+static bool plan_usable(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, bool need_full, int fast_kernel,
+                        const UnitGeom* ug) {
     // the fast kernel's boxes are sized for one interpolation kernel's taps; the general kernel does not care
     return same_key(c, w, W, H, nside) && (!need_full || c->plan_full) &&
-           (fast_kernel < 0 || c->plan_fast_kernel == (fast_kernel == ARGUS_LANCZOS3 ? 1 : 0));
+           (fast_kernel < 0 || c->plan_fast_kernel == (fast_kernel == ARGUS_LANCZOS3 ? 1 : 0)) &&
+           (ug ? (c->plan_unit && memcmp(&c->plan_geom, ug, sizeof(UnitGeom)) == 0) : (fast_kernel < 0 || !c->plan_unit));
 }
 
 // fast_kernel: interpolation kernel the fast (TMA-staged) kernel will run with, -1 = general kernel only (full plan).
+// Scratch of the image-aligned units (resample_unit.cuh), one set per plan slot: segment counts (+ the stray counter),
+// segment records, stray list.  Grown on demand (synchronises the device).
+static int ensure_unit_scratch(argus_ctx* c, size_t n_units, int max_stray) {
+    if (c->unit_block[0] && c->unit_cap >= n_units) return ARGUS_OK;
+    if (c->unit_block[0]) {
+        CUDA_TRY(c, cudaDeviceSynchronize());
+        for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) { cudaFree(c->unit_block[sidx]); c->unit_block[sidx] = nullptr; }
+    }
+    c->plan_valid = false;
+    const size_t want = align_up(n_units + 1, 1024);
+    const size_t o_seg = align_up((want + 1) * sizeof(int), 256), o_stray = o_seg + align_up(want * UNIT_MAXSEG * sizeof(UnitSeg), 256);
+    const size_t total = o_stray + (size_t)max_stray * sizeof(int);
+    for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
+        CUDA_TRY(c, cudaMalloc(&c->unit_block[sidx], total));
+        char* b = (char*)c->unit_block[sidx];
+        c->slot_ub[sidx].nseg = (int*)b;
+        c->slot_ub[sidx].stray_count = (int*)b + n_units;      // zeroed together with nseg; re-pointed below when n_units changes
+        c->slot_ub[sidx].seg = (UnitSeg*)(b + o_seg);
+        c->slot_ub[sidx].stray_list = (int*)(b + o_stray);
+    }
+    c->unit_cap = want - 1;
+    return ARGUS_OK;
+}
+
+// ug: unit geometry when the image-aligned unit kernel will run the frame (segment lists are built), else NULL.
 static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
-                      cudaStream_t caller, int fast_kernel, int prof_slot) {
+                      cudaStream_t caller, int fast_kernel, int prof_slot, const UnitGeom* ug = nullptr) {
     // Lanczos-3: any tile may be handed to the general kernel at run time (masked pixels in its box) => full records
     const bool need_full = fast_kernel != ARGUS_BILINEAR;
     DevWcs dw;
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
     if (rc) return rc;
-    if (plan_usable(c, w, W, H, nside, need_full, fast_kernel)) {
+    if (plan_usable(c, w, W, H, nside, need_full, fast_kernel, ug)) {
         if (out_cap >= 0) {   // cached plan: the capacity of THIS call's outputs still has to be checked
             plan_check_capacity_kernel<<<1, 32, 0, caller>>>(c->pb, out_cap);
             c->n_launches++;
@@ -545,7 +589,12 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
         c->side_next ^= 1;
         if (c->slot_used[ps]) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_free[ps], 0));
     }
+    if (ug) {
+        int rcu = ensure_unit_scratch(c, (size_t)ug->nux * (size_t)ug->nuy, ug->max_stray);
+        if (rcu) return rcu;
+    }
     c->pb = c->slot_pb[ps];
+    c->pb.unit_mode = ug ? 1 : 0;
     c->cur_slot = ps;
     {   // tap apron and stage capacity the fast kernel's boxes are sized for (a full plan keeps bilinear boxes)
         const int fk = fast_kernel == ARGUS_LANCZOS3 ? 1 : 0;
@@ -586,6 +635,17 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
         plan_offsets_kernel<<<gb < 1 ? 1 : gb, 256, 0, st>>>(c->pb, out_cap);
     }
     c->n_launches += 2;
+    if (ug) {   // segment lists of the image-aligned units (resample_unit.cuh)
+        const size_t n_units = (size_t)ug->nux * (size_t)ug->nuy;
+        c->slot_ub[ps].stray_count = c->slot_ub[ps].nseg + n_units;
+        CUDA_TRY(c, cudaMemsetAsync(c->slot_ub[ps].nseg, 0, (n_units + 1) * sizeof(int), st));
+        {   // one warp per tile, all tiles in flight at once (the kernel is a chain of latencies per tile)
+            long long bound = tile_bound < c->pb.max_tiles ? tile_bound : c->pb.max_tiles;
+            int gu = (int)((bound + 7) / 8);
+            plan_units_kernel<<<gu < 1 ? 1 : gu, 256, 0, st>>>(c->pb, *ug, c->slot_ub[ps]);
+        }
+        c->n_launches++;
+    }
     CUDA_TRY(c, cudaGetLastError());
     if (prof_slot >= 0) cudaEventRecord(c->ev[prof_slot][1], st);
     if (c->overlap) {
@@ -598,6 +658,8 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     c->plan_valid = true;
     c->plan_full = need_full;
     c->plan_fast_kernel = fast_kernel == ARGUS_LANCZOS3 ? 1 : 0;
+    c->plan_unit = ug != nullptr;
+    if (ug) c->plan_geom = *ug;
     return ARGUS_OK;
 }
 
@@ -780,6 +842,193 @@ static bool fast_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H) {
     return true;
 }
 
+// ------------------------------------------------------------------------- image-aligned units: host side
+static unsigned long long host_spread(unsigned v) {      // bit i -> bit 2 i
+    unsigned long long r = 0;
+    for (int b = 0; b < 32; ++b) r |= (unsigned long long)((v >> b) & 1u) << (2 * b);
+    return r;
+}
+
+static void host_vec_to_xy(const DevWcs& w, const double v[3], double& x, double& y) {   // inverse TAN (+ SIP), as vec_to_xy
+    const double cosc = v[0] * w.er[0] + v[1] * w.er[1] + v[2] * w.er[2], inv = 1.0 / cosc;
+    const double xi = (v[0] * w.ee[0] + v[1] * w.ee[1] + v[2] * w.ee[2]) * inv, eta = (v[0] * w.en[0] + v[1] * w.en[1] + v[2] * w.en[2]) * inv;
+    const double U = w.m[0][0] * xi + w.m[0][1] * eta, V = w.m[1][0] * xi + w.m[1][1] * eta;
+    double fu = 0.0, fv = 0.0, up = 1.0;
+    for (int p = 0; p <= w.sip_order && w.sip_order > 0; ++p) {
+        double m = up;
+        for (int q = 0; p + q <= w.sip_order; ++q) { fu += w.ap[p * 6 + q] * m; fv += w.bp[p * 6 + q] * m; m *= V; }
+        up *= U;
+    }
+    x = U + fu + w.crpix[0];
+    y = V + fv + w.crpix[1];
+}
+
+// Extent (cells) of a 4 x 4-pixel sub-block about its centre, per image axis: 1.5 (|dx/dix| + |dx/diy|) from the Jacobian
+// of the pixel -> image mapping at the HEALPix pixel nearest to the sky direction v (descent by closest child centre).
+static void unit_extent_at(const DevWcs& w, const argus_wcs* wc, int64_t nside, const double v[3], double& ex, double& ey) {
+    long long p = 0;
+    double best = -2.0;
+    for (int b = 0; b < 12; ++b) {
+        double c[3];
+        host_cell_centre(1, b, c);
+        const double d = c[0] * v[0] + c[1] * v[1] + c[2] * v[2];
+        if (d > best) { best = d; p = b; }
+    }
+    for (int64_t ns = 2; ns <= nside; ns <<= 1) {
+        long long bp = 4 * p;
+        best = -2.0;
+        for (int ch = 0; ch < 4; ++ch) {
+            double c[3];
+            host_cell_centre(ns, 4 * p + ch, c);
+            const double d = c[0] * v[0] + c[1] * v[1] + c[2] * v[2];
+            if (d > best) { best = d; bp = 4 * p + ch; }
+        }
+        p = bp;
+    }
+    const int k = ilog2(nside);
+    int face, ix, iy;
+    nest_to_xyf(p, k, face, ix, iy);
+    const int dx = ix + 1 < nside ? 1 : -1, dy = iy + 1 < nside ? 1 : -1;
+    double c0[3], c1[3], c2[3], x0, y0, x1, y1, x2, y2;
+    const long long fb = (long long)face << (2 * k);
+    host_cell_centre(nside, p, c0);
+    host_cell_centre(nside, fb | (long long)(host_spread((unsigned)(ix + dx)) | (host_spread((unsigned)iy) << 1)), c1);
+    host_cell_centre(nside, fb | (long long)(host_spread((unsigned)ix) | (host_spread((unsigned)(iy + dy)) << 1)), c2);
+    host_vec_to_xy(w, c0, x0, y0); host_vec_to_xy(w, c1, x1, y1); host_vec_to_xy(w, c2, x2, y2);
+    (void)wc;
+    ex = 1.5 * (fabs(x1 - x0) + fabs(x2 - x0));
+    ey = 1.5 * (fabs(y1 - y0) + fabs(y2 - y0));
+}
+
+// Unit geometry for (wcs, W, H, nside, kernel): false when units do not fit a stage (very coarse HEALPix pixels) -- the tile
+// kernel or the general kernel then runs the frame.  The extents are ESTIMATES from nine sky directions (centre, corners,
+// edge midpoints); a sub-block that exceeds them anyway is found by plan_units_kernel and served by the stray kernel.
+static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, double s_rad, int kernel, UnitGeom* g,
+                          bool* tiles_fit) {
+    if (kernel != ARGUS_BILINEAR) return false;
+    double ex = 0.0, ey = 0.0;
+    *tiles_fit = true;
+    for (int sy = -1; sy <= 1; ++sy)
+        for (int sx = -1; sx <= 1; ++sx) {
+            const double px = 0.45 * sx * (double)W, py = 0.45 * sy * (double)H;       // pixel offsets from CRPIX (about the frame centre)
+            const double d2r = kPi / 180.0;
+            const double xi = (w->cd[0][0] * px + w->cd[0][1] * py) * d2r, eta = (w->cd[1][0] * px + w->cd[1][1] * py) * d2r;
+            double v[3];
+            for (int i = 0; i < 3; ++i) v[i] = dw.er[i] + xi * dw.ee[i] + eta * dw.en[i];
+            const double nrm = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+            for (int i = 0; i < 3; ++i) v[i] /= nrm;
+            double ax, ay;
+            unit_extent_at(dw, w, nside, v, ax, ay);
+            if (!(ax < 64.0) || !(ay < 64.0)) return false;
+            ex = fmax(ex, ax); ey = fmax(ey, ay);
+            {   // would a whole 32 x 32-pixel tile fit the tile kernel's stage here?  (mirror of fast_box, worst-case alignment)
+                const int span_x = (int)ceil(31.0 / 1.5 * ax) + 1, span_y = (int)ceil(31.0 / 1.5 * ay) + 1;
+                const int bw = span_x + 1 + 7, bh = span_y + 1;
+                const int boxw = bw <= 40 ? 40 : (bw + 7) / 8 * 8, boxh = bh <= 48 ? 48 : (bh + 7) / 8 * 8;
+                if (bw > 72 || bh > 72 || boxw * boxh > FAST_CAP_PX) *tiles_fit = false;
+            }
+        }
+    memset(g, 0, sizeof(*g));
+    g->tl = 0; g->tr = 1;
+    g->Mx = (int)ceil(1.03 * ex + 0.02); g->My = (int)ceil(1.03 * ey + 0.02);
+    g->BW = UNIT_BOXW;
+    g->RW = (g->BW - 2 * g->Mx - g->tl - g->tr) & ~7;
+    int bh = UNIT_CAP / g->BW;
+    g->RH = bh - 2 * g->My - g->tl - g->tr;
+    if (g->RW < 16 || g->RH < 8) return false;
+    // sub-blocks per unit: owned cells x HEALPix pixels per cell / 16; keep the expected number below 0.55 of the list
+    const double hp_per_cell = s_rad * s_rad / (4.0 * kPi / (12.0 * (double)nside * (double)nside));
+    while (g->RH > 8 && (double)g->RW * g->RH * hp_per_cell / 16.0 > 0.55 * UNIT_MAXSB) g->RH -= 2;
+    if ((double)g->RW * g->RH * hp_per_cell / 16.0 > 0.55 * UNIT_MAXSB) return false;
+    if ((double)g->RW * g->RH * hp_per_cell < 64.0) return false;     // a handful of outputs per unit: not worth a stage
+    g->BH = g->RH + 2 * g->My + g->tl + g->tr;
+    const int kx = (g->Mx + g->tl + 1 + 7) / 8;
+    g->x_off = g->Mx + g->tl - 8 * kx;                                  // <= -1 and (x_off - Mx - tl) % 8 == 0
+    g->y_off = -1;
+    g->nux = (int)((W - g->x_off + g->RW - 1) / g->RW);
+    g->nuy = (int)((H - g->y_off + g->RH - 1) / g->RH);
+    if ((long long)g->nux * g->nuy > (1ll << 24)) return false;
+    g->max_stray = 1 << 16;
+    return true;
+}
+
+// TMA descriptors of the unit kernel: one {BW, BH} box per array.  Off-frame elements: zero fill for raw / bias / dark /
+// flat (flat = 0 < flat_min: masked), NaN fill for the pre-fused gain (NaN gain: masked).
+static bool unit_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H, const UnitGeom& g) {
+    if (!c->encode_tried) {
+        c->encode_tried = true;
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+            c->encode_fn = fn;
+        else
+            (void)cudaGetLastError();
+    }
+    if (!c->encode_fn) return false;
+    const void* key[4] = {f.raw, f.pre ? f.offset : (const void*)f.bias, f.pre ? f.gain : (const void*)f.dark, f.pre ? nullptr : (const void*)f.flat};
+    if (memcmp(key, c->umaps_key, sizeof(key)) == 0 && c->umaps_W == W && c->umaps_H == H && c->umaps_bw == g.BW && c->umaps_bh == g.BH &&
+        c->umaps_fmt == f.pre)
+        return true;
+    encode_tiled_fn enc = (encode_tiled_fn)c->encode_fn;
+    const int narr = f.pre ? 3 : 4;
+    for (int a = 0; a < narr; ++a) {
+        const bool half = f.pre == 2 && a > 0;
+        const unsigned es = a == 0 ? 2u : (half ? 2u : 4u);
+        cuuint64_t dims[2] = {(cuuint64_t)W, (cuuint64_t)H};
+        cuuint64_t strides[1] = {(cuuint64_t)W * es};
+        cuuint32_t box[2] = {(cuuint32_t)g.BW, (cuuint32_t)g.BH};
+        cuuint32_t el[2] = {1, 1};
+        const CUtensorMapDataType dt = a == 0 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : (half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32);
+        const CUtensorMapFloatOOBfill fill = (f.pre && a == 2) ? CU_TENSOR_MAP_FLOAT_OOB_FILL_NAN_REQUEST_ZERO_FMA : CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE;
+        CUresult r = enc(&c->umaps.m[a], dt, 2, const_cast<void*>(key[a]), dims, strides, box, el, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, fill);
+        if (r != CUDA_SUCCESS) { c->umaps_W = -1; return false; }
+    }
+    memcpy(c->umaps_key, key, sizeof(key));
+    c->umaps_W = W; c->umaps_H = H; c->umaps_bw = g.BW; c->umaps_bh = g.BH; c->umaps_fmt = f.pre;
+    return true;
+}
+
+// Which kernel runs the planned frame: 2 = image-aligned units, 1 = tile kernel (resample_fast.cuh), 0 = general kernel.
+static int choose_path(argus_ctx* c, const FrameArgs& f, bool fused, int kernel, const argus_wcs* wcs, int64_t W, int64_t H, int64_t nside,
+                       UnitGeom* ug) {
+    if (!fused || !c->fast_enabled) return 0;
+    if (c->unit_enabled && kernel == ARGUS_BILINEAR && f.raw && !f.bpm && W % 8 == 0 && W >= 8 && aligned(f.raw, 16) &&
+        (f.pre ? (aligned(f.offset, 16) && aligned(f.gain, 16)) : (aligned(f.bias, 16) && aligned(f.dark, 16) && aligned(f.flat, 16)))) {
+        DevWcs dw;
+        double rho, s_rad;
+        // units where the tile kernel cannot run the frame: pre-fused masters, or tiles whose bounding box does not fit its
+        // stage somewhere on the frame (HEALPix tiles are wide near the equator and tall in the polar caps); where its
+        // boxes fit, the tile kernel is the faster one (0.28 vs 0.33 ms at configs[1]: DESIGN.md 6.6)
+        bool tiles_fit = true;
+        if (make_devwcs(wcs, W, H, nside, &dw, &rho, &s_rad) == ARGUS_OK && unit_geometry(dw, wcs, W, H, nside, s_rad, kernel, ug, &tiles_fit) &&
+            (f.pre || !tiles_fit || c->unit_forced) && unit_maps(c, f, W, H, *ug))
+            return 2;
+    }
+    return fast_maps(c, f, W, H) ? 1 : 0;
+}
+
+template <bool COADD>
+static int launch_units(argus_ctx* c, const UnitGeom& g, const FrameArgs& f, float w_min, float* v, float* wt, long long cap,
+                        const CoaddArgs& ca, cudaStream_t st) {
+    if (!c->unit_attr_set) {
+#define UA(CO, M) CUDA_TRY(c, cudaFuncSetAttribute(resample_unit_kernel<CO, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(UnitSmem<M>)))
+        UA(false, 0); UA(true, 0); UA(false, 1); UA(true, 1); UA(false, 2); UA(true, 2);
+#undef UA
+        c->unit_attr_set = true;
+    }
+    const UnitBuffers& ub = c->slot_ub[c->cur_slot];
+    const int grid = c->sm_count * 2;
+#define UL(M) resample_unit_kernel<COADD, M><<<grid, RF_THREADS, sizeof(UnitSmem<M>), st>>>(c->umaps, c->pb, ub, g, f, w_min, v, wt, cap, ca)
+    if (f.pre == 0) UL(0); else if (f.pre == 1) UL(1); else UL(2);
+#undef UL
+    resample_stray_kernel<COADD><<<c->sm_count, 256, 0, st>>>(c->dw, c->pb, ub, g.max_stray, f, w_min, v, wt, cap, ca);
+    // the plan's slow list (ring / pole tiles, tiles whose cubic does not fit the fixed-point split): general kernel
+    resample_tiles_kernel<0, true, COADD><<<c->sm_count * 2, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca, 1);
+    c->n_launches += 3;
+    return ARGUS_OK;
+}
+
 template <bool COADD>
 static int launch_tiles(argus_ctx* c, int kernel, bool fused, bool use_fast, const FrameArgs& f, int64_t W, int64_t H, float w_min,
                         float* v, float* wt, long long cap, const CoaddArgs& ca, cudaStream_t st) {
@@ -843,14 +1092,17 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
         return ARGUS_OK;
     }
     int slot = c->prof_n & 255;
-    const bool use_fast = fused && fast_maps(c, f, W, H);
-    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1);
-    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, use_fast ? kernel : -1, c->profile ? slot : -1);
+    UnitGeom ug;
+    const int path = choose_path(c, f, fused, kernel, wcs, W, H, nside, &ug);
+    const bool use_fast = path != 0;
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1, path == 2 ? &ug : nullptr);
+    rc = build_plan(c, wcs, W, H, nside, (long long)n, st, use_fast ? kernel : -1, c->profile ? slot : -1, path == 2 ? &ug : nullptr);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
     CoaddArgs ca;
     memset(&ca, 0, sizeof(ca));
-    rc = launch_tiles<false>(c, kernel, fused, use_fast, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
+    if (path == 2) rc = launch_units<false>(c, ug, f, w_min, value_out, weight_out, (long long)n, ca, st);
+    else rc = launch_tiles<false>(c, kernel, fused, use_fast, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
     if (rc) return rc;
     mark_slot_read(c, st);
     if (c->profile) { cudaEventRecord(c->ev[slot][3], st); c->ev_plan[slot] = replanned; c->prof_n++; }
@@ -1002,12 +1254,15 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
     int slot = c->prof_n & 255;
-    const bool use_fast = fused && fast_maps(c, f, W, H);
-    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1);
-    rc = build_plan(c, wcs, W, H, nside, -1, st, use_fast ? kernel : -1, c->profile ? slot : -1);
+    UnitGeom ug;
+    const int path = choose_path(c, f, fused, kernel, wcs, W, H, nside, &ug);
+    const bool use_fast = path != 0;
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1, path == 2 ? &ug : nullptr);
+    rc = build_plan(c, wcs, W, H, nside, -1, st, use_fast ? kernel : -1, c->profile ? slot : -1, path == 2 ? &ug : nullptr);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
-    rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
+    if (path == 2) rc = launch_units<true>(c, ug, f, w_min, nullptr, nullptr, 0, ca, st);
+    else rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
     if (rc) return rc;
     mark_slot_read(c, st);
     if (c->profile) { cudaEventRecord(c->ev[slot][3], st); c->ev_plan[slot] = replanned; c->prof_n++; }

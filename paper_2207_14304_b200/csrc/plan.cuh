@@ -50,6 +50,7 @@ struct PlanBuffers {
     double* bcoef;              // [max_tiles/64][32] block quartics (15 x, 15 y), [30] = zone or -1 (no block fit)
     int max_slots, max_tiles, max_hard;
     int fast_tl, fast_tr, fast_cap;   // tap apron and stage capacity (pixels) of the fast kernel this plan is for
+    int unit_mode;                    // the image-aligned unit kernel runs the frame: no per-tile box limits (resample_unit.cuh)
 };
 
 // Overflow bits (PlanStats.overflow) live in the plan slot and are zeroed by the next plan into it; the context-wide
@@ -250,7 +251,7 @@ __device__ inline void emit_tile(const PlanBuffers& pb, int t, long long tile, i
         f.mask_slot = r.mask_slot;
         f.poly_ok = poly_ok ? 1 : 0;
         if (cls == TC_INSIDE) {
-            if (poly_ok && fast_box(pb, r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f)) { f.cls = TC_INSIDE; fast_inside = true; }
+            if (poly_ok && (pb.unit_mode || fast_box(pb, r.bx0, r.bx1, r.by0, r.by1, f.X0, f.Y0, f))) { f.cls = TC_INSIDE; fast_inside = true; }
             else slow_push(pb, t);
         }   // TC_BORDER: plan_members_kernel finalises the box and decides
         if (!(lite && fast_inside)) {
@@ -448,7 +449,7 @@ __global__ void __launch_bounds__(256, 4) plan_members_kernel(DevWcs w, PlanBuff
                 if (cls == TC_BORDER) {
                     FastRec* fr = &pb.frec[t];
                     FastRec f = *fr;
-                    if (f.poly_ok && fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f)) {
+                    if (f.poly_ok && (pb.unit_mode || fast_box(pb, e0, e1, e2, e3, f.X0, f.Y0, f))) {
                         f.cls = TC_BORDER;
                         *fr = f;
                     } else {
