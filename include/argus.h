@@ -137,6 +137,8 @@ typedef struct argus_plan_stats {
     int64_t n_border;     /* tiles cut by the frame border */
     int64_t n_exact;      /* tiles evaluated per pixel in FP64 (belt/cap ring, poles, failed fits) */
     int64_t n_empty;      /* candidate tiles that turned out empty */
+    int64_t n_units;      /* image-aligned work units of the plan (0: the tile or general kernel runs the frame) */
+    int64_t n_stray;      /* 4 x 4-pixel sub-blocks no unit can serve (per-pixel FP64 path); normally 0 */
 } argus_plan_stats;
 
 const char* argus_strerror(int status);

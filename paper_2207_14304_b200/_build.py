@@ -28,7 +28,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not os.path.exists(nvcc):
         nvcc = "nvcc"
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+    extra = os.environ.get("ARGUS_NVCC_EXTRA", "").split()   # e.g. -DARGUS_DEBUG_BOUNDS (tests), tuning macros
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
     subprocess.run(cmd, check=True, cwd=CSRC)
     os.replace(tmp, LIB)
     return LIB

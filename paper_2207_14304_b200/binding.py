@@ -56,7 +56,7 @@ class _SubParams(C.Structure):
 
 
 class _PlanStats(C.Structure):
-    _fields_ = [(n, C.c_int64) for n in ("n_footprint", "n_tiles", "n_inside", "n_border", "n_exact", "n_empty")]
+    _fields_ = [(n, C.c_int64) for n in ("n_footprint", "n_tiles", "n_inside", "n_border", "n_exact", "n_empty", "n_units", "n_stray")]
 
 
 _lib = None

@@ -187,7 +187,7 @@ static cudaError_t alloc_plan_slot(int64_t max_tiles, int64_t max_slots, PlanBuf
     pb.max_tiles = (int)max_tiles;
     pb.max_slots = (int)max_slots;
     pb.max_hard = (int)(max_tiles / 4 < 1024 ? 1024 : max_tiles / 4);
-    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4, o_bc2, o_sp;
+    size_t o = 0, o_flag, o_bc, o_tid, o_rec, o_cnt, o_off, o_nt, o_hc, o_hl, o_mask, o_stats, o_pinv, o_dc, o_cls, o_bs, o_bb, o_fr, o_sc, o_sl, o_bid, o_nb, o_fc, o_fl, o_tk, o_p4, o_bc2, o_sp, o_cs;
     o_flag = o;  o = align_up(o + (size_t)pb.max_slots, 256);
     o_bc = o;    o = align_up(o + sizeof(int) * (pb.max_slots / 256 + 1), 256);
     o_tid = o;   o = align_up(o + sizeof(long long) * pb.max_tiles, 256);
@@ -208,6 +208,7 @@ static cudaError_t alloc_plan_slot(int64_t max_tiles, int64_t max_slots, PlanBuf
     o_sc = o;    o = align_up(o + sizeof(int), 256);
     o_sl = o;    o = align_up(o + sizeof(int) * (size_t)pb.max_tiles, 256);   // any tile may end up on the slow list
     o_sp = o;    o = align_up(o + sizeof(int), 256);
+    o_cs = o;    o = align_up(o + sizeof(long long) * (size_t)pb.max_tiles, 256);
     o_bid = o;   o = align_up(o + sizeof(long long) * (pb.max_tiles / 64 + 1), 256);
     o_nb = o;    o = align_up(o + sizeof(int), 256);
     o_fc = o;    o = align_up(o + sizeof(int), 256);
@@ -239,6 +240,7 @@ static cudaError_t alloc_plan_slot(int64_t max_tiles, int64_t max_slots, PlanBuf
     pb.slow_count = (int*)(b + o_sc);
     pb.slow_list = (int*)(b + o_sl);
     pb.slow_plan = (int*)(b + o_sp);
+    pb.cslot = (long long*)(b + o_cs);
     pb.block_id = (long long*)(b + o_bid);
     pb.n_blocks = (int*)(b + o_nb);
     pb.fb_count = (int*)(b + o_fc);
@@ -292,7 +294,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
     cudaError_t e2 = cudaMalloc((void**)&c->d_latch, 2 * sizeof(int));
     if (e2 == cudaSuccess) e2 = cudaMemset(c->d_latch, 0, 2 * sizeof(int));
-    if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_latch, sizeof(int));
+    if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_latch, 2 * sizeof(int));
     if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
     int rc_slots = ARGUS_OK;
     if (e2 == cudaSuccess && !c->auto_tiles) rc_slots = alloc_plan_slots(c, max_tiles, default_max_slots(max_tiles));
@@ -757,6 +759,9 @@ static int fetch_stats(argus_ctx* c, cudaStream_t st, int* latched) {
     plan_latch_fetch_kernel<<<1, 32, 0, st>>>(c->d_latch, c->d_latch + 1);
     c->n_launches++;
     CUDA_TRY(c, cudaMemcpyAsync(c->h_latch, c->d_latch + 1, sizeof(int), cudaMemcpyDeviceToHost, st));
+    c->h_latch[1] = 0;
+    if (c->plan_valid && c->plan_unit)
+        CUDA_TRY(c, cudaMemcpyAsync(c->h_latch + 1, c->slot_ub[c->cur_slot].stray_count, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaStreamSynchronize(st));
     *latched = *c->h_latch;
     return ARGUS_OK;
@@ -795,6 +800,8 @@ extern "C" int argus_plan_info(argus_ctx* c, argus_plan_stats* out, void* stream
     const PlanStats* s = c->h_stats;
     out->n_footprint = s->n_footprint; out->n_tiles = s->n_tiles; out->n_inside = s->n_inside;
     out->n_border = s->n_border; out->n_exact = s->n_exact; out->n_empty = s->n_empty;
+    out->n_units = (c->plan_valid && c->plan_unit) ? (int64_t)c->plan_geom.nux * c->plan_geom.nuy : 0;
+    out->n_stray = c->h_latch[1];
     if (s->overflow) c->plan_valid = false;
     if (s->overflow || latched) return ARGUS_ERR_CAPACITY;
     return ARGUS_OK;
@@ -922,7 +929,7 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
             if (!(ax < 64.0) || !(ay < 64.0)) return false;
             ex = fmax(ex, ax); ey = fmax(ey, ay);
             {   // would a whole 32 x 32-pixel tile fit the tile kernel's stage here?  (mirror of fast_box, worst-case alignment)
-                const int span_x = (int)ceil(31.0 / 1.5 * ax) + 1, span_y = (int)ceil(31.0 / 1.5 * ay) + 1;
+                const int span_x = (int)ceil(31.0 / 1.5 * ax) + 3, span_y = (int)ceil(31.0 / 1.5 * ay) + 3;   // + tile-to-tile variation
                 const int bw = span_x + 1 + 7, bh = span_y + 1;
                 const int boxw = bw <= 40 ? 40 : (bw + 7) / 8 * 8, boxh = bh <= 48 ? 48 : (bh + 7) / 8 * 8;
                 if (bw > 72 || bh > 72 || boxw * boxh > FAST_CAP_PX) *tiles_fit = false;
@@ -942,11 +949,13 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
     if ((double)g->RW * g->RH * hp_per_cell / 16.0 > 0.55 * UNIT_MAXSB) return false;
     if ((double)g->RW * g->RH * hp_per_cell < 64.0) return false;     // a handful of outputs per unit: not worth a stage
     g->BH = g->RH + 2 * g->My + g->tl + g->tr;
-    const int kx = (g->Mx + g->tl + 1 + 7) / 8;
-    g->x_off = g->Mx + g->tl - 8 * kx;                                  // <= -1 and (x_off - Mx - tl) % 8 == 0
-    g->y_off = -1;
-    g->nux = (int)((W - g->x_off + g->RW - 1) / g->RW);
-    g->nuy = (int)((H - g->y_off + g->RH - 1) / g->RH);
+    // the centre of a border tile's sub-block can lie up to its extent outside the frame: the grid starts at or below cell
+    // -(M + 2) and ends at or beyond cell W + M + 1
+    const int kx = (2 * g->Mx + g->tl + 2 + 7) / 8;
+    g->x_off = g->Mx + g->tl - 8 * kx;                                  // <= -(Mx + 2) and (x_off - Mx - tl) % 8 == 0
+    g->y_off = -(g->My + 2);
+    g->nux = (int)((W + g->Mx + 2 - g->x_off + g->RW - 1) / g->RW);
+    g->nuy = (int)((H + g->My + 2 - g->y_off + g->RH - 1) / g->RH);
     if ((long long)g->nux * g->nuy > (1ll << 24)) return false;
     g->max_stray = 1 << 16;
     return true;
@@ -1019,7 +1028,7 @@ static int launch_units(argus_ctx* c, const UnitGeom& g, const FrameArgs& f, flo
     }
     const UnitBuffers& ub = c->slot_ub[c->cur_slot];
     const int grid = c->sm_count * 2;
-#define UL(M) resample_unit_kernel<COADD, M><<<grid, RF_THREADS, sizeof(UnitSmem<M>), st>>>(c->umaps, c->pb, ub, g, f, w_min, v, wt, cap, ca)
+#define UL(M) resample_unit_kernel<COADD, M><<<grid, UNIT_THREADS, sizeof(UnitSmem<M>), st>>>(c->umaps, c->pb, ub, g, f, w_min, v, wt, cap, ca)
     if (f.pre == 0) UL(0); else if (f.pre == 1) UL(1); else UL(2);
 #undef UL
     resample_stray_kernel<COADD><<<c->sm_count, 256, 0, st>>>(c->dw, c->pb, ub, g.max_stray, f, w_min, v, wt, cap, ca);
@@ -1261,6 +1270,10 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     rc = build_plan(c, wcs, W, H, nside, -1, st, use_fast ? kernel : -1, c->profile ? slot : -1, path == 2 ? &ug : nullptr);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
+    if (use_fast) {
+        coadd_slots_kernel<<<c->sm_count, 256, 0, st>>>(c->pb, ca);
+        c->n_launches++;
+    }
     if (path == 2) rc = launch_units<true>(c, ug, f, w_min, nullptr, nullptr, 0, ca, st);
     else rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
     if (rc) return rc;

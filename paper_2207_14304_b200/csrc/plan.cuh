@@ -40,6 +40,7 @@ struct PlanBuffers {
     int* slow_plan;             // device scalar: slow_count as the plan left it; the Lanczos-3 fast kernel appends behind
                                 // it at run time and the general kernel restores it when it is done (a cached plan is reused)
     int* slow_list;             // [max_tiles] tiles the fast kernel leaves to the general kernel
+    long long* cslot;           // [max_tiles] coadd slot of each tile's first pixel for the layout of the current call (-1 = absent)
     int* latch;                 // context-wide: every overflow bit is also ORed in here; cleared only when read
     long long* block_id;        // [max_tiles/64] candidate blocks (8x8 tiles), ascending nested ids at block level
     int* n_blocks;              // device scalar

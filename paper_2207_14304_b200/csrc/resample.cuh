@@ -441,6 +441,23 @@ __global__ void __launch_bounds__(RS_THREADS, KERNEL == 0 ? RS_MIN_CTAS : 2) res
     }
 }
 
+// Coadd slot of every plan tile for this call's layout, once per call (a binary search per tile in the producers of the
+// staged kernels would sit on their critical path: 8 dependent loads per tile).
+__global__ void __launch_bounds__(256) coadd_slots_kernel(PlanBuffers pb, CoaddArgs ca) {
+    const int n = *pb.n_tiles;
+    for (int t = blockIdx.x * 256 + threadIdx.x; t < n; t += gridDim.x * 256) {
+        const long long tile = pb.tile_id[t];
+        long long key = tile >> ca.shift, lo = 0, hi = ca.n_tiles - 1, pos = -1;
+        while (lo <= hi) {
+            const long long mid = (lo + hi) >> 1, tv = __ldg(ca.tiles + mid);
+            if (tv == key) { pos = mid; break; }
+            if (tv < key) lo = mid + 1; else hi = mid - 1;
+        }
+        const long long ppt = 1ll << (ca.shift + 10);
+        pb.cslot[t] = pos < 0 ? -1 : pos * ppt + ((tile << 10) & (ppt - 1));
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // General path for an explicit pixel list (argus_resample with idx != NULL): one thread per pixel,
 // exact FP64 coordinates, taps straight from global memory.

@@ -370,17 +370,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
             if (lane == 0) {
                 d.off = off_c;
                 d.t = t;
-                if (COADD) {
-                    long long tile = pb.tile_id[t];
-                    long long key = tile >> ca.shift, lo = 0, hi = ca.n_tiles - 1, pos = -1;
-                    while (lo <= hi) {
-                        long long mid = (lo + hi) >> 1, tv = ca.tiles[mid];
-                        if (tv == key) { pos = mid; break; }
-                        if (tv < key) lo = mid + 1; else hi = mid - 1;
-                    }
-                    long long ppt = 1ll << (ca.shift + 10);
-                    d.cslot = pos < 0 ? -1 : pos * ppt + ((tile << 10) & (ppt - 1));
-                }
+                if (COADD) d.cslot = pb.cslot[t];               // coadd_slots_kernel, once per call
             }
             __syncwarp();
             if (lane == 0) mbar_arrive_expect_tx(&sm.full[ds], tx_bytes);   // releases the descriptor to the consumers

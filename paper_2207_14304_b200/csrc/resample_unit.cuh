@@ -26,7 +26,12 @@
 #define UNIT_MAXSEG 16                 // segments (distinct tiles) per unit
 #define UNIT_MAXSB 384                 // sub-blocks per unit
 #define UNIT_BOXW 72                   // staged box width (cells); 72 = 8 mod 16: pitch 72 is bank-conflict free
+#ifndef UNIT_CAP
 #define UNIT_CAP 3072                  // staged source pixels per stage (box width x box rows)
+#endif
+#ifndef UNIT_STAGES0
+#define UNIT_STAGES0 2                  // stages with raw masters (14 B per staged pixel)
+#endif
 
 struct UnitGeom {
     int RW, RH;                        // cells owned by a unit
@@ -92,15 +97,14 @@ __global__ void __launch_bounds__(256) plan_units_kernel(PlanBuffers pb, UnitGeo
                 const int cx = r.X0 + (xf >> FAST_FRAC_BITS), cy = r.Y0 + (yf >> FAST_FRAC_BITS);
                 const int i = floor_div(cx - g.x_off, g.RW), j = floor_div(cy - g.y_off, g.RH);
                 bool ok = i >= 0 && i < g.nux && j >= 0 && j < g.nuy;
-                const int x_lo = g.x_off + i * g.RW - g.Mx, x_hi = g.x_off + (i + 1) * g.RW - 1 + g.Mx;
-                const int y_lo = g.y_off + j * g.RH - g.My, y_hi = g.y_off + (j + 1) * g.RH - 1 + g.My;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {                      // the four corner pixels bound the sub-block's extent
-                    const int u = 4 * a + 3 * (q & 1), v = 4 * b + 3 * (q >> 1);
-                    unit_eval(r, 2 * u - 31, 2 * v - 31, xf, yf);
-                    const int px = r.X0 + (xf >> FAST_FRAC_BITS), py = r.Y0 + (yf >> FAST_FRAC_BITS);
-                    ok = ok && px >= x_lo && px <= x_hi && py >= y_lo && py <= y_hi;
-                }
+                // extent of the sub-block's pixels about its centre: the corner pixels are 3 half-pixel steps away in s and
+                // in t; linear part exact, + 2^-6 px for the cubic's variation over 1.5 pixels (< 4e-3 px) and rounding
+                const long long exl = 3ll * (llabs((long long)r.ax) + llabs((long long)r.bx)) + (1 << 18);
+                const long long eyl = 3ll * (llabs((long long)r.ay) + llabs((long long)r.by)) + (1 << 18);
+                const long long xc = ((long long)r.X0 << FAST_FRAC_BITS) + xf, yc = ((long long)r.Y0 << FAST_FRAC_BITS) + yf;
+                const long long x_lo = (long long)(g.x_off + i * g.RW - g.Mx) << FAST_FRAC_BITS, x_hi = (long long)(g.x_off + (i + 1) * g.RW + g.Mx) << FAST_FRAC_BITS;
+                const long long y_lo = (long long)(g.y_off + j * g.RH - g.My) << FAST_FRAC_BITS, y_hi = (long long)(g.y_off + (j + 1) * g.RH + g.My) << FAST_FRAC_BITS;
+                ok = ok && xc - exl >= x_lo && xc + exl < x_hi && yc - eyl >= y_lo && yc + eyl < y_hi;
                 key[h] = ok ? j * g.nux + i : -2;
             }
         }
@@ -157,7 +161,7 @@ template <int MASTERS> struct UnitCfg {
     static constexpr int ES = MASTERS == 2 ? 2 : 4;                       // bytes per master element
     static constexpr int PX_BYTES = 2 + (NARR - 1) * ES;
     static constexpr int STAGE_BYTES = UNIT_CAP * PX_BYTES;
-    static constexpr int STAGES = MASTERS == 2 ? 3 : 2;                   // 43 / 30 / 18 KB per stage: two CTAs per SM
+    static constexpr int STAGES = MASTERS == 2 ? 3 : (MASTERS == 0 ? UNIT_STAGES0 : 2);                   // 43 / 30 / 18 KB per stage: two CTAs per SM
 };
 
 struct __align__(16) UnitSegD {
@@ -168,10 +172,14 @@ struct __align__(16) UnitSegD {
     int mb;               // row of the border tables, -1 for inside tiles
     int pad[2];
 };
+#define UNIT_PREFETCH 0                // L2 prefetch distance of the box loads in units of one CTA; 0 = off (measured: 3 is 7 % slower)
+#define UNIT_PRODUCERS 2                // producer warps: the per-unit chain (records, offsets, work list) is a chain of latencies;
+                                        // warp p prepares the CTA's units number p, p + PRODUCERS, ... (the kernel was producer-bound with one)
+#define UNIT_THREADS (RF_CONSUMERS + 32 * UNIT_PRODUCERS)
 #define UNIT_NDESC 4                   // descriptors are prepared up to three units ahead of the stage they describe
 #define UNIT_MAXBORDER 6               // border-tile tables per unit (more: membership straight from global memory)
 struct __align__(16) UnitDesc {
-    int n_seg, n_sb, pad0, pad1;          // n_seg < 0: end of work; pad0 = bit set of the border segments
+    int n_seg, n_sb, pad0, pad1;          // n_seg < 0: end of work; pad0 / pad1 = bit sets of the border segments / of segments absent from the coadd layout
     UnitSegD seg[UNIT_MAXSEG];
     unsigned sb[UNIT_MAXSB];              // work list, grouped by segment: segment << 12 | sub-block << 6 | a << 3 | b
     unsigned bmask[UNIT_MAXBORDER][32];   // border tiles: membership bits and exclusive prefix of their popcounts
@@ -188,6 +196,10 @@ struct __align__(128) UnitSmem {
 
 struct UnitMaps { CUtensorMap m[4]; };    // raw, then the masters in stage order
 
+__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap* map, int x, int y) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(map), "r"(x), "r"(y) : "memory");
+}
+
 __device__ __forceinline__ float calib_unit_pre(unsigned magic_r, float off, float g, float sat_f) {
     const float rf = __uint_as_float(magic_r) - 8388608.0f;
     const float c = (rf - off) * g;                                        // R-M4; NaN gain (invalid, off-frame) -> NaN
@@ -196,7 +208,7 @@ __device__ __forceinline__ float calib_unit_pre(unsigned magic_r, float off, flo
 
 // ------------------------------------------------------------------------------------------- the kernel
 template <bool COADD, int MASTERS>
-__global__ void __launch_bounds__(RF_THREADS, 2)
+__global__ void __launch_bounds__(UNIT_THREADS, 2)
     resample_unit_kernel(const __grid_constant__ UnitMaps maps, PlanBuffers pb, UnitBuffers ub, UnitGeom g, FrameArgs f, float w_min,
                          float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap, CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -216,8 +228,8 @@ __global__ void __launch_bounds__(RF_THREADS, 2)
 
     if (tid >= RF_CONSUMERS) {
         // ================================================================ producer warp
-        const int lane = tid - RF_CONSUMERS;
-        int issued = 0;
+        const int lane = tid & 31, pw = (tid - RF_CONSUMERS) >> 5;      // producer warp pw of UNIT_PRODUCERS
+        int issued = 0;                                                 // sequence number of the CTA's non-empty units
         int u_n = blockIdx.x, nseg_n = 0;
         UnitSeg sg_n = {0, 0u, 0u, 0};
         if (u_n < n_units) {
@@ -235,6 +247,11 @@ __global__ void __launch_bounds__(RF_THREADS, 2)
                 if (lane < nseg_n) sg_n = ub.seg[(size_t)u_n * UNIT_MAXSEG + lane];
             }
             if (!last && nseg == 0) continue;
+            if (issued % UNIT_PRODUCERS != pw) {                        // another producer warp's unit
+                if (last) break;
+                ++issued;
+                continue;
+            }
             const int slot = issued % Cfg::STAGES, ds = issued % UNIT_NDESC;
             // descriptor slot free: the consumers are done with the unit that used it UNIT_NDESC units ago
             if (issued >= UNIT_NDESC) mbar_wait(&sm.dfree[ds], (unsigned)((issued / UNIT_NDESC - 1) & 1));
@@ -245,6 +262,16 @@ __global__ void __launch_bounds__(RF_THREADS, 2)
             }
             const int ui = u % g.nux, uj = u / g.nux;
             const int gx0 = g.x_off + ui * g.RW - g.Mx - g.tl, gy0 = g.y_off + uj * g.RH - g.My - g.tl;
+            // The kernel is bound by the latency of its box loads (two stages in flight per CTA are less than the
+            // bandwidth-delay product): the boxes of the unit UNIT_PREFETCH steps ahead are pulled into L2 now, so that its
+            // TMA copies find them there.
+            {
+                const int up = u + UNIT_PREFETCH * (int)gridDim.x;
+                if (UNIT_PREFETCH > 0 && lane < Cfg::NARR && up < n_units && __ldg(ub.nseg + up) > 0) {
+                    const int pi = up % g.nux, pj = up / g.nux;
+                    tma_prefetch_2d(&maps.m[lane], g.x_off + pi * g.RW - g.Mx - g.tl, g.y_off + pj * g.RH - g.My - g.tl);
+                }
+            }
             // tile records of the segments: lane l copies half (5 x 16 B) of segment l / 2's record
             {
                 const int t_l = __shfl_sync(0xffffffffu, sg.t, lane >> 1);
@@ -261,17 +288,7 @@ __global__ void __launch_bounds__(RF_THREADS, 2)
             long long off_l = 0, cs_l = -1;
             if (lane < nseg) {
                 off_l = tile_out_offset(pb, sg.t);
-                if (COADD) {
-                    const long long tile = pb.tile_id[sg.t];
-                    long long key = tile >> ca.shift, lo = 0, hi = ca.n_tiles - 1, pos = -1;
-                    while (lo <= hi) {
-                        const long long mid = (lo + hi) >> 1, tv = ca.tiles[mid];
-                        if (tv == key) { pos = mid; break; }
-                        if (tv < key) lo = mid + 1; else hi = mid - 1;
-                    }
-                    const long long ppt = 1ll << (ca.shift + 10);
-                    cs_l = pos < 0 ? -1 : pos * ppt + ((tile << 10) & (ppt - 1));
-                }
+                if (COADD) cs_l = pb.cslot[sg.t];               // coadd_slots_kernel, once per call
             }
             __syncwarp();
             int cls_l = 0, mslot_l = 0;
@@ -327,7 +344,8 @@ __global__ void __launch_bounds__(RF_THREADS, 2)
                 d.bmask[row][lane] = w;
                 d.bpref[row][lane] = ic - c;
             }
-            if (lane == 0) { d.n_seg = nseg; d.n_sb = min(total, UNIT_MAXSB); d.pad0 = (int)border; }
+            const unsigned absent = __ballot_sync(0xffffffffu, COADD && lane < nseg && cs_l < 0);
+            if (lane == 0) { d.n_seg = nseg; d.n_sb = min(total, UNIT_MAXSB); d.pad0 = (int)border; d.pad1 = (int)absent; }
             __syncwarp();
             // stage free: every consumer is done with the unit that used it STAGES units ago; then the bulk copies
             if (issued >= Cfg::STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / Cfg::STAGES - 1) & 1));
@@ -440,17 +458,53 @@ __global__ void __launch_bounds__(RF_THREADS, 2)
     const int yf = c0y + ayi * s + byi * t + __float_as_int(fmaf(T, fmaf(T, fmaf(T, py9, Cy), By), Ay));           \
     const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));
         // a unit without border tiles and without a masked pixel in its box (nearly all): no membership, no weights
-        if (!COADD && !any_bad && d.pad0 == 0) {
-            float* vq = value_out + q;
-            float* wq = weight_out + q;
-            for (int e = half; e < n_sb; e += RF_CONSUMERS / 16) {
+        if (!any_bad && d.pad0 == 0 && (!COADD || d.pad1 == 0)) {
+            // eight threads per sub-block, two vertically adjacent pixels each (same column: the S-dependent Horner
+            // coefficients are shared): in-block Morton indices q0 and q0 + 2
+            const int oct = gt >> 3, i8 = gt & 7;
+            const int q0 = (i8 & 1) | ((i8 >> 1) << 2);
+            const int sdu2 = 2 * (i8 & 3) - 31, sdv2 = 4 * (i8 >> 2) - 31;
+            float* vq = value_out + q0;
+            float* wq = weight_out + q0;
+            for (int e = oct; e < n_sb; e += RF_CONSUMERS / 8) {
                 const unsigned ent = d.sb[e];
                 const int sgi = (int)(ent >> 12);
-                if (sgi != cur) UNIT_LOAD_SEG(sgi)                  // uniform over the half-warp
-                UNIT_POSITION(ent)
+                if (sgi != cur) UNIT_LOAD_SEG(sgi)                  // uniform over the eight threads
+                // A6: the accumulator loads are issued before the position arithmetic, their latency hides under it
+                float* sp = nullptr;
+                float* wp = nullptr;
+                float s_a0 = 0.f, s_a1 = 0.f, w_a0 = 0.f, w_a1 = 0.f;
+                if (COADD) {
+                    sp = ca.sum + cslot + ((ent >> 2) & 0x3f0u) + q0;
+                    wp = ca.wsum + cslot + ((ent >> 2) & 0x3f0u) + q0;
+                    s_a0 = sp[0]; s_a1 = sp[2]; w_a0 = wp[0]; w_a1 = wp[2];
+                }
+                const int s = 8 * (int)((ent >> 3) & 7u) + sdu2, t = 8 * (int)(ent & 7u) + sdv2;
+                const float S = (float)s * 0.03125f, T0 = (float)t * 0.03125f, T1 = T0 + 0.0625f;
+                const float Ax = fmaf(S, fmaf(S, fmaf(S, px6, px3), px1), px0), Bx = fmaf(S, fmaf(S, px7, px4), px2), Cx = fmaf(S, px8, px5);
+                const float Ay = fmaf(S, fmaf(S, fmaf(S, py6, py3), py1), py0), By = fmaf(S, fmaf(S, py7, py4), py2), Cy = fmaf(S, py8, py5);
+                const int lx = c0x + axi * s + bxi * t, ly = c0y + ayi * s + byi * t;
+                const int xf0 = lx + __float_as_int(fmaf(T0, fmaf(T0, fmaf(T0, px9, Cx), Bx), Ax));
+                const int yf0 = ly + __float_as_int(fmaf(T0, fmaf(T0, fmaf(T0, py9, Cy), By), Ay));
+                const int xf1 = lx + 2 * bxi + __float_as_int(fmaf(T1, fmaf(T1, fmaf(T1, px9, Cx), Bx), Ax));
+                const int yf1 = ly + 2 * byi + __float_as_int(fmaf(T1, fmaf(T1, fmaf(T1, py9, Cy), By), Ay));
+                const float* a0 = cb + ((yf0 >> FAST_FRAC_BITS) * pitch + (xf0 >> FAST_FRAC_BITS));
+                const float* a1 = cb + ((yf1 >> FAST_FRAC_BITS) * pitch + (xf1 >> FAST_FRAC_BITS));
+                const float v0 = interp_clean<0>(a0, pitch, fast_frac(xf0), fast_frac(yf0));
+                const float v1 = interp_clean<0>(a1, pitch, fast_frac(xf1), fast_frac(yf1));
+                if (COADD) {        // footprint pixels are unique within a frame: plain read-modify-write, deterministic
+                    sp[0] = s_a0 + v0; sp[2] = s_a1 + v1;
+                    wp[0] = w_a0 + 1.0f; wp[2] = w_a1 + 1.0f;
+                    continue;
+                }
                 const long long o = off + (long long)((ent >> 2) & 0x3f0u);      // 16 * sub-block
-                const float val = interp_clean<0>(a, pitch, fast_frac(xf), fast_frac(yf));
-                if (o + q < out_cap) { vq[o] = val; wq[o] = 1.0f; }
+                if (o + 16 <= out_cap) {
+                    vq[o] = v0; vq[o + 2] = v1;
+                    wq[o] = 1.0f; wq[o + 2] = 1.0f;
+                } else {
+                    if (o + q0 < out_cap) { vq[o] = v0; wq[o] = 1.0f; }
+                    if (o + q0 + 2 < out_cap) { vq[o + 2] = v1; wq[o + 2] = 1.0f; }
+                }
             }
         } else {
             for (int e = half; e < n_sb; e += RF_CONSUMERS / 16) {
