@@ -75,6 +75,10 @@ enum {
                                * order (slot(p) of argus_coadd).  1: every tile is a row-major image of side
                                * nside / nside_tile: pixel (ix, iy) of the tile (ix = even bits, iy = odd bits of the
                                * in-tile nested index, the HEALPix face coordinates) goes to iy * side + ix. */
+    ARGUS_OPT_UNIT_MARGIN = 6, /* test hook, default 0: added to the unit kernel's estimated sub-block overhang (cells).  A negative
+                                  value makes plan_units_kernel find sub-blocks that leave their unit's box: they are served by the
+                                  stray kernel (per pixel, FP64), which normal geometries never exercise.  9 .. 40: self-test of the
+                                  ARGUS_DEBUG_BOUNDS build (its check treats the staged box as value - 8 cells narrower) */
     ARGUS_OPT_PROFILE = 2     /* 1: argus_resample / argus_resample_coadd (idx == NULL) record CUDA events on
                                  the caller's stream around the plan kernels and around the fused kernel
                                  (ring of 256 calls); read them back with argus_profile_read.  Default 0. */

@@ -20,19 +20,30 @@ def _stale() -> bool:
     return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile if sources are newer than the library.  Raises if nvcc is missing or fails."""
+DEBUG_LIB = os.path.join(HERE, "libargus_debug.so")
+
+
+def build(force: bool = False, verbose: bool = False, debug_bounds: bool = False) -> str:
+    """Compile if sources are newer than the library.  Raises if nvcc is missing or fails.
+    debug_bounds: the ARGUS_DEBUG_BOUNDS build (every shared-memory gather checked against its staged box) into
+    libargus_debug.so; the product library is not touched."""
+    if debug_bounds:
+        return _compile(DEBUG_LIB, ["-DARGUS_DEBUG_BOUNDS"], verbose)
     if not force and not _stale():
         return LIB
+    return _compile(LIB, [], verbose)
+
+
+def _compile(out: str, defines, verbose: bool) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     if not os.path.exists(nvcc):
         nvcc = "nvcc"
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    extra = os.environ.get("ARGUS_NVCC_EXTRA", "").split()   # e.g. -DARGUS_DEBUG_BOUNDS (tests), tuning macros
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+    tmp = out + ".tmp.%d" % os.getpid()
+    extra = os.environ.get("ARGUS_NVCC_EXTRA", "").split()   # tuning macros for experiments
+    cmd = [nvcc] + NVCC_FLAGS + list(defines) + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
     subprocess.run(cmd, check=True, cwd=CSRC)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, out)
+    return out
 
 
 if __name__ == "__main__":

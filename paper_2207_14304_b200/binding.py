@@ -17,6 +17,7 @@ ARGUS_OPT_PROFILE = 2
 ARGUS_OPT_FAST_PATH = 3
 ARGUS_OPT_PLAN_OVERLAP = 4
 ARGUS_OPT_SEGMENT_RASTER = 5
+ARGUS_OPT_UNIT_MARGIN = 6
 _KERNELS = {"bilinear": ARGUS_BILINEAR, "lanczos3": ARGUS_LANCZOS3, 0: 0, 1: 1}
 
 EXPORTS = [
@@ -63,7 +64,9 @@ _lib = None
 
 
 def library_path() -> str:
-    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libargus.so")
+    """libargus.so beside this file; ARGUS_LIBRARY names another build of the same sources (the ARGUS_DEBUG_BOUNDS build of
+    tests/test_gpu_debug_bounds.py)."""
+    return os.environ.get("ARGUS_LIBRARY") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libargus.so")
 
 
 def load_library():
@@ -76,11 +79,12 @@ def load_library():
     # of stale sources is an error: running an old library against new sources would hide it.  Without nvcc (a box that
     # only received the built .so) the existing library is used as it is.
     from . import _build
-    try:
-        _build.build()
-    except FileNotFoundError:
-        if not os.path.exists(path):
-            raise
+    if not os.environ.get("ARGUS_LIBRARY"):
+        try:
+            _build.build()
+        except FileNotFoundError:
+            if not os.path.exists(path):
+                raise
     if not os.path.exists(path):
         raise ImportError("libargus.so not built: run `python -m paper_2207_14304_b200._build` "
                           "(or __graft_entry__.build()); there is no CPU fallback")
@@ -227,6 +231,11 @@ class Context:
 
     def set_plan_overlap(self, on: bool):
         rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_PLAN_OVERLAP, 1 if on else 0)
+        if rc:
+            raise ArgusError(rc, "argus_ctx_set_option")
+
+    def set_unit_margin(self, delta: int):
+        rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_UNIT_MARGIN, int(delta))
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")
 

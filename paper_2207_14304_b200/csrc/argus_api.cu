@@ -54,6 +54,7 @@ struct argus_ctx {
     void* encode_fn;      // cuTensorMapEncodeTiled, resolved at first use (no link-time libcuda dependency)
     bool encode_tried;
     bool fast_enabled;    // ARGUS_OPT_FAST_PATH != 0
+    int unit_margin;      // ARGUS_OPT_UNIT_MARGIN
     bool unit_forced;     // ARGUS_OPT_FAST_PATH == 3: units wherever their geometry allows (diagnostic)
     bool unit_enabled;    // ARGUS_OPT_FAST_PATH == 1 or 3: image-aligned work units (resample_unit.cuh) where the geometry allows
     bool fast_attr_set;
@@ -381,6 +382,12 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
     }
     if (option == ARGUS_OPT_SEGMENT_RASTER) {
         c->seg_raster = value != 0;
+        return ARGUS_OK;
+    }
+    if (option == ARGUS_OPT_UNIT_MARGIN) {
+        if (value < -8 || value > 40) return ARGUS_ERR_SHAPE;     // 9 .. 40: self-test of the ARGUS_DEBUG_BOUNDS check (box pretended value - 8 narrower)
+        c->unit_margin = (int)value;
+        c->plan_valid = false;
         return ARGUS_OK;
     }
     if (option == ARGUS_OPT_FAST_PATH) {
@@ -911,7 +918,7 @@ static void unit_extent_at(const DevWcs& w, const argus_wcs* wc, int64_t nside, 
 // kernel or the general kernel then runs the frame.  The extents are ESTIMATES from nine sky directions (centre, corners,
 // edge midpoints); a sub-block that exceeds them anyway is found by plan_units_kernel and served by the stray kernel.
 static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, double s_rad, int kernel, UnitGeom* g,
-                          bool* tiles_fit) {
+                          bool* tiles_fit, int margin_delta) {
     if (kernel != ARGUS_BILINEAR) return false;
     double ex = 0.0, ey = 0.0;
     *tiles_fit = true;
@@ -937,7 +944,11 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
         }
     memset(g, 0, sizeof(*g));
     g->tl = 0; g->tr = 1;
-    g->Mx = (int)ceil(1.03 * ex + 0.02); g->My = (int)ceil(1.03 * ey + 0.02);
+    const int chk = margin_delta > 8 ? margin_delta - 8 : 0;
+    if (margin_delta > 8) margin_delta = 0;
+    g->Mx = (int)ceil(1.03 * ex + 0.02) + margin_delta; g->My = (int)ceil(1.03 * ey + 0.02) + margin_delta;
+    if (g->Mx < 0) g->Mx = 0;
+    if (g->My < 0) g->My = 0;
     g->BW = UNIT_BOXW;
     g->RW = (g->BW - 2 * g->Mx - g->tl - g->tr) & ~7;
     int bh = UNIT_CAP / g->BW;
@@ -958,6 +969,7 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
     g->nuy = (int)((H + g->My + 2 - g->y_off + g->RH - 1) / g->RH);
     if ((long long)g->nux * g->nuy > (1ll << 24)) return false;
     g->max_stray = 1 << 16;
+    g->chk_shrink = chk;
     return true;
 }
 
@@ -1010,7 +1022,7 @@ static int choose_path(argus_ctx* c, const FrameArgs& f, bool fused, int kernel,
         // stage somewhere on the frame (HEALPix tiles are wide near the equator and tall in the polar caps); where its
         // boxes fit, the tile kernel is the faster one (0.28 vs 0.33 ms at configs[1]: DESIGN.md 6.6)
         bool tiles_fit = true;
-        if (make_devwcs(wcs, W, H, nside, &dw, &rho, &s_rad) == ARGUS_OK && unit_geometry(dw, wcs, W, H, nside, s_rad, kernel, ug, &tiles_fit) &&
+        if (make_devwcs(wcs, W, H, nside, &dw, &rho, &s_rad) == ARGUS_OK && unit_geometry(dw, wcs, W, H, nside, s_rad, kernel, ug, &tiles_fit, c->unit_margin) &&
             (f.pre || !tiles_fit || c->unit_forced) && unit_maps(c, f, W, H, *ug))
             return 2;
     }

@@ -253,6 +253,16 @@ __device__ __forceinline__ void interp_masked(const float* __restrict__ a, int p
     if (!(w < w_min) && (S - B > 0.f)) { val = V1 / (S - B); wgt = fminf(w, 1.0f); }
 }
 
+// ARGUS_DEBUG_BOUNDS build (tests/test_gpu_debug_bounds.py; compute-sanitizer is not available on the GPU pool): every
+// shared-memory gather is checked against the staged box -- cell column / row of the position plus the kernel's taps must
+// lie inside [0, box width) x [0, rows) -- and a violation is latched (bit 8 of the overflow latch: argus_plan_info fails).
+#ifdef ARGUS_DEBUG_BOUNDS
+#define RF_CHECK_BOX(PB, COL, ROW, TL, TR, BOXW, ROWS)                                                                  \
+    if ((COL) - (TL) < 0 || (COL) + (TR) >= (BOXW) || (ROW) - (TL) < 0 || (ROW) + (TR) >= (ROWS)) plan_overflow(PB, 8);
+#else
+#define RF_CHECK_BOX(PB, COL, ROW, TL, TR, BOXW, ROWS)
+#endif
+
 // ------------------------------------------------------------------------------------------ kernel
 // Bilinear, 80 registers: two CTAs leave 19 K registers per SM free, enough for one CTA of any plan kernel -- the plan
 // of the next frame runs on a side stream underneath this kernel (argus_api.cu, ARGUS_OPT_PLAN_OVERLAP).
@@ -473,6 +483,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
 #define RF_HOT(Q)                                                                            \
     {                                                                                        \
         const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);    \
+        RF_CHECK_BOX(pb, d.r.X0 - d.r.gx0 + (xf >> FAST_FRAC_BITS), d.r.Y0 - d.r.gy0 + (yf >> FAST_FRAC_BITS), Cfg::TL, Cfg::TR, boxw, d.r.bh) \
         const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));     \
         vp[RF_CONSUMERS * Q] = interp_clean<KERNEL>(a, pitch, fast_frac(xf), fast_frac(yf)); \
         wp[RF_CONSUMERS * Q] = 1.0f;                                                         \
@@ -494,6 +505,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
 #define RF_ACC(Q)                                                                            \
     {                                                                                        \
         const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);    \
+        RF_CHECK_BOX(pb, d.r.X0 - d.r.gx0 + (xf >> FAST_FRAC_BITS), d.r.Y0 - d.r.gy0 + (yf >> FAST_FRAC_BITS), Cfg::TL, Cfg::TR, boxw, d.r.bh) \
         const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));     \
         sp[RF_CONSUMERS * Q] = s_acc[Q] + interp_clean<KERNEL>(a, pitch, fast_frac(xf), fast_frac(yf)); \
         wp[RF_CONSUMERS * Q] = w_acc[Q] + 1.0f;                                              \
@@ -518,6 +530,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
         }                                                                                                  \
         if (member) {                                                                                      \
             const int xf = fast_axis_eval<Q>(ax, T0, T1), yf = fast_axis_eval<Q>(ay, T0, T1);              \
+            RF_CHECK_BOX(pb, d.r.X0 - d.r.gx0 + (xf >> FAST_FRAC_BITS), d.r.Y0 - d.r.gy0 + (yf >> FAST_FRAC_BITS), Cfg::TL, Cfg::TR, boxw, d.r.bh) \
             const float* a = cb + ((yf >> FAST_FRAC_BITS) * pitch + (xf >> FAST_FRAC_BITS));               \
             float val, wgt;                                                                                \
             interp_masked<KERNEL>(a, pitch, fast_frac(xf), fast_frac(yf), w_min, val, wgt);                \

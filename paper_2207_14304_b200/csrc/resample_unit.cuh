@@ -41,6 +41,7 @@ struct UnitGeom {
     int BW, BH;                        // staged box: cells [x0 - Mx - tl, ...) , BW x BH (BW % 8 == 0, origin % 8 == 0)
     int tl, tr;
     int max_stray;
+    int chk_shrink;                    // ARGUS_DEBUG_BOUNDS self-test: the check pretends the box is this much narrower
 };
 
 struct __align__(16) UnitSeg {         // one (unit, tile) pair
@@ -179,6 +180,7 @@ struct __align__(16) UnitSegD {
 #define UNIT_NDESC 4                   // descriptors are prepared up to three units ahead of the stage they describe
 #define UNIT_MAXBORDER 6               // border-tile tables per unit (more: membership straight from global memory)
 struct __align__(16) UnitDesc {
+    int gx0, gy0, pad2, pad3;             // origin of the staged box (debug bounds check)
     int n_seg, n_sb, pad0, pad1;          // n_seg < 0: end of work; pad0 / pad1 = bit sets of the border segments / of segments absent from the coadd layout
     UnitSegD seg[UNIT_MAXSEG];
     unsigned sb[UNIT_MAXSB];              // work list, grouped by segment: segment << 12 | sub-block << 6 | a << 3 | b
@@ -345,7 +347,7 @@ __global__ void __launch_bounds__(UNIT_THREADS, 2)
                 d.bpref[row][lane] = ic - c;
             }
             const unsigned absent = __ballot_sync(0xffffffffu, COADD && lane < nseg && cs_l < 0);
-            if (lane == 0) { d.n_seg = nseg; d.n_sb = min(total, UNIT_MAXSB); d.pad0 = (int)border; d.pad1 = (int)absent; }
+            if (lane == 0) { d.n_seg = nseg; d.n_sb = min(total, UNIT_MAXSB); d.pad0 = (int)border; d.pad1 = (int)absent; d.gx0 = gx0; d.gy0 = gy0; }
             __syncwarp();
             // stage free: every consumer is done with the unit that used it STAGES units ago; then the bulk copies
             if (issued >= Cfg::STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / Cfg::STAGES - 1) & 1));
@@ -437,6 +439,8 @@ __global__ void __launch_bounds__(UNIT_THREADS, 2)
         int c0x = 0, axi = 0, bxi = 0, c0y = 0, ayi = 0, byi = 0, mb = -1;
         const float* cb = cal;
         long long off = 0, cslot = -1;
+        int dbg_x = 0, dbg_y = 0;
+        (void)dbg_x; (void)dbg_y;
         const int sdu = 2 * du - 31, sdv = 2 * dv - 31;
 #define UNIT_LOAD_SEG(SGI)                                                                                        \
     {                                                                                                             \
@@ -447,6 +451,7 @@ __global__ void __launch_bounds__(UNIT_THREADS, 2)
         py5 = sd.r.py[5]; py6 = sd.r.py[6]; py7 = sd.r.py[7]; py8 = sd.r.py[8]; py9 = sd.r.py[9];                 \
         c0x = sd.r.c0x; axi = sd.r.ax; bxi = sd.r.bx; c0y = sd.r.c0y; ayi = sd.r.ay; byi = sd.r.by;               \
         cb = cal + sd.kofs; mb = sd.mb; off = sd.off; cslot = sd.cslot;                                           \
+        dbg_x = sd.r.X0 - d.gx0; dbg_y = sd.r.Y0 - d.gy0;                                                         \
         cur = SGI;                                                                                                \
     }
 #define UNIT_POSITION(ENT)                                                                                        \
@@ -488,6 +493,8 @@ __global__ void __launch_bounds__(UNIT_THREADS, 2)
                 const int yf0 = ly + __float_as_int(fmaf(T0, fmaf(T0, fmaf(T0, py9, Cy), By), Ay));
                 const int xf1 = lx + 2 * bxi + __float_as_int(fmaf(T1, fmaf(T1, fmaf(T1, px9, Cx), Bx), Ax));
                 const int yf1 = ly + 2 * byi + __float_as_int(fmaf(T1, fmaf(T1, fmaf(T1, py9, Cy), By), Ay));
+                RF_CHECK_BOX(pb, dbg_x + (xf0 >> FAST_FRAC_BITS), dbg_y + (yf0 >> FAST_FRAC_BITS), g.tl, g.tr, g.BW - g.chk_shrink, g.BH)
+                RF_CHECK_BOX(pb, dbg_x + (xf1 >> FAST_FRAC_BITS), dbg_y + (yf1 >> FAST_FRAC_BITS), g.tl, g.tr, g.BW - g.chk_shrink, g.BH)
                 const float* a0 = cb + ((yf0 >> FAST_FRAC_BITS) * pitch + (xf0 >> FAST_FRAC_BITS));
                 const float* a1 = cb + ((yf1 >> FAST_FRAC_BITS) * pitch + (xf1 >> FAST_FRAC_BITS));
                 const float v0 = interp_clean<0>(a0, pitch, fast_frac(xf0), fast_frac(yf0));
@@ -529,6 +536,7 @@ __global__ void __launch_bounds__(UNIT_THREADS, 2)
                     for (int k = 0; k < (sb >> 1); ++k) pos += __popc(mkp[k]);
                 }
                 if (!member) continue;
+                RF_CHECK_BOX(pb, dbg_x + (xf >> FAST_FRAC_BITS), dbg_y + (yf >> FAST_FRAC_BITS), g.tl, g.tr, g.BW - g.chk_shrink, g.BH)
                 const float fx = fast_frac(xf), fy = fast_frac(yf);
                 float val, wgt;
                 if (!any_bad) { val = interp_clean<0>(a, pitch, fx, fy); wgt = 1.0f; }
