@@ -431,33 +431,66 @@ def run_gpu(args):
         h_val = torch.empty(max(n_fps), dtype=torch.float32).pin_memory()
         h_wgt = torch.empty(max(n_fps), dtype=torch.float32).pin_memory()
 
+    def masters_of(fr, d):
+        return (dict(offset=d["offset"], gain=d["gain"], sat_adu=fr.sat_adu) if args.prefused else
+                dict(bias=d["bias"], dark=d["dark"], flat=d["flat"], t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min))
+
+    def e2e_vw_step():        # value + weight back to the host (8 B per footprint pixel)
+        for (fr, wcs), (_, d), n in zip(jobs_host, jobs, n_fps):
+            argus.argus_resample_host(ctx, wcs, W, H, nside, kernel, n, h_raws[id(fr)], h_val, h_wgt, **masters_of(fr, d))
+
+    # the paper's per-frame PRODUCT back to the host: binary16 segment data + low-resolution map
+    products = not coadd and nside >= (1 << 14)
+    if products:
+        mini_cap = int(max(n_fps) // 64 * 1.3) + 4096
+        h_seg = torch.empty(max(n_fps), dtype=torch.int16).pin_memory()
+        h_mid = torch.empty(mini_cap, dtype=torch.int64).pin_memory()
+        h_mv, h_mw = torch.empty(mini_cap, dtype=torch.float32).pin_memory(), torch.empty(mini_cap, dtype=torch.float32).pin_memory()
+        h_nm = torch.zeros(1, dtype=torch.int64).pin_memory()
+
     def e2e_step():
         for (fr, wcs), (_, d), n in zip(jobs_host, jobs, n_fps):
-            m = (dict(offset=d["offset"], gain=d["gain"], sat_adu=fr.sat_adu) if args.prefused else
-                 dict(bias=d["bias"], dark=d["dark"], flat=d["flat"], t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min))
             if coadd:
-                argus.argus_resample_coadd_host(ctx, wcs, W, H, nside, kernel, h_raws[id(fr)], tiles, 256, csum, cwsum, None, **m)
+                argus.argus_resample_coadd_host(ctx, wcs, W, H, nside, kernel, h_raws[id(fr)], tiles, 256, csum, cwsum, None, **masters_of(fr, d))
+            elif products:
+                argus.argus_reduce_frame_host(ctx, wcs, W, H, nside, kernel, n, h_raws[id(fr)], h_seg, h_mid, h_mv, h_mw, h_nm,
+                                              nside_mini=1 << 14, **masters_of(fr, d))
             else:
-                argus.argus_resample_host(ctx, wcs, W, H, nside, kernel, n, h_raws[id(fr)], h_val, h_wgt, **m)
+                argus.argus_resample_host(ctx, wcs, W, H, nside, kernel, n, h_raws[id(fr)], h_val, h_wgt, **masters_of(fr, d))
         if coadd:   # the step's result: the coadd itself
             h_sum.copy_(csum, non_blocking=True)
             h_wsum.copy_(cwsum, non_blocking=True)
 
-    for _ in range(2 if n_frames == 1 else 1):
-        e2e_step()
-    argus.argus_host_wait(ctx)
-    barrier()
-    e2e_steps = max(4, min(args.steps, 10)) if n_frames == 1 else 2
-    t_e0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e2e_step()
-    argus.argus_host_wait(ctx)
-    torch.cuda.synchronize()
-    e2e_ms = 1e3 * (time.perf_counter() - t_e0)   # host wall clock around enqueue + completion (copies run on the library's streams)
-    barrier()
-    e2e_ms, _, _ = reduce_over_ranks(e2e_ms, 0, 0, dist if world > 1 else None, dev)
+    def time_e2e(fn):
+        for _ in range(2 if n_frames == 1 else 1):
+            fn()
+        argus.argus_host_wait(ctx)
+        barrier()
+        steps = max(4, min(args.steps, 10)) if n_frames == 1 else 2
+        t_e0 = time.perf_counter()
+        for _ in range(steps):
+            fn()
+        argus.argus_host_wait(ctx)
+        torch.cuda.synchronize()
+        wall = 1e3 * (time.perf_counter() - t_e0)   # host wall clock around enqueue + completion (copies run on the library's streams)
+        barrier()
+        wall, _, _ = reduce_over_ranks(wall, 0, 0, dist if world > 1 else None, dev)
+        return wall, steps
+
+    e2e_ms, e2e_steps = time_e2e(e2e_step)
     h2d = int(W * H * 2 * n_frames)
-    d2h = int(2 * 4 * csum.numel()) if coadd else int(8 * n_out_step)
+    if coadd:
+        d2h = int(2 * 4 * csum.numel())
+    elif products:
+        n_mini = int(h_nm.item())
+        d2h = int(2 * n_out_step + n_frames * (16 * mini_cap + 8))
+    else:
+        d2h = int(8 * n_out_step)
+    e2e_vw = None
+    if products and n_frames == 1:
+        vw_ms, vw_steps = time_e2e(e2e_vw_step)
+        e2e_vw = {"value": px_in_all * vw_steps / (vw_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_step": vw_ms / vw_steps,
+                  "d2h_bytes_per_step": int(8 * n_out_step), "note": "argus_resample_host: float32 value + weight back to the host instead of the products"}
 
     if rank == 0:
         peak, peak_src = _peaks()
@@ -515,8 +548,11 @@ def run_gpu(args):
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / e2e_steps,
                     "note": ("argus_resample_coadd_host per frame (raw from pinned host memory), the coadd (sum, wsum) back to pinned host memory once per step"
                              if coadd else
-                             "argus_resample_host: raw frame from pinned host memory each frame, value + weight back to pinned host memory; masters resident per pointing")
+                             ("argus_reduce_frame_host: raw frame from pinned host memory each frame; the paper's per-frame product back to pinned host memory: binary16 segment data (2 B per footprint pixel, PAPER.md:145) + low-resolution map on the NSIDE-16384 minipix grid (PAPER.md:149); masters resident per pointing"
+                              if products else
+                              "argus_resample_host: raw frame from pinned host memory each frame, value + weight back to pinned host memory; masters resident per pointing"))
                             + "; upload / kernels / download of consecutive frames pipelined by the library; host wall clock"},
+            "e2e_value_weight": e2e_vw,
             "gpu_launches": launches,
             "clocks": clocks,
         }

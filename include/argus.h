@@ -229,7 +229,18 @@ int argus_resample_host(argus_ctx* ctx, const argus_frame* frame, const argus_wc
 int argus_resample_coadd_host(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
                               int64_t nside, int kernel, float w_min, const argus_coadd* layout, float* sum, float* wsum,
                               int64_t* n_skipped_dev, void* stream);
-/* Blocks until every upload and download enqueued by argus_resample_host / argus_resample_coadd_host has completed. */
+/* The paper's per-frame PRODUCT with HOST buffers: the resampled frame as IEEE binary16 segment data and the
+ * low-resolution map on the minipix grid (argus_segment_products without stamping).  frame->raw: HOST
+ * (pinned); masters: DEVICE.  n = footprint size (argus_healpix_footprint); seg16_host[n]: element i <-> i-th footprint pixel
+ * ascending; mini_*_host[mini_capacity], *n_mini_host: as argus_segment_products (all HOST, pinned for asynchronous copies;
+ * entries beyond n_mini are unspecified).  2 bytes per footprint pixel + 16 per minipix leave the device instead of the 8
+ * per pixel of argus_resample_host.  Pipelined like argus_resample_host; complete after argus_host_wait. */
+int argus_reduce_frame_host(argus_ctx* ctx, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H, int64_t nside,
+                            int kernel, float w_min, int64_t nside_mini, size_t n, size_t mini_capacity, uint16_t* seg16_host,
+                            int64_t* mini_id_host, float* mini_value_host, float* mini_weight_host, int64_t* n_mini_host,
+                            void* stream);
+/* Blocks until every upload and download enqueued by argus_resample_host / argus_resample_coadd_host / argus_reduce_frame_host
+ * has completed. */
 int argus_host_wait(argus_ctx* ctx);
 
 /* A6: sum[slot(idx[i])] += weight[i] * value[i]; wsum[slot] += weight[i] for i < n.  idx must hold

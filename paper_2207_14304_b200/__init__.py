@@ -22,6 +22,7 @@ from .binding import (  # noqa: F401
     argus_resample_coadd,
     argus_resample_host,
     argus_resample_coadd_host,
+    argus_reduce_frame_host,
     argus_host_wait,
     argus_segment_products,
     argus_subtract_tiles,

@@ -24,7 +24,7 @@ EXPORTS = [
     "argus_strerror", "argus_version", "argus_ctx_create", "argus_ctx_destroy", "argus_ctx_set_option",
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_prepare_masters", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
-    "argus_resample_host", "argus_resample_coadd_host", "argus_host_wait", "argus_subtract_tiles", "argus_segment_products", "argus_background_map", "argus_detect_sources",
+    "argus_resample_host", "argus_resample_coadd_host", "argus_reduce_frame_host", "argus_host_wait", "argus_subtract_tiles", "argus_segment_products", "argus_background_map", "argus_detect_sources",
 ]
 
 
@@ -109,6 +109,8 @@ def load_library():
     L.argus_resample_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, sz, vp, vp, vp]
     L.argus_resample_coadd_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32,
                                             C.POINTER(_Coadd), vp, vp, vp, vp]
+    L.argus_reduce_frame_host.argtypes = [vp, C.POINTER(_Frame), C.POINTER(_Wcs), i64, i64, i64, C.c_int, f32, i64, sz, sz, vp, vp, vp,
+                                          vp, vp, vp]
     L.argus_host_wait.argtypes = [vp]
     L.argus_segment_products.argtypes = [vp, i64, i64, vp, vp, vp, sz, vp, sz, C.POINTER(_Coadd), vp, vp, vp, vp, vp, sz,
                                          vp, C.POINTER(sz), vp]
@@ -378,6 +380,28 @@ def argus_resample_host(ctx, wcs, W, H, nside, kernel, n, raw_host, value_host, 
     rc = load_library().argus_resample_host(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min), int(n),
                                             value_host.data_ptr(), weight_host.data_ptr(), _stream(stream))
     _check(ctx, rc, "argus_resample_host")
+
+
+def argus_reduce_frame_host(ctx, wcs, W, H, nside, kernel, n, raw_host, seg16_host, mini_id_host, mini_value_host,
+                            mini_weight_host, n_mini_host, nside_mini=1 << 14, w_min=0.5, stream=None, bias=None, dark=None,
+                            flat=None, t_exp=0.0, sat_adu=65535, flat_min=0.1, offset=None, gain=None):
+    """The per-frame product with HOST buffers (pinned CPU tensors): binary16 segment data (int16 / uint16 / float16 tensor
+    of n elements) + low-resolution map (mini_* of one capacity, n_mini_host int64[1]).  Masters are CUDA tensors."""
+    cap = mini_id_host.numel()
+    for t, dts, name in ((raw_host, (torch.uint16,), "raw_host"), (seg16_host, (torch.int16, torch.uint16, torch.float16), "seg16_host"),
+                         (mini_id_host, (torch.int64,), "mini_id_host"), (mini_value_host, (torch.float32,), "mini_value_host"),
+                         (mini_weight_host, (torch.float32,), "mini_weight_host"), (n_mini_host, (torch.int64,), "n_mini_host")):
+        if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype not in dts or not t.is_contiguous():
+            raise TypeError("%s must be a contiguous CPU tensor of dtype %s" % (name, dts))
+    if raw_host.numel() != W * H or seg16_host.numel() < n or mini_value_host.numel() < cap or mini_weight_host.numel() < cap:
+        raise ValueError("host buffers too small")
+    f = _host_frame_struct(raw_host, bias, dark, flat, offset, gain, t_exp, sat_adu, flat_min)
+    w = _wcs_struct(wcs)
+    rc = load_library().argus_reduce_frame_host(ctx._h, C.byref(f), C.byref(w), W, H, nside, _KERNELS[kernel], float(w_min),
+                                                int(nside_mini), int(n), int(cap), seg16_host.data_ptr(), mini_id_host.data_ptr(),
+                                                mini_value_host.data_ptr(), mini_weight_host.data_ptr(), n_mini_host.data_ptr(),
+                                                _stream(stream))
+    _check(ctx, rc, "argus_reduce_frame_host")
 
 
 def argus_host_wait(ctx):

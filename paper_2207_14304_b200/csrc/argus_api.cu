@@ -80,6 +80,9 @@ struct argus_ctx {
     struct HostBuf {
         uint16_t* raw; float* val; float* wgt;
         size_t cap_px, cap_n;
+        // argus_reduce_frame_host: footprint list, binary16 segment data, low-resolution map
+        long long* idx; uint16_t* seg16; size_t cap_prod;
+        long long* mini_id; float* mini_val; float* mini_wgt; long long* n_mini; size_t cap_mini;
         cudaEvent_t up, run, down;
         bool used, down_used, ev_ok;
     } hb[2];
@@ -340,6 +343,12 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
         if (c->hb[i].raw) cudaFree(c->hb[i].raw);
         if (c->hb[i].val) cudaFree(c->hb[i].val);
         if (c->hb[i].wgt) cudaFree(c->hb[i].wgt);
+        if (c->hb[i].idx) cudaFree(c->hb[i].idx);
+        if (c->hb[i].seg16) cudaFree(c->hb[i].seg16);
+        if (c->hb[i].mini_id) cudaFree(c->hb[i].mini_id);
+        if (c->hb[i].mini_val) cudaFree(c->hb[i].mini_val);
+        if (c->hb[i].mini_wgt) cudaFree(c->hb[i].mini_wgt);
+        if (c->hb[i].n_mini) cudaFree(c->hb[i].n_mini);
         if (c->hb[i].ev_ok) { cudaEventDestroy(c->hb[i].up); cudaEventDestroy(c->hb[i].run); cudaEventDestroy(c->hb[i].down); }
     }
     if (c->seg.mini_start) cudaFree(c->seg.mini_start);
@@ -1214,6 +1223,69 @@ extern "C" int argus_resample_coadd_host(argus_ctx* c, const argus_frame* frame,
     if (rc) return rc;
     CUDA_TRY(c, cudaEventRecord(b->run, st));
     b->used = true;
+    return ARGUS_OK;
+}
+
+// The paper's per-frame product through one call with HOST buffers (PAPER.md:145 16-bit float segment data, :149 / :73 the
+// low-resolution map): upload, plan, fused calibrate + resample, footprint list, segment products, download -- 2 bytes
+// per footprint pixel leave the device instead of the 8 of value + weight.
+extern "C" int argus_reduce_frame_host(argus_ctx* c, const argus_frame* frame, const argus_wcs* wcs, int64_t W, int64_t H,
+                                       int64_t nside, int kernel, float w_min, int64_t nside_mini, size_t n, size_t mini_capacity,
+                                       uint16_t* seg16_host, int64_t* mini_id_host, float* mini_value_host, float* mini_weight_host,
+                                       int64_t* n_mini_host, void* stream) {
+    if (!c || !frame || !wcs || !frame->raw || !seg16_host || !mini_id_host || !mini_value_host || !mini_weight_host || !n_mini_host)
+        return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n == 0 || n > ((size_t)1 << 34) || mini_capacity == 0 ||
+        mini_capacity > ((size_t)1 << 34))
+        return ARGUS_ERR_SHAPE;
+    if (!is_pow2(nside_mini) || nside_mini > nside) return ARGUS_ERR_NSIDE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    argus_ctx::HostBuf* b;
+    int rc = host_stage_upload(c, frame, W, H, n, st, &b);
+    if (rc) return rc;
+    if (b->cap_prod < n || b->cap_mini < mini_capacity) {
+        CUDA_TRY(c, cudaDeviceSynchronize());
+        if (b->cap_prod < n) {
+            if (b->idx) cudaFree(b->idx);
+            if (b->seg16) cudaFree(b->seg16);
+            b->idx = nullptr; b->seg16 = nullptr; b->cap_prod = 0;
+            CUDA_TRY(c, cudaMalloc((void**)&b->idx, n * sizeof(long long)));
+            CUDA_TRY(c, cudaMalloc((void**)&b->seg16, n * sizeof(uint16_t)));
+            b->cap_prod = n;
+        }
+        if (b->cap_mini < mini_capacity) {
+            if (b->mini_id) cudaFree(b->mini_id);
+            if (b->mini_val) cudaFree(b->mini_val);
+            if (b->mini_wgt) cudaFree(b->mini_wgt);
+            b->mini_id = nullptr; b->mini_val = b->mini_wgt = nullptr; b->cap_mini = 0;
+            CUDA_TRY(c, cudaMalloc((void**)&b->mini_id, mini_capacity * sizeof(long long)));
+            CUDA_TRY(c, cudaMalloc((void**)&b->mini_val, mini_capacity * sizeof(float)));
+            CUDA_TRY(c, cudaMalloc((void**)&b->mini_wgt, mini_capacity * sizeof(float)));
+            b->cap_mini = mini_capacity;
+        }
+        if (!b->n_mini) CUDA_TRY(c, cudaMalloc((void**)&b->n_mini, sizeof(long long)));
+    }
+    argus_frame fr = *frame;
+    fr.raw = b->raw;
+    rc = argus_resample(c, &fr, wcs, W, H, nside, kernel, w_min, nullptr, n, b->val, b->wgt, stream);
+    if (rc) return rc;
+    plan_write_indices_kernel<<<c->sm_count * 8, 256, 0, st>>>(c->pb, b->idx, (long long)n);
+    c->n_launches++;
+    mark_slot_read(c, st);
+    rc = argus_segment_products(c, nside, nside_mini, (const int64_t*)b->idx, b->val, b->wgt, n, nullptr, 0, nullptr, b->seg16,
+                                (int64_t*)b->mini_id, b->mini_val, b->mini_wgt, nullptr, mini_capacity, (int64_t*)b->n_mini, nullptr, stream);
+    if (rc) return rc;
+    CUDA_TRY(c, cudaEventRecord(b->run, st));
+    b->used = true;
+    CUDA_TRY(c, cudaStreamWaitEvent(c->s_down, b->run, 0));
+    CUDA_TRY(c, cudaMemcpyAsync(seg16_host, b->seg16, n * sizeof(uint16_t), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaMemcpyAsync(mini_id_host, b->mini_id, mini_capacity * sizeof(long long), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaMemcpyAsync(mini_value_host, b->mini_val, mini_capacity * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaMemcpyAsync(mini_weight_host, b->mini_wgt, mini_capacity * sizeof(float), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaMemcpyAsync(n_mini_host, b->n_mini, sizeof(long long), cudaMemcpyDeviceToHost, c->s_down));
+    CUDA_TRY(c, cudaEventRecord(b->down, c->s_down));
+    b->down_used = true;
     return ARGUS_OK;
 }
 

@@ -226,3 +226,38 @@ def test_on_a_real_footprint(argus, ctx):
     g = _run(argus, ctx, fr.nside, 1 << 14, idx_h, v_h, w_h, targets)
     _compare(g, o)
     assert 0 < o["mini_keep"].sum() < o["mini_keep"].size
+
+
+def test_reduce_frame_host_equals_the_device_path(argus, ctx):
+    """argus_reduce_frame_host (raw frame and products in HOST memory, pipelined) == argus_resample ->
+    argus_healpix_footprint list -> argus_segment_products on device buffers, bit for bit, over several frames."""
+    from gpu_util import upload
+    fr = synth.config0()
+    d = upload(fr)
+    n, idx = argus.argus_healpix_footprint(ctx, fr.wcs, 512, 512, fr.nside)
+    v = torch.empty(n, dtype=torch.float32, device="cuda")
+    w = torch.empty_like(v)
+    argus.argus_resample(ctx, fr.wcs, 512, 512, fr.nside, "bilinear", v, w, **d)
+    none = torch.zeros(0, dtype=torch.int64, device="cuda")
+    nm = argus.argus_segment_products(ctx, fr.nside, 1 << 14, idx, v, w, none)
+    cap = nm + 7
+    ref = dict(seg16=torch.empty(n, dtype=torch.int16, device="cuda"), mini_id=torch.empty(cap, dtype=torch.int64, device="cuda"),
+               mini_value=torch.empty(cap, dtype=torch.float32, device="cuda"), mini_weight=torch.empty(cap, dtype=torch.float32, device="cuda"))
+    assert argus.argus_segment_products(ctx, fr.nside, 1 << 14, idx, v, w, None, **ref) == nm
+    torch.cuda.synchronize()
+    h_raw = torch.from_numpy(fr.raw).pin_memory()
+    outs = []
+    for _ in range(4):
+        o = dict(seg16_host=torch.zeros(n, dtype=torch.int16).pin_memory(), mini_id_host=torch.zeros(cap, dtype=torch.int64).pin_memory(),
+                 mini_value_host=torch.zeros(cap, dtype=torch.float32).pin_memory(), mini_weight_host=torch.zeros(cap, dtype=torch.float32).pin_memory(),
+                 n_mini_host=torch.zeros(1, dtype=torch.int64).pin_memory())
+        argus.argus_reduce_frame_host(ctx, fr.wcs, 512, 512, fr.nside, "bilinear", n, h_raw, bias=d["bias"], dark=d["dark"], flat=d["flat"],
+                                      t_exp=fr.t_exp, sat_adu=fr.sat_adu, flat_min=fr.flat_min, **o)
+        outs.append(o)
+    argus.argus_host_wait(ctx)
+    for o in outs:
+        assert int(o["n_mini_host"].item()) == nm
+        assert torch.equal(o["seg16_host"], ref["seg16"].cpu())
+        assert torch.equal(o["mini_id_host"][:nm], ref["mini_id"].cpu()[:nm])
+        assert torch.equal(o["mini_value_host"][:nm], ref["mini_value"].cpu()[:nm])
+        assert torch.equal(o["mini_weight_host"][:nm], ref["mini_weight"].cpu()[:nm])
