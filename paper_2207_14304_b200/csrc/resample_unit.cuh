@@ -209,8 +209,14 @@ __device__ __forceinline__ float calib_unit_pre(unsigned magic_r, float off, flo
 }
 
 // ------------------------------------------------------------------------------------------- the kernel
+// 80 registers (no spills): two CTAs use 51 K of the SM's 64 K registers, the plan kernels of the next frame fit beside them
+// (ARGUS_OPT_PLAN_OVERLAP)
+#ifndef UNIT_MAXREG
+#define UNIT_MAXREG 80
+#endif
+#define UNIT_BOUNDS __maxnreg__(UNIT_MAXREG)
 template <bool COADD, int MASTERS>
-__global__ void __launch_bounds__(UNIT_THREADS, 2)
+__global__ void UNIT_BOUNDS
     resample_unit_kernel(const __grid_constant__ UnitMaps maps, PlanBuffers pb, UnitBuffers ub, UnitGeom g, FrameArgs f, float w_min,
                          float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap, CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
