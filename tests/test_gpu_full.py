@@ -62,6 +62,16 @@ def test_config1_full_frame(argus, ctx):
     assert info["n_inside"] > 0.9 * (info["n_tiles"] - info["n_empty"])
 
 
+def test_config1_full_frame_unit_kernel(argus, ctx):
+    """configs[1] through the image-aligned unit kernel (bench.py --unit-kernel), every output against the oracle."""
+    ctx.set_fast_path(3)
+    try:
+        info = _full_frame_parity(argus, ctx, synth.config1(), "config1, unit kernel")
+    finally:
+        ctx.set_fast_path(1)
+    assert info["n_units"] > 20000 and info["n_stray"] == 0
+
+
 @pytest.mark.parametrize("k", [0, 25, 37])
 def test_config2_frames(argus, ctx, k):
     info = _full_frame_parity(argus, ctx, synth.config2_frame(k), "config2[%d]" % k)

@@ -454,3 +454,38 @@ def test_capacity_and_errors(argus, ctx, cfg0):
     n, idx = argus.argus_healpix_footprint(ctx, synth.make_wcs((10, 10), (0, 0), 0.0), 1, 1, 1 << 17)
     n_or = len(oracle.footprint(synth.make_wcs((10, 10), (0, 0), 0.0), 1, 1, 1 << 17)[0])
     assert n == n_or
+
+
+@pytest.mark.parametrize("defects", [False, True])
+def test_unit_kernel_forced(argus, cfg0, cfg0_fp, defects):
+    """The image-aligned unit kernel (resample_unit.cuh) on config 0, where the default choice is the tile kernel:
+    ARGUS_OPT_FAST_PATH = 3.  Value + weight form and the fused coadd form, clean and with defects (saturated block, low /
+    NaN flat: the masked loop; a bad-pixel mask sends the frame to the general kernel, so the bpm is dropped here)."""
+    from gpu_util import assert_coadd_matches, assert_values_match, coadd_oracle, gpu_resample_planned, oracle_reference, upload
+    c = argus.Context(0)
+    try:
+        c.set_fast_path(3)
+        fr = cfg0
+        if defects:
+            fr = synth.inject_defects(cfg0)
+            fr.bpm = None
+        idx_or = cfg0_fp[0]
+        d = upload(fr)
+        n, v, w = gpu_resample_planned(c, fr, d, "bilinear")
+        info = argus.argus_plan_info(c)
+        assert info["n_units"] > 0 and info["n_stray"] == 0
+        vo, wo, fl = oracle_reference(fr, idx_or, "bilinear")
+        assert_values_match(v, w, vo, wo, fl, "unit kernel, config 0, defects=%s" % defects, min_amb_count=8)
+        tiles = np.unique(idx_or >> 18)[1:]            # one tile absent from the layout
+        ppt = 1 << 18
+        ref = coadd_oracle([fr, fr], [idx_or, idx_or], tiles, ppt, fr.nside, "bilinear")
+        s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
+        ws = torch.zeros_like(s)
+        sk = torch.zeros(1, dtype=torch.int64, device="cuda")
+        for _ in range(2):
+            argus.argus_resample_coadd(c, fr.wcs, 512, 512, fr.nside, "bilinear", torch.from_numpy(tiles).cuda(), 256, s, ws, sk, **d)
+        torch.cuda.synchronize()
+        assert int(sk.item()) == ref["skipped"] > 0
+        assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "unit kernel coadd, defects=%s" % defects)
+    finally:
+        c.close()
