@@ -1634,19 +1634,30 @@ extern "C" int argus_subtract_tiles(argus_ctx* c, const argus_coadd* layout, int
     int split = (int)(ppt / 8192);
     if (split < 1) split = 1;
     if (split > SUB_SPLIT_MAX) split = SUB_SPLIT_MAX;
-    if (have_stats) {
-        if (n_tiles * split > 0x7fffffffll) return ARGUS_ERR_SHAPE;
-        sub_stats_kernel<<<(unsigned)(n_tiles * split), 256, 0, st>>>(sci_sum, sci_wsum, ref_sum, ref_wsum, ppt, split, p, c->sub.partial);
-        c->n_launches++;
+    // The affine match needs every valid pixel of a tile before the first difference can be formed: two passes over the inputs.
+    // (Tried: tiles in chunks of 12 / 24 whose inputs fit L2, statistics -> fit -> difference per chunk, so that the second pass
+    // reads from L2: 0.95 / 0.78 ms against 0.54 ms for one chunk -- 18 / 9 times three small launches with their tails cost
+    // more than the saved HBM reads.  The kernels keep their chunk arguments; one chunk is used.)
+    const long long bpt = ppt / SUB_BLOCK;
+    const long long chunk = n_tiles;
+    if (have_stats && chunk * split > 0x7fffffffll) return ARGUS_ERR_SHAPE;
+    for (long long t0 = 0; t0 < n_tiles; t0 += chunk) {
+        const long long t1 = t0 + chunk < n_tiles ? t0 + chunk : n_tiles;
+        if (have_stats) {
+            sub_stats_kernel<<<(unsigned)((t1 - t0) * split), 256, 0, st>>>(sci_sum, sci_wsum, ref_sum, ref_wsum, ppt, split, t0, p, c->sub.partial);
+            c->n_launches++;
+        }
+        sub_fit_kernel<<<(unsigned)((t1 - t0 + 127) / 128), 128, 0, st>>>(c->sub.partial, t0, t1, split, p, have_stats, c->sub.fit, alpha_out,
+                                                                         beta_out, (int*)nvalid_out);
+        const long long nb = (t1 - t0) * bpt;
+        long long grid = nb < (long long)c->sm_count * 32 ? nb : (long long)c->sm_count * 32;
+        sub_tiles_kernel<<<(unsigned)grid, 256, 0, st>>>(sci_sum, sci_wsum, ref_sum, ref_wsum, (const long long*)layout->tiles, ppt, side_log2,
+                                                        t0 * bpt, t1 * bpt, p, c->sub.fit, diff_out, sig_out, c->sub.tmp, (unsigned)capacity,
+                                                        c->sub.blocks, c->sub.ctl);
+        c->n_launches += 2;
     }
-    sub_fit_kernel<<<(unsigned)((n_tiles + 127) / 128), 128, 0, st>>>(c->sub.partial, n_tiles, split, p, have_stats, c->sub.fit, alpha_out,
-                                                                    beta_out, (int*)nvalid_out);
-    long long grid = n_blocks < (long long)c->sm_count * 32 ? n_blocks : (long long)c->sm_count * 32;
-    sub_tiles_kernel<<<(unsigned)grid, 256, 0, st>>>(sci_sum, sci_wsum, ref_sum, ref_wsum, (const long long*)layout->tiles, ppt, side_log2,
-                                                    n_blocks, p, c->sub.fit, diff_out, sig_out, c->sub.tmp, (unsigned)capacity,
-                                                    c->sub.blocks, c->sub.ctl);
     det_scan_kernel<<<1, 1024, 0, st>>>(c->sub.blocks, (int)n_blocks, offsets, c->sub.ctl, (long long*)n_dev);
-    c->n_launches += 3;
+    c->n_launches += 1;
     if (capacity > 0) {
         sub_gather_kernel<<<(unsigned)((n_blocks + 7) / 8), 256, 0, st>>>(c->sub.blocks, offsets, n_blocks, c->sub.tmp,
                                                                         (ArgusTransientRec*)cat_out, (unsigned)capacity);

@@ -41,12 +41,12 @@ __device__ __forceinline__ unsigned spread_bits16(unsigned v) {       // bit i -
 }
 
 // ---------------------------------------------------------------------------------------------- statistics
-// grid = n_tiles * split CTAs of 256 threads; CTA (t, j) covers pixels [j, j + 1) * ppt / split of tile t.
+// grid = (tiles of the chunk) * split CTAs of 256 threads; CTA (t, j) covers pixels [j, j + 1) * ppt / split of tile tile0 + t.
 __global__ void __launch_bounds__(256) sub_stats_kernel(const float* __restrict__ ss, const float* __restrict__ sw,
                                                        const float* __restrict__ rs, const float* __restrict__ rw,
-                                                       long long ppt, int split, SubParams p, double* __restrict__ partial) {
+                                                       long long ppt, int split, long long tile0, SubParams p, double* __restrict__ partial) {
     __shared__ double s_red[8][5];
-    const long long tile = blockIdx.x / split;
+    const long long tile = tile0 + blockIdx.x / split;
     const int j = blockIdx.x % split;
     const long long n4 = (ppt / split) >> 2;                    // float4 items of this slice (ppt / split >= 1024 / 32 ...)
     const size_t base = (size_t)tile * ppt + (size_t)j * (ppt / split);
@@ -81,10 +81,10 @@ __global__ void __launch_bounds__(256) sub_stats_kernel(const float* __restrict_
 }
 
 // R-X2.  One thread per tile.  fit[t] = (alpha, beta) as floats for the per-pixel pass.
-__global__ void sub_fit_kernel(const double* __restrict__ partial, long long n_tiles, int split, SubParams p, int have_stats,
+__global__ void sub_fit_kernel(const double* __restrict__ partial, long long tile0, long long n_tiles, int split, SubParams p, int have_stats,
                                float2* __restrict__ fit, float* __restrict__ alpha_out, float* __restrict__ beta_out,
                                int* __restrict__ nvalid_out) {
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long t = tile0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;     // tiles [tile0, n_tiles) of this chunk
     if (t >= n_tiles) return;
     double alpha = 1.0, beta = 0.0, n = 0;
     if (have_stats) {
@@ -127,7 +127,7 @@ __device__ __forceinline__ void sub_px(float ssv, float swv, float rsv, float rw
 __global__ void __launch_bounds__(256) sub_tiles_kernel(const float* __restrict__ ss, const float* __restrict__ sw,
                                                        const float* __restrict__ rs, const float* __restrict__ rw,
                                                        const long long* __restrict__ tiles, long long ppt, int side_log2,
-                                                       long long n_blocks, SubParams p, const float2* __restrict__ fit,
+                                                       long long b0, long long n_blocks, SubParams p, const float2* __restrict__ fit,
                                                        float* __restrict__ diff_out, float* __restrict__ sig_out,
                                                        ArgusTransientRec* __restrict__ tmp, unsigned capacity,
                                                        uint2* __restrict__ block_info, unsigned* __restrict__ total) {
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(256) sub_tiles_kernel(const float* __restrict_
     const int side = 1 << side_log2;
     const int gx = 2 * (int)compact_even_bits((unsigned)tid), gy = 2 * (int)compact_even_bits((unsigned)tid >> 1);   // 2 x 2 group origin
     const float ninf = __int_as_float(0xff800000);
-    for (long long b = blockIdx.x; b < n_blocks; b += gridDim.x) {
+    for (long long b = b0 + blockIdx.x; b < n_blocks; b += gridDim.x) {      // blocks [b0, n_blocks) of this chunk
         const long long tile = b >> bpt_log2;
         const unsigned bi = (unsigned)(b & ((1ll << bpt_log2) - 1));
         const int Bx = 32 * (int)compact_even_bits(bi), By = 32 * (int)compact_even_bits(bi >> 1);
