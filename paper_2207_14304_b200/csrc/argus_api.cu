@@ -518,8 +518,8 @@ static int ensure_unit_scratch(argus_ctx* c, size_t n_units, int max_stray) {
     }
     c->plan_valid = false;
     const size_t want = align_up(n_units + 1, 1024);
-    const size_t o_seg = align_up((want + 1) * sizeof(int), 256), o_stray = o_seg + align_up(want * UNIT_MAXSEG * sizeof(UnitSeg), 256);
-    const size_t total = o_stray + (size_t)max_stray * sizeof(int);
+    const size_t o_seg = align_up((want + 2) * sizeof(int), 256), o_stray = o_seg + align_up(want * UNIT_MAXSEG * sizeof(UnitSeg), 256);
+    const size_t total = o_stray + 2 * (size_t)max_stray * sizeof(int);
     for (int sidx = 0; sidx < PLAN_SLOTS; ++sidx) {
         CUDA_TRY(c, cudaMalloc(&c->unit_block[sidx], total));
         char* b = (char*)c->unit_block[sidx];
@@ -536,7 +536,7 @@ static int ensure_unit_scratch(argus_ctx* c, size_t n_units, int max_stray) {
 static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, long long out_cap,
                       cudaStream_t caller, int fast_kernel, int prof_slot, const UnitGeom* ug = nullptr) {
     // Lanczos-3: any tile may be handed to the general kernel at run time (masked pixels in its box) => full records
-    const bool need_full = fast_kernel != ARGUS_BILINEAR;
+    const bool need_full = fast_kernel != ARGUS_BILINEAR && !ug;      // (the unit kernel hands over to the stray kernel instead)
     DevWcs dw;
     double rho, s_rad;
     int rc = make_devwcs(w, W, H, nside, &dw, &rho, &s_rad);
@@ -656,7 +656,8 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     if (ug) {   // segment lists of the image-aligned units (resample_unit.cuh)
         const size_t n_units = (size_t)ug->nux * (size_t)ug->nuy;
         c->slot_ub[ps].stray_count = c->slot_ub[ps].nseg + n_units;
-        CUDA_TRY(c, cudaMemsetAsync(c->slot_ub[ps].nseg, 0, (n_units + 1) * sizeof(int), st));
+        c->slot_ub[ps].stray_rt = c->slot_ub[ps].nseg + n_units + 1;
+        CUDA_TRY(c, cudaMemsetAsync(c->slot_ub[ps].nseg, 0, (n_units + 2) * sizeof(int), st));
         {   // one warp per tile, all tiles in flight at once (the kernel is a chain of latencies per tile)
             long long bound = tile_bound < c->pb.max_tiles ? tile_bound : c->pb.max_tiles;
             int gu = (int)((bound + 7) / 8);
@@ -928,7 +929,8 @@ static void unit_extent_at(const DevWcs& w, const argus_wcs* wc, int64_t nside, 
 // edge midpoints); a sub-block that exceeds them anyway is found by plan_units_kernel and served by the stray kernel.
 static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, double s_rad, int kernel, UnitGeom* g,
                           bool* tiles_fit, int margin_delta) {
-    if (kernel != ARGUS_BILINEAR) return false;
+    const int ktl = kernel == ARGUS_LANCZOS3 ? 2 : 0, ktr = kernel == ARGUS_LANCZOS3 ? 3 : 1;
+    const int kcap = kernel == ARGUS_LANCZOS3 ? FAST_CAP_PX_LZ : FAST_CAP_PX;
     double ex = 0.0, ey = 0.0;
     *tiles_fit = true;
     for (int sy = -1; sy <= 1; ++sy)
@@ -946,13 +948,13 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
             ex = fmax(ex, ax); ey = fmax(ey, ay);
             {   // would a whole 32 x 32-pixel tile fit the tile kernel's stage here?  (mirror of fast_box, worst-case alignment)
                 const int span_x = (int)ceil(31.0 / 1.5 * ax) + 3, span_y = (int)ceil(31.0 / 1.5 * ay) + 3;   // + tile-to-tile variation
-                const int bw = span_x + 1 + 7, bh = span_y + 1;
+                const int bw = span_x + ktl + ktr + 7, bh = span_y + ktl + ktr;
                 const int boxw = bw <= 40 ? 40 : (bw + 7) / 8 * 8, boxh = bh <= 48 ? 48 : (bh + 7) / 8 * 8;
-                if (bw > 72 || bh > 72 || boxw * boxh > FAST_CAP_PX) *tiles_fit = false;
+                if (bw > 72 || bh > 72 || boxw * boxh > kcap) *tiles_fit = false;
             }
         }
     memset(g, 0, sizeof(*g));
-    g->tl = 0; g->tr = 1;
+    g->tl = ktl; g->tr = ktr;
     const int chk = margin_delta > 8 ? margin_delta - 8 : 0;
     if (margin_delta > 8) margin_delta = 0;
     g->Mx = (int)ceil(1.03 * ex + 0.02) + margin_delta; g->My = (int)ceil(1.03 * ey + 0.02) + margin_delta;
@@ -977,7 +979,7 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
     g->nux = (int)((W + g->Mx + 2 - g->x_off + g->RW - 1) / g->RW);
     g->nuy = (int)((H + g->My + 2 - g->y_off + g->RH - 1) / g->RH);
     if ((long long)g->nux * g->nuy > (1ll << 24)) return false;
-    g->max_stray = 1 << 16;
+    g->max_stray = 1 << 18;
     g->chk_shrink = chk;
     return true;
 }
@@ -1023,7 +1025,7 @@ static bool unit_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H, co
 static int choose_path(argus_ctx* c, const FrameArgs& f, bool fused, int kernel, const argus_wcs* wcs, int64_t W, int64_t H, int64_t nside,
                        UnitGeom* ug) {
     if (!fused || !c->fast_enabled) return 0;
-    if (c->unit_enabled && kernel == ARGUS_BILINEAR && f.raw && !f.bpm && W % 8 == 0 && W >= 8 && aligned(f.raw, 16) &&
+    if (c->unit_enabled && f.raw && !f.bpm && W % 8 == 0 && W >= 8 && aligned(f.raw, 16) &&
         (f.pre ? (aligned(f.offset, 16) && aligned(f.gain, 16)) : (aligned(f.bias, 16) && aligned(f.dark, 16) && aligned(f.flat, 16)))) {
         DevWcs dw;
         double rho, s_rad;
@@ -1039,22 +1041,30 @@ static int choose_path(argus_ctx* c, const FrameArgs& f, bool fused, int kernel,
 }
 
 template <bool COADD>
-static int launch_units(argus_ctx* c, const UnitGeom& g, const FrameArgs& f, float w_min, float* v, float* wt, long long cap,
+static int launch_units(argus_ctx* c, int kernel, const UnitGeom& g, const FrameArgs& f, float w_min, float* v, float* wt, long long cap,
                         const CoaddArgs& ca, cudaStream_t st) {
     if (!c->unit_attr_set) {
-#define UA(CO, M) CUDA_TRY(c, cudaFuncSetAttribute(resample_unit_kernel<CO, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(UnitSmem<M>)))
-        UA(false, 0); UA(true, 0); UA(false, 1); UA(true, 1); UA(false, 2); UA(true, 2);
+#define UA(CO, K, M) CUDA_TRY(c, cudaFuncSetAttribute(resample_unit_kernel<CO, K, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(UnitSmem<M>)))
+        UA(false, 0, 0); UA(true, 0, 0); UA(false, 0, 1); UA(true, 0, 1); UA(false, 0, 2); UA(true, 0, 2);
+        UA(false, 1, 0); UA(true, 1, 0); UA(false, 1, 1); UA(true, 1, 1); UA(false, 1, 2); UA(true, 1, 2);
 #undef UA
         c->unit_attr_set = true;
     }
     const UnitBuffers& ub = c->slot_ub[c->cur_slot];
     const int grid = c->sm_count * 2;
-#define UL(M) resample_unit_kernel<COADD, M><<<grid, UNIT_THREADS, sizeof(UnitSmem<M>), st>>>(c->umaps, c->pb, ub, g, f, w_min, v, wt, cap, ca)
-    if (f.pre == 0) UL(0); else if (f.pre == 1) UL(1); else UL(2);
+    CUDA_TRY(c, cudaMemsetAsync(ub.stray_rt, 0, sizeof(int), st));      // run-time hand-overs of the previous call (cached plan)
+#define UL(K, M) resample_unit_kernel<COADD, K, M><<<grid, UNIT_THREADS, sizeof(UnitSmem<M>), st>>>(c->umaps, c->pb, ub, g, f, w_min, v, wt, cap, ca)
+    if (kernel == ARGUS_BILINEAR) { if (f.pre == 0) UL(0, 0); else if (f.pre == 1) UL(0, 1); else UL(0, 2); }
+    else { if (f.pre == 0) UL(1, 0); else if (f.pre == 1) UL(1, 1); else UL(1, 2); }
 #undef UL
-    resample_stray_kernel<COADD><<<c->sm_count, 256, 0, st>>>(c->dw, c->pb, ub, g.max_stray, f, w_min, v, wt, cap, ca);
-    // the plan's slow list (ring / pole tiles, tiles whose cubic does not fit the fixed-point split): general kernel
-    resample_tiles_kernel<0, true, COADD><<<c->sm_count * 2, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca, 1);
+    // strays, then the plan's slow list (ring / pole tiles, tiles whose cubic does not fit the fixed-point split): general kernel
+    if (kernel == ARGUS_BILINEAR) {
+        resample_stray_kernel<0, COADD><<<c->sm_count, 256, 0, st>>>(c->dw, c->pb, ub, g.max_stray, f, w_min, v, wt, cap, ca);
+        resample_tiles_kernel<0, true, COADD><<<c->sm_count * 2, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca, 1);
+    } else {
+        resample_stray_kernel<1, COADD><<<c->sm_count * 4, 256, 0, st>>>(c->dw, c->pb, ub, g.max_stray, f, w_min, v, wt, cap, ca);
+        resample_tiles_kernel<1, true, COADD><<<c->sm_count * 2, RS_THREADS, 0, st>>>(c->dw, c->pb, f, w_min, v, wt, cap, ca, 1);
+    }
     c->n_launches += 3;
     return ARGUS_OK;
 }
@@ -1125,13 +1135,13 @@ extern "C" int argus_resample(argus_ctx* c, const argus_frame* frame, const argu
     UnitGeom ug;
     const int path = choose_path(c, f, fused, kernel, wcs, W, H, nside, &ug);
     const bool use_fast = path != 0;
-    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1, path == 2 ? &ug : nullptr);
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && (kernel == ARGUS_BILINEAR || path == 2)), use_fast ? kernel : -1, path == 2 ? &ug : nullptr);
     rc = build_plan(c, wcs, W, H, nside, (long long)n, st, use_fast ? kernel : -1, c->profile ? slot : -1, path == 2 ? &ug : nullptr);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
     CoaddArgs ca;
     memset(&ca, 0, sizeof(ca));
-    if (path == 2) rc = launch_units<false>(c, ug, f, w_min, value_out, weight_out, (long long)n, ca, st);
+    if (path == 2) rc = launch_units<false>(c, kernel, ug, f, w_min, value_out, weight_out, (long long)n, ca, st);
     else rc = launch_tiles<false>(c, kernel, fused, use_fast, f, W, H, w_min, value_out, weight_out, (long long)n, ca, st);
     if (rc) return rc;
     mark_slot_read(c, st);
@@ -1350,7 +1360,7 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
     UnitGeom ug;
     const int path = choose_path(c, f, fused, kernel, wcs, W, H, nside, &ug);
     const bool use_fast = path != 0;
-    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && kernel == ARGUS_BILINEAR), use_fast ? kernel : -1, path == 2 ? &ug : nullptr);
+    bool replanned = !plan_usable(c, wcs, W, H, nside, !(use_fast && (kernel == ARGUS_BILINEAR || path == 2)), use_fast ? kernel : -1, path == 2 ? &ug : nullptr);
     rc = build_plan(c, wcs, W, H, nside, -1, st, use_fast ? kernel : -1, c->profile ? slot : -1, path == 2 ? &ug : nullptr);
     if (rc) return rc;
     if (c->profile) cudaEventRecord(c->ev[slot][2], st);
@@ -1358,7 +1368,7 @@ extern "C" int argus_resample_coadd(argus_ctx* c, const argus_frame* frame, cons
         coadd_slots_kernel<<<c->sm_count, 256, 0, st>>>(c->pb, ca);
         c->n_launches++;
     }
-    if (path == 2) rc = launch_units<true>(c, ug, f, w_min, nullptr, nullptr, 0, ca, st);
+    if (path == 2) rc = launch_units<true>(c, kernel, ug, f, w_min, nullptr, nullptr, 0, ca, st);
     else rc = launch_tiles<true>(c, kernel, fused, use_fast, f, W, H, w_min, nullptr, nullptr, 0, ca, st);
     if (rc) return rc;
     mark_slot_read(c, st);

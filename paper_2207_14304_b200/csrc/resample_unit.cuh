@@ -1,4 +1,5 @@
-// resample_unit.cuh -- A2..A5 (+A6) fused, bilinear, with IMAGE-ALIGNED work units: the second generation of the hot kernel.
+// resample_unit.cuh -- A2..A5 (+A6) fused, bilinear or Lanczos-3, with IMAGE-ALIGNED work units: the second generation of the
+// staged kernel.
 //
 // Why: a 32 x 32-pixel HEALPix tile is a diamond in the image, so the bounding box the tile kernel (resample_fast.cuh)
 // stages holds 3.5 source pixels per output pixel, and its shape changes over the sky (polar-cap tiles are taller
@@ -12,12 +13,13 @@
 //   plan_units_kernel      (plan time) one warp per tile: unit of each of the tile's 64 sub-blocks from the tile cubic
 //                          at the sub-block centre; per (unit, tile) one SEGMENT record {tile, 64-bit sub-block mask};
 //                          sub-blocks whose pixels would leave their unit's box go to the stray list
-//   resample_unit_kernel   persistent CTAs, 8 consumer warps + 1 producer warp, 2 stages; producer: TMA boxes, segment
+//   resample_unit_kernel   persistent CTAs, 8 consumer warps + 2 producer warps, 2 stages; producer: TMA boxes, segment
 //                          records (tile polynomials, output offsets, coadd slots, membership masks of border tiles),
 //                          sub-block work list; consumers: calibrate the box once in place (as the tile kernel), then every
 //                          half-warp takes one sub-block at a time: exact tile cubic per pixel (coefficients cached in
 //                          registers while the segment stays the same), 2 x 2 taps, 64-byte contiguous stores
-//   resample_stray_kernel  the stray sub-blocks, per pixel in FP64 with taps from global memory (normally none)
+//   resample_stray_kernel  the stray sub-blocks, per pixel in FP64 with taps from global memory (none found by the plan in
+//                          normal geometries; Lanczos-3 units with masked AND bright pixels hand theirs over at run time)
 // Tiles the plan classifies TC_EXACT (belt/cap ring, poles) or whose cubic does not fit the fixed-point split stay on
 // the slow list of the general kernel, exactly as with the tile kernel.
 #pragma once
@@ -53,8 +55,9 @@ struct __align__(16) UnitSeg {         // one (unit, tile) pair
 struct UnitBuffers {
     int* nseg;                         // [n_units]
     UnitSeg* seg;                      // [n_units][UNIT_MAXSEG]
-    int* stray_count;                  // device scalar
-    int* stray_list;                   // [max_stray]  tile * 64 + sub-block
+    int* stray_count;                  // device scalar: strays found by the plan
+    int* stray_rt;                     // device scalar: sub-blocks handed over at run time (Lanczos-3: masked + bright boxes)
+    int* stray_list;                   // [2 max_stray]  tile * 64 + sub-block; run-time entries from max_stray on
 };
 
 // Source position (2^-24 px relative to the record's integer base) of the point with doubled centred offsets (s, t):
@@ -171,7 +174,7 @@ struct __align__(16) UnitSegD {
     long long cslot;      // coadd slot of the tile's first pixel, -1 = tile absent from the layout
     int kofs;             // (Y0 - gy0) * pitch + (X0 - gx0)
     int mb;               // row of the border tables, -1 for inside tiles
-    int pad[2];
+    int pad[2];           // [0] = tile index in the plan
 };
 #define UNIT_PREFETCH 0                // L2 prefetch distance of the box loads in units of one CTA; 0 = off (measured: 3 is 7 % slower)
 #define UNIT_PRODUCERS 2                // producer warps: the per-unit chain (records, offsets, work list) is a chain of latencies;
@@ -215,7 +218,7 @@ __device__ __forceinline__ float calib_unit_pre(unsigned magic_r, float off, flo
 #define UNIT_MAXREG 80
 #endif
 #define UNIT_BOUNDS __maxnreg__(UNIT_MAXREG)
-template <bool COADD, int MASTERS>
+template <bool COADD, int KERNEL, int MASTERS>
 __global__ void UNIT_BOUNDS
     resample_unit_kernel(const __grid_constant__ UnitMaps maps, PlanBuffers pb, UnitBuffers ub, UnitGeom g, FrameArgs f, float w_min,
                          float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap, CoaddArgs ca) {
@@ -303,7 +306,7 @@ __global__ void UNIT_BOUNDS
             if (lane < nseg) {
                 UnitSegD& sd = d.seg[lane];
                 cls_l = sd.r.cls; mslot_l = sd.r.mask_slot;
-                sd.off = off_l; sd.cslot = cs_l;
+                sd.off = off_l; sd.cslot = cs_l; sd.pad[0] = sg.t;
                 sd.kofs = (sd.r.Y0 - gy0) * pitch + (sd.r.X0 - gx0);
             }
             const unsigned border = __ballot_sync(0xffffffffu, lane < nseg && cls_l == TC_BORDER);
@@ -390,7 +393,7 @@ __global__ void UNIT_BOUNDS
         float* cal = reinterpret_cast<float*>(st);
         // ---- A2: calibrate the staged box once (dense: item v <-> 4 pixels), registers -> barrier -> in place
         float4 o4[NI];
-        int bad = 0;
+        int bad = 0, big = 0;
 #pragma unroll
         for (int j = 0; j < NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;
@@ -402,10 +405,10 @@ __global__ void UNIT_BOUNDS
                     const float4 b = reinterpret_cast<const float4*>(st + UNIT_CAP * 2)[v];
                     const float4 dk = reinterpret_cast<const float4*>(st + UNIT_CAP * 6)[v];
                     const float4 fl = reinterpret_cast<const float4*>(st + UNIT_CAP * 10)[v];
-                    o4[j].x = calib_fast<false>(m0, b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
-                    o4[j].y = calib_fast<false>(m1, b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
-                    o4[j].z = calib_fast<false>(m2, b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
-                    o4[j].w = calib_fast<false>(m3, b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
+                    o4[j].x = calib_fast<KERNEL == 1>(m0, b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
+                    o4[j].y = calib_fast<KERNEL == 1>(m1, b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
+                    o4[j].z = calib_fast<KERNEL == 1>(m2, b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
+                    o4[j].w = calib_fast<KERNEL == 1>(m3, b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
                 } else {
                     float4 of, gn;
                     if (MASTERS == 1) {
@@ -424,9 +427,11 @@ __global__ void UNIT_BOUNDS
                     o4[j].w = calib_unit_pre(m3, of.w, gn.w, sat_f);
                 }
                 bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
+                if (KERNEL == 1) big |= (fmaxf(fmaxf(fabsf(o4[j].x), fabsf(o4[j].y)), fmaxf(fabsf(o4[j].z), fabsf(o4[j].w))) > RF_LZ_BIG_ADU);
             }
         }
         const int any_bad = bar_sync_or<1>(bad);
+        const int any_big = KERNEL == 1 ? bar_sync_or<1>(big) : 0;
 #pragma unroll
         for (int j = 0; j < NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;
@@ -436,9 +441,22 @@ __global__ void UNIT_BOUNDS
             }
         }
         bar_sync<1>();
+        const int n_sb = d.n_sb;
+        if (KERNEL == 1 && any_big && any_bad) {
+            // Lanczos-3 with masked taps next to bright pixels (saturated star cores) needs FP64 weights and coordinates
+            // (DESIGN.md 6.2): the unit's sub-blocks are handed to the stray kernel, which runs after this one.
+            for (int e = gt; e < n_sb; e += RF_CONSUMERS) {
+                const unsigned ent = d.sb[e];
+                const int k = atomicAdd(ub.stray_rt, 1);
+                if (k < g.max_stray) ub.stray_list[g.max_stray + k] = d.seg[ent >> 12].pad[0] * 64 + (int)((ent >> 6) & 63u);
+                else plan_overflow(pb, 2);
+            }
+            mbar_arrive(&sm.empty[slot]);
+            mbar_arrive(&sm.dfree[ds]);
+            continue;
+        }
 
         // ---- A3..A5: one sub-block per half-warp and pass; the segment's coefficients stay in registers
-        const int n_sb = d.n_sb;
         int cur = -1;
         float px0 = 0, px1 = 0, px2 = 0, px3 = 0, px4 = 0, px5 = 0, px6 = 0, px7 = 0, px8 = 0, px9 = 0;
         float py0 = 0, py1 = 0, py2 = 0, py3 = 0, py4 = 0, py5 = 0, py6 = 0, py7 = 0, py8 = 0, py9 = 0;
@@ -503,8 +521,8 @@ __global__ void UNIT_BOUNDS
                 RF_CHECK_BOX(pb, dbg_x + (xf1 >> FAST_FRAC_BITS), dbg_y + (yf1 >> FAST_FRAC_BITS), g.tl, g.tr, g.BW - g.chk_shrink, g.BH)
                 const float* a0 = cb + ((yf0 >> FAST_FRAC_BITS) * pitch + (xf0 >> FAST_FRAC_BITS));
                 const float* a1 = cb + ((yf1 >> FAST_FRAC_BITS) * pitch + (xf1 >> FAST_FRAC_BITS));
-                const float v0 = interp_clean<0>(a0, pitch, fast_frac(xf0), fast_frac(yf0));
-                const float v1 = interp_clean<0>(a1, pitch, fast_frac(xf1), fast_frac(yf1));
+                const float v0 = interp_clean<KERNEL>(a0, pitch, fast_frac(xf0), fast_frac(yf0));
+                const float v1 = interp_clean<KERNEL>(a1, pitch, fast_frac(xf1), fast_frac(yf1));
                 if (COADD) {        // footprint pixels are unique within a frame: plain read-modify-write, deterministic
                     sp[0] = s_a0 + v0; sp[2] = s_a1 + v1;
                     wp[0] = w_a0 + 1.0f; wp[2] = w_a1 + 1.0f;
@@ -545,8 +563,8 @@ __global__ void UNIT_BOUNDS
                 RF_CHECK_BOX(pb, dbg_x + (xf >> FAST_FRAC_BITS), dbg_y + (yf >> FAST_FRAC_BITS), g.tl, g.tr, g.BW - g.chk_shrink, g.BH)
                 const float fx = fast_frac(xf), fy = fast_frac(yf);
                 float val, wgt;
-                if (!any_bad) { val = interp_clean<0>(a, pitch, fx, fy); wgt = 1.0f; }
-                else interp_masked<0>(a, pitch, fx, fy, w_min, val, wgt);
+                if (!any_bad) { val = interp_clean<KERNEL>(a, pitch, fx, fy); wgt = 1.0f; }
+                else interp_masked<KERNEL>(a, pitch, fx, fy, w_min, val, wgt);
                 if (COADD) {
                     if (cslot >= 0) {
                         // footprint pixels are unique within a frame: plain read-modify-write, deterministic
@@ -571,14 +589,17 @@ __global__ void UNIT_BOUNDS
 }
 
 // ------------------------------------------------------------------------------------------- strays
-// Sub-blocks the unit kernel does not serve: per pixel, exact FP64 coordinates, taps from global memory.
-template <bool COADD>
+// Sub-blocks the unit kernel does not serve -- found by the plan (their pixels would leave the unit's box) or handed over at
+// run time (Lanczos-3 next to masked + bright pixels) -- per pixel, exact FP64 coordinates, taps from global memory, FP64
+// Lanczos weights.
+template <int KERNEL, bool COADD>
 __global__ void __launch_bounds__(256) resample_stray_kernel(DevWcs w, PlanBuffers pb, UnitBuffers ub, int max_stray, FrameArgs f,
                                                             float w_min, float* __restrict__ value_out, float* __restrict__ weight_out,
                                                             long long out_cap, CoaddArgs ca) {
-    const int n = min(*ub.stray_count, max_stray);
-    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < 16ll * n; i += (long long)gridDim.x * 256) {
-        const int ent = ub.stray_list[i >> 4], t = ent >> 6, sb = ent & 63, q = (int)(i & 15);
+    const int n0 = min(*ub.stray_count, max_stray), n1 = min(*ub.stray_rt, max_stray);
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < 16ll * (n0 + n1); i += (long long)gridDim.x * 256) {
+        const long long e = i >> 4;
+        const int ent = ub.stray_list[e < n0 ? e : max_stray + (e - n0)], t = ent >> 6, sb = ent & 63, q = (int)(i & 15);
         const int m = 16 * sb + q;
         const long long tile = pb.tile_id[t];
         long long pos = m;
@@ -595,21 +616,15 @@ __global__ void __launch_bounds__(256) resample_stray_kernel(DevWcs w, PlanBuffe
         double x, y;
         pixel_to_xy(w, face, tx * 32 + u, ty * 32 + v, x, y);
         const double flx = floor(x), fly = floor(y);
-        GlobalTaps<true, false> gt{&f, w.W, w.H};
+        GlobalTaps<true, KERNEL == 1> gt{&f, w.W, w.H};
         float val, wgt;
-        interp_bilinear_masked(gt, (int)flx, (int)fly, (float)(x - flx), (float)(y - fly), w_min, val, wgt);
+        if (KERNEL == 0) interp_bilinear_masked(gt, (int)flx, (int)fly, (float)(x - flx), (float)(y - fly), w_min, val, wgt);
+        else interp_lanczos3_masked(gt, (int)flx, (int)fly, x - flx, y - fly, w_min, val, wgt);
         if (COADD) {
-            const long long key = tile >> ca.shift;
-            long long lo = 0, hi = ca.n_tiles - 1, p = -1;
-            while (lo <= hi) {
-                const long long mid = (lo + hi) >> 1, tv = ca.tiles[mid];
-                if (tv == key) { p = mid; break; }
-                if (tv < key) lo = mid + 1; else hi = mid - 1;
-            }
-            if (p >= 0) {
-                const long long ppt = 1ll << (ca.shift + 10), sl = p * ppt + ((tile << 10) & (ppt - 1)) + m;
-                ca.sum[sl] = fmaf(wgt, val, ca.sum[sl]);
-                ca.wsum[sl] += wgt;
+            const long long sl0 = pb.cslot[t];                       // coadd_slots_kernel
+            if (sl0 >= 0) {
+                ca.sum[sl0 + m] = fmaf(wgt, val, ca.sum[sl0 + m]);
+                ca.wsum[sl0 + m] += wgt;
             } else if (ca.n_skipped) {
                 atomicAdd(ca.n_skipped, 1ull);
             }

@@ -476,6 +476,10 @@ def test_unit_kernel_forced(argus, cfg0, cfg0_fp, defects):
         assert info["n_units"] > 0 and info["n_stray"] == 0
         vo, wo, fl = oracle_reference(fr, idx_or, "bilinear")
         assert_values_match(v, w, vo, wo, fl, "unit kernel, config 0, defects=%s" % defects, min_amb_count=8)
+        n, v, w = gpu_resample_planned(c, fr, d, "lanczos3")
+        assert argus.argus_plan_info(c)["n_units"] > 0
+        vo, wo, fl = oracle_reference(fr, idx_or, "lanczos3")
+        assert_values_match(v, w, vo, wo, fl, "unit kernel, Lanczos-3, config 0, defects=%s" % defects, min_amb_count=8)
         tiles = np.unique(idx_or >> 18)[1:]            # one tile absent from the layout
         ppt = 1 << 18
         ref = coadd_oracle([fr, fr], [idx_or, idx_or], tiles, ppt, fr.nside, "bilinear")
@@ -487,5 +491,37 @@ def test_unit_kernel_forced(argus, cfg0, cfg0_fp, defects):
         torch.cuda.synchronize()
         assert int(sk.item()) == ref["skipped"] > 0
         assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "unit kernel coadd, defects=%s" % defects)
+    finally:
+        c.close()
+
+
+def test_unit_kernel_lanczos_saturated_stars(argus):
+    """Lanczos-3 through the unit kernel next to saturated star cores: units with masked AND bright pixels hand their
+    sub-blocks to the FP64 stray kernel at run time; repeated calls on the cached plan give identical results (the
+    run-time list is reset per call), value + weight and coadd forms."""
+    from gpu_util import assert_coadd_matches, assert_values_match, coadd_oracle, gpu_resample_planned, oracle_reference, upload
+    fr = _saturated_star_frame()
+    c = argus.Context(0)
+    try:
+        c.set_fast_path(3)
+        idx_or, _ = oracle.footprint(fr.wcs, 512, 512, fr.nside)
+        d = upload(fr)
+        vo, wo, fl = oracle_reference(fr, idx_or, "lanczos3")
+        outs = []
+        for _ in range(3):
+            n, v, w = gpu_resample_planned(c, fr, d, "lanczos3")
+            outs.append((v, w))
+        assert_values_match(outs[0][0], outs[0][1], vo, wo, fl, "unit kernel, Lanczos-3, saturated stars")
+        assert np.array_equal(outs[0][0], outs[2][0]) and np.array_equal(outs[0][1], outs[2][1])
+        tiles = np.unique(idx_or >> 18)
+        ppt = 1 << 18
+        ref = coadd_oracle([fr] * 3, [idx_or] * 3, tiles, ppt, fr.nside, "lanczos3")
+        s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
+        ws = torch.zeros_like(s)
+        for _ in range(3):
+            argus.argus_resample_coadd(c, fr.wcs, 512, 512, fr.nside, "lanczos3", torch.from_numpy(tiles).cuda(), 256, s, ws, None, **d)
+        torch.cuda.synchronize()
+        argus.argus_plan_info(c)
+        assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "unit kernel, Lanczos-3 coadd, same WCS three times")
     finally:
         c.close()
