@@ -222,7 +222,7 @@ def test_config1_full_frame_fused(argus, ctx):
     g = gpu_background(argus, ctx, W, H, 64, 16, d)
     bkg, nse = compare_grids(g, cal, mask, 64, 16, exact=False)
     rec = gpu_detect(argus, ctx, W, H, 64, 5.0, g["dev"]["bkg"], g["dev"]["nse"], d, cap=1 << 18)
-    n_must, n_amb = compare_catalogue(rec, cal, mask, bkg, nse, W, 64, 5.0, max_ambiguous=40)
+    n_must, n_amb = compare_catalogue(rec, cal, mask, bkg, nse, W, 64, 5.0, max_ambiguous=17)   # measured: 14 of 32 749 (+ 20 %)
     print("config1 detect: %d records, %d clear sources, %d ambiguous decisions" % (rec.size, n_must, n_amb))
     assert n_must > 20000
 
@@ -242,5 +242,5 @@ def test_mixed_sign_values_zeros_and_duplicates(argus, ctx, B):
     g = gpu_background(argus, ctx, W, H, B, 4, _dev_cal(cal32, mask))
     bkg, nse = compare_grids(g, cal32.astype(np.float64), mask, B, 4, exact=True)
     rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
-    n_must, n_amb = compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0, max_ambiguous=400)
+    n_must, n_amb = compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0)   # measured: 0 ambiguous (default bound 3)
     print("mixed-sign B=%d: %d records, %d clear sources, %d ambiguous decisions" % (B, rec.size, n_must, n_amb))

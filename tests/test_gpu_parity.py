@@ -525,3 +525,24 @@ def test_unit_kernel_lanczos_saturated_stars(argus):
         assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "unit kernel, Lanczos-3 coadd, same WCS three times")
     finally:
         c.close()
+
+
+def test_resample_coadd_host_matches_device_path(argus, ctx, cfg0, cfg0_fp):
+    """argus_resample_coadd_host (raw frame in HOST memory, pipelined uploads) accumulates exactly what
+    argus_resample_coadd does from device memory, over several frames."""
+    from gpu_util import upload
+    d = upload(cfg0)
+    tiles = torch.from_numpy(np.unique(cfg0_fp[0] >> 18)).cuda()
+    n_slots = tiles.numel() << 18
+    ref_s = torch.zeros(n_slots, dtype=torch.float32, device="cuda")
+    ref_w = torch.zeros_like(ref_s)
+    s = torch.zeros_like(ref_s)
+    w = torch.zeros_like(ref_s)
+    h_raw = torch.from_numpy(cfg0.raw).pin_memory()
+    for _ in range(4):
+        argus.argus_resample_coadd(ctx, cfg0.wcs, 512, 512, cfg0.nside, "bilinear", tiles, 256, ref_s, ref_w, None, **d)
+        argus.argus_resample_coadd_host(ctx, cfg0.wcs, 512, 512, cfg0.nside, "bilinear", h_raw, tiles, 256, s, w, None, bias=d["bias"],
+                                        dark=d["dark"], flat=d["flat"], t_exp=cfg0.t_exp, sat_adu=cfg0.sat_adu, flat_min=cfg0.flat_min)
+    argus.argus_host_wait(ctx)
+    torch.cuda.synchronize()
+    assert torch.equal(s, ref_s) and torch.equal(w, ref_w) and float(w.sum()) > 4 * 0.9 * len(cfg0_fp[0])
