@@ -306,6 +306,26 @@ int argus_background_map(argus_ctx* ctx, const argus_frame* frame, int64_t W, in
                          float* bkg_out, float* nse_out, float* med_out, float* sig_out, int32_t* ngood_out,
                          void* stream);
 
+/* argus_background_map_static: argus_background_map for callers that may not allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  The same two kernels, the same outputs bit for bit
+ * (R-D1, R-D2; Table 2 "Median-filtered background map"), but the 12 bytes of scratch per cell (med, sig,
+ * ngood) live in one file-scope device array of the library instead of the context, so the call needs no context and
+ * calls no cudaMalloc / cudaFree / allocating library routine, in any call including the first.
+ *   - Works on the device that is CURRENT at the call.  The scratch array holds ARGUS_BG_STATIC_MAX_CELLS cells
+ *     (12 MiB); every GPU that loads the library holds it until the process exits.  A grid with
+ *     GX * GY > ARGUS_BG_STATIC_MAX_CELLS is rejected with ARGUS_ERR_CAPACITY before anything is launched.
+ *   - The first call on a device resolves the array's device address (cudaGetSymbolAddress: no allocation, but make it
+ *     outside stream capture); later calls only launch.
+ *   - All calls on a device share the array and it keeps the last call's contents.  Nothing has to start at zero: the
+ *     first kernel writes every one of the GX * GY cells the second kernel reads, the rest is never read.  Two calls
+ *     that overlap on the GPU (different streams, or two host threads on one device) RACE on it: serialise them.
+ *   frame, W, H, cell, n_min, bkg_out, nse_out: as argus_background_map (DEVICE pointers of the current device).
+ *   cuda_error_out: HOST int (may be NULL): receives the cudaError_t when the call returns ARGUS_ERR_CUDA.
+ * Asynchronous on stream. */
+#define ARGUS_BG_STATIC_MAX_CELLS (1 << 20)
+int argus_background_map_static(const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
+                                float* bkg_out, float* nse_out, int32_t* cuda_error_out, void* stream);
+
 /* One detected source (32 bytes). */
 typedef struct argus_source {
     int32_t x, y;      /* peak pixel */

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     SOURCE_DTYPE,
     TRANSIENT_DTYPE,
     argus_background_map,
+    argus_background_map_static,
     argus_calibrate,
     argus_coadd_accumulate,
     argus_detect_sources,

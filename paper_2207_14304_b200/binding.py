@@ -25,6 +25,7 @@ EXPORTS = [
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_prepare_masters", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
     "argus_resample_host", "argus_resample_coadd_host", "argus_reduce_frame_host", "argus_host_wait", "argus_subtract_tiles", "argus_segment_products", "argus_background_map", "argus_detect_sources",
+    "argus_background_map_static",
 ]
 
 
@@ -116,6 +117,7 @@ def load_library():
                                          vp, C.POINTER(sz), vp]
     L.argus_background_map.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, i32, vp, vp, vp, vp, vp, vp]
     L.argus_detect_sources.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, vp, vp, f32, vp, sz, vp, C.POINTER(sz), vp]
+    L.argus_background_map_static.argtypes = [C.POINTER(_Frame), i64, i64, i32, i32, vp, vp, C.POINTER(i32), vp]
     L.argus_subtract_tiles.argtypes = [vp, C.POINTER(_Coadd), i64, vp, vp, vp, vp, C.POINTER(_SubParams), vp, vp, vp, vp, vp, vp, sz,
                                        vp, C.POINTER(sz), vp]
     L.argus_plan_info.argtypes = [vp, C.POINTER(_PlanStats), vp]
@@ -516,6 +518,33 @@ def argus_background_map(ctx, W, H, bkg_out, nse_out, cell=64, n_min=16, med_out
         _dev(sig_out, torch.float32, "sig_out", allow_none=True), _dev(ngood_out, torch.int32, "ngood_out", allow_none=True),
         _stream(stream))
     _check(ctx, rc, "argus_background_map")
+
+
+ARGUS_BG_STATIC_MAX_CELLS = 1 << 20
+
+
+def argus_background_map_static(W, H, bkg_out, nse_out, cell=64, n_min=16, stream=None, **frame):
+    """argus_background_map without a context and without any allocation: the cell scratch is a file-scope device array of
+    the library holding ARGUS_BG_STATIC_MAX_CELLS cells (more: ARGUS_ERR_CAPACITY).  Runs on the tensors' device, which
+    must be the current one; calls sharing a device must not overlap on the GPU."""
+    g = -(-int(H) // int(cell)) * -(-int(W) // int(cell))
+    for name, t in (("bkg_out", bkg_out), ("nse_out", nse_out)):
+        if t.numel() < g:
+            raise ValueError("%s holds %d elements, %d needed" % (name, t.numel(), g))
+    if bkg_out.device.index != torch.cuda.current_device():
+        raise ValueError("argus_background_map_static works on the current device")
+    f = _frame_struct(**frame)
+    err = C.c_int32(0)
+    rc = load_library().argus_background_map_static(
+        C.byref(f), int(W), int(H), int(cell), int(n_min), _dev(bkg_out, torch.float32, "bkg_out"),
+        _dev(nse_out, torch.float32, "nse_out"), C.byref(err), _stream(stream))
+    if rc:
+        detail = ""
+        if rc == -8:
+            detail = "cudaError=%d" % err.value
+        elif rc == -6:
+            detail = "%d cells > ARGUS_BG_STATIC_MAX_CELLS = %d" % (g, ARGUS_BG_STATIC_MAX_CELLS)
+        raise ArgusError(rc, "argus_background_map_static", detail)
 
 
 def argus_detect_sources(ctx, W, H, bkg, nse, out, cell=64, k_sigma=5.0, n_dev=None, sync=True, stream=None, **frame):

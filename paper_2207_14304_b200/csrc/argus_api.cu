@@ -6,6 +6,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1516,6 +1517,65 @@ extern "C" int argus_background_map(argus_ctx* c, const argus_frame* frame, int6
     bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
     c->n_launches += 2;
     CUDA_TRY(c, cudaGetLastError());
+    return ARGUS_OK;
+}
+
+// ---- argus_background_map_static: the same two kernels with the cell scratch in a file-scope device array (no allocation).
+// In host code `g_bg_static_cells` is only a host-side stand-in for the symbol, never a device address: the address of the
+// array on a device comes from cudaGetSymbolAddress with that device current, once per device (bg_static_address).
+// Layout as the context's bg.cells: med [MAX] | sig [MAX] | ngood [MAX] (int bits), 12 bytes per cell.
+#define BG_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) float g_bg_static_cells[3 * (size_t)ARGUS_BG_STATIC_MAX_CELLS];
+static std::mutex g_bg_static_mutex;
+static float* g_bg_static_ptr[BG_STATIC_MAX_DEVICES];   // device address of g_bg_static_cells per device, nullptr = not resolved yet
+
+static cudaError_t bg_static_address(float** ptr) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= BG_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_bg_static_mutex);
+    if (!g_bg_static_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_bg_static_cells);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_bg_static_ptr[dev] = (float*)p;
+    }
+    *ptr = g_bg_static_ptr[dev];
+    return cudaSuccess;
+}
+
+extern "C" int argus_background_map_static(const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
+                                           float* bkg_out, float* nse_out, int32_t* cuda_error_out, void* stream) {
+    if (!frame || !bkg_out || !nse_out) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n_min < 0) return ARGUS_ERR_SHAPE;
+    if (bg_check_cell(cell)) return ARGUS_ERR_SHAPE;
+    if (!aligned(bkg_out, 4) || !aligned(nse_out, 4)) return ARGUS_ERR_ALIGN;
+    FrameArgs f;
+    bool fused;
+    int rc = make_frameargs(frame, W, H, &f, &fused);
+    if (rc) return rc;
+    const int64_t GX = (W + cell - 1) / cell, GY = (H + cell - 1) / cell, G = GX * GY;
+    if (G > (int64_t)ARGUS_BG_STATIC_MAX_CELLS) return ARGUS_ERR_CAPACITY;   // the static scratch holds no more cells
+    cudaStream_t st = (cudaStream_t)stream;
+    float* cells = nullptr;
+    cudaError_t e = bg_static_address(&cells);
+    if (e == cudaSuccess) {
+        float* med = cells;
+        float* sig = cells + (size_t)ARGUS_BG_STATIC_MAX_CELLS;
+        int* ngood = (int*)(cells + 2 * (size_t)ARGUS_BG_STATIC_MAX_CELLS);
+        if (fused)
+            bg_cells_kernel<true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+        else
+            bg_cells_kernel<false><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+        bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+        if (cuda_error_out) *cuda_error_out = (int32_t)e;
+        return ARGUS_ERR_CUDA;
+    }
     return ARGUS_OK;
 }
 
