@@ -352,6 +352,24 @@ int argus_detect_sources(argus_ctx* ctx, const argus_frame* frame, int64_t W, in
                          const float* nse, float k_sigma, argus_source* out, size_t capacity, int64_t* n_dev,
                          size_t* n_out, void* stream);
 
+/* argus_detect_frame: argus_background_map followed by argus_detect_sources in ONE call that reads the frame once
+ * (Table 2: the two stages run back to back on every frame; DESIGN.md section 11 "one pass").  While a
+ * cell's pixels are in registers for its median, every good pixel above cut = med + kappa * sig of its cell
+ * (kappa = max(k_sigma - 2, 2.5); all good pixels of an invalid cell) is noted as a candidate of its 64 x 32-pixel tile.
+ * After the 3 x 3 filter a tile is served from its candidates alone when min over the nodes it touches of
+ * (bkg + k_sigma * nse) lies above the cuts of the cells it overlaps (then no other pixel can pass the threshold); the
+ * other tiles, and tiles with more than 48 candidates, are scanned in full as argus_detect_sources does.
+ * bkg_out, nse_out (DEVICE, GX * GY floats, required), out / capacity / n_dev / n_out / error behaviour: exactly the
+ * results of the two calls, bit for bit, catalogue order included.  Scratch: 12 + 4 bytes per cell, 116 bytes per
+ * tile, 40 bytes per record of capacity, grown on demand (which synchronises the device); otherwise asynchronous. */
+int argus_detect_frame(argus_ctx* ctx, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
+                       float k_sigma, float* bkg_out, float* nse_out, argus_source* out, size_t capacity, int64_t* n_dev,
+                       size_t* n_out, void* stream);
+
+/* Synchronises the stream and reports how many tiles the last argus_detect_frame of this context scanned in full
+ * (HOST pointer).  ARGUS_ERR_STATE before the first call. */
+int argus_detect_frame_info(argus_ctx* ctx, int64_t* n_full_tiles, void* stream);
+
 /* ---- Direct image subtraction per tile: "Transient detection is performed using image subtraction in
  * the reprojected HEALPix image segments, leveraging long-term coadds as reference frames ... the direct image
  * subtraction method ... for real-time operation in 1-second cadence data" (sec. 5.2), per tile,

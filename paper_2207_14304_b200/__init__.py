@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     argus_background_map_static,
     argus_calibrate,
     argus_coadd_accumulate,
+    argus_detect_frame,
+    argus_detect_frame_info,
     argus_detect_sources,
     argus_healpix_footprint,
     argus_plan_info,

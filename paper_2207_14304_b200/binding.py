@@ -25,7 +25,7 @@ EXPORTS = [
     "argus_last_cuda_error", "argus_launch_count", "argus_calibrate", "argus_prepare_masters", "argus_healpix_footprint", "argus_resample",
     "argus_coadd_accumulate", "argus_resample_coadd", "argus_plan_info", "argus_profile_read",
     "argus_resample_host", "argus_resample_coadd_host", "argus_reduce_frame_host", "argus_host_wait", "argus_subtract_tiles", "argus_segment_products", "argus_background_map", "argus_detect_sources",
-    "argus_background_map_static",
+    "argus_background_map_static", "argus_detect_frame", "argus_detect_frame_info",
 ]
 
 
@@ -117,6 +117,8 @@ def load_library():
                                          vp, C.POINTER(sz), vp]
     L.argus_background_map.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, i32, vp, vp, vp, vp, vp, vp]
     L.argus_detect_sources.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, vp, vp, f32, vp, sz, vp, C.POINTER(sz), vp]
+    L.argus_detect_frame.argtypes = [vp, C.POINTER(_Frame), i64, i64, i32, i32, f32, vp, vp, vp, sz, vp, C.POINTER(sz), vp]
+    L.argus_detect_frame_info.argtypes = [vp, C.POINTER(i64), vp]
     L.argus_background_map_static.argtypes = [C.POINTER(_Frame), i64, i64, i32, i32, vp, vp, C.POINTER(i32), vp]
     L.argus_subtract_tiles.argtypes = [vp, C.POINTER(_Coadd), i64, vp, vp, vp, vp, C.POINTER(_SubParams), vp, vp, vp, vp, vp, vp, sz,
                                        vp, C.POINTER(sz), vp]
@@ -566,6 +568,36 @@ def argus_detect_sources(ctx, W, H, bkg, nse, out, cell=64, k_sigma=5.0, n_dev=N
         raise ArgusError(rc, "argus_detect_sources", "n_sources=%d" % n.value)
     _check(ctx, rc, "argus_detect_sources")
     return int(n.value) if sync else None
+
+
+def argus_detect_frame(ctx, W, H, bkg_out, nse_out, out, cell=64, n_min=16, k_sigma=5.0, n_dev=None, sync=True, stream=None,
+                       **frame):
+    """argus_background_map + argus_detect_sources in one call that reads the frame once (identical results).  Returns the
+    number of sources found when sync, else None."""
+    cap = 0 if out is None else out.numel() // 32
+    if out is not None and out.dtype != torch.uint8:
+        raise TypeError("out must be a uint8 tensor (32 bytes per record)")
+    g = -(-int(H) // int(cell)) * -(-int(W) // int(cell))
+    if bkg_out.numel() < g or nse_out.numel() < g:
+        raise ValueError("bkg_out / nse_out hold fewer than %d cells" % g)
+    f = _frame_struct(**frame)
+    n = C.c_size_t(0)
+    rc = load_library().argus_detect_frame(
+        ctx._h, C.byref(f), int(W), int(H), int(cell), int(n_min), float(k_sigma), _dev(bkg_out, torch.float32, "bkg_out"),
+        _dev(nse_out, torch.float32, "nse_out"), _dev(out, torch.uint8, "out", allow_none=True), cap,
+        _dev(n_dev, torch.int64, "n_dev", allow_none=True), C.byref(n) if sync else None, _stream(stream))
+    if rc == -6 and sync:
+        raise ArgusError(rc, "argus_detect_frame", "n_sources=%d" % n.value)
+    _check(ctx, rc, "argus_detect_frame")
+    return int(n.value) if sync else None
+
+
+def argus_detect_frame_info(ctx, stream=None) -> int:
+    """Tiles the last argus_detect_frame scanned in full (synchronises)."""
+    v = C.c_int64(0)
+    rc = load_library().argus_detect_frame_info(ctx._h, C.byref(v), _stream(stream))
+    _check(ctx, rc, "argus_detect_frame_info")
+    return int(v.value)
 
 
 # numpy view of argus_transient records (argus.h)

@@ -6,6 +6,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -104,6 +105,8 @@ struct argus_ctx {
         uint2* ord;                              // (band-local raster key, position in tmp) per record, cap_tmp entries
         unsigned* ctl;                           // [0] running total (atomics), [1] final count
         long long* h_n;                          // pinned
+        unsigned char* cand; size_t cap_cand;    // argus_detect_frame: cuts, candidate lists, handed-over tiles (bytes)
+        unsigned* last_fb;                       // device word: tiles the last argus_detect_frame scanned in full
     } bg;
     // argus_subtract_tiles: per-slice partial sums, per-tile fit, per-block (base, count) + offsets, record staging
     struct SubScratch {
@@ -356,6 +359,7 @@ extern "C" int argus_ctx_destroy(argus_ctx* c) {
     if (c->seg.ctl) cudaFree(c->seg.ctl);
     if (c->seg.h_n) cudaFreeHost(c->seg.h_n);
     if (c->bg.cells) cudaFree(c->bg.cells);
+    if (c->bg.cand) cudaFree(c->bg.cand);
     if (c->bg.tiles) cudaFree(c->bg.tiles);
     if (c->bg.tmp) cudaFree(c->bg.tmp);
     if (c->bg.ord) cudaFree(c->bg.ord);
@@ -1511,9 +1515,9 @@ extern "C" int argus_background_map(argus_ctx* c, const argus_frame* frame, int6
     float* sig = sig_out ? sig_out : c->bg.cells + c->bg.cap_cells;
     int* ngood = ngood_out ? (int*)ngood_out : (int*)(c->bg.cells + 2 * c->bg.cap_cells);
     if (fused)
-        bg_cells_kernel<true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+        bg_cells_kernel<true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, BgCand{});
     else
-        bg_cells_kernel<false><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+        bg_cells_kernel<false><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, BgCand{});
     bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
     c->n_launches += 2;
     CUDA_TRY(c, cudaGetLastError());
@@ -1566,15 +1570,65 @@ extern "C" int argus_background_map_static(const argus_frame* frame, int64_t W, 
         float* sig = cells + (size_t)ARGUS_BG_STATIC_MAX_CELLS;
         int* ngood = (int*)(cells + 2 * (size_t)ARGUS_BG_STATIC_MAX_CELLS);
         if (fused)
-            bg_cells_kernel<true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+            bg_cells_kernel<true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, BgCand{});
         else
-            bg_cells_kernel<false><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood);
+            bg_cells_kernel<false><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, BgCand{});
         bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) {
         if (cuda_error_out) *cuda_error_out = (int32_t)e;
         return ARGUS_ERR_CUDA;
+    }
+    return ARGUS_OK;
+}
+
+// Detection scratch (grown on demand, which synchronises the device): pinned count, control words, per-tile
+// (base, count) + offsets, record staging for `capacity` records.
+static int det_ensure_scratch(argus_ctx* c, int64_t n_tiles, size_t capacity) {
+    if (!c->bg.h_n) CUDA_TRY(c, cudaMallocHost((void**)&c->bg.h_n, sizeof(long long)));
+    if (!c->bg.ctl) CUDA_TRY(c, cudaMalloc((void**)&c->bg.ctl, 16));
+    if (c->bg.cap_tiles < (size_t)n_tiles || !c->bg.tiles) {
+        if (c->bg.tiles) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tiles); c->bg.tiles = nullptr; }
+        size_t want = align_up((size_t)n_tiles, 4096);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tiles, want * 12));
+        c->bg.cap_tiles = want;
+    }
+    if (c->bg.cap_tmp < capacity || !c->bg.tmp) {
+        if (c->bg.tmp) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tmp); cudaFree(c->bg.ord); c->bg.tmp = nullptr; c->bg.ord = nullptr; }
+        size_t want = align_up(capacity + 1, 65536);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tmp, want * sizeof(ArgusSourceRec)));
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.ord, want * sizeof(uint2)));
+        c->bg.cap_tmp = want;
+    }
+    return ARGUS_OK;
+}
+
+static DetGrid det_grid(const float* bkg, const float* nse, int64_t W, int64_t H, int32_t cell, float k_sigma) {
+    DetGrid g;
+    g.bkg = bkg; g.nse = nse; g.B = cell;
+    g.GX = (int)((W + cell - 1) / cell); g.GY = (int)((H + cell - 1) / cell);
+    g.inv_B = 1.0f / (float)cell; g.half = 0.5f * (float)(cell - 1); g.k_sigma = k_sigma;
+    return g;
+}
+
+// Tile counts -> offsets, records -> catalogue order, count to the caller (R-D6; shared by both detection entry points).
+static int det_finish(argus_ctx* c, int64_t n_tiles, int64_t tiles_x, int64_t tiles_y, int64_t W, argus_source* out,
+                      size_t capacity, int64_t* n_dev, size_t* n_out, cudaStream_t st) {
+    unsigned* offsets = (unsigned*)(c->bg.tiles + c->bg.cap_tiles);
+    det_scan_kernel<<<1, 1024, 0, st>>>(c->bg.tiles, (int)n_tiles, offsets, c->bg.ctl, (long long*)n_dev);
+    c->n_launches++;
+    if (capacity > 0) {
+        det_order_kernel<<<(unsigned)tiles_y, 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, (int)tiles_x, (int)W, c->bg.ctl,
+                                                           c->bg.tmp, c->bg.ord, (ArgusSourceRec*)out, (unsigned)capacity);
+        c->n_launches++;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    if (n_out) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->bg.h_n, c->bg.ctl, 8, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        *n_out = (size_t)(((unsigned long long)*c->bg.h_n) >> 32);     // ctl[1]
+        if (capacity > 0 && *n_out > capacity) return ARGUS_ERR_CAPACITY;
     }
     return ARGUS_OK;
 }
@@ -1596,26 +1650,9 @@ extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int6
     if (n_tiles > 0x7fffffffll) return ARGUS_ERR_SHAPE;
     cudaStream_t st = (cudaStream_t)stream;
     CUDA_TRY(c, cudaSetDevice(c->device));
-    if (!c->bg.h_n) CUDA_TRY(c, cudaMallocHost((void**)&c->bg.h_n, sizeof(long long)));
-    if (!c->bg.ctl) CUDA_TRY(c, cudaMalloc((void**)&c->bg.ctl, 16));
-    if (c->bg.cap_tiles < (size_t)n_tiles || !c->bg.tiles) {
-        if (c->bg.tiles) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tiles); c->bg.tiles = nullptr; }
-        size_t want = align_up((size_t)n_tiles, 4096);
-        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tiles, want * 12));
-        c->bg.cap_tiles = want;
-    }
-    if (c->bg.cap_tmp < capacity || !c->bg.tmp) {
-        if (c->bg.tmp) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tmp); cudaFree(c->bg.ord); c->bg.tmp = nullptr; c->bg.ord = nullptr; }
-        size_t want = align_up(capacity + 1, 65536);
-        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tmp, want * sizeof(ArgusSourceRec)));
-        CUDA_TRY(c, cudaMalloc((void**)&c->bg.ord, want * sizeof(uint2)));
-        c->bg.cap_tmp = want;
-    }
-    unsigned* offsets = (unsigned*)(c->bg.tiles + c->bg.cap_tiles);
-    DetGrid g;
-    g.bkg = bkg; g.nse = nse; g.B = cell;
-    g.GX = (int)((W + cell - 1) / cell); g.GY = (int)((H + cell - 1) / cell);
-    g.inv_B = 1.0f / (float)cell; g.half = 0.5f * (float)(cell - 1); g.k_sigma = k_sigma;
+    rc = det_ensure_scratch(c, n_tiles, capacity);
+    if (rc) return rc;
+    const DetGrid g = det_grid(bkg, nse, W, H, cell, k_sigma);
     CUDA_TRY(c, cudaMemsetAsync(c->bg.ctl, 0, 16, st));
     if (fused)
         det_tiles_kernel<true><<<(unsigned)n_tiles, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity,
@@ -1623,20 +1660,93 @@ extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int6
     else
         det_tiles_kernel<false><<<(unsigned)n_tiles, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity,
                                                                 c->bg.tiles, c->bg.ctl);
-    det_scan_kernel<<<1, 1024, 0, st>>>(c->bg.tiles, (int)n_tiles, offsets, c->bg.ctl, (long long*)n_dev);
-    c->n_launches += 2;
-    if (capacity > 0) {
-        det_order_kernel<<<(unsigned)tiles_y, 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, (int)tiles_x, (int)W, c->bg.ctl,
-                                                           c->bg.tmp, c->bg.ord, (ArgusSourceRec*)out, (unsigned)capacity);
-        c->n_launches++;
+    c->n_launches++;
+    return det_finish(c, n_tiles, tiles_x, tiles_y, W, out, capacity, n_dev, n_out, st);
+}
+
+// Background map + detection in one call: the candidates of every tile are collected while the cell statistics are formed,
+// so the frame is read once; results identical to argus_background_map followed by argus_detect_sources.
+extern "C" int argus_detect_frame(argus_ctx* c, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
+                                  float k_sigma, float* bkg_out, float* nse_out, argus_source* out, size_t capacity,
+                                  int64_t* n_dev, size_t* n_out, void* stream) {
+    if (!c) return ARGUS_ERR_NULL;
+    if (n_out) *n_out = 0;
+    if (!frame || !bkg_out || !nse_out || (capacity > 0 && !out)) return ARGUS_ERR_NULL;
+    if (W < 1 || H < 1 || W > (1 << 20) || H > (1 << 20) || n_min < 0 || capacity > 0x7fffffffull) return ARGUS_ERR_SHAPE;
+    if (bg_check_cell(cell) || !(k_sigma >= 0.0f) || !(k_sigma < INFINITY)) return ARGUS_ERR_SHAPE;
+    if (!aligned(bkg_out, 4) || !aligned(nse_out, 4) || !aligned(out, 16) || !aligned(n_dev, 8)) return ARGUS_ERR_ALIGN;
+    FrameArgs f;
+    bool fused;
+    int rc = make_frameargs(frame, W, H, &f, &fused);
+    if (rc) return rc;
+    const int64_t GX = (W + cell - 1) / cell, GY = (H + cell - 1) / cell, G = GX * GY;
+    const int64_t tiles_x = (W + DET_TW - 1) / DET_TW, tiles_y = (H + DET_TH - 1) / DET_TH, n_tiles = tiles_x * tiles_y;
+    if (G > 0x7fffffffll || n_tiles > 0x7fffffffll) return ARGUS_ERR_SHAPE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    if (c->bg.cap_cells < (size_t)G || !c->bg.cells) {
+        if (c->bg.cells) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.cells); c->bg.cells = nullptr; }
+        size_t want = align_up((size_t)G, 4096);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.cells, want * 12));
+        c->bg.cap_cells = want;
     }
-    CUDA_TRY(c, cudaGetLastError());
-    if (n_out) {
-        CUDA_TRY(c, cudaMemcpyAsync(c->bg.h_n, c->bg.ctl, 8, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(c, cudaStreamSynchronize(st));
-        *n_out = (size_t)(((unsigned long long)*c->bg.h_n) >> 32);     // ctl[1]
-        if (capacity > 0 && *n_out > capacity) return ARGUS_ERR_CAPACITY;
+    // candidate scratch: cut [G] | cnt [n_lists] | fb_count (4 words) | fb_list [n_tiles] | list [n_lists][cap] u16
+    const size_t n_lists = (cell == 64 ? 2 : 1) * (size_t)G, Gp = align_up((size_t)G, 64), Lp = align_up(n_lists, 64), Tp = align_up((size_t)n_tiles, 64);
+    const size_t cand_bytes = (Gp + Lp + 4 + Tp) * 4 + Lp * (size_t)det_cand_cap(cell) * 2;
+    if (c->bg.cap_cand < cand_bytes || !c->bg.cand) {
+        if (c->bg.cand) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.cand); c->bg.cand = nullptr; }
+        const size_t want = align_up(cand_bytes, (size_t)1 << 20);
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.cand, want));
+        c->bg.cap_cand = want;
     }
+    rc = det_ensure_scratch(c, n_tiles, capacity);
+    if (rc) return rc;
+    BgCand cd;
+    cd.cut = (float*)c->bg.cand;
+    cd.cnt = (unsigned*)(cd.cut + Gp);
+    unsigned* fb_count = cd.cnt + Lp;
+    unsigned* fb_list = fb_count + 4;
+    cd.list = (unsigned short*)(fb_list + Tp);
+    // the cut must leave room below the threshold for the proof of det_cand_kernel and keep the lists short
+    cd.kappa = fmaxf(k_sigma - 2.0f, 2.5f);
+    float* med = c->bg.cells;
+    float* sig = c->bg.cells + c->bg.cap_cells;
+    int* ngood = (int*)(c->bg.cells + 2 * c->bg.cap_cells);
+    const DetGrid g = det_grid(bkg_out, nse_out, W, H, cell, k_sigma);
+    CUDA_TRY(c, cudaMemsetAsync(c->bg.ctl, 0, 16, st));
+    CUDA_TRY(c, cudaMemsetAsync(fb_count, 0, 16, st));
+    const unsigned fb_grid = (unsigned)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * 8);
+    if (fused) {
+        bg_cells_kernel<true, true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, cd);
+        bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
+        det_cand_kernel<true><<<(unsigned)((n_tiles + 7) / 8), 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, (int)n_tiles, cd.cnt, cd.list,
+                                                                             cd.cut, c->bg.tmp, (unsigned)capacity, c->bg.tiles, c->bg.ctl,
+                                                                             fb_list, fb_count);
+        det_tiles_list_kernel<true><<<fb_grid, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity, c->bg.tiles,
+                                                             c->bg.ctl, fb_list, fb_count);
+    } else {
+        bg_cells_kernel<false, true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, cd);
+        bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
+        det_cand_kernel<false><<<(unsigned)((n_tiles + 7) / 8), 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, (int)n_tiles, cd.cnt, cd.list,
+                                                                              cd.cut, c->bg.tmp, (unsigned)capacity, c->bg.tiles, c->bg.ctl,
+                                                                              fb_list, fb_count);
+        det_tiles_list_kernel<false><<<fb_grid, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity, c->bg.tiles,
+                                                              c->bg.ctl, fb_list, fb_count);
+    }
+    c->n_launches += 4;
+    c->bg.last_fb = fb_count;
+    return det_finish(c, n_tiles, tiles_x, tiles_y, W, out, capacity, n_dev, n_out, st);
+}
+
+extern "C" int argus_detect_frame_info(argus_ctx* c, int64_t* n_full_tiles, void* stream) {
+    if (!c || !n_full_tiles) return ARGUS_ERR_NULL;
+    *n_full_tiles = 0;
+    if (!c->bg.last_fb) return ARGUS_ERR_STATE;
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    unsigned v = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&v, c->bg.last_fb, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
+    *n_full_tiles = (int64_t)v;
     return ARGUS_OK;
 }
 

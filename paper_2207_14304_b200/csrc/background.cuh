@@ -206,16 +206,59 @@ __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], i
     }
 }
 
+// Detection candidates of argus_detect_frame ("one pass"): while a cell's pixels are in registers,
+// bg_cells_kernel<., true> notes every good pixel with |v - med| > kappa * sig (all good pixels of an invalid cell) in the
+// cell's own candidate list and stores cut = med + kappa * sig per cell (-inf: invalid cell).  det_cand_kernel later proves
+// per 64 x 32-pixel detection tile that no pixel below its cells' cuts can pass the detection threshold and then looks at
+// the candidates of the cells it overlaps only; tiles where the proof fails or a list overflowed are scanned in full.
+// Lists are per cell, so bg_cells_kernel writes them with plain stores (no global atomic, nothing to clear): a cell of
+// B <= 32 lies in one tile (one list of det_cand_cap(B) entries); a cell of 64 is two stacked tiles (two lists).
+#define DET_TW 64
+#define DET_TH 32
+#define DET_CAND_CAP 48              // candidates looked at per tile (2.3 % of its pixels); more: the tile is scanned in full
+__host__ __device__ __forceinline__ int det_cand_cap(int B) { return B == 64 ? DET_CAND_CAP : B == 32 ? 24 : B == 16 ? 8 : 4; }
+struct BgCand {
+    unsigned* cnt;                   // [n_lists] candidates found per list (may exceed its capacity); n_lists = G (2 G at B = 64)
+    unsigned short* list;            // [n_lists][det_cand_cap(B)] position in the tile: (y - y0) * 64 + (x - x0)
+    float* cut;                      // [G]
+    float kappa;
+};
+
+struct BgCandShared {
+    unsigned short loc[2][DET_CAND_CAP];
+    unsigned n[2];
+};
+__device__ __forceinline__ void bg_cand_push(BgCandShared& sc, int x0, int y0, int lx, int ly, int B) {
+    const int h = (B == 64) ? (ly >> 5) : 0;
+    const unsigned pos = atomicAdd(&sc.n[h], 1u);
+    if (pos < DET_CAND_CAP) sc.loc[h][pos] = (unsigned short)(((y0 + ly) % DET_TH) * DET_TW + (x0 + lx) % DET_TW);
+}
+// all threads of the CTA, after the last push
+__device__ __forceinline__ void bg_cand_flush(BgCandShared& sc, const BgCand& cd, int cell, int B) {
+    __syncthreads();
+    const int tid = threadIdx.x, h = tid >> 6, t = tid & 63, cap = det_cand_cap(B);
+    if (h >= (B == 64 ? 2 : 1)) return;
+    const size_t l = (B == 64) ? 2 * (size_t)cell + h : (size_t)cell;
+    const unsigned n = sc.n[h];
+    if (t == 0) cd.cnt[l] = n;
+    if (t < min(n, (unsigned)cap)) cd.list[l * cap + t] = sc.loc[h][t];
+}
+
 // R-D1: per-cell median, 1.4826 MAD and good-pixel count.  grid = GX * GY CTAs of 256 threads; B in {8,16,32,64}.
-template <bool FUSED>
-__global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W, int H, int B, int GX, int n_min,
+#ifndef BG_MINB
+#define BG_MINB 5                    // 48 registers: the kernel waits at its barriers, residency pays (4 CTAs/SM: 9 % slower)
+#endif
+template <bool FUSED, bool CAND = false>
+__global__ void __launch_bounds__(BG_THREADS, BG_MINB) bg_cells_kernel(FrameArgs f, int W, int H, int B, int GX, int n_min,
                                                               float* __restrict__ med_out, float* __restrict__ sig_out,
-                                                              int* __restrict__ ngood_out) {
+                                                              int* __restrict__ ngood_out, BgCand cd) {
     __shared__ __align__(16) int s_red[20];
     __shared__ unsigned s_list[BG_FINISH + 2];
     __shared__ int s_hist[256 + 12];
     __shared__ int s_cnt;
+    __shared__ BgCandShared s_cand;
     if (threadIdx.x < 3) s_red[16 + threadIdx.x] = 0;
+    if (CAND && threadIdx.x < 2) s_cand.n[threadIdx.x] = 0u;
     __syncthreads();
     const int cell = blockIdx.x, gx = cell % GX, gy = cell / GX;
     const int x0 = gx * B, y0 = gy * B, x_end = min(x0 + B, W), y_end = min(y0 + B, H);
@@ -241,6 +284,18 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
     n = bg_block_sum(n, s_red, par, it);
     if (n < max(n_min, 1)) {
         if (threadIdx.x == 0) { med_out[cell] = 0.f; sig_out[cell] = 0.f; ngood_out[cell] = n; }
+        if (CAND) {                                  // no statistics to cut on: every good pixel is a candidate
+            if (threadIdx.x == 0) cd.cut[cell] = __int_as_float(0xff800000);
+            unsigned m = 0u;
+#pragma unroll
+            for (int i = 0; i < BG_KPT; ++i) m |= (key[i] != BG_SENTINEL) ? (1u << i) : 0u;
+            while (m) {
+                const int i = __ffs(m) - 1;
+                m &= m - 1u;
+                bg_cand_push(s_cand, x0, y0, col + (i & 3), row + 16 * (i >> 2), B);
+            }
+            bg_cand_flush(s_cand, cd, cell, B);
+        }
         return;
     }
     lo = bg_block_min(lo, s_red, par);
@@ -263,6 +318,19 @@ __global__ void __launch_bounds__(BG_THREADS) bg_cells_kernel(FrameArgs f, int W
     bg_central_pair(key, n, lo, hi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
     const float mad = 0.5f * (__uint_as_float(k1) + __uint_as_float(k2));
     if (threadIdx.x == 0) { med_out[cell] = med; sig_out[cell] = BG_MAD_TO_SIGMA * mad; ngood_out[cell] = n; }
+    if (CAND) {
+        const float cthr = cd.kappa * (BG_MAD_TO_SIGMA * mad);
+        if (threadIdx.x == 0) cd.cut[cell] = med + cthr;
+        unsigned m = 0u;                             // the sentinel reads as NaN: never above the cut
+#pragma unroll
+        for (int i = 0; i < BG_KPT; ++i) m |= (__uint_as_float(key[i]) > cthr) ? (1u << i) : 0u;
+        while (m) {                                  // 0.9 % of the pixels: one or two rounds per warp
+            const int i = __ffs(m) - 1;
+            m &= m - 1u;
+            bg_cand_push(s_cand, x0, y0, col + (i & 3), row + 16 * (i >> 2), B);
+        }
+        bg_cand_flush(s_cand, cd, cell, B);
+    }
 }
 
 // R-D2: 3x3 median over the valid cells (clipped to the grid); no valid cell: bkg = 0, nse = +inf.
@@ -293,8 +361,6 @@ __global__ void __launch_bounds__(128) bg_filter_kernel(const float* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------ detection
-#define DET_TW 64
-#define DET_TH 32
 #define DET_PITCH 66                 // 64 + 2 apron columns; 66 mod 32 = 2 spreads a warp's four rows over the banks
 #define DET_PCOLS 12                 // node columns a tile can touch: (DET_TW + 2) / 8 + 2 at B = 8
 
@@ -315,10 +381,29 @@ __device__ __forceinline__ void det_node(int p, const DetGrid& g, int G, int& g0
 // R-D4 / R-D5 on one 64 x 32 tile.  tile_info[tile] = (base of the tile's records in tmp, count); *total counts all.
 // Staging: the grids are interpolated along y once per tile row (s_rb / s_rn, straight from the L2-resident grids), the
 // x node and fraction of every tile column are tabulated (s_col): a pixel's background costs two shared loads + one FMA.
+// R-D5 record of the source at (x, y): q = s over its 3 x 3 window in raster order (-inf: masked or off-frame), bkg / nse the
+// interpolated maps at the peak.  One function for both detection paths (their catalogues are identical bit for bit).
+__device__ __forceinline__ void det_write_record(ArgusSourceRec* __restrict__ dst_rec, int x, int y, const float (&q)[9], float bkg,
+                                                 float nse) {
+    const float ninf = __int_as_float(0xff800000);
+    float flux = 0.f, mx = 0.f, my = 0.f;
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float v = q[3 * r + c];
+            if (v != ninf) { flux += v; mx += v * (float)(c - 1); my += v * (float)(r - 1); }
+        }
+    const float cx = flux > 0.f ? mx / flux : 0.f, cy = flux > 0.f ? my / flux : 0.f;
+    uint4* dst = reinterpret_cast<uint4*>(dst_rec);
+    dst[0] = make_uint4((unsigned)x, (unsigned)y, __float_as_uint(q[4]), __float_as_uint(flux));
+    dst[1] = make_uint4(__float_as_uint(cx), __float_as_uint(cy), __float_as_uint(bkg), __float_as_uint(nse));
+}
+
 template <bool FUSED>
-__global__ void __launch_bounds__(256, 8) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
-                                                           ArgusSourceRec* __restrict__ tmp, unsigned capacity,
-                                                           uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
+__device__ __forceinline__ void det_tile_body(const int tile, const FrameArgs& f, int W, int H, const DetGrid& g, int tiles_x,
+                                              ArgusSourceRec* __restrict__ tmp, unsigned capacity,
+                                              uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
     __shared__ float s_s[(DET_TH + 2) * DET_PITCH];
     __shared__ float s_rb[DET_TH + 2][DET_PCOLS], s_rn[DET_TH + 2][DET_PCOLS];
     __shared__ float2 s_col[DET_PITCH];              // (.x: node offsets lx | lx1 << 8 as int bits, .y: tx)
@@ -326,7 +411,7 @@ __global__ void __launch_bounds__(256, 8) det_tiles_kernel(FrameArgs f, int W, i
     __shared__ unsigned s_base, s_nmin;              // s_nmin: bits of the smallest noise node the tile touches
     if (threadIdx.x == 0) s_nmin = 0x7f800000u;
     __syncthreads();
-    const int tile = blockIdx.x, x0 = (tile % tiles_x) * DET_TW, y0 = (tile / tiles_x) * DET_TH, tid = threadIdx.x;
+    const int x0 = (tile % tiles_x) * DET_TW, y0 = (tile / tiles_x) * DET_TH, tid = threadIdx.x;
     int pgx;
     float tdummy;
     det_node(x0 - 1, g, g.GX, pgx, tdummy);
@@ -437,28 +522,253 @@ __global__ void __launch_bounds__(256, 8) det_tiles_kernel(FrameArgs f, int W, i
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
         if (!((bits >> j) & 1u)) continue;
-        float flux = 0.f, mx = 0.f, my = 0.f;
+        float q[9];
 #pragma unroll
         for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const float q = row[j + (r - 1) * DET_PITCH + (c - 1)];
-                if (q != ninf) { flux += q; mx += q * (float)(c - 1); my += q * (float)(r - 1); }
-            }
+            for (int c = 0; c < 3; ++c) q[3 * r + c] = row[j + (r - 1) * DET_PITCH + (c - 1)];
         const float2 ci = s_col[cx0 + j + 1];
         const int lx = __float_as_int(ci.x) & 0xff, lx1 = __float_as_int(ci.x) >> 8;
         const float b0 = s_rb[ry + 1][lx], n0 = s_rn[ry + 1][lx];
-        ArgusSourceRec rec;
-        rec.x = x0 + cx0 + j; rec.y = py;
-        rec.peak = row[j]; rec.flux = flux;
-        rec.cx = flux > 0.f ? mx / flux : 0.f;
-        rec.cy = flux > 0.f ? my / flux : 0.f;
-        rec.bkg = fmaf(ci.y, s_rb[ry + 1][lx1] - b0, b0);
-        rec.nse = fmaf(ci.y, s_rn[ry + 1][lx1] - n0, n0);
+        if (pos < capacity)
+            det_write_record(tmp + pos, x0 + cx0 + j, py, q, fmaf(ci.y, s_rb[ry + 1][lx1] - b0, b0),
+                             fmaf(ci.y, s_rn[ry + 1][lx1] - n0, n0));
+        ++pos;
+    }
+}
+
+template <bool FUSED>
+__global__ void __launch_bounds__(256, 8) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
+                                                           ArgusSourceRec* __restrict__ tmp, unsigned capacity,
+                                                           uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
+    det_tile_body<FUSED>((int)blockIdx.x, f, W, H, g, tiles_x, tmp, capacity, tile_info, total);
+}
+
+// The same on a list of tiles (the tiles det_cand_kernel hands over): CTAs stride over list[0 .. *n_list).
+template <bool FUSED>
+__global__ void __launch_bounds__(256, 8) det_tiles_list_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
+                                                                ArgusSourceRec* __restrict__ tmp, unsigned capacity,
+                                                                uint2* __restrict__ tile_info, unsigned* __restrict__ total,
+                                                                const unsigned* __restrict__ list, const unsigned* __restrict__ n_list) {
+    const unsigned n = *n_list;
+    for (unsigned i = blockIdx.x; i < n; i += gridDim.x) {
+        __syncthreads();                              // the previous tile's shared tables are still being read
+        det_tile_body<FUSED>((int)list[i], f, W, H, g, tiles_x, tmp, capacity, tile_info, total);
+    }
+}
+
+// ---- candidate path of argus_detect_frame.  s and the maps at one pixel, with the arithmetic of det_tile_body: the grids are
+// interpolated along y first (fmaf(ty, b1 - b0, b0) per node column), then along x.
+struct DetAt {
+    int q00, q01, q10, q11;
+    float tx, ty;
+};
+__device__ __forceinline__ DetAt det_at(const DetGrid& g, int x, int y) {
+    DetAt a;
+    int gx0, gy0;
+    det_node(x, g, g.GX, gx0, a.tx);
+    det_node(y, g, g.GY, gy0, a.ty);
+    const int c1 = min(gx0 + 1, g.GX - 1), r1 = min(gy0 + 1, g.GY - 1);
+    a.q00 = gy0 * g.GX + gx0; a.q01 = gy0 * g.GX + c1; a.q10 = r1 * g.GX + gx0; a.q11 = r1 * g.GX + c1;
+    return a;
+}
+__device__ __forceinline__ float det_lerp(const float* __restrict__ grid, const DetAt& a) {
+    const float v00 = __ldg(grid + a.q00), v01 = __ldg(grid + a.q01), v10 = __ldg(grid + a.q10), v11 = __ldg(grid + a.q11);
+    const float r0 = fmaf(a.ty, v10 - v00, v00), r1 = fmaf(a.ty, v11 - v01, v01);
+    return fmaf(a.tx, r1 - r0, r0);
+}
+// MODE 0: cal + mask, 1: raw + masters, 2: raw + pre-fused masters.  Pixel at element offset o (clamped into the frame by
+// the caller, `in` = the pixel lies in the frame): no branch on the data, so that the loads of a 3 x 3 window are issued
+// together; the values are those of load_px.
+template <int MODE>
+__device__ __forceinline__ float det_px(const FrameArgs& f, size_t o, bool in) {
+    float v;
+    if (MODE == 2) {
+        const int r = f.raw[o];
+        v = calib_pre<false>((float)r, pre_load(f.offset, o, f.pre), pre_load(f.gain, o, f.pre), r >= f.sat_adu);
+    } else if (MODE == 1) {
+        const int r = f.raw[o];
+        const float b = f.bias[o], d = f.dark[o], fl = f.flat[o];
+        const bool bad = (r >= f.sat_adu) || (f.bpm && f.bpm[o] != 0);
+        v = calib_px((float)r, b, d, fl, bad, f.t_exp, f.flat_min);
+    } else {
+        const float c = f.cal[o];
+        v = f.mask[o] ? c : nanf_();
+    }
+    return in ? v : nanf_();
+}
+
+// One tile's candidates in one warp: R-D4 with the decisions of det_tile_body (threshold, then the 8 neighbours), records of
+// the sources staged in shared memory (rec: DET_CAND_CAP x 2 uint4 of this warp).  Returns the lane's flags: bit it = its
+// candidate it * 32 + lane is a source.  The node and fraction of the three columns and rows of the window are formed once.
+template <int MODE>
+__device__ __forceinline__ unsigned det_cand_tile(const FrameArgs& f, int W, int H, const DetGrid& g, int x0, int y0, unsigned cnt,
+                                                  const unsigned short* mine, uint4* rec, int lane) {
+    const float ninf = __int_as_float(0xff800000);
+    unsigned flags = 0;
+    for (unsigned it = 0; it * 32 < cnt; ++it) {
+        const unsigned i = it * 32 + lane;
+        if (i >= cnt) break;
+        const int loc = mine[i], x = x0 + (loc & (DET_TW - 1)), y = y0 + (loc >> 6);
+        int gx0[3], gx1[3], gy0[3], gy1[3], xs[3];
+        float tx[3], ty[3];
+        size_t ro[3];
+        bool inx[3], iny[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int xx = x + k - 1, yy = y + k - 1, yc = min(max(yy, 0), H - 1);
+            inx[k] = (unsigned)xx < (unsigned)W; iny[k] = (unsigned)yy < (unsigned)H;
+            xs[k] = min(max(xx, 0), W - 1);
+            det_node(xs[k], g, g.GX, gx0[k], tx[k]);
+            det_node(yc, g, g.GY, gy0[k], ty[k]);
+            gx1[k] = min(gx0[k] + 1, g.GX - 1);
+            gy1[k] = min(gy0[k] + 1, g.GY - 1) * g.GX;
+            gy0[k] *= g.GX;
+            ro[k] = (size_t)yc * W;
+        }
+        DetAt a;
+        a.q00 = gy0[1] + gx0[1]; a.q01 = gy0[1] + gx1[1]; a.q10 = gy1[1] + gx0[1]; a.q11 = gy1[1] + gx1[1];
+        a.tx = tx[1]; a.ty = ty[1];
+        const float v = det_px<MODE>(f, ro[1] + xs[1], true);
+        const float bkg = det_lerp(g.bkg, a), nse = det_lerp(g.nse, a);
+        const float c = (v == v) ? v - bkg : ninf;
+        if (!(c > 0.f && c > g.k_sigma * nse)) continue;   // false for nse = +inf or NaN (undefined background)
+        float q[9];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+                if (r == 1 && cc == 1) { q[4] = c; continue; }
+                DetAt b;
+                b.q00 = gy0[r] + gx0[cc]; b.q01 = gy0[r] + gx1[cc]; b.q10 = gy1[r] + gx0[cc]; b.q11 = gy1[r] + gx1[cc];
+                b.tx = tx[cc]; b.ty = ty[r];
+                const float vn = det_px<MODE>(f, ro[r] + xs[cc], inx[cc] && iny[r]);
+                const float sn = vn - det_lerp(g.bkg, b);
+                q[3 * r + cc] = (vn == vn) ? sn : ninf;
+            }
+        const float e4 = fmaxf(fmaxf(q[0], q[1]), fmaxf(q[2], q[3])), l4 = fmaxf(fmaxf(q[5], q[6]), fmaxf(q[7], q[8]));
+        if (c > e4 && c >= l4) {                          // raster-first pixel wins ties
+            flags |= 1u << it;
+            det_write_record(reinterpret_cast<ArgusSourceRec*>(rec + 2 * i), x, y, q, bkg, nse);
+        }
+    }
+    return flags;
+}
+
+// One warp per tile.  (1) Proof that the candidates are complete: every threshold bkg(p) + k nse(p) in the tile is a convex
+// combination of bkg_g + k nse_g over the nodes g the tile touches, so a pixel that passes has v >= L - rounding with
+// L = min_g (bkg_g + k nse_g); if L - slack >= max cut over the cells the tile overlaps, every such pixel was recorded by
+// bg_cells_kernel (v > cut).  Otherwise, or when the list overflowed, the tile goes to fb_list (det_tiles_list_kernel).
+// (2) R-D4 on the candidates with the decisions of det_tile_body (threshold, then the 8 neighbours), (3) records.
+#ifndef DET_CAND_MINB
+#define DET_CAND_MINB 4
+#endif
+template <bool FUSED>
+__global__ void __launch_bounds__(256, DET_CAND_MINB) det_cand_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x, int n_tiles,
+                                                       const unsigned* __restrict__ cand_cnt,
+                                                       const unsigned short* __restrict__ cand_list, const float* __restrict__ cut,
+                                                       ArgusSourceRec* __restrict__ tmp, unsigned capacity,
+                                                       uint2* __restrict__ tile_info, unsigned* __restrict__ total,
+                                                       unsigned* __restrict__ fb_list, unsigned* __restrict__ fb_count) {
+    const int lane = threadIdx.x & 31, tile = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (tile >= n_tiles) return;
+    const float inf = __int_as_float(0x7f800000);
+    const int x0 = (tile % tiles_x) * DET_TW, y0 = (tile / tiles_x) * DET_TH;
+    const int x1 = min(x0 + DET_TW, W) - 1, y1 = min(y0 + DET_TH, H) - 1;
+    // Every load of this phase is issued before the first use: the counts and (speculatively) all entries of the candidate
+    // lists of the cells the tile overlaps (one cell per lane, at most 32 cells of 8 pixels; <= 128 entries), the nodes and
+    // the cuts of the proof.
+    const int lb = 31 - __clz(g.B);                  // B is a power of two
+    const int cap = det_cand_cap(g.B), cxa = x0 >> lb, cw = (x1 >> lb) - cxa + 1, cya = y0 >> lb, nc = cw * ((y1 >> lb) - cya + 1);
+    const int hsel = (y0 / DET_TH) & 1;
+    // e / d for e < 2^10 and d <= 48 as (e * m) >> 16, m = 2^16 / d + 1 (exact there)
+    const unsigned m_cap = 65536u / (unsigned)cap + 1u, m_cw = 65536u / (unsigned)cw + 1u;
+    unsigned n_l = 0;
+    float M = -inf;
+    if (lane < nc) {
+        const int r = (int)(((unsigned)lane * m_cw) >> 16), cell = (cya + r) * g.GX + cxa + (lane - r * cw);
+        n_l = cand_cnt[(g.B == 64) ? 2 * (size_t)cell + hsel : (size_t)cell];
+        M = __ldg(cut + cell);
+    }
+    unsigned short slot[4];
+#pragma unroll
+    for (int sidx = 0; sidx < 4; ++sidx) {
+        const int e = lane + 32 * sidx, ci = (int)(((unsigned)e * m_cap) >> 16), j = e - ci * cap;
+        slot[sidx] = 0;
+        if (ci < nc) {
+            const int r = (int)(((unsigned)ci * m_cw) >> 16), cell = (cya + r) * g.GX + cxa + (ci - r * cw);
+            slot[sidx] = cand_list[((g.B == 64) ? 2 * (size_t)cell + hsel : (size_t)cell) * cap + j];
+        }
+    }
+    int gxa, gxb, gya, gyb;
+    float t;
+    det_node(x0, g, g.GX, gxa, t); det_node(x1, g, g.GX, gxb, t);
+    det_node(y0, g, g.GY, gya, t); det_node(y1, g, g.GY, gyb, t);
+    gxb = min(gxb + 1, g.GX - 1); gyb = min(gyb + 1, g.GY - 1);
+    const int nw = gxb - gxa + 1, nn = nw * (gyb - gya + 1);
+    const unsigned m_nw = 65536u / (unsigned)nw + 1u;
+    float L = inf, A = 0.f;
+    for (int e = lane; e < nn; e += 32) {
+        const int r = (int)(((unsigned)e * m_nw) >> 16), q = (gya + r) * g.GX + gxa + (e - r * nw);
+        const float n = __ldg(g.nse + q), b = __ldg(g.bkg + q);
+        if (n < inf) { L = fminf(L, fmaf(g.k_sigma, n, b)); A = fmaxf(A, fmaf(g.k_sigma, n, fabsf(b))); }
+    }
+    unsigned off = n_l;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned o = __shfl_up_sync(0xffffffffu, off, d);
+        if (lane >= d) off += o;
+    }
+    const unsigned cnt = __shfl_sync(0xffffffffu, off, 31);
+    off -= n_l;
+#pragma unroll
+    for (int d = 16; d; d >>= 1) {
+        L = fminf(L, __shfl_xor_sync(0xffffffffu, L, d));
+        A = fmaxf(A, __shfl_xor_sync(0xffffffffu, A, d));
+        M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, d));
+    }
+    // L = +inf: no defined noise node, nothing can be a source; M = -inf: every good pixel is a candidate
+    const bool complete = cnt <= DET_CAND_CAP && !__any_sync(0xffffffffu, n_l > (unsigned)cap) &&
+                          ((L == inf) || (M == -inf) || (L - 4e-6f * (A + fabsf(M)) - 1e-30f >= M));
+    if (!complete) {
+        if (lane == 0) fb_list[atomicAdd(fb_count, 1u)] = (unsigned)tile;
+        return;
+    }
+    __shared__ uint4 s_rec[8][2 * DET_CAND_CAP];
+    __shared__ unsigned short s_list[8][DET_CAND_CAP];
+    uint4* rec = s_rec[threadIdx.x >> 5];
+    unsigned short* mine = s_list[threadIdx.x >> 5];
+#pragma unroll
+    for (int sidx = 0; sidx < 4; ++sidx) {
+        const int e = lane + 32 * sidx, ci = (int)(((unsigned)e * m_cap) >> 16), j = e - ci * cap;
+        const unsigned n_c = __shfl_sync(0xffffffffu, n_l, ci & 31), off_c = __shfl_sync(0xffffffffu, off, ci & 31);
+        if (ci < nc && (unsigned)j < n_c) mine[off_c + j] = slot[sidx];
+    }
+    __syncwarp();
+    const unsigned flags = !FUSED ? det_cand_tile<0>(f, W, H, g, x0, y0, cnt, mine, rec, lane)
+                           : f.pre ? det_cand_tile<2>(f, W, H, g, x0, y0, cnt, mine, rec, lane)
+                                   : det_cand_tile<1>(f, W, H, g, x0, y0, cnt, mine, rec, lane);
+    const int my_n = __popc(flags);
+    int inc = my_n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += o;
+    }
+    const int tile_cnt = __shfl_sync(0xffffffffu, inc, 31);
+    unsigned base = 0;
+    if (lane == 0) {
+        base = tile_cnt ? atomicAdd(total, (unsigned)tile_cnt) : 0u;
+        tile_info[tile] = make_uint2(base, (unsigned)tile_cnt);
+    }
+    base = __shfl_sync(0xffffffffu, base, 0);
+    unsigned pos = base + (unsigned)(inc - my_n);
+    for (unsigned it = 0; flags >> it; ++it) {
+        if (!((flags >> it) & 1u)) continue;
         if (pos < capacity) {
             uint4* dst = reinterpret_cast<uint4*>(tmp + pos);
-            dst[0] = make_uint4((unsigned)rec.x, (unsigned)rec.y, __float_as_uint(rec.peak), __float_as_uint(rec.flux));
-            dst[1] = make_uint4(__float_as_uint(rec.cx), __float_as_uint(rec.cy), __float_as_uint(rec.bkg), __float_as_uint(rec.nse));
+            dst[0] = rec[2 * (it * 32 + lane)];
+            dst[1] = rec[2 * (it * 32 + lane) + 1];
         }
         ++pos;
     }

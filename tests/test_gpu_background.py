@@ -65,6 +65,28 @@ def gpu_detect(argus, ctx, W, H, B, k, bkg_dev, nse_dev, frame, cap=200000):
     return out.cpu().numpy()[:n * 32].view(argus.SOURCE_DTYPE)
 
 
+def check_detect_frame(argus, ctx, W, H, B, n_min, k, frame, g, rec, cap=200000, expect_full=None):
+    """argus_detect_frame (one call, the frame read once, detection from per-tile candidate lists) must give exactly what
+    argus_background_map + argus_detect_sources gave: both grids and the catalogue, bit for bit and in the same order.
+    Returns the number of tiles it scanned in full."""
+    GY, GX = _grid(W, H, B)
+    bkg = torch.full((GY * GX,), float("nan"), dtype=torch.float32, device=DEV)
+    nse = torch.full((GY * GX,), float("nan"), dtype=torch.float32, device=DEV)
+    out = torch.zeros((cap * 32,), dtype=torch.uint8, device=DEV)
+    n_dev = torch.full((1,), -1, dtype=torch.int64, device=DEV)
+    n = argus.argus_detect_frame(ctx, W, H, bkg, nse, out, cell=B, n_min=n_min, k_sigma=k, n_dev=n_dev, **frame)
+    assert int(n_dev.item()) == n == rec.size
+    assert np.array_equal(bkg.cpu().numpy().view(np.uint32), g["bkg"].reshape(-1).view(np.uint32))
+    assert np.array_equal(nse.cpu().numpy().view(np.uint32), g["nse"].reshape(-1).view(np.uint32))
+    assert out.cpu().numpy()[:n * 32].tobytes() == rec.tobytes(), "catalogue of argus_detect_frame differs"
+    n_full = argus.argus_detect_frame_info(ctx)
+    n_tiles = -(-W // 64) * -(-H // 32)
+    assert 0 <= n_full <= n_tiles
+    if expect_full is not None:
+        assert (n_full == n_tiles) if expect_full else (n_full < n_tiles), "%d of %d tiles scanned in full" % (n_full, n_tiles)
+    return n_full
+
+
 def tol(v):
     return VALUE_ATOL + VALUE_RTOL * np.abs(v)
 
@@ -138,6 +160,7 @@ def test_config0_calibrated_frame_is_bit_exact(argus, ctx, B, n_min):
     rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
     n_must, _ = compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0)
     assert n_must > 50          # config 0 plants 300 stars
+    check_detect_frame(argus, ctx, W, H, B, n_min, 5.0, _dev_cal(cal32, mask), g, rec, expect_full=False)
 
 
 @pytest.mark.parametrize("B", [64, 16])
@@ -160,6 +183,7 @@ def test_config0_fused_calibration(argus, ctx, B):
         assert np.array_equal(g[k], g2[k]), k
     rec2 = gpu_detect(argus, ctx, W, H, B, 5.0, g2["dev"]["bkg"], g2["dev"]["nse"], dict(cal=calg, mask=maskg))
     assert rec.tobytes() == rec2.tobytes()
+    check_detect_frame(argus, ctx, W, H, B, 16, 5.0, d, g, rec, expect_full=False)
 
 
 @pytest.mark.parametrize("W,H,B", [(500, 391, 64), (333, 130, 32), (70, 45, 16), (64, 32, 64), (5, 3, 8)])
@@ -177,6 +201,10 @@ def test_ragged_shapes_defects_and_unaligned_rows(argus, ctx, W, H, B):
     bkg, nse = compare_grids(g, cal32.astype(np.float64), mask, B, n_min, exact=True)
     rec = gpu_detect(argus, ctx, W, H, B, 4.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
     compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 4.0, max_ambiguous=6)
+    check_detect_frame(argus, ctx, W, H, B, n_min, 4.0, _dev_cal(cal32, mask), g, rec)
+    # a threshold below the candidate cut (kappa = 2.5): the proof fails everywhere, every tile is scanned in full
+    rec_low = gpu_detect(argus, ctx, W, H, B, 1.5, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
+    check_detect_frame(argus, ctx, W, H, B, n_min, 1.5, _dev_cal(cal32, mask), g, rec_low, expect_full=True if W > 100 else None)
 
 
 def test_hand_built_sources_and_capacity(argus, ctx):
@@ -191,6 +219,7 @@ def test_hand_built_sources_and_capacity(argus, ctx):
     assert list(zip(rec["y"].tolist(), rec["x"].tolist())) == [(10, 20), (20, 8), (30, 40), (40, 50)]
     assert rec["peak"].tolist() == [100, 30, 50, 80] and rec["flux"].tolist() == [100, 60, 100, 100]
     assert rec["cx"].tolist() == [0, 0, 0.5, pytest.approx(0.2)] and rec["cy"].tolist() == [0, 0.5, 0, 0]
+    check_detect_frame(argus, ctx, W, H, B, 16, 5.0, fr, g, rec, cap=16)
     # count only, then too small a capacity: the count is reported with ARGUS_ERR_CAPACITY
     assert argus.argus_detect_sources(ctx, W, H, g["dev"]["bkg"], g["dev"]["nse"], None, cell=B, **fr) == 4
     small = torch.zeros((2 * 32,), dtype=torch.uint8, device=DEV)
@@ -210,6 +239,7 @@ def test_undefined_background_suppresses_detection(argus, ctx):
     assert np.isinf(g["nse"][:, 3]).all() and np.isfinite(g["nse"][:, :3]).all() and np.all(g["bkg"][:, 3] == 0)
     rec = gpu_detect(argus, ctx, 64, 32, 16, 5.0, g["dev"]["bkg"], g["dev"]["nse"], fr)
     assert list(zip(rec["y"].tolist(), rec["x"].tolist())) == [(8, 8)]
+    check_detect_frame(argus, ctx, 64, 32, 16, 16, 5.0, fr, g, rec)
 
 
 def test_config1_full_frame_fused(argus, ctx):
@@ -225,6 +255,9 @@ def test_config1_full_frame_fused(argus, ctx):
     n_must, n_amb = compare_catalogue(rec, cal, mask, bkg, nse, W, 64, 5.0, max_ambiguous=17)   # measured: 14 of 32 749 (+ 20 %)
     print("config1 detect: %d records, %d clear sources, %d ambiguous decisions" % (rec.size, n_must, n_amb))
     assert n_must > 20000
+    n_full = check_detect_frame(argus, ctx, W, H, 64, 16, 5.0, d, g, rec, cap=1 << 18)
+    print("config1 argus_detect_frame: %d of %d tiles scanned in full" % (n_full, -(-W // 64) * -(-H // 32)))
+    assert n_full < 0.1 * (-(-W // 64) * -(-H // 32))
 
 
 @pytest.mark.parametrize("B", [64, 8])
@@ -244,3 +277,4 @@ def test_mixed_sign_values_zeros_and_duplicates(argus, ctx, B):
     rec = gpu_detect(argus, ctx, W, H, B, 5.0, g["dev"]["bkg"], g["dev"]["nse"], _dev_cal(cal32, mask))
     n_must, n_amb = compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0)   # measured: 0 ambiguous (default bound 3)
     print("mixed-sign B=%d: %d records, %d clear sources, %d ambiguous decisions" % (B, rec.size, n_must, n_amb))
+    check_detect_frame(argus, ctx, W, H, B, 4, 5.0, _dev_cal(cal32, mask), g, rec)
