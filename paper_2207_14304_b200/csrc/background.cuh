@@ -23,6 +23,7 @@
 #define BG_KPT 16                    // keys per thread: 256 x 16 = 4096 = 64 x 64
 #define BG_SENTINEL 0xffffffffu      // masked / outside the cell: sorts after every value
 #define BG_FINISH 32                 // rank the survivors directly once this few remain
+#define BG_SAMPLE_MIN 24             // valid keys among the 64 sampled below which no range is guessed
 #define BG_MAD_TO_SIGMA 1.4826f
 
 struct ArgusSourceRec {              // == argus_source (argus.h)
@@ -31,11 +32,21 @@ struct ArgusSourceRec {              // == argus_source (argus.h)
 };
 
 __device__ __forceinline__ unsigned bg_key(float v) {
-    unsigned u = __float_as_uint(v);
-    return (v != v) ? BG_SENTINEL : ((u & 0x80000000u) ? ~u : (u | 0x80000000u));
+    const unsigned u = __float_as_uint(v);
+    // negative: all bits flipped, else the sign bit set
+    return (v != v) ? BG_SENTINEL : (u ^ ((unsigned)((int)u >> 31) | 0x80000000u));
 }
 __device__ __forceinline__ float bg_unkey(unsigned k) {
     return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k);
+}
+// ++hist[bin] when d <= span.  Written without a branch: keys outside the range count into the spare word BG_HIST_SPARE
+// (never read), which the hardware folds into one increment per warp (ATOMS.POPC.INC); the compiler's form of
+// `if (d <= span) atomicAdd(...)` is a divergent region per key with the shared window address re-derived inside
+// (13 instructions per key instead of 6).  hist_s: shared-window address of the histogram.
+#define BG_HIST_SPARE 268
+__device__ __forceinline__ void bg_hist_add(unsigned hist_s, unsigned d, unsigned span, int sh) {
+    const unsigned bin = (d <= span) ? (d >> sh) : (unsigned)BG_HIST_SPARE;
+    asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(hist_s + (bin << 2)) : "memory");
 }
 
 // Four consecutive pixels starting at (x, y), x % 4 == 0: calibrated value, NaN where masked / outside [0, x_end).
@@ -106,27 +117,38 @@ __device__ __forceinline__ unsigned bg_block_max_valid(unsigned v, int* s_red, i
     return max(max(max(a.x, a.y), max(a.z, a.w)), max(max(b.x, b.y), max(b.z, b.w)));
 }
 
-// k-th smallest (0-based, k < n) of the n non-sentinel keys held by the CTA (BG_KPT per thread); kmin / kmax are
-// their extremes.  Multi-level counting select: the live key range [lo, hi] is cut into <= 256 equal bins (width a
-// power of two), the keys inside it are counted into a shared histogram, a CTA-wide scan finds the bin that holds
-// rank k, and that bin becomes the new range -- 8 bits per level, the first level starting at the common prefix
-// of kmin and kmax.  Once <= BG_FINISH keys remain they are ranked directly in one warp.  Exact.
-// s_hist: 256 + 12 words, s_list: BG_FINISH + 2 words, s_cnt: 1 word of shared memory.
-__device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned kmin, unsigned kmax,
-                                              int* s_hist, unsigned* s_list, int* s_cnt, unsigned& next, bool& have_next) {
-    unsigned lo = kmin, hi = kmax;
+// k-th smallest (0-based, k < n) of the n non-sentinel keys held by the CTA (BG_KPT per thread).
+// Multi-level counting select: the live key range [lo, hi] is cut into <= 256 equal bins (width a power of two), the keys
+// inside it are counted into a shared histogram, a CTA-wide scan finds the bin that holds rank k, and that bin becomes the
+// new range -- 8 bits per level.  Once <= BG_FINISH keys remain they are ranked directly in one warp.  Exact.
+// The first range is either [kmin, kmax], the extremes of the keys (GUESS = false: c_lo = 0, cnt = n), or a GUESS from a
+// sample (bg_sample_range): then the first level also counts the keys below the range, and the call returns false, with
+// nothing selected, when rank k lies outside it (the caller falls back to the extremes).
+// s_hist: 256 + 12 + 4 words, s_list: BG_FINISH + 2 words, s_cnt: 1 word of shared memory.
+template <bool GUESS>
+__device__ __forceinline__ bool bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned lo, unsigned hi,
+                                          int* s_hist, unsigned* s_list, int* s_cnt, unsigned& kth, unsigned& next, bool& have_next) {
     int c_lo = 0, cnt = n;                          // #{key < lo}, #{lo <= key <= hi}
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    int* s_w = s_hist + 256;                        // [0..7] warp totals, [8..10] picked bin, its prefix, its count
-    while (cnt > BG_FINISH && hi > lo) {
+    int* s_w = s_hist + 256;                        // [0..7] warp totals, [8..10] picked bin, its prefix, its count, [11] keys below
+    bool first = GUESS;
+    if (GUESS) __syncthreads();                     // s_w[8..11] of the previous select are still being read
+    while (first || (cnt > BG_FINISH && hi > lo)) {
         const int sh = max(0, 24 - __clz(hi - lo)); // (hi - lo) >> sh <= 255
         s_hist[tid] = 0;
+        if (first && tid < 4) s_w[8 + tid] = (tid == 0) ? -1 : 0;
         __syncthreads();
-        const unsigned span = hi - lo;
+        const unsigned span = hi - lo, hist_s = (unsigned)__cvta_generic_to_shared(s_hist);
+        int below = 0;
 #pragma unroll
         for (int i = 0; i < BG_KPT; ++i) {
             const unsigned d = key[i] - lo;             // wraps to a huge value below lo: one compare covers both ends
-            if (d <= span) atomicAdd(s_hist + (d >> sh), 1);
+            bg_hist_add(hist_s, d, span, sh);
+            if (GUESS) below += (key[i] < lo) ? 1 : 0;
+        }
+        if (first) {
+            below = __reduce_add_sync(0xffffffffu, below);
+            if (lane == 0 && below) atomicAdd(s_w + 11, below);
         }
         __syncthreads();
         const int h = s_hist[tid];
@@ -140,9 +162,12 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
         __syncthreads();
 #pragma unroll
         for (int w = 0; w < 7; ++w) inc += (w < wid) ? s_w[w] : 0;
+        if (first) c_lo = s_w[11];
         const int krel = k - c_lo;
         if (inc - h <= krel && krel < inc) { s_w[8] = tid; s_w[9] = inc - h; s_w[10] = h; }
         __syncthreads();
+        if (first && s_w[8] < 0) return false;        // rank k is not in the guessed range (uniform: every thread reads s_w[8])
+        first = false;
         const unsigned bin = (unsigned)s_w[8];
         c_lo += s_w[9];
         cnt = s_w[10];
@@ -151,7 +176,7 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
         hi = (top < lo) ? hi : min(hi, top);          // top < lo: wrapped past 2^32
     }
     // `next` = the key of rank k + 1 when it lies in the same final range (have_next), for the even-n median
-    if (hi == lo) { have_next = (k - c_lo + 1 < cnt); next = lo; return lo; }
+    if (hi == lo) { have_next = (k - c_lo + 1 < cnt); next = lo; kth = lo; return true; }
     // at most BG_FINISH keys remain in [lo, hi]: rank them directly (ties by list position)
     if (tid == 0) *s_cnt = 0;
     __syncthreads();
@@ -176,17 +201,30 @@ __device__ __forceinline__ unsigned bg_select(const unsigned (&key)[BG_KPT], int
     __syncthreads();
     have_next = (k - c_lo + 1 < m);
     next = s_list[BG_FINISH + 1];
-    return s_list[BG_FINISH];
+    kth = s_list[BG_FINISH];
+    return true;
 }
 
-// median rule of R-D1: (v_((n-1)/2) + v_(n/2)) / 2 as keys -> the two central keys.
-__device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], int n, unsigned kmin, unsigned kmax, int* s_red,
+// median rule of R-D1: (v_((n-1)/2) + v_(n/2)) / 2 as keys -> the two central keys.  [glo, ghi] (glo <= ghi): a guess of a
+// range that holds them (bg_sample_range); when it does not, or there is none (glo > ghi), the select starts from the
+// extremes of the keys, which are then found first.
+__device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], int n, unsigned glo, unsigned ghi, int* s_red,
                                                 int& par, int& it, int* s_hist, unsigned* s_list, int* s_cnt, unsigned& k1,
                                                 unsigned& k2) {
     const int r = (n - 1) >> 1;
     unsigned nxt_sel;
     bool have_next;
-    k1 = bg_select(key, r, n, kmin, kmax, s_hist, s_list, s_cnt, nxt_sel, have_next);
+    if (glo > ghi || !bg_select<true>(key, r, n, glo, ghi, s_hist, s_list, s_cnt, k1, nxt_sel, have_next)) {
+        unsigned lo = BG_SENTINEL, hi = 0u;
+#pragma unroll
+        for (int i = 0; i < BG_KPT; ++i) {
+            lo = min(lo, key[i]);
+            hi = max(hi, key[i] != BG_SENTINEL ? key[i] : 0u);
+        }
+        lo = bg_block_min(lo, s_red, par);
+        hi = bg_block_max_valid(hi, s_red, par);
+        bg_select<false>(key, r, n, lo, hi, s_hist, s_list, s_cnt, k1, nxt_sel, have_next);
+    }
     k2 = k1;
     if ((n & 1) == 0) {
         if (have_next) {                            // rank r + 1 fell into the same final range (the usual case)
@@ -204,6 +242,35 @@ __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], i
             if (r + 1 >= c) k2 = nxt;
         }
     }
+}
+
+// Sample quartiles: 64 of the cell's keys (one of every fourth thread) are ranked by two warps; q[0..2] = the sample's quartile keys, q[3] = number of valid samples (all threads).  They only steer
+// where the exact select starts.
+__device__ __forceinline__ void bg_sample_quartiles(const unsigned (&key)[BG_KPT], unsigned* s_samp, unsigned (&q)[4]) {
+    const int tid = threadIdx.x;
+    if ((tid & 3) == 0) {                           // column group c of the cell, row block c: a diagonal of 16 x 4 pixels
+        const int j = (tid >> 2) & 3;
+        s_samp[tid >> 2] = j == 0 ? key[1] : j == 1 ? key[5] : j == 2 ? key[9] : key[13];
+    }
+    if (tid < 4) s_samp[64 + tid] = 0u;
+    __syncthreads();
+    if (tid < 64) {
+        const unsigned mine = s_samp[tid];
+        int rank = 0, nv = 0;
+#pragma unroll
+        for (int j = 0; j < 64; j += 4) {
+            const uint4 o = *reinterpret_cast<const uint4*>(s_samp + j);
+            rank += (o.x < mine || (o.x == mine && j < tid)) + (o.y < mine || (o.y == mine && j + 1 < tid)) +
+                    (o.z < mine || (o.z == mine && j + 2 < tid)) + (o.w < mine || (o.w == mine && j + 3 < tid));
+            nv += (o.x != BG_SENTINEL) + (o.y != BG_SENTINEL) + (o.z != BG_SENTINEL) + (o.w != BG_SENTINEL);
+        }
+        if (rank == nv >> 2) s_samp[64] = mine;
+        if (rank == nv >> 1) s_samp[65] = mine;
+        if (rank == (3 * nv) >> 2) s_samp[66] = mine;
+        if (tid == 0) s_samp[67] = (unsigned)nv;
+    }
+    __syncthreads();
+    q[0] = s_samp[64]; q[1] = s_samp[65]; q[2] = s_samp[66]; q[3] = s_samp[67];
 }
 
 // Detection candidates of argus_detect_frame ("one pass"): while a cell's pixels are in registers,
@@ -254,8 +321,9 @@ __global__ void __launch_bounds__(BG_THREADS, BG_MINB) bg_cells_kernel(FrameArgs
                                                               int* __restrict__ ngood_out, BgCand cd) {
     __shared__ __align__(16) int s_red[20];
     __shared__ unsigned s_list[BG_FINISH + 2];
-    __shared__ int s_hist[256 + 12];
+    __shared__ int s_hist[256 + 12 + 4];
     __shared__ int s_cnt;
+    __shared__ __align__(16) unsigned s_samp[68];
     __shared__ BgCandShared s_cand;
     if (threadIdx.x < 3) s_red[16 + threadIdx.x] = 0;
     if (CAND && threadIdx.x < 2) s_cand.n[threadIdx.x] = 0u;
@@ -273,14 +341,8 @@ __global__ void __launch_bounds__(BG_THREADS, BG_MINB) bg_cells_kernel(FrameArgs
     }
     int par = 0, it = 0;
     int n = 0;
-    unsigned lo = BG_SENTINEL, hi = 0u;
 #pragma unroll
-    for (int i = 0; i < BG_KPT; ++i) {
-        const bool ok = key[i] != BG_SENTINEL;
-        n += ok ? 1 : 0;
-        lo = min(lo, key[i]);
-        hi = max(hi, ok ? key[i] : 0u);
-    }
+    for (int i = 0; i < BG_KPT; ++i) n += (key[i] != BG_SENTINEL) ? 1 : 0;
     n = bg_block_sum(n, s_red, par, it);
     if (n < max(n_min, 1)) {
         if (threadIdx.x == 0) { med_out[cell] = 0.f; sig_out[cell] = 0.f; ngood_out[cell] = n; }
@@ -298,24 +360,26 @@ __global__ void __launch_bounds__(BG_THREADS, BG_MINB) bg_cells_kernel(FrameArgs
         }
         return;
     }
-    lo = bg_block_min(lo, s_red, par);
-    hi = bg_block_max_valid(hi, s_red, par);
+    // where the selects start: [median - sigma, median + sigma] and 1.4826 MAD in [0.35, 1.35] sigma of a 64-key sample
+    // (the exact selects fall back to the extremes of the keys when the rank is not in there)
+    unsigned q[4];
+    bg_sample_quartiles(key, s_samp, q);
+    unsigned glo = 1u, ghi = 0u, dlo = 1u, dhi = 0u;  // lo > hi: no guess
+    if (q[3] >= BG_SAMPLE_MIN) {
+        const float m0 = bg_unkey(q[1]), s0 = 0.7413f * (bg_unkey(q[2]) - bg_unkey(q[0]));
+        if (s0 >= 0.f && s0 < __int_as_float(0x7f800000)) {
+            glo = bg_key(m0 - s0); ghi = bg_key(m0 + s0);
+            dlo = __float_as_uint(0.35f * 0.6745f * s0); dhi = __float_as_uint(1.35f * 0.6745f * s0);
+        }
+    }
     unsigned k1, k2;
-    bg_central_pair(key, n, lo, hi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
+    bg_central_pair(key, n, glo, ghi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
     const float med = 0.5f * (bg_unkey(k1) + bg_unkey(k2));
     // MAD: |v - med| >= 0, whose bit patterns are already ordered
-    lo = BG_SENTINEL; hi = 0u;
 #pragma unroll
-    for (int i = 0; i < BG_KPT; ++i) {
-        const bool ok = key[i] != BG_SENTINEL;
-        const unsigned d = ok ? __float_as_uint(fabsf(bg_unkey(key[i]) - med)) : BG_SENTINEL;
-        key[i] = d;
-        lo = min(lo, d);
-        hi = max(hi, ok ? d : 0u);
-    }
-    lo = bg_block_min(lo, s_red, par);
-    hi = bg_block_max_valid(hi, s_red, par);
-    bg_central_pair(key, n, lo, hi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
+    for (int i = 0; i < BG_KPT; ++i)
+        key[i] = (key[i] != BG_SENTINEL) ? __float_as_uint(fabsf(bg_unkey(key[i]) - med)) : BG_SENTINEL;
+    bg_central_pair(key, n, dlo, dhi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
     const float mad = 0.5f * (__uint_as_float(k1) + __uint_as_float(k2));
     if (threadIdx.x == 0) { med_out[cell] = med; sig_out[cell] = BG_MAD_TO_SIGMA * mad; ngood_out[cell] = n; }
     if (CAND) {
