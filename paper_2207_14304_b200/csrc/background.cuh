@@ -49,6 +49,11 @@ __device__ __forceinline__ void bg_hist_add(unsigned hist_s, unsigned d, unsigne
     asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(hist_s + (bin << 2)) : "memory");
 }
 
+// the scalar path of bg_load4 (ragged cells, unaligned frames): out of line, it is rare and sixteen inlined copies of it
+// spread the hot path of bg_cells_kernel over the instruction cache
+template <bool FUSED>
+__device__ __noinline__ float bg_load_slow(const FrameArgs f, int W, int H, int x, int y) { return load_px<FUSED>(f, W, H, x, y); }
+
 // Four consecutive pixels starting at (x, y), x % 4 == 0: calibrated value, NaN where masked / outside [0, x_end).
 template <bool FUSED>
 __device__ __forceinline__ void bg_load4(const FrameArgs& f, int W, int H, int x, int y, int x_end, float v[4]) {
@@ -79,7 +84,7 @@ __device__ __forceinline__ void bg_load4(const FrameArgs& f, int W, int H, int x
         }
     } else {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) v[i] = (x + i < x_end) ? load_px<FUSED>(f, W, H, x + i, y) : nanf_();
+        for (int i = 0; i < 4; ++i) v[i] = (x + i < x_end) ? bg_load_slow<FUSED>(f, W, H, x + i, y) : nanf_();
     }
 }
 
@@ -125,8 +130,7 @@ __device__ __forceinline__ unsigned bg_block_max_valid(unsigned v, int* s_red, i
 // sample (bg_sample_range): then the first level also counts the keys below the range, and the call returns false, with
 // nothing selected, when rank k lies outside it (the caller falls back to the extremes).
 // s_hist: 256 + 12 + 4 words, s_list: BG_FINISH + 2 words, s_cnt: 1 word of shared memory.
-template <bool GUESS>
-__device__ __forceinline__ bool bg_select(const unsigned (&key)[BG_KPT], int k, int n, unsigned lo, unsigned hi,
+__device__ __forceinline__ bool bg_select(const bool GUESS, const unsigned (&key)[BG_KPT], int k, int n, unsigned lo, unsigned hi,
                                           int* s_hist, unsigned* s_list, int* s_cnt, unsigned& kth, unsigned& next, bool& have_next) {
     int c_lo = 0, cnt = n;                          // #{key < lo}, #{lo <= key <= hi}
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -214,16 +218,23 @@ __device__ __forceinline__ void bg_central_pair(const unsigned (&key)[BG_KPT], i
     const int r = (n - 1) >> 1;
     unsigned nxt_sel;
     bool have_next;
-    if (glo > ghi || !bg_select<true>(key, r, n, glo, ghi, s_hist, s_list, s_cnt, k1, nxt_sel, have_next)) {
-        unsigned lo = BG_SENTINEL, hi = 0u;
+    // one copy of the select in the instruction stream (the kernel is instruction-fetch bound otherwise): a failed guess
+    // comes round again from the extremes
+    bool guess = glo <= ghi;
+#pragma unroll 1
+    for (;;) {
+        if (!guess) {
+            unsigned lo = BG_SENTINEL, hi = 0u;
 #pragma unroll
-        for (int i = 0; i < BG_KPT; ++i) {
-            lo = min(lo, key[i]);
-            hi = max(hi, key[i] != BG_SENTINEL ? key[i] : 0u);
+            for (int i = 0; i < BG_KPT; ++i) {
+                lo = min(lo, key[i]);
+                hi = max(hi, key[i] != BG_SENTINEL ? key[i] : 0u);
+            }
+            glo = bg_block_min(lo, s_red, par);
+            ghi = bg_block_max_valid(hi, s_red, par);
         }
-        lo = bg_block_min(lo, s_red, par);
-        hi = bg_block_max_valid(hi, s_red, par);
-        bg_select<false>(key, r, n, lo, hi, s_hist, s_list, s_cnt, k1, nxt_sel, have_next);
+        if (bg_select(guess, key, r, n, glo, ghi, s_hist, s_list, s_cnt, k1, nxt_sel, have_next)) break;
+        guess = false;
     }
     k2 = k1;
     if ((n & 1) == 0) {
@@ -373,13 +384,18 @@ __global__ void __launch_bounds__(BG_THREADS, BG_MINB) bg_cells_kernel(FrameArgs
         }
     }
     unsigned k1, k2;
-    bg_central_pair(key, n, glo, ghi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
-    const float med = 0.5f * (bg_unkey(k1) + bg_unkey(k2));
-    // MAD: |v - med| >= 0, whose bit patterns are already ordered
+    float med = 0.f;
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {           // median of the values, then of |v - med| (one copy of the code)
+        bg_central_pair(key, n, pass ? dlo : glo, pass ? dhi : ghi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
+        if (pass == 0) {
+            med = 0.5f * (bg_unkey(k1) + bg_unkey(k2));
+            // MAD: |v - med| >= 0, whose bit patterns are already ordered
 #pragma unroll
-    for (int i = 0; i < BG_KPT; ++i)
-        key[i] = (key[i] != BG_SENTINEL) ? __float_as_uint(fabsf(bg_unkey(key[i]) - med)) : BG_SENTINEL;
-    bg_central_pair(key, n, dlo, dhi, s_red, par, it, s_hist, s_list, &s_cnt, k1, k2);
+            for (int i = 0; i < BG_KPT; ++i)
+                key[i] = (key[i] != BG_SENTINEL) ? __float_as_uint(fabsf(bg_unkey(key[i]) - med)) : BG_SENTINEL;
+        }
+    }
     const float mad = 0.5f * (__uint_as_float(k1) + __uint_as_float(k2));
     if (threadIdx.x == 0) { med_out[cell] = med; sig_out[cell] = BG_MAD_TO_SIGMA * mad; ngood_out[cell] = n; }
     if (CAND) {
