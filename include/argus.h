@@ -346,7 +346,7 @@ typedef struct argus_source {
  *   n_out     HOST (may be NULL): when given the call synchronises the stream and stores the number found; if that
  *             exceeds a non-zero capacity the call returns ARGUS_ERR_CAPACITY, the contents of out are unspecified
  *             (nothing is written beyond capacity) and *n_out is the capacity to call again with.
- * capacity = 0 only counts.  Scratch: 12 bytes per 64 x 32-pixel work tile + 40 bytes per record of capacity, grown on demand (which
+ * capacity = 0 only counts.  Scratch: 16 bytes per 64 x 32-pixel work tile + 40 bytes per record of capacity, grown on demand (which
  * synchronises the device).  Otherwise asynchronous on stream. */
 int argus_detect_sources(argus_ctx* ctx, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, const float* bkg,
                          const float* nse, float k_sigma, argus_source* out, size_t capacity, int64_t* n_dev,
@@ -360,7 +360,7 @@ int argus_detect_sources(argus_ctx* ctx, const argus_frame* frame, int64_t W, in
  * (bkg + k_sigma * nse) lies above the cuts of the cells it overlaps (then no other pixel can pass the threshold); the
  * other tiles, and tiles with more than 48 candidates, are scanned in full as argus_detect_sources does.
  * bkg_out, nse_out (DEVICE, GX * GY floats, required), out / capacity / n_dev / n_out / error behaviour: exactly the
- * results of the two calls, bit for bit, catalogue order included.  Scratch: 12 + 4 bytes per cell, 116 bytes per
+ * results of the two calls, bit for bit, catalogue order included.  Scratch: 12 + 4 bytes per cell, 120 bytes per
  * tile, 40 bytes per record of capacity, grown on demand (which synchronises the device); otherwise asynchronous. */
 int argus_detect_frame(argus_ctx* ctx, const argus_frame* frame, int64_t W, int64_t H, int32_t cell, int32_t n_min,
                        float k_sigma, float* bkg_out, float* nse_out, argus_source* out, size_t capacity, int64_t* n_dev,

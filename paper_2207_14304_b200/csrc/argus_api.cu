@@ -1591,7 +1591,7 @@ static int det_ensure_scratch(argus_ctx* c, int64_t n_tiles, size_t capacity) {
     if (c->bg.cap_tiles < (size_t)n_tiles || !c->bg.tiles) {
         if (c->bg.tiles) { CUDA_TRY(c, cudaDeviceSynchronize()); cudaFree(c->bg.tiles); c->bg.tiles = nullptr; }
         size_t want = align_up((size_t)n_tiles, 4096);
-        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tiles, want * 12));
+        CUDA_TRY(c, cudaMalloc((void**)&c->bg.tiles, want * 16));   // tile_info (8 B) | offsets (4 B) | per-band counts (<= one per tile)
         c->bg.cap_tiles = want;
     }
     if (c->bg.cap_tmp < capacity || !c->bg.tmp) {
@@ -1612,24 +1612,31 @@ static DetGrid det_grid(const float* bkg, const float* nse, int64_t W, int64_t H
     return g;
 }
 
-// Tile counts -> offsets, records -> catalogue order, count to the caller (R-D6; shared by both detection entry points).
+// Records -> catalogue order (R-D6), count to the caller (shared by both detection entry points).
 static int det_finish(argus_ctx* c, int64_t n_tiles, int64_t tiles_x, int64_t tiles_y, int64_t W, argus_source* out,
                       size_t capacity, int64_t* n_dev, size_t* n_out, cudaStream_t st) {
     unsigned* offsets = (unsigned*)(c->bg.tiles + c->bg.cap_tiles);
-    det_scan_kernel<<<1, 1024, 0, st>>>(c->bg.tiles, (int)n_tiles, offsets, c->bg.ctl, (long long*)n_dev);
+    if (capacity > 0)
+        det_order_kernel<<<(unsigned)tiles_y, 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, (int)tiles_x, (int)W, offsets + c->bg.cap_tiles,
+                                                           c->bg.tmp, c->bg.ord, (ArgusSourceRec*)out, (unsigned)capacity, (long long*)n_dev);
+    else
+        det_count_kernel<<<1, 1, 0, st>>>(c->bg.ctl, (long long*)n_dev);
     c->n_launches++;
-    if (capacity > 0) {
-        det_order_kernel<<<(unsigned)tiles_y, 256, 0, st>>>(c->bg.tiles, offsets, (int)n_tiles, (int)tiles_x, (int)W, c->bg.ctl,
-                                                           c->bg.tmp, c->bg.ord, (ArgusSourceRec*)out, (unsigned)capacity);
-        c->n_launches++;
-    }
     CUDA_TRY(c, cudaGetLastError());
     if (n_out) {
         CUDA_TRY(c, cudaMemcpyAsync(c->bg.h_n, c->bg.ctl, 8, cudaMemcpyDeviceToHost, st));
         CUDA_TRY(c, cudaStreamSynchronize(st));
-        *n_out = (size_t)(((unsigned long long)*c->bg.h_n) >> 32);     // ctl[1]
+        *n_out = (size_t)(((unsigned long long)*c->bg.h_n) & 0xffffffffull);     // ctl[0]: the running total of the tile kernels
         if (capacity > 0 && *n_out > capacity) return ARGUS_ERR_CAPACITY;
     }
+    return ARGUS_OK;
+}
+
+// ctl and the per-band counts start at zero
+static int det_clear(argus_ctx* c, int64_t tiles_y, cudaStream_t st) {
+    unsigned* band_cnt = (unsigned*)(c->bg.tiles + c->bg.cap_tiles) + c->bg.cap_tiles;
+    CUDA_TRY(c, cudaMemsetAsync(c->bg.ctl, 0, 16, st));
+    CUDA_TRY(c, cudaMemsetAsync(band_cnt, 0, (size_t)tiles_y * 4, st));
     return ARGUS_OK;
 }
 
@@ -1653,13 +1660,15 @@ extern "C" int argus_detect_sources(argus_ctx* c, const argus_frame* frame, int6
     rc = det_ensure_scratch(c, n_tiles, capacity);
     if (rc) return rc;
     const DetGrid g = det_grid(bkg, nse, W, H, cell, k_sigma);
-    CUDA_TRY(c, cudaMemsetAsync(c->bg.ctl, 0, 16, st));
+    rc = det_clear(c, tiles_y, st);
+    if (rc) return rc;
+    unsigned* band_cnt = (unsigned*)(c->bg.tiles + c->bg.cap_tiles) + c->bg.cap_tiles;
     if (fused)
         det_tiles_kernel<true><<<(unsigned)n_tiles, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity,
-                                                               c->bg.tiles, c->bg.ctl);
+                                                               c->bg.tiles, c->bg.ctl, band_cnt);
     else
         det_tiles_kernel<false><<<(unsigned)n_tiles, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity,
-                                                                c->bg.tiles, c->bg.ctl);
+                                                                c->bg.tiles, c->bg.ctl, band_cnt);
     c->n_launches++;
     return det_finish(c, n_tiles, tiles_x, tiles_y, W, out, capacity, n_dev, n_out, st);
 }
@@ -1713,7 +1722,9 @@ extern "C" int argus_detect_frame(argus_ctx* c, const argus_frame* frame, int64_
     float* sig = c->bg.cells + c->bg.cap_cells;
     int* ngood = (int*)(c->bg.cells + 2 * c->bg.cap_cells);
     const DetGrid g = det_grid(bkg_out, nse_out, W, H, cell, k_sigma);
-    CUDA_TRY(c, cudaMemsetAsync(c->bg.ctl, 0, 16, st));
+    rc = det_clear(c, tiles_y, st);
+    if (rc) return rc;
+    unsigned* band_cnt = (unsigned*)(c->bg.tiles + c->bg.cap_tiles) + c->bg.cap_tiles;
     CUDA_TRY(c, cudaMemsetAsync(fb_count, 0, 16, st));
     const unsigned fb_grid = (unsigned)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * 8);
     if (fused) {
@@ -1721,17 +1732,17 @@ extern "C" int argus_detect_frame(argus_ctx* c, const argus_frame* frame, int64_
         bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
         det_cand_kernel<true><<<(unsigned)((n_tiles + 7) / 8), 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, (int)n_tiles, cd.cnt, cd.list,
                                                                              cd.cut, c->bg.tmp, (unsigned)capacity, c->bg.tiles, c->bg.ctl,
-                                                                             fb_list, fb_count);
+                                                                             band_cnt, fb_list, fb_count);
         det_tiles_list_kernel<true><<<fb_grid, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity, c->bg.tiles,
-                                                             c->bg.ctl, fb_list, fb_count);
+                                                             c->bg.ctl, band_cnt, fb_list, fb_count);
     } else {
         bg_cells_kernel<false, true><<<(unsigned)G, BG_THREADS, 0, st>>>(f, (int)W, (int)H, cell, (int)GX, n_min, med, sig, ngood, cd);
         bg_filter_kernel<<<(unsigned)((G + 127) / 128), 128, 0, st>>>(med, sig, ngood, (int)GX, (int)GY, n_min, bkg_out, nse_out);
         det_cand_kernel<false><<<(unsigned)((n_tiles + 7) / 8), 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, (int)n_tiles, cd.cnt, cd.list,
                                                                               cd.cut, c->bg.tmp, (unsigned)capacity, c->bg.tiles, c->bg.ctl,
-                                                                              fb_list, fb_count);
+                                                                              band_cnt, fb_list, fb_count);
         det_tiles_list_kernel<false><<<fb_grid, 256, 0, st>>>(f, (int)W, (int)H, g, (int)tiles_x, c->bg.tmp, (unsigned)capacity, c->bg.tiles,
-                                                              c->bg.ctl, fb_list, fb_count);
+                                                              c->bg.ctl, band_cnt, fb_list, fb_count);
     }
     c->n_launches += 4;
     c->bg.last_fb = fb_count;

@@ -13,9 +13,10 @@
 //   det_tiles_kernel   one CTA per 64 x 32-pixel tile: s = cal - bkg(x, y) for the tile + 1-pixel apron in shared
 //                      memory, thresholded raster-first local maxima, 3x3 flux and centroid; records go to a
 //                      scratch list at an atomically reserved base, (base, count) per tile.
-//   det_scan_kernel    exclusive scan of the per-tile counts.
-//   det_order_kernel   one CTA per tile row: ranks the row's records by raster index and writes them to their final
-//                      position (catalogue order = ascending y * W + x, R-D6).
+//   det_order_kernel   one CTA per tile row: start of the row in the catalogue from the per-row counts, then ranks the row's
+//                      records by raster index and writes them to their final position (catalogue order = ascending
+//                      y * W + x, R-D6).
+//   det_scan_kernel    exclusive scan of per-block counts (argus_subtract_tiles).
 #pragma once
 #include "resample.cuh"
 
@@ -483,7 +484,8 @@ __device__ __forceinline__ void det_write_record(ArgusSourceRec* __restrict__ ds
 template <bool FUSED>
 __device__ __forceinline__ void det_tile_body(const int tile, const FrameArgs& f, int W, int H, const DetGrid& g, int tiles_x,
                                               ArgusSourceRec* __restrict__ tmp, unsigned capacity,
-                                              uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
+                                              uint2* __restrict__ tile_info, unsigned* __restrict__ total,
+                                              unsigned* __restrict__ band_cnt) {
     __shared__ float s_s[(DET_TH + 2) * DET_PITCH];
     __shared__ float s_rb[DET_TH + 2][DET_PCOLS], s_rn[DET_TH + 2][DET_PCOLS];
     __shared__ float2 s_col[DET_PITCH];              // (.x: node offsets lx | lx1 << 8 as int bits, .y: tx)
@@ -593,6 +595,7 @@ __device__ __forceinline__ void det_tile_body(const int tile, const FrameArgs& f
     }
     if (tid == 0) {
         const unsigned base = tile_cnt ? atomicAdd(total, (unsigned)tile_cnt) : 0u;
+        if (tile_cnt) atomicAdd(band_cnt + tile / tiles_x, (unsigned)tile_cnt);
         tile_info[tile] = make_uint2(base, (unsigned)tile_cnt);
         s_base = base;
     }
@@ -620,8 +623,9 @@ __device__ __forceinline__ void det_tile_body(const int tile, const FrameArgs& f
 template <bool FUSED>
 __global__ void __launch_bounds__(256, 8) det_tiles_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
                                                            ArgusSourceRec* __restrict__ tmp, unsigned capacity,
-                                                           uint2* __restrict__ tile_info, unsigned* __restrict__ total) {
-    det_tile_body<FUSED>((int)blockIdx.x, f, W, H, g, tiles_x, tmp, capacity, tile_info, total);
+                                                           uint2* __restrict__ tile_info, unsigned* __restrict__ total,
+                                                           unsigned* __restrict__ band_cnt) {
+    det_tile_body<FUSED>((int)blockIdx.x, f, W, H, g, tiles_x, tmp, capacity, tile_info, total, band_cnt);
 }
 
 // The same on a list of tiles (the tiles det_cand_kernel hands over): CTAs stride over list[0 .. *n_list).
@@ -629,11 +633,12 @@ template <bool FUSED>
 __global__ void __launch_bounds__(256, 8) det_tiles_list_kernel(FrameArgs f, int W, int H, DetGrid g, int tiles_x,
                                                                 ArgusSourceRec* __restrict__ tmp, unsigned capacity,
                                                                 uint2* __restrict__ tile_info, unsigned* __restrict__ total,
+                                                                unsigned* __restrict__ band_cnt,
                                                                 const unsigned* __restrict__ list, const unsigned* __restrict__ n_list) {
     const unsigned n = *n_list;
     for (unsigned i = blockIdx.x; i < n; i += gridDim.x) {
         __syncthreads();                              // the previous tile's shared tables are still being read
-        det_tile_body<FUSED>((int)list[i], f, W, H, g, tiles_x, tmp, capacity, tile_info, total);
+        det_tile_body<FUSED>((int)list[i], f, W, H, g, tiles_x, tmp, capacity, tile_info, total, band_cnt);
     }
 }
 
@@ -749,6 +754,7 @@ __global__ void __launch_bounds__(256, DET_CAND_MINB) det_cand_kernel(FrameArgs 
                                                        const unsigned short* __restrict__ cand_list, const float* __restrict__ cut,
                                                        ArgusSourceRec* __restrict__ tmp, unsigned capacity,
                                                        uint2* __restrict__ tile_info, unsigned* __restrict__ total,
+                                                       unsigned* __restrict__ band_cnt,
                                                        unsigned* __restrict__ fb_list, unsigned* __restrict__ fb_count) {
     const int lane = threadIdx.x & 31, tile = blockIdx.x * 8 + (threadIdx.x >> 5);
     if (tile >= n_tiles) return;
@@ -839,6 +845,7 @@ __global__ void __launch_bounds__(256, DET_CAND_MINB) det_cand_kernel(FrameArgs 
     unsigned base = 0;
     if (lane == 0) {
         base = tile_cnt ? atomicAdd(total, (unsigned)tile_cnt) : 0u;
+        if (tile_cnt) atomicAdd(band_cnt + tile / tiles_x, (unsigned)tile_cnt);
         tile_info[tile] = make_uint2(base, (unsigned)tile_cnt);
     }
     base = __shfl_sync(0xffffffffu, base, 0);
@@ -854,6 +861,7 @@ __global__ void __launch_bounds__(256, DET_CAND_MINB) det_cand_kernel(FrameArgs 
     }
 }
 
+// (used by argus_subtract_tiles; detection folds this scan into det_order_kernel)
 // Exclusive scan of the tile counts in tile order; *n_dev (may be NULL) and ctl[1] receive the total.  One CTA of
 // 1024 threads; 16 x 1024 tiles per round: every thread loads its (coalesced) element of all 16 chunks at once, scans
 // each within its warp, the 16 x 32 warp totals are scanned once by the whole CTA -- five barriers per round instead
@@ -925,26 +933,66 @@ __global__ void __launch_bounds__(1024) det_scan_kernel(const uint2* __restrict_
     }
 }
 
-// Catalogue order (R-D6: ascending raster index y * W + x).  det_tiles_kernel leaves every tile's records in raster
-// order at an arbitrary base of tmp; tiles of one tile row ("band", DET_TH image rows) interleave in raster order.  One
-// CTA per band: (1) band-local keys (y - y0) * W + x (< 2^25) and source positions of the band's records, in tile order,
-// to scratch; (2) rank of every record = number of smaller keys in the band (keys are unique), counted against chunks of
-// 1024 keys staged in shared memory (a 61-MPix frame has ~160 records per band); (3) record -> out[band start + rank].
-// Bands are consecutive in tile order, so band start = offsets[first tile of the band].
+// Count-only calls: the number of sources (the running total of the tile kernels) to the caller's device word.
+__global__ void det_count_kernel(const unsigned* __restrict__ ctl, long long* __restrict__ n_dev) {
+    if (n_dev) *n_dev = (long long)ctl[0];
+}
+
+// Catalogue order (R-D6: ascending raster index y * W + x).  The tile kernels leave every tile's records at an arbitrary
+// base of tmp (in any order inside the tile) and the number of records of every tile row ("band", DET_TH image rows) in
+// band_cnt.  One CTA per band: (0) start of the band in the catalogue = sum of the earlier bands' counts, start of every tile
+// inside it = running sum of the tile counts (to offsets[]: no separate scan kernel); (1) band-local keys (y - y0) * W + x
+// (< 2^25) and source positions of the band's records to scratch; (2) rank of every record = number of smaller keys in the
+// band (keys are unique), counted against chunks of 1024 keys staged in shared memory (a 61-MPix frame has ~160 records
+// per band); (3) record -> out[band start + rank].  The last band stores the total in *n_dev.
 #define DET_ORD_CHUNK 1024
-__global__ void __launch_bounds__(256) det_order_kernel(const uint2* __restrict__ tile_info, const unsigned* __restrict__ offsets,
-                                                        int n_tiles, int tiles_x, int W, const unsigned* __restrict__ ctl,
+__global__ void __launch_bounds__(256) det_order_kernel(const uint2* __restrict__ tile_info, unsigned* __restrict__ offsets,
+                                                        int n_tiles, int tiles_x, int W, const unsigned* __restrict__ band_cnt,
                                                         const ArgusSourceRec* __restrict__ tmp, uint2* __restrict__ ord,
-                                                        ArgusSourceRec* __restrict__ out, unsigned capacity) {
+                                                        ArgusSourceRec* __restrict__ out, unsigned capacity,
+                                                        long long* __restrict__ n_dev) {
     __shared__ unsigned s_key[DET_ORD_CHUNK];
+    __shared__ unsigned s_w[8], s_carry;
     const int band = blockIdx.x, t0 = band * tiles_x, t1 = min(t0 + tiles_x, n_tiles);
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const unsigned band_off = offsets[t0], band_end = (t1 < n_tiles) ? offsets[t1] : ctl[1];
+    // (0) band start
+    unsigned part = 0;
+    for (int b = tid; b < band; b += 256) part += band_cnt[b];
+    part = __reduce_add_sync(0xffffffffu, part);
+    if (lane == 0) s_w[wid] = part;
+    __syncthreads();
+    unsigned band_off = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) band_off += s_w[w];
+    const unsigned n_band = band_cnt[band], band_end = band_off + n_band;
+    if (band == (int)gridDim.x - 1 && tid == 0 && n_dev) *n_dev = (long long)band_end;
     if (band_end > capacity) {
         if (band_off >= capacity) return;       // overflow: the contents of out are unspecified, nothing beyond capacity
     }
     const unsigned n_b = min(band_end, capacity) - band_off;
     if (n_b == 0) return;
+    // tile starts: exclusive scan of the band's tile counts, 256 tiles per round
+    if (tid == 0) s_carry = band_off;
+    __syncthreads();
+    for (int c0 = t0; c0 < t1; c0 += 256) {
+        const int tile = c0 + tid;
+        const unsigned cnt = tile < t1 ? tile_info[tile].y : 0u;
+        unsigned inc = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned o = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += o;
+        }
+        if (lane == 31) s_w[wid] = inc;
+        __syncthreads();
+        unsigned before = s_carry;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) before += (w < wid) ? s_w[w] : 0u;
+        if (tile < t1) offsets[tile] = before + inc - cnt;
+        __syncthreads();
+        if (tid == 255) s_carry = before + inc;
+    }
+    __syncthreads();
     const int y0 = band * DET_TH;
     for (int tile = t0 + wid; tile < t1; tile += 8) {
         const uint2 info = tile_info[tile];
