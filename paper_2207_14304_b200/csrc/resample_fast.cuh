@@ -380,7 +380,17 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
             if (lane == 0) {
                 d.off = off_c;
                 d.t = t;
-                if (COADD) d.cslot = pb.cslot[t];               // coadd_slots_kernel, once per call
+                if (COADD) {
+                    d.cslot = pb.cslot[t];                      // coadd_slots_kernel, once per call
+#ifndef ARGUS_NO_COADD_PREFETCH
+                    // the tile's accumulators (2 x 4 KB, contiguous in the tile-dense layout) into L2 one or two tiles ahead of
+                    // the consumers' read-modify-write: their loads were the kernel's longest stall (DRAM latency at 18 warps/SM)
+                    if (d.cslot >= 0) {
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.sum + d.cslot), "r"(ARGUS_TILE_PIX * 4) : "memory");
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.wsum + d.cslot), "r"(ARGUS_TILE_PIX * 4) : "memory");
+                    }
+#endif
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive_expect_tx(&sm.full[ds], tx_bytes);   // releases the descriptor to the consumers
