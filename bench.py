@@ -47,13 +47,19 @@ def _peaks():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def _kernel_sources_sha():
-    """Hash of the CUDA sources: a dram-traffic figure taken from an ncu profile is only quoted while the kernels are
-    the ones that were profiled."""
+# kernel sources behind each workload's dominant kernels (device code only: argus_api.cu holds validation and launches)
+_RESAMPLE_SRC = ("common.cuh", "plan.cuh", "plan_block.cuh", "resample.cuh", "resample_fast.cuh", "resample_unit.cuh")
+KERNEL_SOURCES = {"segments": ("common.cuh", "segments.cuh"), "detect": ("common.cuh", "resample.cuh", "background.cuh"),
+                  "subtract": ("common.cuh", "resample.cuh", "background.cuh", "subtract.cuh")}
+
+
+def _kernel_sources_sha(key="config1"):
+    """Hash of the CUDA sources of a workload's kernels: a dram-traffic figure taken from an ncu profile is only quoted
+    while the kernels are the ones that were profiled."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2207_14304_b200", "csrc")
-    for name in sorted(os.listdir(d)):
+    for name in KERNEL_SOURCES.get(key.split("_")[0], _RESAMPLE_SRC):
         with open(os.path.join(d, name), "rb") as f:
             h.update(name.encode() + b"\0" + f.read())
     return h.hexdigest()[:16]
@@ -67,7 +73,7 @@ def ncu_traffic(key):
             t = json.load(f)[key]
     except Exception:
         return None, "no ncu capture recorded for this workload (profiles/traffic.json)"
-    if t.get("csrc_sha16") != _kernel_sources_sha():
+    if t.get("csrc_sha16") != _kernel_sources_sha(key):
         return None, "kernels changed since %s was captured (profiles/traffic.json)" % t.get("profile")
     return int(t["dram_bytes"]), "%s, csrc %s" % (t["profile"], t["csrc_sha16"])
 
