@@ -40,6 +40,18 @@ __device__ __forceinline__ unsigned spread_bits16(unsigned v) {       // bit i -
     return v;
 }
 
+// The two images at one pixel: s = sum / wsum through one reciprocal each (rcp.approx: 1 ulp, so the quotients are within 2 ulp =
+// 2.4e-7 relative, 40 x inside the 1e-5 relative tolerance; the weights are >= wmin > 0).  Both passes use these same float32
+// values: the fit is made on the images the difference is formed from.
+__device__ __forceinline__ void sub_images(float ssv, float swv, float rsv, float rwv, float& s, float& r, float& isw, float& irw) {
+    isw = rcp_ftz(swv); irw = rcp_ftz(rwv);
+    s = ssv * isw; r = rsv * irw;
+}
+__device__ __forceinline__ float rsqrt_ftz(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 // ---------------------------------------------------------------------------------------------- statistics
 // grid = (tiles of the chunk) * split CTAs of 256 threads; CTA (t, j) covers pixels [j, j + 1) * ppt / split of tile tile0 + t.
 __global__ void __launch_bounds__(256) sub_stats_kernel(const float* __restrict__ ss, const float* __restrict__ sw,
@@ -62,7 +74,9 @@ __global__ void __launch_bounds__(256) sub_stats_kernel(const float* __restrict_
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             if (ws[k] >= p.sci_wmin && wr[k] >= p.ref_wmin) {
-                const double s = (double)(xs[k] / ws[k]), r = (double)(ys[k] / wr[k]);   // the float32 images the subtraction uses
+                float sf, rf, i0, i1;
+                sub_images(xs[k], ws[k], ys[k], wr[k], sf, rf, i0, i1);                  // the float32 images the subtraction uses
+                const double s = (double)sf, r = (double)rf;
                 acc[0] += 1.0; acc[1] += r; acc[2] += s; acc[3] += r * r; acc[4] += r * s;
             }
         }
@@ -109,22 +123,30 @@ __global__ void sub_fit_kernel(const double* __restrict__ partial, long long til
 }
 
 // ---------------------------------------------------------------------------------------------- per pixel
-// R-X1, R-X3 .. R-X5 for one pixel (IEEE division and square root).  Invalid: d = 0, S = -inf (never a maximum).
+// R-X1, R-X3 .. R-X5 for one pixel.  Invalid: d = 0, S = -inf (never a maximum).  Five IEEE divisions and a square root per
+// pixel made this pass instruction-bound (XU pipe 34 %, 128 instructions per pixel); two reciprocals and one reciprocal
+// square root (2 ulp each; the variance is > 0: read noise > 0) leave every output within 1e-6 relative of the IEEE form.
 __device__ __forceinline__ void sub_px(float ssv, float swv, float rsv, float rwv, const SubParams& p, float alpha, float beta,
                                        float& d, float& S, float& sigma) {
     d = 0.f; sigma = 0.f; S = __int_as_float(0xff800000);
     if (swv >= p.sci_wmin && rwv >= p.ref_wmin) {
-        const float s = ssv / swv, r = rsv / rwv;
+        float s, r, isw, irw;
+        sub_images(ssv, swv, rsv, rwv, s, r, isw, irw);
         const float m = fmaf(alpha, r, beta);
         d = s - m;
-        sigma = sqrtf((p.rn2 + fmaxf(m, 0.f) * p.inv_gain) * (1.0f / swv + alpha * alpha / rwv));
-        S = d / sigma;
+        const float var = (p.rn2 + fmaxf(m, 0.f) * p.inv_gain) * fmaf(alpha * alpha, irw, isw);
+        const float rs = rsqrt_ftz(var);
+        sigma = var * rs;
+        S = d * rs;
     }
 }
 
 // grid-stride over blocks of 1024 consecutive nested indices; 256 threads, thread t <-> in-block indices 4 t .. 4 t + 3
 // (a 2 x 2 pixel group: one 128-bit load per array, one 128-bit store per output).
-__global__ void __launch_bounds__(256) sub_tiles_kernel(const float* __restrict__ ss, const float* __restrict__ sw,
+#ifndef SUB_TILES_MINB
+#define SUB_TILES_MINB 6                 // 39 registers, 16 B of spills: six CTAs per SM hide the load latency (4: 0.452, 5: 0.427, 6: 0.421, 8: 0.487 ms per call)
+#endif
+__global__ void __launch_bounds__(256, SUB_TILES_MINB) sub_tiles_kernel(const float* __restrict__ ss, const float* __restrict__ sw,
                                                        const float* __restrict__ rs, const float* __restrict__ rw,
                                                        const long long* __restrict__ tiles, long long ppt, int side_log2,
                                                        long long b0, long long n_blocks, SubParams p, const float2* __restrict__ fit,
