@@ -325,7 +325,7 @@ __device__ __forceinline__ void bg_cand_flush(BgCandShared& sc, const BgCand& cd
 
 // R-D1: per-cell median, 1.4826 MAD and good-pixel count.  grid = GX * GY CTAs of 256 threads; B in {8,16,32,64}.
 #ifndef BG_MINB
-#define BG_MINB 5                    // 48 registers: the kernel waits at its barriers, residency pays (4 CTAs/SM: 9 % slower)
+#define BG_MINB 6                    // 40 registers, no spills: the kernel waits at its barriers, residency pays (4 / 5 CTAs per SM: 11 % / 2 % slower)
 #endif
 template <bool FUSED, bool CAND = false>
 __global__ void __launch_bounds__(BG_THREADS, BG_MINB) bg_cells_kernel(FrameArgs f, int W, int H, int B, int GX, int n_min,
