@@ -278,3 +278,38 @@ def test_mixed_sign_values_zeros_and_duplicates(argus, ctx, B):
     n_must, n_amb = compare_catalogue(rec, cal32.astype(np.float64), mask, bkg, nse, W, B, 5.0)   # measured: 0 ambiguous (default bound 3)
     print("mixed-sign B=%d: %d records, %d clear sources, %d ambiguous decisions" % (B, rec.size, n_must, n_amb))
     check_detect_frame(argus, ctx, W, H, B, 4, 5.0, _dev_cal(cal32, mask), g, rec)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_detect_frame_fuzz_identical_to_two_calls(argus, ctx, seed):
+    """argus_detect_frame's proof (no pixel below the cells' cuts can pass the threshold of the tile) on frames built to
+    strain it: steep background gradients, steps across cell boundaries, bright extended blobs whose cells run ahead of
+    their neighbours' filtered values, star fields of every brightness, masked holes and rows, noise of varying level;
+    every cell size, thresholds from below the candidate cut to 12 sigma, n_min from 1 to above a cell's size.  The
+    result must be what argus_background_map + argus_detect_sources give, bit for bit."""
+    rng = np.random.default_rng(9000 + seed)
+    H, W = int(rng.integers(90, 420)), int(rng.integers(130, 700))
+    yy, xx = np.mgrid[0:H, 0:W].astype(np.float64)
+    sky = rng.uniform(-50, 2000) + rng.uniform(-3, 3) * xx + rng.uniform(-3, 3) * yy          # gradient
+    if seed % 3 == 0:
+        sky += rng.uniform(50, 800) * (xx > rng.uniform(0.2, 0.8) * W)                          # a step
+    sigma = rng.uniform(1.0, 40.0) * (1.0 + (seed % 2) * xx / W)                                # noise level varies across the frame
+    img = sky + rng.normal(0.0, 1.0, (H, W)) * sigma
+    for _ in range(int(rng.integers(5, 60))):                                                   # stars: faint to saturated
+        cy, cx, a, w = rng.uniform(0, H), rng.uniform(0, W), 10.0 ** rng.uniform(0.5, 4.5), rng.uniform(0.7, 6.0)
+        img += a * np.exp(-((xx - cx) ** 2 + (yy - cy) ** 2) / (2 * w * w))
+    cal32 = img.astype(np.float32)
+    mask = (rng.random((H, W)) > rng.choice([0.0, 0.02, 0.3])).astype(np.uint8)
+    if seed % 4 == 1:
+        mask[H // 3:H // 3 + 70, W // 4:W // 4 + 90] = 0                                        # a hole larger than a cell
+        mask[(2 * H) // 3, :] = 0
+    cal32[mask == 0] = 0.0
+    fr = _dev_cal(cal32, mask)
+    n_full_seen = []
+    for B in (64, 32, 16, 8):
+        for k, n_min in ((5.0, 16), (3.5, 1), (12.0, 70), (2.0, 16)):
+            g = gpu_background(argus, ctx, W, H, B, n_min, fr)
+            rec = gpu_detect(argus, ctx, W, H, B, k, g["dev"]["bkg"], g["dev"]["nse"], fr)
+            n_full_seen.append(check_detect_frame(argus, ctx, W, H, B, n_min, k, fr, g, rec))
+    n_tiles = -(-W // 64) * -(-H // 32)
+    assert min(n_full_seen) < n_tiles          # the candidate path did serve tiles in some configuration
