@@ -48,7 +48,8 @@ def _peaks():
 
 
 # kernel sources behind each workload's dominant kernels (device code only: argus_api.cu holds validation and launches)
-_RESAMPLE_SRC = ("common.cuh", "plan.cuh", "plan_block.cuh", "resample.cuh", "resample_fast.cuh", "resample_unit.cuh")
+# (the configs profiled for profiles/traffic.json run the tile kernel of resample_fast.cuh, not the unit kernel)
+_RESAMPLE_SRC = ("common.cuh", "plan.cuh", "plan_block.cuh", "resample.cuh", "resample_fast.cuh")
 KERNEL_SOURCES = {"segments": ("common.cuh", "segments.cuh"), "detect": ("common.cuh", "resample.cuh", "background.cuh"),
                   "subtract": ("common.cuh", "resample.cuh", "background.cuh", "subtract.cuh")}
 

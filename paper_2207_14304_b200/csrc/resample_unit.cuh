@@ -299,7 +299,17 @@ __global__ void UNIT_BOUNDS
             long long off_l = 0, cs_l = -1;
             if (lane < nseg) {
                 off_l = tile_out_offset(pb, sg.t);
-                if (COADD) cs_l = pb.cslot[sg.t];               // coadd_slots_kernel, once per call
+                if (COADD) {
+                    cs_l = pb.cslot[sg.t];                      // coadd_slots_kernel, once per call
+#ifndef ARGUS_NO_COADD_PREFETCH
+                    // the segment's tile accumulators towards L2 ahead of the consumers' read-modify-write (as in the tile kernel;
+                    // the units that share a tile find it there already)
+                    if (cs_l >= 0) {
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.sum + cs_l), "r"(ARGUS_TILE_PIX * 4) : "memory");
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.wsum + cs_l), "r"(ARGUS_TILE_PIX * 4) : "memory");
+                    }
+#endif
+                }
             }
             __syncwarp();
             int cls_l = 0, mslot_l = 0;
