@@ -385,7 +385,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
 #ifndef ARGUS_NO_COADD_PREFETCH
                     // the tile's accumulators (2 x 4 KB, contiguous in the tile-dense layout) into L2 one or two tiles ahead of
                     // the consumers' read-modify-write: their loads were the kernel's longest stall (DRAM latency at 18 warps/SM)
-                    if (d.cslot >= 0) {
+                    if (d.cslot >= 0 && ((((unsigned long long)ca.sum | (unsigned long long)ca.wsum) & 15ull) == 0ull)) {   // (the API asks for 4-byte alignment only)
                         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.sum + d.cslot), "r"(ARGUS_TILE_PIX * 4) : "memory");
                         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.wsum + d.cslot), "r"(ARGUS_TILE_PIX * 4) : "memory");
                     }

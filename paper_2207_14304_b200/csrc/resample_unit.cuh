@@ -304,7 +304,7 @@ __global__ void UNIT_BOUNDS
 #ifndef ARGUS_NO_COADD_PREFETCH
                     // the segment's tile accumulators towards L2 ahead of the consumers' read-modify-write (as in the tile kernel;
                     // the units that share a tile find it there already)
-                    if (cs_l >= 0) {
+                    if (cs_l >= 0 && ((((unsigned long long)ca.sum | (unsigned long long)ca.wsum) & 15ull) == 0ull)) {   // (the API asks for 4-byte alignment only)
                         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.sum + cs_l), "r"(ARGUS_TILE_PIX * 4) : "memory");
                         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(ca.wsum + cs_l), "r"(ARGUS_TILE_PIX * 4) : "memory");
                     }

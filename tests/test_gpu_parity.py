@@ -305,6 +305,39 @@ def test_coadd_three_frames(argus, ctx):
         assert_coadd_matches(s.cpu().numpy(), ws.cpu().numpy(), ref, "coadd of 3 frames, fused=%s" % fused)
 
 
+@pytest.mark.parametrize("force_unit", [False, True])
+def test_coadd_buffers_aligned_to_4_bytes_only(argus, ctx, force_unit):
+    """The header asks for float alignment of sum / wsum, nothing more; the kernels' L2 prefetch of the accumulators needs
+    16 bytes and must step aside: accumulators that start 4 bytes into an allocation give the bits of aligned ones."""
+    from gpu_util import upload
+    W = H = 512
+    nside = 1 << 17
+    f = synth.config3_frame(0, W, H)
+    fp = oracle.footprint(f.wcs, W, H, nside)[0]
+    tiles = np.unique(fp >> 18)
+    ppt = 1 << 18
+    dt = torch.from_numpy(tiles).cuda()
+    d = upload(f)
+    if force_unit:
+        ctx.set_fast_path(3)
+    try:
+        out = []
+        for shift in (0, 1):
+            s = torch.zeros(len(tiles) * ppt + 4, dtype=torch.float32, device="cuda")
+            ws = torch.zeros_like(s)
+            sv, wv = s[shift:shift + len(tiles) * ppt], ws[shift:shift + len(tiles) * ppt]
+            assert sv.data_ptr() % 16 == 4 * shift
+            for _ in range(2):
+                argus.argus_resample_coadd(ctx, f.wcs, W, H, nside, "bilinear", dt, 256, sv, wv, None, **d)
+            torch.cuda.synchronize()
+            out.append((sv.clone(), wv.clone()))
+    finally:
+        if force_unit:
+            ctx.set_fast_path(1)
+    assert torch.equal(out[0][0].view(torch.int32), out[1][0].view(torch.int32)) and torch.equal(out[0][1], out[1][1])
+    assert float(out[0][1].sum()) > 0
+
+
 def _saturated_star_frame(seed=11, kernel="lanczos3"):
     """512 x 512 frame with six stars whose cores clip at 65535 (=> masked) and wings up to ~6e4 ADU."""
     W = H = 512
