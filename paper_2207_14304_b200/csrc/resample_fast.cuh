@@ -132,6 +132,34 @@ __device__ __forceinline__ void consumers_sync(int group) {
 }
 
 // ------------------------------------------------------------------------------------ coordinates
+// ---- packed FP32 (Blackwell FFMA2 / FMUL2 / FADD2: two IEEE operations per instruction, either operand may be a scalar
+// broadcast).  The clean interpolation loops are bound by instruction issue, and their x and y halves (and neighbouring rows
+// of taps) run the same operations on different data: packed, the Lanczos-3 weights + gather take 60 instructions less per
+// output.  Each lane of a packed operation rounds exactly as the scalar one: results are bit-identical to the scalar form.
+#ifndef ARGUS_NO_F32X2
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)),
+        "l"(*reinterpret_cast<unsigned long long*>(&c)));
+    return *reinterpret_cast<float2*>(&d);
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+    unsigned long long d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)));
+    return *reinterpret_cast<float2*>(&d);
+}
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)));
+    return *reinterpret_cast<float2*>(&d);
+}
+#else
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
+#endif
+__device__ __forceinline__ float2 bc2(float s) { return make_float2(s, s); }
+
 struct FastAxis {
     float A0, A1, B0, B1, C0, C1, c9;   // Horner in T; index = S variant (pixel column u or u + 16)
     int lin;                            // c0 + a*s0 + b*t0
@@ -188,31 +216,84 @@ __device__ __forceinline__ void lanczos3_weights_f32(float f, float k[6]) {
     k[5] = C * rcp_ftz(t5 * t5);
 }
 
+// sinpi_third / cospi_sixth / lanczos3_weights_f32 for the x and the y fraction at once (.x: x axis, .y: y axis); the
+// operations and their order are those of the scalar functions.  Neither fraction may be zero.
+__device__ __forceinline__ float2 sinpi_third2(float2 u) {
+    const float2 u2 = mul2(u, u);
+    float2 p = fma2(u2, bc2(-0.007370430945714348f), bc2(0.08214588661112819f));
+    p = fma2(u2, p, bc2(-0.5992645293207919f));
+    p = fma2(u2, p, bc2(2.550164039877345f));
+    p = fma2(u2, p, bc2(-5.167712780049969f));
+    p = fma2(u2, p, bc2(3.141592653589793f));
+    return mul2(u, p);
+}
+__device__ __forceinline__ float2 cospi_sixth2(float2 w) {
+    const float2 w2 = mul2(w, w);
+    float2 p = fma2(w2, bc2(0.23533063035889312f), bc2(-1.3352627688545893f));
+    p = fma2(w2, p, bc2(4.058712126416768f));
+    p = fma2(w2, p, bc2(-4.934802200544679f));
+    return fma2(w2, p, bc2(1.0f));
+}
+__device__ __forceinline__ float2 rcp2_ftz(float2 v) { return make_float2(rcp_ftz(v.x), rcp_ftz(v.y)); }
+__device__ __forceinline__ void lanczos3_weights_f32x2(float2 f, float2 k[6]) {
+    const float2 A = sinpi_third2(mul2(add2(bc2(1.0f), make_float2(-f.x, -f.y)), bc2(0.33333334f)));
+    const float2 Bc = cospi_sixth2(fma2(f, bc2(0.33333334f), bc2(-0.16666667f))), B = make_float2(-Bc.x, -Bc.y);
+    const float2 C = sinpi_third2(mul2(f, bc2(0.33333334f)));
+    const float2 t0 = add2(f, bc2(2.0f)), t1 = add2(f, bc2(1.0f)), t3 = add2(f, bc2(-1.0f)), t4 = add2(f, bc2(-2.0f)), t5 = add2(f, bc2(-3.0f));
+    k[0] = mul2(A, rcp2_ftz(mul2(t0, t0)));
+    k[1] = mul2(B, rcp2_ftz(mul2(t1, t1)));
+    k[2] = mul2(C, rcp2_ftz(mul2(f, f)));
+    k[3] = mul2(A, rcp2_ftz(mul2(t3, t3)));
+    k[4] = mul2(B, rcp2_ftz(mul2(t4, t4)));
+    k[5] = mul2(C, rcp2_ftz(mul2(t5, t5)));
+}
+
 // No masked tap in the tile's box: weight == 1.  a = address of the cell (floor x, floor y) in the calibrated box.
 template <int KERNEL>
 __device__ __forceinline__ float interp_clean(const float* __restrict__ a, int pitch, float fx, float fy) {
     if (KERNEL == 0) {
         const float c00 = a[0], c01 = a[1], c10 = a[pitch], c11 = a[pitch + 1];
-        const float top = fmaf(fx, c01 - c00, c00), bot = fmaf(fx, c11 - c10, c10);
-        return fmaf(fy, bot - top, top);
+        // (top, bot) = fx * ((c01, c11) - (c00, c10)) + (c00, c10)
+        const float2 lo = make_float2(c00, c10);
+        const float2 tb = fma2(bc2(fx), add2(make_float2(c01, c11), make_float2(-c00, -c10)), lo);
+        return fmaf(fy, tb.y - tb.x, tb.x);
     } else {
-        float kx[6], ky[6];
-        lanczos3_weights_f32(fx, kx);
-        lanczos3_weights_f32(fy, ky);
+        if (fx == 0.0f || fy == 0.0f) {              // a tap exactly on a pixel centre (1 in 2^23 fractions): the scalar form
+            float kx[6], ky[6];
+            lanczos3_weights_f32(fx, kx);
+            lanczos3_weights_f32(fy, ky);
+            const float* r = a - 2 * pitch - 2;
+            float V = 0.0f;
+#pragma unroll 1
+            for (int b = 0; b < 6; ++b) {
+                float rs = kx[0] * r[0];
+#pragma unroll
+                for (int q = 1; q < 6; ++q) rs = fmaf(kx[q], r[q], rs);
+                V = fmaf(ky[b], rs, V);
+                r += pitch;
+            }
+            const float sx = ((kx[0] + kx[5]) + (kx[1] + kx[4])) + (kx[2] + kx[3]);
+            const float sy = ((ky[0] + ky[5]) + (ky[1] + ky[4])) + (ky[2] + ky[3]);
+            return __fdividef(V, sx * sy);
+        }
+        float2 k[6];                                  // (kx[q], ky[q])
+        lanczos3_weights_f32x2(make_float2(fx, fy), k);
         const float* r = a - 2 * pitch - 2;
-        // FP32 accumulation is enough where no tap is masked (full-size parity: worst 0.61 x tolerance over 3.2e8 pixels)
+        // FP32 accumulation is enough where no tap is masked (full-size parity: worst 0.61 x tolerance over 3.2e8 pixels).
+        // Two rows of taps per packed operation; the sum over the rows stays in its order.
         float V = 0.0f;
 #pragma unroll
-        for (int b = 0; b < 6; ++b) {
-            float rs = kx[0] * r[0];
+        for (int b = 0; b < 6; b += 2) {
+            const float* r1 = r + pitch;
+            float2 rs = mul2(bc2(k[0].x), make_float2(r[0], r1[0]));
 #pragma unroll
-            for (int q = 1; q < 6; ++q) rs = fmaf(kx[q], r[q], rs);
-            V = fmaf(ky[b], rs, V);
-            r += pitch;
+            for (int q = 1; q < 6; ++q) rs = fma2(bc2(k[q].x), make_float2(r[q], r1[q]), rs);
+            V = fmaf(k[b].y, rs.x, V);
+            V = fmaf(k[b + 1].y, rs.y, V);
+            r += 2 * pitch;
         }
-        const float sx = ((kx[0] + kx[5]) + (kx[1] + kx[4])) + (kx[2] + kx[3]);
-        const float sy = ((ky[0] + ky[5]) + (ky[1] + ky[4])) + (ky[2] + ky[3]);
-        return __fdividef(V, sx * sy);   // 2 ulp: 2.4e-7 relative, 40x inside the relative tolerance
+        const float2 s = add2(add2(add2(k[0], k[5]), add2(k[1], k[4])), add2(k[2], k[3]));   // (sum kx, sum ky)
+        return __fdividef(V, s.x * s.y);   // 2 ulp: 2.4e-7 relative, 40x inside the relative tolerance
     }
 }
 
