@@ -129,6 +129,30 @@ __device__ __forceinline__ float calib_fast(unsigned magic_r, float b, float d, 
     return good ? c : nanf_();
 }
 
+// Four consecutive pixels through calib_fast, two per packed FP32 instruction (the operations and their order are
+// calib_fast's: bit-identical).  rw: the four 16-bit raw values.
+template <bool REFINE = false>
+__device__ __forceinline__ float4 calib_fast4(uint2 rw, float4 b, float4 d, float4 fl, float t_exp, float sat_f, unsigned fmin_bits,
+                                              unsigned frange) {
+    const float2 m01 = make_float2(__uint_as_float(__byte_perm(rw.x, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(rw.x, 0x4B000000u, 0x7632)));
+    const float2 m23 = make_float2(__uint_as_float(__byte_perm(rw.y, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(rw.y, 0x4B000000u, 0x7632)));
+    const float2 rf01 = add2(m01, bc2(-8388608.0f)), rf23 = add2(m23, bc2(-8388608.0f));
+    const float2 t01 = fma2(make_float2(-d.x, -d.y), bc2(t_exp), add2(rf01, make_float2(-b.x, -b.y)));
+    const float2 t23 = fma2(make_float2(-d.z, -d.w), bc2(t_exp), add2(rf23, make_float2(-b.z, -b.w)));
+    const float2 r01 = make_float2(rcp_ftz(fl.x), rcp_ftz(fl.y)), r23 = make_float2(rcp_ftz(fl.z), rcp_ftz(fl.w));
+    float2 c01 = mul2(t01, r01), c23 = mul2(t23, r23);
+    if (REFINE) {
+        c01 = fma2(fma2(make_float2(-c01.x, -c01.y), make_float2(fl.x, fl.y), t01), r01, c01);
+        c23 = fma2(fma2(make_float2(-c23.x, -c23.y), make_float2(fl.z, fl.w), t23), r23, c23);
+    }
+    float4 o;
+    o.x = ((rf01.x < sat_f) && ((__float_as_uint(fl.x) - fmin_bits) < frange) && (fabsf(c01.x) < INFINITY)) ? c01.x : nanf_();
+    o.y = ((rf01.y < sat_f) && ((__float_as_uint(fl.y) - fmin_bits) < frange) && (fabsf(c01.y) < INFINITY)) ? c01.y : nanf_();
+    o.z = ((rf23.x < sat_f) && ((__float_as_uint(fl.z) - fmin_bits) < frange) && (fabsf(c23.x) < INFINITY)) ? c23.x : nanf_();
+    o.w = ((rf23.y < sat_f) && ((__float_as_uint(fl.w) - fmin_bits) < frange) && (fabsf(c23.y) < INFINITY)) ? c23.y : nanf_();
+    return o;
+}
+
 // Stage the box [gx0, gx0+bw) x [gy0, gy0+bh) (gx0, bw multiples of 4) into s_box (pitch bw).
 // Returns non-zero for threads that stored a masked pixel.
 template <bool FUSED, bool PRECISE>

@@ -132,34 +132,6 @@ __device__ __forceinline__ void consumers_sync(int group) {
 }
 
 // ------------------------------------------------------------------------------------ coordinates
-// ---- packed FP32 (Blackwell FFMA2 / FMUL2 / FADD2: two IEEE operations per instruction, either operand may be a scalar
-// broadcast).  The clean interpolation loops are bound by instruction issue, and their x and y halves (and neighbouring rows
-// of taps) run the same operations on different data: packed, the Lanczos-3 weights + gather take 60 instructions less per
-// output.  Each lane of a packed operation rounds exactly as the scalar one: results are bit-identical to the scalar form.
-#ifndef ARGUS_NO_F32X2
-__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
-    unsigned long long d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)),
-        "l"(*reinterpret_cast<unsigned long long*>(&c)));
-    return *reinterpret_cast<float2*>(&d);
-}
-__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
-    unsigned long long d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)));
-    return *reinterpret_cast<float2*>(&d);
-}
-__device__ __forceinline__ float2 add2(float2 a, float2 b) {
-    unsigned long long d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)));
-    return *reinterpret_cast<float2*>(&d);
-}
-#else
-__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)); }
-__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
-__device__ __forceinline__ float2 add2(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
-#endif
-__device__ __forceinline__ float2 bc2(float s) { return make_float2(s, s); }
-
 struct FastAxis {
     float A0, A1, B0, B1, C0, C1, c9;   // Horner in T; index = S variant (pixel column u or u + 16)
     int lin;                            // c0 + a*s0 + b*t0
@@ -516,10 +488,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
                 const float4 b = reinterpret_cast<const float4*>(sg.bias)[v];
                 const float4 dk = reinterpret_cast<const float4*>(sg.dark)[v];
                 const float4 fl = reinterpret_cast<const float4*>(sg.flat)[v];
-                o4[j].x = calib_fast<KERNEL == 1>(__byte_perm(rw.x, 0x4B000000u, 0x7610), b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
-                o4[j].y = calib_fast<KERNEL == 1>(__byte_perm(rw.x, 0x4B000000u, 0x7632), b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
-                o4[j].z = calib_fast<KERNEL == 1>(__byte_perm(rw.y, 0x4B000000u, 0x7610), b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
-                o4[j].w = calib_fast<KERNEL == 1>(__byte_perm(rw.y, 0x4B000000u, 0x7632), b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
+                o4[j] = calib_fast4<KERNEL == 1>(rw, b, dk, fl, t_exp, sat_f, fmin_bits, frange);
                 bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
                 if (KERNEL == 1) big |= (fmaxf(fmaxf(fabsf(o4[j].x), fabsf(o4[j].y)), fmaxf(fabsf(o4[j].z), fabsf(o4[j].w))) > RF_LZ_BIG_ADU);
             }

@@ -415,10 +415,7 @@ __global__ void UNIT_BOUNDS
                     const float4 b = reinterpret_cast<const float4*>(st + UNIT_CAP * 2)[v];
                     const float4 dk = reinterpret_cast<const float4*>(st + UNIT_CAP * 6)[v];
                     const float4 fl = reinterpret_cast<const float4*>(st + UNIT_CAP * 10)[v];
-                    o4[j].x = calib_fast<KERNEL == 1>(m0, b.x, dk.x, fl.x, false, t_exp, sat_f, fmin_bits, frange);
-                    o4[j].y = calib_fast<KERNEL == 1>(m1, b.y, dk.y, fl.y, false, t_exp, sat_f, fmin_bits, frange);
-                    o4[j].z = calib_fast<KERNEL == 1>(m2, b.z, dk.z, fl.z, false, t_exp, sat_f, fmin_bits, frange);
-                    o4[j].w = calib_fast<KERNEL == 1>(m3, b.w, dk.w, fl.w, false, t_exp, sat_f, fmin_bits, frange);
+                    o4[j] = calib_fast4<KERNEL == 1>(rw, b, dk, fl, t_exp, sat_f, fmin_bits, frange);
                 } else {
                     float4 of, gn;
                     if (MASTERS == 1) {
