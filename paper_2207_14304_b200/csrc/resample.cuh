@@ -133,7 +133,7 @@ __device__ __forceinline__ float calib_fast(unsigned magic_r, float b, float d, 
 // calib_fast's: bit-identical).  rw: the four 16-bit raw values.
 template <bool REFINE = false>
 __device__ __forceinline__ float4 calib_fast4(uint2 rw, float4 b, float4 d, float4 fl, float t_exp, float sat_f, unsigned fmin_bits,
-                                              unsigned frange) {
+                                              unsigned frange, int& bad) {
     const float2 m01 = make_float2(__uint_as_float(__byte_perm(rw.x, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(rw.x, 0x4B000000u, 0x7632)));
     const float2 m23 = make_float2(__uint_as_float(__byte_perm(rw.y, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(rw.y, 0x4B000000u, 0x7632)));
     const float2 rf01 = add2(m01, bc2(-8388608.0f)), rf23 = add2(m23, bc2(-8388608.0f));
@@ -145,12 +145,12 @@ __device__ __forceinline__ float4 calib_fast4(uint2 rw, float4 b, float4 d, floa
         c01 = fma2(fma2(make_float2(-c01.x, -c01.y), make_float2(fl.x, fl.y), t01), r01, c01);
         c23 = fma2(fma2(make_float2(-c23.x, -c23.y), make_float2(fl.z, fl.w), t23), r23, c23);
     }
-    float4 o;
-    o.x = ((rf01.x < sat_f) && ((__float_as_uint(fl.x) - fmin_bits) < frange) && (fabsf(c01.x) < INFINITY)) ? c01.x : nanf_();
-    o.y = ((rf01.y < sat_f) && ((__float_as_uint(fl.y) - fmin_bits) < frange) && (fabsf(c01.y) < INFINITY)) ? c01.y : nanf_();
-    o.z = ((rf23.x < sat_f) && ((__float_as_uint(fl.z) - fmin_bits) < frange) && (fabsf(c23.x) < INFINITY)) ? c23.x : nanf_();
-    o.w = ((rf23.y < sat_f) && ((__float_as_uint(fl.w) - fmin_bits) < frange) && (fabsf(c23.y) < INFINITY)) ? c23.y : nanf_();
-    return o;
+    const bool g0 = (rf01.x < sat_f) && ((__float_as_uint(fl.x) - fmin_bits) < frange) && (fabsf(c01.x) < INFINITY);
+    const bool g1 = (rf01.y < sat_f) && ((__float_as_uint(fl.y) - fmin_bits) < frange) && (fabsf(c01.y) < INFINITY);
+    const bool g2 = (rf23.x < sat_f) && ((__float_as_uint(fl.z) - fmin_bits) < frange) && (fabsf(c23.x) < INFINITY);
+    const bool g3 = (rf23.y < sat_f) && ((__float_as_uint(fl.w) - fmin_bits) < frange) && (fabsf(c23.y) < INFINITY);
+    bad |= !(g0 && g1 && g2 && g3);                  // a masked pixel among the four (the caller need not test for NaN)
+    return make_float4(g0 ? c01.x : nanf_(), g1 ? c01.y : nanf_(), g2 ? c23.x : nanf_(), g3 ? c23.y : nanf_());
 }
 
 // Stage the box [gx0, gx0+bw) x [gy0, gy0+bh) (gx0, bw multiples of 4) into s_box (pitch bw).

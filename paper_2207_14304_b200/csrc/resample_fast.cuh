@@ -488,8 +488,7 @@ __global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
                 const float4 b = reinterpret_cast<const float4*>(sg.bias)[v];
                 const float4 dk = reinterpret_cast<const float4*>(sg.dark)[v];
                 const float4 fl = reinterpret_cast<const float4*>(sg.flat)[v];
-                o4[j] = calib_fast4<KERNEL == 1>(rw, b, dk, fl, t_exp, sat_f, fmin_bits, frange);
-                bad |= (o4[j].x != o4[j].x) | (o4[j].y != o4[j].y) | (o4[j].z != o4[j].z) | (o4[j].w != o4[j].w);
+                o4[j] = calib_fast4<KERNEL == 1>(rw, b, dk, fl, t_exp, sat_f, fmin_bits, frange, bad);
                 if (KERNEL == 1) big |= (fmaxf(fmaxf(fabsf(o4[j].x), fabsf(o4[j].y)), fmaxf(fabsf(o4[j].z), fabsf(o4[j].w))) > RF_LZ_BIG_ADU);
             }
         }

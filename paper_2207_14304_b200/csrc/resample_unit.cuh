@@ -415,7 +415,8 @@ __global__ void UNIT_BOUNDS
                     const float4 b = reinterpret_cast<const float4*>(st + UNIT_CAP * 2)[v];
                     const float4 dk = reinterpret_cast<const float4*>(st + UNIT_CAP * 6)[v];
                     const float4 fl = reinterpret_cast<const float4*>(st + UNIT_CAP * 10)[v];
-                    o4[j] = calib_fast4<KERNEL == 1>(rw, b, dk, fl, t_exp, sat_f, fmin_bits, frange);
+                    int bad4 = 0;                    // (the NaN test below covers both kinds of masters)
+                    o4[j] = calib_fast4<KERNEL == 1>(rw, b, dk, fl, t_exp, sat_f, fmin_bits, frange, bad4);
                 } else {
                     float4 of, gn;
                     if (MASTERS == 1) {
