@@ -145,6 +145,14 @@ __device__ __forceinline__ float4 calib_fast4(uint2 rw, float4 b, float4 d, floa
         c01 = fma2(fma2(make_float2(-c01.x, -c01.y), make_float2(fl.x, fl.y), t01), r01, c01);
         c23 = fma2(fma2(make_float2(-c23.x, -c23.y), make_float2(fl.z, fl.w), t23), r23, c23);
     }
+    // all four good (the usual case) from three maxima: no per-pixel predicate logic and no selects on that path
+    const float rmax = fmaxf(fmaxf(rf01.x, rf01.y), fmaxf(rf23.x, rf23.y));
+    const unsigned fmax = max(max(__float_as_uint(fl.x) - fmin_bits, __float_as_uint(fl.y) - fmin_bits),
+                              max(__float_as_uint(fl.z) - fmin_bits, __float_as_uint(fl.w) - fmin_bits));
+    const float cmax = fmaxf(fmaxf(fabsf(c01.x), fabsf(c01.y)), fmaxf(fabsf(c23.x), fabsf(c23.y)));   // NaN operands drop out of fmaxf:
+    const float2 cs2 = add2(c01, c23);
+    const float csum = cs2.x + cs2.y;                                                                   // ... so NaN is caught by the sum
+    if ((rmax < sat_f) && (fmax < frange) && (cmax < INFINITY) && (csum == csum)) return make_float4(c01.x, c01.y, c23.x, c23.y);
     const bool g0 = (rf01.x < sat_f) && ((__float_as_uint(fl.x) - fmin_bits) < frange) && (fabsf(c01.x) < INFINITY);
     const bool g1 = (rf01.y < sat_f) && ((__float_as_uint(fl.y) - fmin_bits) < frange) && (fabsf(c01.y) < INFINITY);
     const bool g2 = (rf23.x < sat_f) && ((__float_as_uint(fl.z) - fmin_bits) < frange) && (fabsf(c23.x) < INFINITY);
