@@ -70,11 +70,25 @@ __device__ __forceinline__ void bg_load4(const FrameArgs& f, int W, int H, int x
             float4 d = __ldg(reinterpret_cast<const float4*>(f.dark + o));
             float4 fl = __ldg(reinterpret_cast<const float4*>(f.flat + o));
             unsigned bp = f.bpm ? __ldg(reinterpret_cast<const unsigned*>(f.bpm + o)) : 0u;
+#ifndef BG_SCALAR_CALIB
+            // four pixels in packed FP32 with the all-good fast path (calib_fast4: the values calib_px gives for normal flats)
+            int bad4 = 0;
+            const unsigned fmin_bits = __float_as_uint(f.flat_min);
+            const float4 c = calib_fast4<false>(rw, b, d, fl, f.t_exp, (float)f.sat_adu, fmin_bits, 0x7f800000u - fmin_bits, bad4);
+            v[0] = c.x; v[1] = c.y; v[2] = c.z; v[3] = c.w;
+            if (bp) {
+                if (bp & 0xffu) v[0] = nanf_();
+                if (bp & 0xff00u) v[1] = nanf_();
+                if (bp & 0xff0000u) v[2] = nanf_();
+                if (bp & 0xff000000u) v[3] = nanf_();
+            }
+#else
             int r0 = rw.x & 0xffff, r1 = rw.x >> 16, r2 = rw.y & 0xffff, r3 = rw.y >> 16;
             v[0] = calib_px((float)r0, b.x, d.x, fl.x, r0 >= f.sat_adu || (bp & 0xffu), f.t_exp, f.flat_min);
             v[1] = calib_px((float)r1, b.y, d.y, fl.y, r1 >= f.sat_adu || (bp & 0xff00u), f.t_exp, f.flat_min);
             v[2] = calib_px((float)r2, b.z, d.z, fl.z, r2 >= f.sat_adu || (bp & 0xff0000u), f.t_exp, f.flat_min);
             v[3] = calib_px((float)r3, b.w, d.w, fl.w, r3 >= f.sat_adu || (bp & 0xff000000u), f.t_exp, f.flat_min);
+#endif
         } else {
             float4 c = __ldg(reinterpret_cast<const float4*>(f.cal + o));
             unsigned m = __ldg(reinterpret_cast<const unsigned*>(f.mask + o));
