@@ -508,9 +508,11 @@ def run_gpu(args):
         roof = rooflines(kernel, W * H, px_out_frame, coadd, k_ms, clocks and clocks.get("sm_mhz"), peak, peak_src, in_bytes)
         roof["input_bytes_per_px"] = in_bytes
         alg_step = roof["algorithmic_bytes"] * n_frames
-        roof["kernel"] = ("resample_fast_kernel<%s,%d> (TMA-staged, fused calibration%s) + resample_tiles_kernel on its slow list; "
+        # nside 2^18 at this pixel scale: every box fits 48 x 48 pixels, the library runs the two-stage Lanczos-3 form
+        variant = ",1" if (kernel == "lanczos3" and nside >= (1 << 18) and not args.tile_kernel) else ""
+        roof["kernel"] = ("resample_fast_kernel<%s,%d%s> (TMA-staged, fused calibration%s) + resample_tiles_kernel on its slow list; "
                           "per frame, CUDA events around the resample launches" % ("true" if coadd else "false", 1 if kernel == "lanczos3" else 0,
-                                                                                  ", coadd read-modify-write" if coadd else ""))
+                                                                                  variant, ", coadd read-modify-write" if coadd else ""))
         roof["step_frac"] = (alg_step / (ms_step * 1e-3) / 1e9) / peak
         tr, tr_src = ncu_traffic(name + ("" if not args.prefused else "_" + args.prefused))
         roof["traffic"], roof["traffic_source"] = tr, tr_src

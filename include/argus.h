@@ -67,7 +67,10 @@ enum {
                                  1 (default): the TMA-staged tile kernel (resample_fast_kernel, both interpolation kernels) where
                                     every 32 x 32-pixel tile's source box fits its stage, else -- and always with pre-fused
                                     masters -- the image-aligned unit kernel (resample_unit_kernel, bilinear);
-                                 2: tile kernel only; 3: unit kernel wherever its geometry allows; 0: always the general kernel */
+                                    Lanczos-3 frames whose boxes all fit 48 x 48 source pixels (fine grids: nside 2^18 at 0.08 pixels
+                                    per HEALPix pixel) run the tile kernel with two half-size stages instead of one;
+                                 2: tile kernel only (one-stage Lanczos-3 form); 3: unit kernel wherever its geometry allows;
+                                 4: as 1 without the two-stage Lanczos-3 form (diagnostic); 0: always the general kernel */
     ARGUS_OPT_PLAN_OVERLAP = 4, /* 1 (default): the plan of a new WCS is built on an internal high-priority stream in a second
                                  set of scratch buffers, so that it runs underneath the previous frame's kernels; the
                                  caller's stream waits for it (stream order of results is unchanged); 0: in place */

@@ -230,7 +230,8 @@ class Context:
             raise ArgusError(rc, "argus_ctx_set_option")
 
     def set_fast_path(self, on):
-        """False / 0: general kernel only; True / 1: default choice; 2: tile kernel only; 3: unit kernel where possible."""
+        """False / 0: general kernel only; True / 1: default choice; 2: tile kernel only; 3: unit kernel where possible;
+        4: default choice without the two-stage Lanczos-3 form of fine grids (include/argus.h, ARGUS_OPT_FAST_PATH)."""
         rc = load_library().argus_ctx_set_option(self._h, ARGUS_OPT_FAST_PATH, int(on))
         if rc:
             raise ArgusError(rc, "argus_ctx_set_option")

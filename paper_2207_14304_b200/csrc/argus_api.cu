@@ -31,6 +31,9 @@ struct argus_ctx {
     bool plan_valid;
     bool plan_full;       // the cached plan holds TileRec / FP64 coefficients for every tile (general kernel)
     int plan_fast_kernel; // interpolation kernel whose tap apron sized the fast kernel's boxes in the cached plan
+    int plan_fast_cap;    // stage capacity those boxes were checked against (FastCfg<..>::CAP)
+    bool lz_small_enabled;// ARGUS_OPT_FAST_PATH != 4
+    bool lz_small;        // choose_path: every tile of this frame fits the small Lanczos-3 stage (FastCfg<1, 1>)
     argus_wcs key_wcs;
     int64_t key_W, key_H, key_nside;
     DevWcs dw;
@@ -296,6 +299,7 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     c->plan_cache = true;
     c->fast_enabled = true;
     c->unit_enabled = true;
+    c->lz_small_enabled = true;
     c->auto_tiles = max_tiles == 0;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -406,8 +410,9 @@ extern "C" int argus_ctx_set_option(argus_ctx* c, int option, int64_t value) {
     }
     if (option == ARGUS_OPT_FAST_PATH) {
         c->fast_enabled = value != 0;
-        c->unit_enabled = value == 1 || value == 3;
+        c->unit_enabled = value == 1 || value == 3 || value == 4;
         c->unit_forced = value == 3;
+        c->lz_small_enabled = value != 4;
         return ARGUS_OK;
     }
     return ARGUS_ERR_SHAPE;
@@ -504,11 +509,14 @@ static bool same_key(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t 
 }
 
 // Enqueue the plan kernels (A0 + A1).  No host synchronisation.
+static int fast_stage_cap(const argus_ctx* c, int fast_kernel) {
+    return fast_kernel == ARGUS_LANCZOS3 ? (c->lz_small ? FastCfg<1, 1>::CAP : FastCfg<1, 0>::CAP) : FastCfg<0, 0>::CAP;
+}
 static bool plan_usable(const argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, bool need_full, int fast_kernel,
                         const UnitGeom* ug) {
-    // the fast kernel's boxes are sized for one interpolation kernel's taps; the general kernel does not care
+    // the fast kernel's boxes are sized for one interpolation kernel's taps and one stage capacity; the general kernel does not care
     return same_key(c, w, W, H, nside) && (!need_full || c->plan_full) &&
-           (fast_kernel < 0 || c->plan_fast_kernel == (fast_kernel == ARGUS_LANCZOS3 ? 1 : 0)) &&
+           (fast_kernel < 0 || (c->plan_fast_kernel == (fast_kernel == ARGUS_LANCZOS3 ? 1 : 0) && (ug || c->plan_fast_cap == fast_stage_cap(c, fast_kernel)))) &&
            (ug ? (c->plan_unit && memcmp(&c->plan_geom, ug, sizeof(UnitGeom)) == 0) : (fast_kernel < 0 || !c->plan_unit));
 }
 
@@ -623,7 +631,7 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
         const int fk = fast_kernel == ARGUS_LANCZOS3 ? 1 : 0;
         c->pb.fast_tl = fk ? FastCfg<1>::TL : FastCfg<0>::TL;
         c->pb.fast_tr = fk ? FastCfg<1>::TR : FastCfg<0>::TR;
-        c->pb.fast_cap = fk ? FastCfg<1>::CAP : FastCfg<0>::CAP;
+        c->pb.fast_cap = fast_stage_cap(c, fast_kernel);
     }
     if (prof_slot >= 0) cudaEventRecord(c->ev[prof_slot][0], st);
     if (n_slots == 0) n_slots = 1;
@@ -682,6 +690,7 @@ static int build_plan(argus_ctx* c, const argus_wcs* w, int64_t W, int64_t H, in
     c->plan_valid = true;
     c->plan_full = need_full;
     c->plan_fast_kernel = fast_kernel == ARGUS_LANCZOS3 ? 1 : 0;
+    c->plan_fast_cap = fast_stage_cap(c, fast_kernel);
     c->plan_unit = ug != nullptr;
     if (ug) c->plan_geom = *ug;
     return ARGUS_OK;
@@ -933,11 +942,13 @@ static void unit_extent_at(const DevWcs& w, const argus_wcs* wc, int64_t nside, 
 // kernel or the general kernel then runs the frame.  The extents are ESTIMATES from nine sky directions (centre, corners,
 // edge midpoints); a sub-block that exceeds them anyway is found by plan_units_kernel and served by the stray kernel.
 static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64_t H, int64_t nside, double s_rad, int kernel, UnitGeom* g,
-                          bool* tiles_fit, int margin_delta) {
+                          bool* tiles_fit, bool* tiles_small, int margin_delta) {
     const int ktl = kernel == ARGUS_LANCZOS3 ? 2 : 0, ktr = kernel == ARGUS_LANCZOS3 ? 3 : 1;
     const int kcap = kernel == ARGUS_LANCZOS3 ? FAST_CAP_PX_LZ : FAST_CAP_PX;
     double ex = 0.0, ey = 0.0;
     *tiles_fit = true;
+    *tiles_small = false;
+    bool small = kernel == ARGUS_LANCZOS3;
     for (int sy = -1; sy <= 1; ++sy)
         for (int sx = -1; sx <= 1; ++sx) {
             const double px = 0.45 * sx * (double)W, py = 0.45 * sy * (double)H;       // pixel offsets from CRPIX (about the frame centre)
@@ -956,8 +967,10 @@ static bool unit_geometry(const DevWcs& dw, const argus_wcs* w, int64_t W, int64
                 const int bw = span_x + ktl + ktr + 7, bh = span_y + ktl + ktr;
                 const int boxw = bw <= 40 ? 40 : (bw + 7) / 8 * 8, boxh = bh <= 48 ? 48 : (bh + 7) / 8 * 8;
                 if (bw > 72 || bh > 72 || boxw * boxh > kcap) *tiles_fit = false;
+                if (boxw * boxh > FAST_CAP_PX_LZ_SMALL || bh * fast_cal_pitch(boxw) > FAST_CAP_PX_LZ_SMALL * 9 / 8) small = false;
             }
         }
+    *tiles_small = small && *tiles_fit;
     memset(g, 0, sizeof(*g));
     g->tl = ktl; g->tr = ktr;
     const int chk = margin_delta > 8 ? margin_delta - 8 : 0;
@@ -1029,6 +1042,7 @@ static bool unit_maps(argus_ctx* c, const FrameArgs& f, int64_t W, int64_t H, co
 // Which kernel runs the planned frame: 2 = image-aligned units, 1 = tile kernel (resample_fast.cuh), 0 = general kernel.
 static int choose_path(argus_ctx* c, const FrameArgs& f, bool fused, int kernel, const argus_wcs* wcs, int64_t W, int64_t H, int64_t nside,
                        UnitGeom* ug) {
+    c->lz_small = false;
     if (!fused || !c->fast_enabled) return 0;
     if (c->unit_enabled && f.raw && !f.bpm && W % 8 == 0 && W >= 8 && aligned(f.raw, 16) &&
         (f.pre ? (aligned(f.offset, 16) && aligned(f.gain, 16)) : (aligned(f.bias, 16) && aligned(f.dark, 16) && aligned(f.flat, 16)))) {
@@ -1037,10 +1051,14 @@ static int choose_path(argus_ctx* c, const FrameArgs& f, bool fused, int kernel,
         // units where the tile kernel cannot run the frame: pre-fused masters, or tiles whose bounding box does not fit its
         // stage somewhere on the frame (HEALPix tiles are wide near the equator and tall in the polar caps); where its
         // boxes fit, the tile kernel is the faster one (0.28 vs 0.33 ms at configs[1]: DESIGN.md 6.6)
-        bool tiles_fit = true;
-        if (make_devwcs(wcs, W, H, nside, &dw, &rho, &s_rad) == ARGUS_OK && unit_geometry(dw, wcs, W, H, nside, s_rad, kernel, ug, &tiles_fit, c->unit_margin) &&
-            (f.pre || !tiles_fit || c->unit_forced) && unit_maps(c, f, W, H, *ug))
+        bool tiles_fit = true, tiles_small = false;
+        const bool units = make_devwcs(wcs, W, H, nside, &dw, &rho, &s_rad) == ARGUS_OK &&
+                           unit_geometry(dw, wcs, W, H, nside, s_rad, kernel, ug, &tiles_fit, &tiles_small, c->unit_margin);
+        if (units && (f.pre || !tiles_fit || c->unit_forced) && unit_maps(c, f, W, H, *ug))
             return 2;
+        // fine HEALPix grids: every tile's box fits half the Lanczos-3 stage, the tile kernel then runs with two stages (a tile
+        // that does not fit after all fails fast_box in the plan and goes to the general kernel)
+        c->lz_small = tiles_small && c->lz_small_enabled;
     }
     return fast_maps(c, f, W, H) ? 1 : 0;
 }
@@ -1086,10 +1104,15 @@ static int launch_tiles(argus_ctx* c, int kernel, bool fused, bool use_fast, con
             CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<0>)));
             CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<1>)));
             CUDA_TRY(c, cudaFuncSetAttribute(resample_fast_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<1>)));
+            CUDA_TRY(c, (cudaFuncSetAttribute(resample_fast_kernel<false, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<1, 1>))));
+            CUDA_TRY(c, (cudaFuncSetAttribute(resample_fast_kernel<true, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem<1, 1>))));
             c->fast_attr_set = true;
         }
         if (kernel == ARGUS_BILINEAR)
             resample_fast_kernel<COADD, 0><<<c->sm_count * FastCfg<0>::CTAS, RF_THREADS, sizeof(FastSmem<0>), st>>>(
+                c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
+        else if (c->pb.fast_cap == FastCfg<1, 1>::CAP)
+            resample_fast_kernel<COADD, 1, 1><<<c->sm_count * FastCfg<1, 1>::CTAS, RF_THREADS, sizeof(FastSmem<1, 1>), st>>>(
                 c->maps, c->pb, f, (int)W, (int)H, w_min, v, wt, cap, ca);
         else
             resample_fast_kernel<COADD, 1><<<c->sm_count * FastCfg<1>::CTAS, RF_THREADS, sizeof(FastSmem<1>), st>>>(

@@ -28,14 +28,19 @@
 #define RF_GROUPS 1                      // consumer groups per CTA, tiles dealt round-robin
 #define RF_THREADS (RF_GROUPS * RF_CONSUMERS + 32)
 
-// Per interpolation kernel: stage capacity, stages per CTA, CTAs per SM, register cap.
-//   bilinear : 2 stages x 50 KB, 2 CTAs / SM, 80 registers (leaves room for a plan CTA beside it, argus_api.cu)
-//   Lanczos-3: the gather dominates (36 taps, 12 kernel weights per pixel): 1 stage x 64.5 KB + a
+// Per interpolation kernel (and variant): stage capacity, stages per CTA, CTAs per SM, register cap.
+//   bilinear            : 2 stages x 50 KB, 2 CTAs / SM, 80 registers (leaves room for a plan CTA beside it, argus_api.cu)
+//   Lanczos-3           : the gather dominates (36 taps, 12 kernel weights per pixel): 1 stage x 64.5 KB calibrated in place,
+//                         3 CTAs / SM hide one another's stage fills
+//   Lanczos-3, VAR = 1  : frames whose tiles all fit a 48 x 48 box (fine HEALPix grids: nside 2^18 at configs[4]'s pixel
+//                         scale), chosen on the host from the WCS: 2 stages x 32 KB in the same shared memory, so a CTA's
+//                         next box lands while it gathers
+#define FAST_CAP_PX_LZ_SMALL 2304         // Lanczos-3 on fine grids (every box at most 48 x 48 pixels), 2 stages
 #define RF_LZ_BIG_ADU 1500.0f              // Lanczos-3: a box with masked AND brighter pixels goes to the FP64 kernel
-template <int KERNEL> struct FastCfg;
-//              separate calibrated box, so the stage is refilled while the long gather runs; 2 CTAs / SM
-template <> struct FastCfg<0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1, CALBUF = 0, REGS = 80; };
-template <> struct FastCfg<1> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
+template <int KERNEL, int VAR = 0> struct FastCfg;
+template <> struct FastCfg<0, 0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1, CALBUF = 0, REGS = 80; };
+template <> struct FastCfg<1, 0> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
+template <> struct FastCfg<1, 1> { static constexpr int CAP = FAST_CAP_PX_LZ_SMALL, STAGES = 2, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
 
 struct FastMaps {
     CUtensorMap m[4][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
@@ -62,13 +67,13 @@ struct __align__(128) FastStage {
     float dark[CAP];
     float flat[CAP];
 };
-template <int KERNEL>
+template <int KERNEL, int VAR = 0>
 struct __align__(128) FastSmem {
-    FastStage<FastCfg<KERNEL>::CAP> stage[FastCfg<KERNEL>::STAGES];
-    float calbuf[FastCfg<KERNEL>::CALBUF > 0 ? FastCfg<KERNEL>::CALBUF : 4];   // separate calibrated box (Lanczos-3)
+    FastStage<FastCfg<KERNEL, VAR>::CAP> stage[FastCfg<KERNEL, VAR>::STAGES];
+    float calbuf[FastCfg<KERNEL, VAR>::CALBUF > 0 ? FastCfg<KERNEL, VAR>::CALBUF : 4];   // separate calibrated box (Lanczos-3)
     FastDesc desc[2];                                    // tile k uses descriptor k & 1 and stage k % STAGES
     unsigned long long full[2];                          // descriptor written and TMA bytes landed (1 arrival + tx)
-    unsigned long long empty[FastCfg<KERNEL>::STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
+    unsigned long long empty[FastCfg<KERNEL, VAR>::STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
 };
 
 // ---------------------------------------------------------------------------------- PTX wrappers
@@ -324,15 +329,15 @@ __device__ __forceinline__ void interp_masked(const float* __restrict__ a, int p
 // ------------------------------------------------------------------------------------------ kernel
 // Bilinear, 80 registers: two CTAs leave 19 K registers per SM free, enough for one CTA of any plan kernel -- the plan
 // of the next frame runs on a side stream underneath this kernel (argus_api.cu, ARGUS_OPT_PLAN_OVERLAP).
-template <bool COADD, int KERNEL>
-__global__ void __maxnreg__(FastCfg<KERNEL>::REGS)
+template <bool COADD, int KERNEL, int VAR = 0>
+__global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
     resample_fast_kernel(const __grid_constant__ FastMaps maps, PlanBuffers pb, FrameArgs f, int W, int H, float w_min, float* __restrict__ value_out, float* __restrict__ weight_out, long long out_cap,
                          CoaddArgs ca) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    typedef FastCfg<KERNEL> Cfg;
+    typedef FastCfg<KERNEL, VAR> Cfg;
     constexpr int RF_STAGES = Cfg::STAGES;
     constexpr int RF_NI = (Cfg::CAP / 4 + RF_CONSUMERS - 1) / RF_CONSUMERS;   // calibration items (float4) per thread
-    FastSmem<KERNEL>& sm = *reinterpret_cast<FastSmem<KERNEL>*>(smem_raw);
+    FastSmem<KERNEL, VAR>& sm = *reinterpret_cast<FastSmem<KERNEL, VAR>*>(smem_raw);
     const int tid = threadIdx.x;
     const int n_tiles = *pb.n_tiles;
     const float t_exp = f.t_exp, flat_min = f.flat_min;

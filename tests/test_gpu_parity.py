@@ -412,6 +412,51 @@ def test_coadd_lanczos_repeated_wcs_cached_plan(argus, ctx):
     assert np.array_equal(outs[0][0], outs[2][0]) and np.array_equal(outs[0][1], outs[2][1])
 
 
+def test_lanczos_fine_grid_two_stage_form(argus, ctx):
+    """nside 2^18 at the configs' pixel scale: every tile's source box fits 48 x 48 pixels, so the tile kernel runs its
+    two-stage Lanczos-3 form (FastCfg<1, 1>, resample_fast.cuh).  Values + weights and a coadd of three calls against
+    the oracle, on a frame with saturated stars (run-time hand-over to the FP64 kernel); values + weights bit for bit
+    against the one-stage form (ARGUS_OPT_FAST_PATH = 4): the same arithmetic per tile in another pipeline."""
+    from gpu_util import (assert_coadd_matches, assert_values_match, coadd_oracle, gpu_resample_planned,
+                          oracle_reference, upload)
+    W = H = 512
+    fr = _saturated_star_frame()
+    fr.nside = nside = 1 << 18
+    fp, _ = oracle.footprint(fr.wcs, W, H, nside)
+    d = upload(fr)
+    n, v, w = gpu_resample_planned(ctx, fr, d, "lanczos3")
+    assert n == len(fp)
+    vo, wo, fl = oracle_reference(fr, fp, "lanczos3")
+    assert (wo < 1).sum() > 100
+    assert_values_match(v, w, vo, wo, fl, "nside 2^18 Lanczos-3, two-stage form")
+    ppt = (nside // 256) ** 2                 # pixels of an NSIDE-256 coadd tile: 2^20 at nside 2^18
+    tiles = np.unique(fp // ppt)
+    ref = coadd_oracle([fr] * 3, [fp] * 3, tiles, ppt, nside, "lanczos3")
+    dt = torch.from_numpy(tiles).cuda()
+
+    def coadd():
+        s = torch.zeros(len(tiles) * ppt, dtype=torch.float32, device="cuda")
+        ws = torch.zeros_like(s)
+        for _ in range(3):
+            argus.argus_resample_coadd(ctx, fr.wcs, W, H, nside, "lanczos3", dt, 256, s, ws, None, **d)
+        torch.cuda.synchronize()
+        return s.cpu().numpy(), ws.cpu().numpy()
+
+    s2, w2 = coadd()
+    assert_coadd_matches(s2, w2, ref, "nside 2^18 Lanczos-3 coadd, two-stage form")
+    ctx.set_fast_path(4)
+    try:
+        n1, v1, w1 = gpu_resample_planned(ctx, fr, d, "lanczos3")
+        s1, ws1 = coadd()
+    finally:
+        ctx.set_fast_path(True)
+    assert n1 == n and np.array_equal(v1, v) and np.array_equal(w1, w)
+    # the coadd instantiations of the two forms are compiled apart and differ by single roundings (1 ulp on some 4e-3 of the
+    # slots): each is held to the oracle, and the same tiles must have been handed over (weights equal to rounding)
+    assert_coadd_matches(s1, ws1, ref, "nside 2^18 Lanczos-3 coadd, one-stage form")
+    assert np.abs(ws1 - w2).max() <= 3 * 2.0 ** -22 and np.abs(s1 - s2).max() <= 3 * 2.0 ** -13
+
+
 def test_overflow_of_an_earlier_frame_is_latched(argus, cfg0):
     """An output-capacity overflow of frame k must still be reported when the check comes after frame k + 1 was planned
     (plan statistics live in rotating scratch sets; the error is latched context-wide until read)."""
