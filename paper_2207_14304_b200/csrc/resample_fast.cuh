@@ -38,9 +38,15 @@
 #define FAST_CAP_PX_LZ_SMALL 2304         // Lanczos-3 on fine grids (every box at most 48 x 48 pixels), 2 stages
 #define RF_LZ_BIG_ADU 1500.0f              // Lanczos-3: a box with masked AND brighter pixels goes to the FP64 kernel
 template <int KERNEL, int VAR = 0> struct FastCfg;
-template <> struct FastCfg<0, 0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1, CALBUF = 0, REGS = 80; };
-template <> struct FastCfg<1, 0> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
-template <> struct FastCfg<1, 1> { static constexpr int CAP = FAST_CAP_PX_LZ_SMALL, STAGES = 2, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72; };
+//   SPLIT (one-stage Lanczos-3): the calibrated box overwrites bias + a pad of its own, so raw / dark / flat are dead once
+//                         the calibration has read them: the producer refills them for the CTA's next tile during the
+//                         gather, and only the bias box (18 of 64.5 KB, prefetched into L2) is loaded after it
+#ifndef RF_LZ_SPLIT
+#define RF_LZ_SPLIT 1
+#endif
+template <> struct FastCfg<0, 0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1, CALBUF = 0, REGS = 80, SPLIT = 0; };
+template <> struct FastCfg<1, 0> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72, SPLIT = RF_LZ_SPLIT; };
+template <> struct FastCfg<1, 1> { static constexpr int CAP = FAST_CAP_PX_LZ_SMALL, STAGES = 2, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72, SPLIT = 0; };
 
 struct FastMaps {
     CUtensorMap m[4][5][4];   // [height class][width class][raw, bias, dark, flat]; box = (40 + 8 w) x (48 + 8 h)
@@ -59,21 +65,24 @@ struct __align__(16) FastDesc {
 
 // One stage: the raw + master boxes as the TMA delivers them (dense, pitch = box width).  After the consumers have
 // read them into registers, the calibrated box overwrites the stage from `bias` on (pitch 8 or 24 mod 32 floats,
-// up to CAP * 9/8 floats = bias + the head of dark).
-template <int CAP>
+// up to CAP * 9/8 floats = bias + the head of dark; with PAD = CAP / 8 the tail lands in a pad of its own instead).
+template <int CAP, int PAD = 32>
 struct __align__(128) FastStage {
     unsigned short raw[CAP];
     float bias[CAP];
+    float calpad[PAD];
     float dark[CAP];
     float flat[CAP];
 };
 template <int KERNEL, int VAR = 0>
 struct __align__(128) FastSmem {
-    FastStage<FastCfg<KERNEL, VAR>::CAP> stage[FastCfg<KERNEL, VAR>::STAGES];
+    typedef FastStage<FastCfg<KERNEL, VAR>::CAP, FastCfg<KERNEL, VAR>::SPLIT ? FastCfg<KERNEL, VAR>::CAP / 8 : 32> Stage;
+    Stage stage[FastCfg<KERNEL, VAR>::STAGES];
     float calbuf[FastCfg<KERNEL, VAR>::CALBUF > 0 ? FastCfg<KERNEL, VAR>::CALBUF : 4];   // separate calibrated box (Lanczos-3)
     FastDesc desc[2];                                    // tile k uses descriptor k & 1 and stage k % STAGES
     unsigned long long full[2];                          // descriptor written and TMA bytes landed (1 arrival + tx)
     unsigned long long empty[FastCfg<KERNEL, VAR>::STAGES];   // all consumers are done with the stage (RF_CONSUMERS arrivals)
+    unsigned long long empty_a;                          // SPLIT: all consumers have read raw / dark / flat of the stage
 };
 
 // ---------------------------------------------------------------------------------- PTX wrappers
@@ -99,6 +108,9 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
         "}\n" ::"r"(smem_u32(b)),
         "r"(parity)
         : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap* map, int x, int y) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(map), "r"(x), "r"(y) : "memory");
 }
 __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int x, int y, unsigned long long* bar) {
     asm volatile(
@@ -346,6 +358,7 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
     if (tid == 0) {
         for (int i = 0; i < 2; ++i) mbar_init(&sm.full[i], 1);
         for (int i = 0; i < RF_STAGES; ++i) mbar_init(&sm.empty[i], RF_CONSUMERS);
+        mbar_init(&sm.empty_a, RF_CONSUMERS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -379,7 +392,10 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
             const int slot = issued % RF_STAGES, ds = issued & 1;
             // stage free: every consumer is done with the tile that used it RF_STAGES tiles ago.  That also frees
             // descriptor ds: the consumers released tile issued-1's stage after they had finished tile issued-2.
-            if (issued >= RF_STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / RF_STAGES - 1) & 1));
+            // SPLIT: raw / dark / flat are free once tile issued-1 has been calibrated (its gather still reads the calibrated box
+            // over bias + pad); by then the consumers have finished tile issued-2, so descriptor ds is free as well
+            if (Cfg::SPLIT) { if (issued >= 1) mbar_wait(&sm.empty_a, (unsigned)((issued - 1) & 1)); }
+            else if (issued >= RF_STAGES) mbar_wait(&sm.empty[slot], (unsigned)((issued / RF_STAGES - 1) & 1));
             FastDesc& d = sm.desc[ds];
             if (last) {
                 // end of work: one sentinel per consumer group (consecutive tiles go to distinct groups)
@@ -403,9 +419,10 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
                 tx_bytes = (unsigned)(boxh * boxw * 14);
                 if (lane == 0) {
                     const CUtensorMap* mp = &maps.m[hc][wc][0];
-                    FastStage<Cfg::CAP>& sg = sm.stage[slot];
+                    typename FastSmem<KERNEL, VAR>::Stage& sg = sm.stage[slot];
                     tma_load_2d(sg.raw, mp + 0, gx0, gy0, &sm.full[ds]);
-                    tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[ds]);
+                    if (!Cfg::SPLIT) tma_load_2d(sg.bias, mp + 1, gx0, gy0, &sm.full[ds]);
+                    else tma_prefetch_2d(mp + 1, gx0, gy0);         // loaded below, once the previous tile's gather is over
                     tma_load_2d(sg.dark, mp + 2, gx0, gy0, &sm.full[ds]);
                     tma_load_2d(sg.flat, mp + 3, gx0, gy0, &sm.full[ds]);
                 }
@@ -456,6 +473,11 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
                 }
             }
             __syncwarp();
+            if (Cfg::SPLIT) {
+                // the bias box lands where the previous tile's calibrated box is still being gathered from
+                if (issued >= 1) mbar_wait(&sm.empty[slot], (unsigned)((issued - 1) & 1));
+                if (lane == 0) tma_load_2d(sm.stage[slot].bias, &maps.m[wclass >> 4][wclass & 15][1], gx0, gy0, &sm.full[ds]);
+            }
             if (lane == 0) mbar_arrive_expect_tx(&sm.full[ds], tx_bytes);   // releases the descriptor to the consumers
             ++issued;
         }
@@ -478,7 +500,7 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
         const FastDesc& d = sm.desc[ds];
         const int cls = d.r.cls;
         if (cls < 0) break;
-        FastStage<Cfg::CAP>& sg = sm.stage[slot];
+        typename FastSmem<KERNEL, VAR>::Stage& sg = sm.stage[slot];
         float* cal = Cfg::CALBUF > 0 ? sm.calbuf : sg.bias;
         const int boxw = 40 + 8 * (d.r.wclass & 15), pitch = fast_cal_pitch(boxw);
         // every column of the box is calibrated: restricting the items to the tap columns made the 128-bit shared
@@ -508,6 +530,7 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
         // separate calibrated box (Lanczos-3): every thread has read its part of the stage, the producer may refill it
         // while the gather runs
         if (Cfg::CALBUF > 0) mbar_arrive(&sm.empty[slot]);
+        if (Cfg::SPLIT) mbar_arrive(&sm.empty_a);         // raw / dark / flat may be refilled; bias + pad hold the calibrated box
 #pragma unroll
         for (int j = 0; j < RF_NI; ++j) {
             const int v = gt + RF_CONSUMERS * j;

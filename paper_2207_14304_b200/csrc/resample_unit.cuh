@@ -201,10 +201,6 @@ struct __align__(128) UnitSmem {
 
 struct UnitMaps { CUtensorMap m[4]; };    // raw, then the masters in stage order
 
-__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap* map, int x, int y) {
-    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(map), "r"(x), "r"(y) : "memory");
-}
-
 __device__ __forceinline__ float calib_unit_pre(unsigned magic_r, float off, float g, float sat_f) {
     const float rf = __uint_as_float(magic_r) - 8388608.0f;
     const float c = (rf - off) * g;                                        // R-M4; NaN gain (invalid, off-frame) -> NaN
