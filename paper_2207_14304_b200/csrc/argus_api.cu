@@ -304,8 +304,8 @@ extern "C" int argus_ctx_create(argus_ctx** out, int device, int64_t max_tiles) 
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) { delete c; return ARGUS_ERR_CUDA; }
-    cudaError_t e2 = cudaMalloc((void**)&c->d_latch, 2 * sizeof(int));
-    if (e2 == cudaSuccess) e2 = cudaMemset(c->d_latch, 0, 2 * sizeof(int));
+    cudaError_t e2 = cudaMalloc((void**)&c->d_latch, 4 * sizeof(int));     // + [2], [3]: the tile kernel's claim / finish counters
+    if (e2 == cudaSuccess) e2 = cudaMemset(c->d_latch, 0, 4 * sizeof(int));
     if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_latch, 2 * sizeof(int));
     if (e2 == cudaSuccess) e2 = cudaMallocHost((void**)&c->h_stats, sizeof(PlanStats));
     int rc_slots = ARGUS_OK;

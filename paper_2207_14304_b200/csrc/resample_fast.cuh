@@ -44,6 +44,9 @@ template <int KERNEL, int VAR = 0> struct FastCfg;
 #ifndef RF_LZ_SPLIT
 #define RF_LZ_SPLIT 1
 #endif
+#ifndef RF_SCHED_DYNAMIC
+#define RF_SCHED_DYNAMIC 1               // 1: Lanczos-3 tiles claimed from a counter instead of dealt round-robin; 2: bilinear too
+#endif
 template <> struct FastCfg<0, 0> { static constexpr int CAP = FAST_CAP_PX, STAGES = 2, CTAS = 2, TL = 0, TR = 1, CALBUF = 0, REGS = 80, SPLIT = 0; };
 template <> struct FastCfg<1, 0> { static constexpr int CAP = FAST_CAP_PX_LZ, STAGES = 1, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72, SPLIT = RF_LZ_SPLIT; };
 template <> struct FastCfg<1, 1> { static constexpr int CAP = FAST_CAP_PX_LZ_SMALL, STAGES = 2, CTAS = 3, TL = 2, TR = 3, CALBUF = 0, REGS = 72, SPLIT = 0; };
@@ -371,7 +374,22 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
         // handled (one producer serves RF_GROUPS groups, so its own load latency must stay off the critical path)
         float4 rv_n = make_float4(0.f, 0.f, 0.f, 0.f);
         long long off_n = 0;
-        int t_n = blockIdx.x;
+#if RF_SCHED_DYNAMIC
+        // tiles are claimed from a context-wide counter (pb.latch[2]) instead of dealt round-robin: the CTAs of an SM that shares
+        // its issue slots with a plan kernel of the next frame (ARGUS_OPT_PLAN_OVERLAP) take fewer tiles, the others more, and the
+        // kernel does not wait for the slowest SM's fixed share.  Claims stay in plan order, so concurrently staged boxes still
+        // overlap in L2.  The last producer to finish (pb.latch[3]) resets both words for the next launch on the stream.
+        // Claims run two tiles ahead and the record load one: the atomic's round trip and the load's are each a tile period in
+        // flight (in one period together they made the producer the bottleneck of the bilinear kernel, 1.5 us per tile).
+        int* const sched = pb.latch + 2;
+        constexpr bool DYN = KERNEL == 1 || RF_SCHED_DYNAMIC > 1;
+        int t_n = DYN ? __shfl_sync(0xffffffffu, lane == 0 ? atomicAdd(sched, 1) : 0, 0) : (int)blockIdx.x;
+        int claim_nn = (DYN && lane == 0 && t_n < n_tiles) ? atomicAdd(sched, 1) : 0x7fffffff;   // lane 0's, broadcast when it is needed
+#else
+        constexpr bool DYN = false;
+        int* const sched = nullptr;
+        int t_n = blockIdx.x, claim_nn = 0;
+#endif
         if (t_n < n_tiles) {
             if (lane < 10) rv_n = __ldg(reinterpret_cast<const float4*>(pb.frec + t_n) + lane);
             if (lane == 0) off_n = tile_out_offset(pb, t_n);
@@ -381,7 +399,14 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
             const bool last = t >= n_tiles;
             const float4 rv = rv_n;
             const long long off_c = off_n;
-            t_n = t + gridDim.x;
+            if (DYN) {
+                if (!last) {
+                    t_n = __shfl_sync(0xffffffffu, claim_nn, 0);
+                    claim_nn = (lane == 0 && t_n < n_tiles) ? atomicAdd(sched, 1) : 0x7fffffff;
+                }
+            } else {
+                t_n = t + gridDim.x;
+            }
             if (t_n < n_tiles) {
                 if (lane < 10) rv_n = __ldg(reinterpret_cast<const float4*>(pb.frec + t_n) + lane);
                 if (lane == 0) off_n = tile_out_offset(pb, t_n);
@@ -480,6 +505,10 @@ __global__ void __maxnreg__((FastCfg<KERNEL, VAR>::REGS))
             }
             if (lane == 0) mbar_arrive_expect_tx(&sm.full[ds], tx_bytes);   // releases the descriptor to the consumers
             ++issued;
+        }
+        if (DYN && lane == 0 && atomicAdd(sched + 1, 1) == (int)gridDim.x - 1) {   // every CTA has made its last claim
+            sched[0] = 0;
+            sched[1] = 0;
         }
         return;
     }
