@@ -159,7 +159,9 @@ int argus_version(void);
  *               when a later frame needs more; never shrunk.
  *   max_tiles in 64 .. 2^24: allocated now, fixed; a frame with more candidate tiles reports ARGUS_ERR_CAPACITY.
  * device = CUDA ordinal.  Synchronous.  A context is not thread-safe: use one per host thread (contexts are
- * independent). */
+ * independent).  Its calls share device scratch (plan sets, the tile kernels' claim counter): enqueue the calls of one
+ * context on ONE stream at a time (or order the streams with events); frames that should run concurrently on one GPU take
+ * one context each. */
 int argus_ctx_create(argus_ctx** ctx, int device, int64_t max_tiles);
 int argus_ctx_destroy(argus_ctx* ctx);
 int argus_ctx_set_option(argus_ctx* ctx, int option, int64_t value);
